@@ -1,0 +1,141 @@
+/* muser.h -- C ABI of the B200-native MUSER dirty-imaging hot path (arXiv 1712.06913).
+ *
+ * The path: calibrated visibilities -> [A1] coordinates + binning (counting sort by uv tile)
+ *        -> [A2/A3/A4] convolutional gridding (2-D, w-projection planes, batched grids)
+ *        -> [A5] 2-D inverse FFT (cuFFT) -> [A6] fused grid correction + fftshift + real part
+ *        -> dirty image and dirty beam (PSF).
+ * Paper passages (PAPER.md = the paper's text; DESIGN.md restates every reading R1..R21):
+ *   "Gridding is the convolution of the visibilities with a particular function, which resamples the
+ *    visibilities to lie on a regular rectangular grid"                        PAPER.md:78  (sec. 2)
+ *   truncated spheroidal gridding convolution function                          PAPER.md:136-138 (sec. 3.2.3)
+ *   "Inverse FFT is performed after gridding for generating dirty image"
+ *   inputs "Visibilities and UVW (Phase corrected, Flagged)"                     PAPER.md:213 (Alg. 1)
+ *   grid is float2, row-major iv*nu+iu, Hermitian                               PAPER.md:216-228 (Alg. 1 l.1-6)
+ *   natural weighting multiplies by 1                                           PAPER.md:240-243 (Alg. 1 l.12-13)
+ *   DIRTY_IMAGE: w-projection, gridding, inverse FFT "with the sun disk at the center",
+ *   returns dirty image and dirty beam                                          PAPER.md:249-256 (Alg. 1 l.17-20)
+ *   w-projection is used for the w-term                                         PAPER.md:126 (sec. 3.2.2)
+ *
+ * General rules
+ *   - Plain C, no C++/torch types.  Every pointer argument says HOST or DEVICE.  DEVICE pointers must be on
+ *     the CUDA device that was current when the handle was created.
+ *   - The caller owns every data buffer; the library never frees or keeps them beyond the work it enqueues.
+ *     The library owns the handle: grids, sort scratch, tables, correctors, cuFFT plan.  Scratch only grows.
+ *   - Calls taking a muser_stream only ENQUEUE work on it (no host synchronisation) unless stated.
+ *   - Every int-returning call returns MUSER_OK (0) or an error code; no exception or abort crosses the ABI.
+ *     muser_last_error(h) gives the text of the last error on that handle (h = NULL: last create error).
+ *   - Arrays are row-major [y][x] = [v][u].  Grid cell (iu, iv) <-> u = (iu - nx/2)/(nx*cell) wavelengths.
+ *     Image pixel (x, y) <-> direction cosines l = (x - nx/2)*cell, m = (y - ny/2)*cell (no sky flip).
+ *   - Outputs are un-normalised: a unit point source at the phase centre gives a peak of sum_weights
+ *     (sum over gridded samples, conjugates included).
+ *   - There is no CPU fallback anywhere: without a CUDA device create fails with MUSER_ECUDA.
+ */
+#ifndef MUSER_H_
+#define MUSER_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct muser_imager muser_imager;     /* opaque; owned by the library */
+typedef void* muser_stream;                   /* a cudaStream_t; NULL = the legacy default stream */
+
+enum { MUSER_OK = 0, MUSER_EINVAL = 1, MUSER_ECUDA = 2, MUSER_ENOMEM = 3, MUSER_ESTATE = 4, MUSER_EUNSUPPORTED = 5 };
+enum { MUSER_KERNEL_PSWF = 0, MUSER_KERNEL_GAUSS = 1 };
+/* gridding strategies (muser_set_strategy): AUTO picks TILED for single grids and DIRECT for batches of small grids */
+enum { MUSER_STRATEGY_AUTO = 0, MUSER_STRATEGY_DIRECT = 1, MUSER_STRATEGY_TILED = 2 };
+/* stage ids of muser_get_profile */
+enum { MUSER_STAGE_BIN = 0, MUSER_STAGE_GRID = 1, MUSER_STAGE_PACK = 2, MUSER_STAGE_FFT = 3, MUSER_STAGE_CORRECT = 4,
+       MUSER_STAGE_COUNT = 5 };
+
+/* ---- A0 setup -------------------------------------------------------------------------------------------
+ * Create an imager for nx x ny grids/images with pixel size cell_arcsec, a separable gridding kernel of FULL
+ * width `support` cells (odd, R1) tabulated at `oversample` sub-cell phases (even), PSWF by default
+ * (R2).  Requirements: nx, ny multiples of 4 and >= 2*(support+1); support odd in [1,63];
+ * oversample even in [2,256]; cell_arcsec > 0.  Builds the table and the per-axis correctors (fp64 on the
+ * host), allocates grids (zeroed), makes the cuFFT plan.  May synchronise.  Returns NULL on error. */
+muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int support, int oversample);
+/* Frees everything the handle owns.  NULL is a no-op.  Synchronises the device. */
+int muser_imager_destroy(muser_imager* h);
+/* Choose the 2-D kernel: MUSER_KERNEL_PSWF (param ignored) or MUSER_KERNEL_GAUSS (param = a in cells of
+ * exp(-(x/a)^2), 0 -> 1.55; R3).  Rebuilds table + correctors, leaves w-plane mode, zeroes the grids. */
+int muser_set_kernel(muser_imager* h, int kind, double param);
+/* Number of independent grids (A4, batched imaging: one grid per frame/channel/polarisation).
+ * Reallocates and zeroes the grids.  ngrids >= 1. */
+int muser_set_batch(muser_imager* h, int ngrids);
+/* A3: w-projection with nplanes planes (R15).  HOST arrays, copied: w_centres[p] >= 0 (plane
+ * centres in wavelengths of |w|), supports[p] odd in [1,63]; tables_c64[p] = supports[p]*oversample+1
+ * interleaved (re,im) FLOAT pairs of the per-axis kernel, or tables_c64 == NULL: the library generates the
+ * Fresnel-separable kernels of R15.  Plane 0's (real part) table defines the grid correction.
+ * nplanes == 0 returns to 2-D mode.  Zeroes the grids (the beam grid becomes complex). */
+int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, const int* supports,
+                      const float* const* tables_c64);
+int muser_set_strategy(muser_imager* h, int strategy);
+/* 1 (default): A6 divides by the kernel's transform; 0: A6 only shifts/takes the real part (parity gate R9(i)). */
+int muser_set_grid_correction(muser_imager* h, int enabled);
+
+/* ---- A1..A4 gridding --------------------------------------------------------------------------------------
+ * Zero the grids, the sum of weights and the counters (asynchronous on s). */
+int muser_reset(muser_imager* h, muser_stream s);
+/* Grid nvis visibilities AND their Hermitian conjugates (-u,-v,-w, conj V) (R6), accumulating
+ * onto what is already there (time integration; R16).  DEVICE pointers:
+ *   uvw_m   float  [nvis][3]  baseline coordinates in metres
+ *   freq_hz double [nvis]     observing frequency of each visibility (u_lambda = u_m * freq/c)
+ *   vis_c64 float  [nvis][2]  complex visibility (re, im)
+ *   weight  float  [nvis]     weight; <= 0 or non-finite inputs flag the visibility (skipped and counted)
+ * Visibilities whose kernel footprint (either sample's) leaves cells [1, n-1] are dropped and counted (R5).
+ * nvis == 0 is a no-op.  grid_id (batched): int [nvis], 0 <= grid_id < ngrids, else flagged. */
+int muser_grid(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+               const float* weight, long long nvis, muser_stream s);
+int muser_grid_batched(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                       const float* weight, const int* grid_id, long long nvis, muser_stream s);
+
+/* ---- A5 + A6 imaging --------------------------------------------------------------------------------------
+ * DEVICE outputs float [ngrids][ny][nx].  One complex inverse FFT of H = G + i*Gw yields both images (the
+ * dirty image is its real part, the beam its imaginary part, because G and Gw are Hermitian); muser_dirty and
+ * muser_psf share that transform when called back to back.  The accumulated grids are NOT destroyed: both may
+ * be called, in either order, and gridding may continue afterwards.  Either output of muser_dirty_psf may be NULL. */
+int muser_dirty(muser_imager* h, float* image_out, muser_stream s);
+int muser_psf(muser_imager* h, float* beam_out, muser_stream s);
+int muser_dirty_psf(muser_imager* h, float* image_out, float* beam_out, muser_stream s);
+
+/* ---- whole path with HOST buffers (end-to-end entry point) ------------------------------------------------
+ * reset -> copy the inputs to the device -> grid -> dirty + psf -> copy the images back, all on s, then
+ * synchronises s.  HOST pointers (pinned memory makes the copies asynchronous); grid_id may be NULL;
+ * image_out / beam_out (float [ngrids][ny][nx]) may each be NULL. */
+int muser_frame_host(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                     const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
+                     muser_stream s);
+
+/* ---- inspection ---------------------------------------------------------------------------------------------
+ * Copy the centred grids (DC at [ny/2][nx/2]) to DEVICE buffers: grid_c64_out float [ngrids][ny][nx][2];
+ * wgrid_out float [ngrids][ny][nx] (2-D mode) or [ngrids][ny][nx][2] (w mode).  Either may be NULL. */
+int muser_get_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_stream s);
+/* Kernel table of `plane` as used on the device, in the oracle's order T[t], t = 0..S*Q (2-D mode: floats;
+ * w mode: (re,im) pairs).  HOST output; *len in: capacity in floats, out: floats written. */
+int muser_get_table(muser_imager* h, int plane, float* table_out_host, int* len);
+/* HOST outputs (any may be NULL).  Synchronises the last stream used.  sum_weights counts both samples of a
+ * kept visibility; n_gridded counts kept visibilities. */
+int muser_get_stats(muser_imager* h, double* sum_weights, long long* n_gridded, long long* n_dropped,
+                    long long* n_flagged);
+const char* muser_last_error(const muser_imager* h);
+
+/* ---- measurement -----------------------------------------------------------------------------------------
+ * enabled = 1: bracket every stage with CUDA events on the caller's stream (adds host work; do not enable it
+ * inside a throughput measurement).  muser_get_profile synchronises and returns, per stage, the summed device
+ * time in milliseconds and the number of launches since profiling was enabled (HOST arrays of MUSER_STAGE_COUNT). */
+int muser_set_profiling(muser_imager* h, int enabled);
+int muser_get_profile(muser_imager* h, double* stage_ms, long long* stage_launches);
+
+/* ---- host-only helpers (no GPU needed; used by the table-parity tests) ---------------------------------------
+ * The library's own fp64 generators: kernel table T[t], t = 0..S*Q (kind as above; param: Gaussian a), and
+ * the per-axis corrector c[x], x = 0..n-1, of a real table.  HOST outputs of S*Q+1 and n doubles. */
+int muser_host_table(int kind, int support, int oversample, double param, double* table_out);
+int muser_host_wtable(int support, int oversample, double w_lambda, double fov_rad, double* table_out_re_im);
+int muser_host_corrector(const double* table, int support, int oversample, int n, double* corr_out);
+const char* muser_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MUSER_H_ */

@@ -1,0 +1,605 @@
+// C ABI of the MUSER dirty-imaging library (include/muser.h): handle, validation, setup (A0), stage sequencing.
+// Every step of the data path runs in the kernels of muser_kernels.cu (+ cuFFT for A5); this file only
+// validates, allocates and enqueues.
+#include "../../include/muser.h"
+#include "muser_internal.h"
+#include "tables.h"
+
+#include <cufft.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace muser;
+
+static thread_local std::string g_create_error;
+static const double kArcsec = 3.14159265358979323846 / 648000.0;
+
+struct StageEvent {
+    cudaEvent_t a, b;
+    int stage;
+};
+
+struct muser_imager {
+    int nx = 0, ny = 0, S = 0, Q = 0;
+    double cell_arcsec = 0;
+    int kind = MUSER_KERNEL_PSWF;
+    double gauss_a = 1.55;
+    int ngrids = 1, nplanes = 0, strategy = MUSER_STRATEGY_AUTO, correction = 1;
+    int device = 0, num_sms = 148, max_smem = 0;
+    Geom geom{};
+    std::vector<PlaneMeta> planes_h;
+    std::vector<std::vector<float>> tables_f32;     // per plane, oracle order T[t] (floats or (re,im) pairs)
+    PlaneMeta* planes_d = nullptr;
+    float* tables_d = nullptr;
+    float *icx_d = nullptr, *icy_d = nullptr, *ones_d = nullptr;
+    float2* G = nullptr;
+    float* Gw = nullptr;
+    float2* H = nullptr;
+    Staged* staged = nullptr;
+    Sample* sorted = nullptr;
+    size_t sample_cap = 0;
+    uint32_t *bin_count = nullptr, *bin_offset = nullptr, *nitems_d = nullptr;
+    Item* items = nullptr;
+    size_t bins_cap = 0, items_cap = 0;
+    Stats* stats_d = nullptr;
+    cufftHandle plan = 0;
+    bool plan_ok = false, fft_valid = false;
+    cudaStream_t last_stream = nullptr;
+    // host-frame staging (muser_frame_host)
+    float* in_uvw = nullptr; double* in_freq = nullptr; float2* in_vis = nullptr; float* in_wt = nullptr; int* in_gid = nullptr;
+    size_t in_cap = 0;
+    float *out_dirty = nullptr, *out_psf = nullptr;
+    // profiling
+    bool profiling = false;
+    std::vector<StageEvent> ev_used, ev_free;
+    double stage_ms[MUSER_STAGE_COUNT] = {0};
+    long long stage_n[MUSER_STAGE_COUNT] = {0};
+    std::string err;
+};
+
+static int fail(muser_imager* h, int code, const std::string& msg) {
+    if (h) h->err = msg; else g_create_error = msg;
+    return code;
+}
+#define CU(h, expr)                                                                                   \
+    do {                                                                                              \
+        cudaError_t e_ = (expr);                                                                      \
+        if (e_ != cudaSuccess)                                                                        \
+            return fail(h, e_ == cudaErrorMemoryAllocation ? MUSER_ENOMEM : MUSER_ECUDA,              \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                          \
+    } while (0)
+
+namespace {
+
+struct StageScope {       // brackets a stage with events when profiling is on
+    muser_imager* h; cudaStream_t s; StageEvent ev; bool on;
+    StageScope(muser_imager* h_, int stage, cudaStream_t s_) : h(h_), s(s_), on(h_->profiling) {
+        if (!on) return;
+        if (!h->ev_free.empty()) { ev = h->ev_free.back(); h->ev_free.pop_back(); }
+        else { cudaEventCreate(&ev.a); cudaEventCreate(&ev.b); }
+        ev.stage = stage;
+        cudaEventRecord(ev.a, s);
+    }
+    ~StageScope() {
+        if (!on) return;
+        cudaEventRecord(ev.b, s);
+        h->ev_used.push_back(ev);
+    }
+};
+
+size_t grid_cells(const muser_imager* h) { return (size_t)h->ngrids * h->ny * h->nx; }
+bool wmode(const muser_imager* h) { return h->nplanes > 0; }
+
+void free_grids(muser_imager* h) {
+    cudaFree(h->G); cudaFree(h->Gw); cudaFree(h->H); cudaFree(h->out_dirty); cudaFree(h->out_psf);
+    h->G = nullptr; h->Gw = nullptr; h->H = nullptr; h->out_dirty = h->out_psf = nullptr;
+    if (h->plan_ok) { cufftDestroy(h->plan); h->plan_ok = false; }
+}
+
+void free_bins(muser_imager* h) {
+    cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
+    h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
+}
+
+int rebuild_geom(muser_imager* h) {
+    Geom& g = h->geom;
+    g.nx = h->nx; g.ny = h->ny; g.Q = h->Q; g.ngrids = h->ngrids;
+    g.nplanes = wmode(h) ? h->nplanes : 1;
+    g.wmode = wmode(h) ? 1 : 0;
+    const double cell = h->cell_arcsec * kArcsec;       // same operation order as DESIGN.md O1
+    g.su = (double)h->nx * cell;
+    g.sv = (double)h->ny * cell;
+    g.ntx = (h->nx - 1 + kTile / 2) / kTile + 1;
+    g.nty = (h->ny - 1 + kTile / 2) / kTile + 1;
+    const unsigned long long nb = (unsigned long long)h->ngrids * g.nplanes * g.nty * g.ntx;
+    if (nb >= 0x7FFFFFFFull) return fail(h, MUSER_EUNSUPPORTED, "too many (grid, plane, tile) bins");
+    g.nbins = (uint32_t)nb;
+    g.chunk = 512;
+    return MUSER_OK;
+}
+
+// (re)allocate and zero the grids for the current nx, ny, ngrids, mode
+int alloc_grids(muser_imager* h) {
+    free_grids(h);
+    free_bins(h);
+    const size_t nc = grid_cells(h);
+    CU(h, cudaMalloc(&h->G, nc * sizeof(float2)));
+    CU(h, cudaMalloc(&h->Gw, nc * (wmode(h) ? sizeof(float2) : sizeof(float))));
+    CU(h, cudaMalloc(&h->H, nc * sizeof(float2)));
+    CU(h, cudaMemset(h->G, 0, nc * sizeof(float2)));
+    CU(h, cudaMemset(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float))));
+    CU(h, cudaMemset(h->stats_d, 0, sizeof(Stats)));
+    h->fft_valid = false;
+    return MUSER_OK;
+}
+
+// upload tables (transposed TT[r][j] = T[j*Q + r]) + plane metadata + correctors from fp64 host tables
+int upload_tables(muser_imager* h, const std::vector<std::vector<double>>& t64, const std::vector<int>& supports,
+                  const std::vector<double>& wc) {
+    const int P = (int)t64.size(), Q = h->Q;
+    const bool wm = wmode(h);
+    h->planes_h.assign(P, PlaneMeta{});
+    h->tables_f32.assign(P, {});
+    std::vector<float> dev;
+    for (int p = 0; p < P; ++p) {
+        const int S = supports[p], pitch = (S + 4) & ~3, comp = wm ? 2 : 1;
+        PlaneMeta& pm = h->planes_h[p];
+        pm.support = S; pm.pitch = pitch; pm.offset = (int)(dev.size() / comp); pm.pad = 0; pm.wc = wc[p];
+        const size_t L = (size_t)S * Q + 1;
+        h->tables_f32[p].resize(L * comp);
+        for (size_t i = 0; i < L * comp; ++i) h->tables_f32[p][i] = (float)t64[p][i];
+        const size_t base = dev.size();
+        dev.resize(base + (size_t)(Q + 1) * pitch * comp, 0.f);
+        for (int r = 0; r <= Q; ++r)
+            for (int j = 0; j < S; ++j)
+                for (int c = 0; c < comp; ++c)
+                    dev[base + ((size_t)r * pitch + j) * comp + c] = h->tables_f32[p][((size_t)j * Q + r) * comp + c];
+    }
+    cudaFree(h->tables_d); cudaFree(h->planes_d);
+    h->tables_d = nullptr; h->planes_d = nullptr;
+    CU(h, cudaMalloc(&h->tables_d, dev.size() * sizeof(float)));
+    CU(h, cudaMemcpy(h->tables_d, dev.data(), dev.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CU(h, cudaMalloc(&h->planes_d, P * sizeof(PlaneMeta)));
+    CU(h, cudaMemcpy(h->planes_d, h->planes_h.data(), P * sizeof(PlaneMeta), cudaMemcpyHostToDevice));
+    // correctors from plane 0 (real part), fp64 -> reciprocal -> fp32
+    std::vector<double> t0((size_t)supports[0] * Q + 1);
+    for (size_t i = 0; i < t0.size(); ++i) t0[i] = wm ? t64[0][2 * i] : t64[0][i];
+    const std::vector<double> cx = muser_host::corrector(t0.data(), supports[0], Q, h->nx);
+    const std::vector<double> cy = muser_host::corrector(t0.data(), supports[0], Q, h->ny);
+    std::vector<float> icx(h->nx), icy(h->ny), ones(std::max(h->nx, h->ny), 1.0f);
+    for (int x = 0; x < h->nx; ++x) icx[x] = (float)(1.0 / cx[x]);
+    for (int y = 0; y < h->ny; ++y) icy[y] = (float)(1.0 / cy[y]);
+    if (!h->icx_d) {
+        CU(h, cudaMalloc(&h->icx_d, h->nx * sizeof(float)));
+        CU(h, cudaMalloc(&h->icy_d, h->ny * sizeof(float)));
+        CU(h, cudaMalloc(&h->ones_d, ones.size() * sizeof(float)));
+        CU(h, cudaMemcpy(h->ones_d, ones.data(), ones.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    CU(h, cudaMemcpy(h->icx_d, icx.data(), h->nx * sizeof(float), cudaMemcpyHostToDevice));
+    CU(h, cudaMemcpy(h->icy_d, icy.data(), h->ny * sizeof(float), cudaMemcpyHostToDevice));
+    return MUSER_OK;
+}
+
+int build_2d_tables(muser_imager* h) {
+    std::vector<std::vector<double>> t64(1);
+    t64[0] = h->kind == MUSER_KERNEL_GAUSS ? muser_host::table_gauss(h->S, h->Q, h->gauss_a)
+                                           : muser_host::table_pswf(h->S, h->Q);
+    return upload_tables(h, t64, {h->S}, {0.0});
+}
+
+int ensure_scratch(muser_imager* h, long long nvis, bool tiled) {
+    const size_t ns = (size_t)2 * (size_t)nvis;
+    if (ns > h->sample_cap) {
+        cudaFree(h->staged); cudaFree(h->sorted);
+        h->staged = nullptr; h->sorted = nullptr; h->sample_cap = 0;
+        const size_t cap = ns + ns / 8 + 1024;
+        CU(h, cudaMalloc(&h->staged, cap * sizeof(Staged)));
+        CU(h, cudaMalloc(&h->sorted, cap * sizeof(Sample)));
+        h->sample_cap = cap;
+    }
+    if (tiled) {
+        const size_t nb = h->geom.nbins;
+        if (nb + 1 > h->bins_cap) {
+            cudaFree(h->bin_count); cudaFree(h->bin_offset);
+            h->bin_count = h->bin_offset = nullptr; h->bins_cap = 0;
+            CU(h, cudaMalloc(&h->bin_count, (nb + 1) * sizeof(uint32_t)));
+            CU(h, cudaMalloc(&h->bin_offset, (nb + 1) * sizeof(uint32_t)));
+            CU(h, cudaMemset(h->bin_count, 0, (nb + 1) * sizeof(uint32_t)));   // K2 re-zeroes it after every use
+            h->bins_cap = nb + 1;
+        }
+        const size_t ni = std::min(nb, h->sample_cap) + h->sample_cap / (size_t)h->geom.chunk + 2;
+        if (ni > h->items_cap) {
+            cudaFree(h->items); h->items = nullptr; h->items_cap = 0;
+            CU(h, cudaMalloc(&h->items, ni * sizeof(Item)));
+            h->items_cap = ni;
+        }
+    }
+    return MUSER_OK;
+}
+
+bool use_tiled(const muser_imager* h) {
+    if (h->strategy == MUSER_STRATEGY_TILED) return true;
+    if (h->strategy == MUSER_STRATEGY_DIRECT) return false;
+    return h->ngrids <= 4;
+}
+
+int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void* vis, const float* wt,
+              const int* gid, long long nvis, cudaStream_t s) {
+    if (nvis < 0 || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "nvis out of range [0, 2^30]");
+    if (nvis == 0) return MUSER_OK;
+    if (!uvw || !freq || !vis || !wt) return fail(h, MUSER_EINVAL, "null input pointer");
+    const bool tiled = use_tiled(h);
+    int rc = ensure_scratch(h, nvis, tiled);
+    if (rc) return rc;
+    h->last_stream = s;
+    h->fft_valid = false;
+    const Geom& g = h->geom;
+    GridPtrs gp{h->G, h->Gw};
+    {
+        StageScope sc(h, MUSER_STAGE_BIN, s);
+        CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
+                            h->stats_d, tiled ? 1 : 0, s));
+        if (tiled) {
+            CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, s));
+            CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
+        }
+    }
+    {
+        StageScope sc(h, MUSER_STAGE_GRID, s);
+        if (tiled)
+            CU(h, launch_grid_tiled(g, h->sorted, h->items, h->nitems_d, h->planes_d, h->planes_h.data(), h->tables_d,
+                                    gp, h->num_sms, s));
+        else
+            CU(h, launch_grid_direct(g, h->staged, 2 * nvis, h->planes_d, h->tables_d, gp, s));
+    }
+    return MUSER_OK;
+}
+
+int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
+    if (!dirty && !psf) return MUSER_OK;
+    h->last_stream = s;
+    if (!h->plan_ok) {
+        int dims[2] = {h->ny, h->nx};
+        cufftResult r = cufftPlanMany(&h->plan, 2, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, h->ngrids);
+        if (r != CUFFT_SUCCESS) return fail(h, MUSER_ECUDA, "cufftPlanMany failed: " + std::to_string((int)r));
+        h->plan_ok = true;
+    }
+    if (!h->fft_valid) {
+        {
+            StageScope sc(h, MUSER_STAGE_PACK, s);
+            CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, s));
+        }
+        {
+            StageScope sc(h, MUSER_STAGE_FFT, s);
+            cufftResult r = cufftSetStream(h->plan, s);
+            if (r == CUFFT_SUCCESS) r = cufftExecC2C(h->plan, (cufftComplex*)h->H, (cufftComplex*)h->H, CUFFT_INVERSE);
+            if (r != CUFFT_SUCCESS) return fail(h, MUSER_ECUDA, "cufftExecC2C failed: " + std::to_string((int)r));
+        }
+        h->fft_valid = true;
+    }
+    {
+        StageScope sc(h, MUSER_STAGE_CORRECT, s);
+        const float* cx = h->correction ? h->icx_d : h->ones_d;
+        const float* cy = h->correction ? h->icy_d : h->ones_d;
+        CU(h, launch_correct(h->geom, h->H, cx, cy, dirty, psf, s));
+    }
+    return MUSER_OK;
+}
+
+int reset_impl(muser_imager* h, cudaStream_t s) {
+    const size_t nc = grid_cells(h);
+    h->last_stream = s;
+    h->fft_valid = false;
+    CU(h, cudaMemsetAsync(h->G, 0, nc * sizeof(float2), s));
+    CU(h, cudaMemsetAsync(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), s));
+    CU(h, cudaMemsetAsync(h->stats_d, 0, sizeof(Stats), s));
+    return MUSER_OK;
+}
+
+}  // namespace
+
+// =================================================================================================== ABI
+extern "C" {
+
+const char* muser_version(void) { return "muser-b200 0.1 (sm_100a)"; }
+
+const char* muser_last_error(const muser_imager* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int support, int oversample) {
+    g_create_error.clear();
+    if (support < 1 || support > 63 || (support & 1) == 0) { fail(nullptr, MUSER_EINVAL, "support must be odd in [1,63]"); return nullptr; }
+    if (oversample < 2 || oversample > 256 || (oversample & 1)) { fail(nullptr, MUSER_EINVAL, "oversample must be even in [2,256]"); return nullptr; }
+    if (nx < 2 * (support + 1) || ny < 2 * (support + 1) || (nx & 3) || (ny & 3) || nx > 32768 || ny > 32768) {
+        fail(nullptr, MUSER_EINVAL, "nx, ny must be multiples of 4 in [2*(support+1), 32768]"); return nullptr;
+    }
+    if (!(cell_arcsec > 0) || !std::isfinite(cell_arcsec)) { fail(nullptr, MUSER_EINVAL, "cell_arcsec must be > 0"); return nullptr; }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        fail(nullptr, MUSER_ECUDA, std::string("no CUDA device (there is no CPU fallback): ") + cudaGetErrorString(e));
+        return nullptr;
+    }
+    muser_imager* h = new muser_imager();
+    h->nx = nx; h->ny = ny; h->cell_arcsec = cell_arcsec; h->S = support; h->Q = oversample;
+    cudaGetDevice(&h->device);
+    cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device);
+    cudaDeviceGetAttribute(&h->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+    int rc = rebuild_geom(h);
+    auto bail = [&](const char* what) -> muser_imager* {
+        g_create_error = std::string(what) + ": " + h->err;
+        muser_imager_destroy(h);
+        return nullptr;
+    };
+    if (rc) return bail("geometry");
+    if (tiled_kernel_setup(h->max_smem) != cudaSuccess) { h->err = cudaGetErrorString(cudaGetLastError()); return bail("kernel setup"); }
+    if (cudaMalloc(&h->stats_d, sizeof(Stats)) != cudaSuccess || cudaMalloc(&h->nitems_d, sizeof(uint32_t)) != cudaSuccess) {
+        h->err = "cudaMalloc failed"; return bail("alloc");
+    }
+    if (build_2d_tables(h)) return bail("tables");
+    if (alloc_grids(h)) return bail("grids");
+    return h;
+}
+
+int muser_imager_destroy(muser_imager* h) {
+    if (!h) return MUSER_OK;
+    cudaDeviceSynchronize();
+    free_grids(h);
+    free_bins(h);
+    cudaFree(h->staged); cudaFree(h->sorted); cudaFree(h->stats_d); cudaFree(h->nitems_d);
+    cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
+    cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
+    for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    delete h;
+    return MUSER_OK;
+}
+
+int muser_set_kernel(muser_imager* h, int kind, double param) {
+    if (!h) return MUSER_EINVAL;
+    if (kind != MUSER_KERNEL_PSWF && kind != MUSER_KERNEL_GAUSS) return fail(h, MUSER_EINVAL, "unknown kernel kind");
+    if (kind == MUSER_KERNEL_GAUSS && (param < 0 || !std::isfinite(param))) return fail(h, MUSER_EINVAL, "gaussian width must be >= 0");
+    cudaDeviceSynchronize();
+    h->kind = kind;
+    h->gauss_a = (kind == MUSER_KERNEL_GAUSS && param > 0) ? param : 1.55;
+    const bool was_w = wmode(h);
+    h->nplanes = 0;
+    int rc = rebuild_geom(h);
+    if (rc) return rc;
+    if ((rc = build_2d_tables(h))) return rc;
+    if (was_w) return alloc_grids(h);
+    return reset_impl(h, nullptr);
+}
+
+int muser_set_batch(muser_imager* h, int ngrids) {
+    if (!h) return MUSER_EINVAL;
+    if (ngrids < 1 || ngrids > (1 << 24) - 1) return fail(h, MUSER_EINVAL, "ngrids must be in [1, 2^24)");
+    cudaDeviceSynchronize();
+    const int old = h->ngrids;
+    h->ngrids = ngrids;
+    int rc = rebuild_geom(h);
+    if (rc) { h->ngrids = old; rebuild_geom(h); return rc; }
+    return alloc_grids(h);
+}
+
+int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, const int* supports,
+                      const float* const* tables_c64) {
+    if (!h) return MUSER_EINVAL;
+    if (nplanes < 0 || nplanes > kMaxPlanes) return fail(h, MUSER_EINVAL, "nplanes must be in [0, 64]");
+    cudaDeviceSynchronize();
+    if (nplanes == 0) {
+        const bool was_w = wmode(h);
+        h->nplanes = 0;
+        int rc = rebuild_geom(h);
+        if (rc) return rc;
+        if ((rc = build_2d_tables(h))) return rc;
+        return was_w ? alloc_grids(h) : reset_impl(h, nullptr);
+    }
+    if (!w_centres || !supports) return fail(h, MUSER_EINVAL, "w_centres and supports are required");
+    std::vector<int> sup(nplanes);
+    std::vector<double> wc(nplanes);
+    for (int p = 0; p < nplanes; ++p) {
+        sup[p] = supports[p]; wc[p] = w_centres[p];
+        if (sup[p] < 1 || sup[p] > 63 || !(sup[p] & 1)) return fail(h, MUSER_EINVAL, "plane supports must be odd in [1,63]");
+        if (!(wc[p] >= 0) || !std::isfinite(wc[p])) return fail(h, MUSER_EINVAL, "plane centres must be finite and >= 0");
+        if (h->nx < 2 * (sup[p] + 1) || h->ny < 2 * (sup[p] + 1)) return fail(h, MUSER_EINVAL, "grid too small for a plane support");
+    }
+    std::vector<std::vector<double>> t64(nplanes);
+    if (tables_c64) {
+        for (int p = 0; p < nplanes; ++p) {
+            if (!tables_c64[p]) return fail(h, MUSER_EINVAL, "null plane table");
+            const size_t L = ((size_t)sup[p] * h->Q + 1) * 2;
+            t64[p].resize(L);
+            for (size_t i = 0; i < L; ++i) t64[p][i] = (double)tables_c64[p][i];
+        }
+    } else {
+        const muser_host::WKernelGen gen(4096);
+        const double fov = (double)h->nx * (h->cell_arcsec * kArcsec);
+        for (int p = 0; p < nplanes; ++p) {
+            const auto t = gen.table(sup[p], h->Q, wc[p], fov);
+            t64[p].resize(t.size() * 2);
+            for (size_t i = 0; i < t.size(); ++i) { t64[p][2 * i] = t[i].real(); t64[p][2 * i + 1] = t[i].imag(); }
+        }
+    }
+    h->nplanes = nplanes;
+    int rc = rebuild_geom(h);
+    if (rc) return rc;
+    if ((rc = upload_tables(h, t64, sup, wc))) return rc;
+    return alloc_grids(h);
+}
+
+int muser_set_strategy(muser_imager* h, int strategy) {
+    if (!h) return MUSER_EINVAL;
+    if (strategy < MUSER_STRATEGY_AUTO || strategy > MUSER_STRATEGY_TILED) return fail(h, MUSER_EINVAL, "unknown strategy");
+    h->strategy = strategy;
+    return MUSER_OK;
+}
+
+int muser_set_grid_correction(muser_imager* h, int enabled) {
+    if (!h) return MUSER_EINVAL;
+    h->correction = enabled ? 1 : 0;
+    return MUSER_OK;
+}
+
+int muser_reset(muser_imager* h, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    return reset_impl(h, (cudaStream_t)s);
+}
+
+int muser_grid(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64, const float* weight,
+               long long nvis, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    return grid_impl(h, uvw_m, freq_hz, vis_c64, weight, nullptr, nvis, (cudaStream_t)s);
+}
+
+int muser_grid_batched(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                       const float* weight, const int* grid_id, long long nvis, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    if (!grid_id && nvis > 0) return fail(h, MUSER_EINVAL, "grid_id is required");
+    return grid_impl(h, uvw_m, freq_hz, vis_c64, weight, grid_id, nvis, (cudaStream_t)s);
+}
+
+int muser_dirty(muser_imager* h, float* image_out, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    if (!image_out) return fail(h, MUSER_EINVAL, "image_out is null");
+    return image_impl(h, image_out, nullptr, (cudaStream_t)s);
+}
+
+int muser_psf(muser_imager* h, float* beam_out, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    if (!beam_out) return fail(h, MUSER_EINVAL, "beam_out is null");
+    return image_impl(h, nullptr, beam_out, (cudaStream_t)s);
+}
+
+int muser_dirty_psf(muser_imager* h, float* image_out, float* beam_out, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    return image_impl(h, image_out, beam_out, (cudaStream_t)s);
+}
+
+int muser_frame_host(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                     const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
+                     muser_stream sv) {
+    if (!h) return MUSER_EINVAL;
+    if (nvis < 0 || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "nvis out of range");
+    if (nvis > 0 && (!uvw_m || !freq_hz || !vis_c64 || !weight)) return fail(h, MUSER_EINVAL, "null input pointer");
+    cudaStream_t s = (cudaStream_t)sv;
+    if ((size_t)nvis > h->in_cap) {
+        cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
+        h->in_uvw = nullptr; h->in_freq = nullptr; h->in_vis = nullptr; h->in_wt = nullptr; h->in_gid = nullptr; h->in_cap = 0;
+        const size_t cap = (size_t)nvis + 1024;
+        CU(h, cudaMalloc(&h->in_uvw, cap * 3 * sizeof(float)));
+        CU(h, cudaMalloc(&h->in_freq, cap * sizeof(double)));
+        CU(h, cudaMalloc(&h->in_vis, cap * sizeof(float2)));
+        CU(h, cudaMalloc(&h->in_wt, cap * sizeof(float)));
+        CU(h, cudaMalloc(&h->in_gid, cap * sizeof(int)));
+        h->in_cap = cap;
+    }
+    const size_t img_bytes = grid_cells(h) * sizeof(float);
+    if (image_out && !h->out_dirty) CU(h, cudaMalloc(&h->out_dirty, img_bytes));
+    if (beam_out && !h->out_psf) CU(h, cudaMalloc(&h->out_psf, img_bytes));
+    int rc = reset_impl(h, s);
+    if (rc) return rc;
+    if (nvis > 0) {
+        CU(h, cudaMemcpyAsync(h->in_uvw, uvw_m, (size_t)nvis * 3 * sizeof(float), cudaMemcpyHostToDevice, s));
+        CU(h, cudaMemcpyAsync(h->in_freq, freq_hz, (size_t)nvis * sizeof(double), cudaMemcpyHostToDevice, s));
+        CU(h, cudaMemcpyAsync(h->in_vis, vis_c64, (size_t)nvis * sizeof(float2), cudaMemcpyHostToDevice, s));
+        CU(h, cudaMemcpyAsync(h->in_wt, weight, (size_t)nvis * sizeof(float), cudaMemcpyHostToDevice, s));
+        if (grid_id) CU(h, cudaMemcpyAsync(h->in_gid, grid_id, (size_t)nvis * sizeof(int), cudaMemcpyHostToDevice, s));
+        rc = grid_impl(h, h->in_uvw, h->in_freq, h->in_vis, h->in_wt, grid_id ? h->in_gid : nullptr, nvis, s);
+        if (rc) return rc;
+    }
+    rc = image_impl(h, image_out ? h->out_dirty : nullptr, beam_out ? h->out_psf : nullptr, s);
+    if (rc) return rc;
+    if (image_out) CU(h, cudaMemcpyAsync(image_out, h->out_dirty, img_bytes, cudaMemcpyDeviceToHost, s));
+    if (beam_out) CU(h, cudaMemcpyAsync(beam_out, h->out_psf, img_bytes, cudaMemcpyDeviceToHost, s));
+    CU(h, cudaStreamSynchronize(s));
+    return MUSER_OK;
+}
+
+int muser_get_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_stream sv) {
+    if (!h) return MUSER_EINVAL;
+    cudaStream_t s = (cudaStream_t)sv;
+    const size_t nc = grid_cells(h);
+    h->last_stream = s;
+    if (grid_c64_out) CU(h, cudaMemcpyAsync(grid_c64_out, h->G, nc * sizeof(float2), cudaMemcpyDeviceToDevice, s));
+    if (wgrid_out) CU(h, cudaMemcpyAsync(wgrid_out, h->Gw, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), cudaMemcpyDeviceToDevice, s));
+    return MUSER_OK;
+}
+
+int muser_get_table(muser_imager* h, int plane, float* table_out_host, int* len) {
+    if (!h || !len) return MUSER_EINVAL;
+    if (plane < 0 || plane >= (int)h->tables_f32.size()) return fail(h, MUSER_EINVAL, "plane out of range");
+    const std::vector<float>& t = h->tables_f32[plane];
+    if (!table_out_host || *len < (int)t.size()) { *len = (int)t.size(); return table_out_host ? fail(h, MUSER_EINVAL, "table buffer too small") : MUSER_OK; }
+    std::memcpy(table_out_host, t.data(), t.size() * sizeof(float));
+    *len = (int)t.size();
+    return MUSER_OK;
+}
+
+int muser_get_stats(muser_imager* h, double* sum_weights, long long* n_gridded, long long* n_dropped, long long* n_flagged) {
+    if (!h) return MUSER_EINVAL;
+    CU(h, cudaStreamSynchronize(h->last_stream));
+    Stats st;
+    CU(h, cudaMemcpy(&st, h->stats_d, sizeof(Stats), cudaMemcpyDeviceToHost));
+    if (sum_weights) *sum_weights = st.sum_weights;
+    if (n_gridded) *n_gridded = (long long)st.n_gridded;
+    if (n_dropped) *n_dropped = (long long)st.n_dropped;
+    if (n_flagged) *n_flagged = (long long)st.n_flagged;
+    return MUSER_OK;
+}
+
+int muser_set_profiling(muser_imager* h, int enabled) {
+    if (!h) return MUSER_EINVAL;
+    cudaDeviceSynchronize();
+    for (auto& ev : h->ev_used) h->ev_free.push_back(ev);
+    h->ev_used.clear();
+    for (int i = 0; i < MUSER_STAGE_COUNT; ++i) { h->stage_ms[i] = 0; h->stage_n[i] = 0; }
+    h->profiling = enabled != 0;
+    return MUSER_OK;
+}
+
+int muser_get_profile(muser_imager* h, double* stage_ms, long long* stage_launches) {
+    if (!h) return MUSER_EINVAL;
+    CU(h, cudaDeviceSynchronize());
+    for (auto& ev : h->ev_used) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, ev.a, ev.b) == cudaSuccess) { h->stage_ms[ev.stage] += ms; h->stage_n[ev.stage] += 1; }
+        h->ev_free.push_back(ev);
+    }
+    h->ev_used.clear();
+    for (int i = 0; i < MUSER_STAGE_COUNT; ++i) {
+        if (stage_ms) stage_ms[i] = h->stage_ms[i];
+        if (stage_launches) stage_launches[i] = h->stage_n[i];
+    }
+    return MUSER_OK;
+}
+
+int muser_host_table(int kind, int support, int oversample, double param, double* table_out) {
+    if (!table_out || support < 1 || support > 63 || !(support & 1) || oversample < 2 || oversample > 256 || (oversample & 1)) return MUSER_EINVAL;
+    std::vector<double> t;
+    if (kind == MUSER_KERNEL_PSWF) t = muser_host::table_pswf(support, oversample);
+    else if (kind == MUSER_KERNEL_GAUSS) t = muser_host::table_gauss(support, oversample, param > 0 ? param : 1.55);
+    else return MUSER_EINVAL;
+    std::memcpy(table_out, t.data(), t.size() * sizeof(double));
+    return MUSER_OK;
+}
+
+int muser_host_wtable(int support, int oversample, double w_lambda, double fov_rad, double* table_out_re_im) {
+    if (!table_out_re_im || support < 1 || support > 63 || !(support & 1) || oversample < 2 || oversample > 256 || (oversample & 1)) return MUSER_EINVAL;
+    const muser_host::WKernelGen gen(4096);
+    const auto t = gen.table(support, oversample, w_lambda, fov_rad);
+    for (size_t i = 0; i < t.size(); ++i) { table_out_re_im[2 * i] = t[i].real(); table_out_re_im[2 * i + 1] = t[i].imag(); }
+    return MUSER_OK;
+}
+
+int muser_host_corrector(const double* table, int support, int oversample, int n, double* corr_out) {
+    if (!table || !corr_out || support < 1 || oversample < 2 || n < 1) return MUSER_EINVAL;
+    const std::vector<double> c = muser_host::corrector(table, support, oversample, n);
+    std::memcpy(corr_out, c.data(), c.size() * sizeof(double));
+    return MUSER_OK;
+}
+
+}  // extern "C"

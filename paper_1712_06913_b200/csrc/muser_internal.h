@@ -1,0 +1,80 @@
+// Internal declarations shared by the kernels (muser_kernels.cu) and the C ABI (muser_api.cu).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace muser {
+
+constexpr int kTile = 32;          // uv tile edge in cells (A1 sort key, A2 shared-memory accumulator)
+constexpr int kTileShift = 5;
+constexpr int kMaxPlanes = 64;
+constexpr uint32_t kNoBin = 0xFFFFFFFFu;
+
+// Geometry and mode, passed by value to every kernel.
+struct Geom {
+    int nx, ny, Q, ngrids, nplanes, wmode;
+    double su, sv;                 // nx*cell, ny*cell (rad): u_pix = u_lambda*su + nx/2 (O1)
+    int ntx, nty;                  // tiles per axis; tile tx covers cells [tx*32-16, tx*32+16) so DC sits mid-tile
+    uint32_t nbins;                // ngrids*max(nplanes,1)*nty*ntx
+    int chunk;                     // samples per work item of the tiled gridder
+};
+
+// Per-plane kernel metadata in constant-ish device memory.
+struct PlaneMeta {
+    int support;                   // S_p (odd)
+    int pitch;                     // row pitch of the transposed table TT[r][j], j < pitch, entries >= S_p are 0
+    int offset;                    // offset of the plane's TT in the table buffer (floats in 2-D mode, float2 in w mode)
+    int pad;
+    double wc;                     // plane centre in |w| wavelengths
+};
+
+// K1 output, one per SAMPLE (2 per visibility; slot 2k = primary, 2k+1 = conjugate).
+struct __align__(16) Staged {
+    float re, im, wt;              // wt*Re V, +-wt*Im V, wt
+    uint32_t cell;                 // iu0 | iv0 << 16 (nearest grid cell)
+    uint32_t phase;                // rx | ry << 9 | kconj << 18, rx = Q/2 - ru in [0, Q]
+    uint32_t bin;                  // ((g*P + p)*nty + ty)*ntx + tx, or kNoBin if the sample is not gridded
+    uint32_t rank;                 // arrival order inside the bin (tiled strategy)
+    uint32_t gp;                   // grid | plane << 24
+};
+
+// K3 output, tile-sorted, 16 B: what the tiled gridder streams.
+struct __align__(16) Sample {
+    float re, im, wt;
+    uint32_t packed;               // lx | ly << 5 | rx << 10 | ry << 19 | kconj << 28 (lx, ly: cell inside the tile)
+};
+
+struct Item {                      // work item of the tiled gridder: <= chunk samples of one bin
+    uint32_t bin, start, count;
+};
+
+struct Stats {
+    double sum_weights;
+    unsigned long long n_gridded, n_dropped, n_flagged;
+};
+
+struct GridPtrs {
+    float2* G;                     // [ngrids][ny][nx] complex
+    float* Gw;                     // [ngrids][ny][nx] real (2-D) or complex interleaved (w mode)
+};
+
+// ---- launch wrappers (muser_kernels.cu); all asynchronous on `s` -------------------------------------------
+cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                          const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
+                          uint32_t* bin_count, Stats* stats, int do_bin, cudaStream_t s);
+cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,
+                              uint32_t* nitems, cudaStream_t s);
+cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsamples, const uint32_t* bin_offset,
+                           Sample* sorted, cudaStream_t s);
+cudaError_t launch_grid_direct(const Geom& g, const Staged* staged, long long nsamples, const PlaneMeta* planes,
+                               const float* tables, GridPtrs grids, cudaStream_t s);
+cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* nitems,
+                              const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
+                              GridPtrs grids, int num_sms, cudaStream_t s);
+cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, cudaStream_t s);
+cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, float* dirty,
+                           float* psf, cudaStream_t s);
+cudaError_t tiled_kernel_setup(int max_smem_bytes);
+
+}  // namespace muser

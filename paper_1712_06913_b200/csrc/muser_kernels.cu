@@ -1,0 +1,557 @@
+// Device kernels of the MUSER dirty-imaging hot path, sm_100a.
+//   K1 k_coords       A1: fp64 coordinates, keep/drop, Hermitian conjugate sample, tile histogram + rank
+//   K2 k_scan_items   A1: exclusive scan of the tile histogram, work items of <= chunk samples
+//   K3 k_scatter      A1: counting-sort scatter into 16-byte tile-local samples
+//   K4 k_grid_*       A2/A3/A4: convolutional gridding (tiled shared-memory accumulators, or direct reductions)
+//   Kp k_pack         H = G + i*Gw, the single FFT input that yields dirty image and beam together
+//   K5 k_correct      A6: fused fftshift (index roll + checkerboard sign) + grid correction + real/imag part
+// Passages: PAPER.md:78 (gridding = convolution onto a regular grid), :136-138 (spheroidal GCF, inverse FFT),
+// :216-228 (float2 grid, row-major iv*nu+iu, Hermitian), :249-256 (DIRTY_IMAGE).  Arithmetic order of the
+// coordinates follows DESIGN.md O1 exactly (fp64, no FMA contraction) so that every integer decision
+// (cell, oversample phase, plane, keep/drop) is the oracle's decision.
+#include "muser_internal.h"
+
+#include <math_constants.h>
+
+namespace muser {
+
+static constexpr double kC = 299792458.0;   // m/s
+
+// ------------------------------------------------------------------------------------------------- K1
+// O1 for one axis: p = c*scale + n/2; i0 = floor(p + 0.5); r = floor((p - i0)*Q + 0.5).  Explicit _rn
+// intrinsics keep nvcc from contracting mul+add into an FMA (the oracle has none).
+__device__ __forceinline__ void cell_phase(double c_lambda, double scale, int n, int Q, double& i0, double& r) {
+    const double p = __dadd_rn(__dmul_rn(c_lambda, scale), (double)(n / 2));
+    i0 = floor(__dadd_rn(p, 0.5));
+    const double fr = __dsub_rn(p, i0);
+    r = floor(__dadd_rn(__dmul_rn(fr, (double)Q), 0.5));
+}
+
+__global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __restrict__ uvw,
+                                                const double* __restrict__ freq, const float2* __restrict__ vis,
+                                                const float* __restrict__ weight, const int* __restrict__ grid_id,
+                                                const long long nvis, const PlaneMeta* __restrict__ planes,
+                                                Staged* __restrict__ staged, uint32_t* __restrict__ bin_count,
+                                                Stats* __restrict__ stats, const int do_bin) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int flagged = 0, dropped = 0, kept = 0;
+    double wsum = 0.0;
+    if (k < nvis) {
+        const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
+        const double f = freq[k];
+        const float2 V = vis[k];
+        const float wt = weight[k];
+        const int gid = grid_id ? grid_id[k] : 0;
+        const double il = __ddiv_rn(f, kC);
+        const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
+        const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) &&
+                        isfinite(V.y) && isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
+        Staged s0, s1;
+        s0.bin = s1.bin = kNoBin;
+        if (!ok) {
+            flagged = 1;
+        } else {
+            int p = 0;
+            if (g.wmode) {                                   // O6: nearest plane centre in |w|, tie -> lower p
+                const double aw = fabs(wl);
+                double best = fabs(__dsub_rn(aw, planes[0].wc));
+                for (int q = 1; q < g.nplanes; ++q) {
+                    const double d = fabs(__dsub_rn(aw, planes[q].wc));
+                    if (d < best) { best = d; p = q; }
+                }
+            }
+            const int S = planes[p].support, h = (S - 1) >> 1;
+            double iu[2], iv[2], ru[2], rv[2];
+            bool inside = true;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const double sgn = s ? -1.0 : 1.0;
+                cell_phase(sgn * ul, g.su, g.nx, g.Q, iu[s], ru[s]);
+                cell_phase(sgn * vl, g.sv, g.ny, g.Q, iv[s], rv[s]);
+                inside = inside && iu[s] >= (double)(h + 1) && iu[s] <= (double)(g.nx - 1 - h) &&
+                         iv[s] >= (double)(h + 1) && iv[s] <= (double)(g.ny - 1 - h);
+            }
+            if (!inside) {
+                dropped = 1;
+            } else {
+                kept = 1;
+                wsum = 2.0 * (double)wt;
+                const int P = g.wmode ? g.nplanes : 1;
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    Staged& o = s ? s1 : s0;
+                    const int cu = (int)iu[s], cv = (int)iv[s];
+                    const int rx = g.Q / 2 - (int)ru[s], ry = g.Q / 2 - (int)rv[s];
+                    const int kconj = g.wmode && ((s ? -wl : wl) < 0.0);
+                    o.re = wt * V.x;
+                    o.im = s ? -(wt * V.y) : wt * V.y;
+                    o.wt = wt;
+                    o.cell = (uint32_t)cu | ((uint32_t)cv << 16);
+                    o.phase = (uint32_t)rx | ((uint32_t)ry << 9) | ((uint32_t)kconj << 18);
+                    o.gp = (uint32_t)gid | ((uint32_t)p << 24);
+                    const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
+                    o.bin = (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
+                    o.rank = do_bin ? atomicAdd(&bin_count[o.bin], 1u) : 0u;
+                }
+            }
+        }
+        uint4* dst = reinterpret_cast<uint4*>(staged + 2 * k);
+        const uint4* a = reinterpret_cast<const uint4*>(&s0);
+        const uint4* b = reinterpret_cast<const uint4*>(&s1);
+        dst[0] = a[0]; dst[1] = a[1]; dst[2] = b[0]; dst[3] = b[1];
+    }
+    // block reduction of the counters, one atomic set per block
+    __shared__ int s_cnt[3][8];
+    __shared__ double s_w[8];
+    const unsigned full = 0xffffffffu;
+    int c0 = __reduce_add_sync(full, kept), c1 = __reduce_add_sync(full, dropped), c2 = __reduce_add_sync(full, flagged);
+    for (int o = 16; o > 0; o >>= 1) wsum += __shfl_xor_sync(full, wsum, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { s_cnt[0][warp] = c0; s_cnt[1][warp] = c1; s_cnt[2][warp] = c2; s_w[warp] = wsum; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t0 = 0, t1 = 0, t2 = 0;
+        double tw = 0.0;
+        for (int w = 0; w < 8; ++w) { t0 += s_cnt[0][w]; t1 += s_cnt[1][w]; t2 += s_cnt[2][w]; tw += s_w[w]; }
+        if (t0) { atomicAdd(&stats->n_gridded, (unsigned long long)t0); atomicAdd(&stats->sum_weights, tw); }
+        if (t1) atomicAdd(&stats->n_dropped, (unsigned long long)t1);
+        if (t2) atomicAdd(&stats->n_flagged, (unsigned long long)t2);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- K2
+// One CTA walks the histogram 1024 bins at a time: exclusive offsets, work items, and re-zeroes the histogram
+// for the next call.
+__global__ void __launch_bounds__(1024) k_scan_items(const Geom g, uint32_t* __restrict__ bin_count,
+                                                     uint32_t* __restrict__ bin_offset, Item* __restrict__ items,
+                                                     uint32_t* __restrict__ nitems) {
+    __shared__ uint32_t s_wsum[2][32];
+    __shared__ uint32_t s_carry[2];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) { s_carry[0] = 0; s_carry[1] = 0; }
+    __syncthreads();
+    const uint32_t CH = (uint32_t)g.chunk;
+    for (uint32_t base = 0; base < g.nbins; base += 1024) {
+        const uint32_t b = base + threadIdx.x;
+        uint32_t c = 0;
+        if (b < g.nbins) { c = bin_count[b]; if (c) bin_count[b] = 0; }
+        const uint32_t n = (c + CH - 1) / CH;
+        uint32_t ic = c, in = n;                                      // inclusive warp scans
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t tc = __shfl_up_sync(0xffffffffu, ic, o), tn = __shfl_up_sync(0xffffffffu, in, o);
+            if (lane >= o) { ic += tc; in += tn; }
+        }
+        if (lane == 31) { s_wsum[0][warp] = ic; s_wsum[1][warp] = in; }
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t wc = s_wsum[0][lane], wn = s_wsum[1][lane];
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t tc = __shfl_up_sync(0xffffffffu, wc, o), tn = __shfl_up_sync(0xffffffffu, wn, o);
+                if (lane >= o) { wc += tc; wn += tn; }
+            }
+            s_wsum[0][lane] = wc; s_wsum[1][lane] = wn;               // inclusive over warps
+        }
+        __syncthreads();
+        const uint32_t off = s_carry[0] + (warp ? s_wsum[0][warp - 1] : 0) + ic - c;
+        const uint32_t ioff = s_carry[1] + (warp ? s_wsum[1][warp - 1] : 0) + in - n;
+        if (b < g.nbins) {
+            bin_offset[b] = off;
+            for (uint32_t j = 0; j < n; ++j) {
+                Item it;
+                it.bin = b; it.start = off + j * CH; it.count = min(CH, c - j * CH);
+                items[ioff + j] = it;
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) { s_carry[0] = off + c; s_carry[1] = ioff + n; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { bin_offset[g.nbins] = s_carry[0]; *nitems = s_carry[1]; }
+}
+
+// ------------------------------------------------------------------------------------------------- K3
+__global__ void __launch_bounds__(256) k_scatter(const Geom g, const Staged* __restrict__ staged,
+                                                 const long long nsamples, const uint32_t* __restrict__ bin_offset,
+                                                 Sample* __restrict__ sorted) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nsamples) return;
+    const uint4* src = reinterpret_cast<const uint4*>(staged + i);
+    const uint4 a = src[0], b = src[1];                                // a: re im wt cell ; b: phase bin rank gp
+    if (b.y == kNoBin) return;
+    const uint32_t tx = b.y % (uint32_t)g.ntx, ty = (b.y / (uint32_t)g.ntx) % (uint32_t)g.nty;
+    const int cu = (int)(a.w & 0xFFFFu), cv = (int)(a.w >> 16);
+    const int lx = cu - ((int)tx * kTile - kTile / 2), ly = cv - ((int)ty * kTile - kTile / 2);
+    const uint32_t rx = b.x & 511u, ry = (b.x >> 9) & 511u, kc = (b.x >> 18) & 1u;
+    uint4 o;
+    o.x = a.x; o.y = a.y; o.z = a.z;
+    o.w = (uint32_t)lx | ((uint32_t)ly << 5) | (rx << 10) | (ry << 19) | (kc << 28);
+    reinterpret_cast<uint4*>(sorted)[bin_offset[b.y] + b.z] = o;
+}
+
+// ------------------------------------------------------------------------------------------------- K4 direct
+// One warp per sample, lanes over the S*S footprint, vector reductions straight to the L2-resident grids.
+// Used for batches of small grids (A4) where a tile holds only a handful of samples.
+template <int WMODE>
+__global__ void __launch_bounds__(256) k_grid_direct(const Geom g, const Staged* __restrict__ staged,
+                                                     const long long nsamples, const PlaneMeta* __restrict__ planes,
+                                                     const float* __restrict__ tables, GridPtrs grids) {
+    const int lane = threadIdx.x & 31;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < nsamples; i += nwarps) {
+        const uint4* src = reinterpret_cast<const uint4*>(staged + i);
+        const uint4 a = __ldg(src), b = __ldg(src + 1);
+        if (b.y == kNoBin) continue;
+        const float re = __uint_as_float(a.x), im = __uint_as_float(a.y), wt = __uint_as_float(a.z);
+        const int cu = (int)(a.w & 0xFFFFu), cv = (int)(a.w >> 16);
+        const int rx = (int)(b.x & 511u), ry = (int)((b.x >> 9) & 511u), kc = (int)((b.x >> 18) & 1u);
+        const int gi = (int)(b.w & 0xFFFFFFu), p = (int)(b.w >> 24);
+        const PlaneMeta pm = planes[p];
+        const int S = pm.support, h = (S - 1) >> 1;
+        const size_t gbase = (size_t)gi * g.ny * g.nx;
+        for (int c = lane; c < S * S; c += 32) {
+            const int jy = c / S, jx = c - jy * S;
+            const size_t idx = gbase + (size_t)(cv - h + jy) * g.nx + (size_t)(cu - h + jx);
+            if (WMODE == 0) {
+                const float kk = __ldg(tables + pm.offset + rx * pm.pitch + jx) * __ldg(tables + pm.offset + ry * pm.pitch + jy);
+                atomicAdd(&grids.G[idx], make_float2(kk * re, kk * im));
+                atomicAdd(&grids.Gw[idx], kk * wt);
+            } else {
+                const float2* tc = reinterpret_cast<const float2*>(tables);
+                float2 kx = __ldg(tc + pm.offset + rx * pm.pitch + jx), ky = __ldg(tc + pm.offset + ry * pm.pitch + jy);
+                if (kc) { kx.y = -kx.y; ky.y = -ky.y; }
+                const float kr = kx.x * ky.x - kx.y * ky.y, ki = kx.x * ky.y + kx.y * ky.x;
+                atomicAdd(&grids.G[idx], make_float2(kr * re - ki * im, kr * im + ki * re));
+                atomicAdd(reinterpret_cast<float2*>(grids.Gw) + idx, make_float2(kr * wt, ki * wt));
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- K4 tiled
+__device__ __forceinline__ void decode_bin(const Geom& g, uint32_t bin, int& gi, int& p, int& ty, int& tx) {
+    tx = (int)(bin % (uint32_t)g.ntx); bin /= (uint32_t)g.ntx;
+    ty = (int)(bin % (uint32_t)g.nty); bin /= (uint32_t)g.nty;
+    const uint32_t P = g.wmode ? (uint32_t)g.nplanes : 1u;
+    p = (int)(bin % P);
+    gi = (int)(bin / P);
+}
+
+// Generic tiled gridder (any support, 2-D or w mode): one work item = <= chunk samples of one (grid, plane,
+// tile).  The CTA accumulates the tile plus its halo ((32+2h)^2 cells) in shared memory with one warp per
+// sample, then adds the touched cells to the grids with vector reductions.
+template <int WMODE>
+__global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const Sample* __restrict__ sorted,
+                                                            const Item* __restrict__ items,
+                                                            const uint32_t* __restrict__ nitems,
+                                                            const PlaneMeta* __restrict__ planes,
+                                                            const float* __restrict__ tables, GridPtrs grids) {
+    extern __shared__ __align__(16) float smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t n_items = *nitems;
+    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+        const Item item = items[it];
+        int gi, p, ty, tx;
+        decode_bin(g, item.bin, gi, p, ty, tx);
+        const PlaneMeta pm = planes[p];
+        const int S = pm.support, h = (S - 1) >> 1, R = kTile + 2 * h, RR = R * R;
+        constexpr int NPL = WMODE ? 4 : 3;                          // planes: G.re G.im W(.re) [W.im]
+        for (int i = threadIdx.x; i < NPL * RR; i += blockDim.x) smem[i] = 0.f;
+        __syncthreads();
+        for (uint32_t i = warp; i < item.count; i += 8) {
+            const uint4 a = __ldg(reinterpret_cast<const uint4*>(sorted + item.start + i));
+            const float re = __uint_as_float(a.x), im = __uint_as_float(a.y), wt = __uint_as_float(a.z);
+            const int lx = (int)(a.w & 31u), ly = (int)((a.w >> 5) & 31u);
+            const int rx = (int)((a.w >> 10) & 511u), ry = (int)((a.w >> 19) & 511u), kc = (int)((a.w >> 28) & 1u);
+            for (int c = lane; c < S * S; c += 32) {
+                const int jy = c / S, jx = c - jy * S;
+                const int si = (ly + jy) * R + lx + jx;              // region origin is (tile origin - h)
+                if (WMODE == 0) {
+                    const float kk = __ldg(tables + pm.offset + rx * pm.pitch + jx) * __ldg(tables + pm.offset + ry * pm.pitch + jy);
+                    atomicAdd(&smem[si], kk * re);
+                    atomicAdd(&smem[RR + si], kk * im);
+                    atomicAdd(&smem[2 * RR + si], kk * wt);
+                } else {
+                    const float2* tc = reinterpret_cast<const float2*>(tables);
+                    float2 kx = __ldg(tc + pm.offset + rx * pm.pitch + jx), ky = __ldg(tc + pm.offset + ry * pm.pitch + jy);
+                    if (kc) { kx.y = -kx.y; ky.y = -ky.y; }
+                    const float kr = kx.x * ky.x - kx.y * ky.y, ki = kx.x * ky.y + kx.y * ky.x;
+                    atomicAdd(&smem[si], kr * re - ki * im);
+                    atomicAdd(&smem[RR + si], kr * im + ki * re);
+                    atomicAdd(&smem[2 * RR + si], kr * wt);
+                    atomicAdd(&smem[3 * RR + si], ki * wt);
+                }
+            }
+        }
+        __syncthreads();
+        const int x0 = tx * kTile - kTile / 2 - h, y0 = ty * kTile - kTile / 2 - h;
+        const size_t gbase = (size_t)gi * g.ny * g.nx;
+        for (int i = threadIdx.x; i < RR; i += blockDim.x) {
+            const int y = i / R, x = i - y * R;
+            const int gx = x0 + x, gy = y0 + y;
+            if (gx < 0 || gx >= g.nx || gy < 0 || gy >= g.ny) continue;
+            const size_t idx = gbase + (size_t)gy * g.nx + gx;
+            const float vr = smem[i], vi = smem[RR + i], wr = smem[2 * RR + i];
+            if (vr != 0.f || vi != 0.f) atomicAdd(&grids.G[idx], make_float2(vr, vi));
+            if (WMODE == 0) {
+                if (wr != 0.f) atomicAdd(&grids.Gw[idx], wr);
+            } else {
+                const float wi = smem[3 * RR + i];
+                if (wr != 0.f || wi != 0.f) atomicAdd(reinterpret_cast<float2*>(grids.Gw) + idx, make_float2(wr, wi));
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// Fast path: 2-D mode, support 7.  Per work item the CTA (1) counting-sorts its <= 512 samples by nearest
+// cell inside the tile, (2) lets each warp walk an equal slice of the sorted list with the 7x7 footprint held
+// in registers (lane = (row jy, column jx), two rows per lane), flushing to the shared tile only when the
+// nearest cell changes -- MUSER's uv coverage puts many samples on the same cell -- and (3) adds the touched
+// cells of the 38x38 region to the grids.
+constexpr int kFastChunk = 512;
+constexpr int kFastR = 38, kFastPitch = 40;                 // pitch 40 = 8 mod 32: the 4 rows of a warp hit disjoint banks
+
+__global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sample* __restrict__ sorted,
+                                                       const Item* __restrict__ items,
+                                                       const uint32_t* __restrict__ nitems,
+                                                       const PlaneMeta* __restrict__ planes,
+                                                       const float* __restrict__ tables, GridPtrs grids) {
+    extern __shared__ __align__(16) float smem[];
+    constexpr int PL = kFastR * kFastPitch;                 // floats per accumulator plane
+    float* s_re = smem;
+    float* s_im = smem + PL;
+    float* s_w = smem + 2 * PL;
+    uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + 3 * PL);           // 1024 cells of the tile
+    float4* s_rec = reinterpret_cast<float4*>(smem + 3 * PL + 1024);         // kFastChunk samples, cell-sorted
+    float* s_tt = smem + 3 * PL + 1024 + 4 * kFastChunk;                    // (Q+1) x 8 transposed table
+    __shared__ uint32_t s_wsum[8];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int jx = lane & 7, jy = lane >> 3;
+    const PlaneMeta pm = planes[0];
+    for (int i = threadIdx.x; i < (g.Q + 1) * 8; i += blockDim.x) s_tt[i] = __ldg(tables + pm.offset + i);
+    const uint32_t n_items = *nitems;
+    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+        const Item item = items[it];
+        int gi, p, ty, tx;
+        decode_bin(g, item.bin, gi, p, ty, tx);
+        {   // zero accumulators and histogram
+            float4* z = reinterpret_cast<float4*>(smem);
+            for (int i = threadIdx.x; i < (3 * PL + 1024) / 4; i += blockDim.x) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        __syncthreads();
+        // (1) local counting sort by cell
+        float4 rec[kFastChunk / 256];
+        uint32_t rnk[kFastChunk / 256];
+#pragma unroll
+        for (int j = 0; j < kFastChunk / 256; ++j) {
+            const uint32_t i = threadIdx.x + j * 256;
+            if (i < item.count) {
+                rec[j] = __ldg(reinterpret_cast<const float4*>(sorted + item.start + i));
+                rnk[j] = atomicAdd(&s_hist[__float_as_uint(rec[j].w) & 1023u], 1u);
+            }
+        }
+        __syncthreads();
+        {
+            uint4 hv = reinterpret_cast<uint4*>(s_hist)[threadIdx.x];
+            const uint32_t tot = hv.x + hv.y + hv.z + hv.w;
+            uint32_t inc = tot;
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (lane == 31) s_wsum[warp] = inc;
+            __syncthreads();
+            uint32_t base = inc - tot;
+            for (int w = 0; w < warp; ++w) base += s_wsum[w];
+            uint4 ov;
+            ov.x = base; ov.y = base + hv.x; ov.z = ov.y + hv.y; ov.w = ov.z + hv.z;
+            reinterpret_cast<uint4*>(s_hist)[threadIdx.x] = ov;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kFastChunk / 256; ++j) {
+            const uint32_t i = threadIdx.x + j * 256;
+            if (i < item.count) s_rec[s_hist[__float_as_uint(rec[j].w) & 1023u] + rnk[j]] = rec[j];
+        }
+        __syncthreads();
+        // (2) register accumulation over runs of equal cell
+        {
+            const int n = (int)item.count, per = (n + 7) >> 3;
+            const int b = warp * per, e = min(n, b + per);
+            float a0r = 0.f, a0i = 0.f, a0w = 0.f, a1r = 0.f, a1i = 0.f, a1w = 0.f;
+            int cur = -1;
+            auto flush = [&]() {
+                if (cur >= 0 && jx < 7) {
+                    const int lx = cur & 31, ly = cur >> 5;
+                    const int s0 = (ly + jy) * kFastPitch + lx + jx;
+                    atomicAdd(&s_re[s0], a0r); atomicAdd(&s_im[s0], a0i); atomicAdd(&s_w[s0], a0w);
+                    if (jy < 3) {
+                        const int s1 = s0 + 4 * kFastPitch;
+                        atomicAdd(&s_re[s1], a1r); atomicAdd(&s_im[s1], a1i); atomicAdd(&s_w[s1], a1w);
+                    }
+                }
+            };
+            for (int i = b; i < e; ++i) {
+                const float4 r = s_rec[i];
+                const uint32_t pk = __float_as_uint(r.w);
+                const int cell = (int)(pk & 1023u);
+                if (cell != cur) {
+                    flush();
+                    cur = cell;
+                    a0r = a0i = a0w = a1r = a1i = a1w = 0.f;
+                }
+                const int rx = (int)((pk >> 10) & 511u), ry = (int)((pk >> 19) & 511u);
+                const float kx = s_tt[rx * 8 + jx];
+                const float ky0 = s_tt[ry * 8 + jy], ky1 = s_tt[ry * 8 + jy + 4];
+                const float k0 = kx * ky0, k1 = kx * ky1;
+                a0r = fmaf(k0, r.x, a0r); a0i = fmaf(k0, r.y, a0i); a0w = fmaf(k0, r.z, a0w);
+                a1r = fmaf(k1, r.x, a1r); a1i = fmaf(k1, r.y, a1i); a1w = fmaf(k1, r.z, a1w);
+            }
+            flush();
+        }
+        __syncthreads();
+        // (3) add the touched cells of the region to the grids
+        const int x0 = tx * kTile - kTile / 2 - 3, y0 = ty * kTile - kTile / 2 - 3;
+        const size_t gbase = (size_t)gi * g.ny * g.nx;
+        for (int i = threadIdx.x; i < PL; i += blockDim.x) {
+            const int y = i / kFastPitch, x = i - y * kFastPitch;
+            const int gx = x0 + x, gy = y0 + y;
+            if (x >= kFastR || gx < 0 || gx >= g.nx || gy < 0 || gy >= g.ny) continue;
+            const size_t idx = gbase + (size_t)gy * g.nx + gx;
+            const float vr = s_re[i], vi = s_im[i], vw = s_w[i];
+            if (vr != 0.f || vi != 0.f) atomicAdd(&grids.G[idx], make_float2(vr, vi));
+            if (vw != 0.f) atomicAdd(&grids.Gw[idx], vw);
+        }
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- pack, K5
+// H = G + i*Gw: G and Gw are both Hermitian, so their inverse transforms are real and one complex FFT of H
+// returns the dirty image in the real part and the beam in the imaginary part.
+template <int WMODE>
+__global__ void __launch_bounds__(256) k_pack(const size_t ncell2, const float4* __restrict__ G,
+                                              const float* __restrict__ Gw, float4* __restrict__ H) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // two cells per thread
+    if (i >= ncell2) return;
+    const float4 gv = G[i];
+    float4 o;
+    if (WMODE == 0) {
+        const float2 w = reinterpret_cast<const float2*>(Gw)[i];
+        o = make_float4(gv.x, gv.y + w.x, gv.z, gv.w + w.y);
+    } else {
+        const float4 w = reinterpret_cast<const float4*>(Gw)[i];
+        o = make_float4(gv.x - w.y, gv.y + w.x, gv.z - w.w, gv.w + w.z);
+    }
+    H[i] = o;
+}
+
+// A6: img[y][x] = (-1)^(x+y) * F_raw[(y+ny/2)%ny][(x+nx/2)%nx] * icx[x] * icy[y]  (nx/2, ny/2 even);
+// dirty from the real part, beam from the imaginary part.  Four pixels per thread.
+__global__ void __launch_bounds__(256) k_correct(const int nx, const int ny, const int ngrids,
+                                                 const float2* __restrict__ F, const float* __restrict__ icx,
+                                                 const float* __restrict__ icy, float* __restrict__ dirty,
+                                                 float* __restrict__ psf) {
+    const int nx4 = nx >> 2;
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t total = (size_t)ngrids * ny * nx4;
+    if (t >= total) return;
+    const int x = (int)(t % nx4) << 2;
+    const size_t row = t / nx4;
+    const int y = (int)(row % ny);
+    const size_t gi = row / ny;
+    const int sy = (y + (ny >> 1)) % ny;
+    const int sx0 = (x + (nx >> 1)) % nx, sx2 = (x + 2 + (nx >> 1)) % nx;  // pairs never wrap (nx/2 is even)
+    const float2* srow = F + (gi * ny + sy) * (size_t)nx;
+    const float4 f01 = *reinterpret_cast<const float4*>(srow + sx0);
+    const float4 f23 = *reinterpret_cast<const float4*>(srow + sx2);
+    const float4 cx = *reinterpret_cast<const float4*>(icx + x);
+    const float cy = (y & 1) ? -icy[y] : icy[y];                         // x is a multiple of 4: sign = (-1)^y * (+,-,+,-)
+    const float m0 = cx.x * cy, m1 = -cx.y * cy, m2 = cx.z * cy, m3 = -cx.w * cy;
+    const size_t o = (gi * ny + y) * (size_t)nx + x;
+    if (dirty) *reinterpret_cast<float4*>(dirty + o) = make_float4(f01.x * m0, f01.z * m1, f23.x * m2, f23.z * m3);
+    if (psf) *reinterpret_cast<float4*>(psf + o) = make_float4(f01.y * m0, f01.w * m1, f23.y * m2, f23.w * m3);
+}
+
+// ------------------------------------------------------------------------------------------------- launchers
+static inline unsigned blocks_for(long long n, int per) { return (unsigned)((n + per - 1) / per); }
+
+cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                          const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
+                          uint32_t* bin_count, Stats* stats, int do_bin, cudaStream_t s) {
+    k_coords<<<blocks_for(nvis, 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, planes, staged, bin_count,
+                                                   stats, do_bin);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,
+                              uint32_t* nitems, cudaStream_t s) {
+    k_scan_items<<<1, 1024, 0, s>>>(g, bin_count, bin_offset, items, nitems);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsamples, const uint32_t* bin_offset,
+                           Sample* sorted, cudaStream_t s) {
+    k_scatter<<<blocks_for(nsamples, 256), 256, 0, s>>>(g, staged, nsamples, bin_offset, sorted);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_grid_direct(const Geom& g, const Staged* staged, long long nsamples, const PlaneMeta* planes,
+                               const float* tables, GridPtrs grids, cudaStream_t s) {
+    const long long want = (nsamples + 7) / 8;                            // 8 warps per CTA, one sample per warp pass
+    const unsigned blocks = (unsigned)(want < 1 ? 1 : (want > 148LL * 64 ? 148LL * 64 : want));
+    if (g.wmode) k_grid_direct<1><<<blocks, 256, 0, s>>>(g, staged, nsamples, planes, tables, grids);
+    else k_grid_direct<0><<<blocks, 256, 0, s>>>(g, staged, nsamples, planes, tables, grids);
+    return cudaGetLastError();
+}
+
+static size_t generic_smem_bytes(int wmode, int smax) {
+    const int R = kTile + (smax - 1);
+    return (size_t)(wmode ? 4 : 3) * R * R * sizeof(float);
+}
+static size_t fast_smem_bytes(int Q) {
+    return (size_t)(3 * kFastR * kFastPitch + 1024 + 4 * kFastChunk + (Q + 1) * 8) * sizeof(float);
+}
+
+cudaError_t tiled_kernel_setup(int max_smem_bytes) {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_grid_tiled_s7, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
+    return cudaSuccess;
+}
+
+cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* nitems,
+                              const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
+                              GridPtrs grids, int num_sms, cudaStream_t s) {
+    const int P = g.wmode ? g.nplanes : 1;
+    int smax = 1;
+    for (int p = 0; p < P; ++p) smax = planes_host[p].support > smax ? planes_host[p].support : smax;
+    if (!g.wmode && smax == 7 && g.chunk == kFastChunk) {
+        k_grid_tiled_s7<<<num_sms * 4, 256, fast_smem_bytes(g.Q), s>>>(g, sorted, items, nitems, planes, tables, grids);
+    } else {
+        const size_t smem = generic_smem_bytes(g.wmode, smax);
+        const int per_sm = smem > 110 * 1024 ? 1 : (smem > 70 * 1024 ? 2 : 4);
+        if (g.wmode) k_grid_tiled_generic<1><<<num_sms * per_sm, 256, smem, s>>>(g, sorted, items, nitems, planes, tables, grids);
+        else k_grid_tiled_generic<0><<<num_sms * per_sm, 256, smem, s>>>(g, sorted, items, nitems, planes, tables, grids);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, cudaStream_t s) {
+    const size_t ncell2 = (size_t)g.ngrids * g.ny * g.nx / 2;
+    const unsigned blocks = (unsigned)((ncell2 + 255) / 256);
+    if (g.wmode) k_pack<1><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H));
+    else k_pack<0><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, float* dirty,
+                           float* psf, cudaStream_t s) {
+    const size_t total = (size_t)g.ngrids * g.ny * (g.nx / 4);
+    k_correct<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(g.nx, g.ny, g.ngrids, F, icx, icy, dirty, psf);
+    return cudaGetLastError();
+}
+
+}  // namespace muser

@@ -1,0 +1,246 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI / binding) against the fp64 oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's: grid relative L2 <= 1e-5, images max-abs <= 1e-4 of
+the peak (gates of DESIGN.md R9).  Integer results (counters) must be equal."""
+import numpy as np
+import pytest
+
+from oracle import muser_oracle as mo
+from oracle import oracle_c as oc
+from paper_1712_06913_b200 import binding, synth
+
+import gpu_util as gu
+
+pytestmark = pytest.mark.gpu
+
+DIRECT, TILED = binding.MUSER_STRATEGY_DIRECT, binding.MUSER_STRATEGY_TILED
+
+
+@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_single_grid_configs_match_oracle(cfg, strategy):
+    fr = synth.make_frame(cfg)
+    p = fr.params
+    res = gu.run_case(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, p.n, p.cell_arcsec, p.support, p.oversample,
+                      kernel=p.kernel, strategy=strategy)
+    assert res["stats"]["n_gridded"] > 0.9 * fr.nvis
+
+
+@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("S,Q,nvis", [(7, 128, 1), (7, 16, 31), (7, 128, 5000), (3, 8, 777), (5, 32, 1000), (9, 64, 1500),
+                                      (1, 2, 100), (15, 16, 300)])
+def test_random_visibilities_any_support(S, Q, nvis, strategy):
+    n, cell = 128, 40.0
+    uvw, freq, vis, wt = synth.random_visibilities(7 + S, nvis, n, cell, margin_cells=S / 2 + 2)
+    gu.run_case(uvw, freq, vis, wt, n, cell, S, Q, strategy=strategy)
+
+
+@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+def test_accumulation_over_calls_equals_one_call(strategy):
+    fr = synth.make_frame(2)
+    p = fr.params
+    gu.run_case(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, p.n, p.cell_arcsec, p.support, p.oversample,
+                strategy=strategy, splits=5, images=False)
+
+
+@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+def test_flagged_and_off_grid_visibilities_are_skipped_and_counted(strategy):
+    n, cell = 256, 20.0
+    uvw, freq, vis, wt = synth.random_visibilities(3, 4000, n, cell, margin_cells=0.0)   # some fall off the grid
+    rng = np.random.default_rng(5)
+    bad = rng.choice(4000, 400, replace=False)
+    wt[bad[:100]] = 0.0
+    wt[bad[100:150]] = -1.0
+    wt[bad[150:180]] = np.nan
+    vis[bad[180:230]] = np.nan + 0j
+    vis[bad[230:260]] = complex(0.0, np.inf)
+    uvw[bad[260:300], 0] = np.inf
+    uvw[bad[300:340], 2] = np.nan
+    freq[bad[340:370]] = np.nan
+    uvw[bad[370:400], 1] = 1e30          # finite but absurdly far off the grid -> dropped, not flagged
+    res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, 32, strategy=strategy)
+    assert res["stats"]["n_flagged"] == 370
+    assert res["stats"]["n_dropped"] >= 30
+
+
+def test_empty_input_and_reset():
+    import torch
+    im = gu.make_imager(128, 40.0, 7, 8)
+    try:
+        z = torch.zeros(0, device="cuda")
+        im.grid(z.reshape(0, 3), z.double(), z.reshape(0, 2), z)            # nvis = 0: no-op
+        uvw, freq, vis, wt = synth.random_visibilities(0, 100, 128, 40.0)
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        assert im.get_stats()["n_gridded"] == 100
+        im.reset()
+        G, Gw = gu.gpu_grids(im)
+        assert not G.any() and not Gw.any()
+        st = im.get_stats()
+        assert st == dict(sum_weights=0.0, n_gridded=0, n_dropped=0, n_flagged=0)
+        d, p = gu.gpu_images(im)
+        assert not d.any() and not p.any()
+    finally:
+        im.destroy()
+
+
+def test_dirty_and_psf_separately_equal_the_fused_call():
+    import torch
+    fr = synth.make_frame(1)
+    p = fr.params
+    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample, kernel=p.kernel)
+    try:
+        im.grid(gu.to_dev(fr.uvw_m), gu.to_dev(fr.freq_hz), gu.to_dev(fr.vis), gu.to_dev(fr.weight))
+        a = torch.empty((p.n, p.n), device="cuda"); b = torch.empty_like(a); c = torch.empty_like(a); d = torch.empty_like(a)
+        im.psf(b); im.dirty(a)                # either order; the transform is shared
+        im.dirty_psf(c, d)
+        torch.cuda.synchronize()
+        assert torch.equal(a, c) and torch.equal(b, d)
+        # gridding more afterwards still works (the grids are not consumed by imaging)
+        im.grid(gu.to_dev(fr.uvw_m), gu.to_dev(fr.freq_hz), gu.to_dev(fr.vis), gu.to_dev(fr.weight))
+        im.dirty(c)
+        torch.cuda.synchronize()
+        assert torch.allclose(c, 2 * a, rtol=1e-4, atol=1e-3 * float(a.abs().max()))
+    finally:
+        im.destroy()
+
+
+def test_point_source_peak_is_sum_of_weights_P1():
+    fr = synth.make_frame(2)
+    p = fr.params
+    vis = np.ones_like(fr.vis)
+    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample)
+    try:
+        im.grid(gu.to_dev(fr.uvw_m), gu.to_dev(fr.freq_hz), gu.to_dev(vis), gu.to_dev(fr.weight))
+        d, b = gu.gpu_images(im)
+        sw = im.get_stats()["sum_weights"]
+        assert abs(d[0, p.n // 2, p.n // 2] / sw - 1) < 2e-3
+        assert np.unravel_index(np.argmax(d[0]), d[0].shape) == (p.n // 2, p.n // 2)
+        assert np.abs(d - b).max() <= 1e-4 * sw          # V = 1: dirty image == beam
+    finally:
+        im.destroy()
+
+
+def test_device_table_matches_oracle_table():
+    for kernel, S, Q in (("pswf", 7, 128), ("gauss", 7, 8)):
+        im = gu.make_imager(64, 60.0, S, Q, kernel=kernel)
+        try:
+            assert np.abs(im.get_table(0) - gu.oracle_table(kernel, S, Q)).max() <= 1e-7
+        finally:
+            im.destroy()
+
+
+def _wplane_case(n, cell, P, Q, nvis, w_max, seed, library_tables):
+    wc, sup = mo.wplane_layout(n, cell, P, w_max)
+    fov = n * cell * mo.ARCSEC
+    tabs = [mo.table_wkernel(int(S), Q, float(w), fov) for S, w in zip(sup, wc)]
+    uvw, freq, vis, wt = synth.random_visibilities(seed, nvis, n, cell, margin_cells=sup.max() / 2 + 2, w_max_lambda=w_max)
+    return wc, sup, tabs, (uvw, freq, vis, wt)
+
+
+@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("library_tables", [False, True])
+def test_wprojection_planes_match_oracle(strategy, library_tables):
+    n, cell, P, Q, w_max = 256, 60.0, 6, 16, 4000.0          # fov 4.3 deg: supports 7..17
+    wc, sup, tabs, (uvw, freq, vis, wt) = _wplane_case(n, cell, P, Q, 3000, w_max, 11, library_tables)
+    assert sup.max() >= 13
+    im = gu.make_imager(n, cell, 7, Q, strategy=strategy)
+    try:
+        im.set_wplanes(wc, sup, None if library_tables else [t.astype(np.complex64) for t in tabs])
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        G, Gw = gu.gpu_grids(im)
+        G_or, Gw_or, st_or = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, sup, tabs, wc=wc)
+        st = im.get_stats()
+        assert (st["n_gridded"], st["n_dropped"], st["n_flagged"]) == (st_or["n_gridded"], st_or["n_dropped"], st_or["n_flagged"])
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL
+        assert gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        gu.check_images(im, G_or, Gw_or, tabs[0].real, int(sup[0]), Q)
+        for p_ in range(P):
+            assert np.abs(im.get_table(p_).view(np.complex64) - tabs[p_]).max() <= 2e-7
+    finally:
+        im.destroy()
+
+
+@pytest.mark.parametrize("strategy", [DIRECT, TILED])
+def test_batched_grids_cfg4_slice(strategy):
+    fr = synth.make_frame(4, nframes=1)                       # 32 grids of 512x512, 1770 visibilities each
+    p = fr.params
+    assert p.ngrids == 32
+    gu.run_case(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, p.n, p.cell_arcsec, p.support, p.oversample,
+                strategy=strategy, grid_id=fr.grid_id, ngrids=p.ngrids)
+
+
+def test_batched_rejects_out_of_range_grid_ids_as_flagged():
+    n, cell = 128, 40.0
+    uvw, freq, vis, wt = synth.random_visibilities(1, 500, n, cell)
+    gid = (np.arange(500) % 5 - 1).astype(np.int32)           # -1 and 3 are outside [0, 3)
+    res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, 8, grid_id=np.clip(gid, 0, 2), ngrids=3, images=False)
+    im = gu.make_imager(n, cell, 7, 8, ngrids=3)
+    try:
+        im.grid_batched(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), gu.to_dev(gid))
+        st = im.get_stats()
+        assert st["n_flagged"] == int(((gid < 0) | (gid >= 3)).sum())
+        assert st["n_gridded"] + st["n_dropped"] + st["n_flagged"] == 500
+    finally:
+        im.destroy()
+    assert res["stats"]["n_flagged"] == 0
+
+
+def test_cfg5_reduced_wprojection_4096():
+    fr = synth.make_frame(5, nsnap=2)                         # 113,280 visibilities, 4096^2 grid, 32 planes
+    p = fr.params
+    w_max = float(np.abs(fr.uvw_m[:, 2].astype(np.float64) * fr.freq_hz / mo.C_M_S).max())
+    wc, sup = mo.wplane_layout(p.n, p.cell_arcsec, p.nplanes, 19900.0)
+    assert w_max < 19900.0 and sup.min() == 7 and sup.max() == 31
+    fov = p.n * p.cell_arcsec * mo.ARCSEC
+    tabs = [mo.table_wkernel(int(S), p.oversample, float(w), fov) for S, w in zip(sup, wc)]
+    im = gu.make_imager(p.n, p.cell_arcsec, 7, p.oversample)
+    try:
+        im.set_wplanes(wc, sup, [t.astype(np.complex64) for t in tabs])
+        im.grid(gu.to_dev(fr.uvw_m), gu.to_dev(fr.freq_hz), gu.to_dev(fr.vis), gu.to_dev(fr.weight))
+        G, Gw = gu.gpu_grids(im)
+        G_or, Gw_or, st_or = oc.grid(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, p.n, p.n, p.cell_arcsec, p.oversample,
+                                     sup, tabs, wc=wc)
+        assert im.get_stats()["n_gridded"] == st_or["n_gridded"]
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL
+        assert gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        gu.check_images(im, G_or, Gw_or, tabs[0].real, 7, p.oversample)
+    finally:
+        im.destroy()
+
+
+def test_frame_host_end_to_end_equals_device_path():
+    import torch
+    fr = synth.make_frame(2)
+    p = fr.params
+    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample)
+    try:
+        d_host = np.empty((p.n, p.n), np.float32); b_host = np.empty((p.n, p.n), np.float32)
+        im.frame_host(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, None, d_host, b_host)
+        im.frame_host(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, None, d_host, b_host)   # resets: no accumulation
+        d = torch.empty((p.n, p.n), device="cuda"); b = torch.empty_like(d)
+        im.reset()
+        im.grid(gu.to_dev(fr.uvw_m), gu.to_dev(fr.freq_hz), gu.to_dev(fr.vis), gu.to_dev(fr.weight))
+        im.dirty_psf(d, b)
+        torch.cuda.synchronize()
+        peak = float(d.abs().max())
+        assert np.abs(d_host - d.cpu().numpy()).max() <= 1e-5 * peak
+        assert np.abs(b_host - b.cpu().numpy()).max() <= 1e-5 * float(b.abs().max())
+    finally:
+        im.destroy()
+
+
+def test_abi_argument_errors_on_device():
+    L = binding.lib()
+    im = gu.make_imager(128, 40.0, 7, 8)
+    try:
+        h = im._h
+        assert L.muser_grid(h, None, None, None, None, 5, None) == binding.MUSER_EINVAL
+        assert L.muser_grid(h, None, None, None, None, -1, None) == binding.MUSER_EINVAL
+        assert L.muser_grid(h, None, None, None, None, 0, None) == binding.MUSER_OK
+        assert L.muser_dirty(h, None, None) == binding.MUSER_EINVAL
+        assert L.muser_set_batch(h, 0) == binding.MUSER_EINVAL
+        assert L.muser_set_kernel(h, 9, 0.0) == binding.MUSER_EINVAL
+        assert L.muser_set_strategy(h, 17) == binding.MUSER_EINVAL
+        assert b"strategy" in L.muser_last_error(h)
+        assert L.muser_set_wplanes(h, 2, None, None, None) == binding.MUSER_EINVAL
+    finally:
+        im.destroy()
