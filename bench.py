@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the MUSER dirty-imaging hot path (BASELINE.json: "gridded visibilities/s and dirty
+images/s (MUSER-II frame), % of roofline").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Workload: BASELINE.json configs[2], the MUSER-II full frame (60 antennas -> 1770 baselines x 16 channels x 2
+polarisations = 56,640 visibilities -> 113,280 gridded samples, 1024^2 grid, PSWF support 7, oversample 128).
+One STEP = one pass of the whole hot path (reset -> bin -> grid -> pack -> cuFFT -> correct: dirty image + beam)
+over a batch of FRAMES_PER_STEP = 80 distinct seeded synthetic frames (145 MB of inputs, larger than the 126 MB
+L2, so every frame's inputs come from HBM).  value = input visibilities gridded per second over all ranks, inputs
+resident in HBM; e2e = the same through muser_frame_host with pinned HOST buffers (H2D + D2H inside the timing).
+Multi-GPU: frames are independent, so ranks process disjoint frames with no data-path collective (weak scaling).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+CFG = 3
+FRAMES_PER_STEP = 80
+METRIC = "gridded_visibilities_per_s"
+UNIT = "vis/s"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def make_frames(nframes, seed0=0):
+    """nframes distinct frames of the cfg-3 shape: the array geometry and sky are those of synth.make_frame(3); every
+    frame gets its own noise realisation (so buffers differ and nothing is cached between frames)."""
+    from paper_1712_06913_b200 import synth
+    base = synth.make_frame(CFG)
+    frames = []
+    for k in range(nframes):
+        rng = np.random.default_rng([synth.SEED0, 1000 + CFG, seed0 + k])
+        noise = (rng.standard_normal((base.nvis, 2)) * 0.05).astype(np.float32)
+        vis = (base.vis + (noise[:, 0] + 1j * noise[:, 1]).astype(np.complex64)).astype(np.complex64)
+        frames.append((base.uvw_m.copy(), base.freq_hz.copy(), vis, base.weight.copy()))
+    return base.params, frames
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and clock-event reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def sample(self):
+        if not self.nv:
+            return
+        nv = self.nv
+        try:
+            self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+            r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+            names = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown,
+                     "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
+                     "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown,
+                     "sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap}
+            for k, bit in names.items():
+                if r & bit:
+                    self.reasons.add(k)
+        except Exception:
+            pass
+
+    def run(self):
+        while not self.stop_flag:
+            self.sample()
+            time.sleep(0.002)
+
+    def result(self):
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+def cpu_oracle_frame(params, frame, T, cx):
+    """One frame through the oracle as it stands: plain-C fp64 gridder + numpy fp64 centred inverse FFT + correction
+    (dirty image and beam)."""
+    from oracle import muser_oracle as mo
+    from oracle import oracle_c as oc
+    uvw, freq, vis, wt = frame
+    G, Gw, st = oc.grid(uvw, freq, vis, wt, params.n, params.n, params.cell_arcsec, params.oversample, params.support, T)
+    d, _ = mo.dirty_image(G[0], cx, cx)
+    p, _ = mo.dirty_image(Gw[0].astype(np.complex128), cx, cx)
+    return d, p, st
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores; each step = ORACLE_FRAMES_PER_STEP frames of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import muser_oracle as mo
+    params, frames = make_frames(4)
+    T = mo.table_pswf(params.support, params.oversample)
+    cx = mo.corrector(T, params.support, params.oversample, params.n)
+    nvis = frames[0][2].shape[0]
+    per_step = 2
+    for w in range(args.warmup):
+        cpu_oracle_frame(params, frames[w % 4], T, cx)
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        for j in range(per_step):
+            cpu_oracle_frame(params, frames[(k * per_step + j) % 4], T, cx)
+    dt = time.perf_counter() - t0
+    value = args.steps * per_step * nvis / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[2] MUSER-II full frame: 56,640 vis -> 1024^2 dirty image + beam",
+                   "frames_per_step": per_step},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"{args.steps * per_step} whole frames (oracle_c gridder + numpy fp64 FFT + correction)"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "images_per_s": args.steps * per_step / dt,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="muser")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_1712_06913_b200 import binding, build
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if dist:
+        dist.barrier()
+    W = max(args.warmup, 3)
+
+    params, frames = make_frames(FRAMES_PER_STEP, seed0=rank * FRAMES_PER_STEP)
+    n, nvis = params.n, frames[0][2].shape[0]
+    dev = [[torch.from_numpy(a).cuda() for a in fr] for fr in frames]
+    im = binding.Imager(n, n, params.cell_arcsec, params.support, params.oversample)
+    dirty = torch.empty((n, n), device="cuda")
+    psf = torch.empty((n, n), device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for fr in dev:
+            im.reset()
+            im.grid(*fr)
+            im.dirty_psf(dirty, psf)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(W):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.sample()
+    sampler.start()
+    l0 = im.get_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    sampler.sample()
+    launches = im.get_launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    if dist:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    frames_total = args.steps * FRAMES_PER_STEP * world
+    value = frames_total * nvis / (ms * 1e-3)
+
+    # ---- per-stage device time, live, with CUDA events on the launching stream (second timed pass)
+    im.set_profiling(True)
+    for _ in range(max(1, min(args.steps, 5))):
+        step()
+    prof = im.get_profile()
+    im.set_profiling(False)
+    stage_us = {k: (1e3 * v[0] / v[1] if v[1] else None) for k, v in prof.items()}
+    grid_us = stage_us["grid"]
+    # algorithmic bytes of one gridding launch: 32 B per visibility (its two 16-byte samples)
+    # + every cell of G (8 B) and Gw (4 B) once
+    alg_bytes = 32.0 * nvis + 12.0 * n * n
+    peak, peak_src = _peaks()
+    achieved = alg_bytes / (grid_us * 1e-6) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_grid_tiled_s7", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "kernel_us": grid_us, "stage_us": stage_us}
+
+    # ---- end to end through the host-buffer entry point (pinned host memory; H2D + D2H inside the timed region)
+    pin = [[torch.from_numpy(a).pin_memory() for a in fr] for fr in frames[:16]]
+    d_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
+    p_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
+    for fr in pin[:3]:
+        im.frame_host(fr[0], fr[1], fr[2], fr[3], None, d_host, p_host)
+    barrier()
+    e2e_frames = max(16, min(args.steps * FRAMES_PER_STEP, 400))
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for k in range(e2e_frames):
+        fr = pin[k % len(pin)]
+        im.frame_host(fr[0], fr[1], fr[2], fr[3], None, d_host, p_host)
+    e1.record(stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    if dist:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = e2e_frames * world * nvis / (e2e_ms * 1e-3)
+    h2d = nvis * 32 * FRAMES_PER_STEP
+    d2h = 2 * n * n * 4 * FRAMES_PER_STEP
+
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        from oracle import muser_oracle as mo
+        T = mo.table_pswf(params.support, params.oversample)
+        cx = mo.corrector(T, params.support, params.oversample, n)
+        cpu_oracle_frame(params, frames[0], T, cx)
+        t0 = time.perf_counter()
+        done = 0
+        while done < 3 or (time.perf_counter() - t0 < 10.0 and done < FRAMES_PER_STEP):
+            cpu_oracle_frame(params, frames[done % len(frames)], T, cx)
+            done += 1
+        dt = time.perf_counter() - t0
+        cpu = {"value": done * nvis / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{done} whole frames of the workload (oracle_c fp64 gridder + numpy fp64 FFT + correction), "
+                         f"{dt:.1f} s on {os.cpu_count()} available cores, 1 used",
+               "images_per_s": done / dt}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "configs[2] MUSER-II full frame: 56,640 vis (113,280 samples) -> 1024^2 grid, PSWF S=7 Q=128 "
+                                   "-> dirty image + beam", "frames_per_step": FRAMES_PER_STEP, "nvis_per_frame": nvis,
+                       "l2_policy": "inputs rotate over 80 distinct frames (145 MB > 126 MB L2)", "launch": "stream",
+                       "parallelism": f"frames x{world}" if world > 1 else "single"},
+            "images_per_s": frames_total / (ms * 1e-3), "us_per_frame": 1e3 * ms / (args.steps * FRAMES_PER_STEP),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "frames_timed": e2e_frames, "us_per_frame": 1e3 * e2e_ms / e2e_frames},
+            "gpu_launches": int(launches), "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    im.destroy()
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

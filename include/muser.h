@@ -126,6 +126,8 @@ const char* muser_last_error(const muser_imager* h);
  * time in milliseconds and the number of launches since profiling was enabled (HOST arrays of MUSER_STAGE_COUNT). */
 int muser_set_profiling(muser_imager* h, int enabled);
 int muser_get_profile(muser_imager* h, double* stage_ms, long long* stage_launches);
+/* Number of the library's own kernels launched on this handle since creation (cuFFT's and memsets not counted). */
+long long muser_get_launch_count(const muser_imager* h);
 
 /* ---- host-only helpers (no GPU needed; used by the table-parity tests) ---------------------------------------
  * The library's own fp64 generators: kernel table T[t], t = 0..S*Q (kind as above; param: Gaussian a), and

@@ -42,6 +42,7 @@ SIGNATURES = {
     "muser_last_error": (_c.c_char_p, [_vp]),
     "muser_set_profiling": (_i, [_vp, _i]),
     "muser_get_profile": (_i, [_vp, _vp, _vp]),
+    "muser_get_launch_count": (_ll, [_vp]),
     "muser_host_table": (_i, [_i, _i, _i, _d, _vp]),
     "muser_host_wtable": (_i, [_i, _i, _d, _d, _vp]),
     "muser_host_corrector": (_i, [_vp, _i, _i, _i, _vp]),
@@ -197,6 +198,10 @@ class Imager:
         n = (ctypes.c_longlong * len(STAGES))()
         self._ck(lib().muser_get_profile(self._h, ms, n))
         return {s: (ms[i], n[i]) for i, s in enumerate(STAGES)}
+
+
+    def get_launch_count(self):
+        return int(lib().muser_get_launch_count(self._h))
 
 
 # ---- host-only helpers (no GPU): the library's own fp64 generators

@@ -58,6 +58,7 @@ struct muser_imager {
     std::vector<StageEvent> ev_used, ev_free;
     double stage_ms[MUSER_STAGE_COUNT] = {0};
     long long stage_n[MUSER_STAGE_COUNT] = {0};
+    long long n_launches = 0;
     std::string err;
 };
 
@@ -247,6 +248,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
             CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, s));
             CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
         }
+        h->n_launches += tiled ? 3 : 1;
     }
     {
         StageScope sc(h, MUSER_STAGE_GRID, s);
@@ -255,6 +257,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
                                     gp, h->num_sms, s));
         else
             CU(h, launch_grid_direct(g, h->staged, 2 * nvis, h->planes_d, h->tables_d, gp, s));
+        h->n_launches += 1;
     }
     return MUSER_OK;
 }
@@ -271,7 +274,8 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     if (!h->fft_valid) {
         {
             StageScope sc(h, MUSER_STAGE_PACK, s);
-            CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, s));
+            CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, h->stats_d, s));
+            h->n_launches += 1;
         }
         {
             StageScope sc(h, MUSER_STAGE_FFT, s);
@@ -285,7 +289,8 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         StageScope sc(h, MUSER_STAGE_CORRECT, s);
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
-        CU(h, launch_correct(h->geom, h->H, cx, cy, dirty, psf, s));
+        CU(h, launch_correct(h->geom, h->H, cx, cy, h->stats_d, dirty, psf, s));
+        h->n_launches += 1;
     }
     return MUSER_OK;
 }
@@ -576,6 +581,8 @@ int muser_get_profile(muser_imager* h, double* stage_ms, long long* stage_launch
     }
     return MUSER_OK;
 }
+
+long long muser_get_launch_count(const muser_imager* h) { return h ? h->n_launches : 0; }
 
 int muser_host_table(int kind, int support, int oversample, double param, double* table_out) {
     if (!table_out || support < 1 || support > 63 || !(support & 1) || oversample < 2 || oversample > 256 || (oversample & 1)) return MUSER_EINVAL;

@@ -52,6 +52,8 @@ struct Item {                      // work item of the tiled gridder: <= chunk s
 struct Stats {
     double sum_weights;
     unsigned long long n_gridded, n_dropped, n_flagged;
+    double sum_val2, sum_wt2;      // sum |wt*V|^2 and sum wt^2 over kept visibilities: scale of G against Gw
+    float alpha, inv_alpha;        // written by k_pack: H = G + i*alpha*Gw, alpha a power of two
 };
 
 struct GridPtrs {
@@ -72,9 +74,9 @@ cudaError_t launch_grid_direct(const Geom& g, const Staged* staged, long long ns
 cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* nitems,
                               const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
                               GridPtrs grids, int num_sms, cudaStream_t s);
-cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, cudaStream_t s);
-cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, float* dirty,
-                           float* psf, cudaStream_t s);
+cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, Stats* stats, cudaStream_t s);
+cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, const Stats* stats,
+                           float* dirty, float* psf, cudaStream_t s);
 cudaError_t tiled_kernel_setup(int max_smem_bytes);
 
 }  // namespace muser

@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                                                 Stats* __restrict__ stats, const int do_bin) {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int flagged = 0, dropped = 0, kept = 0;
-    double wsum = 0.0;
+    double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
     if (k < nvis) {
         const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
         const double f = freq[k];
@@ -76,6 +76,8 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
             } else {
                 kept = 1;
                 wsum = 2.0 * (double)wt;
+                w2sum = (double)wt * (double)wt;
+                v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
                 const int P = g.wmode ? g.nplanes : 1;
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
@@ -102,18 +104,30 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
     }
     // block reduction of the counters, one atomic set per block
     __shared__ int s_cnt[3][8];
-    __shared__ double s_w[8];
+    __shared__ double s_w[3][8];
     const unsigned full = 0xffffffffu;
     int c0 = __reduce_add_sync(full, kept), c1 = __reduce_add_sync(full, dropped), c2 = __reduce_add_sync(full, flagged);
-    for (int o = 16; o > 0; o >>= 1) wsum += __shfl_xor_sync(full, wsum, o);
+    for (int o = 16; o > 0; o >>= 1) {
+        wsum += __shfl_xor_sync(full, wsum, o);
+        v2sum += __shfl_xor_sync(full, v2sum, o);
+        w2sum += __shfl_xor_sync(full, w2sum, o);
+    }
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (lane == 0) { s_cnt[0][warp] = c0; s_cnt[1][warp] = c1; s_cnt[2][warp] = c2; s_w[warp] = wsum; }
+    if (lane == 0) { s_cnt[0][warp] = c0; s_cnt[1][warp] = c1; s_cnt[2][warp] = c2; s_w[0][warp] = wsum; s_w[1][warp] = v2sum; s_w[2][warp] = w2sum; }
     __syncthreads();
     if (threadIdx.x == 0) {
         int t0 = 0, t1 = 0, t2 = 0;
-        double tw = 0.0;
-        for (int w = 0; w < 8; ++w) { t0 += s_cnt[0][w]; t1 += s_cnt[1][w]; t2 += s_cnt[2][w]; tw += s_w[w]; }
-        if (t0) { atomicAdd(&stats->n_gridded, (unsigned long long)t0); atomicAdd(&stats->sum_weights, tw); }
+        double tw = 0.0, tv2 = 0.0, tw2 = 0.0;
+        for (int w = 0; w < 8; ++w) {
+            t0 += s_cnt[0][w]; t1 += s_cnt[1][w]; t2 += s_cnt[2][w];
+            tw += s_w[0][w]; tv2 += s_w[1][w]; tw2 += s_w[2][w];
+        }
+        if (t0) {
+            atomicAdd(&stats->n_gridded, (unsigned long long)t0);
+            atomicAdd(&stats->sum_weights, tw);
+            atomicAdd(&stats->sum_val2, tv2);
+            atomicAdd(&stats->sum_wt2, tw2);
+        }
         if (t1) atomicAdd(&stats->n_dropped, (unsigned long long)t1);
         if (t2) atomicAdd(&stats->n_flagged, (unsigned long long)t2);
     }
@@ -428,21 +442,29 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
 }
 
 // ------------------------------------------------------------------------------------------------- pack, K5
-// H = G + i*Gw: G and Gw are both Hermitian, so their inverse transforms are real and one complex FFT of H
-// returns the dirty image in the real part and the beam in the imaginary part.
+// H = G + i*alpha*Gw: G and Gw are both Hermitian, so their inverse transforms are real and one complex FFT of
+// H returns the dirty image in the real part and alpha * beam in the imaginary part.  alpha is the power of two
+// nearest to rms|wt*V| / rms(wt): it balances the two parts so that fp32 rounding of the (much larger) beam does
+// not leak into the dirty image; a power of two keeps the scaling exact.
 template <int WMODE>
 __global__ void __launch_bounds__(256) k_pack(const size_t ncell2, const float4* __restrict__ G,
-                                              const float* __restrict__ Gw, float4* __restrict__ H) {
+                                              const float* __restrict__ Gw, float4* __restrict__ H,
+                                              Stats* __restrict__ stats) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // two cells per thread
+    const double v2 = stats->sum_val2, w2 = stats->sum_wt2;
+    float al = 1.0f;
+    if (v2 > 0.0 && w2 > 0.0) al = exp2f(rintf(0.5f * log2f((float)(v2 / w2))));
+    al = fminf(fmaxf(al, 9.5367431640625e-07f), 1048576.0f);
+    if (i == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
     if (i >= ncell2) return;
     const float4 gv = G[i];
     float4 o;
     if (WMODE == 0) {
         const float2 w = reinterpret_cast<const float2*>(Gw)[i];
-        o = make_float4(gv.x, gv.y + w.x, gv.z, gv.w + w.y);
+        o = make_float4(gv.x, gv.y + al * w.x, gv.z, gv.w + al * w.y);
     } else {
         const float4 w = reinterpret_cast<const float4*>(Gw)[i];
-        o = make_float4(gv.x - w.y, gv.y + w.x, gv.z - w.w, gv.w + w.z);
+        o = make_float4(gv.x - al * w.y, gv.y + al * w.x, gv.z - al * w.w, gv.w + al * w.z);
     }
     H[i] = o;
 }
@@ -451,8 +473,8 @@ __global__ void __launch_bounds__(256) k_pack(const size_t ncell2, const float4*
 // dirty from the real part, beam from the imaginary part.  Four pixels per thread.
 __global__ void __launch_bounds__(256) k_correct(const int nx, const int ny, const int ngrids,
                                                  const float2* __restrict__ F, const float* __restrict__ icx,
-                                                 const float* __restrict__ icy, float* __restrict__ dirty,
-                                                 float* __restrict__ psf) {
+                                                 const float* __restrict__ icy, const Stats* __restrict__ stats,
+                                                 float* __restrict__ dirty, float* __restrict__ psf) {
     const int nx4 = nx >> 2;
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t total = (size_t)ngrids * ny * nx4;
@@ -471,7 +493,10 @@ __global__ void __launch_bounds__(256) k_correct(const int nx, const int ny, con
     const float m0 = cx.x * cy, m1 = -cx.y * cy, m2 = cx.z * cy, m3 = -cx.w * cy;
     const size_t o = (gi * ny + y) * (size_t)nx + x;
     if (dirty) *reinterpret_cast<float4*>(dirty + o) = make_float4(f01.x * m0, f01.z * m1, f23.x * m2, f23.z * m3);
-    if (psf) *reinterpret_cast<float4*>(psf + o) = make_float4(f01.y * m0, f01.w * m1, f23.y * m2, f23.w * m3);
+    if (psf) {
+        const float ia = stats->inv_alpha;                               // exact power of two
+        *reinterpret_cast<float4*>(psf + o) = make_float4(f01.y * m0 * ia, f01.w * m1 * ia, f23.y * m2 * ia, f23.w * m3 * ia);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------- launchers
@@ -518,7 +543,7 @@ cudaError_t tiled_kernel_setup(int max_smem_bytes) {
     cudaError_t e;
     if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
     if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
-    if ((e = cudaFuncSetAttribute(k_grid_tiled_s7, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_grid_tiled_s7, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
     return cudaSuccess;
 }
 
@@ -539,18 +564,18 @@ cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* i
     return cudaGetLastError();
 }
 
-cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, cudaStream_t s) {
+cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, Stats* stats, cudaStream_t s) {
     const size_t ncell2 = (size_t)g.ngrids * g.ny * g.nx / 2;
     const unsigned blocks = (unsigned)((ncell2 + 255) / 256);
-    if (g.wmode) k_pack<1><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H));
-    else k_pack<0><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H));
+    if (g.wmode) k_pack<1><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H), stats);
+    else k_pack<0><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H), stats);
     return cudaGetLastError();
 }
 
-cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, float* dirty,
-                           float* psf, cudaStream_t s) {
+cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, const Stats* stats,
+                           float* dirty, float* psf, cudaStream_t s) {
     const size_t total = (size_t)g.ngrids * g.ny * (g.nx / 4);
-    k_correct<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(g.nx, g.ny, g.ngrids, F, icx, icy, dirty, psf);
+    k_correct<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(g.nx, g.ny, g.ngrids, F, icx, icy, stats, dirty, psf);
     return cudaGetLastError();
 }
 

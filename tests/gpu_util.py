@@ -72,9 +72,18 @@ def oracle_images(G, Gw, T, S, Q):
     return Fd.real, Fd.real / corr, Fp.real, Fp.real / corr, max(np.abs(Fd.imag).max(), np.abs(Fp.imag).max())
 
 
-def inner_box(n, frac=0.75):
+# R9 gate region: the central 75% of each axis, further limited (for kernels wider than the S = 7 PSWF of the
+# configs) to where the per-axis corrector has not fallen below its S = 7 value at the 75% edge, c(0.375)/c(0) =
+# 0.0329 -- beyond that 1/(cx*cy) amplifies fp32 rounding past any fixed fraction of the peak.
+CORR_FLOOR = 0.0329
+
+
+def inner_box(n, corr=None, frac=0.75):
     c = np.arange(n) - n // 2
-    return np.abs(c) < frac * n / 2
+    box = np.abs(c) < frac * n / 2
+    if corr is not None:
+        box &= corr / corr[n // 2] >= CORR_FLOOR * (1 - 1e-6)
+    return box
 
 
 def check_images(im, G_or, Gw_or, T, S, Q, tol=IMG_TOL):
@@ -83,7 +92,7 @@ def check_images(im, G_or, Gw_or, T, S, Q, tol=IMG_TOL):
     g_raw_d, g_raw_p = gpu_images(im, correction=False)
     g_cor_d, g_cor_p = gpu_images(im, correction=True)
     ny, nx = raw_d.shape[-2:]
-    by, bx = inner_box(ny), inner_box(nx)
+    by, bx = inner_box(ny, mo.corrector(T, S, Q, ny)), inner_box(nx, mo.corrector(T, S, Q, nx))
     box = by[:, None] & bx[None, :]
     out = {}
     for name, o_raw, o_cor, g_raw, g_cor in (("dirty", raw_d, cor_d, g_raw_d, g_cor_d), ("psf", raw_p, cor_p, g_raw_p, g_cor_p)):
