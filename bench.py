@@ -29,6 +29,9 @@ if ROOT not in sys.path:
 
 CFG = 3
 FRAMES_PER_STEP = 80
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_grid_owner_s7 launch of this workload, from the committed
+# `ncu --set full` capture (profiles/); None until that capture exists
+TRAFFIC_NCU = None
 METRIC = "gridded_visibilities_per_s"
 UNIT = "vis/s"
 
@@ -172,23 +175,34 @@ def main():
 
     params, frames = make_frames(FRAMES_PER_STEP, seed0=rank * FRAMES_PER_STEP)
     n, nvis = params.n, frames[0][2].shape[0]
-    dev = [[torch.from_numpy(a).cuda() for a in fr] for fr in frames]
+    B = FRAMES_PER_STEP
+    # one batch = B frames back to back in memory, frame b -> grid b (muser_grid_batched)
+    host = [np.ascontiguousarray(np.concatenate([fr[i] for fr in frames])) for i in range(4)]
+    host.append(np.repeat(np.arange(B, dtype=np.int32), nvis))
+    dev = [torch.from_numpy(a).cuda() for a in host]
     im = binding.Imager(n, n, params.cell_arcsec, params.support, params.oversample)
-    dirty = torch.empty((n, n), device="cuda")
-    psf = torch.empty((n, n), device="cuda")
+    im.set_batch(B)
+    dirty = torch.empty((B, n, n), device="cuda")
+    psf = torch.empty((B, n, n), device="cuda")
     stream = torch.cuda.current_stream()
 
     def step():
-        for fr in dev:
-            im.reset()
-            im.grid(*fr)
-            im.dirty_psf(dirty, psf)
+        im.reset()
+        im.grid_batched(*dev)
+        im.dirty_psf(dirty, psf)
 
     def barrier():
         torch.cuda.synchronize()
         if dist:
             dist.barrier()
             torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if dist:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+        return ms
 
     for _ in range(W):
         step()
@@ -207,54 +221,63 @@ def main():
     sampler.join()
     sampler.sample()
     launches = im.get_launch_count() - l0
-    ms = e0.elapsed_time(e1)
-    if dist:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    frames_total = args.steps * FRAMES_PER_STEP * world
+    ms = max_over_ranks(e0.elapsed_time(e1))
+    frames_total = args.steps * B * world
     value = frames_total * nvis / (ms * 1e-3)
 
     # ---- per-stage device time, live, with CUDA events on the launching stream (second timed pass)
     im.set_profiling(True)
-    for _ in range(max(1, min(args.steps, 5))):
+    for _ in range(max(3, min(args.steps, 10))):
         step()
     prof = im.get_profile()
     im.set_profiling(False)
     stage_us = {k: (1e3 * v[0] / v[1] if v[1] else None) for k, v in prof.items()}
     grid_us = stage_us["grid"]
-    # algorithmic bytes of one gridding launch: 32 B per visibility (its two 16-byte samples)
-    # + every cell of G (8 B) and Gw (4 B) once
-    alg_bytes = 32.0 * nvis + 12.0 * n * n
+    # algorithmic bytes of one gridding launch: per frame 32 B per input visibility + every
+    # cell of G (8 B) and Gw (4 B) written once; one launch grids B frames
+    alg_bytes = B * (32.0 * nvis + 12.0 * n * n)
     peak, peak_src = _peaks()
     achieved = alg_bytes / (grid_us * 1e-6) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_grid_tiled_s7", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes, "kernel_us": grid_us, "stage_us": stage_us}
+    roofline = {"bound": "hbm", "kernel": "k_grid_owner_s7", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": TRAFFIC_NCU, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "kernel_us": grid_us,
+                "kernel_us_per_frame": grid_us / B, "stage_us_per_launch": stage_us,
+                "stage_us_per_frame": {k: (v / B if v else None) for k, v in stage_us.items()}}
 
-    # ---- end to end through the host-buffer entry point (pinned host memory; H2D + D2H inside the timed region)
-    pin = [[torch.from_numpy(a).pin_memory() for a in fr] for fr in frames[:16]]
-    d_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
-    p_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
-    for fr in pin[:3]:
-        im.frame_host(fr[0], fr[1], fr[2], fr[3], None, d_host, p_host)
+    # ---- latency of ONE frame through the un-batched calls (reset -> grid -> dirty_psf on one 1024^2 grid)
+    im1 = binding.Imager(n, n, params.cell_arcsec, params.support, params.oversample)
+    dev1 = [[torch.from_numpy(a).cuda() for a in fr] for fr in frames[:16]]
+    d1 = torch.empty((n, n), device="cuda")
+    p1 = torch.empty((n, n), device="cuda")
+    for fr in dev1[:4]:
+        im1.reset(); im1.grid(*fr); im1.dirty_psf(d1, p1)
     barrier()
-    e2e_frames = max(16, min(args.steps * FRAMES_PER_STEP, 400))
-    t0 = time.perf_counter()
     e0.record(stream)
-    for k in range(e2e_frames):
-        fr = pin[k % len(pin)]
-        im.frame_host(fr[0], fr[1], fr[2], fr[3], None, d_host, p_host)
+    for fr in dev1:
+        im1.reset(); im1.grid(*fr); im1.dirty_psf(d1, p1)
     e1.record(stream)
     barrier()
-    e2e_ms = e0.elapsed_time(e1)
-    if dist:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_value = e2e_frames * world * nvis / (e2e_ms * 1e-3)
-    h2d = nvis * 32 * FRAMES_PER_STEP
-    d2h = 2 * n * n * 4 * FRAMES_PER_STEP
+    single_us = 1e3 * e0.elapsed_time(e1) / len(dev1)
+    im1.destroy()
+    del dev1
+
+    # ---- end to end through the host-buffer entry point (pinned host memory; H2D + D2H inside the timed region)
+    pin = [torch.from_numpy(a).pin_memory() for a in host]
+    d_host = torch.empty((B, n, n), dtype=torch.float32).pin_memory()
+    p_host = torch.empty((B, n, n), dtype=torch.float32).pin_memory()
+    for _ in range(2):
+        im.frame_host(pin[0], pin[1], pin[2], pin[3], pin[4], d_host, p_host)
+    barrier()
+    e2e_steps = max(2, min(args.steps, 5))
+    e0.record(stream)
+    for k in range(e2e_steps):
+        im.frame_host(pin[0], pin[1], pin[2], pin[3], pin[4], d_host, p_host)
+    e1.record(stream)
+    barrier()
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1))
+    e2e_value = e2e_steps * B * world * nvis / (e2e_ms * 1e-3)
+    h2d = sum(int(a.nbytes) for a in host)
+    d2h = 2 * B * n * n * 4
 
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
@@ -279,12 +302,15 @@ def main():
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": "configs[2] MUSER-II full frame: 56,640 vis (113,280 samples) -> 1024^2 grid, PSWF S=7 Q=128 "
-                                   "-> dirty image + beam", "frames_per_step": FRAMES_PER_STEP, "nvis_per_frame": nvis,
-                       "l2_policy": "inputs rotate over 80 distinct frames (145 MB > 126 MB L2)", "launch": "stream",
-                       "parallelism": f"frames x{world}" if world > 1 else "single"},
-            "images_per_s": frames_total / (ms * 1e-3), "us_per_frame": 1e3 * ms / (args.steps * FRAMES_PER_STEP),
+                                   "-> dirty image + beam; one step = 80 distinct frames, each onto its own grid, in one "
+                                   "muser_grid_batched + muser_dirty_psf call", "frames_per_step": FRAMES_PER_STEP,
+                       "nvis_per_frame": nvis,
+                       "l2_policy": "per step 145 MB of inputs and 1.0 GB of grids stream through a 126 MB L2",
+                       "launch": "stream", "parallelism": f"frames x{world}" if world > 1 else "single"},
+            "images_per_s": frames_total / (ms * 1e-3), "dirty_and_beam_pairs_per_s": frames_total / (ms * 1e-3),
+            "us_per_frame": 1e3 * ms / (args.steps * FRAMES_PER_STEP), "single_frame_latency_us": single_us,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "frames_timed": e2e_frames, "us_per_frame": 1e3 * e2e_ms / e2e_frames},
+                    "steps_timed": e2e_steps, "us_per_frame": 1e3 * e2e_ms / (e2e_steps * B)},
             "gpu_launches": int(launches), "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu,
         }
         print(json.dumps(line))

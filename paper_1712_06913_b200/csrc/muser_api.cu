@@ -7,6 +7,7 @@
 
 #include <cufft.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -46,6 +47,16 @@ struct muser_imager {
     Item* items = nullptr;
     size_t bins_cap = 0, items_cap = 0;
     Stats* stats_d = nullptr;
+    // owner-tile path
+    float* ttp_d = nullptr;                 // padded transposed table (2-D mode, support 7), else null
+    uint32_t* order_d = nullptr;            // tiles ordered centre-out (the dense ones are scheduled first)
+    OwItem* ow_items = nullptr;
+    uint32_t* ow_tickets = nullptr;
+    float* ow_scratch = nullptr;
+    size_t ow_items_cap = 0, ow_sorted_cap = 0, ow_bins_cap = 0;
+    uint4* ow_sorted = nullptr;
+    uint32_t *ow_count = nullptr, *ow_offset = nullptr;
+    bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     cufftHandle plan = 0;
     bool plan_ok = false, fft_valid = false;
     cudaStream_t last_stream = nullptr;
@@ -104,6 +115,8 @@ void free_grids(muser_imager* h) {
 void free_bins(muser_imager* h) {
     cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
     h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
+    cudaFree(h->ow_count); cudaFree(h->ow_offset);
+    h->ow_count = h->ow_offset = nullptr; h->ow_bins_cap = 0;
 }
 
 int rebuild_geom(muser_imager* h) {
@@ -120,6 +133,8 @@ int rebuild_geom(muser_imager* h) {
     if (nb >= 0x7FFFFFFFull) return fail(h, MUSER_EUNSUPPORTED, "too many (grid, plane, tile) bins");
     g.nbins = (uint32_t)nb;
     g.chunk = 512;
+    g.S = h->planes_h.empty() ? h->S : h->planes_h[0].support;
+    g.ntiles = g.nty * g.ntx;
     return MUSER_OK;
 }
 
@@ -135,6 +150,39 @@ int alloc_grids(muser_imager* h) {
     CU(h, cudaMemset(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float))));
     CU(h, cudaMemset(h->stats_d, 0, sizeof(Stats)));
     h->fft_valid = false;
+    h->zero_pending = false;
+    return MUSER_OK;
+}
+
+// the lazily deferred part of muser_reset: zero the grids now (every consumer but the owner-tile gridder needs it)
+int flush_zero(muser_imager* h, cudaStream_t s) {
+    if (!h->zero_pending) return MUSER_OK;
+    const size_t nc = grid_cells(h);
+    CU(h, cudaMemsetAsync(h->G, 0, nc * sizeof(float2), s));
+    CU(h, cudaMemsetAsync(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), s));
+    h->zero_pending = false;
+    return MUSER_OK;
+}
+
+bool owner_capable(const muser_imager* h) { return !wmode(h) && h->ttp_d != nullptr; }
+
+// tiles of one grid ordered by distance from the uv origin: MUSER's coverage is centrally condensed, so the heavy
+// tiles get the lowest block indices of the gridding launch and start first
+int build_tile_order(muser_imager* h) {
+    const Geom& g = h->geom;
+    std::vector<std::pair<long long, uint32_t>> key((size_t)g.ntiles);
+    const int cx = (h->nx / 2 + kTile / 2) >> kTileShift, cy = (h->ny / 2 + kTile / 2) >> kTileShift;
+    for (int ty = 0; ty < g.nty; ++ty)
+        for (int tx = 0; tx < g.ntx; ++tx) {
+            const long long dx = tx - cx, dy = ty - cy;
+            key[(size_t)ty * g.ntx + tx] = {dx * dx + dy * dy, (uint32_t)(ty * g.ntx + tx)};
+        }
+    std::sort(key.begin(), key.end());
+    std::vector<uint32_t> order((size_t)g.ntiles);
+    for (size_t i = 0; i < key.size(); ++i) order[i] = key[i].second;
+    cudaFree(h->order_d); h->order_d = nullptr;
+    CU(h, cudaMalloc(&h->order_d, order.size() * sizeof(uint32_t)));
+    CU(h, cudaMemcpy(h->order_d, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     return MUSER_OK;
 }
 
@@ -166,6 +214,15 @@ int upload_tables(muser_imager* h, const std::vector<std::vector<double>>& t64, 
     CU(h, cudaMemcpy(h->tables_d, dev.data(), dev.size() * sizeof(float), cudaMemcpyHostToDevice));
     CU(h, cudaMalloc(&h->planes_d, P * sizeof(PlaneMeta)));
     CU(h, cudaMemcpy(h->planes_d, h->planes_h.data(), P * sizeof(PlaneMeta), cudaMemcpyHostToDevice));
+    // owner-tile path: padded transposed table TTp[r][0] = 0, TTp[r][1 + j] = T[j*Q + r], TTp[r][8..9] = 0
+    cudaFree(h->ttp_d); h->ttp_d = nullptr;
+    if (!wm && P == 1 && supports[0] == 7) {
+        std::vector<float> ttp((size_t)(Q + 1) * kOwTablePitch, 0.f);
+        for (int r = 0; r <= Q; ++r)
+            for (int j = 0; j < 7; ++j) ttp[(size_t)r * kOwTablePitch + 1 + j] = h->tables_f32[0][(size_t)j * Q + r];
+        CU(h, cudaMalloc(&h->ttp_d, ttp.size() * sizeof(float)));
+        CU(h, cudaMemcpy(h->ttp_d, ttp.data(), ttp.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
     // correctors from plane 0 (real part), fp64 -> reciprocal -> fp32
     std::vector<double> t0((size_t)supports[0] * Q + 1);
     for (size_t i = 0; i < t0.size(); ++i) t0[i] = wm ? t64[0][2 * i] : t64[0][i];
@@ -222,10 +279,50 @@ int ensure_scratch(muser_imager* h, long long nvis, bool tiled) {
     return MUSER_OK;
 }
 
-bool use_tiled(const muser_imager* h) {
-    if (h->strategy == MUSER_STRATEGY_TILED) return true;
-    if (h->strategy == MUSER_STRATEGY_DIRECT) return false;
-    return h->ngrids <= 4;
+int pick_strategy(const muser_imager* h) {
+    if (h->strategy != MUSER_STRATEGY_AUTO) return h->strategy;
+    if (owner_capable(h)) return MUSER_STRATEGY_OWNER;
+    return h->ngrids <= 4 ? MUSER_STRATEGY_TILED : MUSER_STRATEGY_DIRECT;
+}
+
+uint32_t owner_item_size(long long nvis) {
+    // heavy tiles are split into chunks of item_size samples; the partial-tile scratch holds at most
+    // 16*nvis/item_size + 2 tiles of 12 KB and is kept under 256 MB
+    uint32_t item = 4096;
+    while ((16.0 * (double)nvis / item + 2.0) * kOwTileFloats * sizeof(float) > 256.0 * 1048576.0) item *= 2;
+    return item;
+}
+
+int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, uint32_t* max_items_out) {
+    const size_t nrec = (size_t)8 * (size_t)nvis;                    // <= 2 samples x 4 tiles per visibility
+    if (nrec > h->ow_sorted_cap) {
+        cudaFree(h->ow_sorted); h->ow_sorted = nullptr; h->ow_sorted_cap = 0;
+        const size_t cap = nrec + nrec / 8 + 1024;
+        CU(h, cudaMalloc(&h->ow_sorted, cap * sizeof(uint4)));
+        h->ow_sorted_cap = cap;
+    }
+    const size_t nb = ((size_t)h->geom.nbins + 8) & ~(size_t)3;
+    if (nb > h->ow_bins_cap) {
+        cudaFree(h->ow_count); cudaFree(h->ow_offset);
+        h->ow_count = h->ow_offset = nullptr; h->ow_bins_cap = 0;
+        CU(h, cudaMalloc(&h->ow_count, nb * sizeof(uint32_t)));
+        CU(h, cudaMalloc(&h->ow_offset, nb * sizeof(uint32_t)));
+        CU(h, cudaMemset(h->ow_count, 0, nb * sizeof(uint32_t)));     // every later use leaves it zeroed
+        h->ow_bins_cap = nb;
+    }
+    const size_t ni = (size_t)(16.0 * (double)nvis / item_size) + 2;
+    if (ni > h->ow_items_cap) {
+        cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
+        h->ow_items = nullptr; h->ow_tickets = nullptr; h->ow_scratch = nullptr; h->ow_items_cap = 0;
+        const size_t cap = ni + ni / 4 + 16;
+        CU(h, cudaMalloc(&h->ow_items, cap * sizeof(OwItem)));
+        CU(h, cudaMalloc(&h->ow_tickets, cap * sizeof(uint32_t)));
+        CU(h, cudaMemset(h->ow_tickets, 0, cap * sizeof(uint32_t)));  // the last chunk of a tile re-zeroes its ticket
+        CU(h, cudaMalloc(&h->ow_scratch, cap * kOwTileFloats * sizeof(float)));
+        h->ow_items_cap = cap;
+    }
+    *max_items_out = (uint32_t)ni;
+    return MUSER_OK;
 }
 
 int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void* vis, const float* wt,
@@ -233,13 +330,41 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     if (nvis < 0 || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "nvis out of range [0, 2^30]");
     if (nvis == 0) return MUSER_OK;
     if (!uvw || !freq || !vis || !wt) return fail(h, MUSER_EINVAL, "null input pointer");
-    const bool tiled = use_tiled(h);
-    int rc = ensure_scratch(h, nvis, tiled);
-    if (rc) return rc;
-    h->last_stream = s;
-    h->fft_valid = false;
+    const int strat = pick_strategy(h);
     const Geom& g = h->geom;
     GridPtrs gp{h->G, h->Gw};
+    if (strat == MUSER_STRATEGY_OWNER) {
+        if (!owner_capable(h)) return fail(h, MUSER_EUNSUPPORTED, "the owner-tile strategy needs 2-D mode and support 7");
+        const uint32_t item_size = owner_item_size(nvis);
+        uint32_t max_items = 0;
+        int rc = ensure_owner_scratch(h, nvis, item_size, &max_items);
+        if (rc) return rc;
+        if ((unsigned long long)max_items + g.nbins >= 0x7FFFFFFFull) return fail(h, MUSER_EUNSUPPORTED, "too many tiles for one launch");
+        h->last_stream = s;
+        h->fft_valid = false;
+        {
+            StageScope sc(h, MUSER_STAGE_BIN, s);
+            CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, s));
+            CU(h, launch_owner_scan(g, h->ow_count, h->ow_offset, h->ow_items, h->nitems_d, item_size, s));
+            CU(h, launch_owner_scatter(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_count,
+                                       h->ow_sorted, s));
+        }
+        {
+            StageScope sc(h, MUSER_STAGE_GRID, s);
+            CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_count, h->ow_items, h->nitems_d, max_items,
+                                    item_size, h->order_d, h->ttp_d, gp, h->ow_scratch, h->ow_tickets,
+                                    h->zero_pending ? 1 : 0, s));
+        }
+        h->zero_pending = false;                                      // store mode wrote every tile of every grid
+        h->n_launches += 4;
+        return MUSER_OK;
+    }
+    const bool tiled = strat == MUSER_STRATEGY_TILED;
+    int rc = ensure_scratch(h, nvis, tiled);
+    if (rc) return rc;
+    if ((rc = flush_zero(h, s))) return rc;
+    h->last_stream = s;
+    h->fft_valid = false;
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
         CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
@@ -265,6 +390,8 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
 int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     if (!dirty && !psf) return MUSER_OK;
     h->last_stream = s;
+    int rcz = flush_zero(h, s);
+    if (rcz) return rcz;
     if (!h->plan_ok) {
         int dims[2] = {h->ny, h->nx};
         cufftResult r = cufftPlanMany(&h->plan, 2, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, h->ngrids);
@@ -296,11 +423,15 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
 }
 
 int reset_impl(muser_imager* h, cudaStream_t s) {
-    const size_t nc = grid_cells(h);
     h->last_stream = s;
     h->fft_valid = false;
-    CU(h, cudaMemsetAsync(h->G, 0, nc * sizeof(float2), s));
-    CU(h, cudaMemsetAsync(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), s));
+    // The grids are zeroed lazily: the owner-tile gridder writes every tile of every grid with plain stores, so a
+    // reset followed by muser_grid needs no memset at all; any other consumer calls flush_zero first.
+    h->zero_pending = true;
+    if (!(owner_capable(h) && pick_strategy(h) == MUSER_STRATEGY_OWNER)) {
+        int rc = flush_zero(h, s);
+        if (rc) return rc;
+    }
     CU(h, cudaMemsetAsync(h->stats_d, 0, sizeof(Stats), s));
     return MUSER_OK;
 }
@@ -345,6 +476,8 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
         h->err = "cudaMalloc failed"; return bail("alloc");
     }
     if (build_2d_tables(h)) return bail("tables");
+    if (rebuild_geom(h)) return bail("geometry");
+    if (build_tile_order(h)) return bail("tile order");
     if (alloc_grids(h)) return bail("grids");
     return h;
 }
@@ -357,6 +490,8 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->staged); cudaFree(h->sorted); cudaFree(h->stats_d); cudaFree(h->nitems_d);
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
+    cudaFree(h->ttp_d); cudaFree(h->order_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
+    cudaFree(h->ow_sorted);
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete h;
@@ -438,7 +573,11 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
 
 int muser_set_strategy(muser_imager* h, int strategy) {
     if (!h) return MUSER_EINVAL;
-    if (strategy < MUSER_STRATEGY_AUTO || strategy > MUSER_STRATEGY_TILED) return fail(h, MUSER_EINVAL, "unknown strategy");
+    if (strategy < MUSER_STRATEGY_AUTO || strategy > MUSER_STRATEGY_OWNER) return fail(h, MUSER_EINVAL, "unknown strategy");
+    if (h->zero_pending) {                                            // do not carry a deferred reset across strategies
+        int rc = flush_zero(h, h->last_stream);
+        if (rc) return rc;
+    }
     h->strategy = strategy;
     return MUSER_OK;
 }
@@ -529,6 +668,8 @@ int muser_get_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_
     cudaStream_t s = (cudaStream_t)sv;
     const size_t nc = grid_cells(h);
     h->last_stream = s;
+    int rcz = flush_zero(h, s);
+    if (rcz) return rcz;
     if (grid_c64_out) CU(h, cudaMemcpyAsync(grid_c64_out, h->G, nc * sizeof(float2), cudaMemcpyDeviceToDevice, s));
     if (wgrid_out) CU(h, cudaMemcpyAsync(wgrid_out, h->Gw, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), cudaMemcpyDeviceToDevice, s));
     return MUSER_OK;

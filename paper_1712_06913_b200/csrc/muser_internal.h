@@ -18,6 +18,8 @@ struct Geom {
     int ntx, nty;                  // tiles per axis; tile tx covers cells [tx*32-16, tx*32+16) so DC sits mid-tile
     uint32_t nbins;                // ngrids*max(nplanes,1)*nty*ntx
     int chunk;                     // samples per work item of the tiled gridder
+    int S;                         // support of plane 0 (the 2-D kernel)
+    int ntiles;                    // nty*ntx
 };
 
 // Per-plane kernel metadata in constant-ish device memory.
@@ -78,5 +80,26 @@ cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, Stats* stats, 
 cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, const Stats* stats,
                            float* dirty, float* psf, cudaStream_t s);
 cudaError_t tiled_kernel_setup(int max_smem_bytes);
+
+// ---- owner-tile path (muser_owner.cu): 2-D mode, support 7.  Every 32x32 tile of every grid has exactly one
+// writer, so the grids are written with plain stores (no memset, no global atomics); samples whose footprint
+// crosses a tile edge are listed in every tile they touch.
+constexpr int kOwSub = 1024;                 // samples staged and cell-sorted in shared memory per pass
+constexpr int kOwTileFloats = 32 * 32 * 3;   // one partial tile in the scratch buffer: A[32][32] float2 + B[32][32] float
+constexpr int kOwTablePitch = 10;            // padded transposed table: TTp[rx][0] = 0, [1..7] = T[j*Q+rx], [8..9] = 0
+struct OwItem {                              // one chunk of a heavy tile (more than item_size samples)
+    uint32_t bin, start, count, first_slot, nchunks, chunk;
+};
+cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                               const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, cudaStream_t s);
+cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
+                              uint32_t item_size, cudaStream_t s);
+cudaError_t launch_owner_scatter(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                                 const int* grid_id, long long nvis, const uint32_t* bin_offset, uint32_t* cursor,
+                                 uint4* sorted, cudaStream_t s);
+cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
+                              const OwItem* items, const uint32_t* nitems, uint32_t max_items, uint32_t item_size,
+                              const uint32_t* order, const float* ttp, GridPtrs grids, float* scratch,
+                              uint32_t* tickets, int store_mode, cudaStream_t s);
 
 }  // namespace muser

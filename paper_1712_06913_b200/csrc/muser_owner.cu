@@ -1,0 +1,545 @@
+// Owner-tile gridding path (2-D mode, support 7), sm_100a.
+//
+//   O1 k_owner_count    A1: fp64 coordinates (O1 order), keep/drop, statistics, histogram of the tiles
+//                           each sample's 7x7 footprint touches (1, 2 or 4 tiles; warp-aggregated atomics)
+//   O2 k_owner_scan     A1: exclusive scan of the histogram; tiles with more than item_size samples are split
+//                           into chunk items
+//   O3 k_owner_scatter  A1: recomputes the coordinates and writes one 16-byte record per (sample, touched tile)
+//   O4 k_grid_owner_s7  A2/A4: one CTA per 32x32 tile of one grid.  It stages <= 1024 records at a time in shared
+//                           memory, counting-sorts them by (row, 8-cell column window), and every warp walks an
+//                           equal slice of the sorted list with the 7 x 8 window held in registers (lane = row r,
+//                           column pair c; packed FFMA2), touching shared memory only when the window changes.
+//                           The tile is then written to G and Gw with plain coalesced stores: the grids need no
+//                           memset and receive no global atomics.  Chunks of a heavy tile write partial tiles to a
+//                           scratch buffer; the last chunk to finish adds them up in chunk order.
+// Passages: PAPER.md:78 (gridding = convolution onto a regular grid), :136-138 (spheroidal GCF), :216-228 (float2
+// grid, row-major, Hermitian), :249-256 (DIRTY_IMAGE).  The binning and tiling are this build's design.
+#include "muser_internal.h"
+
+namespace muser {
+
+static constexpr double kC = 299792458.0;   // m/s
+static constexpr unsigned kFull = 0xffffffffu;
+
+// ------------------------------------------------------------------------------------------------- coordinates
+// O1 for one axis (same operation order as the oracle; _rn intrinsics forbid FMA contraction).
+__device__ __forceinline__ void ow_cell_phase(double c_lambda, double scale, int n, int Q, double& i0, double& r) {
+    const double p = __dadd_rn(__dmul_rn(c_lambda, scale), (double)(n / 2));
+    i0 = floor(__dadd_rn(p, 0.5));
+    const double fr = __dsub_rn(p, i0);
+    r = floor(__dadd_rn(__dmul_rn(fr, (double)Q), 0.5));
+}
+
+struct OwLoc {
+    int state;                 // 0 none (k >= nvis), 1 flagged, 2 dropped, 3 kept
+    float re, im, wt;          // wt*Re V, wt*Im V (primary sample; the conjugate negates im), wt
+    int cu[2], cv[2], rx[2], ry[2];
+    int gid;
+};
+
+__device__ __forceinline__ void ow_locate(const Geom& g, const float* __restrict__ uvw, const double* __restrict__ freq,
+                                          const float2* __restrict__ vis, const float* __restrict__ weight,
+                                          const int* __restrict__ grid_id, long long k, long long nvis, OwLoc& L,
+                                          float2& Vraw) {
+    L.state = 0;
+    if (k >= nvis) return;
+    const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
+    const double f = freq[k];
+    const float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
+    const float wt = weight[k];
+    const int gid = grid_id ? grid_id[k] : 0;
+    Vraw = V;
+    const double il = __ddiv_rn(f, kC);
+    const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
+    const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) && isfinite(V.y) &&
+                    isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
+    if (!ok) { L.state = 1; return; }
+    const int h = (g.S - 1) >> 1;
+    bool inside = true;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const double sgn = s ? -1.0 : 1.0;
+        double iu, iv, ru, rv;
+        ow_cell_phase(sgn * ul, g.su, g.nx, g.Q, iu, ru);
+        ow_cell_phase(sgn * vl, g.sv, g.ny, g.Q, iv, rv);
+        inside = inside && iu >= (double)(h + 1) && iu <= (double)(g.nx - 1 - h) && iv >= (double)(h + 1) &&
+                 iv <= (double)(g.ny - 1 - h);
+        L.cu[s] = (int)iu; L.cv[s] = (int)iv;
+        L.rx[s] = g.Q / 2 - (int)ru; L.ry[s] = g.Q / 2 - (int)rv;
+    }
+    if (!inside) { L.state = 2; return; }
+    L.state = 3;
+    L.re = wt * V.x; L.im = wt * V.y; L.wt = wt; L.gid = gid;
+}
+
+// Bin of the q-th tile (q = qx | qy << 1) touched by the footprint of a sample at nearest cell (cu, cv), or kNoBin.
+__device__ __forceinline__ uint32_t ow_bin(const Geom& g, int gid, int cu, int cv, int q, int& tx, int& ty) {
+    const int h = (g.S - 1) >> 1;
+    const int tx0 = (cu - h + kTile / 2) >> kTileShift, tx1 = (cu + h + kTile / 2) >> kTileShift;
+    const int ty0 = (cv - h + kTile / 2) >> kTileShift, ty1 = (cv + h + kTile / 2) >> kTileShift;
+    if (((q & 1) && tx1 == tx0) || ((q & 2) && ty1 == ty0)) return kNoBin;
+    tx = (q & 1) ? tx1 : tx0;
+    ty = (q & 2) ? ty1 : ty0;
+    return (uint32_t)gid * (uint32_t)g.ntiles + (uint32_t)(ty * g.ntx + tx);
+}
+
+// Warp-aggregated counter increment: lanes with the same bin issue one atomicAdd; returns the lane's rank.
+// Every lane of the warp must call it (bin == kNoBin: no increment).
+__device__ __forceinline__ uint32_t ow_agg_inc(uint32_t* __restrict__ cnt, uint32_t bin, int lane) {
+    const unsigned m = __match_any_sync(kFull, bin);
+    const int leader = __ffs(m) - 1;
+    uint32_t base = 0;
+    if (bin != kNoBin && lane == leader) base = atomicAdd(&cnt[bin], (uint32_t)__popc(m));
+    base = __shfl_sync(kFull, base, leader);
+    return base + (uint32_t)__popc(m & ((1u << lane) - 1u));
+}
+
+// ------------------------------------------------------------------------------------------------- O1 count
+__global__ void __launch_bounds__(256) k_owner_count(const Geom g, const float* __restrict__ uvw,
+                                                     const double* __restrict__ freq, const float2* __restrict__ vis,
+                                                     const float* __restrict__ weight, const int* __restrict__ grid_id,
+                                                     const long long nvis, uint32_t* __restrict__ bin_count,
+                                                     Stats* __restrict__ stats) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    OwLoc L;
+    float2 V;
+    ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V);
+    const int kept = L.state == 3, dropped = L.state == 2, flagged = L.state == 1;
+    double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
+    if (kept) {
+        wsum = 2.0 * (double)L.wt;
+        w2sum = (double)L.wt * (double)L.wt;
+        v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
+    }
+    if (__any_sync(kFull, kept)) {
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                int tx, ty;
+                const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
+                if (__any_sync(kFull, bin != kNoBin)) ow_agg_inc(bin_count, bin, lane);
+            }
+        }
+    }
+    // block reduction of the counters, one atomic set per block
+    __shared__ int s_cnt[3][8];
+    __shared__ double s_w[3][8];
+    const int c0 = __reduce_add_sync(kFull, kept), c1 = __reduce_add_sync(kFull, dropped), c2 = __reduce_add_sync(kFull, flagged);
+    for (int o = 16; o > 0; o >>= 1) {
+        wsum += __shfl_xor_sync(kFull, wsum, o);
+        v2sum += __shfl_xor_sync(kFull, v2sum, o);
+        w2sum += __shfl_xor_sync(kFull, w2sum, o);
+    }
+    if (lane == 0) { s_cnt[0][warp] = c0; s_cnt[1][warp] = c1; s_cnt[2][warp] = c2; s_w[0][warp] = wsum; s_w[1][warp] = v2sum; s_w[2][warp] = w2sum; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t0 = 0, t1 = 0, t2 = 0;
+        double tw = 0.0, tv2 = 0.0, tw2 = 0.0;
+        for (int w = 0; w < 8; ++w) {
+            t0 += s_cnt[0][w]; t1 += s_cnt[1][w]; t2 += s_cnt[2][w];
+            tw += s_w[0][w]; tv2 += s_w[1][w]; tw2 += s_w[2][w];
+        }
+        if (t0) {
+            atomicAdd(&stats->n_gridded, (unsigned long long)t0);
+            atomicAdd(&stats->sum_weights, tw);
+            atomicAdd(&stats->sum_val2, tv2);
+            atomicAdd(&stats->sum_wt2, tw2);
+        }
+        if (t1) atomicAdd(&stats->n_dropped, (unsigned long long)t1);
+        if (t2) atomicAdd(&stats->n_flagged, (unsigned long long)t2);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- O2 scan
+// One CTA walks the histogram 4096 bins at a time (4 per thread): exclusive sample offsets, chunk items of the
+// heavy bins, and re-zeroes the histogram (k_owner_scatter reuses it as its cursor).
+__global__ void __launch_bounds__(1024) k_owner_scan(const Geom g, uint32_t* __restrict__ bin_count,
+                                                     uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
+                                                     uint32_t* __restrict__ nitems, const uint32_t item_size) {
+    __shared__ uint32_t s_wsum[2][32];
+    __shared__ uint32_t s_carry[2];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) { s_carry[0] = 0; s_carry[1] = 0; }
+    __syncthreads();
+    for (uint32_t base = 0; base < g.nbins; base += 4096) {
+        const uint32_t b0 = base + 4 * threadIdx.x;
+        uint32_t c[4] = {0, 0, 0, 0}, m[4];
+        if (b0 < g.nbins) {                                            // bin_count is padded to a multiple of 4
+            const uint4 v = *reinterpret_cast<const uint4*>(bin_count + b0);
+            c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
+            if (v.x | v.y | v.z | v.w) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);
+        }
+        uint32_t tc = 0, tm = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            m[j] = c[j] > item_size ? (c[j] + item_size - 1) / item_size : 0u;
+            tc += c[j]; tm += m[j];
+        }
+        uint32_t ic = tc, im = tm;                                      // inclusive warp scans
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t xc = __shfl_up_sync(kFull, ic, o), xm = __shfl_up_sync(kFull, im, o);
+            if (lane >= o) { ic += xc; im += xm; }
+        }
+        if (lane == 31) { s_wsum[0][warp] = ic; s_wsum[1][warp] = im; }
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t wc = s_wsum[0][lane], wm = s_wsum[1][lane];
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t xc = __shfl_up_sync(kFull, wc, o), xm = __shfl_up_sync(kFull, wm, o);
+                if (lane >= o) { wc += xc; wm += xm; }
+            }
+            s_wsum[0][lane] = wc; s_wsum[1][lane] = wm;
+        }
+        __syncthreads();
+        uint32_t off = s_carry[0] + (warp ? s_wsum[0][warp - 1] : 0) + ic - tc;
+        uint32_t slot = s_carry[1] + (warp ? s_wsum[1][warp - 1] : 0) + im - tm;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t b = b0 + j;
+            if (b < g.nbins) {
+                bin_offset[b] = off;
+                for (uint32_t q = 0; q < m[j]; ++q) {
+                    OwItem it;
+                    it.bin = b; it.start = off + q * item_size; it.count = min(item_size, c[j] - q * item_size);
+                    it.first_slot = slot; it.nchunks = m[j]; it.chunk = q;
+                    items[slot + q] = it;
+                }
+            }
+            off += c[j]; slot += m[j];
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) { s_carry[0] = off; s_carry[1] = slot; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { bin_offset[g.nbins] = s_carry[0]; *nitems = s_carry[1]; }
+}
+
+// ------------------------------------------------------------------------------------------------- O3 scatter
+// Record: {wt*Re, +-wt*Im, wt, ox | oy << 6 | rx << 12 | ry << 21}; (ox, oy) = first footprint cell relative to the
+// tile origin, plus 6, in [0, 38); rx = Q/2 - ru, ry = Q/2 - rv in [0, Q].
+__global__ void __launch_bounds__(256) k_owner_scatter(const Geom g, const float* __restrict__ uvw,
+                                                       const double* __restrict__ freq, const float2* __restrict__ vis,
+                                                       const float* __restrict__ weight, const int* __restrict__ grid_id,
+                                                       const long long nvis, const uint32_t* __restrict__ bin_offset,
+                                                       uint32_t* __restrict__ cursor, uint4* __restrict__ sorted) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    OwLoc L;
+    float2 V;
+    ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V);
+    const int kept = L.state == 3;
+    if (!__any_sync(kFull, kept)) return;
+    const int h = (g.S - 1) >> 1;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            int tx = 0, ty = 0;
+            const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
+            if (!__any_sync(kFull, bin != kNoBin)) continue;
+            const uint32_t rank = ow_agg_inc(cursor, bin, lane);
+            if (bin != kNoBin) {
+                const int ox = L.cu[s] - h - (tx * kTile - kTile / 2) + 2 * h;
+                const int oy = L.cv[s] - h - (ty * kTile - kTile / 2) + 2 * h;
+                uint4 o;
+                o.x = __float_as_uint(L.re);
+                o.y = __float_as_uint(s ? -L.im : L.im);
+                o.z = __float_as_uint(L.wt);
+                o.w = (uint32_t)ox | ((uint32_t)oy << 6) | ((uint32_t)L.rx[s] << 12) | ((uint32_t)L.ry[s] << 21);
+                sorted[bin_offset[bin] + rank] = o;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- O4 gridding
+__device__ __forceinline__ unsigned long long ow_pack(float x, float y) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
+    return r;
+}
+__device__ __forceinline__ float2 ow_unpack(unsigned long long v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ unsigned long long ow_fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+// 64-bit shared-memory add of two packed floats (compare-and-swap loop; fp32 has no native shared add).
+__device__ __forceinline__ void ow_sadd2(void* p, unsigned long long v) {
+    unsigned long long* a = reinterpret_cast<unsigned long long*>(p);
+    const float2 f = ow_unpack(v);
+    unsigned long long old = *a, assumed;
+    do {
+        assumed = old;
+        const float2 c = ow_unpack(assumed);
+        old = atomicCAS(a, assumed, ow_pack(c.x + f.x, c.y + f.y));
+    } while (old != assumed);
+}
+
+constexpr int kOwAPitch = 40;     // float2 per row of the (re, im) tile: 32 cells + 8 pad
+constexpr int kOwBPitch = 40;     // floats per row of the weight tile
+constexpr int kOwKeys = 768;      // 38 rows x 19 windows = 722 sort keys, padded to 3 per thread
+constexpr int kOwDirect = 24;     // tiles with at most this many samples skip the shared-memory sort
+
+struct OwWarpAcc {
+    unsigned long long a0, a1, b;  // (re, im) of the lane's two cells; (wt, wt') of the two cells
+    int key;                       // (oy << 5 | ox >> 1) of the window held in registers, -1: none
+    int row, col0, valid;
+};
+
+__device__ __forceinline__ void ow_flush(OwWarpAcc& A, float2* sA, float* sB) {
+    if (A.key >= 0 && A.valid) {
+        ow_sadd2(&sA[A.row * kOwAPitch + A.col0], A.a0);
+        ow_sadd2(&sA[A.row * kOwAPitch + A.col0 + 1], A.a1);
+        ow_sadd2(&sB[A.row * kOwBPitch + A.col0], A.b);
+    }
+    A.a0 = A.a1 = A.b = 0ull;
+}
+
+__device__ __forceinline__ void ow_accumulate(OwWarpAcc& A, const uint4 rec, const float* __restrict__ ttp, const int r,
+                                              const int c, float2* sA, float* sB) {
+    const uint32_t pk = rec.w;
+    const int key = (int)((pk & 0xFFFu) >> 1);
+    if (key != A.key) {                                              // warp-uniform branch
+        ow_flush(A, sA, sB);
+        A.key = key;
+        const int ox = (int)(pk & 63u), oy = (int)((pk >> 6) & 63u);
+        A.row = oy - 6 + r;
+        A.col0 = (ox & ~1) - 6 + 2 * c;
+        A.valid = (r < 7) && ((unsigned)A.row < 32u) && ((unsigned)A.col0 < 32u);
+    }
+    const int par = (int)(pk & 1u);
+    const int rx = (int)((pk >> 12) & 511u), ry = (int)((pk >> 21) & 511u);
+    const float* tx = ttp + rx * kOwTablePitch + (2 * c + 1 - par);
+    const float kx0 = __ldg(tx), kx1 = __ldg(tx + 1);
+    const float ky = __ldg(ttp + ry * kOwTablePitch + r + 1);
+    const float k0 = kx0 * ky, k1 = kx1 * ky;
+    const unsigned long long v = ow_pack(__uint_as_float(rec.x), __uint_as_float(rec.y));
+    const float wt = __uint_as_float(rec.z);
+    A.a0 = ow_fma2(ow_pack(k0, k0), v, A.a0);
+    A.a1 = ow_fma2(ow_pack(k1, k1), v, A.a1);
+    A.b = ow_fma2(ow_pack(k0, k1), ow_pack(wt, wt), A.b);
+}
+
+template <int STORE>
+__global__ void __launch_bounds__(256) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
+                                                       const uint32_t* __restrict__ bin_offset,
+                                                       uint32_t* __restrict__ cursor, const OwItem* __restrict__ items,
+                                                       const uint32_t* __restrict__ nitems, const uint32_t max_items,
+                                                       const uint32_t item_size, const uint32_t* __restrict__ order,
+                                                       const float* __restrict__ ttp, GridPtrs grids,
+                                                       float* __restrict__ scratch, uint32_t* __restrict__ tickets) {
+    __shared__ __align__(16) float2 sA[32 * kOwAPitch];
+    __shared__ __align__(16) float sB[32 * kOwBPitch];
+    __shared__ __align__(16) uint4 sR[kOwSub];
+    __shared__ uint32_t sH[kOwKeys];
+    __shared__ uint32_t sW[8];
+    __shared__ int sLast;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t bin, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
+    const bool heavy = blockIdx.x < max_items;
+    if (heavy) {
+        if (blockIdx.x >= *nitems) return;
+        const OwItem it = items[blockIdx.x];
+        bin = it.bin; start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
+        if (chunk == 0 && tid == 0) cursor[bin] = 0;
+    } else {
+        const uint32_t t = blockIdx.x - max_items;
+        const uint32_t r = t / (uint32_t)g.ngrids, gi = t - r * (uint32_t)g.ngrids;
+        bin = gi * (uint32_t)g.ntiles + order[r];
+        start = bin_offset[bin];
+        cnt = bin_offset[bin + 1] - start;
+        if (cnt > item_size) return;                                  // heavy tile: its chunk items do the work
+        if (cnt && tid == 0) cursor[bin] = 0;
+    }
+    const uint32_t tile = bin % (uint32_t)g.ntiles, gi = bin / (uint32_t)g.ntiles;
+    const int ty = (int)(tile / (uint32_t)g.ntx), tx = (int)(tile % (uint32_t)g.ntx);
+    const int x0 = tx * kTile - kTile / 2, y0 = ty * kTile - kTile / 2;
+    float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
+    float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
+
+    if (cnt == 0) {
+        if (STORE) {
+            for (int i = tid; i < 32 * 16; i += 256) {
+                const int row = i >> 4, gx = x0 + 2 * (i & 15), gy = y0 + row;
+                if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny)
+                    *reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx) = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            {
+                const int row = tid >> 3, gx = x0 + 4 * (tid & 7), gy = y0 + row;
+                if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny)
+                    *reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx) = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
+        return;
+    }
+
+    {   // zero the tile accumulators
+        float4* za = reinterpret_cast<float4*>(sA);
+        for (int i = tid; i < 32 * kOwAPitch / 2; i += 256) za[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4* zb = reinterpret_cast<float4*>(sB);
+        for (int i = tid; i < 32 * kOwBPitch / 4; i += 256) zb[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    const int r = lane >> 2, c = lane & 3;
+    OwWarpAcc A;
+    A.a0 = A.a1 = A.b = 0ull; A.key = -1; A.row = A.col0 = A.valid = 0;
+
+    if (cnt <= (uint32_t)kOwDirect) {
+        __syncthreads();
+        for (uint32_t i = warp; i < cnt; i += 8) ow_accumulate(A, __ldg(sorted + start + i), ttp, r, c, sA, sB);
+        ow_flush(A, sA, sB);
+        __syncthreads();
+    } else {
+        for (uint32_t base = 0; base < cnt; base += kOwSub) {
+            const uint32_t n = min((uint32_t)kOwSub, cnt - base);
+            for (int i = tid; i < kOwKeys; i += 256) sH[i] = 0;
+            __syncthreads();
+            // (1) counting sort by (row, window)
+            uint4 rec[kOwSub / 256];
+            uint32_t rk[kOwSub / 256];
+#pragma unroll
+            for (int j = 0; j < kOwSub / 256; ++j) {
+                const uint32_t i = tid + j * 256;
+                if (i < n) {
+                    rec[j] = __ldg(sorted + start + base + i);
+                    const uint32_t key = ((rec[j].w >> 6) & 63u) * 19u + ((rec[j].w & 63u) >> 1);
+                    rk[j] = atomicAdd(&sH[key], 1u);
+                }
+            }
+            __syncthreads();
+            {
+                const uint32_t h0 = sH[3 * tid], h1 = sH[3 * tid + 1], h2 = sH[3 * tid + 2];
+                const uint32_t tot = h0 + h1 + h2;
+                uint32_t inc = tot;
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t t = __shfl_up_sync(kFull, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                if (lane == 31) sW[warp] = inc;
+                __syncthreads();
+                uint32_t ex = inc - tot;
+                for (int w = 0; w < warp; ++w) ex += sW[w];
+                sH[3 * tid] = ex; sH[3 * tid + 1] = ex + h0; sH[3 * tid + 2] = ex + h0 + h1;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < kOwSub / 256; ++j) {
+                const uint32_t i = tid + j * 256;
+                if (i < n) {
+                    const uint32_t key = ((rec[j].w >> 6) & 63u) * 19u + ((rec[j].w & 63u) >> 1);
+                    sR[sH[key] + rk[j]] = rec[j];
+                }
+            }
+            __syncthreads();
+            // (2) register accumulation over runs of equal window
+            {
+                const int per = ((int)n + 7) >> 3;
+                const int b = warp * per, e = min((int)n, b + per);
+                for (int i = b; i < e; ++i) ow_accumulate(A, sR[i], ttp, r, c, sA, sB);
+                ow_flush(A, sA, sB);
+                A.key = -1;
+            }
+            __syncthreads();
+        }
+    }
+
+    // (3) output
+    if (!heavy) {
+        for (int i = tid; i < 32 * 16; i += 256) {
+            const int row = i >> 4, c2 = i & 15, gx = x0 + 2 * c2, gy = y0 + row;
+            if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+                float4 v = *reinterpret_cast<const float4*>(&sA[row * kOwAPitch + 2 * c2]);
+                float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
+                if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+                *dst = v;
+            }
+        }
+        {
+            const int row = tid >> 3, c4 = tid & 7, gx = x0 + 4 * c4, gy = y0 + row;
+            if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+                float4 v = *reinterpret_cast<const float4*>(&sB[row * kOwBPitch + 4 * c4]);
+                float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
+                if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+                *dst = v;
+            }
+        }
+        return;
+    }
+    // heavy tile: publish this chunk's partial tile; the last chunk to arrive adds them up in chunk order
+    {
+        float4* part = reinterpret_cast<float4*>(scratch + (size_t)(first_slot + chunk) * kOwTileFloats);
+        for (int i = tid; i < 32 * 16; i += 256)
+            __stcg(part + i, *reinterpret_cast<const float4*>(&sA[(i >> 4) * kOwAPitch + 2 * (i & 15)]));
+        __stcg(part + 512 + tid, *reinterpret_cast<const float4*>(&sB[(tid >> 3) * kOwBPitch + 4 * (tid & 7)]));
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const uint32_t t = atomicAdd(&tickets[first_slot], 1u);
+        sLast = (t == nchunks - 1u);
+    }
+    __syncthreads();
+    if (!sLast) return;
+    __threadfence();
+    const float4* parts = reinterpret_cast<const float4*>(scratch + (size_t)first_slot * kOwTileFloats);
+    for (int i = tid; i < 32 * 16 + 256; i += 256) {
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (uint32_t q = 0; q < nchunks; ++q) {
+            const float4 p = __ldcg(parts + (size_t)q * (kOwTileFloats / 4) + i);
+            v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
+        }
+        float4* dst;
+        int gx, gy;
+        if (i < 512) { gx = x0 + 2 * (i & 15); gy = y0 + (i >> 4); dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx); }
+        else { const int j = i - 512; gx = x0 + 4 * (j & 7); gy = y0 + (j >> 3); dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx); }
+        if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+            if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+            *dst = v;
+        }
+    }
+    if (tid == 0) tickets[first_slot] = 0;
+}
+
+// ------------------------------------------------------------------------------------------------- launchers
+cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                               const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, cudaStream_t s) {
+    k_owner_count<<<(unsigned)((nvis + 255) / 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
+                              uint32_t item_size, cudaStream_t s) {
+    k_owner_scan<<<1, 1024, 0, s>>>(g, bin_count, bin_offset, items, nitems, item_size);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_owner_scatter(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                                 const int* grid_id, long long nvis, const uint32_t* bin_offset, uint32_t* cursor,
+                                 uint4* sorted, cudaStream_t s) {
+    k_owner_scatter<<<(unsigned)((nvis + 255) / 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_offset,
+                                                                  cursor, sorted);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
+                              const OwItem* items, const uint32_t* nitems, uint32_t max_items, uint32_t item_size,
+                              const uint32_t* order, const float* ttp, GridPtrs grids, float* scratch,
+                              uint32_t* tickets, int store_mode, cudaStream_t s) {
+    const unsigned blocks = max_items + g.nbins;
+    if (store_mode)
+        k_grid_owner_s7<1><<<blocks, 256, 0, s>>>(g, sorted, bin_offset, cursor, items, nitems, max_items, item_size,
+                                                  order, ttp, grids, scratch, tickets);
+    else
+        k_grid_owner_s7<0><<<blocks, 256, 0, s>>>(g, sorted, bin_offset, cursor, items, nitems, max_items, item_size,
+                                                  order, ttp, grids, scratch, tickets);
+    return cudaGetLastError();
+}
+
+}  // namespace muser

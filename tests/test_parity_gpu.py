@@ -12,10 +12,10 @@ import gpu_util as gu
 
 pytestmark = pytest.mark.gpu
 
-DIRECT, TILED = binding.MUSER_STRATEGY_DIRECT, binding.MUSER_STRATEGY_TILED
+DIRECT, TILED, OWNER = binding.MUSER_STRATEGY_DIRECT, binding.MUSER_STRATEGY_TILED, binding.MUSER_STRATEGY_OWNER
 
 
-@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [OWNER, TILED, DIRECT])
 @pytest.mark.parametrize("cfg", [1, 2, 3])
 def test_single_grid_configs_match_oracle(cfg, strategy):
     fr = synth.make_frame(cfg)
@@ -37,7 +37,7 @@ def test_random_visibilities_any_support(S, Q, nvis, strategy):
     gu.run_case(uvw, freq, vis, wt, n, cell, S, Q, strategy=strategy)
 
 
-@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [OWNER, TILED, DIRECT])
 def test_accumulation_over_calls_equals_one_call(strategy):
     fr = synth.make_frame(2)
     p = fr.params
@@ -45,7 +45,7 @@ def test_accumulation_over_calls_equals_one_call(strategy):
                 strategy=strategy, splits=5, images=False)
 
 
-@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [OWNER, TILED, DIRECT])
 def test_flagged_and_off_grid_visibilities_are_skipped_and_counted(strategy):
     n, cell = 256, 20.0
     uvw, freq, vis, wt = synth.random_visibilities(3, 4000, n, cell, margin_cells=0.0)   # some fall off the grid
@@ -63,6 +63,85 @@ def test_flagged_and_off_grid_visibilities_are_skipped_and_counted(strategy):
     res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, 32, strategy=strategy)
     assert res["stats"]["n_flagged"] == 370
     assert res["stats"]["n_dropped"] >= 30
+
+
+@pytest.mark.parametrize("Q,nvis,n,ny", [(128, 1, 128, None), (16, 31, 128, None), (128, 5000, 128, None), (2, 3000, 64, None),
+                                          (256, 20000, 256, None), (64, 4000, 96, 160)])
+def test_owner_strategy_random_visibilities(Q, nvis, n, ny):
+    """Owner-tile gridder (support 7): ragged tile edges (n = 96, 160 are not multiples of 32), one sample, the
+    largest oversampling, non-square grids."""
+    cell = 40.0
+    uvw, freq, vis, wt = synth.random_visibilities(11 + Q, nvis, n if ny is None else min(n, ny), cell, margin_cells=5.5)
+    if ny is None:
+        gu.run_case(uvw, freq, vis, wt, n, cell, 7, Q, strategy=OWNER)
+    else:
+        im = gu.make_imager(n, cell, 7, Q, strategy=OWNER, ny=ny)
+        try:
+            im.reset()
+            im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+            G, Gw = gu.gpu_grids(im)
+            T = gu.oracle_table("pswf", 7, Q)
+            G_or, Gw_or, st = oc.grid(uvw, freq, vis, wt, n, ny, cell, Q, 7, T)
+            assert im.get_stats()["n_gridded"] == st["n_gridded"]
+            assert gu.rel_l2(G[0], G_or[0]) <= gu.GRID_TOL and gu.rel_l2(Gw[0], Gw_or[0]) <= gu.GRID_TOL
+        finally:
+            im.destroy()
+
+
+def test_owner_heavy_tile_is_split_into_chunks_and_summed():
+    """40,000 visibilities inside +-6 cells of the uv origin: the centre tile holds ~80,000 samples = 20 chunk items
+    whose partial tiles the last chunk adds up; the second call exercises accumulate mode on a heavy tile."""
+    n, cell, Q = 256, 20.0, 64
+    rng = np.random.default_rng(99)
+    nvis = 40000
+    fov = n * cell * mo.ARCSEC
+    uv_l = rng.uniform(-6.0, 6.0, (nvis, 2)) / fov                        # wavelengths
+    freq = np.full(nvis, 1.0e9)
+    uvw = np.zeros((nvis, 3), np.float32)
+    uvw[:, :2] = (uv_l * mo.C_M_S / 1.0e9).astype(np.float32)
+    vis = (rng.standard_normal(nvis) + 1j * rng.standard_normal(nvis)).astype(np.complex64)
+    wt = rng.uniform(0.5, 1.5, nvis).astype(np.float32)
+    # images=False: with all the power inside +-6 cells of the origin the image is smooth and small against the fp32
+    # FFT noise that 1/(cx*cy) amplifies towards the edge of the 75% box; the grid gates are what this case is about
+    res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, Q, strategy=OWNER, splits=2, images=False)
+    assert res["stats"]["n_gridded"] == nvis
+
+
+def test_owner_strategy_is_refused_where_it_does_not_apply():
+    im = gu.make_imager(128, 40.0, 5, 8, strategy=OWNER)
+    try:
+        uvw, freq, vis, wt = synth.random_visibilities(1, 10, 128, 40.0)
+        with pytest.raises(binding.MuserError) as e:
+            im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        assert e.value.code == binding.MUSER_EUNSUPPORTED
+    finally:
+        im.destroy()
+
+
+def test_reset_then_read_back_is_zero_with_lazy_zeroing():
+    """muser_reset defers the memset when the owner-tile gridder follows; every other consumer must still see zeros."""
+    im = gu.make_imager(128, 40.0, 7, 8)
+    try:
+        uvw, freq, vis, wt = synth.random_visibilities(2, 300, 128, 40.0)
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        im.reset()
+        G, Gw = gu.gpu_grids(im)
+        assert not G.any() and not Gw.any()
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        im.reset()
+        d, p = gu.gpu_images(im)
+        assert not d.any() and not p.any()
+        im.reset()
+        im.set_strategy(TILED)                                   # a deferred reset must survive a strategy change
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        G1, _ = gu.gpu_grids(im)
+        im.set_strategy(OWNER)
+        im.reset()
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        G2, _ = gu.gpu_grids(im)
+        assert gu.rel_l2(G2, G1) <= 1e-6
+    finally:
+        im.destroy()
 
 
 def test_empty_input_and_reset():
@@ -165,7 +244,7 @@ def test_wprojection_planes_match_oracle(strategy, library_tables):
         im.destroy()
 
 
-@pytest.mark.parametrize("strategy", [DIRECT, TILED])
+@pytest.mark.parametrize("strategy", [OWNER, DIRECT, TILED])
 def test_batched_grids_cfg4_slice(strategy):
     fr = synth.make_frame(4, nframes=1)                       # 32 grids of 512x512, 1770 visibilities each
     p = fr.params
