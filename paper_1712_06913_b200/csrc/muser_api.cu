@@ -179,7 +179,8 @@ int build_tile_order(muser_imager* h) {
         }
     std::sort(key.begin(), key.end());
     std::vector<uint32_t> order((size_t)g.ntiles);
-    for (size_t i = 0; i < key.size(); ++i) order[i] = key[i].second;
+    for (size_t i = 0; i < key.size(); ++i)                          // packed (ty << 16 | tx)
+        order[i] = ((key[i].second / (uint32_t)g.ntx) << 16) | (key[i].second % (uint32_t)g.ntx);
     cudaFree(h->order_d); h->order_d = nullptr;
     CU(h, cudaMalloc(&h->order_d, order.size() * sizeof(uint32_t)));
     CU(h, cudaMemcpy(h->order_d, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
@@ -214,12 +215,14 @@ int upload_tables(muser_imager* h, const std::vector<std::vector<double>>& t64, 
     CU(h, cudaMemcpy(h->tables_d, dev.data(), dev.size() * sizeof(float), cudaMemcpyHostToDevice));
     CU(h, cudaMalloc(&h->planes_d, P * sizeof(PlaneMeta)));
     CU(h, cudaMemcpy(h->planes_d, h->planes_h.data(), P * sizeof(PlaneMeta), cudaMemcpyHostToDevice));
-    // owner-tile path: padded transposed table TTp[r][0] = 0, TTp[r][1 + j] = T[j*Q + r], TTp[r][8..9] = 0
+    // owner-tile path: two-parity transposed table TT2[(par*(Q+1) + r)*8 + par + j] = T[j*Q + r], other entries 0
     cudaFree(h->ttp_d); h->ttp_d = nullptr;
     if (!wm && P == 1 && supports[0] == 7) {
-        std::vector<float> ttp((size_t)(Q + 1) * kOwTablePitch, 0.f);
-        for (int r = 0; r <= Q; ++r)
-            for (int j = 0; j < 7; ++j) ttp[(size_t)r * kOwTablePitch + 1 + j] = h->tables_f32[0][(size_t)j * Q + r];
+        std::vector<float> ttp((size_t)2 * (Q + 1) * 8, 0.f);
+        for (int par = 0; par < 2; ++par)
+            for (int r = 0; r <= Q; ++r)
+                for (int j = 0; j < 7; ++j)
+                    ttp[((size_t)par * (Q + 1) + r) * 8 + par + j] = h->tables_f32[0][(size_t)j * Q + r];
         CU(h, cudaMalloc(&h->ttp_d, ttp.size() * sizeof(float)));
         CU(h, cudaMemcpy(h->ttp_d, ttp.data(), ttp.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
@@ -339,7 +342,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         uint32_t max_items = 0;
         int rc = ensure_owner_scratch(h, nvis, item_size, &max_items);
         if (rc) return rc;
-        if ((unsigned long long)max_items + g.nbins >= 0x7FFFFFFFull) return fail(h, MUSER_EUNSUPPORTED, "too many tiles for one launch");
+        if ((unsigned long long)max_items / g.ngrids + g.ntiles + 1 > 65535ull) return fail(h, MUSER_EUNSUPPORTED, "too many tiles for one launch");
         h->last_stream = s;
         h->fft_valid = false;
         {
@@ -471,7 +474,7 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
         return nullptr;
     };
     if (rc) return bail("geometry");
-    if (tiled_kernel_setup(h->max_smem) != cudaSuccess) { h->err = cudaGetErrorString(cudaGetLastError()); return bail("kernel setup"); }
+    if (tiled_kernel_setup(h->max_smem) != cudaSuccess || owner_kernel_setup(h->max_smem) != cudaSuccess) { h->err = cudaGetErrorString(cudaGetLastError()); return bail("kernel setup"); }
     if (cudaMalloc(&h->stats_d, sizeof(Stats)) != cudaSuccess || cudaMalloc(&h->nitems_d, sizeof(uint32_t)) != cudaSuccess) {
         h->err = "cudaMalloc failed"; return bail("alloc");
     }

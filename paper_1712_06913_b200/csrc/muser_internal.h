@@ -86,7 +86,8 @@ cudaError_t tiled_kernel_setup(int max_smem_bytes);
 // crosses a tile edge are listed in every tile they touch.
 constexpr int kOwSub = 1024;                 // samples staged and cell-sorted in shared memory per pass
 constexpr int kOwTileFloats = 32 * 32 * 3;   // one partial tile in the scratch buffer: A[32][32] float2 + B[32][32] float
-constexpr int kOwTablePitch = 10;            // padded transposed table: TTp[rx][0] = 0, [1..7] = T[j*Q+rx], [8..9] = 0
+// two-parity transposed table TT2[(par*(Q+1) + r)*8 + i]: par 0: i = j (j = 0..6: T[j*Q + r]), [7] = 0;
+// par 1: [0] = 0, i = j + 1
 struct OwItem {                              // one chunk of a heavy tile (more than item_size samples)
     uint32_t bin, start, count, first_slot, nchunks, chunk;
 };
@@ -97,9 +98,10 @@ cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_
 cudaError_t launch_owner_scatter(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                                  const int* grid_id, long long nvis, const uint32_t* bin_offset, uint32_t* cursor,
                                  uint4* sorted, cudaStream_t s);
+cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
                               const OwItem* items, const uint32_t* nitems, uint32_t max_items, uint32_t item_size,
-                              const uint32_t* order, const float* ttp, GridPtrs grids, float* scratch,
+                              const uint32_t* order, const float* tt2, GridPtrs grids, float* scratch,
                               uint32_t* tickets, int store_mode, cudaStream_t s);
 
 }  // namespace muser

@@ -1,17 +1,19 @@
 // Owner-tile gridding path (2-D mode, support 7), sm_100a.
 //
 //   O1 k_owner_count    A1: fp64 coordinates (O1 order), keep/drop, statistics, histogram of the tiles
-//                           each sample's 7x7 footprint touches (1, 2 or 4 tiles; warp-aggregated atomics)
+//                           each sample's 7x7 footprint touches (1, 2 or 4 tiles); counts in a CTA-private shared
+//                           histogram, one global atomic per touched tile per CTA
 //   O2 k_owner_scan     A1: exclusive scan of the histogram; tiles with more than item_size samples are split
 //                           into chunk items
 //   O3 k_owner_scatter  A1: recomputes the coordinates and writes one 16-byte record per (sample, touched tile)
-//   O4 k_grid_owner_s7  A2/A4: one CTA per 32x32 tile of one grid.  It stages <= 1024 records at a time in shared
-//                           memory, counting-sorts them by (row, 8-cell column window), and every warp walks an
-//                           equal slice of the sorted list with the 7 x 8 window held in registers (lane = row r,
-//                           column pair c; packed FFMA2), touching shared memory only when the window changes.
-//                           The tile is then written to G and Gw with plain coalesced stores: the grids need no
-//                           memset and receive no global atomics.  Chunks of a heavy tile write partial tiles to a
-//                           scratch buffer; the last chunk to finish adds them up in chunk order.
+//   O4 k_grid_owner_s7  A2/A4: one CTA per 32x32 tile of one grid (or per chunk of a heavy tile).  It counting-sorts
+//                           up to 4096 records by (row, 8-cell column window), stages them 1024 at a time in shared
+//                           memory in sorted order, and every warp walks an equal slice with the 7-row x 8-column
+//                           window held in registers (lane = row r, column pair c; packed FFMA2; kernel table in
+//                           shared memory), touching the shared tile only when the window changes.  The tile is
+//                           then written to G and Gw with plain coalesced stores: the grids need no memset and
+//                           receive no global atomics.  Chunks of a heavy tile write partial tiles to a scratch
+//                           buffer; the last chunk to finish adds them up in chunk order.
 // Passages: PAPER.md:78 (gridding = convolution onto a regular grid), :136-138 (spheroidal GCF), :216-228 (float2
 // grid, row-major, Hermitian), :249-256 (DIRTY_IMAGE).  The binning and tiling are this build's design.
 #include "muser_internal.h"
@@ -94,12 +96,31 @@ __device__ __forceinline__ uint32_t ow_agg_inc(uint32_t* __restrict__ cnt, uint3
     return base + (uint32_t)__popc(m & ((1u << lane) - 1u));
 }
 
+// CTA-level aggregation for the two binning kernels: when every visibility of the CTA belongs to one grid and that
+// grid's tile count fits the shared histogram, the CTA counts in shared memory and issues ONE global atomic per
+// touched tile (MUSER's central tile takes a third of all samples: per-sample global atomics serialise on it).
+constexpr int kBinThreads = 1024;
+constexpr int kBinSmemTiles = 8192;
+
+__device__ __forceinline__ int ow_cta_uniform_grid(const OwLoc& L, int ntiles, int* s_flag) {
+    // s_flag[0] = first kept grid id seen (or -1), s_flag[1] = 1 if a kept visibility disagrees
+    if (threadIdx.x == 0) { s_flag[0] = -1; s_flag[1] = 0; }
+    __syncthreads();
+    if (L.state == 3) atomicCAS(&s_flag[0], -1, L.gid);
+    __syncthreads();
+    if (L.state == 3 && L.gid != s_flag[0]) s_flag[1] = 1;
+    __syncthreads();
+    return ntiles <= kBinSmemTiles && s_flag[1] == 0 && s_flag[0] >= 0;
+}
+
 // ------------------------------------------------------------------------------------------------- O1 count
-__global__ void __launch_bounds__(256) k_owner_count(const Geom g, const float* __restrict__ uvw,
-                                                     const double* __restrict__ freq, const float2* __restrict__ vis,
-                                                     const float* __restrict__ weight, const int* __restrict__ grid_id,
-                                                     const long long nvis, uint32_t* __restrict__ bin_count,
-                                                     Stats* __restrict__ stats) {
+__global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const float* __restrict__ uvw,
+                                                             const double* __restrict__ freq, const float2* __restrict__ vis,
+                                                             const float* __restrict__ weight, const int* __restrict__ grid_id,
+                                                             const long long nvis, uint32_t* __restrict__ bin_count,
+                                                             Stats* __restrict__ stats) {
+    extern __shared__ uint32_t s_hist[];
+    __shared__ int s_flag[2];
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     OwLoc L;
@@ -112,7 +133,31 @@ __global__ void __launch_bounds__(256) k_owner_count(const Geom g, const float* 
         w2sum = (double)L.wt * (double)L.wt;
         v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
     }
-    if (__any_sync(kFull, kept)) {
+    const int use_smem = ow_cta_uniform_grid(L, g.ntiles, s_flag);
+    if (use_smem) {
+        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) s_hist[i] = 0;
+        __syncthreads();
+        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ntiles;
+        uint32_t first[8];                                            // bit q + 4s set: this thread saw the tile empty
+        uint32_t firstmask = 0;
+        if (kept) {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    int tx, ty;
+                    const uint32_t bin = ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty);
+                    first[q + 4 * s] = bin;
+                    if (bin != kNoBin && atomicAdd(&s_hist[bin - gbase], 1u) == 0u) firstmask |= 1u << (q + 4 * s);
+                }
+        }
+        __syncthreads();
+        if (firstmask) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (firstmask & (1u << j)) atomicAdd(&bin_count[first[j]], s_hist[first[j] - gbase]);
+        }
+    } else if (__any_sync(kFull, kept)) {
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
 #pragma unroll
@@ -124,8 +169,8 @@ __global__ void __launch_bounds__(256) k_owner_count(const Geom g, const float* 
         }
     }
     // block reduction of the counters, one atomic set per block
-    __shared__ int s_cnt[3][8];
-    __shared__ double s_w[3][8];
+    __shared__ int s_cnt[3][32];
+    __shared__ double s_w[3][32];
     const int c0 = __reduce_add_sync(kFull, kept), c1 = __reduce_add_sync(kFull, dropped), c2 = __reduce_add_sync(kFull, flagged);
     for (int o = 16; o > 0; o >>= 1) {
         wsum += __shfl_xor_sync(kFull, wsum, o);
@@ -137,7 +182,7 @@ __global__ void __launch_bounds__(256) k_owner_count(const Geom g, const float* 
     if (threadIdx.x == 0) {
         int t0 = 0, t1 = 0, t2 = 0;
         double tw = 0.0, tv2 = 0.0, tw2 = 0.0;
-        for (int w = 0; w < 8; ++w) {
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
             t0 += s_cnt[0][w]; t1 += s_cnt[1][w]; t2 += s_cnt[2][w];
             tw += s_w[0][w]; tv2 += s_w[1][w]; tw2 += s_w[2][w];
         }
@@ -217,21 +262,85 @@ __global__ void __launch_bounds__(1024) k_owner_scan(const Geom g, uint32_t* __r
 }
 
 // ------------------------------------------------------------------------------------------------- O3 scatter
-// Record: {wt*Re, +-wt*Im, wt, ox | oy << 6 | rx << 12 | ry << 21}; (ox, oy) = first footprint cell relative to the
-// tile origin, plus 6, in [0, 38); rx = Q/2 - ru, ry = Q/2 - rv in [0, Q].
-__global__ void __launch_bounds__(256) k_owner_scatter(const Geom g, const float* __restrict__ uvw,
-                                                       const double* __restrict__ freq, const float2* __restrict__ vis,
-                                                       const float* __restrict__ weight, const int* __restrict__ grid_id,
-                                                       const long long nvis, const uint32_t* __restrict__ bin_offset,
-                                                       uint32_t* __restrict__ cursor, uint4* __restrict__ sorted) {
+// Record: {wt*Re, +-wt*Im, wt, key | X << 11 | ry << 21}.  (ox, oy) = first footprint cell relative to the tile
+// origin, plus 6, in [0, 38); key = oy << 5 | ox >> 1 names the 7-row x 8-column register window (columns
+// 2*(ox>>1) - 6 ... + 7 of the tile) that holds the footprint; par = ox & 1 is the footprint's offset inside it;
+// X = par*(Q+1) + rx and ry select the rows of the two-parity table TT2 (rx = Q/2 - ru, ry = Q/2 - rv in [0, Q]).
+__device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, int s, int tx, int ty, uint4* dst) {
+    const int h = (g.S - 1) >> 1;
+    const int ox = L.cu[s] - (tx * kTile - kTile / 2) + h;
+    const int oy = L.cv[s] - (ty * kTile - kTile / 2) + h;
+    uint4 o;
+    o.x = __float_as_uint(L.re);
+    o.y = __float_as_uint(s ? -L.im : L.im);
+    o.z = __float_as_uint(L.wt);
+    const uint32_t X = (uint32_t)((ox & 1) * (g.Q + 1) + L.rx[s]);
+    o.w = (uint32_t)(oy << 5 | ox >> 1) | (X << 11) | ((uint32_t)L.ry[s] << 21);
+    *dst = o;
+}
+
+__global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, const float* __restrict__ uvw,
+                                                               const double* __restrict__ freq, const float2* __restrict__ vis,
+                                                               const float* __restrict__ weight, const int* __restrict__ grid_id,
+                                                               const long long nvis, const uint32_t* __restrict__ bin_offset,
+                                                               uint32_t* __restrict__ cursor, uint4* __restrict__ sorted) {
+    extern __shared__ uint32_t s_hist[];
+    __shared__ int s_flag[2];
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     OwLoc L;
     float2 V;
     ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V);
     const int kept = L.state == 3;
+    const int use_smem = ow_cta_uniform_grid(L, g.ntiles, s_flag);
+    if (use_smem) {
+        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) s_hist[i] = 0;
+        __syncthreads();
+        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ntiles;
+        uint32_t bins[8], rank[8];
+        uint32_t firstmask = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) bins[j] = kNoBin;
+        if (kept) {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    int tx, ty;
+                    const uint32_t bin = ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty);
+                    bins[q + 4 * s] = bin;
+                    if (bin != kNoBin) {
+                        rank[q + 4 * s] = atomicAdd(&s_hist[bin - gbase], 1u);
+                        if (rank[q + 4 * s] == 0u) firstmask |= 1u << (q + 4 * s);
+                    }
+                }
+        }
+        __syncthreads();
+        if (firstmask) {                                              // reserve this CTA's run in each touched tile
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (firstmask & (1u << j)) {
+                    const uint32_t t = bins[j] - gbase;
+                    s_hist[t] = bin_offset[bins[j]] + atomicAdd(&cursor[bins[j]], s_hist[t]);
+                }
+        }
+        __syncthreads();
+        if (kept) {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t bin = bins[q + 4 * s];
+                    if (bin != kNoBin) {
+                        int tx, ty;
+                        ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty);
+                        ow_write_record(g, L, s, tx, ty, sorted + s_hist[bin - gbase] + rank[q + 4 * s]);
+                    }
+                }
+        }
+        return;
+    }
     if (!__any_sync(kFull, kept)) return;
-    const int h = (g.S - 1) >> 1;
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
 #pragma unroll
@@ -240,16 +349,7 @@ __global__ void __launch_bounds__(256) k_owner_scatter(const Geom g, const float
             const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
             if (!__any_sync(kFull, bin != kNoBin)) continue;
             const uint32_t rank = ow_agg_inc(cursor, bin, lane);
-            if (bin != kNoBin) {
-                const int ox = L.cu[s] - h - (tx * kTile - kTile / 2) + 2 * h;
-                const int oy = L.cv[s] - h - (ty * kTile - kTile / 2) + 2 * h;
-                uint4 o;
-                o.x = __float_as_uint(L.re);
-                o.y = __float_as_uint(s ? -L.im : L.im);
-                o.z = __float_as_uint(L.wt);
-                o.w = (uint32_t)ox | ((uint32_t)oy << 6) | ((uint32_t)L.rx[s] << 12) | ((uint32_t)L.ry[s] << 21);
-                sorted[bin_offset[bin] + rank] = o;
-            }
+            if (bin != kNoBin) ow_write_record(g, L, s, tx, ty, sorted + bin_offset[bin] + rank);
         }
     }
 }
@@ -286,40 +386,48 @@ constexpr int kOwAPitch = 40;     // float2 per row of the (re, im) tile: 32 cel
 constexpr int kOwBPitch = 40;     // floats per row of the weight tile
 constexpr int kOwKeys = 768;      // 38 rows x 19 windows = 722 sort keys, padded to 3 per thread
 constexpr int kOwDirect = 24;     // tiles with at most this many samples skip the shared-memory sort
+constexpr int kOwUnit = 4096;     // samples counting-sorted together (in kOwSub-sized rounds)
+
+// shared-memory layout (bytes); the table region is sized by Q at launch
+constexpr int kOwOffA = 0;
+constexpr int kOwOffB = kOwOffA + 32 * kOwAPitch * 8;
+constexpr int kOwOffR = kOwOffB + 32 * kOwBPitch * 4;
+constexpr int kOwOffH = kOwOffR + kOwSub * 16;
+constexpr int kOwOffP = kOwOffH + kOwKeys * 4;
+constexpr int kOwOffT = kOwOffP + kOwUnit * 2;
+static size_t owner_smem_bytes(int Q) { return (size_t)kOwOffT + (size_t)2 * (Q + 1) * 8 * sizeof(float); }
 
 struct OwWarpAcc {
     unsigned long long a0, a1, b;  // (re, im) of the lane's two cells; (wt, wt') of the two cells
-    int key;                       // (oy << 5 | ox >> 1) of the window held in registers, -1: none
-    int row, col0, valid;
+    uint32_t key;                  // oy << 5 | ox >> 1 of the window held in registers, 0xFFFFFFFF: none
+    int offA, offB;                // float2 / float index of the lane's first cell in sA / sB, or -1 if outside the tile
 };
 
 __device__ __forceinline__ void ow_flush(OwWarpAcc& A, float2* sA, float* sB) {
-    if (A.key >= 0 && A.valid) {
-        ow_sadd2(&sA[A.row * kOwAPitch + A.col0], A.a0);
-        ow_sadd2(&sA[A.row * kOwAPitch + A.col0 + 1], A.a1);
-        ow_sadd2(&sB[A.row * kOwBPitch + A.col0], A.b);
+    if (A.offA >= 0) {
+        ow_sadd2(&sA[A.offA], A.a0);
+        ow_sadd2(&sA[A.offA + 1], A.a1);
+        ow_sadd2(&sB[A.offB], A.b);
     }
     A.a0 = A.a1 = A.b = 0ull;
 }
 
-__device__ __forceinline__ void ow_accumulate(OwWarpAcc& A, const uint4 rec, const float* __restrict__ ttp, const int r,
+// One sample into the warp's register window.  tbx = table + 2c floats, tby = table + r floats (shared memory).
+__device__ __forceinline__ void ow_accumulate(OwWarpAcc& A, const uint4 rec, const char* tbx, const char* tby, const int r,
                                               const int c, float2* sA, float* sB) {
     const uint32_t pk = rec.w;
-    const int key = (int)((pk & 0xFFFu) >> 1);
+    const uint32_t key = pk & 0x7FFu;
     if (key != A.key) {                                              // warp-uniform branch
-        ow_flush(A, sA, sB);
+        if (A.key != 0xFFFFFFFFu) ow_flush(A, sA, sB);
         A.key = key;
-        const int ox = (int)(pk & 63u), oy = (int)((pk >> 6) & 63u);
-        A.row = oy - 6 + r;
-        A.col0 = (ox & ~1) - 6 + 2 * c;
-        A.valid = (r < 7) && ((unsigned)A.row < 32u) && ((unsigned)A.col0 < 32u);
+        const int row = (int)(key >> 5) - 6 + r, col0 = 2 * (int)(key & 31u) - 6 + 2 * c;
+        const bool valid = (r < 7) && ((unsigned)row < 32u) && ((unsigned)col0 < 32u);
+        A.offA = valid ? row * kOwAPitch + col0 : -1;
+        A.offB = row * kOwBPitch + col0;
     }
-    const int par = (int)(pk & 1u);
-    const int rx = (int)((pk >> 12) & 511u), ry = (int)((pk >> 21) & 511u);
-    const float* tx = ttp + rx * kOwTablePitch + (2 * c + 1 - par);
-    const float kx0 = __ldg(tx), kx1 = __ldg(tx + 1);
-    const float ky = __ldg(ttp + ry * kOwTablePitch + r + 1);
-    const float k0 = kx0 * ky, k1 = kx1 * ky;
+    const float2 kx = *reinterpret_cast<const float2*>(tbx + ((pk >> 6) & 0x7FE0u));     // X * 32 bytes
+    const float ky = *reinterpret_cast<const float*>(tby + ((pk >> 16) & 0x3FE0u));      // ry * 32 bytes
+    const float k0 = kx.x * ky, k1 = kx.y * ky;
     const unsigned long long v = ow_pack(__uint_as_float(rec.x), __uint_as_float(rec.y));
     const float wt = __uint_as_float(rec.z);
     A.a0 = ow_fma2(ow_pack(k0, k0), v, A.a0);
@@ -327,40 +435,50 @@ __device__ __forceinline__ void ow_accumulate(OwWarpAcc& A, const uint4 rec, con
     A.b = ow_fma2(ow_pack(k0, k1), ow_pack(wt, wt), A.b);
 }
 
+__device__ __forceinline__ uint32_t ow_sortkey(uint32_t w) { return ((w >> 5) & 63u) * 19u + (w & 31u); }
+
+// Launch grid: x = grid index (fastest), y = [item rows | tile rank, centre-out].  Item rows come first so that
+// the chunks of heavy tiles start before anything else.
 template <int STORE>
-__global__ void __launch_bounds__(256) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
-                                                       const uint32_t* __restrict__ bin_offset,
-                                                       uint32_t* __restrict__ cursor, const OwItem* __restrict__ items,
-                                                       const uint32_t* __restrict__ nitems, const uint32_t max_items,
-                                                       const uint32_t item_size, const uint32_t* __restrict__ order,
-                                                       const float* __restrict__ ttp, GridPtrs grids,
-                                                       float* __restrict__ scratch, uint32_t* __restrict__ tickets) {
-    __shared__ __align__(16) float2 sA[32 * kOwAPitch];
-    __shared__ __align__(16) float sB[32 * kOwBPitch];
-    __shared__ __align__(16) uint4 sR[kOwSub];
-    __shared__ uint32_t sH[kOwKeys];
+__global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
+                                                          const uint32_t* __restrict__ bin_offset,
+                                                          uint32_t* __restrict__ cursor, const OwItem* __restrict__ items,
+                                                          const uint32_t* __restrict__ nitems, const uint32_t item_rows,
+                                                          const uint32_t item_size, const uint32_t* __restrict__ order,
+                                                          const float* __restrict__ tt2, GridPtrs grids,
+                                                          float* __restrict__ scratch, uint32_t* __restrict__ tickets) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    float2* sA = reinterpret_cast<float2*>(smem + kOwOffA);
+    float* sB = reinterpret_cast<float*>(smem + kOwOffB);
+    uint4* sR = reinterpret_cast<uint4*>(smem + kOwOffR);
+    uint32_t* sH = reinterpret_cast<uint32_t*>(smem + kOwOffH);
+    unsigned short* sP = reinterpret_cast<unsigned short*>(smem + kOwOffP);
+    float* sT = reinterpret_cast<float*>(smem + kOwOffT);
     __shared__ uint32_t sW[8];
     __shared__ int sLast;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    uint32_t bin, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
-    const bool heavy = blockIdx.x < max_items;
+    uint32_t gi, tile, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
+    const bool heavy = blockIdx.y < item_rows;
     if (heavy) {
-        if (blockIdx.x >= *nitems) return;
-        const OwItem it = items[blockIdx.x];
-        bin = it.bin; start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
-        if (chunk == 0 && tid == 0) cursor[bin] = 0;
+        const uint32_t idx = blockIdx.y * gridDim.x + blockIdx.x;
+        if (idx >= *nitems) return;
+        const OwItem it = items[idx];
+        gi = it.bin / (uint32_t)g.ntiles; tile = it.bin - gi * (uint32_t)g.ntiles;
+        tile = ((tile / (uint32_t)g.ntx) << 16) | (tile % (uint32_t)g.ntx);   // packed (ty << 16 | tx)
+        start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
+        if (chunk == 0 && tid == 0) cursor[it.bin] = 0;
     } else {
-        const uint32_t t = blockIdx.x - max_items;
-        const uint32_t r = t / (uint32_t)g.ngrids, gi = t - r * (uint32_t)g.ngrids;
-        bin = gi * (uint32_t)g.ntiles + order[r];
+        gi = blockIdx.x;
+        const uint32_t t = order[blockIdx.y - item_rows];             // packed (ty << 16 | tx), centre-out
+        const uint32_t bin = gi * (uint32_t)g.ntiles + (t >> 16) * (uint32_t)g.ntx + (t & 0xFFFFu);
+        tile = t;
         start = bin_offset[bin];
         cnt = bin_offset[bin + 1] - start;
         if (cnt > item_size) return;                                  // heavy tile: its chunk items do the work
         if (cnt && tid == 0) cursor[bin] = 0;
     }
-    const uint32_t tile = bin % (uint32_t)g.ntiles, gi = bin / (uint32_t)g.ntiles;
-    const int ty = (int)(tile / (uint32_t)g.ntx), tx = (int)(tile % (uint32_t)g.ntx);
+    const int ty = (int)(tile >> 16), tx = (int)(tile & 0xFFFFu);
     const int x0 = tx * kTile - kTile / 2, y0 = ty * kTile - kTile / 2;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
     float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
@@ -381,38 +499,32 @@ __global__ void __launch_bounds__(256) k_grid_owner_s7(const Geom g, const uint4
         return;
     }
 
-    {   // zero the tile accumulators
-        float4* za = reinterpret_cast<float4*>(sA);
-        for (int i = tid; i < 32 * kOwAPitch / 2; i += 256) za[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        float4* zb = reinterpret_cast<float4*>(sB);
-        for (int i = tid; i < 32 * kOwBPitch / 4; i += 256) zb[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    {   // zero the tile accumulators, stage the two-parity table
+        float4* za = reinterpret_cast<float4*>(smem + kOwOffA);
+        for (int i = tid; i < (kOwOffR - kOwOffA) / 16; i += 256) za[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4* src = reinterpret_cast<const float4*>(tt2);
+        float4* dst = reinterpret_cast<float4*>(sT);
+        for (int i = tid; i < 2 * (g.Q + 1) * 2; i += 256) dst[i] = __ldg(src + i);
     }
     const int r = lane >> 2, c = lane & 3;
+    const char* tbx = reinterpret_cast<const char*>(sT + 2 * c);
+    const char* tby = reinterpret_cast<const char*>(sT + r);
     OwWarpAcc A;
-    A.a0 = A.a1 = A.b = 0ull; A.key = -1; A.row = A.col0 = A.valid = 0;
+    A.a0 = A.a1 = A.b = 0ull; A.key = 0xFFFFFFFFu; A.offA = -1; A.offB = 0;
 
     if (cnt <= (uint32_t)kOwDirect) {
         __syncthreads();
-        for (uint32_t i = warp; i < cnt; i += 8) ow_accumulate(A, __ldg(sorted + start + i), ttp, r, c, sA, sB);
-        ow_flush(A, sA, sB);
+        for (uint32_t i = warp; i < cnt; i += 8) ow_accumulate(A, __ldg(sorted + start + i), tbx, tby, r, c, sA, sB);
+        if (A.key != 0xFFFFFFFFu) ow_flush(A, sA, sB);
         __syncthreads();
     } else {
-        for (uint32_t base = 0; base < cnt; base += kOwSub) {
-            const uint32_t n = min((uint32_t)kOwSub, cnt - base);
+        for (uint32_t ubase = 0; ubase < cnt; ubase += kOwUnit) {
+            const uint32_t n = min((uint32_t)kOwUnit, cnt - ubase);
+            const uint4* __restrict__ src = sorted + start + ubase;
             for (int i = tid; i < kOwKeys; i += 256) sH[i] = 0;
             __syncthreads();
-            // (1) counting sort by (row, window)
-            uint4 rec[kOwSub / 256];
-            uint32_t rk[kOwSub / 256];
-#pragma unroll
-            for (int j = 0; j < kOwSub / 256; ++j) {
-                const uint32_t i = tid + j * 256;
-                if (i < n) {
-                    rec[j] = __ldg(sorted + start + base + i);
-                    const uint32_t key = ((rec[j].w >> 6) & 63u) * 19u + ((rec[j].w & 63u) >> 1);
-                    rk[j] = atomicAdd(&sH[key], 1u);
-                }
-            }
+            // (1) counting sort of the unit by window (row-major): sorted position of every record
+            for (uint32_t i = tid; i < n; i += 256) sP[i] = (unsigned short)atomicAdd(&sH[ow_sortkey(__ldg(&src[i].w))], 1u);
             __syncthreads();
             {
                 const uint32_t h0 = sH[3 * tid], h1 = sH[3 * tid + 1], h2 = sH[3 * tid + 2];
@@ -429,24 +541,24 @@ __global__ void __launch_bounds__(256) k_grid_owner_s7(const Geom g, const uint4
                 sH[3 * tid] = ex; sH[3 * tid + 1] = ex + h0; sH[3 * tid + 2] = ex + h0 + h1;
             }
             __syncthreads();
-#pragma unroll
-            for (int j = 0; j < kOwSub / 256; ++j) {
-                const uint32_t i = tid + j * 256;
-                if (i < n) {
-                    const uint32_t key = ((rec[j].w >> 6) & 63u) * 19u + ((rec[j].w & 63u) >> 1);
-                    sR[sH[key] + rk[j]] = rec[j];
+            for (uint32_t i = tid; i < n; i += 256) sP[i] = (unsigned short)(sP[i] + sH[ow_sortkey(__ldg(&src[i].w))]);
+            __syncthreads();
+            // (2) rounds of kOwSub sorted records: stage, then every warp walks an equal slice with the window in registers
+            for (uint32_t lo = 0; lo < n; lo += kOwSub) {
+                for (uint32_t i = tid; i < n; i += 256) {
+                    const uint32_t p = (uint32_t)sP[i] - lo;
+                    if (p < (uint32_t)kOwSub) sR[p] = __ldg(src + i);
                 }
+                __syncthreads();
+                const int m = (int)min((uint32_t)kOwSub, n - lo);
+                const int per = (m + 7) >> 3;
+                const int b = warp * per, e = min(m, b + per);
+#pragma unroll 4
+                for (int i = b; i < e; ++i) ow_accumulate(A, sR[i], tbx, tby, r, c, sA, sB);
+                if (A.key != 0xFFFFFFFFu) ow_flush(A, sA, sB);
+                A.key = 0xFFFFFFFFu;
+                __syncthreads();
             }
-            __syncthreads();
-            // (2) register accumulation over runs of equal window
-            {
-                const int per = ((int)n + 7) >> 3;
-                const int b = warp * per, e = min((int)n, b + per);
-                for (int i = b; i < e; ++i) ow_accumulate(A, sR[i], ttp, r, c, sA, sB);
-                ow_flush(A, sA, sB);
-                A.key = -1;
-            }
-            __syncthreads();
         }
     }
 
@@ -508,9 +620,12 @@ __global__ void __launch_bounds__(256) k_grid_owner_s7(const Geom g, const uint4
 }
 
 // ------------------------------------------------------------------------------------------------- launchers
+static size_t bin_smem_bytes(const Geom& g) { return g.ntiles <= kBinSmemTiles ? (size_t)g.ntiles * sizeof(uint32_t) : 0; }
+
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                                const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, cudaStream_t s) {
-    k_owner_count<<<(unsigned)((nvis + 255) / 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats);
+    k_owner_count<<<(unsigned)((nvis + kBinThreads - 1) / kBinThreads), kBinThreads, bin_smem_bytes(g), s>>>(
+        g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats);
     return cudaGetLastError();
 }
 
@@ -523,22 +638,31 @@ cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_
 cudaError_t launch_owner_scatter(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                                  const int* grid_id, long long nvis, const uint32_t* bin_offset, uint32_t* cursor,
                                  uint4* sorted, cudaStream_t s) {
-    k_owner_scatter<<<(unsigned)((nvis + 255) / 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_offset,
-                                                                  cursor, sorted);
+    k_owner_scatter<<<(unsigned)((nvis + kBinThreads - 1) / kBinThreads), kBinThreads, bin_smem_bytes(g), s>>>(
+        g, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
     return cudaGetLastError();
+}
+
+cudaError_t owner_kernel_setup(int max_smem_bytes) {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(k_grid_owner_s7<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
+    if ((e = cudaFuncSetAttribute(k_grid_owner_s7<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
+    return cudaSuccess;
 }
 
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
                               const OwItem* items, const uint32_t* nitems, uint32_t max_items, uint32_t item_size,
-                              const uint32_t* order, const float* ttp, GridPtrs grids, float* scratch,
+                              const uint32_t* order, const float* tt2, GridPtrs grids, float* scratch,
                               uint32_t* tickets, int store_mode, cudaStream_t s) {
-    const unsigned blocks = max_items + g.nbins;
+    const uint32_t item_rows = (max_items + (uint32_t)g.ngrids - 1) / (uint32_t)g.ngrids;
+    const dim3 blocks((unsigned)g.ngrids, item_rows + (unsigned)g.ntiles);
+    const size_t smem = owner_smem_bytes(g.Q);
     if (store_mode)
-        k_grid_owner_s7<1><<<blocks, 256, 0, s>>>(g, sorted, bin_offset, cursor, items, nitems, max_items, item_size,
-                                                  order, ttp, grids, scratch, tickets);
+        k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, item_rows, item_size,
+                                                     order, tt2, grids, scratch, tickets);
     else
-        k_grid_owner_s7<0><<<blocks, 256, 0, s>>>(g, sorted, bin_offset, cursor, items, nitems, max_items, item_size,
-                                                  order, ttp, grids, scratch, tickets);
+        k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, item_rows, item_size,
+                                                     order, tt2, grids, scratch, tickets);
     return cudaGetLastError();
 }
 
