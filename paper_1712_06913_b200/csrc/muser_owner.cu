@@ -262,10 +262,11 @@ __global__ void __launch_bounds__(1024) k_owner_scan(const Geom g, uint32_t* __r
 }
 
 // ------------------------------------------------------------------------------------------------- O3 scatter
-// Record: {wt*Re, +-wt*Im, wt, key | X << 11 | ry << 21}.  (ox, oy) = first footprint cell relative to the tile
-// origin, plus 6, in [0, 38); key = oy << 5 | ox >> 1 names the 7-row x 8-column register window (columns
-// 2*(ox>>1) - 6 ... + 7 of the tile) that holds the footprint; par = ox & 1 is the footprint's offset inside it;
-// X = par*(Q+1) + rx and ry select the rows of the two-parity table TT2 (rx = Q/2 - ru, ry = Q/2 - rv in [0, Q]).
+// Record: {wt*Re, +-wt*Im, wt, key | X << 10 | Y << 20}.  (ox, oy) = first footprint cell relative to the tile
+// origin, plus 6, in [0, 38); key = (oy >> 1) << 5 | ox >> 1 names the 8 x 8 register window (rows 2*(oy>>1) - 6 ...
+// + 7, columns 2*(ox>>1) - 6 ... + 7 of the tile) that holds the 7 x 7 footprint; (ox & 1, oy & 1) is the
+// footprint's offset inside it; X = (ox&1)*(Q+1) + rx and Y = (oy&1)*(Q+1) + ry select the rows of the two-parity
+// table TT2 (rx = Q/2 - ru, ry = Q/2 - rv in [0, Q]).
 __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, int s, int tx, int ty, uint4* dst) {
     const int h = (g.S - 1) >> 1;
     const int ox = L.cu[s] - (tx * kTile - kTile / 2) + h;
@@ -275,7 +276,8 @@ __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, i
     o.y = __float_as_uint(s ? -L.im : L.im);
     o.z = __float_as_uint(L.wt);
     const uint32_t X = (uint32_t)((ox & 1) * (g.Q + 1) + L.rx[s]);
-    o.w = (uint32_t)(oy << 5 | ox >> 1) | (X << 11) | ((uint32_t)L.ry[s] << 21);
+    const uint32_t Y = (uint32_t)((oy & 1) * (g.Q + 1) + L.ry[s]);
+    o.w = (uint32_t)((oy >> 1) << 5 | ox >> 1) | (X << 10) | (Y << 20);
     *dst = o;
 }
 
@@ -384,7 +386,7 @@ __device__ __forceinline__ void ow_sadd2(void* p, unsigned long long v) {
 
 constexpr int kOwAPitch = 40;     // float2 per row of the (re, im) tile: 32 cells + 8 pad
 constexpr int kOwBPitch = 40;     // floats per row of the weight tile
-constexpr int kOwKeys = 768;      // 38 rows x 19 windows = 722 sort keys, padded to 3 per thread
+constexpr int kOwKeys = 512;      // 19 x 19 = 361 windows, padded to 2 per thread
 constexpr int kOwDirect = 24;     // tiles with at most this many samples skip the shared-memory sort
 constexpr int kOwUnit = 4096;     // samples counting-sorted together (in kOwSub-sized rounds)
 
@@ -399,34 +401,31 @@ static size_t owner_smem_bytes(int Q) { return (size_t)kOwOffT + (size_t)2 * (Q 
 
 struct OwWarpAcc {
     unsigned long long a0, a1, b;  // (re, im) of the lane's two cells; (wt, wt') of the two cells
-    uint32_t key;                  // oy << 5 | ox >> 1 of the window held in registers, 0xFFFFFFFF: none
-    int offA, offB;                // float2 / float index of the lane's first cell in sA / sB, or -1 if outside the tile
+    int offA, offB;                // float2 / float index of the lane's first cell in sA / sB, offA = -1 outside the tile
 };
 
-__device__ __forceinline__ void ow_flush(OwWarpAcc& A, float2* sA, float* sB) {
+// Point the warp's 8 x 8 register window at window `key`; lane (r, c) holds row r, columns 2c and 2c + 1.
+__device__ __forceinline__ void ow_window(OwWarpAcc& A, const uint32_t key, const int r, const int c) {
+    const int row = 2 * (int)(key >> 5) - 6 + r, col0 = 2 * (int)(key & 31u) - 6 + 2 * c;
+    const bool valid = ((unsigned)row < 32u) && ((unsigned)col0 < 32u);
+    A.offA = valid ? row * kOwAPitch + col0 : -1;
+    A.offB = row * kOwBPitch + col0;
+    A.a0 = A.a1 = A.b = 0ull;
+}
+
+__device__ __forceinline__ void ow_flush(const OwWarpAcc& A, float2* sA, float* sB) {
     if (A.offA >= 0) {
         ow_sadd2(&sA[A.offA], A.a0);
         ow_sadd2(&sA[A.offA + 1], A.a1);
         ow_sadd2(&sB[A.offB], A.b);
     }
-    A.a0 = A.a1 = A.b = 0ull;
 }
 
-// One sample into the warp's register window.  tbx = table + 2c floats, tby = table + r floats (shared memory).
-__device__ __forceinline__ void ow_accumulate(OwWarpAcc& A, const uint4 rec, const char* tbx, const char* tby, const int r,
-                                              const int c, float2* sA, float* sB) {
+// One sample into the register window.  tbx = table + 2c floats, tby = table + r floats (shared memory).
+__device__ __forceinline__ void ow_add(OwWarpAcc& A, const uint4 rec, const char* tbx, const char* tby) {
     const uint32_t pk = rec.w;
-    const uint32_t key = pk & 0x7FFu;
-    if (key != A.key) {                                              // warp-uniform branch
-        if (A.key != 0xFFFFFFFFu) ow_flush(A, sA, sB);
-        A.key = key;
-        const int row = (int)(key >> 5) - 6 + r, col0 = 2 * (int)(key & 31u) - 6 + 2 * c;
-        const bool valid = (r < 7) && ((unsigned)row < 32u) && ((unsigned)col0 < 32u);
-        A.offA = valid ? row * kOwAPitch + col0 : -1;
-        A.offB = row * kOwBPitch + col0;
-    }
-    const float2 kx = *reinterpret_cast<const float2*>(tbx + ((pk >> 6) & 0x7FE0u));     // X * 32 bytes
-    const float ky = *reinterpret_cast<const float*>(tby + ((pk >> 16) & 0x3FE0u));      // ry * 32 bytes
+    const float2 kx = *reinterpret_cast<const float2*>(tbx + ((pk >> 5) & 0x7FE0u));      // X * 32 bytes
+    const float ky = *reinterpret_cast<const float*>(tby + ((pk >> 15) & 0x7FE0u));       // Y * 32 bytes
     const float k0 = kx.x * ky, k1 = kx.y * ky;
     const unsigned long long v = ow_pack(__uint_as_float(rec.x), __uint_as_float(rec.y));
     const float wt = __uint_as_float(rec.z);
@@ -435,7 +434,7 @@ __device__ __forceinline__ void ow_accumulate(OwWarpAcc& A, const uint4 rec, con
     A.b = ow_fma2(ow_pack(k0, k1), ow_pack(wt, wt), A.b);
 }
 
-__device__ __forceinline__ uint32_t ow_sortkey(uint32_t w) { return ((w >> 5) & 63u) * 19u + (w & 31u); }
+__device__ __forceinline__ uint32_t ow_sortkey(uint32_t w) { return ((w >> 5) & 31u) * 19u + (w & 31u); }
 
 // Launch grid: x = grid index (fastest), y = [item rows | tile rank, centre-out].  Item rows come first so that
 // the chunks of heavy tiles start before anything else.
@@ -510,12 +509,15 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     const char* tbx = reinterpret_cast<const char*>(sT + 2 * c);
     const char* tby = reinterpret_cast<const char*>(sT + r);
     OwWarpAcc A;
-    A.a0 = A.a1 = A.b = 0ull; A.key = 0xFFFFFFFFu; A.offA = -1; A.offB = 0;
 
     if (cnt <= (uint32_t)kOwDirect) {
         __syncthreads();
-        for (uint32_t i = warp; i < cnt; i += 8) ow_accumulate(A, __ldg(sorted + start + i), tbx, tby, r, c, sA, sB);
-        if (A.key != 0xFFFFFFFFu) ow_flush(A, sA, sB);
+        for (uint32_t i = warp; i < cnt; i += 8) {
+            const uint4 rec = __ldg(sorted + start + i);
+            ow_window(A, rec.w & 0x3FFu, r, c);
+            ow_add(A, rec, tbx, tby);
+            ow_flush(A, sA, sB);
+        }
         __syncthreads();
     } else {
         for (uint32_t ubase = 0; ubase < cnt; ubase += kOwUnit) {
@@ -527,8 +529,8 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             for (uint32_t i = tid; i < n; i += 256) sP[i] = (unsigned short)atomicAdd(&sH[ow_sortkey(__ldg(&src[i].w))], 1u);
             __syncthreads();
             {
-                const uint32_t h0 = sH[3 * tid], h1 = sH[3 * tid + 1], h2 = sH[3 * tid + 2];
-                const uint32_t tot = h0 + h1 + h2;
+                const uint32_t h0 = sH[2 * tid], h1 = sH[2 * tid + 1];
+                const uint32_t tot = h0 + h1;
                 uint32_t inc = tot;
                 for (int o = 1; o < 32; o <<= 1) {
                     const uint32_t t = __shfl_up_sync(kFull, inc, o);
@@ -538,7 +540,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 __syncthreads();
                 uint32_t ex = inc - tot;
                 for (int w = 0; w < warp; ++w) ex += sW[w];
-                sH[3 * tid] = ex; sH[3 * tid + 1] = ex + h0; sH[3 * tid + 2] = ex + h0 + h1;
+                sH[2 * tid] = ex; sH[2 * tid + 1] = ex + h0;
             }
             __syncthreads();
             for (uint32_t i = tid; i < n; i += 256) sP[i] = (unsigned short)(sP[i] + sH[ow_sortkey(__ldg(&src[i].w))]);
@@ -552,11 +554,17 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 __syncthreads();
                 const int m = (int)min((uint32_t)kOwSub, n - lo);
                 const int per = (m + 7) >> 3;
-                const int b = warp * per, e = min(m, b + per);
-#pragma unroll 4
-                for (int i = b; i < e; ++i) ow_accumulate(A, sR[i], tbx, tby, r, c, sA, sB);
-                if (A.key != 0xFFFFFFFFu) ow_flush(A, sA, sB);
-                A.key = 0xFFFFFFFFu;
+                const int e = min(m, (warp + 1) * per);
+                int pos = warp * per;
+                while (pos < e) {                                     // one run of equal window per pass
+                    const uint32_t key = sR[pos].w & 0x3FFu;
+                    const int rend = min(e, (int)sH[(key >> 5) * 19u + (key & 31u) + 1u] - (int)lo);
+                    ow_window(A, key, r, c);
+#pragma unroll 2
+                    for (int i = pos; i < rend; ++i) ow_add(A, sR[i], tbx, tby);
+                    ow_flush(A, sA, sB);
+                    pos = rend;
+                }
                 __syncthreads();
             }
         }
