@@ -372,52 +372,57 @@ __device__ __forceinline__ unsigned long long ow_fma2(unsigned long long a, unsi
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
 }
-// 64-bit shared-memory add of two packed floats (compare-and-swap loop; fp32 has no native shared add).
-__device__ __forceinline__ void ow_sadd2(void* p, unsigned long long v) {
-    unsigned long long* a = reinterpret_cast<unsigned long long*>(p);
-    const float2 f = ow_unpack(v);
-    unsigned long long old = *a, assumed;
-    do {
-        assumed = old;
-        const float2 c = ow_unpack(assumed);
-        old = atomicCAS(a, assumed, ow_pack(c.x + f.x, c.y + f.y));
-    } while (old != assumed);
-}
-
-constexpr int kOwAPitch = 40;     // float2 per row of the (re, im) tile: 32 cells + 8 pad
-constexpr int kOwBPitch = 40;     // floats per row of the weight tile
+constexpr int kOwPitch = 40;      // cells per row of the shared tile: 32 + 8 pad
 constexpr int kOwKeys = 512;      // 19 x 19 = 361 windows, padded to 2 per thread
-constexpr int kOwDirect = 24;     // tiles with at most this many samples skip the shared-memory sort
-constexpr int kOwUnit = 4096;     // samples counting-sorted together (in kOwSub-sized rounds)
+constexpr int kOwDirect = 32;     // tiles with at most this many samples skip the shared-memory sort
+constexpr int kOwUnit = 4096;     // samples counting-sorted together
 
 // shared-memory layout (bytes); the table region is sized by Q at launch
-constexpr int kOwOffA = 0;
-constexpr int kOwOffB = kOwOffA + 32 * kOwAPitch * 8;
-constexpr int kOwOffR = kOwOffB + 32 * kOwBPitch * 4;
-constexpr int kOwOffH = kOwOffR + kOwSub * 16;
-constexpr int kOwOffP = kOwOffH + kOwKeys * 4;
-constexpr int kOwOffT = kOwOffP + kOwUnit * 2;
+constexpr int kOwOffA = 0;                                  // int2 [32][kOwPitch]  fixed-point (re, im)
+constexpr int kOwOffB = kOwOffA + 32 * kOwPitch * 8;        // int  [32][kOwPitch]  fixed-point weight
+constexpr int kOwOffH = kOwOffB + 32 * kOwPitch * 4;        // u32  [kOwKeys]       window histogram / run starts
+constexpr int kOwOffP = kOwOffH + kOwKeys * 4;              // u16  [kOwUnit] ranks, later 8 warps x 2 x 32 records
+constexpr int kOwOffI = kOwOffP + kOwUnit * 2;              // u16  [kOwUnit] record index by sorted position
+constexpr int kOwOffT = kOwOffI + kOwUnit * 2;              // f32  [2(Q+1)][8]     two-parity table
 static size_t owner_smem_bytes(int Q) { return (size_t)kOwOffT + (size_t)2 * (Q + 1) * 8 * sizeof(float); }
+
+// The shared tile is accumulated in 32-bit FIXED POINT: integer shared-memory adds are native single instructions,
+// fp32 adds are compare-and-swap loops.  Per CTA the scale is the power of two that maps the largest possible cell
+// sum (sum of |wt*Re V|, |wt*Im V| resp. wt over the CTA's records; the kernel never exceeds 1) to < 2^30, so a
+// run's fp32 register sum is rounded once, by at most 2^-30 of that bound, when it is merged into the tile.
+struct OwScale {
+    float v, w;                    // fixed-point units per unit of value / of weight (powers of two)
+};
+
+__device__ __forceinline__ float ow_pow2_scale(float bound) {
+    // largest power of two s with bound * s <= 2^30 (bound > 0 and finite); exact exponent arithmetic
+    const int e = (int)((__float_as_uint(bound) >> 23) & 0xFFu) - 127;     // bound in [2^e, 2^(e+1))
+    const int k = min(max(29 - e, -126), 127);
+    return __uint_as_float((uint32_t)(k + 127) << 23);
+}
 
 struct OwWarpAcc {
     unsigned long long a0, a1, b;  // (re, im) of the lane's two cells; (wt, wt') of the two cells
-    int offA, offB;                // float2 / float index of the lane's first cell in sA / sB, offA = -1 outside the tile
+    int off;                       // cell index of the lane's first cell in the shared tile, -1 outside the tile
 };
 
 // Point the warp's 8 x 8 register window at window `key`; lane (r, c) holds row r, columns 2c and 2c + 1.
 __device__ __forceinline__ void ow_window(OwWarpAcc& A, const uint32_t key, const int r, const int c) {
     const int row = 2 * (int)(key >> 5) - 6 + r, col0 = 2 * (int)(key & 31u) - 6 + 2 * c;
-    const bool valid = ((unsigned)row < 32u) && ((unsigned)col0 < 32u);
-    A.offA = valid ? row * kOwAPitch + col0 : -1;
-    A.offB = row * kOwBPitch + col0;
+    A.off = (((unsigned)row < 32u) && ((unsigned)col0 < 32u)) ? row * kOwPitch + col0 : -1;
     A.a0 = A.a1 = A.b = 0ull;
 }
 
-__device__ __forceinline__ void ow_flush(const OwWarpAcc& A, float2* sA, float* sB) {
-    if (A.offA >= 0) {
-        ow_sadd2(&sA[A.offA], A.a0);
-        ow_sadd2(&sA[A.offA + 1], A.a1);
-        ow_sadd2(&sB[A.offB], A.b);
+__device__ __forceinline__ void ow_flush(const OwWarpAcc& A, const OwScale sc, int* sA, int* sB) {
+    if (A.off >= 0) {
+        const float2 c0 = ow_unpack(A.a0), c1 = ow_unpack(A.a1), w = ow_unpack(A.b);
+        int* pa = sA + 2 * A.off;
+        atomicAdd(pa + 0, __float2int_rn(c0.x * sc.v));
+        atomicAdd(pa + 1, __float2int_rn(c0.y * sc.v));
+        atomicAdd(pa + 2, __float2int_rn(c1.x * sc.v));
+        atomicAdd(pa + 3, __float2int_rn(c1.y * sc.v));
+        atomicAdd(sB + A.off, __float2int_rn(w.x * sc.w));
+        atomicAdd(sB + A.off + 1, __float2int_rn(w.y * sc.w));
     }
 }
 
@@ -436,6 +441,21 @@ __device__ __forceinline__ void ow_add(OwWarpAcc& A, const uint4 rec, const char
 
 __device__ __forceinline__ uint32_t ow_sortkey(uint32_t w) { return ((w >> 5) & 31u) * 19u + (w & 31u); }
 
+__device__ __forceinline__ float3 ow_warp_sum3(float3 a) {
+    for (int o = 16; o > 0; o >>= 1) {
+        a.x += __shfl_xor_sync(kFull, a.x, o);
+        a.y += __shfl_xor_sync(kFull, a.y, o);
+        a.z += __shfl_xor_sync(kFull, a.z, o);
+    }
+    return a;
+}
+__device__ __forceinline__ OwScale ow_scale_from(float3 s) {
+    OwScale sc;
+    sc.v = ow_pow2_scale(fmaxf(fmaxf(s.x, s.y), 1e-30f));
+    sc.w = ow_pow2_scale(fmaxf(s.z, 1e-30f));
+    return sc;
+}
+
 // Launch grid: x = grid index (fastest), y = [item rows | tile rank, centre-out].  Item rows come first so that
 // the chunks of heavy tiles start before anything else.
 template <int STORE>
@@ -447,13 +467,14 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                                                           const float* __restrict__ tt2, GridPtrs grids,
                                                           float* __restrict__ scratch, uint32_t* __restrict__ tickets) {
     extern __shared__ __align__(16) unsigned char smem[];
-    float2* sA = reinterpret_cast<float2*>(smem + kOwOffA);
-    float* sB = reinterpret_cast<float*>(smem + kOwOffB);
-    uint4* sR = reinterpret_cast<uint4*>(smem + kOwOffR);
+    int* sA = reinterpret_cast<int*>(smem + kOwOffA);
+    int* sB = reinterpret_cast<int*>(smem + kOwOffB);
     uint32_t* sH = reinterpret_cast<uint32_t*>(smem + kOwOffH);
     unsigned short* sP = reinterpret_cast<unsigned short*>(smem + kOwOffP);
+    unsigned short* sI = reinterpret_cast<unsigned short*>(smem + kOwOffI);
     float* sT = reinterpret_cast<float*>(smem + kOwOffT);
     __shared__ uint32_t sW[8];
+    __shared__ float sSum[8][3];
     __shared__ int sLast;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -498,9 +519,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         return;
     }
 
-    {   // zero the tile accumulators, stage the two-parity table
-        float4* za = reinterpret_cast<float4*>(smem + kOwOffA);
-        for (int i = tid; i < (kOwOffR - kOwOffA) / 16; i += 256) za[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    {   // zero the fixed-point tile, stage the two-parity table
+        int4* za = reinterpret_cast<int4*>(smem + kOwOffA);
+        for (int i = tid; i < (kOwOffH - kOwOffA) / 16; i += 256) za[i] = make_int4(0, 0, 0, 0);
         const float4* src = reinterpret_cast<const float4*>(tt2);
         float4* dst = reinterpret_cast<float4*>(sT);
         for (int i = tid; i < 2 * (g.Q + 1) * 2; i += 256) dst[i] = __ldg(src + i);
@@ -508,26 +529,57 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     const int r = lane >> 2, c = lane & 3;
     const char* tbx = reinterpret_cast<const char*>(sT + 2 * c);
     const char* tby = reinterpret_cast<const char*>(sT + r);
+    const uint4* __restrict__ recs = sorted + start;
     OwWarpAcc A;
+    OwScale sc;
 
     if (cnt <= (uint32_t)kOwDirect) {
+        // every warp derives the scale from all (<= 32) records, then takes every 8th record as a run of one
+        float3 s = make_float3(0.f, 0.f, 0.f);
+        if ((uint32_t)lane < cnt) {
+            const uint4 q = __ldg(recs + lane);
+            s = make_float3(fabsf(__uint_as_float(q.x)), fabsf(__uint_as_float(q.y)), __uint_as_float(q.z));
+        }
+        sc = ow_scale_from(ow_warp_sum3(s));
         __syncthreads();
         for (uint32_t i = warp; i < cnt; i += 8) {
-            const uint4 rec = __ldg(sorted + start + i);
+            const uint4 rec = __ldg(recs + i);
             ow_window(A, rec.w & 0x3FFu, r, c);
             ow_add(A, rec, tbx, tby);
-            ow_flush(A, sA, sB);
+            ow_flush(A, sc, sA, sB);
         }
         __syncthreads();
     } else {
+        float3 s = make_float3(0.f, 0.f, 0.f);
+        if (cnt > (uint32_t)kOwUnit) {                                // several units: bound over all of them first
+            for (uint32_t i = tid; i < cnt; i += 256) {
+                const uint4 q = __ldg(recs + i);
+                s.x += fabsf(__uint_as_float(q.x)); s.y += fabsf(__uint_as_float(q.y)); s.z += __uint_as_float(q.z);
+            }
+        }
         for (uint32_t ubase = 0; ubase < cnt; ubase += kOwUnit) {
             const uint32_t n = min((uint32_t)kOwUnit, cnt - ubase);
-            const uint4* __restrict__ src = sorted + start + ubase;
+            const uint4* __restrict__ src = recs + ubase;
             for (int i = tid; i < kOwKeys; i += 256) sH[i] = 0;
             __syncthreads();
-            // (1) counting sort of the unit by window (row-major): sorted position of every record
-            for (uint32_t i = tid; i < n; i += 256) sP[i] = (unsigned short)atomicAdd(&sH[ow_sortkey(__ldg(&src[i].w))], 1u);
+            // (1) counting sort of the unit by window (row-major): rank of every record inside its window
+            for (uint32_t i = tid; i < n; i += 256) {
+                const uint4 q = __ldg(src + i);
+                sP[i] = (unsigned short)atomicAdd(&sH[ow_sortkey(q.w)], 1u);
+                if (cnt <= (uint32_t)kOwUnit) {
+                    s.x += fabsf(__uint_as_float(q.x)); s.y += fabsf(__uint_as_float(q.y)); s.z += __uint_as_float(q.z);
+                }
+            }
+            if (ubase == 0) {
+                const float3 t = ow_warp_sum3(s);
+                if (lane == 0) { sSum[warp][0] = t.x; sSum[warp][1] = t.y; sSum[warp][2] = t.z; }
+            }
             __syncthreads();
+            if (ubase == 0) {
+                float3 t = make_float3(0.f, 0.f, 0.f);
+                for (int w = 0; w < 8; ++w) { t.x += sSum[w][0]; t.y += sSum[w][1]; t.z += sSum[w][2]; }
+                sc = ow_scale_from(t);
+            }
             {
                 const uint32_t h0 = sH[2 * tid], h1 = sH[2 * tid + 1];
                 const uint32_t tot = h0 + h1;
@@ -543,62 +595,76 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 sH[2 * tid] = ex; sH[2 * tid + 1] = ex + h0;
             }
             __syncthreads();
-            for (uint32_t i = tid; i < n; i += 256) sP[i] = (unsigned short)(sP[i] + sH[ow_sortkey(__ldg(&src[i].w))]);
+            for (uint32_t i = tid; i < n; i += 256) sI[sH[ow_sortkey(__ldg(&src[i].w))] + sP[i]] = (unsigned short)i;
             __syncthreads();
-            // (2) rounds of kOwSub sorted records: stage, then every warp walks an equal slice with the window in registers
-            for (uint32_t lo = 0; lo < n; lo += kOwSub) {
-                for (uint32_t i = tid; i < n; i += 256) {
-                    const uint32_t p = (uint32_t)sP[i] - lo;
-                    if (p < (uint32_t)kOwSub) sR[p] = __ldg(src + i);
-                }
-                __syncthreads();
-                const int m = (int)min((uint32_t)kOwSub, n - lo);
-                const int per = (m + 7) >> 3;
-                const int e = min(m, (warp + 1) * per);
-                int pos = warp * per;
-                while (pos < e) {                                     // one run of equal window per pass
-                    const uint32_t key = sR[pos].w & 0x3FFu;
-                    const int rend = min(e, (int)sH[(key >> 5) * 19u + (key & 31u) + 1u] - (int)lo);
-                    ow_window(A, key, r, c);
+            // (2) every warp streams an equal share of the sorted order through its private 2 x 32-record buffer
+            //     (gather loads one batch ahead); runs of equal window stay in registers across batches
+            {
+                uint4* wb = reinterpret_cast<uint4*>(smem + kOwOffP) + warp * 64;
+                const int per = ((int)n + 7) >> 3;
+                const int e = min((int)n, (warp + 1) * per);
+                int p = warp * per;
+                uint4 nxt = make_uint4(0, 0, 0, 0);
+                if (p + lane < e) nxt = __ldg(src + sI[p + lane]);
+                uint32_t cur = 0xFFFFFFFFu;
+                int buf = 0;
+                while (p < e) {
+                    const int m = min(32, e - p);
+                    wb[buf * 32 + lane] = nxt;
+                    __syncwarp();
+                    if (p + 32 + lane < e) nxt = __ldg(src + sI[p + 32 + lane]);
+                    const uint4* __restrict__ q = wb + buf * 32;
+                    int j = 0;
+                    while (j < m) {
+                        const uint32_t key = q[j].w & 0x3FFu;
+                        if (key != cur) {
+                            if (cur != 0xFFFFFFFFu) ow_flush(A, sc, sA, sB);
+                            ow_window(A, key, r, c);
+                            cur = key;
+                        }
+                        const int rend = min(m, (int)sH[(key >> 5) * 19u + (key & 31u) + 1u] - p);
 #pragma unroll 2
-                    for (int i = pos; i < rend; ++i) ow_add(A, sR[i], tbx, tby);
-                    ow_flush(A, sA, sB);
-                    pos = rend;
+                        for (; j < rend; ++j) ow_add(A, q[j], tbx, tby);
+                    }
+                    buf ^= 1;
+                    p += 32;
                 }
-                __syncthreads();
+                if (cur != 0xFFFFFFFFu) ow_flush(A, sc, sA, sB);
             }
+            __syncthreads();
         }
     }
 
-    // (3) output
-    if (!heavy) {
-        for (int i = tid; i < 32 * 16; i += 256) {
-            const int row = i >> 4, c2 = i & 15, gx = x0 + 2 * c2, gy = y0 + row;
-            if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
-                float4 v = *reinterpret_cast<const float4*>(&sA[row * kOwAPitch + 2 * c2]);
-                float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
-                if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
-                *dst = v;
-            }
+    // (3) output: fixed point -> fp32 (the scales are powers of two)
+    const float iv = 1.0f / sc.v, iw = 1.0f / sc.w;
+    float4* part = nullptr;
+    if (heavy) part = reinterpret_cast<float4*>(scratch + (size_t)(first_slot + chunk) * kOwTileFloats);
+    for (int i = tid; i < 32 * 16; i += 256) {
+        const int row = i >> 4, c2 = i & 15, gx = x0 + 2 * c2, gy = y0 + row;
+        const int4 a = *reinterpret_cast<const int4*>(sA + 2 * (row * kOwPitch + 2 * c2));
+        float4 v = make_float4((float)a.x * iv, (float)a.y * iv, (float)a.z * iv, (float)a.w * iv);
+        if (heavy) {
+            __stcg(part + i, v);
+        } else if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+            float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
+            if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+            *dst = v;
         }
-        {
-            const int row = tid >> 3, c4 = tid & 7, gx = x0 + 4 * c4, gy = y0 + row;
-            if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
-                float4 v = *reinterpret_cast<const float4*>(&sB[row * kOwBPitch + 4 * c4]);
-                float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
-                if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
-                *dst = v;
-            }
-        }
-        return;
     }
-    // heavy tile: publish this chunk's partial tile; the last chunk to arrive adds them up in chunk order
     {
-        float4* part = reinterpret_cast<float4*>(scratch + (size_t)(first_slot + chunk) * kOwTileFloats);
-        for (int i = tid; i < 32 * 16; i += 256)
-            __stcg(part + i, *reinterpret_cast<const float4*>(&sA[(i >> 4) * kOwAPitch + 2 * (i & 15)]));
-        __stcg(part + 512 + tid, *reinterpret_cast<const float4*>(&sB[(tid >> 3) * kOwBPitch + 4 * (tid & 7)]));
+        const int row = tid >> 3, c4 = tid & 7, gx = x0 + 4 * c4, gy = y0 + row;
+        const int4 a = *reinterpret_cast<const int4*>(sB + row * kOwPitch + 4 * c4);
+        float4 v = make_float4((float)a.x * iw, (float)a.y * iw, (float)a.z * iw, (float)a.w * iw);
+        if (heavy) {
+            __stcg(part + 512 + tid, v);
+        } else if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+            float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
+            if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+            *dst = v;
+        }
     }
+    if (!heavy) return;
+    // heavy tile: the last chunk to arrive adds the published partial tiles up in chunk order
     __threadfence();
     __syncthreads();
     if (tid == 0) {
