@@ -57,6 +57,7 @@ struct muser_imager {
     uint4* ow_sorted = nullptr;
     uint32_t *ow_count = nullptr, *ow_offset = nullptr;
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
+    bool h_packed = false;                  // H already holds G + i*alpha*Gw (written by the owner gridder in store mode)
     cufftHandle plan = 0;
     bool plan_ok = false, fft_valid = false;
     cudaStream_t last_stream = nullptr;
@@ -151,6 +152,7 @@ int alloc_grids(muser_imager* h) {
     CU(h, cudaMemset(h->stats_d, 0, sizeof(Stats)));
     h->fft_valid = false;
     h->zero_pending = false;
+    h->h_packed = false;
     return MUSER_OK;
 }
 
@@ -355,11 +357,12 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
             CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_count, h->ow_items, h->nitems_d, max_items,
-                                    item_size, h->order_d, h->ttp_d, gp, h->ow_scratch, h->ow_tickets,
-                                    h->zero_pending ? 1 : 0, s));
+                                    item_size, h->order_d, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->H,
+                                    h->stats_d, h->zero_pending ? 1 : 0, s));
         }
+        h->n_launches += 4;                                           // count, scan, scatter, grid
+        h->h_packed = h->zero_pending;                                // store mode also wrote the FFT input H
         h->zero_pending = false;                                      // store mode wrote every tile of every grid
-        h->n_launches += 4;
         return MUSER_OK;
     }
     const bool tiled = strat == MUSER_STRATEGY_TILED;
@@ -368,6 +371,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     if ((rc = flush_zero(h, s))) return rc;
     h->last_stream = s;
     h->fft_valid = false;
+    h->h_packed = false;
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
         CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
@@ -402,11 +406,12 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         h->plan_ok = true;
     }
     if (!h->fft_valid) {
-        {
+        if (!h->h_packed) {
             StageScope sc(h, MUSER_STAGE_PACK, s);
             CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, h->stats_d, s));
             h->n_launches += 1;
         }
+        h->h_packed = false;                                          // the in-place transform consumes H
         {
             StageScope sc(h, MUSER_STAGE_FFT, s);
             cufftResult r = cufftSetStream(h->plan, s);
@@ -428,6 +433,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
 int reset_impl(muser_imager* h, cudaStream_t s) {
     h->last_stream = s;
     h->fft_valid = false;
+    h->h_packed = false;
     // The grids are zeroed lazily: the owner-tile gridder writes every tile of every grid with plain stores, so a
     // reset followed by muser_grid needs no memset at all; any other consumer calls flush_zero first.
     h->zero_pending = true;

@@ -102,6 +102,6 @@ cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
                               const OwItem* items, const uint32_t* nitems, uint32_t max_items, uint32_t item_size,
                               const uint32_t* order, const float* tt2, GridPtrs grids, float* scratch,
-                              uint32_t* tickets, int store_mode, cudaStream_t s);
+                              uint32_t* tickets, float2* H, Stats* stats, int store_mode, cudaStream_t s);
 
 }  // namespace muser

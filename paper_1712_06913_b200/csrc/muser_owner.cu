@@ -465,7 +465,8 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                                                           const uint32_t* __restrict__ nitems, const uint32_t item_rows,
                                                           const uint32_t item_size, const uint32_t* __restrict__ order,
                                                           const float* __restrict__ tt2, GridPtrs grids,
-                                                          float* __restrict__ scratch, uint32_t* __restrict__ tickets) {
+                                                          float* __restrict__ scratch, uint32_t* __restrict__ tickets,
+                                                          float2* __restrict__ H, Stats* __restrict__ stats) {
     extern __shared__ __align__(16) unsigned char smem[];
     int* sA = reinterpret_cast<int*>(smem + kOwOffA);
     int* sB = reinterpret_cast<int*>(smem + kOwOffB);
@@ -478,6 +479,15 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     __shared__ int sLast;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // STORE mode also writes H = G + i*alpha*Gw, the FFT input (what k_pack would produce): alpha from the sums that
+    // k_owner_count accumulated earlier on the stream
+    float al = 1.0f;
+    if (STORE) {
+        const double v2 = stats->sum_val2, w2 = stats->sum_wt2;
+        if (v2 > 0.0 && w2 > 0.0) al = exp2f(rintf(0.5f * log2f((float)(v2 / w2))));
+        al = fminf(fmaxf(al, 9.5367431640625e-07f), 1048576.0f);
+        if (blockIdx.x == 0 && blockIdx.y == 0 && tid == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
+    }
     uint32_t gi, tile, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
     const bool heavy = blockIdx.y < item_rows;
     if (heavy) {
@@ -502,18 +512,22 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     const int x0 = tx * kTile - kTile / 2, y0 = ty * kTile - kTile / 2;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
     float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
+    float2* __restrict__ Ht = H + (size_t)gi * g.ny * g.nx;
 
     if (cnt == 0) {
         if (STORE) {
+            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
             for (int i = tid; i < 32 * 16; i += 256) {
                 const int row = i >> 4, gx = x0 + 2 * (i & 15), gy = y0 + row;
-                if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny)
-                    *reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx) = make_float4(0.f, 0.f, 0.f, 0.f);
+                if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+                    *reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx) = z;
+                    *reinterpret_cast<float4*>(Ht + (size_t)gy * g.nx + gx) = z;
+                }
             }
             {
                 const int row = tid >> 3, gx = x0 + 4 * (tid & 7), gy = y0 + row;
                 if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny)
-                    *reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx) = make_float4(0.f, 0.f, 0.f, 0.f);
+                    *reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx) = z;
             }
         }
         return;
@@ -649,6 +663,12 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
             if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
             *dst = v;
+            if (STORE) {
+                const int2 wq = *reinterpret_cast<const int2*>(sB + row * kOwPitch + 2 * c2);
+                const float sw = iw * al;
+                *reinterpret_cast<float4*>(Ht + (size_t)gy * g.nx + gx) =
+                    make_float4(v.x, v.y + (float)wq.x * sw, v.z, v.w + (float)wq.y * sw);
+            }
         }
     }
     {
@@ -675,19 +695,38 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     if (!sLast) return;
     __threadfence();
     const float4* parts = reinterpret_cast<const float4*>(scratch + (size_t)first_slot * kOwTileFloats);
-    for (int i = tid; i < 32 * 16 + 256; i += 256) {
+    float* sWsum = reinterpret_cast<float*>(smem + kOwOffB);          // summed weight tile, dense [32][32], for H
+    for (int i = 512 + tid; i < 32 * 16 + 256; i += 256) {            // weights first
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
         for (uint32_t q = 0; q < nchunks; ++q) {
             const float4 p = __ldcg(parts + (size_t)q * (kOwTileFloats / 4) + i);
             v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
         }
-        float4* dst;
-        int gx, gy;
-        if (i < 512) { gx = x0 + 2 * (i & 15); gy = y0 + (i >> 4); dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx); }
-        else { const int j = i - 512; gx = x0 + 4 * (j & 7); gy = y0 + (j >> 3); dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx); }
+        const int j = i - 512, gx = x0 + 4 * (j & 7), gy = y0 + (j >> 3);
+        if (STORE) *reinterpret_cast<float4*>(sWsum + 4 * j) = v;
         if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+            float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
             if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
             *dst = v;
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < 32 * 16; i += 256) {
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (uint32_t q = 0; q < nchunks; ++q) {
+            const float4 p = __ldcg(parts + (size_t)q * (kOwTileFloats / 4) + i);
+            v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
+        }
+        const int gx = x0 + 2 * (i & 15), gy = y0 + (i >> 4);
+        if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
+            float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
+            if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+            *dst = v;
+            if (STORE) {
+                const float2 wq = *reinterpret_cast<const float2*>(sWsum + 2 * i);
+                *reinterpret_cast<float4*>(Ht + (size_t)gy * g.nx + gx) =
+                    make_float4(v.x, v.y + al * wq.x, v.z, v.w + al * wq.y);
+            }
         }
     }
     if (tid == 0) tickets[first_slot] = 0;
@@ -727,16 +766,16 @@ cudaError_t owner_kernel_setup(int max_smem_bytes) {
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
                               const OwItem* items, const uint32_t* nitems, uint32_t max_items, uint32_t item_size,
                               const uint32_t* order, const float* tt2, GridPtrs grids, float* scratch,
-                              uint32_t* tickets, int store_mode, cudaStream_t s) {
+                              uint32_t* tickets, float2* H, Stats* stats, int store_mode, cudaStream_t s) {
     const uint32_t item_rows = (max_items + (uint32_t)g.ngrids - 1) / (uint32_t)g.ngrids;
     const dim3 blocks((unsigned)g.ngrids, item_rows + (unsigned)g.ntiles);
     const size_t smem = owner_smem_bytes(g.Q);
     if (store_mode)
         k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, item_rows, item_size,
-                                                     order, tt2, grids, scratch, tickets);
+                                                     order, tt2, grids, scratch, tickets, H, stats);
     else
         k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, item_rows, item_size,
-                                                     order, tt2, grids, scratch, tickets);
+                                                     order, tt2, grids, scratch, tickets, H, stats);
     return cudaGetLastError();
 }
 
