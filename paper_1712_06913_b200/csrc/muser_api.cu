@@ -55,7 +55,7 @@ struct muser_imager {
     float* ow_scratch = nullptr;
     size_t ow_items_cap = 0, ow_sorted_cap = 0, ow_bins_cap = 0;
     uint4* ow_sorted = nullptr;
-    uint32_t *ow_count = nullptr, *ow_offset = nullptr;
+    uint32_t *ow_count = nullptr, *ow_offset = nullptr, *ow_work = nullptr, *ow_ctl = nullptr;
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     bool h_packed = false;                  // H already holds G + i*alpha*Gw (written by the owner gridder in store mode)
     cufftHandle plan = 0;
@@ -116,8 +116,8 @@ void free_grids(muser_imager* h) {
 void free_bins(muser_imager* h) {
     cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
     h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
-    cudaFree(h->ow_count); cudaFree(h->ow_offset);
-    h->ow_count = h->ow_offset = nullptr; h->ow_bins_cap = 0;
+    cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work);
+    h->ow_count = h->ow_offset = h->ow_work = nullptr; h->ow_bins_cap = 0;
 }
 
 int rebuild_geom(muser_imager* h) {
@@ -308,10 +308,12 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
     }
     const size_t nb = ((size_t)h->geom.nbins + 8) & ~(size_t)3;
     if (nb > h->ow_bins_cap) {
-        cudaFree(h->ow_count); cudaFree(h->ow_offset);
-        h->ow_count = h->ow_offset = nullptr; h->ow_bins_cap = 0;
+        cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work);
+        h->ow_count = h->ow_offset = h->ow_work = nullptr; h->ow_bins_cap = 0;
         CU(h, cudaMalloc(&h->ow_count, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_offset, nb * sizeof(uint32_t)));
+        CU(h, cudaMalloc(&h->ow_work, nb * sizeof(uint32_t)));
+        if (!h->ow_ctl) CU(h, cudaMalloc(&h->ow_ctl, 4 * sizeof(uint32_t)));
         CU(h, cudaMemset(h->ow_count, 0, nb * sizeof(uint32_t)));     // every later use leaves it zeroed
         h->ow_bins_cap = nb;
     }
@@ -344,23 +346,24 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         uint32_t max_items = 0;
         int rc = ensure_owner_scratch(h, nvis, item_size, &max_items);
         if (rc) return rc;
-        if ((unsigned long long)max_items / g.ngrids + g.ntiles + 1 > 65535ull) return fail(h, MUSER_EUNSUPPORTED, "too many tiles for one launch");
+        if (g.nty > 65535 || g.ntx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
         h->last_stream = s;
         h->fft_valid = false;
         {
             StageScope sc(h, MUSER_STAGE_BIN, s);
             CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, s));
-            CU(h, launch_owner_scan(g, h->ow_count, h->ow_offset, h->ow_items, h->nitems_d, item_size, s));
+            CU(h, launch_owner_scan(g, h->ow_count, h->ow_offset, h->ow_items, h->nitems_d, item_size, h->ow_work,
+                                    h->ow_ctl, s));
             CU(h, launch_owner_scatter(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_count,
                                        h->ow_sorted, s));
         }
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
-            CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_count, h->ow_items, h->nitems_d, max_items,
-                                    item_size, h->order_d, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->H,
-                                    h->stats_d, h->zero_pending ? 1 : 0, s));
+            CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_count, h->ow_items, h->nitems_d, h->ow_work,
+                                    h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->H, h->stats_d,
+                                    h->zero_pending ? 1 : 0, h->num_sms, s));
         }
-        h->n_launches += 4;                                           // count, scan, scatter, grid
+        h->n_launches += h->zero_pending ? 5 : 4;                     // count, scan, scatter, (fill,) grid
         h->h_packed = h->zero_pending;                                // store mode also wrote the FFT input H
         h->zero_pending = false;                                      // store mode wrote every tile of every grid
         return MUSER_OK;
@@ -500,7 +503,7 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
     cudaFree(h->ttp_d); cudaFree(h->order_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
-    cudaFree(h->ow_sorted);
+    cudaFree(h->ow_sorted); cudaFree(h->ow_ctl);
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete h;

@@ -202,11 +202,12 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
 // heavy bins, and re-zeroes the histogram (k_owner_scatter reuses it as its cursor).
 __global__ void __launch_bounds__(1024) k_owner_scan(const Geom g, uint32_t* __restrict__ bin_count,
                                                      uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
-                                                     uint32_t* __restrict__ nitems, const uint32_t item_size) {
-    __shared__ uint32_t s_wsum[2][32];
-    __shared__ uint32_t s_carry[2];
+                                                     uint32_t* __restrict__ nitems, const uint32_t item_size,
+                                                     uint32_t* __restrict__ work, uint32_t* __restrict__ ctl) {
+    __shared__ uint32_t s_wsum[3][32];
+    __shared__ uint32_t s_carry[3];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) { s_carry[0] = 0; s_carry[1] = 0; }
+    if (threadIdx.x == 0) { s_carry[0] = 0; s_carry[1] = 0; s_carry[2] = 0; }
     __syncthreads();
     for (uint32_t base = 0; base < g.nbins; base += 4096) {
         const uint32_t b0 = base + 4 * threadIdx.x;
@@ -216,35 +217,37 @@ __global__ void __launch_bounds__(1024) k_owner_scan(const Geom g, uint32_t* __r
             c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
             if (v.x | v.y | v.z | v.w) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);
         }
-        uint32_t tc = 0, tm = 0;
+        uint32_t tc = 0, tm = 0, tl = 0;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             m[j] = c[j] > item_size ? (c[j] + item_size - 1) / item_size : 0u;
-            tc += c[j]; tm += m[j];
+            tc += c[j]; tm += m[j]; tl += (c[j] != 0u && m[j] == 0u);
         }
-        uint32_t ic = tc, im = tm;                                      // inclusive warp scans
+        uint32_t ic = tc, im = tm, il = tl;                             // inclusive warp scans
         for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t xc = __shfl_up_sync(kFull, ic, o), xm = __shfl_up_sync(kFull, im, o);
-            if (lane >= o) { ic += xc; im += xm; }
+            const uint32_t xc = __shfl_up_sync(kFull, ic, o), xm = __shfl_up_sync(kFull, im, o), xl = __shfl_up_sync(kFull, il, o);
+            if (lane >= o) { ic += xc; im += xm; il += xl; }
         }
-        if (lane == 31) { s_wsum[0][warp] = ic; s_wsum[1][warp] = im; }
+        if (lane == 31) { s_wsum[0][warp] = ic; s_wsum[1][warp] = im; s_wsum[2][warp] = il; }
         __syncthreads();
         if (warp == 0) {
-            uint32_t wc = s_wsum[0][lane], wm = s_wsum[1][lane];
+            uint32_t wc = s_wsum[0][lane], wm = s_wsum[1][lane], wl = s_wsum[2][lane];
             for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t xc = __shfl_up_sync(kFull, wc, o), xm = __shfl_up_sync(kFull, wm, o);
-                if (lane >= o) { wc += xc; wm += xm; }
+                const uint32_t xc = __shfl_up_sync(kFull, wc, o), xm = __shfl_up_sync(kFull, wm, o), xl = __shfl_up_sync(kFull, wl, o);
+                if (lane >= o) { wc += xc; wm += xm; wl += xl; }
             }
-            s_wsum[0][lane] = wc; s_wsum[1][lane] = wm;
+            s_wsum[0][lane] = wc; s_wsum[1][lane] = wm; s_wsum[2][lane] = wl;
         }
         __syncthreads();
         uint32_t off = s_carry[0] + (warp ? s_wsum[0][warp - 1] : 0) + ic - tc;
         uint32_t slot = s_carry[1] + (warp ? s_wsum[1][warp - 1] : 0) + im - tm;
+        uint32_t wpos = s_carry[2] + (warp ? s_wsum[2][warp - 1] : 0) + il - tl;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const uint32_t b = b0 + j;
             if (b < g.nbins) {
                 bin_offset[b] = off;
+                if (c[j] != 0u && m[j] == 0u) work[wpos++] = b;        // light non-empty tile: one work unit
                 for (uint32_t q = 0; q < m[j]; ++q) {
                     OwItem it;
                     it.bin = b; it.start = off + q * item_size; it.count = min(item_size, c[j] - q * item_size);
@@ -255,10 +258,10 @@ __global__ void __launch_bounds__(1024) k_owner_scan(const Geom g, uint32_t* __r
             off += c[j]; slot += m[j];
         }
         __syncthreads();
-        if (threadIdx.x == 1023) { s_carry[0] = off; s_carry[1] = slot; }
+        if (threadIdx.x == 1023) { s_carry[0] = off; s_carry[1] = slot; s_carry[2] = wpos; }
         __syncthreads();
     }
-    if (threadIdx.x == 0) { bin_offset[g.nbins] = s_carry[0]; *nitems = s_carry[1]; }
+    if (threadIdx.x == 0) { bin_offset[g.nbins] = s_carry[0]; *nitems = s_carry[1]; ctl[0] = s_carry[2]; ctl[1] = 0; }
 }
 
 // ------------------------------------------------------------------------------------------------- O3 scatter
@@ -387,19 +390,13 @@ constexpr int kOwOffT = kOwOffI + kOwUnit * 2;              // f32  [2(Q+1)][8] 
 static size_t owner_smem_bytes(int Q) { return (size_t)kOwOffT + (size_t)2 * (Q + 1) * 8 * sizeof(float); }
 
 // The shared tile is accumulated in 32-bit FIXED POINT: integer shared-memory adds are native single instructions,
-// fp32 adds are compare-and-swap loops.  Per CTA the scale is the power of two that maps the largest possible cell
-// sum (sum of |wt*Re V|, |wt*Im V| resp. wt over the CTA's records; the kernel never exceeds 1) to < 2^30, so a
-// run's fp32 register sum is rounded once, by at most 2^-30 of that bound, when it is merged into the tile.
+// fp32 adds are compare-and-swap loops.  Per work unit the scale maps the largest possible cell sum (sum of
+// |wt*Re V|, |wt*Im V| resp. wt over the unit's records; the kernel never exceeds 1) to 0.98 * 2^31, so a run's
+// fp32 register sum is rounded once, by at most 2^-32 of that bound, when it is merged into the tile (the 2 %
+// margin covers the fp32 rounding of the bound itself and the half-unit roundings of up to 4096 merges).
 struct OwScale {
-    float v, w;                    // fixed-point units per unit of value / of weight (powers of two)
+    float v, w;                    // fixed-point units per unit of value / of weight
 };
-
-__device__ __forceinline__ float ow_pow2_scale(float bound) {
-    // largest power of two s with bound * s <= 2^30 (bound > 0 and finite); exact exponent arithmetic
-    const int e = (int)((__float_as_uint(bound) >> 23) & 0xFFu) - 127;     // bound in [2^e, 2^(e+1))
-    const int k = min(max(29 - e, -126), 127);
-    return __uint_as_float((uint32_t)(k + 127) << 23);
-}
 
 struct OwWarpAcc {
     unsigned long long a0, a1, b;  // (re, im) of the lane's two cells; (wt, wt') of the two cells
@@ -451,19 +448,20 @@ __device__ __forceinline__ float3 ow_warp_sum3(float3 a) {
 }
 __device__ __forceinline__ OwScale ow_scale_from(float3 s) {
     OwScale sc;
-    sc.v = ow_pow2_scale(fmaxf(fmaxf(s.x, s.y), 1e-30f));
-    sc.w = ow_pow2_scale(fmaxf(s.z, 1e-30f));
+    sc.v = 2104533975.0f / fmaxf(fmaxf(s.x, s.y), 1e-30f);           // 0.98 * 2^31
+    sc.w = 2104533975.0f / fmaxf(s.z, 1e-30f);
     return sc;
 }
 
-// Launch grid: x = grid index (fastest), y = [item rows | tile rank, centre-out].  Item rows come first so that
-// the chunks of heavy tiles start before anything else.
+// Persistent kernel: 4 CTAs per SM pull work units from a device-side counter.  Units [0, nitems) are the chunk items
+// of heavy tiles (started first), units [nitems, nitems + nlight) the light non-empty tiles listed by k_owner_scan.
+// Empty tiles are zeroed by k_owner_fill (STORE mode) and never reach this kernel.
 template <int STORE>
 __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
                                                           const uint32_t* __restrict__ bin_offset,
                                                           uint32_t* __restrict__ cursor, const OwItem* __restrict__ items,
-                                                          const uint32_t* __restrict__ nitems, const uint32_t item_rows,
-                                                          const uint32_t item_size, const uint32_t* __restrict__ order,
+                                                          const uint32_t* __restrict__ nitems,
+                                                          const uint32_t* __restrict__ work, uint32_t* __restrict__ ctl,
                                                           const float* __restrict__ tt2, GridPtrs grids,
                                                           float* __restrict__ scratch, uint32_t* __restrict__ tickets,
                                                           float2* __restrict__ H, Stats* __restrict__ stats) {
@@ -477,6 +475,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     __shared__ uint32_t sW[8];
     __shared__ float sSum[8][3];
     __shared__ int sLast;
+    __shared__ uint32_t sWork;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // STORE mode also writes H = G + i*alpha*Gw, the FFT input (what k_pack would produce): alpha from the sums that
@@ -486,56 +485,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         const double v2 = stats->sum_val2, w2 = stats->sum_wt2;
         if (v2 > 0.0 && w2 > 0.0) al = exp2f(rintf(0.5f * log2f((float)(v2 / w2))));
         al = fminf(fmaxf(al, 9.5367431640625e-07f), 1048576.0f);
-        if (blockIdx.x == 0 && blockIdx.y == 0 && tid == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
+        if (blockIdx.x == 0 && tid == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
     }
-    uint32_t gi, tile, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
-    const bool heavy = blockIdx.y < item_rows;
-    if (heavy) {
-        const uint32_t idx = blockIdx.y * gridDim.x + blockIdx.x;
-        if (idx >= *nitems) return;
-        const OwItem it = items[idx];
-        gi = it.bin / (uint32_t)g.ntiles; tile = it.bin - gi * (uint32_t)g.ntiles;
-        tile = ((tile / (uint32_t)g.ntx) << 16) | (tile % (uint32_t)g.ntx);   // packed (ty << 16 | tx)
-        start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
-        if (chunk == 0 && tid == 0) cursor[it.bin] = 0;
-    } else {
-        gi = blockIdx.x;
-        const uint32_t t = order[blockIdx.y - item_rows];             // packed (ty << 16 | tx), centre-out
-        const uint32_t bin = gi * (uint32_t)g.ntiles + (t >> 16) * (uint32_t)g.ntx + (t & 0xFFFFu);
-        tile = t;
-        start = bin_offset[bin];
-        cnt = bin_offset[bin + 1] - start;
-        if (cnt > item_size) return;                                  // heavy tile: its chunk items do the work
-        if (cnt && tid == 0) cursor[bin] = 0;
-    }
-    const int ty = (int)(tile >> 16), tx = (int)(tile & 0xFFFFu);
-    const int x0 = tx * kTile - kTile / 2, y0 = ty * kTile - kTile / 2;
-    float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
-    float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
-    float2* __restrict__ Ht = H + (size_t)gi * g.ny * g.nx;
-
-    if (cnt == 0) {
-        if (STORE) {
-            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-            for (int i = tid; i < 32 * 16; i += 256) {
-                const int row = i >> 4, gx = x0 + 2 * (i & 15), gy = y0 + row;
-                if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
-                    *reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx) = z;
-                    *reinterpret_cast<float4*>(Ht + (size_t)gy * g.nx + gx) = z;
-                }
-            }
-            {
-                const int row = tid >> 3, gx = x0 + 4 * (tid & 7), gy = y0 + row;
-                if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny)
-                    *reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx) = z;
-            }
-        }
-        return;
-    }
-
-    {   // zero the fixed-point tile, stage the two-parity table
-        int4* za = reinterpret_cast<int4*>(smem + kOwOffA);
-        for (int i = tid; i < (kOwOffH - kOwOffA) / 16; i += 256) za[i] = make_int4(0, 0, 0, 0);
+    {   // stage the two-parity table once per CTA
         const float4* src = reinterpret_cast<const float4*>(tt2);
         float4* dst = reinterpret_cast<float4*>(sT);
         for (int i = tid; i < 2 * (g.Q + 1) * 2; i += 256) dst[i] = __ldg(src + i);
@@ -543,6 +495,36 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     const int r = lane >> 2, c = lane & 3;
     const char* tbx = reinterpret_cast<const char*>(sT + 2 * c);
     const char* tby = reinterpret_cast<const char*>(sT + r);
+    const uint32_t n_items = *nitems, n_work = n_items + ctl[0];
+
+  for (;;) {
+    __syncthreads();                                                  // the previous unit is done with the shared tile
+    if (tid == 0) sWork = atomicAdd(&ctl[1], 1u);
+    __syncthreads();
+    const uint32_t wi = sWork;
+    if (wi >= n_work) break;
+    uint32_t bin, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
+    const bool heavy = wi < n_items;
+    if (heavy) {
+        const OwItem it = items[wi];
+        bin = it.bin; start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
+        if (chunk == 0 && tid == 0) cursor[bin] = 0;
+    } else {
+        bin = work[wi - n_items];
+        start = bin_offset[bin];
+        cnt = bin_offset[bin + 1] - start;
+        if (tid == 0) cursor[bin] = 0;
+    }
+    const uint32_t gi = bin / (uint32_t)g.ntiles, tile = bin - gi * (uint32_t)g.ntiles;
+    const int ty = (int)(tile / (uint32_t)g.ntx), tx = (int)(tile - (uint32_t)ty * (uint32_t)g.ntx);
+    const int x0 = tx * kTile - kTile / 2, y0 = ty * kTile - kTile / 2;
+    float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
+    float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
+    float2* __restrict__ Ht = H + (size_t)gi * g.ny * g.nx;
+    {   // zero the fixed-point tile
+        int4* za = reinterpret_cast<int4*>(smem + kOwOffA);
+        for (int i = tid; i < (kOwOffH - kOwOffA) / 16; i += 256) za[i] = make_int4(0, 0, 0, 0);
+    }
     const uint4* __restrict__ recs = sorted + start;
     OwWarpAcc A;
     OwScale sc;
@@ -649,7 +631,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         }
     }
 
-    // (3) output: fixed point -> fp32 (the scales are powers of two)
+    // (3) output: fixed point -> fp32
     const float iv = 1.0f / sc.v, iw = 1.0f / sc.w;
     float4* part = nullptr;
     if (heavy) part = reinterpret_cast<float4*>(scratch + (size_t)(first_slot + chunk) * kOwTileFloats);
@@ -683,7 +665,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             *dst = v;
         }
     }
-    if (!heavy) return;
+    if (!heavy) continue;
     // heavy tile: the last chunk to arrive adds the published partial tiles up in chunk order
     __threadfence();
     __syncthreads();
@@ -692,7 +674,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         sLast = (t == nchunks - 1u);
     }
     __syncthreads();
-    if (!sLast) return;
+    if (!sLast) continue;
     __threadfence();
     const float4* parts = reinterpret_cast<const float4*>(scratch + (size_t)first_slot * kOwTileFloats);
     float* sWsum = reinterpret_cast<float*>(smem + kOwOffB);          // summed weight tile, dense [32][32], for H
@@ -730,6 +712,33 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         }
     }
     if (tid == 0) tickets[first_slot] = 0;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------- O4a fill
+// STORE mode: zero the EMPTY tiles of G, Gw and H.  One CTA per (grid, row of tiles): the empty tiles of a tile row
+// are written as long contiguous runs of each cell row (16-byte stores, consecutive threads -> consecutive
+// addresses), a streaming pattern that runs at the copy bandwidth.
+__global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t* __restrict__ bin_offset,
+                                                    GridPtrs grids, float2* __restrict__ H) {
+    __shared__ unsigned char s_empty[1024 + 8];
+    const int gi = blockIdx.x, ty = blockIdx.y;
+    const uint32_t bin0 = (uint32_t)gi * (uint32_t)g.ntiles + (uint32_t)ty * (uint32_t)g.ntx;
+    for (int t = threadIdx.x; t < g.ntx; t += blockDim.x) s_empty[t] = bin_offset[bin0 + t + 1] == bin_offset[bin0 + t];
+    __syncthreads();
+    const int y0 = max(ty * kTile - kTile / 2, 0), y1 = min(ty * kTile + kTile / 2, g.ny);
+    const int nx2 = g.nx >> 1, nx4 = g.nx >> 2;
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int y = y0; y < y1; ++y) {
+        const size_t row = ((size_t)gi * g.ny + y) * (size_t)g.nx;
+        float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row);
+        float4* __restrict__ hr = reinterpret_cast<float4*>(H + row);
+        float4* __restrict__ wr = reinterpret_cast<float4*>(grids.Gw + row);
+        for (int i = threadIdx.x; i < nx2; i += blockDim.x)             // 2 cells of G / H per store
+            if (s_empty[(2 * i + kTile / 2) >> kTileShift]) { gr[i] = z; hr[i] = z; }
+        for (int i = threadIdx.x; i < nx4; i += blockDim.x)             // 4 cells of Gw per store
+            if (s_empty[(4 * i + kTile / 2) >> kTileShift]) wr[i] = z;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------- launchers
@@ -743,8 +752,8 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
 }
 
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
-                              uint32_t item_size, cudaStream_t s) {
-    k_owner_scan<<<1, 1024, 0, s>>>(g, bin_count, bin_offset, items, nitems, item_size);
+                              uint32_t item_size, uint32_t* work, uint32_t* ctl, cudaStream_t s) {
+    k_owner_scan<<<1, 1024, 0, s>>>(g, bin_count, bin_offset, items, nitems, item_size, work, ctl);
     return cudaGetLastError();
 }
 
@@ -764,18 +773,19 @@ cudaError_t owner_kernel_setup(int max_smem_bytes) {
 }
 
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
-                              const OwItem* items, const uint32_t* nitems, uint32_t max_items, uint32_t item_size,
-                              const uint32_t* order, const float* tt2, GridPtrs grids, float* scratch,
-                              uint32_t* tickets, float2* H, Stats* stats, int store_mode, cudaStream_t s) {
-    const uint32_t item_rows = (max_items + (uint32_t)g.ngrids - 1) / (uint32_t)g.ngrids;
-    const dim3 blocks((unsigned)g.ngrids, item_rows + (unsigned)g.ntiles);
+                              const OwItem* items, const uint32_t* nitems, const uint32_t* work, uint32_t* ctl,
+                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, float2* H,
+                              Stats* stats, int store_mode, int num_sms, cudaStream_t s) {
     const size_t smem = owner_smem_bytes(g.Q);
-    if (store_mode)
-        k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, item_rows, item_size,
-                                                     order, tt2, grids, scratch, tickets, H, stats);
-    else
-        k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, item_rows, item_size,
-                                                     order, tt2, grids, scratch, tickets, H, stats);
+    const unsigned blocks = (unsigned)num_sms * 4u;
+    if (store_mode) {
+        k_owner_fill<<<dim3((unsigned)g.ngrids, (unsigned)g.nty), 256, 0, s>>>(g, bin_offset, grids, H);
+        k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, work, ctl, tt2, grids,
+                                                     scratch, tickets, H, stats);
+    } else {
+        k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, work, ctl, tt2, grids,
+                                                     scratch, tickets, H, stats);
+    }
     return cudaGetLastError();
 }
 
