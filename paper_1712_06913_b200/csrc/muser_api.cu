@@ -54,8 +54,8 @@ struct muser_imager {
     uint32_t* ow_tickets = nullptr;
     float* ow_scratch = nullptr;
     size_t ow_items_cap = 0, ow_sorted_cap = 0, ow_bins_cap = 0;
-    uint4* ow_sorted = nullptr;
-    uint32_t *ow_count = nullptr, *ow_offset = nullptr, *ow_work = nullptr, *ow_ctl = nullptr;
+    uint4 *ow_sorted = nullptr, *ow_loc = nullptr;          // tile-sorted records; per-visibility integer result of O1
+    uint32_t *ow_count = nullptr, *ow_offset = nullptr, *ow_work = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     bool h_packed = false;                  // H already holds G + i*alpha*Gw (written by the owner gridder in store mode)
     cufftHandle plan = 0;
@@ -116,8 +116,8 @@ void free_grids(muser_imager* h) {
 void free_bins(muser_imager* h) {
     cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
     h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
-    cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work);
-    h->ow_count = h->ow_offset = h->ow_work = nullptr; h->ow_bins_cap = 0;
+    cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
+    h->ow_count = h->ow_offset = h->ow_work = h->ow_tops = nullptr; h->ow_bins_cap = 0;
 }
 
 int rebuild_geom(muser_imager* h) {
@@ -301,18 +301,20 @@ uint32_t owner_item_size(long long nvis) {
 int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, uint32_t* max_items_out) {
     const size_t nrec = (size_t)8 * (size_t)nvis;                    // <= 2 samples x 4 tiles per visibility
     if (nrec > h->ow_sorted_cap) {
-        cudaFree(h->ow_sorted); h->ow_sorted = nullptr; h->ow_sorted_cap = 0;
+        cudaFree(h->ow_sorted); cudaFree(h->ow_loc); h->ow_sorted = h->ow_loc = nullptr; h->ow_sorted_cap = 0;
         const size_t cap = nrec + nrec / 8 + 1024;
         CU(h, cudaMalloc(&h->ow_sorted, cap * sizeof(uint4)));
+        CU(h, cudaMalloc(&h->ow_loc, (cap / 8 + 1) * sizeof(uint4)));
         h->ow_sorted_cap = cap;
     }
     const size_t nb = ((size_t)h->geom.nbins + 8) & ~(size_t)3;
     if (nb > h->ow_bins_cap) {
-        cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work);
-        h->ow_count = h->ow_offset = h->ow_work = nullptr; h->ow_bins_cap = 0;
+        cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
+        h->ow_count = h->ow_offset = h->ow_work = h->ow_tops = nullptr; h->ow_bins_cap = 0;
         CU(h, cudaMalloc(&h->ow_count, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_offset, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_work, nb * sizeof(uint32_t)));
+        CU(h, cudaMalloc(&h->ow_tops, (nb / 4096 + 2) * 3 * sizeof(uint32_t)));
         if (!h->ow_ctl) CU(h, cudaMalloc(&h->ow_ctl, 4 * sizeof(uint32_t)));
         CU(h, cudaMemset(h->ow_count, 0, nb * sizeof(uint32_t)));     // every later use leaves it zeroed
         h->ow_bins_cap = nb;
@@ -351,10 +353,10 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         h->fft_valid = false;
         {
             StageScope sc(h, MUSER_STAGE_BIN, s);
-            CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, s));
+            CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, h->ow_loc, s));
             CU(h, launch_owner_scan(g, h->ow_count, h->ow_offset, h->ow_items, h->nitems_d, item_size, h->ow_work,
-                                    h->ow_ctl, s));
-            CU(h, launch_owner_scatter(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_count,
+                                    h->ow_ctl, h->ow_tops, s));
+            CU(h, launch_owner_scatter(g, h->ow_loc, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_count,
                                        h->ow_sorted, s));
         }
         {
@@ -363,7 +365,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
                                     h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->H, h->stats_d,
                                     h->zero_pending ? 1 : 0, h->num_sms, s));
         }
-        h->n_launches += h->zero_pending ? 5 : 4;                     // count, scan, scatter, (fill,) grid
+        h->n_launches += h->zero_pending ? 7 : 6;                     // count, 3 x scan, scatter, (fill,) grid
         h->h_packed = h->zero_pending;                                // store mode also wrote the FFT input H
         h->zero_pending = false;                                      // store mode wrote every tile of every grid
         return MUSER_OK;
@@ -503,7 +505,7 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
     cudaFree(h->ttp_d); cudaFree(h->order_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
-    cudaFree(h->ow_sorted); cudaFree(h->ow_ctl);
+    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl);
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete h;

@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
                                                              const double* __restrict__ freq, const float2* __restrict__ vis,
                                                              const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                              const long long nvis, uint32_t* __restrict__ bin_count,
-                                                             Stats* __restrict__ stats) {
+                                                             Stats* __restrict__ stats, uint4* __restrict__ loc) {
     extern __shared__ uint32_t s_hist[];
     __shared__ int s_flag[2];
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -126,6 +126,16 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
     OwLoc L;
     float2 V;
     ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V);
+    if (k < nvis) {                                                   // integer result of O1 for k_owner_scatter
+        uint4 o = make_uint4(0u, 0u, (uint32_t)L.state << 30, 0u);
+        if (L.state == 3) {
+            o.x = (uint32_t)L.cu[0] | ((uint32_t)L.cv[0] << 16);
+            o.y = (uint32_t)L.cu[1] | ((uint32_t)L.cv[1] << 16);
+            o.z |= (uint32_t)L.rx[0] | ((uint32_t)L.ry[0] << 9) | ((uint32_t)L.rx[1] << 18);
+            o.w = (uint32_t)L.ry[1];
+        }
+        loc[k] = o;
+    }
     const int kept = L.state == 3, dropped = L.state == 2, flagged = L.state == 1;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
     if (kept) {
@@ -198,70 +208,112 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
 }
 
 // ------------------------------------------------------------------------------------------------- O2 scan
-// One CTA walks the histogram 4096 bins at a time (4 per thread): exclusive sample offsets, chunk items of the
-// heavy bins, and re-zeroes the histogram (k_owner_scatter reuses it as its cursor).
-__global__ void __launch_bounds__(1024) k_owner_scan(const Geom g, uint32_t* __restrict__ bin_count,
-                                                     uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
-                                                     uint32_t* __restrict__ nitems, const uint32_t item_size,
-                                                     uint32_t* __restrict__ work, uint32_t* __restrict__ ctl) {
-    __shared__ uint32_t s_wsum[3][32];
-    __shared__ uint32_t s_carry[3];
+// Three small launches over the tile histogram, 4096 bins per CTA (4 per thread):
+//   k_owner_scan_reduce   per-CTA totals of (samples, chunk items of heavy tiles, light non-empty tiles)
+//   k_owner_scan_tops     one CTA: exclusive scan of the per-CTA totals, grand totals, work counter reset
+//   k_owner_scan_write    per-CTA local scan + base: sample offsets, chunk items of the heavy tiles (more than
+//                         item_size samples), the work list of light non-empty tiles; re-zeroes the histogram
+//                         (k_owner_scatter reuses it as its cursor)
+struct OwScan3 { uint32_t c, m, l; };
+
+__device__ __forceinline__ OwScan3 ow_block_scan3(OwScan3 v, OwScan3& total, uint32_t (*s_w)[32]) {
+    // exclusive block scan of three counters over 1024 threads; `total` = block sum
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) { s_carry[0] = 0; s_carry[1] = 0; s_carry[2] = 0; }
-    __syncthreads();
-    for (uint32_t base = 0; base < g.nbins; base += 4096) {
-        const uint32_t b0 = base + 4 * threadIdx.x;
-        uint32_t c[4] = {0, 0, 0, 0}, m[4];
-        if (b0 < g.nbins) {                                            // bin_count is padded to a multiple of 4
-            const uint4 v = *reinterpret_cast<const uint4*>(bin_count + b0);
-            c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
-            if (v.x | v.y | v.z | v.w) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);
-        }
-        uint32_t tc = 0, tm = 0, tl = 0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            m[j] = c[j] > item_size ? (c[j] + item_size - 1) / item_size : 0u;
-            tc += c[j]; tm += m[j]; tl += (c[j] != 0u && m[j] == 0u);
-        }
-        uint32_t ic = tc, im = tm, il = tl;                             // inclusive warp scans
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t xc = __shfl_up_sync(kFull, ic, o), xm = __shfl_up_sync(kFull, im, o), xl = __shfl_up_sync(kFull, il, o);
-            if (lane >= o) { ic += xc; im += xm; il += xl; }
-        }
-        if (lane == 31) { s_wsum[0][warp] = ic; s_wsum[1][warp] = im; s_wsum[2][warp] = il; }
-        __syncthreads();
-        if (warp == 0) {
-            uint32_t wc = s_wsum[0][lane], wm = s_wsum[1][lane], wl = s_wsum[2][lane];
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t xc = __shfl_up_sync(kFull, wc, o), xm = __shfl_up_sync(kFull, wm, o), xl = __shfl_up_sync(kFull, wl, o);
-                if (lane >= o) { wc += xc; wm += xm; wl += xl; }
-            }
-            s_wsum[0][lane] = wc; s_wsum[1][lane] = wm; s_wsum[2][lane] = wl;
-        }
-        __syncthreads();
-        uint32_t off = s_carry[0] + (warp ? s_wsum[0][warp - 1] : 0) + ic - tc;
-        uint32_t slot = s_carry[1] + (warp ? s_wsum[1][warp - 1] : 0) + im - tm;
-        uint32_t wpos = s_carry[2] + (warp ? s_wsum[2][warp - 1] : 0) + il - tl;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t b = b0 + j;
-            if (b < g.nbins) {
-                bin_offset[b] = off;
-                if (c[j] != 0u && m[j] == 0u) work[wpos++] = b;        // light non-empty tile: one work unit
-                for (uint32_t q = 0; q < m[j]; ++q) {
-                    OwItem it;
-                    it.bin = b; it.start = off + q * item_size; it.count = min(item_size, c[j] - q * item_size);
-                    it.first_slot = slot; it.nchunks = m[j]; it.chunk = q;
-                    items[slot + q] = it;
-                }
-            }
-            off += c[j]; slot += m[j];
-        }
-        __syncthreads();
-        if (threadIdx.x == 1023) { s_carry[0] = off; s_carry[1] = slot; s_carry[2] = wpos; }
-        __syncthreads();
+    OwScan3 inc = v;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t xc = __shfl_up_sync(kFull, inc.c, o), xm = __shfl_up_sync(kFull, inc.m, o), xl = __shfl_up_sync(kFull, inc.l, o);
+        if (lane >= o) { inc.c += xc; inc.m += xm; inc.l += xl; }
     }
-    if (threadIdx.x == 0) { bin_offset[g.nbins] = s_carry[0]; *nitems = s_carry[1]; ctl[0] = s_carry[2]; ctl[1] = 0; }
+    if (lane == 31) { s_w[0][warp] = inc.c; s_w[1][warp] = inc.m; s_w[2][warp] = inc.l; }
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t wc = s_w[0][lane], wm = s_w[1][lane], wl = s_w[2][lane];
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t xc = __shfl_up_sync(kFull, wc, o), xm = __shfl_up_sync(kFull, wm, o), xl = __shfl_up_sync(kFull, wl, o);
+            if (lane >= o) { wc += xc; wm += xm; wl += xl; }
+        }
+        s_w[0][lane] = wc; s_w[1][lane] = wm; s_w[2][lane] = wl;
+    }
+    __syncthreads();
+    OwScan3 ex;
+    ex.c = (warp ? s_w[0][warp - 1] : 0u) + inc.c - v.c;
+    ex.m = (warp ? s_w[1][warp - 1] : 0u) + inc.m - v.m;
+    ex.l = (warp ? s_w[2][warp - 1] : 0u) + inc.l - v.l;
+    total.c = s_w[0][31]; total.m = s_w[1][31]; total.l = s_w[2][31];
+    __syncthreads();
+    return ex;
+}
+
+__device__ __forceinline__ OwScan3 ow_load4(const Geom& g, const uint32_t* __restrict__ bin_count, uint32_t b0,
+                                            uint32_t item_size, uint32_t c[4], uint32_t m[4]) {
+    c[0] = c[1] = c[2] = c[3] = 0;
+    if (b0 < g.nbins) {                                                // bin_count is padded to a multiple of 4
+        const uint4 v = *reinterpret_cast<const uint4*>(bin_count + b0);
+        c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
+    }
+    OwScan3 t = {0u, 0u, 0u};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        m[j] = c[j] > item_size ? (c[j] + item_size - 1) / item_size : 0u;
+        t.c += c[j]; t.m += m[j]; t.l += (c[j] != 0u && m[j] == 0u);
+    }
+    return t;
+}
+
+__global__ void __launch_bounds__(1024) k_owner_scan_reduce(const Geom g, const uint32_t* __restrict__ bin_count,
+                                                            const uint32_t item_size, uint32_t* __restrict__ tops) {
+    __shared__ uint32_t s_w[3][32];
+    uint32_t c[4], m[4];
+    const OwScan3 t = ow_load4(g, bin_count, blockIdx.x * 4096u + 4u * threadIdx.x, item_size, c, m);
+    OwScan3 total;
+    ow_block_scan3(t, total, s_w);
+    if (threadIdx.x == 0) { tops[3 * blockIdx.x] = total.c; tops[3 * blockIdx.x + 1] = total.m; tops[3 * blockIdx.x + 2] = total.l; }
+}
+
+__global__ void __launch_bounds__(1024) k_owner_scan_tops(const Geom g, const uint32_t nblocks, uint32_t* __restrict__ tops,
+                                                          uint32_t* __restrict__ bin_offset, uint32_t* __restrict__ nitems,
+                                                          uint32_t* __restrict__ ctl) {
+    __shared__ uint32_t s_w[3][32];
+    OwScan3 carry = {0u, 0u, 0u};
+    for (uint32_t base = 0; base < nblocks; base += 1024) {
+        const uint32_t b = base + threadIdx.x;
+        OwScan3 v = {0u, 0u, 0u};
+        if (b < nblocks) { v.c = tops[3 * b]; v.m = tops[3 * b + 1]; v.l = tops[3 * b + 2]; }
+        OwScan3 total;
+        const OwScan3 ex = ow_block_scan3(v, total, s_w);
+        if (b < nblocks) { tops[3 * b] = carry.c + ex.c; tops[3 * b + 1] = carry.m + ex.m; tops[3 * b + 2] = carry.l + ex.l; }
+        carry.c += total.c; carry.m += total.m; carry.l += total.l;
+    }
+    if (threadIdx.x == 0) { bin_offset[g.nbins] = carry.c; *nitems = carry.m; ctl[0] = carry.l; ctl[1] = 0; }
+}
+
+__global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_t* __restrict__ bin_count,
+                                                           const uint32_t item_size, const uint32_t* __restrict__ tops,
+                                                           uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
+                                                           uint32_t* __restrict__ work) {
+    __shared__ uint32_t s_w[3][32];
+    const uint32_t b0 = blockIdx.x * 4096u + 4u * threadIdx.x;
+    uint32_t c[4], m[4];
+    const OwScan3 t = ow_load4(g, bin_count, b0, item_size, c, m);
+    if (t.c) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);
+    OwScan3 total;
+    const OwScan3 ex = ow_block_scan3(t, total, s_w);
+    uint32_t off = tops[3 * blockIdx.x] + ex.c, slot = tops[3 * blockIdx.x + 1] + ex.m, wpos = tops[3 * blockIdx.x + 2] + ex.l;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t b = b0 + j;
+        if (b < g.nbins) {
+            bin_offset[b] = off;
+            if (c[j] != 0u && m[j] == 0u) work[wpos++] = b;            // light non-empty tile: one work unit
+            for (uint32_t q = 0; q < m[j]; ++q) {
+                OwItem it;
+                it.bin = b; it.start = off + q * item_size; it.count = min(item_size, c[j] - q * item_size);
+                it.first_slot = slot; it.nchunks = m[j]; it.chunk = q;
+                items[slot + q] = it;
+            }
+        }
+        off += c[j]; slot += m[j];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------- O3 scatter
@@ -284,8 +336,8 @@ __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, i
     *dst = o;
 }
 
-__global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, const float* __restrict__ uvw,
-                                                               const double* __restrict__ freq, const float2* __restrict__ vis,
+__global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, const uint4* __restrict__ loc,
+                                                               const float2* __restrict__ vis,
                                                                const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                                const long long nvis, const uint32_t* __restrict__ bin_offset,
                                                                uint32_t* __restrict__ cursor, uint4* __restrict__ sorted) {
@@ -294,8 +346,20 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     OwLoc L;
-    float2 V;
-    ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V);
+    L.state = 0;
+    if (k < nvis) {                                                   // k_owner_count's integer decisions
+        const uint4 o = __ldg(loc + k);
+        L.state = (int)(o.z >> 30);
+        if (L.state == 3) {
+            L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
+            L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
+            L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
+            L.ry[1] = (int)(o.w & 511u);
+            const float2 V = vis[k];
+            const float wt = weight[k];
+            L.re = wt * V.x; L.im = wt * V.y; L.wt = wt; L.gid = grid_id ? grid_id[k] : 0;
+        }
+    }
     const int kept = L.state == 3;
     const int use_smem = ow_cta_uniform_grid(L, g.ntiles, s_flag);
     if (use_smem) {
@@ -745,23 +809,27 @@ __global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t
 static size_t bin_smem_bytes(const Geom& g) { return g.ntiles <= kBinSmemTiles ? (size_t)g.ntiles * sizeof(uint32_t) : 0; }
 
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
-                               const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, cudaStream_t s) {
+                               const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, uint4* loc,
+                               cudaStream_t s) {
     k_owner_count<<<(unsigned)((nvis + kBinThreads - 1) / kBinThreads), kBinThreads, bin_smem_bytes(g), s>>>(
-        g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats);
+        g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
     return cudaGetLastError();
 }
 
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
-                              uint32_t item_size, uint32_t* work, uint32_t* ctl, cudaStream_t s) {
-    k_owner_scan<<<1, 1024, 0, s>>>(g, bin_count, bin_offset, items, nitems, item_size, work, ctl);
+                              uint32_t item_size, uint32_t* work, uint32_t* ctl, uint32_t* tops, cudaStream_t s) {
+    const uint32_t nblocks = (g.nbins + 4095u) / 4096u;
+    k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
+    k_owner_scan_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems, ctl);
+    k_owner_scan_write<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops, bin_offset, items, work);
     return cudaGetLastError();
 }
 
-cudaError_t launch_owner_scatter(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
-                                 const int* grid_id, long long nvis, const uint32_t* bin_offset, uint32_t* cursor,
-                                 uint4* sorted, cudaStream_t s) {
+cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float2* vis, const float* wt, const int* grid_id,
+                                 long long nvis, const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted,
+                                 cudaStream_t s) {
     k_owner_scatter<<<(unsigned)((nvis + kBinThreads - 1) / kBinThreads), kBinThreads, bin_smem_bytes(g), s>>>(
-        g, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
+        g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
     return cudaGetLastError();
 }
 
