@@ -100,7 +100,7 @@ __device__ __forceinline__ uint32_t ow_agg_inc(uint32_t* __restrict__ cnt, uint3
 // grid's tile count fits the shared histogram, the CTA counts in shared memory and issues ONE global atomic per
 // touched tile (MUSER's central tile takes a third of all samples: per-sample global atomics serialise on it).
 constexpr int kBinThreads = 1024;
-constexpr int kBinSmemTiles = 8192;
+constexpr int kBinSmemTiles = 4096;      // two u32 arrays of this many tiles must fit the default 48 KB
 
 __device__ __forceinline__ int ow_cta_uniform_grid(const OwLoc& L, int ntiles, int* s_flag) {
     // s_flag[0] = first kept grid id seen (or -1), s_flag[1] = 1 if a kept visibility disagrees
@@ -111,6 +111,20 @@ __device__ __forceinline__ int ow_cta_uniform_grid(const OwLoc& L, int ntiles, i
     if (L.state == 3 && L.gid != s_flag[0]) s_flag[1] = 1;
     __syncthreads();
     return ntiles <= kBinSmemTiles && s_flag[1] == 0 && s_flag[0] >= 0;
+}
+
+// The (at most 2 x 2) tiles a 7x7 footprint at nearest cell (cu, cv) touches: first tile (tx0, ty0) and whether the
+// footprint also reaches the next tile in x / in y.
+struct OwTiles { int tx0, ty0, t00; bool mx, my; };
+__device__ __forceinline__ OwTiles ow_tiles(const Geom& g, int cu, int cv) {
+    const int h = (g.S - 1) >> 1;
+    OwTiles t;
+    t.tx0 = (cu - h + kTile / 2) >> kTileShift;
+    t.ty0 = (cv - h + kTile / 2) >> kTileShift;
+    t.mx = ((cu + h + kTile / 2) >> kTileShift) != t.tx0;
+    t.my = ((cv + h + kTile / 2) >> kTileShift) != t.ty0;
+    t.t00 = t.ty0 * g.ntx + t.tx0;
+    return t;
 }
 
 // ------------------------------------------------------------------------------------------------- O1 count
@@ -148,24 +162,20 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
         for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
         const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ntiles;
-        uint32_t first[8];                                            // bit q + 4s set: this thread saw the tile empty
-        uint32_t firstmask = 0;
         if (kept) {
 #pragma unroll
-            for (int s = 0; s < 2; ++s)
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    int tx, ty;
-                    const uint32_t bin = ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty);
-                    first[q + 4 * s] = bin;
-                    if (bin != kNoBin && atomicAdd(&s_hist[bin - gbase], 1u) == 0u) firstmask |= 1u << (q + 4 * s);
-                }
+            for (int s = 0; s < 2; ++s) {
+                const OwTiles t = ow_tiles(g, L.cu[s], L.cv[s]);
+                atomicAdd(&s_hist[t.t00], 1u);
+                if (t.mx) atomicAdd(&s_hist[t.t00 + 1], 1u);
+                if (t.my) atomicAdd(&s_hist[t.t00 + g.ntx], 1u);
+                if (t.mx && t.my) atomicAdd(&s_hist[t.t00 + g.ntx + 1], 1u);
+            }
         }
         __syncthreads();
-        if (firstmask) {
-#pragma unroll
-            for (int j = 0; j < 8; ++j)
-                if (firstmask & (1u << j)) atomicAdd(&bin_count[first[j]], s_hist[first[j] - gbase]);
+        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) {
+            const uint32_t n = s_hist[i];
+            if (n) atomicAdd(&bin_count[gbase + i], n);
         }
     } else if (__any_sync(kFull, kept)) {
 #pragma unroll
@@ -366,46 +376,35 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
         for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
         const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ntiles;
-        uint32_t bins[8], rank[8];
-        uint32_t firstmask = 0;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) bins[j] = kNoBin;
+        uint32_t* s_base = s_hist + g.ntiles;                         // global position of this CTA's run in each tile
+        OwTiles T[2];
+        uint32_t rk[2][4];
         if (kept) {
 #pragma unroll
-            for (int s = 0; s < 2; ++s)
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    int tx, ty;
-                    const uint32_t bin = ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty);
-                    bins[q + 4 * s] = bin;
-                    if (bin != kNoBin) {
-                        rank[q + 4 * s] = atomicAdd(&s_hist[bin - gbase], 1u);
-                        if (rank[q + 4 * s] == 0u) firstmask |= 1u << (q + 4 * s);
-                    }
-                }
+            for (int s = 0; s < 2; ++s) {
+                T[s] = ow_tiles(g, L.cu[s], L.cv[s]);
+                rk[s][0] = atomicAdd(&s_hist[T[s].t00], 1u);
+                if (T[s].mx) rk[s][1] = atomicAdd(&s_hist[T[s].t00 + 1], 1u);
+                if (T[s].my) rk[s][2] = atomicAdd(&s_hist[T[s].t00 + g.ntx], 1u);
+                if (T[s].mx && T[s].my) rk[s][3] = atomicAdd(&s_hist[T[s].t00 + g.ntx + 1], 1u);
+            }
         }
         __syncthreads();
-        if (firstmask) {                                              // reserve this CTA's run in each touched tile
-#pragma unroll
-            for (int j = 0; j < 8; ++j)
-                if (firstmask & (1u << j)) {
-                    const uint32_t t = bins[j] - gbase;
-                    s_hist[t] = bin_offset[bins[j]] + atomicAdd(&cursor[bins[j]], s_hist[t]);
-                }
+        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) {     // reserve this CTA's run in each touched tile
+            const uint32_t n = s_hist[i];
+            if (n) s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n);
         }
         __syncthreads();
         if (kept) {
 #pragma unroll
-            for (int s = 0; s < 2; ++s)
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const uint32_t bin = bins[q + 4 * s];
-                    if (bin != kNoBin) {
-                        int tx, ty;
-                        ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty);
-                        ow_write_record(g, L, s, tx, ty, sorted + s_hist[bin - gbase] + rank[q + 4 * s]);
-                    }
-                }
+            for (int s = 0; s < 2; ++s) {
+                const OwTiles t = T[s];
+                ow_write_record(g, L, s, t.tx0, t.ty0, sorted + s_base[t.t00] + rk[s][0]);
+                if (t.mx) ow_write_record(g, L, s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + rk[s][1]);
+                if (t.my) ow_write_record(g, L, s, t.tx0, t.ty0 + 1, sorted + s_base[t.t00 + g.ntx] + rk[s][2]);
+                if (t.mx && t.my)
+                    ow_write_record(g, L, s, t.tx0 + 1, t.ty0 + 1, sorted + s_base[t.t00 + g.ntx + 1] + rk[s][3]);
+            }
         }
         return;
     }
@@ -806,7 +805,7 @@ __global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t
 }
 
 // ------------------------------------------------------------------------------------------------- launchers
-static size_t bin_smem_bytes(const Geom& g) { return g.ntiles <= kBinSmemTiles ? (size_t)g.ntiles * sizeof(uint32_t) : 0; }
+static size_t bin_smem_bytes(const Geom& g) { return g.ntiles <= kBinSmemTiles ? (size_t)2 * g.ntiles * sizeof(uint32_t) : 0; }
 
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                                const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, uint4* loc,
