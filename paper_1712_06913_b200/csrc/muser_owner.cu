@@ -473,27 +473,39 @@ __device__ __forceinline__ void ow_window(OwWarpAcc& A, const uint32_t key, cons
     A.a0 = A.a1 = A.b = 0ull;
 }
 
-__device__ __forceinline__ void ow_flush(const OwWarpAcc& A, const OwScale sc, int* sA, int* sB) {
+// Merge the window into the shared tile.  The accumulators are already in fixed-point units (ow_stage scales the
+// values once per record), so this is six conversions and six native integer adds.
+__device__ __forceinline__ void ow_flush(const OwWarpAcc& A, int* sA, int* sB) {
     if (A.off >= 0) {
         const float2 c0 = ow_unpack(A.a0), c1 = ow_unpack(A.a1), w = ow_unpack(A.b);
         int* pa = sA + 2 * A.off;
-        atomicAdd(pa + 0, __float2int_rn(c0.x * sc.v));
-        atomicAdd(pa + 1, __float2int_rn(c0.y * sc.v));
-        atomicAdd(pa + 2, __float2int_rn(c1.x * sc.v));
-        atomicAdd(pa + 3, __float2int_rn(c1.y * sc.v));
-        atomicAdd(sB + A.off, __float2int_rn(w.x * sc.w));
-        atomicAdd(sB + A.off + 1, __float2int_rn(w.y * sc.w));
+        atomicAdd(pa + 0, __float2int_rn(c0.x));
+        atomicAdd(pa + 1, __float2int_rn(c0.y));
+        atomicAdd(pa + 2, __float2int_rn(c1.x));
+        atomicAdd(pa + 3, __float2int_rn(c1.y));
+        atomicAdd(sB + A.off, __float2int_rn(w.x));
+        atomicAdd(sB + A.off + 1, __float2int_rn(w.y));
     }
 }
 
-// One sample into the register window.  tbx = table + 2c floats, tby = table + r floats (shared memory).
-__device__ __forceinline__ void ow_add(OwWarpAcc& A, const uint4 rec, const char* tbx, const char* tby) {
-    const uint32_t pk = rec.w;
-    const float2 kx = *reinterpret_cast<const float2*>(tbx + ((pk >> 5) & 0x7FE0u));      // X * 32 bytes
-    const float ky = *reinterpret_cast<const float*>(tby + ((pk >> 15) & 0x7FE0u));       // Y * 32 bytes
+// Staged form of a record, built once by the lane that loads it: values in fixed-point units, table row byte
+// offsets (X * 32 | Y * 32 << 16) instead of the packed word.
+__device__ __forceinline__ uint4 ow_stage(const uint4 rec, const OwScale sc) {
+    uint4 st;
+    st.x = __float_as_uint(__uint_as_float(rec.x) * sc.v);
+    st.y = __float_as_uint(__uint_as_float(rec.y) * sc.v);
+    st.z = __float_as_uint(__uint_as_float(rec.z) * sc.w);
+    st.w = ((rec.w >> 5) & 0x7FE0u) | (((rec.w >> 15) & 0x7FE0u) << 16);
+    return st;
+}
+
+// One staged sample into the register window.  tbx = table + 2c floats, tby = table + r floats (shared memory).
+__device__ __forceinline__ void ow_add(OwWarpAcc& A, const uint4 st, const char* tbx, const char* tby) {
+    const float2 kx = *reinterpret_cast<const float2*>(tbx + (st.w & 0xFFFFu));
+    const float ky = *reinterpret_cast<const float*>(tby + (st.w >> 16));
     const float k0 = kx.x * ky, k1 = kx.y * ky;
-    const unsigned long long v = ow_pack(__uint_as_float(rec.x), __uint_as_float(rec.y));
-    const float wt = __uint_as_float(rec.z);
+    const unsigned long long v = ow_pack(__uint_as_float(st.x), __uint_as_float(st.y));
+    const float wt = __uint_as_float(st.z);
     A.a0 = ow_fma2(ow_pack(k0, k0), v, A.a0);
     A.a1 = ow_fma2(ow_pack(k1, k1), v, A.a1);
     A.b = ow_fma2(ow_pack(k0, k1), ow_pack(wt, wt), A.b);
@@ -604,8 +616,8 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         for (uint32_t i = warp; i < cnt; i += 8) {
             const uint4 rec = __ldg(recs + i);
             ow_window(A, rec.w & 0x3FFu, r, c);
-            ow_add(A, rec, tbx, tby);
-            ow_flush(A, sc, sA, sB);
+            ow_add(A, ow_stage(rec, sc), tbx, tby);
+            ow_flush(A, sA, sB);
         }
         __syncthreads();
     } else {
@@ -654,7 +666,10 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 sH[2 * tid] = ex; sH[2 * tid + 1] = ex + h0;
             }
             __syncthreads();
-            for (uint32_t i = tid; i < n; i += 256) sI[sH[ow_sortkey(__ldg(&src[i].w))] + sP[i]] = (unsigned short)i;
+            for (uint32_t i = tid; i < n; i += 256) {                  // bit 15: last record of its window
+                const uint32_t k = ow_sortkey(__ldg(&src[i].w)), pos = sH[k] + sP[i];
+                sI[pos] = (unsigned short)(i | ((pos + 1u == sH[k + 1u]) ? 0x8000u : 0u));
+            }
             __syncthreads();
             // (2) every warp streams an equal share of the sorted order through its private 2 x 32-record buffer
             //     (gather loads one batch ahead); runs of equal window stay in registers across batches
@@ -664,31 +679,31 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 const int e = min((int)n, (warp + 1) * per);
                 int p = warp * per;
                 uint4 nxt = make_uint4(0, 0, 0, 0);
-                if (p + lane < e) nxt = __ldg(src + sI[p + lane]);
-                uint32_t cur = 0xFFFFFFFFu;
+                uint32_t nidx = 0;
+                if (p + lane < e) { nidx = sI[p + lane]; nxt = __ldg(src + (nidx & 0xFFFu)); }
                 int buf = 0;
                 while (p < e) {
                     const int m = min(32, e - p);
-                    wb[buf * 32 + lane] = nxt;
+                    wb[buf * 32 + lane] = ow_stage(nxt, sc);
+                    const uint32_t mykey = nxt.w & 0x3FFu;
+                    // a run ends at the last record of its window and at the end of the batch
+                    uint32_t ends = __ballot_sync(kFull, (nidx >> 15) != 0u || lane == m - 1);
                     __syncwarp();
-                    if (p + 32 + lane < e) nxt = __ldg(src + sI[p + 32 + lane]);
+                    if (p + 32 + lane < e) { nidx = sI[p + 32 + lane]; nxt = __ldg(src + (nidx & 0xFFFu)); }
                     const uint4* __restrict__ q = wb + buf * 32;
                     int j = 0;
                     while (j < m) {
-                        const uint32_t key = q[j].w & 0x3FFu;
-                        if (key != cur) {
-                            if (cur != 0xFFFFFFFFu) ow_flush(A, sc, sA, sB);
-                            ow_window(A, key, r, c);
-                            cur = key;
-                        }
-                        const int rend = min(m, (int)sH[(key >> 5) * 19u + (key & 31u) + 1u] - p);
+                        const int len = __ffs(ends);                   // records j .. j + len - 1 share one window
+                        ow_window(A, __shfl_sync(kFull, mykey, j), r, c);
 #pragma unroll 2
-                        for (; j < rend; ++j) ow_add(A, q[j], tbx, tby);
+                        for (int t = 0; t < len; ++t) ow_add(A, q[j + t], tbx, tby);
+                        ow_flush(A, sA, sB);
+                        j += len;
+                        ends = len < 32 ? ends >> len : 0u;
                     }
                     buf ^= 1;
                     p += 32;
                 }
-                if (cur != 0xFFFFFFFFu) ow_flush(A, sc, sA, sB);
             }
             __syncthreads();
         }
@@ -792,15 +807,20 @@ __global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t
     const int y0 = max(ty * kTile - kTile / 2, 0), y1 = min(ty * kTile + kTile / 2, g.ny);
     const int nx2 = g.nx >> 1, nx4 = g.nx >> 2;
     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int y = y0; y < y1; ++y) {
-        const size_t row = ((size_t)gi * g.ny + y) * (size_t)g.nx;
-        float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row);
-        float4* __restrict__ hr = reinterpret_cast<float4*>(H + row);
-        float4* __restrict__ wr = reinterpret_cast<float4*>(grids.Gw + row);
-        for (int i = threadIdx.x; i < nx2; i += blockDim.x)             // 2 cells of G / H per store
-            if (s_empty[(2 * i + kTile / 2) >> kTileShift]) { gr[i] = z; hr[i] = z; }
-        for (int i = threadIdx.x; i < nx4; i += blockDim.x)             // 4 cells of Gw per store
-            if (s_empty[(4 * i + kTile / 2) >> kTileShift]) wr[i] = z;
+    const size_t row0 = ((size_t)gi * g.ny + y0) * (size_t)g.nx;
+    // a thread owns column chunks: the emptiness test is done once per chunk, the loop over the rows only stores
+    for (int i = threadIdx.x; i < nx2; i += blockDim.x) {              // 2 cells of G / H per store
+        if (!s_empty[(2 * i + kTile / 2) >> kTileShift]) continue;
+        float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row0) + i;
+        float4* __restrict__ hr = reinterpret_cast<float4*>(H + row0) + i;
+#pragma unroll 4
+        for (int y = y0; y < y1; ++y, gr += nx2, hr += nx2) { *gr = z; *hr = z; }
+    }
+    for (int i = threadIdx.x; i < nx4; i += blockDim.x) {              // 4 cells of Gw per store
+        if (!s_empty[(4 * i + kTile / 2) >> kTileShift]) continue;
+        float4* __restrict__ wr = reinterpret_cast<float4*>(grids.Gw + row0) + i;
+#pragma unroll 4
+        for (int y = y0; y < y1; ++y, wr += nx4) *wr = z;
     }
 }
 
