@@ -1,19 +1,23 @@
 // Owner-tile gridding path (2-D mode, support 7), sm_100a.
 //
-//   O1 k_owner_count    A1: fp64 coordinates (O1 order), keep/drop, statistics, histogram of the tiles
-//                           each sample's 7x7 footprint touches (1, 2 or 4 tiles); counts in a CTA-private shared
-//                           histogram, one global atomic per touched tile per CTA
-//   O2 k_owner_scan     A1: exclusive scan of the histogram; tiles with more than item_size samples are split
-//                           into chunk items
-//   O3 k_owner_scatter  A1: recomputes the coordinates and writes one 16-byte record per (sample, touched tile)
-//   O4 k_grid_owner_s7  A2/A4: one CTA per 32x32 tile of one grid (or per chunk of a heavy tile).  It counting-sorts
-//                           up to 4096 records by (row, 8-cell column window), stages them 1024 at a time in shared
-//                           memory in sorted order, and every warp walks an equal slice with the 7-row x 8-column
-//                           window held in registers (lane = row r, column pair c; packed FFMA2; kernel table in
-//                           shared memory), touching the shared tile only when the window changes.  The tile is
-//                           then written to G and Gw with plain coalesced stores: the grids need no memset and
-//                           receive no global atomics.  Chunks of a heavy tile write partial tiles to a scratch
-//                           buffer; the last chunk to finish adds them up in chunk order.
+//   O1  k_owner_count      A1: fp64 coordinates (O1 order), keep/drop, statistics; stores the integer
+//                              result per visibility (16 B) and histograms the tiles each sample's 7x7 footprint
+//                              touches (1, 2 or 4) in a CTA-private shared histogram (one global atomic per touched
+//                              tile per CTA)
+//   O2  k_owner_scan_*     A1: multi-CTA exclusive scan of the histogram (3 small launches): sample offsets, chunk
+//                              items of heavy tiles (> item_size samples), work list of light non-empty tiles
+//   O3  k_owner_scatter    A1: reads O1's integer result and writes one 16-byte record per (sample, touched tile)
+//   O4a k_owner_fill       A2: store mode only: zeroes the EMPTY tiles of G, Gw and H in long contiguous runs
+//   O4  k_grid_owner_s7    A2/A4: persistent kernel, 4 CTAs per SM pulling work units (chunks of heavy tiles first,
+//                              then light tiles) from a device counter.  Per unit: counting sort of <= 4096 records by
+//                              8x8 window (shared histogram, 2-byte positions); every warp then streams an equal share
+//                              of the sorted order through a private 2 x 32-record buffer (gather loads one batch
+//                              ahead, records staged in fixed-point units with table row offsets); a run of equal
+//                              window is accumulated in registers (lane = row r, column pair c; three packed FFMA2 per
+//                              sample; kernel table in shared memory) and merged into the 32-bit fixed-point shared
+//                              tile with native integer adds.  The tile is written to G, Gw and (store mode) the FFT
+//                              input H with plain coalesced stores: no memset, no global atomics.  Chunks of a heavy
+//                              tile publish partial tiles; the last chunk to arrive adds them up in chunk order.
 // Passages: PAPER.md:78 (gridding = convolution onto a regular grid), :136-138 (spheroidal GCF), :216-228 (float2
 // grid, row-major, Hermitian), :249-256 (DIRTY_IMAGE).  The binning and tiling are this build's design.
 #include "muser_internal.h"
@@ -99,7 +103,7 @@ __device__ __forceinline__ uint32_t ow_agg_inc(uint32_t* __restrict__ cnt, uint3
 // CTA-level aggregation for the two binning kernels: when every visibility of the CTA belongs to one grid and that
 // grid's tile count fits the shared histogram, the CTA counts in shared memory and issues ONE global atomic per
 // touched tile (MUSER's central tile takes a third of all samples: per-sample global atomics serialise on it).
-constexpr int kBinThreads = 1024;
+constexpr int kBinThreads = 256;
 constexpr int kBinSmemTiles = 4096;      // two u32 arrays of this many tiles must fit the default 48 KB
 
 __device__ __forceinline__ int ow_cta_uniform_grid(const OwLoc& L, int ntiles, int* s_flag) {
