@@ -32,6 +32,8 @@ FRAMES_PER_STEP = 80
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_grid_owner_s7 launch of this workload, from the committed
 # `ncu --set full` capture (profiles/); None until that capture exists
 TRAFFIC_NCU = 1.777e9   # profiles/r01d_owner_path.md: k_owner_fill 925.8 MB + k_grid_owner_s7 851.2 MB (includes the 671 MB FFT input H)
+WORKLOAD = ("configs[2] MUSER-II full frame: 56,640 vis (113,280 samples) -> 1024^2 grid, PSWF S=7 Q=128 "
+            "-> dirty image + beam")
 METRIC = "gridded_visibilities_per_s"
 UNIT = "vis/s"
 
@@ -135,8 +137,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "configs[2] MUSER-II full frame: 56,640 vis -> 1024^2 dirty image + beam",
-                   "frames_per_step": per_step},
+        "config": {"workload": WORKLOAD, "frames_per_step": per_step, "nvis_per_frame": nvis,
+                   "sample": "each step = 2 whole frames of the workload through the oracle on one host core"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
                          "sample": f"{args.steps * per_step} whole frames (oracle_c gridder + numpy fp64 FFT + correction)"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -157,7 +159,7 @@ def main():
         return run_reference(args)
 
     import torch
-    from paper_1712_06913_b200 import binding, build
+    from paper_1712_06913_b200 import binding, build, shard
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -173,7 +175,7 @@ def main():
         dist.barrier()
     W = max(args.warmup, 3)
 
-    params, frames = make_frames(FRAMES_PER_STEP, seed0=rank * FRAMES_PER_STEP)
+    params, frames = make_frames(FRAMES_PER_STEP, seed0=shard.frame_seeds(rank, FRAMES_PER_STEP)[0])
     n, nvis = params.n, frames[0][2].shape[0]
     B = FRAMES_PER_STEP
     # one batch = B frames back to back in memory, frame b -> grid b (muser_grid_batched)
@@ -198,11 +200,7 @@ def main():
             torch.cuda.synchronize()
 
     def max_over_ranks(ms):
-        if dist:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            return float(t.item())
-        return ms
+        return shard.max_over_ranks(ms, dist, device="cuda")
 
     for _ in range(W):
         step()
@@ -223,7 +221,7 @@ def main():
     launches = im.get_launch_count() - l0
     ms = max_over_ranks(e0.elapsed_time(e1))
     frames_total = args.steps * B * world
-    value = frames_total * nvis / (ms * 1e-3)
+    value = shard.aggregate_rate(args.steps * B * nvis, world, ms)
 
     # ---- per-stage device time, live, with CUDA events on the launching stream (second timed pass)
     im.set_profiling(True)
@@ -301,8 +299,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "configs[2] MUSER-II full frame: 56,640 vis (113,280 samples) -> 1024^2 grid, PSWF S=7 Q=128 "
-                                   "-> dirty image + beam; one step = 80 distinct frames, each onto its own grid, in one "
+            "config": {"workload": WORKLOAD, "batching": "one step = 80 distinct frames, each onto its own grid, in one "
                                    "muser_grid_batched + muser_dirty_psf call", "frames_per_step": FRAMES_PER_STEP,
                        "nvis_per_frame": nvis,
                        "l2_policy": "per step 145 MB of inputs and 1.0 GB of grids stream through a 126 MB L2",
