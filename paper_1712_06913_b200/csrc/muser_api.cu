@@ -55,7 +55,8 @@ struct muser_imager {
     float* ow_scratch = nullptr;
     size_t ow_items_cap = 0, ow_sorted_cap = 0, ow_bins_cap = 0;
     uint4 *ow_sorted = nullptr, *ow_loc = nullptr;          // tile-sorted records; per-visibility integer result of O1
-    uint32_t *ow_count = nullptr, *ow_offset = nullptr, *ow_work = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
+    uint32_t *ow_count = nullptr, *ow_offset = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
+    uint4* ow_work = nullptr;
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     bool h_packed = false;                  // H already holds G + i*alpha*Gw (written by the owner gridder in store mode)
     cufftHandle plan = 0;
@@ -117,7 +118,7 @@ void free_bins(muser_imager* h) {
     cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
     h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
     cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
-    h->ow_count = h->ow_offset = h->ow_work = h->ow_tops = nullptr; h->ow_bins_cap = 0;
+    h->ow_count = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
 }
 
 int rebuild_geom(muser_imager* h) {
@@ -312,10 +313,10 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
     const size_t nb = ((size_t)h->geom.nbins + 8) & ~(size_t)3;
     if (nb > h->ow_bins_cap) {
         cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
-        h->ow_count = h->ow_offset = h->ow_work = h->ow_tops = nullptr; h->ow_bins_cap = 0;
+        h->ow_count = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
         CU(h, cudaMalloc(&h->ow_count, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_offset, nb * sizeof(uint32_t)));
-        CU(h, cudaMalloc(&h->ow_work, nb * sizeof(uint32_t)));
+        CU(h, cudaMalloc(&h->ow_work, nb * sizeof(uint4)));
         CU(h, cudaMalloc(&h->ow_tops, (nb / 4096 + 2) * 3 * sizeof(uint32_t)));
         if (!h->ow_ctl) CU(h, cudaMalloc(&h->ow_ctl, 4 * sizeof(uint32_t)));
         CU(h, cudaMemset(h->ow_count, 0, nb * sizeof(uint32_t)));     // every later use leaves it zeroed

@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(1024) k_owner_scan_tops(const Geom g, const ui
 __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_t* __restrict__ bin_count,
                                                            const uint32_t item_size, const uint32_t* __restrict__ tops,
                                                            uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
-                                                           uint32_t* __restrict__ work) {
+                                                           uint4* __restrict__ work) {
     __shared__ uint32_t s_w[3][32];
     const uint32_t b0 = blockIdx.x * 4096u + 4u * threadIdx.x;
     uint32_t c[4], m[4];
@@ -318,7 +318,11 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
         const uint32_t b = b0 + j;
         if (b < g.nbins) {
             bin_offset[b] = off;
-            if (c[j] != 0u && m[j] == 0u) work[wpos++] = b;            // light non-empty tile: one work unit
+            if (c[j] != 0u && m[j] == 0u) {                            // light non-empty tile: one work unit
+                const uint32_t gi = b / (uint32_t)g.ntiles, tile = b - gi * (uint32_t)g.ntiles;
+                const uint32_t ty = tile / (uint32_t)g.ntx;
+                work[wpos++] = make_uint4(b, gi, (ty << 16) | (tile - ty * (uint32_t)g.ntx), c[j]);
+            }
             for (uint32_t q = 0; q < m[j]; ++q) {
                 OwItem it;
                 it.bin = b; it.start = off + q * item_size; it.count = min(item_size, c[j] - q * item_size);
@@ -540,7 +544,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                                                           const uint32_t* __restrict__ bin_offset,
                                                           uint32_t* __restrict__ cursor, const OwItem* __restrict__ items,
                                                           const uint32_t* __restrict__ nitems,
-                                                          const uint32_t* __restrict__ work, uint32_t* __restrict__ ctl,
+                                                          const uint4* __restrict__ work, uint32_t* __restrict__ ctl,
                                                           const float* __restrict__ tt2, GridPtrs grids,
                                                           float* __restrict__ scratch, uint32_t* __restrict__ tickets,
                                                           float2* __restrict__ H, Stats* __restrict__ stats) {
@@ -553,6 +557,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     float* sT = reinterpret_cast<float*>(smem + kOwOffT);
     __shared__ uint32_t sW[8];
     __shared__ float sSum[8][3];
+    __shared__ float sScale[4];                                       // {scale v, scale w, 1/scale v, 1/scale w}
     __shared__ int sLast;
     __shared__ uint32_t sWork;
 
@@ -582,20 +587,22 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     __syncthreads();
     const uint32_t wi = sWork;
     if (wi >= n_work) break;
-    uint32_t bin, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
+    uint32_t bin, gi, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
+    int tx, ty;
     const bool heavy = wi < n_items;
     if (heavy) {
         const OwItem it = items[wi];
         bin = it.bin; start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
         if (chunk == 0 && tid == 0) cursor[bin] = 0;
+        gi = bin / (uint32_t)g.ntiles;
+        const uint32_t tile = bin - gi * (uint32_t)g.ntiles;
+        ty = (int)(tile / (uint32_t)g.ntx); tx = (int)(tile - (uint32_t)ty * (uint32_t)g.ntx);
     } else {
-        bin = work[wi - n_items];
+        const uint4 wk = __ldg(work + (wi - n_items));               // {bin, grid, ty << 16 | tx, count}
+        bin = wk.x; gi = wk.y; ty = (int)(wk.z >> 16); tx = (int)(wk.z & 0xFFFFu); cnt = wk.w;
         start = bin_offset[bin];
-        cnt = bin_offset[bin + 1] - start;
         if (tid == 0) cursor[bin] = 0;
     }
-    const uint32_t gi = bin / (uint32_t)g.ntiles, tile = bin - gi * (uint32_t)g.ntiles;
-    const int ty = (int)(tile / (uint32_t)g.ntx), tx = (int)(tile - (uint32_t)ty * (uint32_t)g.ntx);
     const int x0 = tx * kTile - kTile / 2, y0 = ty * kTile - kTile / 2;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
     float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
@@ -616,6 +623,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             s = make_float3(fabsf(__uint_as_float(q.x)), fabsf(__uint_as_float(q.y)), __uint_as_float(q.z));
         }
         sc = ow_scale_from(ow_warp_sum3(s));
+        if (tid == 0) { sScale[2] = 1.0f / sc.v; sScale[3] = 1.0f / sc.w; }
         __syncthreads();
         for (uint32_t i = warp; i < cnt; i += 8) {
             const uint4 rec = __ldg(recs + i);
@@ -650,10 +658,11 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 if (lane == 0) { sSum[warp][0] = t.x; sSum[warp][1] = t.y; sSum[warp][2] = t.z; }
             }
             __syncthreads();
-            if (ubase == 0) {
+            if (ubase == 0 && tid == 0) {
                 float3 t = make_float3(0.f, 0.f, 0.f);
                 for (int w = 0; w < 8; ++w) { t.x += sSum[w][0]; t.y += sSum[w][1]; t.z += sSum[w][2]; }
-                sc = ow_scale_from(t);
+                const OwScale q = ow_scale_from(t);
+                sScale[0] = q.v; sScale[1] = q.w; sScale[2] = 1.0f / q.v; sScale[3] = 1.0f / q.w;
             }
             {
                 const uint32_t h0 = sH[2 * tid], h1 = sH[2 * tid + 1];
@@ -670,6 +679,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 sH[2 * tid] = ex; sH[2 * tid + 1] = ex + h0;
             }
             __syncthreads();
+            sc.v = sScale[0]; sc.w = sScale[1];
             for (uint32_t i = tid; i < n; i += 256) {                  // bit 15: last record of its window
                 const uint32_t k = ow_sortkey(__ldg(&src[i].w)), pos = sH[k] + sP[i];
                 sI[pos] = (unsigned short)(i | ((pos + 1u == sH[k + 1u]) ? 0x8000u : 0u));
@@ -714,7 +724,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     }
 
     // (3) output: fixed point -> fp32
-    const float iv = 1.0f / sc.v, iw = 1.0f / sc.w;
+    const float iv = sScale[2], iw = sScale[3];
     float4* part = nullptr;
     if (heavy) part = reinterpret_cast<float4*>(scratch + (size_t)(first_slot + chunk) * kOwTileFloats);
     for (int i = tid; i < 32 * 16; i += 256) {
@@ -840,7 +850,7 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
 }
 
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
-                              uint32_t item_size, uint32_t* work, uint32_t* ctl, uint32_t* tops, cudaStream_t s) {
+                              uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops, cudaStream_t s) {
     const uint32_t nblocks = (g.nbins + 4095u) / 4096u;
     k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
     k_owner_scan_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems, ctl);
@@ -864,7 +874,7 @@ cudaError_t owner_kernel_setup(int max_smem_bytes) {
 }
 
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
-                              const OwItem* items, const uint32_t* nitems, const uint32_t* work, uint32_t* ctl,
+                              const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
                               const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, float2* H,
                               Stats* stats, int store_mode, int num_sms, cudaStream_t s) {
     const size_t smem = owner_smem_bytes(g.Q);
