@@ -294,6 +294,8 @@ def main():
                          f"{dt:.1f} s on {os.cpu_count()} available cores, 1 used",
                "images_per_s": done / dt}
 
+    limits = binding.microbench() if rank == 0 else None
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
@@ -309,6 +311,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps_timed": e2e_steps, "us_per_frame": 1e3 * e2e_ms / (e2e_steps * B)},
             "gpu_launches": int(launches), "clocks": sampler.result(), "roofline": roofline, "cpu_baseline": cpu,
+            "device_limits": limits,
         }
         print(json.dumps(line))
     im.destroy()

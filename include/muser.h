@@ -141,6 +141,11 @@ int muser_host_table(int kind, int support, int oversample, double param, double
 int muser_host_wtable(int support, int oversample, double w_lambda, double fov_rad, double* table_out_re_im);
 int muser_host_corrector(const double* table, int support, int oversample, int n, double* corr_out);
 const char* muser_version(void);
+/* Device microbenchmarks behind the roofline discussion; needs a GPU, synchronises the device.
+ * kind 0: FP32 FMA (flop/s), 1: packed FFMA2 (flop/s), 2: native 32-bit shared-memory integer adds (adds/s),
+ * 3: fp32 shared-memory adds = compare-and-swap loops (adds/s), 4: fp32 global reductions over 256 MB (adds/s).
+ * HOST output. */
+int muser_microbench(int kind, double* rate_out);
 
 #ifdef __cplusplus
 }

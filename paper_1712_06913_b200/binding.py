@@ -47,6 +47,7 @@ SIGNATURES = {
     "muser_host_wtable": (_i, [_i, _i, _d, _d, _vp]),
     "muser_host_corrector": (_i, [_vp, _i, _i, _i, _vp]),
     "muser_version": (_c.c_char_p, []),
+    "muser_microbench": (_i, [_i, _vp]),
 }
 
 _lib = None
@@ -230,6 +231,21 @@ def host_corrector(table, support, oversample, n):
     rc = lib().muser_host_corrector(t.ctypes.data, support, oversample, n, out.ctypes.data)
     if rc:
         raise MuserError(rc, "muser_host_corrector")
+    return out
+
+
+MICROBENCH = ("fp32_fma_flops", "fp32_ffma2_flops", "shared_int_adds", "shared_f32_cas_adds", "global_f32_red_adds")
+
+
+def microbench():
+    """Measured device limits (per second) the roofline discussion of DESIGN.md refers to."""
+    out = {}
+    for kind, name in enumerate(MICROBENCH):
+        v = ctypes.c_double()
+        rc = lib().muser_microbench(kind, ctypes.byref(v))
+        if rc:
+            raise MuserError(rc, "muser_microbench")
+        out[name] = v.value
     return out
 
 

@@ -330,3 +330,11 @@ def test_abi_argument_errors_on_device():
         assert L.muser_set_wplanes(h, 2, None, None, None) == binding.MUSER_EINVAL
     finally:
         im.destroy()
+
+
+def test_microbenchmarks_report_plausible_device_limits():
+    mb = binding.microbench()
+    assert set(mb) == set(binding.MICROBENCH)
+    assert 1e13 < mb["fp32_fma_flops"] < 1.2e14                  # B200: 148 SMs x 128 lanes x 2 x <= 1.965 GHz = 74.5e12
+    assert mb["shared_int_adds"] > 1.5 * mb["shared_f32_cas_adds"] > 0   # why the owner gridder merges in fixed point
+    assert mb["global_f32_red_adds"] > 1e11
