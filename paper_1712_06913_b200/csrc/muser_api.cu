@@ -137,6 +137,9 @@ int rebuild_geom(muser_imager* h) {
     g.chunk = 512;
     g.S = h->planes_h.empty() ? h->S : h->planes_h[0].support;
     g.ntiles = g.nty * g.ntx;
+    g.otx = (h->nx - 1 + kOwTileW / 2) / kOwTileW + 1;
+    g.ontiles = g.nty * g.otx;
+    g.onbins = (uint32_t)h->ngrids * (uint32_t)g.ontiles;
     return MUSER_OK;
 }
 
@@ -310,7 +313,7 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
         CU(h, cudaMalloc(&h->ow_loc, (cap / 8 + 1) * sizeof(uint4)));
         h->ow_sorted_cap = cap;
     }
-    const size_t nb = ((size_t)h->geom.nbins + 8) & ~(size_t)3;
+    const size_t nb = ((size_t)h->geom.onbins + 8) & ~(size_t)3;
     if (nb > h->ow_bins_cap) {
         cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
         h->ow_count = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
@@ -351,7 +354,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         uint32_t max_items = 0;
         int rc = ensure_owner_scratch(h, nvis, item_size, &max_items);
         if (rc) return rc;
-        if (g.nty > 65535 || g.ntx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
+        if (g.nty > 65535 || g.otx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
         h->last_stream = s;
         h->fft_valid = false;
         {

@@ -20,6 +20,8 @@ struct Geom {
     int chunk;                     // samples per work item of the tiled gridder
     int S;                         // support of plane 0 (the 2-D kernel)
     int ntiles;                    // nty*ntx
+    int otx, ontiles;              // owner-tile path: tiles per row (kOwTileW cells wide), tiles per grid
+    uint32_t onbins;               // ngrids*ontiles
 };
 
 // Per-plane kernel metadata in constant-ish device memory.
@@ -85,7 +87,8 @@ cudaError_t tiled_kernel_setup(int max_smem_bytes);
 // writer, so the grids are written with plain stores (no memset, no global atomics); samples whose footprint
 // crosses a tile edge are listed in every tile they touch.
 constexpr int kOwSub = 1024;                 // samples staged and cell-sorted in shared memory per pass
-constexpr int kOwTileFloats = 32 * 32 * 3;   // one partial tile in the scratch buffer: A[32][32] float2 + B[32][32] float
+constexpr int kOwTileW = 64;                 // owner tiles are 64 cells wide, 32 tall
+constexpr int kOwTileFloats = kOwTileW * 32 * 3;   // one partial tile in the scratch buffer: A[32][W] float2 + B[32][W] float
 // two-parity transposed table TT2[(par*(Q+1) + r)*8 + i]: par 0: i = j (j = 0..6: T[j*Q + r]), [7] = 0;
 // par 1: [0] = 0, i = j + 1
 struct OwItem {                              // one chunk of a heavy tile (more than item_size samples)

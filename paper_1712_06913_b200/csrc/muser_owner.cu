@@ -27,6 +27,14 @@ namespace muser {
 static constexpr double kC = 299792458.0;   // m/s
 static constexpr unsigned kFull = 0xffffffffu;
 
+// Owner tiles are kOwTW cells wide (x) and kTile = 32 cells tall (y): tile (tx, ty) covers cells
+// [kOwTW*tx - kOwTW/2, ...) x [32*ty - 16, ...), so the uv origin sits in the middle of a tile.  Wider tiles mean fewer
+// records listed twice (halo duplication 1.33 -> 1.19 on MUSER frames) and half as many tiles to set up and store.
+constexpr int kOwTW = kOwTileW, kOwTWS = kOwTW == 64 ? 6 : 5;
+constexpr int kOwNKX = (kOwTW + 6) / 2;          // 8-wide windows per tile row incl. halo: 19 (32-wide) or 35 (64-wide)
+constexpr int kOwKXB = kOwTWS;                   // bits of the window column index in a record
+constexpr uint32_t kOwKeyMask = (1u << (5 + kOwKXB)) - 1u;
+
 // ------------------------------------------------------------------------------------------------- coordinates
 // O1 for one axis (same operation order as the oracle; _rn intrinsics forbid FMA contraction).
 __device__ __forceinline__ void ow_cell_phase(double c_lambda, double scale, int n, int Q, double& i0, double& r) {
@@ -81,12 +89,12 @@ __device__ __forceinline__ void ow_locate(const Geom& g, const float* __restrict
 // Bin of the q-th tile (q = qx | qy << 1) touched by the footprint of a sample at nearest cell (cu, cv), or kNoBin.
 __device__ __forceinline__ uint32_t ow_bin(const Geom& g, int gid, int cu, int cv, int q, int& tx, int& ty) {
     const int h = (g.S - 1) >> 1;
-    const int tx0 = (cu - h + kTile / 2) >> kTileShift, tx1 = (cu + h + kTile / 2) >> kTileShift;
+    const int tx0 = (cu - h + kOwTW / 2) >> kOwTWS, tx1 = (cu + h + kOwTW / 2) >> kOwTWS;
     const int ty0 = (cv - h + kTile / 2) >> kTileShift, ty1 = (cv + h + kTile / 2) >> kTileShift;
     if (((q & 1) && tx1 == tx0) || ((q & 2) && ty1 == ty0)) return kNoBin;
     tx = (q & 1) ? tx1 : tx0;
     ty = (q & 2) ? ty1 : ty0;
-    return (uint32_t)gid * (uint32_t)g.ntiles + (uint32_t)(ty * g.ntx + tx);
+    return (uint32_t)gid * (uint32_t)g.ontiles + (uint32_t)(ty * g.otx + tx);
 }
 
 // Warp-aggregated counter increment: lanes with the same bin issue one atomicAdd; returns the lane's rank.
@@ -123,11 +131,11 @@ struct OwTiles { int tx0, ty0, t00; bool mx, my; };
 __device__ __forceinline__ OwTiles ow_tiles(const Geom& g, int cu, int cv) {
     const int h = (g.S - 1) >> 1;
     OwTiles t;
-    t.tx0 = (cu - h + kTile / 2) >> kTileShift;
+    t.tx0 = (cu - h + kOwTW / 2) >> kOwTWS;
     t.ty0 = (cv - h + kTile / 2) >> kTileShift;
-    t.mx = ((cu + h + kTile / 2) >> kTileShift) != t.tx0;
+    t.mx = ((cu + h + kOwTW / 2) >> kOwTWS) != t.tx0;
     t.my = ((cv + h + kTile / 2) >> kTileShift) != t.ty0;
-    t.t00 = t.ty0 * g.ntx + t.tx0;
+    t.t00 = t.ty0 * g.otx + t.tx0;
     return t;
 }
 
@@ -161,23 +169,23 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
         w2sum = (double)L.wt * (double)L.wt;
         v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
     }
-    const int use_smem = ow_cta_uniform_grid(L, g.ntiles, s_flag);
+    const int use_smem = ow_cta_uniform_grid(L, g.ontiles, s_flag);
     if (use_smem) {
-        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) s_hist[i] = 0;
+        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
-        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ntiles;
+        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ontiles;
         if (kept) {
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 const OwTiles t = ow_tiles(g, L.cu[s], L.cv[s]);
                 atomicAdd(&s_hist[t.t00], 1u);
                 if (t.mx) atomicAdd(&s_hist[t.t00 + 1], 1u);
-                if (t.my) atomicAdd(&s_hist[t.t00 + g.ntx], 1u);
-                if (t.mx && t.my) atomicAdd(&s_hist[t.t00 + g.ntx + 1], 1u);
+                if (t.my) atomicAdd(&s_hist[t.t00 + g.otx], 1u);
+                if (t.mx && t.my) atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u);
             }
         }
         __syncthreads();
-        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) {
+        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) {
             const uint32_t n = s_hist[i];
             if (n) atomicAdd(&bin_count[gbase + i], n);
         }
@@ -261,7 +269,7 @@ __device__ __forceinline__ OwScan3 ow_block_scan3(OwScan3 v, OwScan3& total, uin
 __device__ __forceinline__ OwScan3 ow_load4(const Geom& g, const uint32_t* __restrict__ bin_count, uint32_t b0,
                                             uint32_t item_size, uint32_t c[4], uint32_t m[4]) {
     c[0] = c[1] = c[2] = c[3] = 0;
-    if (b0 < g.nbins) {                                                // bin_count is padded to a multiple of 4
+    if (b0 < g.onbins) {                                                // bin_count is padded to a multiple of 4
         const uint4 v = *reinterpret_cast<const uint4*>(bin_count + b0);
         c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
     }
@@ -298,7 +306,7 @@ __global__ void __launch_bounds__(1024) k_owner_scan_tops(const Geom g, const ui
         if (b < nblocks) { tops[3 * b] = carry.c + ex.c; tops[3 * b + 1] = carry.m + ex.m; tops[3 * b + 2] = carry.l + ex.l; }
         carry.c += total.c; carry.m += total.m; carry.l += total.l;
     }
-    if (threadIdx.x == 0) { bin_offset[g.nbins] = carry.c; *nitems = carry.m; ctl[0] = carry.l; ctl[1] = 0; }
+    if (threadIdx.x == 0) { bin_offset[g.onbins] = carry.c; *nitems = carry.m; ctl[0] = carry.l; ctl[1] = 0; }
 }
 
 __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_t* __restrict__ bin_count,
@@ -316,12 +324,12 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const uint32_t b = b0 + j;
-        if (b < g.nbins) {
+        if (b < g.onbins) {
             bin_offset[b] = off;
             if (c[j] != 0u && m[j] == 0u) {                            // light non-empty tile: one work unit
-                const uint32_t gi = b / (uint32_t)g.ntiles, tile = b - gi * (uint32_t)g.ntiles;
-                const uint32_t ty = tile / (uint32_t)g.ntx;
-                work[wpos++] = make_uint4(b, gi, (ty << 16) | (tile - ty * (uint32_t)g.ntx), c[j]);
+                const uint32_t gi = b / (uint32_t)g.ontiles, tile = b - gi * (uint32_t)g.ontiles;
+                const uint32_t ty = tile / (uint32_t)g.otx;
+                work[wpos++] = make_uint4(b, gi, (ty << 16) | (tile - ty * (uint32_t)g.otx), c[j]);
             }
             for (uint32_t q = 0; q < m[j]; ++q) {
                 OwItem it;
@@ -342,7 +350,7 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
 // table TT2 (rx = Q/2 - ru, ry = Q/2 - rv in [0, Q]).
 __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, int s, int tx, int ty, uint4* dst) {
     const int h = (g.S - 1) >> 1;
-    const int ox = L.cu[s] - (tx * kTile - kTile / 2) + h;
+    const int ox = L.cu[s] - (tx * kOwTW - kOwTW / 2) + h;
     const int oy = L.cv[s] - (ty * kTile - kTile / 2) + h;
     uint4 o;
     o.x = __float_as_uint(L.re);
@@ -350,7 +358,7 @@ __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, i
     o.z = __float_as_uint(L.wt);
     const uint32_t X = (uint32_t)((ox & 1) * (g.Q + 1) + L.rx[s]);
     const uint32_t Y = (uint32_t)((oy & 1) * (g.Q + 1) + L.ry[s]);
-    o.w = (uint32_t)((oy >> 1) << 5 | ox >> 1) | (X << 10) | (Y << 20);
+    o.w = (uint32_t)((oy >> 1) << kOwKXB | ox >> 1) | (X << (5 + kOwKXB)) | (Y << (15 + kOwKXB));
     *dst = o;
 }
 
@@ -379,12 +387,12 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
         }
     }
     const int kept = L.state == 3;
-    const int use_smem = ow_cta_uniform_grid(L, g.ntiles, s_flag);
+    const int use_smem = ow_cta_uniform_grid(L, g.ontiles, s_flag);
     if (use_smem) {
-        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) s_hist[i] = 0;
+        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
-        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ntiles;
-        uint32_t* s_base = s_hist + g.ntiles;                         // global position of this CTA's run in each tile
+        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ontiles;
+        uint32_t* s_base = s_hist + g.ontiles;                         // global position of this CTA's run in each tile
         OwTiles T[2];
         uint32_t rk[2][4];
         if (kept) {
@@ -393,12 +401,12 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
                 T[s] = ow_tiles(g, L.cu[s], L.cv[s]);
                 rk[s][0] = atomicAdd(&s_hist[T[s].t00], 1u);
                 if (T[s].mx) rk[s][1] = atomicAdd(&s_hist[T[s].t00 + 1], 1u);
-                if (T[s].my) rk[s][2] = atomicAdd(&s_hist[T[s].t00 + g.ntx], 1u);
-                if (T[s].mx && T[s].my) rk[s][3] = atomicAdd(&s_hist[T[s].t00 + g.ntx + 1], 1u);
+                if (T[s].my) rk[s][2] = atomicAdd(&s_hist[T[s].t00 + g.otx], 1u);
+                if (T[s].mx && T[s].my) rk[s][3] = atomicAdd(&s_hist[T[s].t00 + g.otx + 1], 1u);
             }
         }
         __syncthreads();
-        for (int i = threadIdx.x; i < g.ntiles; i += blockDim.x) {     // reserve this CTA's run in each touched tile
+        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) {     // reserve this CTA's run in each touched tile
             const uint32_t n = s_hist[i];
             if (n) s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n);
         }
@@ -409,9 +417,9 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
                 const OwTiles t = T[s];
                 ow_write_record(g, L, s, t.tx0, t.ty0, sorted + s_base[t.t00] + rk[s][0]);
                 if (t.mx) ow_write_record(g, L, s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + rk[s][1]);
-                if (t.my) ow_write_record(g, L, s, t.tx0, t.ty0 + 1, sorted + s_base[t.t00 + g.ntx] + rk[s][2]);
+                if (t.my) ow_write_record(g, L, s, t.tx0, t.ty0 + 1, sorted + s_base[t.t00 + g.otx] + rk[s][2]);
                 if (t.mx && t.my)
-                    ow_write_record(g, L, s, t.tx0 + 1, t.ty0 + 1, sorted + s_base[t.t00 + g.ntx + 1] + rk[s][3]);
+                    ow_write_record(g, L, s, t.tx0 + 1, t.ty0 + 1, sorted + s_base[t.t00 + g.otx + 1] + rk[s][3]);
             }
         }
         return;
@@ -446,8 +454,9 @@ __device__ __forceinline__ unsigned long long ow_fma2(unsigned long long a, unsi
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
 }
-constexpr int kOwPitch = 40;      // cells per row of the shared tile: 32 + 8 pad
-constexpr int kOwKeys = 512;      // 19 x 19 = 361 windows, padded to 2 per thread
+constexpr int kOwPitch = kOwTW + 8; // cells per row of the shared tile (8 pad)
+constexpr int kOwKPT = (19 * kOwNKX + 1 + 255) / 256;   // window keys per thread in the scan (2 or 3)
+constexpr int kOwKeys = 256 * kOwKPT;                   // 19 x kOwNKX windows (+1 end marker), padded
 constexpr int kOwDirect = 32;     // tiles with at most this many samples skip the shared-memory sort
 constexpr int kOwUnit = 4096;     // samples counting-sorted together
 
@@ -476,8 +485,8 @@ struct OwWarpAcc {
 
 // Point the warp's 8 x 8 register window at window `key`; lane (r, c) holds row r, columns 2c and 2c + 1.
 __device__ __forceinline__ void ow_window(OwWarpAcc& A, const uint32_t key, const int r, const int c) {
-    const int row = 2 * (int)(key >> 5) - 6 + r, col0 = 2 * (int)(key & 31u) - 6 + 2 * c;
-    A.off = (((unsigned)row < 32u) && ((unsigned)col0 < 32u)) ? row * kOwPitch + col0 : -1;
+    const int row = 2 * (int)(key >> kOwKXB) - 6 + r, col0 = 2 * (int)(key & ((1u << kOwKXB) - 1u)) - 6 + 2 * c;
+    A.off = (((unsigned)row < 32u) && ((unsigned)col0 < (unsigned)kOwTW)) ? row * kOwPitch + col0 : -1;
     A.a0 = A.a1 = A.b = 0ull;
 }
 
@@ -503,7 +512,7 @@ __device__ __forceinline__ uint4 ow_stage(const uint4 rec, const OwScale sc) {
     st.x = __float_as_uint(__uint_as_float(rec.x) * sc.v);
     st.y = __float_as_uint(__uint_as_float(rec.y) * sc.v);
     st.z = __float_as_uint(__uint_as_float(rec.z) * sc.w);
-    st.w = ((rec.w >> 5) & 0x7FE0u) | (((rec.w >> 15) & 0x7FE0u) << 16);
+    st.w = ((rec.w >> kOwKXB) & 0x7FE0u) | (((rec.w >> (10 + kOwKXB)) & 0x7FE0u) << 16);
     return st;
 }
 
@@ -519,7 +528,9 @@ __device__ __forceinline__ void ow_add(OwWarpAcc& A, const uint4 st, const char*
     A.b = ow_fma2(ow_pack(k0, k1), ow_pack(wt, wt), A.b);
 }
 
-__device__ __forceinline__ uint32_t ow_sortkey(uint32_t w) { return ((w >> 5) & 31u) * 19u + (w & 31u); }
+__device__ __forceinline__ uint32_t ow_sortkey(uint32_t w) {
+    return ((w >> kOwKXB) & 31u) * (uint32_t)kOwNKX + (w & ((1u << kOwKXB) - 1u));
+}
 
 __device__ __forceinline__ float3 ow_warp_sum3(float3 a) {
     for (int o = 16; o > 0; o >>= 1) {
@@ -594,16 +605,16 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         const OwItem it = items[wi];
         bin = it.bin; start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
         if (chunk == 0 && tid == 0) cursor[bin] = 0;
-        gi = bin / (uint32_t)g.ntiles;
-        const uint32_t tile = bin - gi * (uint32_t)g.ntiles;
-        ty = (int)(tile / (uint32_t)g.ntx); tx = (int)(tile - (uint32_t)ty * (uint32_t)g.ntx);
+        gi = bin / (uint32_t)g.ontiles;
+        const uint32_t tile = bin - gi * (uint32_t)g.ontiles;
+        ty = (int)(tile / (uint32_t)g.otx); tx = (int)(tile - (uint32_t)ty * (uint32_t)g.otx);
     } else {
         const uint4 wk = __ldg(work + (wi - n_items));               // {bin, grid, ty << 16 | tx, count}
         bin = wk.x; gi = wk.y; ty = (int)(wk.z >> 16); tx = (int)(wk.z & 0xFFFFu); cnt = wk.w;
         start = bin_offset[bin];
         if (tid == 0) cursor[bin] = 0;
     }
-    const int x0 = tx * kTile - kTile / 2, y0 = ty * kTile - kTile / 2;
+    const int x0 = tx * kOwTW - kOwTW / 2, y0 = ty * kTile - kTile / 2;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
     float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
     float2* __restrict__ Ht = H + (size_t)gi * g.ny * g.nx;
@@ -627,7 +638,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         __syncthreads();
         for (uint32_t i = warp; i < cnt; i += 8) {
             const uint4 rec = __ldg(recs + i);
-            ow_window(A, rec.w & 0x3FFu, r, c);
+            ow_window(A, rec.w & kOwKeyMask, r, c);
             ow_add(A, ow_stage(rec, sc), tbx, tby);
             ow_flush(A, sA, sB);
         }
@@ -665,8 +676,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 sScale[0] = q.v; sScale[1] = q.w; sScale[2] = 1.0f / q.v; sScale[3] = 1.0f / q.w;
             }
             {
-                const uint32_t h0 = sH[2 * tid], h1 = sH[2 * tid + 1];
-                const uint32_t tot = h0 + h1;
+                uint32_t hk[kOwKPT], tot = 0;
+#pragma unroll
+                for (int j = 0; j < kOwKPT; ++j) { hk[j] = sH[kOwKPT * tid + j]; tot += hk[j]; }
                 uint32_t inc = tot;
                 for (int o = 1; o < 32; o <<= 1) {
                     const uint32_t t = __shfl_up_sync(kFull, inc, o);
@@ -676,7 +688,8 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 __syncthreads();
                 uint32_t ex = inc - tot;
                 for (int w = 0; w < warp; ++w) ex += sW[w];
-                sH[2 * tid] = ex; sH[2 * tid + 1] = ex + h0;
+#pragma unroll
+                for (int j = 0; j < kOwKPT; ++j) { sH[kOwKPT * tid + j] = ex; ex += hk[j]; }
             }
             __syncthreads();
             sc.v = sScale[0]; sc.w = sScale[1];
@@ -699,7 +712,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 while (p < e) {
                     const int m = min(32, e - p);
                     wb[buf * 32 + lane] = ow_stage(nxt, sc);
-                    const uint32_t mykey = nxt.w & 0x3FFu;
+                    const uint32_t mykey = nxt.w & kOwKeyMask;
                     // a run ends at the last record of its window and at the end of the batch
                     uint32_t ends = __ballot_sync(kFull, (nidx >> 15) != 0u || lane == m - 1);
                     __syncwarp();
@@ -727,8 +740,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     const float iv = sScale[2], iw = sScale[3];
     float4* part = nullptr;
     if (heavy) part = reinterpret_cast<float4*>(scratch + (size_t)(first_slot + chunk) * kOwTileFloats);
-    for (int i = tid; i < 32 * 16; i += 256) {
-        const int row = i >> 4, c2 = i & 15, gx = x0 + 2 * c2, gy = y0 + row;
+    constexpr int kG4 = kOwTW / 2, kW4 = kOwTW / 4;                   // float4 per tile row of G / H and of Gw
+    for (int i = tid; i < 32 * kG4; i += 256) {
+        const int row = i / kG4, c2 = i % kG4, gx = x0 + 2 * c2, gy = y0 + row;
         const int4 a = *reinterpret_cast<const int4*>(sA + 2 * (row * kOwPitch + 2 * c2));
         float4 v = make_float4((float)a.x * iv, (float)a.y * iv, (float)a.z * iv, (float)a.w * iv);
         if (heavy) {
@@ -745,12 +759,12 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             }
         }
     }
-    {
-        const int row = tid >> 3, c4 = tid & 7, gx = x0 + 4 * c4, gy = y0 + row;
+    for (int i = tid; i < 32 * kW4; i += 256) {
+        const int row = i / kW4, c4 = i % kW4, gx = x0 + 4 * c4, gy = y0 + row;
         const int4 a = *reinterpret_cast<const int4*>(sB + row * kOwPitch + 4 * c4);
         float4 v = make_float4((float)a.x * iw, (float)a.y * iw, (float)a.z * iw, (float)a.w * iw);
         if (heavy) {
-            __stcg(part + 512 + tid, v);
+            __stcg(part + 32 * kG4 + i, v);
         } else if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
             float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
             if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
@@ -770,13 +784,14 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     __threadfence();
     const float4* parts = reinterpret_cast<const float4*>(scratch + (size_t)first_slot * kOwTileFloats);
     float* sWsum = reinterpret_cast<float*>(smem + kOwOffB);          // summed weight tile, dense [32][32], for H
-    for (int i = 512 + tid; i < 32 * 16 + 256; i += 256) {            // weights first
+    for (int j = tid; j < 32 * kW4; j += 256) {                       // weights first
+        const int i = 32 * kG4 + j;
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
         for (uint32_t q = 0; q < nchunks; ++q) {
             const float4 p = __ldcg(parts + (size_t)q * (kOwTileFloats / 4) + i);
             v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
         }
-        const int j = i - 512, gx = x0 + 4 * (j & 7), gy = y0 + (j >> 3);
+        const int gx = x0 + 4 * (j % kW4), gy = y0 + (j / kW4);
         if (STORE) *reinterpret_cast<float4*>(sWsum + 4 * j) = v;
         if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
             float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
@@ -785,13 +800,13 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         }
     }
     __syncthreads();
-    for (int i = tid; i < 32 * 16; i += 256) {
+    for (int i = tid; i < 32 * kG4; i += 256) {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
         for (uint32_t q = 0; q < nchunks; ++q) {
             const float4 p = __ldcg(parts + (size_t)q * (kOwTileFloats / 4) + i);
             v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
         }
-        const int gx = x0 + 2 * (i & 15), gy = y0 + (i >> 4);
+        const int gx = x0 + 2 * (i % kG4), gy = y0 + (i / kG4);
         if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
             float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
             if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
@@ -815,8 +830,8 @@ __global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t
                                                     GridPtrs grids, float2* __restrict__ H) {
     __shared__ unsigned char s_empty[1024 + 8];
     const int gi = blockIdx.x, ty = blockIdx.y;
-    const uint32_t bin0 = (uint32_t)gi * (uint32_t)g.ntiles + (uint32_t)ty * (uint32_t)g.ntx;
-    for (int t = threadIdx.x; t < g.ntx; t += blockDim.x) s_empty[t] = bin_offset[bin0 + t + 1] == bin_offset[bin0 + t];
+    const uint32_t bin0 = (uint32_t)gi * (uint32_t)g.ontiles + (uint32_t)ty * (uint32_t)g.otx;
+    for (int t = threadIdx.x; t < g.otx; t += blockDim.x) s_empty[t] = bin_offset[bin0 + t + 1] == bin_offset[bin0 + t];
     __syncthreads();
     const int y0 = max(ty * kTile - kTile / 2, 0), y1 = min(ty * kTile + kTile / 2, g.ny);
     const int nx2 = g.nx >> 1, nx4 = g.nx >> 2;
@@ -824,14 +839,14 @@ __global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t
     const size_t row0 = ((size_t)gi * g.ny + y0) * (size_t)g.nx;
     // a thread owns column chunks: the emptiness test is done once per chunk, the loop over the rows only stores
     for (int i = threadIdx.x; i < nx2; i += blockDim.x) {              // 2 cells of G / H per store
-        if (!s_empty[(2 * i + kTile / 2) >> kTileShift]) continue;
+        if (!s_empty[(2 * i + kOwTW / 2) >> kOwTWS]) continue;
         float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row0) + i;
         float4* __restrict__ hr = reinterpret_cast<float4*>(H + row0) + i;
 #pragma unroll 4
         for (int y = y0; y < y1; ++y, gr += nx2, hr += nx2) { *gr = z; *hr = z; }
     }
     for (int i = threadIdx.x; i < nx4; i += blockDim.x) {              // 4 cells of Gw per store
-        if (!s_empty[(4 * i + kTile / 2) >> kTileShift]) continue;
+        if (!s_empty[(4 * i + kOwTW / 2) >> kOwTWS]) continue;
         float4* __restrict__ wr = reinterpret_cast<float4*>(grids.Gw + row0) + i;
 #pragma unroll 4
         for (int y = y0; y < y1; ++y, wr += nx4) *wr = z;
@@ -839,7 +854,7 @@ __global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t
 }
 
 // ------------------------------------------------------------------------------------------------- launchers
-static size_t bin_smem_bytes(const Geom& g) { return g.ntiles <= kBinSmemTiles ? (size_t)2 * g.ntiles * sizeof(uint32_t) : 0; }
+static size_t bin_smem_bytes(const Geom& g) { return g.ontiles <= kBinSmemTiles ? (size_t)2 * g.ontiles * sizeof(uint32_t) : 0; }
 
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                                const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, uint4* loc,
@@ -851,7 +866,7 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
 
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
                               uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops, cudaStream_t s) {
-    const uint32_t nblocks = (g.nbins + 4095u) / 4096u;
+    const uint32_t nblocks = (g.onbins + 4095u) / 4096u;
     k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
     k_owner_scan_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems, ctl);
     k_owner_scan_write<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops, bin_offset, items, work);
