@@ -371,7 +371,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
                                     h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->H, h->stats_d,
                                     h->zero_pending ? 1 : 0, h->num_sms, s));
         }
-        h->n_launches += h->zero_pending ? 7 : 6;                     // count, 3 x scan, scatter, (fill,) grid
+        h->n_launches += 6;                                           // count, 3 x scan, scatter, grid
         h->h_packed = h->zero_pending;                                // store mode also wrote the FFT input H
         h->zero_pending = false;                                      // store mode wrote every tile of every grid
         return MUSER_OK;

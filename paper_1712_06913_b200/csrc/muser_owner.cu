@@ -7,9 +7,10 @@
 //   O2  k_owner_scan_*     A1: multi-CTA exclusive scan of the histogram (3 small launches): sample offsets, chunk
 //                              items of heavy tiles (> item_size samples), work list of light non-empty tiles
 //   O3  k_owner_scatter    A1: reads O1's integer result and writes one 16-byte record per (sample, touched tile)
-//   O4a k_owner_fill       A2: store mode only: zeroes the EMPTY tiles of G, Gw and H in long contiguous runs
+//   O4a ow_fill_row        A2: store mode only: zero-fill units (one per grid and row of tiles) in the gridder's work
+//                              queue zero the EMPTY tiles of G, Gw and H in long contiguous runs
 //   O4  k_grid_owner_s7    A2/A4: persistent kernel, 4 CTAs per SM pulling work units (chunks of heavy tiles first,
-//                              then light tiles) from a device counter.  Per unit: counting sort of <= 4096 records by
+//                              then light 64x32 tiles interleaved with the fill units) from a device counter.  Per unit: counting sort of <= 4096 records by
 //                              8x8 window (shared histogram, 2-byte positions); every warp then streams an equal share
 //                              of the sorted order through a private 2 x 32-record buffer (gather loads one batch
 //                              ahead, records staged in fixed-point units with table row offsets); a run of equal
@@ -547,9 +548,37 @@ __device__ __forceinline__ OwScale ow_scale_from(float3 s) {
     return sc;
 }
 
+// ------------------------------------------------------------------------------------------------- O4a fill
+// STORE mode: zero the EMPTY tiles of one row of tiles of one grid in G, Gw and H, as long contiguous runs of each
+// cell row (16-byte stores, consecutive threads -> consecutive addresses).  A thread owns column chunks: the emptiness
+// test is done once per chunk, the loop over the rows only stores.  Called by all 256 threads of a CTA.
+__device__ __forceinline__ void ow_fill_row(const Geom& g, const uint32_t* __restrict__ bin_offset, GridPtrs grids,
+                                            float2* __restrict__ H, const int gi, const int ty, unsigned char* s_empty) {
+    const uint32_t bin0 = (uint32_t)gi * (uint32_t)g.ontiles + (uint32_t)ty * (uint32_t)g.otx;
+    for (int t = threadIdx.x; t < g.otx; t += blockDim.x) s_empty[t] = bin_offset[bin0 + t + 1] == bin_offset[bin0 + t];
+    __syncthreads();
+    const int y0 = max(ty * kTile - kTile / 2, 0), y1 = min(ty * kTile + kTile / 2, g.ny);
+    const int nx2 = g.nx >> 1, nx4 = g.nx >> 2;
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    const size_t row0 = ((size_t)gi * g.ny + y0) * (size_t)g.nx;
+    for (int i = threadIdx.x; i < nx2; i += blockDim.x) {              // 2 cells of G / H per store
+        if (!s_empty[(2 * i + kOwTW / 2) >> kOwTWS]) continue;
+        float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row0) + i;
+        float4* __restrict__ hr = reinterpret_cast<float4*>(H + row0) + i;
+#pragma unroll 4
+        for (int y = y0; y < y1; ++y, gr += nx2, hr += nx2) { *gr = z; *hr = z; }
+    }
+    for (int i = threadIdx.x; i < nx4; i += blockDim.x) {              // 4 cells of Gw per store
+        if (!s_empty[(4 * i + kOwTW / 2) >> kOwTWS]) continue;
+        float4* __restrict__ wr = reinterpret_cast<float4*>(grids.Gw + row0) + i;
+#pragma unroll 4
+        for (int y = y0; y < y1; ++y, wr += nx4) *wr = z;
+    }
+}
+
 // Persistent kernel: 4 CTAs per SM pull work units from a device-side counter.  Units [0, nitems) are the chunk items
 // of heavy tiles (started first), units [nitems, nitems + nlight) the light non-empty tiles listed by k_owner_scan.
-// Empty tiles are zeroed by k_owner_fill (STORE mode) and never reach this kernel.
+// In STORE mode the zero-fill units of the empty tiles are part of the same queue.
 template <int STORE>
 __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
                                                           const uint32_t* __restrict__ bin_offset,
@@ -590,7 +619,13 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     const int r = lane >> 2, c = lane & 3;
     const char* tbx = reinterpret_cast<const char*>(sT + 2 * c);
     const char* tby = reinterpret_cast<const char*>(sT + r);
-    const uint32_t n_items = *nitems, n_work = n_items + ctl[0];
+    // Work units: [0, n_items) chunks of heavy tiles; then n_light light tiles with, in STORE mode, the n_fill
+    // zero-fill units (one per grid and row of tiles) spread evenly between them (every k-th position), so that the
+    // store-bound fills and the issue-bound gridding units are resident on an SM at the same time.
+    const uint32_t n_items = *nitems, n_light = ctl[0];
+    const uint32_t n_fill = STORE ? (uint32_t)g.ngrids * (uint32_t)g.nty : 0u;
+    const uint32_t n_rest = n_light + n_fill, n_work = n_items + n_rest;
+    const uint32_t kfill = n_fill ? max(n_rest / n_fill, 1u) : 1u;
 
   for (;;) {
     __syncthreads();                                                  // the previous unit is done with the shared tile
@@ -601,6 +636,16 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     uint32_t bin, gi, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
     int tx, ty;
     const bool heavy = wi < n_items;
+    uint32_t li = wi - n_items;                                       // index into the light-tile list
+    if (STORE && !heavy) {
+        const uint32_t j = li, f = j / kfill;
+        if (f < n_fill && j == f * kfill) {                           // fill unit f: zero the empty tiles of one tile row
+            ow_fill_row(g, bin_offset, grids, H, (int)(f / (uint32_t)g.nty), (int)(f % (uint32_t)g.nty),
+                        reinterpret_cast<unsigned char*>(sH));
+            continue;
+        }
+        li = j - min(n_fill, f + 1u);
+    }
     if (heavy) {
         const OwItem it = items[wi];
         bin = it.bin; start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
@@ -609,7 +654,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         const uint32_t tile = bin - gi * (uint32_t)g.ontiles;
         ty = (int)(tile / (uint32_t)g.otx); tx = (int)(tile - (uint32_t)ty * (uint32_t)g.otx);
     } else {
-        const uint4 wk = __ldg(work + (wi - n_items));               // {bin, grid, ty << 16 | tx, count}
+        const uint4 wk = __ldg(work + li);                           // {bin, grid, ty << 16 | tx, count}
         bin = wk.x; gi = wk.y; ty = (int)(wk.z >> 16); tx = (int)(wk.z & 0xFFFFu); cnt = wk.w;
         start = bin_offset[bin];
         if (tid == 0) cursor[bin] = 0;
@@ -822,37 +867,6 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
   }
 }
 
-// ------------------------------------------------------------------------------------------------- O4a fill
-// STORE mode: zero the EMPTY tiles of G, Gw and H.  One CTA per (grid, row of tiles): the empty tiles of a tile row
-// are written as long contiguous runs of each cell row (16-byte stores, consecutive threads -> consecutive
-// addresses), a streaming pattern that runs at the copy bandwidth.
-__global__ void __launch_bounds__(256) k_owner_fill(const Geom g, const uint32_t* __restrict__ bin_offset,
-                                                    GridPtrs grids, float2* __restrict__ H) {
-    __shared__ unsigned char s_empty[1024 + 8];
-    const int gi = blockIdx.x, ty = blockIdx.y;
-    const uint32_t bin0 = (uint32_t)gi * (uint32_t)g.ontiles + (uint32_t)ty * (uint32_t)g.otx;
-    for (int t = threadIdx.x; t < g.otx; t += blockDim.x) s_empty[t] = bin_offset[bin0 + t + 1] == bin_offset[bin0 + t];
-    __syncthreads();
-    const int y0 = max(ty * kTile - kTile / 2, 0), y1 = min(ty * kTile + kTile / 2, g.ny);
-    const int nx2 = g.nx >> 1, nx4 = g.nx >> 2;
-    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-    const size_t row0 = ((size_t)gi * g.ny + y0) * (size_t)g.nx;
-    // a thread owns column chunks: the emptiness test is done once per chunk, the loop over the rows only stores
-    for (int i = threadIdx.x; i < nx2; i += blockDim.x) {              // 2 cells of G / H per store
-        if (!s_empty[(2 * i + kOwTW / 2) >> kOwTWS]) continue;
-        float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row0) + i;
-        float4* __restrict__ hr = reinterpret_cast<float4*>(H + row0) + i;
-#pragma unroll 4
-        for (int y = y0; y < y1; ++y, gr += nx2, hr += nx2) { *gr = z; *hr = z; }
-    }
-    for (int i = threadIdx.x; i < nx4; i += blockDim.x) {              // 4 cells of Gw per store
-        if (!s_empty[(4 * i + kOwTW / 2) >> kOwTWS]) continue;
-        float4* __restrict__ wr = reinterpret_cast<float4*>(grids.Gw + row0) + i;
-#pragma unroll 4
-        for (int y = y0; y < y1; ++y, wr += nx4) *wr = z;
-    }
-}
-
 // ------------------------------------------------------------------------------------------------- launchers
 static size_t bin_smem_bytes(const Geom& g) { return g.ontiles <= kBinSmemTiles ? (size_t)2 * g.ontiles * sizeof(uint32_t) : 0; }
 
@@ -895,7 +909,6 @@ cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t
     const size_t smem = owner_smem_bytes(g.Q);
     const unsigned blocks = (unsigned)num_sms * 4u;
     if (store_mode) {
-        k_owner_fill<<<dim3((unsigned)g.ngrids, (unsigned)g.nty), 256, 0, s>>>(g, bin_offset, grids, H);
         k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, work, ctl, tt2, grids,
                                                      scratch, tickets, H, stats);
     } else {
