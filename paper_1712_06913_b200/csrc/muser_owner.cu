@@ -754,22 +754,26 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 uint32_t nidx = 0;
                 if (p + lane < e) { nidx = sI[p + lane]; nxt = __ldg(src + (nidx & 0xFFFu)); }
                 int buf = 0;
+                bool open = false;                                    // the window in registers continues from the last batch
                 while (p < e) {
                     const int m = min(32, e - p);
                     wb[buf * 32 + lane] = ow_stage(nxt, sc);
                     const uint32_t mykey = nxt.w & kOwKeyMask;
-                    // a run ends at the last record of its window and at the end of the batch
-                    uint32_t ends = __ballot_sync(kFull, (nidx >> 15) != 0u || lane == m - 1);
+                    // a run ends at the last record of its window and at the end of the warp's share; a run that
+                    // reaches the end of a batch without either stays in registers for the next batch
+                    uint32_t ends = __ballot_sync(kFull, lane < m && ((nidx >> 15) != 0u || (p + 32 >= e && lane == m - 1)));
                     __syncwarp();
                     if (p + 32 + lane < e) { nidx = sI[p + 32 + lane]; nxt = __ldg(src + (nidx & 0xFFFu)); }
                     const uint4* __restrict__ q = wb + buf * 32;
                     int j = 0;
                     while (j < m) {
-                        const int len = __ffs(ends);                   // records j .. j + len - 1 share one window
-                        ow_window(A, __shfl_sync(kFull, mykey, j), r, c);
+                        const bool closes = ends != 0u;
+                        const int len = closes ? __ffs(ends) : m - j;  // records j .. j + len - 1 share one window
+                        if (!open) ow_window(A, __shfl_sync(kFull, mykey, j), r, c);
 #pragma unroll 2
                         for (int t = 0; t < len; ++t) ow_add(A, q[j + t], tbx, tby);
-                        ow_flush(A, sA, sB);
+                        if (closes) ow_flush(A, sA, sB);
+                        open = !closes;
                         j += len;
                         ends = len < 32 ? ends >> len : 0u;
                     }
