@@ -31,7 +31,7 @@ CFG = 3
 FRAMES_PER_STEP = 80
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_grid_owner_s7 launch of this workload, from the committed
 # `ncu --set full` capture (profiles/); None until that capture exists
-TRAFFIC_NCU = 1.777e9   # profiles/r01d_owner_path.md: k_owner_fill 925.8 MB + k_grid_owner_s7 851.2 MB (includes the 671 MB FFT input H)
+TRAFFIC_NCU = 1.858e9   # profiles/r01e_owner_path.md: k_grid_owner_s7 225 MB read + 1,633 MB written (includes the 671 MB FFT input H)
 WORKLOAD = ("configs[2] MUSER-II full frame: 56,640 vis (113,280 samples) -> 1024^2 grid, PSWF S=7 Q=128 "
             "-> dirty image + beam")
 METRIC = "gridded_visibilities_per_s"
@@ -236,7 +236,7 @@ def main():
     alg_bytes = B * (32.0 * nvis + 12.0 * n * n)
     peak, peak_src = _peaks()
     achieved = alg_bytes / (grid_us * 1e-6) / 1e9
-    roofline = {"bound": "hbm", "kernel": "gridding stage = k_owner_fill (empty tiles) + k_grid_owner_s7", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "k_grid_owner_s7 (gridding stage; zero-fill units of empty tiles included)", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": TRAFFIC_NCU, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_us": grid_us,
                 "kernel_us_per_frame": grid_us / B, "stage_us_per_launch": stage_us,
