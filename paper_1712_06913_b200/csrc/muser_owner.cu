@@ -790,37 +790,64 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     float4* part = nullptr;
     if (heavy) part = reinterpret_cast<float4*>(scratch + (size_t)(first_slot + chunk) * kOwTileFloats);
     constexpr int kG4 = kOwTW / 2, kW4 = kOwTW / 4;                   // float4 per tile row of G / H and of Gw
-    for (int i = tid; i < 32 * kG4; i += 256) {
-        const int row = i / kG4, c2 = i % kG4, gx = x0 + 2 * c2, gy = y0 + row;
-        const int4 a = *reinterpret_cast<const int4*>(sA + 2 * (row * kOwPitch + 2 * c2));
-        float4 v = make_float4((float)a.x * iv, (float)a.y * iv, (float)a.z * iv, (float)a.w * iv);
-        if (heavy) {
-            __stcg(part + i, v);
-        } else if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
-            float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
-            if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
-            *dst = v;
-            if (STORE) {
-                const int2 wq = *reinterpret_cast<const int2*>(sB + row * kOwPitch + 2 * c2);
+    if (!heavy) {
+        // a thread owns one 16-byte column chunk and walks down the rows: addresses advance by constants
+        {
+            constexpr int kStep = 256 / kG4;
+            const int c2 = tid % kG4, r0 = tid / kG4, gx = x0 + 2 * c2;
+            if ((unsigned)gx < (unsigned)g.nx) {
+                const int* pa = sA + 2 * (r0 * kOwPitch + 2 * c2);
+                const int* pb = sB + r0 * kOwPitch + 2 * c2;
+                const long long goff = (long long)(y0 + r0) * g.nx + gx;   // before the grid for gy < 0: not dereferenced
+                float4* gd = reinterpret_cast<float4*>(Gt + goff);
+                float4* hd = reinterpret_cast<float4*>(Ht + goff);
+                const size_t gstep = (size_t)kStep * (g.nx >> 1);
                 const float sw = iw * al;
-                *reinterpret_cast<float4*>(Ht + (size_t)gy * g.nx + gx) =
-                    make_float4(v.x, v.y + (float)wq.x * sw, v.z, v.w + (float)wq.y * sw);
+#pragma unroll
+                for (int k = 0; k < 32 / kStep; ++k) {
+                    if ((unsigned)(y0 + r0 + k * kStep) < (unsigned)g.ny) {
+                        const int4 a = *reinterpret_cast<const int4*>(pa + 2 * k * kStep * kOwPitch);
+                        float4 v = make_float4((float)a.x * iv, (float)a.y * iv, (float)a.z * iv, (float)a.w * iv);
+                        if (!STORE) { const float4 o = gd[k * gstep]; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+                        gd[k * gstep] = v;
+                        if (STORE) {
+                            const int2 wq = *reinterpret_cast<const int2*>(pb + k * kStep * kOwPitch);
+                            hd[k * gstep] = make_float4(v.x, v.y + (float)wq.x * sw, v.z, v.w + (float)wq.y * sw);
+                        }
+                    }
+                }
             }
         }
+        {
+            constexpr int kStep = 256 / kW4;
+            const int c4 = tid % kW4, r0 = tid / kW4, gx = x0 + 4 * c4;
+            if ((unsigned)gx < (unsigned)g.nx) {
+                const int* pb = sB + r0 * kOwPitch + 4 * c4;
+                float4* wd = reinterpret_cast<float4*>(Wt + ((long long)(y0 + r0) * g.nx + gx));
+                const size_t wstep = (size_t)kStep * (g.nx >> 2);
+#pragma unroll
+                for (int k = 0; k < 32 / kStep; ++k) {
+                    if ((unsigned)(y0 + r0 + k * kStep) < (unsigned)g.ny) {
+                        const int4 a = *reinterpret_cast<const int4*>(pb + k * kStep * kOwPitch);
+                        float4 v = make_float4((float)a.x * iw, (float)a.y * iw, (float)a.z * iw, (float)a.w * iw);
+                        if (!STORE) { const float4 o = wd[k * wstep]; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+                        wd[k * wstep] = v;
+                    }
+                }
+            }
+        }
+        continue;
+    }
+    for (int i = tid; i < 32 * kG4; i += 256) {                       // heavy chunk: publish the partial tile
+        const int row = i / kG4, c2 = i % kG4;
+        const int4 a = *reinterpret_cast<const int4*>(sA + 2 * (row * kOwPitch + 2 * c2));
+        __stcg(part + i, make_float4((float)a.x * iv, (float)a.y * iv, (float)a.z * iv, (float)a.w * iv));
     }
     for (int i = tid; i < 32 * kW4; i += 256) {
-        const int row = i / kW4, c4 = i % kW4, gx = x0 + 4 * c4, gy = y0 + row;
+        const int row = i / kW4, c4 = i % kW4;
         const int4 a = *reinterpret_cast<const int4*>(sB + row * kOwPitch + 4 * c4);
-        float4 v = make_float4((float)a.x * iw, (float)a.y * iw, (float)a.z * iw, (float)a.w * iw);
-        if (heavy) {
-            __stcg(part + 32 * kG4 + i, v);
-        } else if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
-            float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
-            if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
-            *dst = v;
-        }
+        __stcg(part + 32 * kG4 + i, make_float4((float)a.x * iw, (float)a.y * iw, (float)a.z * iw, (float)a.w * iw));
     }
-    if (!heavy) continue;
     // heavy tile: the last chunk to arrive adds the published partial tiles up in chunk order
     __threadfence();
     __syncthreads();
