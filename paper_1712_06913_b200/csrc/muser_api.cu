@@ -59,8 +59,10 @@ struct muser_imager {
     uint4* ow_work = nullptr;
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     bool h_packed = false;                  // H already holds G + i*alpha*Gw (written by the owner gridder in store mode)
-    cufftHandle plan = 0;
-    bool plan_ok = false, fft_valid = false;
+    cufftHandle plan = 0, plan_rows = 0;
+    bool plan_ok = false, plan_rows_ok = false, fft_valid = false;
+    bool fused_fft = false;                 // row pass by cuFFT, column pass + correction by k_fft_cols_correct
+    float2* tw_d = nullptr;                 // exp(+2 pi i t / ny), t = 0..ny-1
     cudaStream_t last_stream = nullptr;
     // host-frame staging (muser_frame_host)
     float* in_uvw = nullptr; double* in_freq = nullptr; float2* in_vis = nullptr; float* in_wt = nullptr; int* in_gid = nullptr;
@@ -112,6 +114,7 @@ void free_grids(muser_imager* h) {
     cudaFree(h->G); cudaFree(h->Gw); cudaFree(h->H); cudaFree(h->out_dirty); cudaFree(h->out_psf);
     h->G = nullptr; h->Gw = nullptr; h->H = nullptr; h->out_dirty = h->out_psf = nullptr;
     if (h->plan_ok) { cufftDestroy(h->plan); h->plan_ok = false; }
+    if (h->plan_rows_ok) { cufftDestroy(h->plan_rows); h->plan_rows_ok = false; }
 }
 
 void free_bins(muser_imager* h) {
@@ -410,6 +413,35 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     h->last_stream = s;
     int rcz = flush_zero(h, s);
     if (rcz) return rcz;
+    if (h->fused_fft) {
+        // A5 rows by cuFFT (contiguous 1-D transforms), A5 columns + A6 by the fused kernel; H keeps the row transform,
+        // so muser_dirty followed by muser_psf repeats only the column pass
+        if (!h->plan_rows_ok) {
+            int dims[1] = {h->nx};
+            cufftResult r = cufftPlanMany(&h->plan_rows, 1, dims, nullptr, 1, h->nx, nullptr, 1, h->nx, CUFFT_C2C, h->ngrids * h->ny);
+            if (r != CUFFT_SUCCESS) return fail(h, MUSER_ECUDA, "cufftPlanMany (rows) failed: " + std::to_string((int)r));
+            h->plan_rows_ok = true;
+        }
+        if (!h->fft_valid) {
+            if (!h->h_packed) {
+                StageScope sc(h, MUSER_STAGE_PACK, s);
+                CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, h->stats_d, s));
+                h->n_launches += 1;
+            }
+            h->h_packed = false;
+            StageScope sc(h, MUSER_STAGE_FFT, s);
+            cufftResult r = cufftSetStream(h->plan_rows, s);
+            if (r == CUFFT_SUCCESS) r = cufftExecC2C(h->plan_rows, (cufftComplex*)h->H, (cufftComplex*)h->H, CUFFT_INVERSE);
+            if (r != CUFFT_SUCCESS) return fail(h, MUSER_ECUDA, "cufftExecC2C (rows) failed: " + std::to_string((int)r));
+            h->fft_valid = true;
+        }
+        StageScope sc(h, MUSER_STAGE_CORRECT, s);
+        const float* cx = h->correction ? h->icx_d : h->ones_d;
+        const float* cy = h->correction ? h->icy_d : h->ones_d;
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, s));
+        h->n_launches += 1;
+        return MUSER_OK;
+    }
     if (!h->plan_ok) {
         int dims[2] = {h->ny, h->nx};
         cufftResult r = cufftPlanMany(&h->plan, 2, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, h->ngrids);
@@ -499,6 +531,18 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
     if (rebuild_geom(h)) return bail("geometry");
     if (build_tile_order(h)) return bail("tile order");
     if (alloc_grids(h)) return bail("grids");
+    if (fft_cols_supported(nx, ny) && fft_cols_setup() == cudaSuccess) {
+        std::vector<float2> tw((size_t)ny);
+        for (int t = 0; t < ny; ++t) {
+            const double a = 2.0 * 3.14159265358979323846 * (double)t / (double)ny;
+            tw[t] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+        if (cudaMalloc(&h->tw_d, tw.size() * sizeof(float2)) != cudaSuccess ||
+            cudaMemcpy(h->tw_d, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+            h->err = "twiddle table"; return bail("fft");
+        }
+        h->fused_fft = true;
+    }
     return h;
 }
 
@@ -511,7 +555,7 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
     cudaFree(h->ttp_d); cudaFree(h->order_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
-    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl);
+    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->tw_d);
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete h;
