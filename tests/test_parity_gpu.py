@@ -338,3 +338,30 @@ def test_microbenchmarks_report_plausible_device_limits():
     assert 1e13 < mb["fp32_fma_flops"] < 1.2e14                  # B200: 148 SMs x 128 lanes x 2 x <= 1.965 GHz = 74.5e12
     assert mb["shared_int_adds"] > 1.5 * mb["shared_f32_cas_adds"] > 0   # why the owner gridder merges in fixed point
     assert mb["global_f32_red_adds"] > 1e11
+
+
+@pytest.mark.parametrize("nx,ny", [(512, 256), (256, 512), (1024, 1024), (272, 1024)])
+def test_images_on_fused_and_library_fft_paths(nx, ny):
+    """ny = 256 / 1024 with nx a multiple of 16 takes the fused path (cuFFT rows + k_fft_cols_correct), everything else
+    cuFFT 2-D + k_correct; non-square grids; dirty image and beam against the oracle's O4 + O5."""
+    import torch
+    cell, Q = 30.0, 32
+    n = min(nx, ny)
+    uvw, freq, vis, wt = synth.random_visibilities(5 + nx + ny, 3000, n, cell * max(nx, ny) / n, margin_cells=6.0)
+    # a bright point-like component keeps the image peak well above the noise of the random visibilities
+    vis = (vis * 0.05 + 1.0).astype(np.complex64)
+    im = gu.make_imager(nx, cell, 7, Q, ny=ny)
+    try:
+        im.reset()
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        T = gu.oracle_table("pswf", 7, Q)
+        G_or, Gw_or, st = oc.grid(uvw, freq, vis, wt, nx, ny, cell, Q, 7, T)
+        assert im.get_stats()["n_gridded"] == st["n_gridded"] > 2000
+        gu.check_images(im, G_or, Gw_or, T, 7, Q)
+        d = torch.empty((1, ny, nx), device="cuda"); p = torch.empty_like(d); d2 = torch.empty_like(d); p2 = torch.empty_like(d)
+        im.dirty_psf(d, p)
+        im.dirty(d2); im.psf(p2)                             # separate calls re-use the row transform
+        torch.cuda.synchronize()
+        assert torch.equal(d, d2) and torch.equal(p, p2)
+    finally:
+        im.destroy()
