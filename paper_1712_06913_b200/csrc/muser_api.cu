@@ -62,7 +62,7 @@ struct muser_imager {
     cufftHandle plan = 0, plan_rows = 0;
     bool plan_ok = false, plan_rows_ok = false, fft_valid = false;
     bool fused_fft = false;                 // row pass by cuFFT, column pass + correction by k_fft_cols_correct
-    float2* tw_d = nullptr;                 // exp(+2 pi i t / ny), t = 0..ny-1
+    float2* tw_d = nullptr;                 // per-stage twiddles of the fused column transform
     cudaStream_t last_stream = nullptr;
     // host-frame staging (muser_frame_host)
     float* in_uvw = nullptr; double* in_freq = nullptr; float2* in_vis = nullptr; float* in_wt = nullptr; int* in_gid = nullptr;
@@ -532,11 +532,16 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
     if (build_tile_order(h)) return bail("tile order");
     if (alloc_grids(h)) return bail("grids");
     if (fft_cols_supported(nx, ny) && fft_cols_setup() == cudaSuccess) {
-        std::vector<float2> tw((size_t)ny);
-        for (int t = 0; t < ny; ++t) {
-            const double a = 2.0 * 3.14159265358979323846 * (double)t / (double)ny;
-            tw[t] = make_float2((float)std::cos(a), (float)std::sin(a));
-        }
+        // per-stage twiddles of the radix-4 stages in thread order: tw[(3 stage + i - 1) T + j], T = ny/4,
+        // = exp(+2 pi i * i * (j mod Ns) / (4 Ns)), Ns = 16 * 4^stage (fp64 on the host)
+        const int T = ny / 4;
+        std::vector<float2> tw;
+        for (int Ns = 16; Ns < ny; Ns *= 4)
+            for (int i = 1; i <= 3; ++i)
+                for (int j = 0; j < T; ++j) {
+                    const double a = 2.0 * 3.14159265358979323846 * (double)i * (double)(j % Ns) / (4.0 * (double)Ns);
+                    tw.push_back(make_float2((float)std::cos(a), (float)std::sin(a)));
+                }
         if (cudaMalloc(&h->tw_d, tw.size() * sizeof(float2)) != cudaSuccess ||
             cudaMemcpy(h->tw_d, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
             h->err = "twiddle table"; return bail("fft");

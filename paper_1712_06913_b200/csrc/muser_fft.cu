@@ -5,8 +5,8 @@
 //   F[ky][x] = sum_y F1[y][x] * exp(+2 pi i ky y / ny)               (unnormalised inverse, Alg. 1 l.19)
 //   dirty[yo][xo] = (-1)^(xo+yo) * Re F[(yo+ny/2)%ny][(xo+nx/2)%nx] * icx[xo] * icy[yo];  beam from Im F / alpha
 // Stockham autosort FFT, radix 16 (registers, straight from global memory) followed by radix-4 stages in shared
-// memory: ny = 16 * 4^m (256 or 1024), one CTA per strip of 8 columns, thread t owns butterfly t of all 8 columns
-// (one twiddle serves 8 columns).  Shared layout: float4 s[c/2][pad(i)] = (column c, column c+1), pad(i) = i + i/16,
+// memory: ny = 16 * 4^m (256 or 1024), one CTA of ny/2 threads per strip of 8 columns, a thread owns one butterfly of 4
+// columns (one twiddle serves them).  Shared layout: float4 s[c/2][pad(i)] = (column c, column c+1), pad(i) = i + i/16,
 // pitch = 2 (mod 8) float4: the 8-byte stores of the first stage and the 16-byte accesses of the radix-4 stages are
 // bank-conflict free.
 #include "muser_internal.h"
@@ -27,11 +27,14 @@ __device__ __forceinline__ void idft4(float2& a, float2& b, float2& c, float2& d
 }
 
 template <int N>
-__global__ void __launch_bounds__(N / 4, N == 1024 ? 2 : 8) k_fft_cols_correct(const int nx, const float2* __restrict__ F1,
-                                                            const float2* __restrict__ tw, const float* __restrict__ icx,
-                                                            const float* __restrict__ icy, const Stats* __restrict__ stats,
-                                                            float* __restrict__ dirty, float* __restrict__ psf) {
-    constexpr int T = N / 4;                   // threads
+__global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : 8) k_fft_cols_correct(const int nx, const float2* __restrict__ F1,
+                                                                               const float2* __restrict__ tw,
+                                                                               const float* __restrict__ icx,
+                                                                               const float* __restrict__ icy,
+                                                                               const Stats* __restrict__ stats,
+                                                                               float* __restrict__ dirty, float* __restrict__ psf) {
+    constexpr int T = N / 4;                   // butterflies per column and stage
+    constexpr int NT = N / 2;                  // threads: thread (j, half) owns butterfly j of columns 4 half .. 4 half + 3
     constexpr int PITCH = N + N / 16 + 2;      // float4 per column pair, = 2 (mod 8)
     extern __shared__ __align__(16) float4 sm[];
     const int tid = threadIdx.x;
@@ -40,7 +43,7 @@ __global__ void __launch_bounds__(N / 4, N == 1024 ? 2 : 8) k_fft_cols_correct(c
     auto pad = [](int i) { return i + (i >> 4); };
 
     // ---- stage 1: radix 16, Ns = 1, straight from global memory; outputs y[16 j + i]
-    for (int task = tid; task < (N / 16) * kFftC; task += T) {
+    for (int task = tid; task < (N / 16) * kFftC; task += NT) {
         const int c = task & (kFftC - 1), j = task >> 3;
         float2 v[16];
 #pragma unroll
@@ -70,17 +73,19 @@ __global__ void __launch_bounds__(N / 4, N == 1024 ? 2 : 8) k_fft_cols_correct(c
     }
     __syncthreads();
 
-    // ---- radix-4 stages in shared memory: Ns = 16, 64, ... ; the last one (Ns = N/4) ends in registers
-    const int j = tid;
-    float2 v[kFftC][4];
-    int tstep = N / 64;                                                                    // tw index step of exp(2 pi i k / (4 Ns))
+    // ---- radix-4 stages in shared memory: Ns = 16, 64, ... ; the last one (Ns = N/4) ends in registers.
+    // tw[(3 stage + i - 1) T + j] = exp(+2 pi i * i * (j mod Ns) / (4 Ns)): per-stage tables in butterfly order.
+    const int j = tid >> 1, half = tid & 1;
+    float2 v[4][4];
+    const float2* twp = tw + j;
+    float4* colp = sm + 2 * half * PITCH;      // this thread's two column pairs
 #pragma unroll 1
-    for (int Ns = 16; Ns < N; Ns *= 4, tstep >>= 2) {
+    for (int Ns = 16; Ns < N; Ns *= 4, twp += 3 * T) {
         const int k = j & (Ns - 1);
-        const float2 w1 = __ldg(tw + k * tstep), w2 = __ldg(tw + 2 * k * tstep), w3 = __ldg(tw + 3 * k * tstep);
+        const float2 w1 = __ldg(twp), w2 = __ldg(twp + T), w3 = __ldg(twp + 2 * T);
 #pragma unroll
-        for (int cp = 0; cp < kFftC / 2; ++cp) {
-            const float4* src = sm + cp * PITCH;
+        for (int cp = 0; cp < 2; ++cp) {
+            const float4* src = colp + cp * PITCH;
             const float4 q0 = src[pad(j)], q1 = src[pad(j + T)], q2 = src[pad(j + 2 * T)], q3 = src[pad(j + 3 * T)];
             v[2 * cp][0] = make_float2(q0.x, q0.y); v[2 * cp + 1][0] = make_float2(q0.z, q0.w);
             v[2 * cp][1] = cmul(make_float2(q1.x, q1.y), w1); v[2 * cp + 1][1] = cmul(make_float2(q1.z, q1.w), w1);
@@ -93,8 +98,8 @@ __global__ void __launch_bounds__(N / 4, N == 1024 ? 2 : 8) k_fft_cols_correct(c
         __syncthreads();
         const int o = (j - k) * 4 + k;
 #pragma unroll
-        for (int cp = 0; cp < kFftC / 2; ++cp) {
-            float4* dst = sm + cp * PITCH;
+        for (int cp = 0; cp < 2; ++cp) {
+            float4* dst = colp + cp * PITCH;
 #pragma unroll
             for (int i = 0; i < 4; ++i)
                 dst[pad(o + i * Ns)] = make_float4(v[2 * cp][i].x, v[2 * cp][i].y, v[2 * cp + 1][i].x, v[2 * cp + 1][i].y);
@@ -102,36 +107,20 @@ __global__ void __launch_bounds__(N / 4, N == 1024 ? 2 : 8) k_fft_cols_correct(c
         __syncthreads();
     }
 
-    // ---- epilogue: v[c][i] = F[ky = j + i T][sx0 + c]
-    const int x0 = (sx0 + (nx >> 1)) % nx;                                                 // output columns x0 .. x0 + 7
-    const float4 cxa = *reinterpret_cast<const float4*>(icx + x0), cxb = *reinterpret_cast<const float4*>(icx + x0 + 4);
+    // ---- epilogue: v[c][i] = F[ky = j + i T][sx0 + 4 half + c].  The two lanes of a pair (same j) write the two
+    // 16-byte halves of one 32-byte sector of each output row.
+    const int x0 = (sx0 + (nx >> 1)) % nx + 4 * half;                                      // output columns x0 .. x0 + 3
+    const float4 cx = *reinterpret_cast<const float4*>(icx + x0);
     const float ia = stats->inv_alpha;
     const size_t obase = (size_t)blockIdx.y * N * nx;
-    // Lane pairs (2m, 2m+1) hold two consecutive output rows; they swap half a row so that every store instruction
-    // writes both 16-byte halves of a 32-byte sector (one full sector per lane pair instead of two half sectors).
-    const int odd = tid & 1;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int ky = j + i * T, y = (ky + N / 2) & (N - 1);
-        const float cy = (y & 1) ? -icy[y] : icy[y];                                       // x0 is even: sign = (-1)^y * (+,-,+,-,...)
-        const float m[8] = {cxa.x * cy, -cxa.y * cy, cxa.z * cy, -cxa.w * cy, cxb.x * cy, -cxb.y * cy, cxb.z * cy, -cxb.w * cy};
-        const int ya = y & ~1;                                                             // the even lane's row; the odd lane's is ya + 1
-        const size_t oa = obase + (size_t)ya * nx + x0 + 4 * odd, ob = oa + nx;
-#pragma unroll
-        for (int im = 0; im < 2; ++im) {
-            float* out = im ? psf : dirty;
-            if (!out) continue;
-            float d[8];
-#pragma unroll
-            for (int c = 0; c < 8; ++c) d[c] = im ? v[c][i].y * m[c] * ia : v[c][i].x * m[c];
-            float rcv[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) rcv[q] = __shfl_xor_sync(0xffffffffu, odd ? d[q] : d[4 + q], 1);
-            const float4 own = odd ? make_float4(d[4], d[5], d[6], d[7]) : make_float4(d[0], d[1], d[2], d[3]);
-            const float4 got = make_float4(rcv[0], rcv[1], rcv[2], rcv[3]);
-            *reinterpret_cast<float4*>(out + oa) = odd ? got : own;                        // row ya: even lane cols 0-3, odd lane cols 4-7
-            *reinterpret_cast<float4*>(out + ob) = odd ? own : got;                        // row ya + 1
-        }
+        const float cy = (y & 1) ? -icy[y] : icy[y];                                       // x0 is a multiple of 4: sign = (-1)^y * (+,-,+,-)
+        const float m0 = cx.x * cy, m1 = -cx.y * cy, m2 = cx.z * cy, m3 = -cx.w * cy;
+        const size_t o = obase + (size_t)y * nx + x0;
+        if (dirty) *reinterpret_cast<float4*>(dirty + o) = make_float4(v[0][i].x * m0, v[1][i].x * m1, v[2][i].x * m2, v[3][i].x * m3);
+        if (psf) *reinterpret_cast<float4*>(psf + o) = make_float4(v[0][i].y * m0 * ia, v[1][i].y * m1 * ia, v[2][i].y * m2 * ia, v[3][i].y * m3 * ia);
     }
 }
 
@@ -150,9 +139,9 @@ cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float
                                     const Stats* stats, float* dirty, float* psf, cudaStream_t s) {
     const dim3 blocks((unsigned)(g.nx / kFftC), (unsigned)g.ngrids);
     if (g.ny == 256)
-        k_fft_cols_correct<256><<<blocks, 64, fft_smem_bytes(256), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
+        k_fft_cols_correct<256><<<blocks, 128, fft_smem_bytes(256), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
     else
-        k_fft_cols_correct<1024><<<blocks, 256, fft_smem_bytes(1024), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
+        k_fft_cols_correct<1024><<<blocks, 512, fft_smem_bytes(1024), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
     return cudaGetLastError();
 }
 
