@@ -533,10 +533,10 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
     if (alloc_grids(h)) return bail("grids");
     if (fft_cols_supported(nx, ny) && fft_cols_setup() == cudaSuccess) {
         // per-stage twiddles of the radix-4 stages in thread order: tw[(3 stage + i - 1) T + j], T = ny/4,
-        // = exp(+2 pi i * i * (j mod Ns) / (4 Ns)), Ns = 16 * 4^stage (fp64 on the host)
+        // = exp(+2 pi i * i * (j mod Ns) / (4 Ns)), Ns = R1 * 4^stage, R1 = 16 or 8 (fp64 on the host)
         const int T = ny / 4;
         std::vector<float2> tw;
-        for (int Ns = 16; Ns < ny; Ns *= 4)
+        for (int Ns = fft_cols_first_radix(ny); Ns < ny; Ns *= 4)
             for (int i = 1; i <= 3; ++i)
                 for (int j = 0; j < T; ++j) {
                     const double a = 2.0 * 3.14159265358979323846 * (double)i * (double)(j % Ns) / (4.0 * (double)Ns);

@@ -4,8 +4,8 @@
 // grid is never written back and k_correct never runs (16 B per cell instead of 32).
 //   F[ky][x] = sum_y F1[y][x] * exp(+2 pi i ky y / ny)               (unnormalised inverse, Alg. 1 l.19)
 //   dirty[yo][xo] = (-1)^(xo+yo) * Re F[(yo+ny/2)%ny][(xo+nx/2)%nx] * icx[xo] * icy[yo];  beam from Im F / alpha
-// Stockham autosort FFT, radix 16 (registers, straight from global memory) followed by radix-4 stages in shared
-// memory: ny = 16 * 4^m (256 or 1024), one CTA of ny/2 threads per strip of 8 columns, a thread owns one butterfly of 4
+// Stockham autosort FFT, radix 16 or 8 (registers, straight from global memory) followed by radix-4 stages in shared
+// memory: ny = 16 * 4^m (256, 1024) or 8 * 4^m (512), one CTA of ny/2 threads per strip of 8 columns, a thread owns one butterfly of 4
 // columns (one twiddle serves them).  Shared layout: float4 s[c/2][pad(i)] = (column c, column c+1), pad(i) = i + i/16,
 // pitch = 2 (mod 8) float4: the 8-byte stores of the first stage and the 16-byte accesses of the radix-4 stages are
 // bank-conflict free.
@@ -27,7 +27,7 @@ __device__ __forceinline__ void idft4(float2& a, float2& b, float2& c, float2& d
 }
 
 template <int N>
-__global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : 8) k_fft_cols_correct(const int nx, const float2* __restrict__ F1,
+__global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_fft_cols_correct(const int nx, const float2* __restrict__ F1,
                                                                                const float2* __restrict__ tw,
                                                                                const float* __restrict__ icx,
                                                                                const float* __restrict__ icy,
@@ -42,6 +42,30 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : 8) k_fft_cols_correct(c
     const size_t gbase = (size_t)blockIdx.y * N * nx;
     auto pad = [](int i) { return i + (i >> 4); };
 
+    constexpr int R1 = (N == 256 || N == 1024) ? 16 : 8;                                   // radix of the first stage
+    if (R1 == 8) {
+        // ---- stage 1: radix 8, Ns = 1, straight from global memory; outputs y[8 j + i]
+        for (int task = tid; task < (N / 8) * kFftC; task += NT) {
+            const int c = task & (kFftC - 1), j = task >> 3;
+            float2 v[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = __ldg(F1 + gbase + (size_t)(j + i * (N / 8)) * nx + sx0 + c);
+            // n = a + 2 m (a = 0..1, m = 0..3), k = b + 4 c' (b = 0..3, c' = 0..1): X[b + 4 c'] = sum_a W2^{a c'} W8^{a b} sum_m x[a + 2 m] W4^{m b}
+            idft4(v[0], v[2], v[4], v[6]);                                                // a = 0: u[0][b] at v[2 b]
+            idft4(v[1], v[3], v[5], v[7]);                                                // a = 1: u[1][b] at v[2 b + 1]
+            const float h = 0.70710678118654752f;
+            v[3] = cmul(v[3], make_float2(h, h));                                         // W8^1
+            v[5] = make_float2(-v[5].y, v[5].x);                                          // W8^2 = i
+            v[7] = cmul(v[7], make_float2(-h, h));                                        // W8^3
+            float2* dst = reinterpret_cast<float2*>(sm + (c >> 1) * PITCH) + (c & 1);
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const float2 p0 = v[2 * b], p1 = v[2 * b + 1];
+                dst[2 * pad(8 * j + b)] = make_float2(p0.x + p1.x, p0.y + p1.y);
+                dst[2 * pad(8 * j + b + 4)] = make_float2(p0.x - p1.x, p0.y - p1.y);
+            }
+        }
+    } else
     // ---- stage 1: radix 16, Ns = 1, straight from global memory; outputs y[16 j + i]
     for (int task = tid; task < (N / 16) * kFftC; task += NT) {
         const int c = task & (kFftC - 1), j = task >> 3;
@@ -80,7 +104,7 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : 8) k_fft_cols_correct(c
     const float2* twp = tw + j;
     float4* colp = sm + 2 * half * PITCH;      // this thread's two column pairs
 #pragma unroll 1
-    for (int Ns = 16; Ns < N; Ns *= 4, twp += 3 * T) {
+    for (int Ns = R1; Ns < N; Ns *= 4, twp += 3 * T) {
         const int k = j & (Ns - 1);
         const float2 w1 = __ldg(twp), w2 = __ldg(twp + T), w3 = __ldg(twp + 2 * T);
 #pragma unroll
@@ -126,11 +150,13 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : 8) k_fft_cols_correct(c
 
 static size_t fft_smem_bytes(int N) { return (size_t)(kFftC / 2) * (N + N / 16 + 2) * sizeof(float4); }
 
-bool fft_cols_supported(int nx, int ny) { return (ny == 256 || ny == 1024) && (nx % 16) == 0; }
+bool fft_cols_supported(int nx, int ny) { return (ny == 256 || ny == 512 || ny == 1024) && (nx % 16) == 0; }
+int fft_cols_first_radix(int ny) { return (ny == 256 || ny == 1024) ? 16 : 8; }
 
 cudaError_t fft_cols_setup() {
     cudaError_t e;
     if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
     if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
     return cudaSuccess;
 }
@@ -140,6 +166,8 @@ cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float
     const dim3 blocks((unsigned)(g.nx / kFftC), (unsigned)g.ngrids);
     if (g.ny == 256)
         k_fft_cols_correct<256><<<blocks, 128, fft_smem_bytes(256), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
+    else if (g.ny == 512)
+        k_fft_cols_correct<512><<<blocks, 256, fft_smem_bytes(512), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
     else
         k_fft_cols_correct<1024><<<blocks, 512, fft_smem_bytes(1024), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
     return cudaGetLastError();

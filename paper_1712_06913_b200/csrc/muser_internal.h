@@ -108,8 +108,9 @@ cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t
                               const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, float2* H,
                               Stats* stats, int store_mode, int num_sms, cudaStream_t s);
 
-// ---- fused column transform + correction (muser_fft.cu): ny = 256 or 1024, nx a multiple of 16
+// ---- fused column transform + correction (muser_fft.cu): ny = 256, 512 or 1024, nx a multiple of 16
 bool fft_cols_supported(int nx, int ny);
+int fft_cols_first_radix(int ny);
 cudaError_t fft_cols_setup();
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
                                     const Stats* stats, float* dirty, float* psf, cudaStream_t s);
