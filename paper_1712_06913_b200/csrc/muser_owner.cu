@@ -115,15 +115,16 @@ __device__ __forceinline__ uint32_t ow_agg_inc(uint32_t* __restrict__ cnt, uint3
 constexpr int kBinThreads = 256;
 constexpr int kBinSmemTiles = 4096;      // two u32 arrays of this many tiles must fit the default 48 KB
 
-__device__ __forceinline__ int ow_cta_uniform_grid(const OwLoc& L, int ntiles, int* s_flag) {
-    // s_flag[0] = first kept grid id seen (or -1), s_flag[1] = 1 if a kept visibility disagrees
-    if (threadIdx.x == 0) { s_flag[0] = -1; s_flag[1] = 0; }
-    __syncthreads();
-    if (L.state == 3) atomicCAS(&s_flag[0], -1, L.gid);
-    __syncthreads();
-    if (L.state == 3 && L.gid != s_flag[0]) s_flag[1] = 1;
-    __syncthreads();
-    return ntiles <= kBinSmemTiles && s_flag[1] == 0 && s_flag[0] >= 0;
+// One barrier: zero the CTA histogram(s), then agree (barrier-and) that every kept visibility of the CTA has the grid id
+// of the CTA's first visibility.  Returns that grid id, or -1 if the CTA must take the global-atomics path.
+__device__ __forceinline__ int ow_cta_uniform_grid(const Geom& g, const OwLoc& L, const int* __restrict__ grid_id,
+                                                   uint32_t* s_hist, int nhist) {
+    const bool fits = g.ontiles <= kBinSmemTiles;
+    if (fits)
+        for (int i = threadIdx.x; i < nhist * g.ontiles; i += blockDim.x) s_hist[i] = 0;
+    const int ref = grid_id ? grid_id[(long long)blockIdx.x * blockDim.x] : 0;
+    const int same = __syncthreads_and(L.state != 3 || L.gid == ref);
+    return (fits && same && ref >= 0 && ref < g.ngrids) ? ref : -1;
 }
 
 // The (at most 2 x 2) tiles a 7x7 footprint at nearest cell (cu, cv) touches: first tile (tx0, ty0) and whether the
@@ -147,7 +148,6 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
                                                              const long long nvis, uint32_t* __restrict__ bin_count,
                                                              Stats* __restrict__ stats, uint4* __restrict__ loc) {
     extern __shared__ uint32_t s_hist[];
-    __shared__ int s_flag[2];
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     OwLoc L;
@@ -170,11 +170,9 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
         w2sum = (double)L.wt * (double)L.wt;
         v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
     }
-    const int use_smem = ow_cta_uniform_grid(L, g.ontiles, s_flag);
-    if (use_smem) {
-        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) s_hist[i] = 0;
-        __syncthreads();
-        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ontiles;
+    const int ugrid = ow_cta_uniform_grid(g, L, grid_id, s_hist, 1);
+    if (ugrid >= 0) {
+        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
         if (kept) {
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
@@ -369,7 +367,6 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
                                                                const long long nvis, const uint32_t* __restrict__ bin_offset,
                                                                uint32_t* __restrict__ cursor, uint4* __restrict__ sorted) {
     extern __shared__ uint32_t s_hist[];
-    __shared__ int s_flag[2];
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     OwLoc L;
@@ -388,11 +385,9 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
         }
     }
     const int kept = L.state == 3;
-    const int use_smem = ow_cta_uniform_grid(L, g.ontiles, s_flag);
-    if (use_smem) {
-        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) s_hist[i] = 0;
-        __syncthreads();
-        const uint32_t gbase = (uint32_t)s_flag[0] * (uint32_t)g.ontiles;
+    const int ugrid = ow_cta_uniform_grid(g, L, grid_id, s_hist, 1);
+    if (ugrid >= 0) {
+        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
         uint32_t* s_base = s_hist + g.ontiles;                         // global position of this CTA's run in each tile
         OwTiles T[2];
         uint32_t rk[2][4];
