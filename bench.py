@@ -6,7 +6,7 @@ images/s (MUSER-II frame), % of roofline").
 
 Workload: BASELINE.json configs[2], the MUSER-II full frame (60 antennas -> 1770 baselines x 16 channels x 2
 polarisations = 56,640 visibilities -> 113,280 gridded samples, 1024^2 grid, PSWF support 7, oversample 128).
-One STEP = one pass of the whole hot path (reset -> bin -> grid -> pack -> cuFFT -> correct: dirty image + beam)
+One STEP = one pass of the whole hot path (reset -> bin -> grid -> cuFFT rows -> column FFT + correction: dirty image + beam)
 over a batch of FRAMES_PER_STEP = 80 distinct seeded synthetic frames (145 MB of inputs, larger than the 126 MB
 L2, so every frame's inputs come from HBM).  value = input visibilities gridded per second over all ranks, inputs
 resident in HBM; e2e = the same through muser_frame_host with pinned HOST buffers (H2D + D2H inside the timing).
@@ -31,7 +31,7 @@ CFG = 3
 FRAMES_PER_STEP = 80
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_grid_owner_s7 launch of this workload, from the committed
 # `ncu --set full` capture (profiles/); None until that capture exists
-TRAFFIC_NCU = 1.858e9   # profiles/r01e_owner_path.md: k_grid_owner_s7 225 MB read + 1,633 MB written (includes the 671 MB FFT input H)
+TRAFFIC_NCU = 1.859e9   # profiles/r01f_final.md: k_grid_owner_s7 226 MB read + 1,633 MB written (includes the 671 MB FFT input H)
 WORKLOAD = ("configs[2] MUSER-II full frame: 56,640 vis (113,280 samples) -> 1024^2 grid, PSWF S=7 Q=128 "
             "-> dirty image + beam")
 METRIC = "gridded_visibilities_per_s"
