@@ -299,10 +299,14 @@ int pick_strategy(const muser_imager* h) {
     return h->ngrids <= 4 ? MUSER_STRATEGY_TILED : MUSER_STRATEGY_DIRECT;
 }
 
-uint32_t owner_item_size(long long nvis) {
-    // heavy tiles are split into chunks of item_size samples; the partial-tile scratch holds at most
-    // 16*nvis/item_size + 2 tiles of 12 KB and is kept under 256 MB
+uint32_t owner_item_size(long long nvis, int num_sms) {
+    // Heavy tiles are split into chunks of item_size samples.  4096 (the gridder's sort capacity) when the call has
+    // enough work to fill the machine; down to 1024 for a single small frame, whose latency is the critical path of
+    // one chunk (a third of a MUSER frame sits in the tile around the uv origin).  For huge inputs the chunk grows so
+    // that the partial-tile scratch (at most 16*nvis/item_size + 2 tiles) stays under 256 MB.
     uint32_t item = 4096;
+    const double units = 2.4 * (double)nvis / 4096.0;                // ~2.4 records per visibility on MUSER frames
+    while (item > 1024 && units * (4096.0 / item) < 4.0 * num_sms) item /= 2;
     while ((16.0 * (double)nvis / item + 2.0) * kOwTileFloats * sizeof(float) > 256.0 * 1048576.0) item *= 2;
     return item;
 }
@@ -353,7 +357,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     GridPtrs gp{h->G, h->Gw};
     if (strat == MUSER_STRATEGY_OWNER) {
         if (!owner_capable(h)) return fail(h, MUSER_EUNSUPPORTED, "the owner-tile strategy needs 2-D mode and support 7");
-        const uint32_t item_size = owner_item_size(nvis);
+        const uint32_t item_size = owner_item_size(nvis, h->num_sms);
         uint32_t max_items = 0;
         int rc = ensure_owner_scratch(h, nvis, item_size, &max_items);
         if (rc) return rc;
