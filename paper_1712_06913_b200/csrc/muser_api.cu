@@ -49,7 +49,6 @@ struct muser_imager {
     Stats* stats_d = nullptr;
     // owner-tile path
     float* ttp_d = nullptr;                 // padded transposed table (2-D mode, support 7), else null
-    uint32_t* order_d = nullptr;            // tiles ordered centre-out (the dense ones are scheduled first)
     OwItem* ow_items = nullptr;
     uint32_t* ow_tickets = nullptr;
     float* ow_scratch = nullptr;
@@ -174,27 +173,6 @@ int flush_zero(muser_imager* h, cudaStream_t s) {
 }
 
 bool owner_capable(const muser_imager* h) { return !wmode(h) && h->ttp_d != nullptr; }
-
-// tiles of one grid ordered by distance from the uv origin: MUSER's coverage is centrally condensed, so the heavy
-// tiles get the lowest block indices of the gridding launch and start first
-int build_tile_order(muser_imager* h) {
-    const Geom& g = h->geom;
-    std::vector<std::pair<long long, uint32_t>> key((size_t)g.ntiles);
-    const int cx = (h->nx / 2 + kTile / 2) >> kTileShift, cy = (h->ny / 2 + kTile / 2) >> kTileShift;
-    for (int ty = 0; ty < g.nty; ++ty)
-        for (int tx = 0; tx < g.ntx; ++tx) {
-            const long long dx = tx - cx, dy = ty - cy;
-            key[(size_t)ty * g.ntx + tx] = {dx * dx + dy * dy, (uint32_t)(ty * g.ntx + tx)};
-        }
-    std::sort(key.begin(), key.end());
-    std::vector<uint32_t> order((size_t)g.ntiles);
-    for (size_t i = 0; i < key.size(); ++i)                          // packed (ty << 16 | tx)
-        order[i] = ((key[i].second / (uint32_t)g.ntx) << 16) | (key[i].second % (uint32_t)g.ntx);
-    cudaFree(h->order_d); h->order_d = nullptr;
-    CU(h, cudaMalloc(&h->order_d, order.size() * sizeof(uint32_t)));
-    CU(h, cudaMemcpy(h->order_d, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
-    return MUSER_OK;
-}
 
 // upload tables (transposed TT[r][j] = T[j*Q + r]) + plane metadata + correctors from fp64 host tables
 int upload_tables(muser_imager* h, const std::vector<std::vector<double>>& t64, const std::vector<int>& supports,
@@ -378,7 +356,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
                                     h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->H, h->stats_d,
                                     h->zero_pending ? 1 : 0, h->num_sms, s));
         }
-        h->n_launches += 6;                                           // count, 3 x scan, scatter, grid
+        h->n_launches += g.onbins <= 4096u ? 4 : 6;                   // count, scan (1 or 3 launches), scatter, grid
         h->h_packed = h->zero_pending;                                // store mode also wrote the FFT input H
         h->zero_pending = false;                                      // store mode wrote every tile of every grid
         return MUSER_OK;
@@ -533,7 +511,6 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
     }
     if (build_2d_tables(h)) return bail("tables");
     if (rebuild_geom(h)) return bail("geometry");
-    if (build_tile_order(h)) return bail("tile order");
     if (alloc_grids(h)) return bail("grids");
     if (fft_cols_supported(nx, ny) && fft_cols_setup() == cudaSuccess) {
         // per-stage twiddles of the radix-4 stages in thread order: tw[(3 stage + i - 1) T + j], T = ny/4,
@@ -563,7 +540,7 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->staged); cudaFree(h->sorted); cudaFree(h->stats_d); cudaFree(h->nitems_d);
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
-    cudaFree(h->ttp_d); cudaFree(h->order_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
+    cudaFree(h->ttp_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
     cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->tw_d);
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }

@@ -308,10 +308,13 @@ __global__ void __launch_bounds__(1024) k_owner_scan_tops(const Geom g, const ui
     if (threadIdx.x == 0) { bin_offset[g.onbins] = carry.c; *nitems = carry.m; ctl[0] = carry.l; ctl[1] = 0; }
 }
 
+// SINGLE: the whole histogram fits one CTA (<= 4096 bins): no reduce / tops launches, this kernel also writes the totals.
+template <int SINGLE>
 __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_t* __restrict__ bin_count,
                                                            const uint32_t item_size, const uint32_t* __restrict__ tops,
                                                            uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
-                                                           uint4* __restrict__ work) {
+                                                           uint4* __restrict__ work, uint32_t* __restrict__ nitems,
+                                                           uint32_t* __restrict__ ctl) {
     __shared__ uint32_t s_w[3][32];
     const uint32_t b0 = blockIdx.x * 4096u + 4u * threadIdx.x;
     uint32_t c[4], m[4];
@@ -319,7 +322,12 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
     if (t.c) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);
     OwScan3 total;
     const OwScan3 ex = ow_block_scan3(t, total, s_w);
-    uint32_t off = tops[3 * blockIdx.x] + ex.c, slot = tops[3 * blockIdx.x + 1] + ex.m, wpos = tops[3 * blockIdx.x + 2] + ex.l;
+    uint32_t off = ex.c, slot = ex.m, wpos = ex.l;
+    if (SINGLE) {
+        if (threadIdx.x == 0) { bin_offset[g.onbins] = total.c; *nitems = total.m; ctl[0] = total.l; ctl[1] = 0; }
+    } else {
+        off += tops[3 * blockIdx.x]; slot += tops[3 * blockIdx.x + 1]; wpos += tops[3 * blockIdx.x + 2];
+    }
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const uint32_t b = b0 + j;
@@ -907,9 +915,13 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
                               uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops, cudaStream_t s) {
     const uint32_t nblocks = (g.onbins + 4095u) / 4096u;
+    if (nblocks == 1) {
+        k_owner_scan_write<1><<<1, 1024, 0, s>>>(g, bin_count, item_size, tops, bin_offset, items, work, nitems, ctl);
+        return cudaGetLastError();
+    }
     k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
     k_owner_scan_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems, ctl);
-    k_owner_scan_write<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops, bin_offset, items, work);
+    k_owner_scan_write<0><<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops, bin_offset, items, work, nitems, ctl);
     return cudaGetLastError();
 }
 
