@@ -185,7 +185,16 @@ int upload_tables(muser_imager* h, const std::vector<std::vector<double>>& t64, 
     for (int p = 0; p < P; ++p) {
         const int S = supports[p], pitch = (S + 4) & ~3, comp = wm ? 2 : 1;
         PlaneMeta& pm = h->planes_h[p];
-        pm.support = S; pm.pitch = pitch; pm.offset = (int)(dev.size() / comp); pm.pad = 0; pm.wc = wc[p];
+        pm.support = S; pm.pitch = pitch; pm.offset = (int)(dev.size() / comp); pm.wc = wc[p];
+        {   // bound on |kx ky| = (max |T|)^2, at least 1 (library tables peak at 1; caller-supplied ones may not)
+            double m2 = 1.0;
+            for (size_t i = 0; i < (size_t)S * Q + 1; ++i) {
+                const double v2 = wm ? t64[p][2 * i] * t64[p][2 * i] + t64[p][2 * i + 1] * t64[p][2 * i + 1] : t64[p][i] * t64[p][i];
+                m2 = std::max(m2, v2);
+            }
+            const float kb = (float)(m2 * 1.0001);
+            std::memcpy(&pm.pad, &kb, sizeof(float));
+        }
         const size_t L = (size_t)S * Q + 1;
         h->tables_f32[p].resize(L * comp);
         for (size_t i = 0; i < L * comp; ++i) h->tables_f32[p][i] = (float)t64[p][i];

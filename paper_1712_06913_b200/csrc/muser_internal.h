@@ -29,7 +29,7 @@ struct PlaneMeta {
     int support;                   // S_p (odd)
     int pitch;                     // row pitch of the transposed table TT[r][j], j < pitch, entries >= S_p are 0
     int offset;                    // offset of the plane's TT in the table buffer (floats in 2-D mode, float2 in w mode)
-    int pad;
+    int pad;                       // float bits: bound (>= 1) on |kx ky| of the plane's table (fixed-point scale of the tiled gridder)
     double wc;                     // plane centre in |w| wavelengths
 };
 

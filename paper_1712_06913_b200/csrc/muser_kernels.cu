@@ -259,7 +259,11 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
                                                             const uint32_t* __restrict__ nitems,
                                                             const PlaneMeta* __restrict__ planes,
                                                             const float* __restrict__ tables, GridPtrs grids) {
-    extern __shared__ __align__(16) float smem[];
+    // The region is accumulated in 32-bit FIXED POINT: integer shared-memory adds are native single instructions,
+    // fp32 adds are compare-and-swap loops.  Per item the scales map the largest possible cell sum (sum of
+    // |wt Re V| + |wt Im V| resp. wt over the item's samples, times the plane's bound on |kx ky|) to 0.98 * 2^31.
+    extern __shared__ __align__(16) int smem_i[];
+    __shared__ float s_sum[8][2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t n_items = *nitems;
     for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
@@ -269,11 +273,23 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
         const PlaneMeta pm = planes[p];
         const int S = pm.support, h = (S - 1) >> 1, R = kTile + 2 * h, RR = R * R;
         constexpr int NPL = WMODE ? 4 : 3;                          // planes: G.re G.im W(.re) [W.im]
-        for (int i = threadIdx.x; i < NPL * RR; i += blockDim.x) smem[i] = 0.f;
+        for (int i = threadIdx.x; i < NPL * RR; i += blockDim.x) smem_i[i] = 0;
+        float mv = 0.f, mw = 0.f;
+        for (uint32_t i = threadIdx.x; i < item.count; i += blockDim.x) {
+            const uint4 a = __ldg(reinterpret_cast<const uint4*>(sorted + item.start + i));
+            mv += fabsf(__uint_as_float(a.x)) + fabsf(__uint_as_float(a.y));
+            mw += __uint_as_float(a.z);
+        }
+        for (int o = 16; o > 0; o >>= 1) { mv += __shfl_xor_sync(0xffffffffu, mv, o); mw += __shfl_xor_sync(0xffffffffu, mw, o); }
+        if (lane == 0) { s_sum[warp][0] = mv; s_sum[warp][1] = mw; }
         __syncthreads();
+        mv = 0.f; mw = 0.f;
+        for (int w = 0; w < 8; ++w) { mv += s_sum[w][0]; mw += s_sum[w][1]; }
+        const float kb = __int_as_float(pm.pad);                    // bound on |kx ky| of this plane (>= 1)
+        const float sv = 2104533975.0f / fmaxf(mv * kb, 1e-30f), sw = 2104533975.0f / fmaxf(mw * kb, 1e-30f);
         for (uint32_t i = warp; i < item.count; i += 8) {
             const uint4 a = __ldg(reinterpret_cast<const uint4*>(sorted + item.start + i));
-            const float re = __uint_as_float(a.x), im = __uint_as_float(a.y), wt = __uint_as_float(a.z);
+            const float re = __uint_as_float(a.x) * sv, im = __uint_as_float(a.y) * sv, wt = __uint_as_float(a.z) * sw;
             const int lx = (int)(a.w & 31u), ly = (int)((a.w >> 5) & 31u);
             const int rx = (int)((a.w >> 10) & 511u), ry = (int)((a.w >> 19) & 511u), kc = (int)((a.w >> 28) & 1u);
             for (int c = lane; c < S * S; c += 32) {
@@ -281,22 +297,23 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
                 const int si = (ly + jy) * R + lx + jx;              // region origin is (tile origin - h)
                 if (WMODE == 0) {
                     const float kk = __ldg(tables + pm.offset + rx * pm.pitch + jx) * __ldg(tables + pm.offset + ry * pm.pitch + jy);
-                    atomicAdd(&smem[si], kk * re);
-                    atomicAdd(&smem[RR + si], kk * im);
-                    atomicAdd(&smem[2 * RR + si], kk * wt);
+                    atomicAdd(&smem_i[si], __float2int_rn(kk * re));
+                    atomicAdd(&smem_i[RR + si], __float2int_rn(kk * im));
+                    atomicAdd(&smem_i[2 * RR + si], __float2int_rn(kk * wt));
                 } else {
                     const float2* tc = reinterpret_cast<const float2*>(tables);
                     float2 kx = __ldg(tc + pm.offset + rx * pm.pitch + jx), ky = __ldg(tc + pm.offset + ry * pm.pitch + jy);
                     if (kc) { kx.y = -kx.y; ky.y = -ky.y; }
                     const float kr = kx.x * ky.x - kx.y * ky.y, ki = kx.x * ky.y + kx.y * ky.x;
-                    atomicAdd(&smem[si], kr * re - ki * im);
-                    atomicAdd(&smem[RR + si], kr * im + ki * re);
-                    atomicAdd(&smem[2 * RR + si], kr * wt);
-                    atomicAdd(&smem[3 * RR + si], ki * wt);
+                    atomicAdd(&smem_i[si], __float2int_rn(kr * re - ki * im));
+                    atomicAdd(&smem_i[RR + si], __float2int_rn(kr * im + ki * re));
+                    atomicAdd(&smem_i[2 * RR + si], __float2int_rn(kr * wt));
+                    atomicAdd(&smem_i[3 * RR + si], __float2int_rn(ki * wt));
                 }
             }
         }
         __syncthreads();
+        const float iv = 1.0f / sv, iw = 1.0f / sw;
         const int x0 = tx * kTile - kTile / 2 - h, y0 = ty * kTile - kTile / 2 - h;
         const size_t gbase = (size_t)gi * g.ny * g.nx;
         for (int i = threadIdx.x; i < RR; i += blockDim.x) {
@@ -304,13 +321,13 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
             const int gx = x0 + x, gy = y0 + y;
             if (gx < 0 || gx >= g.nx || gy < 0 || gy >= g.ny) continue;
             const size_t idx = gbase + (size_t)gy * g.nx + gx;
-            const float vr = smem[i], vi = smem[RR + i], wr = smem[2 * RR + i];
-            if (vr != 0.f || vi != 0.f) atomicAdd(&grids.G[idx], make_float2(vr, vi));
+            const int vr = smem_i[i], vi = smem_i[RR + i], wr = smem_i[2 * RR + i];
+            if (vr | vi) atomicAdd(&grids.G[idx], make_float2((float)vr * iv, (float)vi * iv));
             if (WMODE == 0) {
-                if (wr != 0.f) atomicAdd(&grids.Gw[idx], wr);
+                if (wr) atomicAdd(&grids.Gw[idx], (float)wr * iw);
             } else {
-                const float wi = smem[3 * RR + i];
-                if (wr != 0.f || wi != 0.f) atomicAdd(reinterpret_cast<float2*>(grids.Gw) + idx, make_float2(wr, wi));
+                const int wi = smem_i[3 * RR + i];
+                if (wr | wi) atomicAdd(reinterpret_cast<float2*>(grids.Gw) + idx, make_float2((float)wr * iw, (float)wi * iw));
             }
         }
         __syncthreads();
@@ -541,8 +558,8 @@ static size_t fast_smem_bytes(int Q) {
 
 cudaError_t tiled_kernel_setup(int max_smem_bytes) {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
-    if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes))) return e;
+    if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
+    if ((e = cudaFuncSetAttribute(k_grid_tiled_generic<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
     if ((e = cudaFuncSetAttribute(k_grid_tiled_s7, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
     return cudaSuccess;
 }
