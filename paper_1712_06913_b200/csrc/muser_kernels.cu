@@ -36,6 +36,9 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int flagged = 0, dropped = 0, kept = 0;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
+    Staged s0, s1;
+    s0.bin = s1.bin = kNoBin;
+    s0.rank = s1.rank = 0u;
     if (k < nvis) {
         const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
         const double f = freq[k];
@@ -46,8 +49,6 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
         const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
         const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) &&
                         isfinite(V.y) && isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
-        Staged s0, s1;
-        s0.bin = s1.bin = kNoBin;
         if (!ok) {
             flagged = 1;
         } else {
@@ -93,10 +94,28 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                     o.gp = (uint32_t)gid | ((uint32_t)p << 24);
                     const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
                     o.bin = (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
-                    o.rank = do_bin ? atomicAdd(&bin_count[o.bin], 1u) : 0u;
                 }
             }
         }
+    }
+    if (do_bin) {
+        // warp-aggregated histogram: lanes with the same bin issue one atomic (the tile at the uv origin receives a
+        // third of a MUSER frame; per-sample atomics serialise on it)
+        const unsigned full_ = 0xffffffffu;
+        const int lane_ = threadIdx.x & 31;
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            Staged& o = s ? s1 : s0;
+            if (!__any_sync(full_, o.bin != kNoBin)) continue;
+            const unsigned m = __match_any_sync(full_, o.bin);
+            const int leader = __ffs(m) - 1;
+            uint32_t base = 0;
+            if (o.bin != kNoBin && lane_ == leader) base = atomicAdd(&bin_count[o.bin], (uint32_t)__popc(m));
+            base = __shfl_sync(full_, base, leader);
+            o.rank = base + (uint32_t)__popc(m & ((1u << lane_) - 1u));
+        }
+    }
+    if (k < nvis) {
         uint4* dst = reinterpret_cast<uint4*>(staged + 2 * k);
         const uint4* a = reinterpret_cast<const uint4*>(&s0);
         const uint4* b = reinterpret_cast<const uint4*>(&s1);
