@@ -291,6 +291,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
         decode_bin(g, item.bin, gi, p, ty, tx);
         const PlaneMeta pm = planes[p];
         const int S = pm.support, h = (S - 1) >> 1, R = kTile + 2 * h, RR = R * R;
+        const int q32 = 32 / S, r32 = 32 - q32 * S;                 // 32 = q32 * S + r32: how (jy, jx) advance per pass
         constexpr int NPL = WMODE ? 4 : 3;                          // planes: G.re G.im W(.re) [W.im]
         for (int i = threadIdx.x; i < NPL * RR; i += blockDim.x) smem_i[i] = 0;
         float mv = 0.f, mw = 0.f;
@@ -311,8 +312,9 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
             const float re = __uint_as_float(a.x) * sv, im = __uint_as_float(a.y) * sv, wt = __uint_as_float(a.z) * sw;
             const int lx = (int)(a.w & 31u), ly = (int)((a.w >> 5) & 31u);
             const int rx = (int)((a.w >> 10) & 511u), ry = (int)((a.w >> 19) & 511u), kc = (int)((a.w >> 28) & 1u);
-            for (int c = lane; c < S * S; c += 32) {
-                const int jy = c / S, jx = c - jy * S;
+            int jy = lane / S, jx = lane - jy * S;                  // footprint cell of this lane, advanced by 32 per pass
+            for (int c = lane; c < S * S; c += 32, jx += r32, jy += q32) {
+                if (jx >= S) { jx -= S; ++jy; }
                 const int si = (ly + jy) * R + lx + jx;              // region origin is (tile origin - h)
                 if (WMODE == 0) {
                     const float kk = __ldg(tables + pm.offset + rx * pm.pitch + jx) * __ldg(tables + pm.offset + ry * pm.pitch + jy);
