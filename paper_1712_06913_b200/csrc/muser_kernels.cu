@@ -292,6 +292,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
         const PlaneMeta pm = planes[p];
         const int S = pm.support, h = (S - 1) >> 1, R = kTile + 2 * h, RR = R * R;
         const int q32 = 32 / S, r32 = 32 - q32 * S;                 // 32 = q32 * S + r32: how (jy, jx) advance per pass
+        const int jy0 = lane / S, jx0 = lane - jy0 * S;             // footprint cell of this lane in the first pass
         constexpr int NPL = WMODE ? 4 : 3;                          // planes: G.re G.im W(.re) [W.im]
         for (int i = threadIdx.x; i < NPL * RR; i += blockDim.x) smem_i[i] = 0;
         float mv = 0.f, mw = 0.f;
@@ -312,7 +313,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
             const float re = __uint_as_float(a.x) * sv, im = __uint_as_float(a.y) * sv, wt = __uint_as_float(a.z) * sw;
             const int lx = (int)(a.w & 31u), ly = (int)((a.w >> 5) & 31u);
             const int rx = (int)((a.w >> 10) & 511u), ry = (int)((a.w >> 19) & 511u), kc = (int)((a.w >> 28) & 1u);
-            int jy = lane / S, jx = lane - jy * S;                  // footprint cell of this lane, advanced by 32 per pass
+            int jy = jy0, jx = jx0;                                 // advanced by 32 cells per pass
             for (int c = lane; c < S * S; c += 32, jx += r32, jy += q32) {
                 if (jx >= S) { jx -= S; ++jy; }
                 const int si = (ly + jy) * R + lx + jx;              // region origin is (tile origin - h)
@@ -337,8 +338,9 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
         const float iv = 1.0f / sv, iw = 1.0f / sw;
         const int x0 = tx * kTile - kTile / 2 - h, y0 = ty * kTile - kTile / 2 - h;
         const size_t gbase = (size_t)gi * g.ny * g.nx;
-        for (int i = threadIdx.x; i < RR; i += blockDim.x) {
-            const int y = i / R, x = i - y * R;
+        for (int y = warp; y < R; y += 8)
+          for (int x = lane; x < R; x += 32) {
+            const int i = y * R + x;
             const int gx = x0 + x, gy = y0 + y;
             if (gx < 0 || gx >= g.nx || gy < 0 || gy >= g.ny) continue;
             const size_t idx = gbase + (size_t)gy * g.nx + gx;
