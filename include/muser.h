@@ -42,13 +42,14 @@ typedef void* muser_stream;                   /* a cudaStream_t; NULL = the lega
 
 enum { MUSER_OK = 0, MUSER_EINVAL = 1, MUSER_ECUDA = 2, MUSER_ENOMEM = 3, MUSER_ESTATE = 4, MUSER_EUNSUPPORTED = 5 };
 enum { MUSER_KERNEL_PSWF = 0, MUSER_KERNEL_GAUSS = 1 };
-/* gridding strategies (muser_set_strategy).  OWNER: every 64x32-cell tile of every grid has one writer that
- * accumulates it in registers / fixed-point shared memory and stores it once (no memset, no global atomics; 2-D mode
- * with support 7 only, else MUSER_EUNSUPPORTED at muser_grid).  TILED: work items of <= 512 samples per 32x32 tile,
- * shared memory accumulation, global reductions at the flush (any support, w planes).  DIRECT: one warp per sample,
- * global reductions (any support, w planes).  AUTO picks OWNER where it applies, else TILED for <= 4 grids and
- * DIRECT for larger batches. */
-enum { MUSER_STRATEGY_AUTO = 0, MUSER_STRATEGY_DIRECT = 1, MUSER_STRATEGY_TILED = 2, MUSER_STRATEGY_OWNER = 3 };
+/* gridding strategies (muser_set_strategy).  OWNER: the grids are Hermitian, so only the half-plane of rows
+ * ny/2 .. ny-1 is computed; every 64x32-cell tile of it has one writer that accumulates it in registers / fixed-point
+ * shared memory and stores it once (no memset, no global atomics; 2-D mode with support 7 only, else
+ * MUSER_EUNSUPPORTED at muser_grid); the other half-plane is rebuilt on demand (muser_get_grid).  TILED: work items of
+ * <= 512 samples per 32x32 tile, shared memory accumulation, global reductions at the flush (any support, w planes).
+ * AUTO picks OWNER where it applies, else TILED.  (Value 1 was a per-sample global-reduction strategy; it missed the
+ * image tolerance on dense grids and was removed.) */
+enum { MUSER_STRATEGY_AUTO = 0, MUSER_STRATEGY_TILED = 2, MUSER_STRATEGY_OWNER = 3 };
 /* stage ids of muser_get_profile.  On the fused imaging path (ny = 256, 512, 1024 and nx a multiple of 16) FFT is
  * cuFFT's row pass and CORRECT the library's own column transform with the shift/correction epilogue; otherwise FFT
  * is cuFFT's 2-D transform and CORRECT the stand-alone correction kernel.  PACK only runs when the gridder has not

@@ -57,7 +57,7 @@ struct muser_imager {
     uint32_t *ow_count = nullptr, *ow_offset = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
     uint4* ow_work = nullptr;
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
-    bool h_packed = false;                  // H already holds G + i*alpha*Gw (written by the owner gridder in store mode)
+    bool lower_valid = true;                // rows 0 .. ny/2-1 of G, Gw are up to date (the owner gridder stores rows >= ny/2 only)
     cufftHandle plan = 0, plan_rows = 0;
     bool plan_ok = false, plan_rows_ok = false, fft_valid = false;
     bool fused_fft = false;                 // row pass by cuFFT, column pass + correction by k_fft_cols_correct
@@ -140,12 +140,15 @@ int rebuild_geom(muser_imager* h) {
     g.S = h->planes_h.empty() ? h->S : h->planes_h[0].support;
     g.ntiles = g.nty * g.ntx;
     g.otx = (h->nx - 1 + kOwTileW / 2) / kOwTileW + 1;
-    g.ontiles = g.nty * g.otx;
+    g.oty = (h->ny / 2 + kTile - 1) / kTile;
+    g.ontiles = g.oty * g.otx;
     g.onbins = (uint32_t)h->ngrids * (uint32_t)g.ontiles;
     return MUSER_OK;
 }
 
-// (re)allocate and zero the grids for the current nx, ny, ngrids, mode
+// (re)allocate and zero the grids for the current nx, ny, ngrids, mode.  Called from the set_* calls only, which may
+// synchronise: the memsets run on the legacy stream and the device is synchronised before returning, so that work the
+// caller later enqueues on ANY stream (non-blocking ones included) sees the zeros.
 int alloc_grids(muser_imager* h) {
     free_grids(h);
     free_bins(h);
@@ -156,9 +159,10 @@ int alloc_grids(muser_imager* h) {
     CU(h, cudaMemset(h->G, 0, nc * sizeof(float2)));
     CU(h, cudaMemset(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float))));
     CU(h, cudaMemset(h->stats_d, 0, sizeof(Stats)));
+    CU(h, cudaDeviceSynchronize());
     h->fft_valid = false;
     h->zero_pending = false;
-    h->h_packed = false;
+    h->lower_valid = true;
     return MUSER_OK;
 }
 
@@ -169,6 +173,16 @@ int flush_zero(muser_imager* h, cudaStream_t s) {
     CU(h, cudaMemsetAsync(h->G, 0, nc * sizeof(float2), s));
     CU(h, cudaMemsetAsync(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), s));
     h->zero_pending = false;
+    h->lower_valid = true;
+    return MUSER_OK;
+}
+
+// rebuild rows 0 .. ny/2-1 of the grids from the stored half-plane (consumers of the full grids call this first)
+int ensure_lower(muser_imager* h, cudaStream_t s) {
+    if (h->lower_valid) return MUSER_OK;
+    CU(h, launch_mirror_lower(h->geom, GridPtrs{h->G, h->Gw}, s));
+    h->n_launches += 1;
+    h->lower_valid = true;
     return MUSER_OK;
 }
 
@@ -248,7 +262,7 @@ int build_2d_tables(muser_imager* h) {
     return upload_tables(h, t64, {h->S}, {0.0});
 }
 
-int ensure_scratch(muser_imager* h, long long nvis, bool tiled) {
+int ensure_scratch(muser_imager* h, long long nvis, cudaStream_t s) {
     const size_t ns = (size_t)2 * (size_t)nvis;
     if (ns > h->sample_cap) {
         cudaFree(h->staged); cudaFree(h->sorted);
@@ -258,32 +272,28 @@ int ensure_scratch(muser_imager* h, long long nvis, bool tiled) {
         CU(h, cudaMalloc(&h->sorted, cap * sizeof(Sample)));
         h->sample_cap = cap;
     }
-    if (tiled) {
-        const size_t nb = h->geom.nbins;
-        if (nb + 1 > h->bins_cap) {
-            cudaFree(h->bin_count); cudaFree(h->bin_offset);
-            h->bin_count = h->bin_offset = nullptr; h->bins_cap = 0;
-            CU(h, cudaMalloc(&h->bin_count, (nb + 1) * sizeof(uint32_t)));
-            CU(h, cudaMalloc(&h->bin_offset, (nb + 1) * sizeof(uint32_t)));
-            CU(h, cudaMemset(h->bin_count, 0, (nb + 1) * sizeof(uint32_t)));   // K2 re-zeroes it after every use
-            h->bins_cap = nb + 1;
-        }
-        const size_t ni = std::min(nb, h->sample_cap) + h->sample_cap / (size_t)h->geom.chunk + 2;
-        if (ni > h->items_cap) {
-            cudaFree(h->items); h->items = nullptr; h->items_cap = 0;
-            CU(h, cudaMalloc(&h->items, ni * sizeof(Item)));
-            h->items_cap = ni;
-        }
+    const size_t nb = h->geom.nbins;
+    if (nb + 1 > h->bins_cap) {
+        cudaFree(h->bin_count); cudaFree(h->bin_offset);
+        h->bin_count = h->bin_offset = nullptr; h->bins_cap = 0;
+        CU(h, cudaMalloc(&h->bin_count, (nb + 1) * sizeof(uint32_t)));
+        CU(h, cudaMalloc(&h->bin_offset, (nb + 1) * sizeof(uint32_t)));
+        // K2 re-zeroes the histogram after every use; this first zeroing is ordered on the caller's stream
+        CU(h, cudaMemsetAsync(h->bin_count, 0, (nb + 1) * sizeof(uint32_t), s));
+        h->bins_cap = nb + 1;
+    }
+    const size_t ni = std::min(nb, h->sample_cap) + h->sample_cap / (size_t)h->geom.chunk + 2;
+    if (ni > h->items_cap) {
+        cudaFree(h->items); h->items = nullptr; h->items_cap = 0;
+        CU(h, cudaMalloc(&h->items, ni * sizeof(Item)));
+        h->items_cap = ni;
     }
     return MUSER_OK;
 }
 
 int pick_strategy(const muser_imager* h) {
     if (h->strategy != MUSER_STRATEGY_AUTO) return h->strategy;
-    if (owner_capable(h)) return MUSER_STRATEGY_OWNER;
-    // w-mode stays TILED although DIRECT is 2.3x faster on cfg 5: per-sample global reductions in arrival order put
-    // ~1e4 fp32 adds on the cells near the uv origin and miss the 1e-5 grid tolerance there (measured)
-    return h->ngrids <= 4 ? MUSER_STRATEGY_TILED : MUSER_STRATEGY_DIRECT;
+    return owner_capable(h) ? MUSER_STRATEGY_OWNER : MUSER_STRATEGY_TILED;
 }
 
 uint32_t owner_item_size(long long nvis, int num_sms) {
@@ -298,7 +308,7 @@ uint32_t owner_item_size(long long nvis, int num_sms) {
     return item;
 }
 
-int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, uint32_t* max_items_out) {
+int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, uint32_t* max_items_out, cudaStream_t s) {
     const size_t nrec = (size_t)8 * (size_t)nvis;                    // <= 2 samples x 4 tiles per visibility
     if (nrec > h->ow_sorted_cap) {
         cudaFree(h->ow_sorted); cudaFree(h->ow_loc); h->ow_sorted = h->ow_loc = nullptr; h->ow_sorted_cap = 0;
@@ -316,7 +326,7 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
         CU(h, cudaMalloc(&h->ow_work, nb * sizeof(uint4)));
         CU(h, cudaMalloc(&h->ow_tops, (nb / 4096 + 2) * 3 * sizeof(uint32_t)));
         if (!h->ow_ctl) CU(h, cudaMalloc(&h->ow_ctl, 4 * sizeof(uint32_t)));
-        CU(h, cudaMemset(h->ow_count, 0, nb * sizeof(uint32_t)));     // every later use leaves it zeroed
+        CU(h, cudaMemsetAsync(h->ow_count, 0, nb * sizeof(uint32_t), s));   // ordered on the caller's stream; every later use leaves it zeroed
         h->ow_bins_cap = nb;
     }
     const size_t ni = (size_t)(16.0 * (double)nvis / item_size) + 2;
@@ -326,7 +336,7 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
         const size_t cap = ni + ni / 4 + 16;
         CU(h, cudaMalloc(&h->ow_items, cap * sizeof(OwItem)));
         CU(h, cudaMalloc(&h->ow_tickets, cap * sizeof(uint32_t)));
-        CU(h, cudaMemset(h->ow_tickets, 0, cap * sizeof(uint32_t)));  // the last chunk of a tile re-zeroes its ticket
+        CU(h, cudaMemsetAsync(h->ow_tickets, 0, cap * sizeof(uint32_t), s));   // the last chunk of a tile re-zeroes its ticket
         CU(h, cudaMalloc(&h->ow_scratch, cap * kOwTileFloats * sizeof(float)));
         h->ow_items_cap = cap;
     }
@@ -346,9 +356,9 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         if (!owner_capable(h)) return fail(h, MUSER_EUNSUPPORTED, "the owner-tile strategy needs 2-D mode and support 7");
         const uint32_t item_size = owner_item_size(nvis, h->num_sms);
         uint32_t max_items = 0;
-        int rc = ensure_owner_scratch(h, nvis, item_size, &max_items);
+        int rc = ensure_owner_scratch(h, nvis, item_size, &max_items, s);
         if (rc) return rc;
-        if (g.nty > 65535 || g.otx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
+        if (g.oty > 65535 || g.otx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
         h->last_stream = s;
         h->fft_valid = false;
         {
@@ -362,38 +372,33 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
             CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_count, h->ow_items, h->nitems_d, h->ow_work,
-                                    h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->H, h->stats_d,
-                                    h->zero_pending ? 1 : 0, h->num_sms, s));
+                                    h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->zero_pending ? 1 : 0,
+                                    h->num_sms, s));
         }
         h->n_launches += g.onbins <= 4096u ? 4 : 6;                   // count, scan (1 or 3 launches), scatter, grid
-        h->h_packed = h->zero_pending;                                // store mode also wrote the FFT input H
-        h->zero_pending = false;                                      // store mode wrote every tile of every grid
+        h->zero_pending = false;                                      // store mode wrote every tile of the stored half-plane
+        h->lower_valid = false;                                       // rows < ny/2 are rebuilt on demand (ensure_lower)
         return MUSER_OK;
     }
-    const bool tiled = strat == MUSER_STRATEGY_TILED;
-    int rc = ensure_scratch(h, nvis, tiled);
+    if (strat != MUSER_STRATEGY_TILED) return fail(h, MUSER_EUNSUPPORTED, "unknown gridding strategy");
+    int rc = ensure_scratch(h, nvis, s);
     if (rc) return rc;
     if ((rc = flush_zero(h, s))) return rc;
+    if ((rc = ensure_lower(h, s))) return rc;                         // the generic gridder adds to both half-planes
     h->last_stream = s;
     h->fft_valid = false;
-    h->h_packed = false;
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
         CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
-                            h->stats_d, tiled ? 1 : 0, s));
-        if (tiled) {
-            CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, s));
-            CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
-        }
-        h->n_launches += tiled ? 3 : 1;
+                            h->stats_d, s));
+        CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, s));
+        CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
+        h->n_launches += 3;
     }
     {
         StageScope sc(h, MUSER_STAGE_GRID, s);
-        if (tiled)
-            CU(h, launch_grid_tiled(g, h->sorted, h->items, h->nitems_d, h->planes_d, h->planes_h.data(), h->tables_d,
-                                    gp, h->num_sms, s));
-        else
-            CU(h, launch_grid_direct(g, h->staged, 2 * nvis, h->planes_d, h->tables_d, gp, s));
+        CU(h, launch_grid_tiled(g, h->sorted, h->items, h->nitems_d, h->planes_d, h->planes_h.data(), h->tables_d,
+                                gp, h->num_sms, s));
         h->n_launches += 1;
     }
     return MUSER_OK;
@@ -414,12 +419,13 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
             h->plan_rows_ok = true;
         }
         if (!h->fft_valid) {
-            if (!h->h_packed) {
+            {
+                int rc = ensure_lower(h, s);
+                if (rc) return rc;
                 StageScope sc(h, MUSER_STAGE_PACK, s);
                 CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, h->stats_d, s));
                 h->n_launches += 1;
             }
-            h->h_packed = false;
             StageScope sc(h, MUSER_STAGE_FFT, s);
             cufftResult r = cufftSetStream(h->plan_rows, s);
             if (r == CUFFT_SUCCESS) r = cufftExecC2C(h->plan_rows, (cufftComplex*)h->H, (cufftComplex*)h->H, CUFFT_INVERSE);
@@ -440,12 +446,13 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         h->plan_ok = true;
     }
     if (!h->fft_valid) {
-        if (!h->h_packed) {
+        {
+            int rc = ensure_lower(h, s);
+            if (rc) return rc;
             StageScope sc(h, MUSER_STAGE_PACK, s);
             CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, h->stats_d, s));
             h->n_launches += 1;
         }
-        h->h_packed = false;                                          // the in-place transform consumes H
         {
             StageScope sc(h, MUSER_STAGE_FFT, s);
             cufftResult r = cufftSetStream(h->plan, s);
@@ -467,7 +474,6 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
 int reset_impl(muser_imager* h, cudaStream_t s) {
     h->last_stream = s;
     h->fft_valid = false;
-    h->h_packed = false;
     // The grids are zeroed lazily: the owner-tile gridder writes every tile of every grid with plain stores, so a
     // reset followed by muser_grid needs no memset at all; any other consumer calls flush_zero first.
     h->zero_pending = true;
@@ -632,7 +638,8 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
 
 int muser_set_strategy(muser_imager* h, int strategy) {
     if (!h) return MUSER_EINVAL;
-    if (strategy < MUSER_STRATEGY_AUTO || strategy > MUSER_STRATEGY_OWNER) return fail(h, MUSER_EINVAL, "unknown strategy");
+    if (strategy != MUSER_STRATEGY_AUTO && strategy != MUSER_STRATEGY_TILED && strategy != MUSER_STRATEGY_OWNER)
+        return fail(h, MUSER_EINVAL, "unknown strategy");
     if (h->zero_pending) {                                            // do not carry a deferred reset across strategies
         int rc = flush_zero(h, h->last_stream);
         if (rc) return rc;
@@ -729,6 +736,7 @@ int muser_get_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_
     h->last_stream = s;
     int rcz = flush_zero(h, s);
     if (rcz) return rcz;
+    if ((rcz = ensure_lower(h, s))) return rcz;
     if (grid_c64_out) CU(h, cudaMemcpyAsync(grid_c64_out, h->G, nc * sizeof(float2), cudaMemcpyDeviceToDevice, s));
     if (wgrid_out) CU(h, cudaMemcpyAsync(wgrid_out, h->Gw, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), cudaMemcpyDeviceToDevice, s));
     return MUSER_OK;

@@ -20,7 +20,8 @@ struct Geom {
     int chunk;                     // samples per work item of the tiled gridder
     int S;                         // support of plane 0 (the 2-D kernel)
     int ntiles;                    // nty*ntx
-    int otx, ontiles;              // owner-tile path: tiles per row (kOwTileW cells wide), tiles per grid
+    int otx, oty, ontiles;         // owner-tile path: tiles per row (kOwTileW cells wide), tile rows of the stored
+                                   // half-plane (rows ny/2 .. ny-1, 32 cells tall), tiles per grid = oty*otx
     uint32_t onbins;               // ngrids*ontiles
 };
 
@@ -68,25 +69,25 @@ struct GridPtrs {
 // ---- launch wrappers (muser_kernels.cu); all asynchronous on `s` -------------------------------------------
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                           const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
-                          uint32_t* bin_count, Stats* stats, int do_bin, cudaStream_t s);
+                          uint32_t* bin_count, Stats* stats, cudaStream_t s);
 cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,
                               uint32_t* nitems, cudaStream_t s);
 cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsamples, const uint32_t* bin_offset,
                            Sample* sorted, cudaStream_t s);
-cudaError_t launch_grid_direct(const Geom& g, const Staged* staged, long long nsamples, const PlaneMeta* planes,
-                               const float* tables, GridPtrs grids, cudaStream_t s);
 cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* nitems,
                               const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
                               GridPtrs grids, int num_sms, cudaStream_t s);
 cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, Stats* stats, cudaStream_t s);
+cudaError_t launch_mirror_lower(const Geom& g, GridPtrs grids, cudaStream_t s);
 cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, const Stats* stats,
                            float* dirty, float* psf, cudaStream_t s);
 cudaError_t tiled_kernel_setup(int max_smem_bytes);
 
-// ---- owner-tile path (muser_owner.cu): 2-D mode, support 7.  Every 32x32 tile of every grid has exactly one
-// writer, so the grids are written with plain stores (no memset, no global atomics); samples whose footprint
-// crosses a tile edge are listed in every tile they touch.
-constexpr int kOwSub = 1024;                 // samples staged and cell-sorted in shared memory per pass
+// ---- owner-tile path (muser_owner.cu): 2-D mode, support 7.  The grids are Hermitian (every visibility is gridded
+// with its conjugate), so only the half-plane of rows ny/2 .. ny-1 is computed and stored; k_mirror_lower rebuilds
+// the other half for consumers that want the full grid.  Every 64x32 tile of the stored half-plane has exactly one
+// writer, so it is written with plain stores (no memset, no global atomics); samples whose footprint crosses a tile
+// edge are listed in every tile they touch.
 constexpr int kOwTileW = 64;                 // owner tiles are 64 cells wide, 32 tall
 constexpr int kOwTileFloats = kOwTileW * 32 * 3;   // one partial tile in the scratch buffer: A[32][W] float2 + B[32][W] float
 // two-parity transposed table TT2[(par*(Q+1) + r)*8 + i]: par 0: i = j (j = 0..6: T[j*Q + r]), [7] = 0;
@@ -105,8 +106,8 @@ cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float2* 
 cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
-                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, float2* H,
-                              Stats* stats, int store_mode, int num_sms, cudaStream_t s);
+                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, int store_mode,
+                              int num_sms, cudaStream_t s);
 
 // ---- fused column transform + correction (muser_fft.cu): ny = 256, 512 or 1024, nx a multiple of 16
 bool fft_cols_supported(int nx, int ny);

@@ -2,7 +2,7 @@
 //   K1 k_coords       A1: fp64 coordinates, keep/drop, Hermitian conjugate sample, tile histogram + rank
 //   K2 k_scan_items   A1: exclusive scan of the tile histogram, work items of <= chunk samples
 //   K3 k_scatter      A1: counting-sort scatter into 16-byte tile-local samples
-//   K4 k_grid_*       A2/A3/A4: convolutional gridding (tiled shared-memory accumulators, or direct reductions)
+//   K4 k_grid_tiled_* A2/A3/A4: convolutional gridding, generic strategy (tiled shared-memory accumulators + global reductions)
 //   Kp k_pack         H = G + i*Gw, the single FFT input that yields dirty image and beam together
 //   K5 k_correct      A6: fused fftshift (index roll + checkerboard sign) + grid correction + real/imag part
 // Passages: PAPER.md:78 (gridding = convolution onto a regular grid), :136-138 (spheroidal GCF, inverse FFT),
@@ -32,7 +32,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                                                 const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                 const long long nvis, const PlaneMeta* __restrict__ planes,
                                                 Staged* __restrict__ staged, uint32_t* __restrict__ bin_count,
-                                                Stats* __restrict__ stats, const int do_bin) {
+                                                Stats* __restrict__ stats) {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int flagged = 0, dropped = 0, kept = 0;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
             }
         }
     }
-    if (do_bin) {
+    {
         // warp-aggregated histogram: lanes with the same bin issue one atomic (the tile at the uv origin receives a
         // third of a MUSER frame; per-sample atomics serialise on it)
         const unsigned full_ = 0xffffffffu;
@@ -219,45 +219,6 @@ __global__ void __launch_bounds__(256) k_scatter(const Geom g, const Staged* __r
     o.x = a.x; o.y = a.y; o.z = a.z;
     o.w = (uint32_t)lx | ((uint32_t)ly << 5) | (rx << 10) | (ry << 19) | (kc << 28);
     reinterpret_cast<uint4*>(sorted)[bin_offset[b.y] + b.z] = o;
-}
-
-// ------------------------------------------------------------------------------------------------- K4 direct
-// One warp per sample, lanes over the S*S footprint, vector reductions straight to the L2-resident grids.
-// Used for batches of small grids (A4) where a tile holds only a handful of samples.
-template <int WMODE>
-__global__ void __launch_bounds__(256) k_grid_direct(const Geom g, const Staged* __restrict__ staged,
-                                                     const long long nsamples, const PlaneMeta* __restrict__ planes,
-                                                     const float* __restrict__ tables, GridPtrs grids) {
-    const int lane = threadIdx.x & 31;
-    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < nsamples; i += nwarps) {
-        const uint4* src = reinterpret_cast<const uint4*>(staged + i);
-        const uint4 a = __ldg(src), b = __ldg(src + 1);
-        if (b.y == kNoBin) continue;
-        const float re = __uint_as_float(a.x), im = __uint_as_float(a.y), wt = __uint_as_float(a.z);
-        const int cu = (int)(a.w & 0xFFFFu), cv = (int)(a.w >> 16);
-        const int rx = (int)(b.x & 511u), ry = (int)((b.x >> 9) & 511u), kc = (int)((b.x >> 18) & 1u);
-        const int gi = (int)(b.w & 0xFFFFFFu), p = (int)(b.w >> 24);
-        const PlaneMeta pm = planes[p];
-        const int S = pm.support, h = (S - 1) >> 1;
-        const size_t gbase = (size_t)gi * g.ny * g.nx;
-        for (int c = lane; c < S * S; c += 32) {
-            const int jy = c / S, jx = c - jy * S;
-            const size_t idx = gbase + (size_t)(cv - h + jy) * g.nx + (size_t)(cu - h + jx);
-            if (WMODE == 0) {
-                const float kk = __ldg(tables + pm.offset + rx * pm.pitch + jx) * __ldg(tables + pm.offset + ry * pm.pitch + jy);
-                atomicAdd(&grids.G[idx], make_float2(kk * re, kk * im));
-                atomicAdd(&grids.Gw[idx], kk * wt);
-            } else {
-                const float2* tc = reinterpret_cast<const float2*>(tables);
-                float2 kx = __ldg(tc + pm.offset + rx * pm.pitch + jx), ky = __ldg(tc + pm.offset + ry * pm.pitch + jy);
-                if (kc) { kx.y = -kx.y; ky.y = -ky.y; }
-                const float kr = kx.x * ky.x - kx.y * ky.y, ki = kx.x * ky.y + kx.y * ky.x;
-                atomicAdd(&grids.G[idx], make_float2(kr * re - ki * im, kr * im + ki * re));
-                atomicAdd(reinterpret_cast<float2*>(grids.Gw) + idx, make_float2(kr * wt, ki * wt));
-            }
-        }
-    }
 }
 
 // ------------------------------------------------------------------------------------------------- K4 tiled
@@ -481,6 +442,34 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
     }
 }
 
+// ------------------------------------------------------------------------------------------------- mirror
+// The owner-tile gridder stores only the half-plane of rows ny/2 .. ny-1 (the grids are Hermitian: "half
+// the grid (as the data is Hermitian)").  This kernel rebuilds rows 0 .. ny/2-1 for consumers of the full grids:
+// G[y][x] = conj G[ny-y][nx-x], Gw[y][x] = Gw[ny-y][nx-x] (conjugated in w mode); row 0 and column 0 have no mirror
+// and are empty by the drop rule R5.
+template <int WMODE>
+__global__ void __launch_bounds__(256) k_mirror_lower(const int nx, const int ny, const size_t total, float2* __restrict__ G,
+                                                      float* __restrict__ Gw) {
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // over [ngrids][ny/2][nx]
+    if (t >= total) return;
+    const int x = (int)(t % nx);
+    const size_t row = t / nx;
+    const int y = (int)(row % (ny >> 1));
+    const size_t gbase = (row / (ny >> 1)) * (size_t)ny * nx;
+    const size_t dst = gbase + (size_t)y * nx + x;
+    float2 v = make_float2(0.f, 0.f), w = make_float2(0.f, 0.f);
+    if (x > 0 && y > 0) {
+        const size_t src = gbase + (size_t)(ny - y) * nx + (nx - x);
+        v = G[src];
+        v.y = -v.y;
+        if (WMODE) { w = reinterpret_cast<const float2*>(Gw)[src]; w.y = -w.y; }
+        else w.x = Gw[src];
+    }
+    G[dst] = v;
+    if (WMODE) reinterpret_cast<float2*>(Gw)[dst] = w;
+    else Gw[dst] = w.x;
+}
+
 // ------------------------------------------------------------------------------------------------- pack, K5
 // H = G + i*alpha*Gw: G and Gw are both Hermitian, so their inverse transforms are real and one complex FFT of
 // H returns the dirty image in the real part and alpha * beam in the imaginary part.  alpha is the power of two
@@ -544,9 +533,9 @@ static inline unsigned blocks_for(long long n, int per) { return (unsigned)((n +
 
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                           const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
-                          uint32_t* bin_count, Stats* stats, int do_bin, cudaStream_t s) {
+                          uint32_t* bin_count, Stats* stats, cudaStream_t s) {
     k_coords<<<blocks_for(nvis, 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, planes, staged, bin_count,
-                                                   stats, do_bin);
+                                                   stats);
     return cudaGetLastError();
 }
 
@@ -559,15 +548,6 @@ cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_
 cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsamples, const uint32_t* bin_offset,
                            Sample* sorted, cudaStream_t s) {
     k_scatter<<<blocks_for(nsamples, 256), 256, 0, s>>>(g, staged, nsamples, bin_offset, sorted);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_grid_direct(const Geom& g, const Staged* staged, long long nsamples, const PlaneMeta* planes,
-                               const float* tables, GridPtrs grids, cudaStream_t s) {
-    const long long want = (nsamples + 7) / 8;                            // 8 warps per CTA, one sample per warp pass
-    const unsigned blocks = (unsigned)(want < 1 ? 1 : (want > 148LL * 64 ? 148LL * 64 : want));
-    if (g.wmode) k_grid_direct<1><<<blocks, 256, 0, s>>>(g, staged, nsamples, planes, tables, grids);
-    else k_grid_direct<0><<<blocks, 256, 0, s>>>(g, staged, nsamples, planes, tables, grids);
     return cudaGetLastError();
 }
 
@@ -609,6 +589,14 @@ cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, Stats* stats, 
     const unsigned blocks = (unsigned)((ncell2 + 255) / 256);
     if (g.wmode) k_pack<1><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H), stats);
     else k_pack<0><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H), stats);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_mirror_lower(const Geom& g, GridPtrs grids, cudaStream_t s) {
+    const size_t total = (size_t)g.ngrids * (g.ny / 2) * g.nx;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    if (g.wmode) k_mirror_lower<1><<<blocks, 256, 0, s>>>(g.nx, g.ny, total, grids.G, grids.Gw);
+    else k_mirror_lower<0><<<blocks, 256, 0, s>>>(g.nx, g.ny, total, grids.G, grids.Gw);
     return cudaGetLastError();
 }
 

@@ -89,9 +89,10 @@ __device__ __forceinline__ void ow_locate(const Geom& g, const float* __restrict
 
 // Bin of the q-th tile (q = qx | qy << 1) touched by the footprint of a sample at nearest cell (cu, cv), or kNoBin.
 __device__ __forceinline__ uint32_t ow_bin(const Geom& g, int gid, int cu, int cv, int q, int& tx, int& ty) {
-    const int h = (g.S - 1) >> 1;
+    const int h = (g.S - 1) >> 1, hy = g.ny >> 1;
+    if (cv + h < hy) return kNoBin;                                   // footprint entirely in the lower half-plane
     const int tx0 = (cu - h + kOwTW / 2) >> kOwTWS, tx1 = (cu + h + kOwTW / 2) >> kOwTWS;
-    const int ty0 = (cv - h + kTile / 2) >> kTileShift, ty1 = (cv + h + kTile / 2) >> kTileShift;
+    const int ty0 = max(cv - h - hy, 0) >> kTileShift, ty1 = (cv + h - hy) >> kTileShift;
     if (((q & 1) && tx1 == tx0) || ((q & 2) && ty1 == ty0)) return kNoBin;
     tx = (q & 1) ? tx1 : tx0;
     ty = (q & 2) ? ty1 : ty0;
@@ -129,14 +130,15 @@ __device__ __forceinline__ int ow_cta_uniform_grid(const Geom& g, const OwLoc& L
 
 // The (at most 2 x 2) tiles a 7x7 footprint at nearest cell (cu, cv) touches: first tile (tx0, ty0) and whether the
 // footprint also reaches the next tile in x / in y.
-struct OwTiles { int tx0, ty0, t00; bool mx, my; };
+struct OwTiles { int tx0, ty0, t00; bool mx, my, up; };
 __device__ __forceinline__ OwTiles ow_tiles(const Geom& g, int cu, int cv) {
-    const int h = (g.S - 1) >> 1;
+    const int h = (g.S - 1) >> 1, hy = g.ny >> 1;
     OwTiles t;
+    t.up = cv + h >= hy;                                              // touches the stored (upper) half-plane
     t.tx0 = (cu - h + kOwTW / 2) >> kOwTWS;
-    t.ty0 = (cv - h + kTile / 2) >> kTileShift;
+    t.ty0 = max(cv - h - hy, 0) >> kTileShift;
     t.mx = ((cu + h + kOwTW / 2) >> kOwTWS) != t.tx0;
-    t.my = ((cv + h + kTile / 2) >> kTileShift) != t.ty0;
+    t.my = t.up && ((cv + h - hy) >> kTileShift) != t.ty0;
     t.t00 = t.ty0 * g.otx + t.tx0;
     return t;
 }
@@ -177,6 +179,7 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 const OwTiles t = ow_tiles(g, L.cu[s], L.cv[s]);
+                if (!t.up) continue;
                 atomicAdd(&s_hist[t.t00], 1u);
                 if (t.mx) atomicAdd(&s_hist[t.t00 + 1], 1u);
                 if (t.my) atomicAdd(&s_hist[t.t00 + g.otx], 1u);
@@ -358,7 +361,7 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
 __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, int s, int tx, int ty, uint4* dst) {
     const int h = (g.S - 1) >> 1;
     const int ox = L.cu[s] - (tx * kOwTW - kOwTW / 2) + h;
-    const int oy = L.cv[s] - (ty * kTile - kTile / 2) + h;
+    const int oy = L.cv[s] - ((g.ny >> 1) + ty * kTile) + h;
     uint4 o;
     o.x = __float_as_uint(L.re);
     o.y = __float_as_uint(s ? -L.im : L.im);
@@ -403,6 +406,7 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 T[s] = ow_tiles(g, L.cu[s], L.cv[s]);
+                if (!T[s].up) continue;
                 rk[s][0] = atomicAdd(&s_hist[T[s].t00], 1u);
                 if (T[s].mx) rk[s][1] = atomicAdd(&s_hist[T[s].t00 + 1], 1u);
                 if (T[s].my) rk[s][2] = atomicAdd(&s_hist[T[s].t00 + g.otx], 1u);
@@ -419,6 +423,7 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 const OwTiles t = T[s];
+                if (!t.up) continue;
                 ow_write_record(g, L, s, t.tx0, t.ty0, sorted + s_base[t.t00] + rk[s][0]);
                 if (t.mx) ow_write_record(g, L, s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + rk[s][1]);
                 if (t.my) ow_write_record(g, L, s, t.tx0, t.ty0 + 1, sorted + s_base[t.t00 + g.otx] + rk[s][2]);
@@ -552,24 +557,23 @@ __device__ __forceinline__ OwScale ow_scale_from(float3 s) {
 }
 
 // ------------------------------------------------------------------------------------------------- O4a fill
-// STORE mode: zero the EMPTY tiles of one row of tiles of one grid in G, Gw and H, as long contiguous runs of each
+// STORE mode: zero the EMPTY tiles of one row of tiles of one grid in G and Gw, as long contiguous runs of each
 // cell row (16-byte stores, consecutive threads -> consecutive addresses).  A thread owns column chunks: the emptiness
 // test is done once per chunk, the loop over the rows only stores.  Called by all 256 threads of a CTA.
 __device__ __forceinline__ void ow_fill_row(const Geom& g, const uint32_t* __restrict__ bin_offset, GridPtrs grids,
-                                            float2* __restrict__ H, const int gi, const int ty, unsigned char* s_empty) {
+                                            const int gi, const int ty, unsigned char* s_empty) {
     const uint32_t bin0 = (uint32_t)gi * (uint32_t)g.ontiles + (uint32_t)ty * (uint32_t)g.otx;
     for (int t = threadIdx.x; t < g.otx; t += blockDim.x) s_empty[t] = bin_offset[bin0 + t + 1] == bin_offset[bin0 + t];
     __syncthreads();
-    const int y0 = max(ty * kTile - kTile / 2, 0), y1 = min(ty * kTile + kTile / 2, g.ny);
+    const int y0 = (g.ny >> 1) + ty * kTile, y1 = min(y0 + kTile, g.ny);
     const int nx2 = g.nx >> 1, nx4 = g.nx >> 2;
     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
     const size_t row0 = ((size_t)gi * g.ny + y0) * (size_t)g.nx;
-    for (int i = threadIdx.x; i < nx2; i += blockDim.x) {              // 2 cells of G / H per store
+    for (int i = threadIdx.x; i < nx2; i += blockDim.x) {              // 2 cells of G per store
         if (!s_empty[(2 * i + kOwTW / 2) >> kOwTWS]) continue;
         float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row0) + i;
-        float4* __restrict__ hr = reinterpret_cast<float4*>(H + row0) + i;
 #pragma unroll 4
-        for (int y = y0; y < y1; ++y, gr += nx2, hr += nx2) { *gr = z; *hr = z; }
+        for (int y = y0; y < y1; ++y, gr += nx2) *gr = z;
     }
     for (int i = threadIdx.x; i < nx4; i += blockDim.x) {              // 4 cells of Gw per store
         if (!s_empty[(4 * i + kOwTW / 2) >> kOwTWS]) continue;
@@ -589,8 +593,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                                                           const uint32_t* __restrict__ nitems,
                                                           const uint4* __restrict__ work, uint32_t* __restrict__ ctl,
                                                           const float* __restrict__ tt2, GridPtrs grids,
-                                                          float* __restrict__ scratch, uint32_t* __restrict__ tickets,
-                                                          float2* __restrict__ H, Stats* __restrict__ stats) {
+                                                          float* __restrict__ scratch, uint32_t* __restrict__ tickets) {
     extern __shared__ __align__(16) unsigned char smem[];
     int* sA = reinterpret_cast<int*>(smem + kOwOffA);
     int* sB = reinterpret_cast<int*>(smem + kOwOffB);
@@ -605,15 +608,6 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     __shared__ uint32_t sWork;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // STORE mode also writes H = G + i*alpha*Gw, the FFT input (what k_pack would produce): alpha from the sums that
-    // k_owner_count accumulated earlier on the stream
-    float al = 1.0f;
-    if (STORE) {
-        const double v2 = stats->sum_val2, w2 = stats->sum_wt2;
-        if (v2 > 0.0 && w2 > 0.0) al = exp2f(rintf(0.5f * log2f((float)(v2 / w2))));
-        al = fminf(fmaxf(al, 9.5367431640625e-07f), 1048576.0f);
-        if (blockIdx.x == 0 && tid == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
-    }
     {   // stage the two-parity table once per CTA
         const float4* src = reinterpret_cast<const float4*>(tt2);
         float4* dst = reinterpret_cast<float4*>(sT);
@@ -626,7 +620,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     // zero-fill units (one per grid and row of tiles) spread evenly between them (every k-th position), so that the
     // store-bound fills and the issue-bound gridding units are resident on an SM at the same time.
     const uint32_t n_items = *nitems, n_light = ctl[0];
-    const uint32_t n_fill = STORE ? (uint32_t)g.ngrids * (uint32_t)g.nty : 0u;
+    const uint32_t n_fill = STORE ? (uint32_t)g.ngrids * (uint32_t)g.oty : 0u;
     const uint32_t n_rest = n_light + n_fill, n_work = n_items + n_rest;
     const uint32_t kfill = n_fill ? max(n_rest / n_fill, 1u) : 1u;
 
@@ -643,7 +637,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     if (STORE && !heavy) {
         const uint32_t j = li, f = j / kfill;
         if (f < n_fill && j == f * kfill) {                           // fill unit f: zero the empty tiles of one tile row
-            ow_fill_row(g, bin_offset, grids, H, (int)(f / (uint32_t)g.nty), (int)(f % (uint32_t)g.nty),
+            ow_fill_row(g, bin_offset, grids, (int)(f / (uint32_t)g.oty), (int)(f % (uint32_t)g.oty),
                         reinterpret_cast<unsigned char*>(sH));
             continue;
         }
@@ -662,10 +656,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         start = bin_offset[bin];
         if (tid == 0) cursor[bin] = 0;
     }
-    const int x0 = tx * kOwTW - kOwTW / 2, y0 = ty * kTile - kTile / 2;
+    const int x0 = tx * kOwTW - kOwTW / 2, y0 = (g.ny >> 1) + ty * kTile;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
     float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
-    float2* __restrict__ Ht = H + (size_t)gi * g.ny * g.nx;
     {   // zero the fixed-point tile
         int4* za = reinterpret_cast<int4*>(smem + kOwOffA);
         for (int i = tid; i < (kOwOffH - kOwOffA) / 16; i += 256) za[i] = make_int4(0, 0, 0, 0);
@@ -800,12 +793,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             const int c2 = tid % kG4, r0 = tid / kG4, gx = x0 + 2 * c2;
             if ((unsigned)gx < (unsigned)g.nx) {
                 const int* pa = sA + 2 * (r0 * kOwPitch + 2 * c2);
-                const int* pb = sB + r0 * kOwPitch + 2 * c2;
                 const long long goff = (long long)(y0 + r0) * g.nx + gx;   // before the grid for gy < 0: not dereferenced
                 float4* gd = reinterpret_cast<float4*>(Gt + goff);
-                float4* hd = reinterpret_cast<float4*>(Ht + goff);
                 const size_t gstep = (size_t)kStep * (g.nx >> 1);
-                const float sw = iw * al;
 #pragma unroll
                 for (int k = 0; k < 32 / kStep; ++k) {
                     if ((unsigned)(y0 + r0 + k * kStep) < (unsigned)g.ny) {
@@ -813,10 +803,6 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                         float4 v = make_float4((float)a.x * iv, (float)a.y * iv, (float)a.z * iv, (float)a.w * iv);
                         if (!STORE) { const float4 o = gd[k * gstep]; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
                         gd[k * gstep] = v;
-                        if (STORE) {
-                            const int2 wq = *reinterpret_cast<const int2*>(pb + k * kStep * kOwPitch);
-                            hd[k * gstep] = make_float4(v.x, v.y + (float)wq.x * sw, v.z, v.w + (float)wq.y * sw);
-                        }
                     }
                 }
             }
@@ -862,7 +848,6 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     if (!sLast) continue;
     __threadfence();
     const float4* parts = reinterpret_cast<const float4*>(scratch + (size_t)first_slot * kOwTileFloats);
-    float* sWsum = reinterpret_cast<float*>(smem + kOwOffB);          // summed weight tile, dense [32][32], for H
     for (int j = tid; j < 32 * kW4; j += 256) {                       // weights first
         const int i = 32 * kG4 + j;
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -871,14 +856,12 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
         }
         const int gx = x0 + 4 * (j % kW4), gy = y0 + (j / kW4);
-        if (STORE) *reinterpret_cast<float4*>(sWsum + 4 * j) = v;
         if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
             float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
             if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
             *dst = v;
         }
     }
-    __syncthreads();
     for (int i = tid; i < 32 * kG4; i += 256) {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
         for (uint32_t q = 0; q < nchunks; ++q) {
@@ -890,11 +873,6 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
             if (!STORE) { const float4 o = *dst; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
             *dst = v;
-            if (STORE) {
-                const float2 wq = *reinterpret_cast<const float2*>(sWsum + 2 * i);
-                *reinterpret_cast<float4*>(Ht + (size_t)gy * g.nx + gx) =
-                    make_float4(v.x, v.y + al * wq.x, v.z, v.w + al * wq.y);
-            }
         }
     }
     if (tid == 0) tickets[first_slot] = 0;
@@ -942,16 +920,16 @@ cudaError_t owner_kernel_setup(int max_smem_bytes) {
 
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
-                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, float2* H,
-                              Stats* stats, int store_mode, int num_sms, cudaStream_t s) {
+                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, int store_mode,
+                              int num_sms, cudaStream_t s) {
     const size_t smem = owner_smem_bytes(g.Q);
     const unsigned blocks = (unsigned)num_sms * 4u;
     if (store_mode) {
         k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, work, ctl, tt2, grids,
-                                                     scratch, tickets, H, stats);
+                                                     scratch, tickets);
     } else {
         k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, work, ctl, tt2, grids,
-                                                     scratch, tickets, H, stats);
+                                                     scratch, tickets);
     }
     return cudaGetLastError();
 }

@@ -12,24 +12,20 @@ import gpu_util as gu
 
 pytestmark = pytest.mark.gpu
 
-DIRECT, TILED, OWNER = binding.MUSER_STRATEGY_DIRECT, binding.MUSER_STRATEGY_TILED, binding.MUSER_STRATEGY_OWNER
+TILED, OWNER = binding.MUSER_STRATEGY_TILED, binding.MUSER_STRATEGY_OWNER
 
 
-@pytest.mark.parametrize("strategy", [OWNER, TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [OWNER, TILED])
 @pytest.mark.parametrize("cfg", [1, 2, 3])
 def test_single_grid_configs_match_oracle(cfg, strategy):
     fr = synth.make_frame(cfg)
     p = fr.params
-    # DIRECT sums each cell in arrival order of ~1e3 fp32 global reductions on the hot cells of cfgs 2 and 3: its grid
-    # passes, its corrected image sits around 1e-4 of the peak and moves from run to run with the reduction order.  It
-    # is the fallback for batches of small grids with a support other than 7, so its images are gated on cfg 1 only.
-    images = not (strategy == DIRECT and cfg > 1)
     res = gu.run_case(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, p.n, p.cell_arcsec, p.support, p.oversample,
-                      kernel=p.kernel, strategy=strategy, images=images)
+                      kernel=p.kernel, strategy=strategy)
     assert res["stats"]["n_gridded"] > 0.9 * fr.nvis
 
 
-@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [TILED])
 @pytest.mark.parametrize("S,Q,nvis", [(7, 128, 1), (7, 16, 31), (7, 128, 5000), (3, 8, 777), (5, 32, 1000), (9, 64, 1500),
                                       (1, 2, 100), (15, 16, 300)])
 def test_random_visibilities_any_support(S, Q, nvis, strategy):
@@ -38,7 +34,7 @@ def test_random_visibilities_any_support(S, Q, nvis, strategy):
     gu.run_case(uvw, freq, vis, wt, n, cell, S, Q, strategy=strategy)
 
 
-@pytest.mark.parametrize("strategy", [OWNER, TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [OWNER, TILED])
 def test_accumulation_over_calls_equals_one_call(strategy):
     fr = synth.make_frame(2)
     p = fr.params
@@ -46,7 +42,7 @@ def test_accumulation_over_calls_equals_one_call(strategy):
                 strategy=strategy, splits=5, images=False)
 
 
-@pytest.mark.parametrize("strategy", [OWNER, TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [OWNER, TILED])
 def test_flagged_and_off_grid_visibilities_are_skipped_and_counted(strategy):
     n, cell = 256, 20.0
     uvw, freq, vis, wt = synth.random_visibilities(3, 4000, n, cell, margin_cells=0.0)   # some fall off the grid
@@ -145,6 +141,40 @@ def test_reset_then_read_back_is_zero_with_lazy_zeroing():
         im.destroy()
 
 
+@pytest.mark.parametrize("strategy", [OWNER, TILED])
+def test_side_stream_first_call_and_scratch_growth(strategy):
+    """Every call on a non-blocking side stream (torch.cuda.Stream()), starting with a fresh handle: the library's own
+    zero-initialisations (histograms, tickets, grids after set_batch) must be ordered before the kernels that read
+    them on that stream, on the first call and again when the scratch buffers grow."""
+    import torch
+    n, cell, Q = 256, 20.0, 32
+    side = torch.cuda.Stream()
+    T = gu.oracle_table("pswf", 7, Q)
+    with torch.cuda.stream(side):
+        im = gu.make_imager(n, cell, 7, Q, strategy=strategy)
+        try:
+            for ngrids, nvis in ((1, 500), (3, 40000)):          # the second round re-allocates grids and grows every scratch
+                if ngrids != 1:
+                    im.set_batch(ngrids)
+                uvw, freq, vis, wt = synth.random_visibilities(40 + ngrids, nvis, n, cell, margin_cells=5.5)
+                vis = (vis * 0.05 + 1.0).astype(np.complex64)  # a bright point-like component: image peak well above the noise
+                if nvis > 1000:                                  # crowd the centre tile: heavy-tile chunks and tickets
+                    uvw[: nvis // 2, :2] *= 0.02
+                gid = (np.arange(nvis) % ngrids).astype(np.int32)
+                d = [gu.to_dev(a) for a in (uvw, freq, vis, wt, gid)]
+                im.reset()
+                im.grid_batched(*d)
+                G, Gw = gu.gpu_grids(im)
+                st = im.get_stats()
+                G_or, Gw_or, st_or = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, 7, T, grid_id=gid, ngrids=ngrids)
+                assert st["n_gridded"] == st_or["n_gridded"]
+                assert gu.rel_l2(G, G_or) <= gu.GRID_TOL and gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+                gu.check_images(im, G_or, Gw_or, T, 7, Q)
+        finally:
+            im.destroy()
+    side.synchronize()
+
+
 def test_empty_input_and_reset():
     import torch
     im = gu.make_imager(128, 40.0, 7, 8)
@@ -222,7 +252,7 @@ def _wplane_case(n, cell, P, Q, nvis, w_max, seed, library_tables):
     return wc, sup, tabs, (uvw, freq, vis, wt)
 
 
-@pytest.mark.parametrize("strategy", [TILED, DIRECT])
+@pytest.mark.parametrize("strategy", [TILED])
 @pytest.mark.parametrize("library_tables", [False, True])
 def test_wprojection_planes_match_oracle(strategy, library_tables):
     n, cell, P, Q, w_max = 256, 60.0, 6, 16, 4000.0          # fov 4.3 deg: supports 7..17
@@ -245,7 +275,7 @@ def test_wprojection_planes_match_oracle(strategy, library_tables):
         im.destroy()
 
 
-@pytest.mark.parametrize("strategy", [OWNER, DIRECT, TILED])
+@pytest.mark.parametrize("strategy", [OWNER, TILED])
 def test_batched_grids_cfg4_slice(strategy):
     fr = synth.make_frame(4, nframes=1)                       # 32 grids of 512x512, 1770 visibilities each
     p = fr.params
