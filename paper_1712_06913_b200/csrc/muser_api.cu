@@ -61,7 +61,9 @@ struct muser_imager {
     cufftHandle plan = 0, plan_rows = 0;
     bool plan_ok = false, plan_rows_ok = false, fft_valid = false;
     bool fused_fft = false;                 // row pass by cuFFT, column pass + correction by k_fft_cols_correct
+    bool fused_rows = false;                // row pass by k_fft_rows_half on the stored half-plane (nx a power of two)
     float2* tw_d = nullptr;                 // per-stage twiddles of the fused column transform
+    float2* tw_rows_d = nullptr;            // ... and of the row transform
     cudaStream_t last_stream = nullptr;
     // host-frame staging (muser_frame_host)
     float* in_uvw = nullptr; double* in_freq = nullptr; float2* in_vis = nullptr; float* in_wt = nullptr; int* in_gid = nullptr;
@@ -409,9 +411,25 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     h->last_stream = s;
     int rcz = flush_zero(h, s);
     if (rcz) return rcz;
+    if (h->fused_fft && h->fused_rows) {
+        // A5 rows by k_fft_rows_half straight from the stored half-planes of G and Gw (H = G + i alpha Gw is never
+        // materialised and rows < ny/2 are never read), A5 columns + A6 by the fused column kernel; H keeps the row
+        // transform, so muser_dirty followed by muser_psf repeats only the column pass
+        if (!h->fft_valid) {
+            StageScope sc(h, MUSER_STAGE_FFT, s);
+            CU(h, launch_fft_rows_half(h->geom, h->G, h->Gw, h->tw_rows_d, h->stats_d, h->H, h->num_sms, s));
+            h->n_launches += 1;
+            h->fft_valid = true;
+        }
+        StageScope sc(h, MUSER_STAGE_CORRECT, s);
+        const float* cx = h->correction ? h->icx_d : h->ones_d;
+        const float* cy = h->correction ? h->icy_d : h->ones_d;
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, s));
+        h->n_launches += 1;
+        return MUSER_OK;
+    }
     if (h->fused_fft) {
-        // A5 rows by cuFFT (contiguous 1-D transforms), A5 columns + A6 by the fused kernel; H keeps the row transform,
-        // so muser_dirty followed by muser_psf repeats only the column pass
+        // nx not a power of two: rows by cuFFT (contiguous 1-D transforms of the packed full grid), then as above
         if (!h->plan_rows_ok) {
             int dims[1] = {h->nx};
             cufftResult r = cufftPlanMany(&h->plan_rows, 1, dims, nullptr, 1, h->nx, nullptr, 1, h->nx, CUFFT_C2C, h->ngrids * h->ny);
@@ -527,22 +545,27 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
     if (build_2d_tables(h)) return bail("tables");
     if (rebuild_geom(h)) return bail("geometry");
     if (alloc_grids(h)) return bail("grids");
-    if (fft_cols_supported(nx, ny) && fft_cols_setup() == cudaSuccess) {
-        // per-stage twiddles of the radix-4 stages in thread order: tw[(3 stage + i - 1) T + j], T = ny/4,
-        // = exp(+2 pi i * i * (j mod Ns) / (4 Ns)), Ns = R1 * 4^stage, R1 = 16 or 8 (fp64 on the host)
-        const int T = ny / 4;
+    // per-stage twiddles of the radix-4 stages of a length-n transform in thread order: tw[(3 stage + i - 1) T + j],
+    // T = n/4, = exp(+2 pi i * i * (j mod Ns) / (4 Ns)), Ns = R1 * 4^stage, R1 = 16 or 8 (fp64 on the host)
+    auto twiddles = [&](int n, int r1, float2** out) -> bool {
+        const int T = n / 4;
         std::vector<float2> tw;
-        for (int Ns = fft_cols_first_radix(ny); Ns < ny; Ns *= 4)
+        for (int Ns = r1; Ns < n; Ns *= 4)
             for (int i = 1; i <= 3; ++i)
                 for (int j = 0; j < T; ++j) {
                     const double a = 2.0 * 3.14159265358979323846 * (double)i * (double)(j % Ns) / (4.0 * (double)Ns);
                     tw.push_back(make_float2((float)std::cos(a), (float)std::sin(a)));
                 }
-        if (cudaMalloc(&h->tw_d, tw.size() * sizeof(float2)) != cudaSuccess ||
-            cudaMemcpy(h->tw_d, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
-            h->err = "twiddle table"; return bail("fft");
-        }
+        return cudaMalloc(out, tw.size() * sizeof(float2)) == cudaSuccess &&
+               cudaMemcpy(*out, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess;
+    };
+    if (fft_cols_supported(nx, ny) && fft_cols_setup() == cudaSuccess) {
+        if (!twiddles(ny, fft_cols_first_radix(ny), &h->tw_d)) { h->err = "twiddle table"; return bail("fft"); }
         h->fused_fft = true;
+        if (fft_rows_supported(nx, ny, 0) && fft_rows_supported(nx, ny, 1) && fft_rows_setup() == cudaSuccess) {
+            if (!twiddles(nx, fft_rows_first_radix(nx), &h->tw_rows_d)) { h->err = "twiddle table"; return bail("fft"); }
+            h->fused_rows = true;
+        }
     }
     return h;
 }
@@ -556,7 +579,7 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
     cudaFree(h->ttp_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
-    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->tw_d);
+    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->tw_d); cudaFree(h->tw_rows_d);
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete h;

@@ -148,6 +148,193 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
     }
 }
 
+// ------------------------------------------------------------------------------------------------- row pass
+// A5 (first half) on the STORED HALF-PLANE.  G and Gw are Hermitian about the centre cell [ny/2][nx/2] (every
+// visibility is gridded with its conjugate; "half the grid (as the data is Hermitian)"), and the owner
+// gridder stores rows ny/2 .. ny-1 only.  For a stored row iy the row transforms
+//     a[kx] = sum_ix G [iy][ix] exp(+2 pi i ix kx / nx),      b[kx] = alpha * sum_ix Gw[iy][ix] exp(+2 pi i ix kx / nx)
+// give BOTH rows of the column pass's input Z = rowIFFT(G + i alpha Gw):
+//     Z[iy][kx] = a + i b,        Z[ny - iy][kx] = conj(a) + i conj(b)          (row 0 has no mirror and is zero),
+// because G[ny-iy][nx-ix] = conj G[iy][ix] (column 0 and row 0 are empty by the drop rule R5).  So the lower half-plane
+// is never read (nor written by the gridder), and H = G + i alpha Gw is never materialised.  In 2-D mode Gw is real:
+// two rows are packed into one complex transform, P = FFT(alpha (B1 + i B2)), and separated with
+// b1 = (P[k] + conj P[-k]) / 2, b2 = (P[k] - conj P[-k]) / (2i): 3 transforms per 2 stored rows.
+// Same Stockham scheme as the column pass: radix-16 / radix-8 first stage in registers straight from global memory,
+// radix-4 stages in shared memory on float4 = two sequences (padded, conflict-free), last stage ends in registers.
+template <int N, int WMODE>
+struct RowCfg {
+    static constexpr int ROWS = WMODE ? (N <= 2048 ? 2 : 1) : (N <= 1024 ? 4 : 2);   // stored rows per CTA pass
+    static constexpr int NSEQ = WMODE ? 2 * ROWS : ROWS + ROWS / 2;                 // complex sequences transformed
+    static constexpr int NP = (NSEQ + 1) / 2;                                       // float4 pairs
+    static constexpr int T = N / 4;                                                 // threads = radix-4 butterflies
+    static constexpr int PITCH = N + N / 16 + 2;
+    static constexpr int R1 = (N == 64 || N == 256 || N == 1024 || N == 4096) ? 16 : 8;
+    static constexpr size_t SMEM = (size_t)NP * PITCH * sizeof(float4);
+};
+
+// 16-point inverse DFT in registers: in v[i] = x[i], out v[4 b + c] = X[b + 4 c]
+__device__ __forceinline__ void idft16(float2 (&v)[16]) {
+#pragma unroll
+    for (int a = 0; a < 4; ++a) idft4(v[a], v[a + 4], v[a + 8], v[a + 12]);              // -> u[a][b] at v[a + 4 b]
+    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
+    v[1 + 4 * 1] = cmul(v[1 + 4 * 1], make_float2(c1, s1));
+    v[2 + 4 * 1] = cmul(v[2 + 4 * 1], make_float2(h, h));
+    v[3 + 4 * 1] = cmul(v[3 + 4 * 1], make_float2(s1, c1));
+    v[1 + 4 * 2] = cmul(v[1 + 4 * 2], make_float2(h, h));
+    v[2 + 4 * 2] = make_float2(-v[2 + 4 * 2].y, v[2 + 4 * 2].x);
+    v[3 + 4 * 2] = cmul(v[3 + 4 * 2], make_float2(-h, h));
+    v[1 + 4 * 3] = cmul(v[1 + 4 * 3], make_float2(s1, c1));
+    v[2 + 4 * 3] = cmul(v[2 + 4 * 3], make_float2(-h, h));
+    v[3 + 4 * 3] = cmul(v[3 + 4 * 3], make_float2(-c1, -s1));
+#pragma unroll
+    for (int b = 0; b < 4; ++b) idft4(v[4 * b], v[4 * b + 1], v[4 * b + 2], v[4 * b + 3]);
+}
+// 8-point inverse DFT in registers: in v[i] = x[i], out X[b] = v[2 b] + v[2 b + 1], X[b + 4] = v[2 b] - v[2 b + 1]
+__device__ __forceinline__ void idft8_half(float2 (&v)[8]) {
+    idft4(v[0], v[2], v[4], v[6]);
+    idft4(v[1], v[3], v[5], v[7]);
+    const float h = 0.70710678118654752f;
+    v[3] = cmul(v[3], make_float2(h, h));
+    v[5] = make_float2(-v[5].y, v[5].x);
+    v[7] = cmul(v[7], make_float2(-h, h));
+}
+
+template <int N, int WMODE>
+__global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int ngroups, const float2* __restrict__ G,
+                                                         const float* __restrict__ Gw, const float2* __restrict__ tw,
+                                                         Stats* __restrict__ stats, float2* __restrict__ Z) {
+    using C = RowCfg<N, WMODE>;
+    constexpr int T = C::T, PITCH = C::PITCH, R1 = C::R1, ROWS = C::ROWS, NSEQ = C::NSEQ, NP = C::NP;
+    extern __shared__ __align__(16) float4 sm[];
+    const int tid = threadIdx.x;
+    auto pad = [](int i) { return i + (i >> 4); };
+    // alpha balances G against Gw in the packed transform (power of two: exact); same rule as k_pack
+    float al = 1.0f;
+    {
+        const double v2 = stats->sum_val2, w2 = stats->sum_wt2;
+        if (v2 > 0.0 && w2 > 0.0) al = exp2f(rintf(0.5f * log2f((float)(v2 / w2))));
+        al = fminf(fmaxf(al, 9.5367431640625e-07f), 1048576.0f);
+        if (blockIdx.x == 0 && tid == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
+    }
+    const int hy = ny >> 1, gpg = hy / ROWS;                       // row groups per grid
+    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const int gi = grp / gpg, iy0 = hy + (grp - gi * gpg) * ROWS;
+        const size_t gbase = (size_t)gi * ny * N;
+        __syncthreads();                                           // the previous group is done with the shared buffers
+        // ---- stage 1: radix R1 straight from global memory; sequence s, butterfly j -> y_s[R1 j + i]
+        for (int task = tid; task < NSEQ * (N / R1); task += T) {
+            const int s = task / (N / R1), j = task - s * (N / R1);
+            float2 v[R1];
+            if (WMODE) {
+                const size_t row = gbase + (size_t)(iy0 + (s >> 1)) * N;
+                if (s & 1) {
+                    const float2* src = reinterpret_cast<const float2*>(Gw) + row;
+#pragma unroll
+                    for (int i = 0; i < R1; ++i) { const float2 q = __ldg(src + j + i * (N / R1)); v[i] = make_float2(al * q.x, al * q.y); }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < R1; ++i) v[i] = __ldg(G + row + j + i * (N / R1));
+                }
+            } else if (s < ROWS) {
+                const size_t row = gbase + (size_t)(iy0 + s) * N;
+#pragma unroll
+                for (int i = 0; i < R1; ++i) v[i] = __ldg(G + row + j + i * (N / R1));
+            } else {
+                const size_t row = gbase + (size_t)(iy0 + 2 * (s - ROWS)) * N;
+#pragma unroll
+                for (int i = 0; i < R1; ++i)
+                    v[i] = make_float2(al * __ldg(Gw + row + j + i * (N / R1)), al * __ldg(Gw + row + N + j + i * (N / R1)));
+            }
+            float2* dst = reinterpret_cast<float2*>(sm + (s >> 1) * PITCH) + (s & 1);
+            if constexpr (R1 == 16) {
+                idft16(v);
+#pragma unroll
+                for (int b = 0; b < 4; ++b)
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc) dst[2 * pad(16 * j + b + 4 * cc)] = v[4 * b + cc];
+            } else {
+                idft8_half(v);
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const float2 p0 = v[2 * b], p1 = v[2 * b + 1];
+                    dst[2 * pad(8 * j + b)] = make_float2(p0.x + p1.x, p0.y + p1.y);
+                    dst[2 * pad(8 * j + b + 4)] = make_float2(p0.x - p1.x, p0.y - p1.y);
+                }
+            }
+        }
+        __syncthreads();
+        // ---- radix-4 stages in shared memory; the last one ends in registers: v[s][i] = X_s[j + i T]
+        const int j = tid;
+        float2 v[2 * NP][4];
+        const float2* twp = tw + j;
+#pragma unroll 1
+        for (int Ns = R1; Ns < N; Ns *= 4, twp += 3 * T) {
+            const int k = j & (Ns - 1);
+            const float2 w1 = __ldg(twp), w2 = __ldg(twp + T), w3 = __ldg(twp + 2 * T);
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                const float4* src = sm + p * PITCH;
+                const float4 q0 = src[pad(j)], q1 = src[pad(j + T)], q2 = src[pad(j + 2 * T)], q3 = src[pad(j + 3 * T)];
+                v[2 * p][0] = make_float2(q0.x, q0.y); v[2 * p + 1][0] = make_float2(q0.z, q0.w);
+                v[2 * p][1] = cmul(make_float2(q1.x, q1.y), w1); v[2 * p + 1][1] = cmul(make_float2(q1.z, q1.w), w1);
+                v[2 * p][2] = cmul(make_float2(q2.x, q2.y), w2); v[2 * p + 1][2] = cmul(make_float2(q2.z, q2.w), w2);
+                v[2 * p][3] = cmul(make_float2(q3.x, q3.y), w3); v[2 * p + 1][3] = cmul(make_float2(q3.z, q3.w), w3);
+                idft4(v[2 * p][0], v[2 * p][1], v[2 * p][2], v[2 * p][3]);
+                idft4(v[2 * p + 1][0], v[2 * p + 1][1], v[2 * p + 1][2], v[2 * p + 1][3]);
+            }
+            if (Ns * 4 == N) break;
+            __syncthreads();
+            const int o = (j - k) * 4 + k;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                float4* dst = sm + p * PITCH;
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    dst[pad(o + i * Ns)] = make_float4(v[2 * p][i].x, v[2 * p][i].y, v[2 * p + 1][i].x, v[2 * p + 1][i].y);
+            }
+            __syncthreads();
+        }
+        // ---- epilogue: both rows of Z per stored row
+        if (!WMODE) {
+            // the packed weight transforms go through shared memory once more: every thread needs P[N - kx]
+            __syncthreads();
+            float4* pp = sm + (NP - 1) * PITCH;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float2 p0 = v[ROWS][i], p1 = (ROWS == 4) ? v[ROWS + 1][i] : make_float2(0.f, 0.f);
+                pp[pad(j + i * T)] = make_float4(p0.x, p0.y, p1.x, p1.y);
+            }
+            __syncthreads();
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int kx = j + i * T;
+            float2 b[ROWS];
+            if (WMODE) {
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) b[r] = v[2 * r + 1][i];
+            } else {
+                const float4 pm = sm[(NP - 1) * PITCH + pad((N - kx) & (N - 1))];
+#pragma unroll
+                for (int q = 0; q < ROWS / 2; ++q) {
+                    const float2 P = v[ROWS + q][i];
+                    const float2 Pc = q ? make_float2(pm.z, -pm.w) : make_float2(pm.x, -pm.y);      // conj P[-k]
+                    b[2 * q] = make_float2(0.5f * (P.x + Pc.x), 0.5f * (P.y + Pc.y));
+                    b[2 * q + 1] = make_float2(0.5f * (P.y - Pc.y), -0.5f * (P.x - Pc.x));         // (P - Pc) / (2i)
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                const float2 a = WMODE ? v[2 * r][i] : v[r][i];
+                const int iy = iy0 + r;
+                Z[gbase + (size_t)iy * N + kx] = make_float2(a.x - b[r].y, a.y + b[r].x);
+                const float2 lo = (iy == hy) ? make_float2(0.f, 0.f) : make_float2(a.x + b[r].y, b[r].x - a.y);
+                Z[gbase + (size_t)(iy == hy ? 0 : ny - iy) * N + kx] = lo;
+            }
+        }
+    }
+}
+
 static size_t fft_smem_bytes(int N) { return (size_t)(kFftC / 2) * (N + N / 16 + 2) * sizeof(float4); }
 
 bool fft_cols_supported(int nx, int ny) { return (ny == 256 || ny == 512 || ny == 1024) && (nx % 16) == 0; }
@@ -159,6 +346,57 @@ cudaError_t fft_cols_setup() {
     if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
     if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
     return cudaSuccess;
+}
+
+template <int N, int WMODE>
+static cudaError_t launch_rows_t(const Geom& g, const float2* G, const float* Gw, const float2* tw, Stats* stats, float2* Z,
+                                 int num_sms, cudaStream_t s) {
+    using C = RowCfg<N, WMODE>;
+    const int ngroups = g.ngrids * ((g.ny / 2) / C::ROWS);
+    int per_sm = (int)(200 * 1024 / (C::SMEM + 1024));
+    per_sm = per_sm < 1 ? 1 : (per_sm > 2048 / C::T ? 2048 / C::T : per_sm);
+    const int blocks = ngroups < num_sms * per_sm ? ngroups : num_sms * per_sm;
+    k_fft_rows_half<N, WMODE><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, tw, stats, Z);
+    return cudaGetLastError();
+}
+
+template <int N>
+static cudaError_t rows_setup_t() {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(k_fft_rows_half<N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 0>::SMEM))) return e;
+    return cudaFuncSetAttribute(k_fft_rows_half<N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 1>::SMEM);
+}
+
+int fft_rows_first_radix(int nx) { return (nx == 64 || nx == 256 || nx == 1024 || nx == 4096) ? 16 : 8; }
+int fft_rows_group(int nx, int wmode) { return wmode ? (nx <= 2048 ? 2 : 1) : (nx <= 1024 ? 4 : 2); }
+bool fft_rows_supported(int nx, int ny, int wmode) {
+    const bool pow2 = nx >= 64 && nx <= 4096 && (nx & (nx - 1)) == 0;
+    return pow2 && ((ny / 2) % fft_rows_group(nx, wmode)) == 0;
+}
+
+cudaError_t fft_rows_setup() {
+    cudaError_t e;
+    if ((e = rows_setup_t<64>())) return e;
+    if ((e = rows_setup_t<128>())) return e;
+    if ((e = rows_setup_t<256>())) return e;
+    if ((e = rows_setup_t<512>())) return e;
+    if ((e = rows_setup_t<1024>())) return e;
+    if ((e = rows_setup_t<2048>())) return e;
+    return rows_setup_t<4096>();
+}
+
+cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const float2* tw, Stats* stats, float2* Z,
+                                 int num_sms, cudaStream_t s) {
+#define MUSER_ROWS_CASE(NN)                                                                                     \
+    case NN:                                                                                                    \
+        return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, tw, stats, Z, num_sms, s)                               \
+                       : launch_rows_t<NN, 0>(g, G, Gw, tw, stats, Z, num_sms, s);
+    switch (g.nx) {
+        MUSER_ROWS_CASE(64) MUSER_ROWS_CASE(128) MUSER_ROWS_CASE(256) MUSER_ROWS_CASE(512) MUSER_ROWS_CASE(1024)
+        MUSER_ROWS_CASE(2048) MUSER_ROWS_CASE(4096)
+        default: return cudaErrorInvalidValue;
+    }
+#undef MUSER_ROWS_CASE
 }
 
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,

@@ -113,6 +113,12 @@ cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t
 bool fft_cols_supported(int nx, int ny);
 int fft_cols_first_radix(int ny);
 cudaError_t fft_cols_setup();
+// row pass on the stored half-plane (nx a power of two in [64, 4096]): Z = row transform of G + i alpha Gw, all ny rows
+bool fft_rows_supported(int nx, int ny, int wmode);
+int fft_rows_first_radix(int nx);
+cudaError_t fft_rows_setup();
+cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const float2* tw, Stats* stats, float2* Z,
+                                 int num_sms, cudaStream_t s);
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
                                     const Stats* stats, float* dirty, float* psf, cudaStream_t s);
 
