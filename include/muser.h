@@ -80,6 +80,11 @@ int muser_set_batch(muser_imager* h, int ngrids);
 int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, const int* supports,
                       const float* const* tables_c64);
 int muser_set_strategy(muser_imager* h, int strategy);
+/* Tuning knobs of the OWNER strategy (results do not depend on them beyond fp32 summation order).  ITEM_SIZE: records
+ * per chunk of a heavy tile (a tile with more records is split into chunks gridded by different CTAs and summed);
+ * 0 (default) = chosen from the size of the call. */
+enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_COUNT = 1 };
+int muser_set_tuning(muser_imager* h, int key, int value);
 /* 1 (default): A6 divides by the kernel's transform; 0: A6 only shifts/takes the real part (parity gate R9(i)). */
 int muser_set_grid_correction(muser_imager* h, int enabled);
 

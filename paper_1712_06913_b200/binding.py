@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libmuser.so")
 MUSER_OK, MUSER_EINVAL, MUSER_ECUDA, MUSER_ENOMEM, MUSER_ESTATE, MUSER_EUNSUPPORTED = range(6)
 MUSER_KERNEL_PSWF, MUSER_KERNEL_GAUSS = 0, 1
 MUSER_STRATEGY_AUTO, MUSER_STRATEGY_TILED, MUSER_STRATEGY_OWNER = 0, 2, 3
+MUSER_TUNE_ITEM_SIZE = 0
 STAGES = ("bin", "grid", "pack", "fft", "correct")
 
 _c = ctypes
@@ -28,6 +29,7 @@ SIGNATURES = {
     "muser_set_batch": (_i, [_vp, _i]),
     "muser_set_wplanes": (_i, [_vp, _i, _vp, _vp, _vp]),
     "muser_set_strategy": (_i, [_vp, _i]),
+    "muser_set_tuning": (_i, [_vp, _i, _i]),
     "muser_set_grid_correction": (_i, [_vp, _i]),
     "muser_reset": (_i, [_vp, _vp]),
     "muser_grid": (_i, [_vp, _vp, _vp, _vp, _vp, _ll, _vp]),
@@ -144,6 +146,9 @@ class Imager:
 
     def set_strategy(self, strategy):
         self._ck(lib().muser_set_strategy(self._h, strategy))
+
+    def set_tuning(self, key, value):
+        self._ck(lib().muser_set_tuning(self._h, key, int(value)))
 
     def set_grid_correction(self, enabled):
         self._ck(lib().muser_set_grid_correction(self._h, 1 if enabled else 0))

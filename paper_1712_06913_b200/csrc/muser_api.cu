@@ -31,6 +31,7 @@ struct muser_imager {
     double gauss_a = 1.55;
     int ngrids = 1, nplanes = 0, strategy = MUSER_STRATEGY_AUTO, correction = 1;
     int device = 0, num_sms = 148, max_smem = 0;
+    int tune[MUSER_TUNE_COUNT] = {0};
     Geom geom{};
     std::vector<PlaneMeta> planes_h;
     std::vector<std::vector<float>> tables_f32;     // per plane, oracle order T[t] (floats or (re,im) pairs)
@@ -54,7 +55,7 @@ struct muser_imager {
     float* ow_scratch = nullptr;
     size_t ow_items_cap = 0, ow_sorted_cap = 0, ow_bins_cap = 0;
     uint4 *ow_sorted = nullptr, *ow_loc = nullptr;          // tile-sorted records; per-visibility integer result of O1
-    uint32_t *ow_count = nullptr, *ow_offset = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
+    uint32_t *ow_count = nullptr, *ow_cursor = nullptr, *ow_offset = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
     uint4* ow_work = nullptr;
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     bool lower_valid = true;                // rows 0 .. ny/2-1 of G, Gw are up to date (the owner gridder stores rows >= ny/2 only)
@@ -121,8 +122,8 @@ void free_grids(muser_imager* h) {
 void free_bins(muser_imager* h) {
     cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
     h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
-    cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
-    h->ow_count = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
+    cudaFree(h->ow_count); cudaFree(h->ow_cursor); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
+    h->ow_count = h->ow_cursor = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
 }
 
 int rebuild_geom(muser_imager* h) {
@@ -298,11 +299,12 @@ int pick_strategy(const muser_imager* h) {
     return owner_capable(h) ? MUSER_STRATEGY_OWNER : MUSER_STRATEGY_TILED;
 }
 
-uint32_t owner_item_size(long long nvis, int num_sms) {
+uint32_t owner_item_size(long long nvis, int num_sms, int item_override) {
     // Heavy tiles are split into chunks of item_size samples.  4096 (the gridder's sort capacity) when the call has
     // enough work to fill the machine; down to 1024 for a single small frame, whose latency is the critical path of
     // one chunk (a third of a MUSER frame sits in the tile around the uv origin).  For huge inputs the chunk grows so
     // that the partial-tile scratch (at most 16*nvis/item_size + 2 tiles) stays under 256 MB.
+    if (item_override > 0) return (uint32_t)item_override;
     uint32_t item = 4096;
     const double units = 2.4 * (double)nvis / 4096.0;                // ~2.4 records per visibility on MUSER frames
     while (item > 1024 && units * (4096.0 / item) < 4.0 * num_sms) item /= 2;
@@ -321,9 +323,10 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
     }
     const size_t nb = ((size_t)h->geom.onbins + 8) & ~(size_t)3;
     if (nb > h->ow_bins_cap) {
-        cudaFree(h->ow_count); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
-        h->ow_count = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
+        cudaFree(h->ow_count); cudaFree(h->ow_cursor); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
+        h->ow_count = h->ow_cursor = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
         CU(h, cudaMalloc(&h->ow_count, nb * sizeof(uint32_t)));
+        CU(h, cudaMalloc(&h->ow_cursor, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_offset, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_work, nb * sizeof(uint4)));
         CU(h, cudaMalloc(&h->ow_tops, (nb / 4096 + 2) * 3 * sizeof(uint32_t)));
@@ -356,7 +359,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     GridPtrs gp{h->G, h->Gw};
     if (strat == MUSER_STRATEGY_OWNER) {
         if (!owner_capable(h)) return fail(h, MUSER_EUNSUPPORTED, "the owner-tile strategy needs 2-D mode and support 7");
-        const uint32_t item_size = owner_item_size(nvis, h->num_sms);
+        const uint32_t item_size = owner_item_size(nvis, h->num_sms, h->tune[MUSER_TUNE_ITEM_SIZE]);
         uint32_t max_items = 0;
         int rc = ensure_owner_scratch(h, nvis, item_size, &max_items, s);
         if (rc) return rc;
@@ -366,14 +369,14 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         {
             StageScope sc(h, MUSER_STAGE_BIN, s);
             CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, h->ow_loc, s));
-            CU(h, launch_owner_scan(g, h->ow_count, h->ow_offset, h->ow_items, h->nitems_d, item_size, h->ow_work,
-                                    h->ow_ctl, h->ow_tops, s));
-            CU(h, launch_owner_scatter(g, h->ow_loc, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_count,
+            CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size,
+                                    h->ow_work, h->ow_ctl, h->ow_tops, s));
+            CU(h, launch_owner_scatter(g, h->ow_loc, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_cursor,
                                        h->ow_sorted, s));
         }
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
-            CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_count, h->ow_items, h->nitems_d, h->ow_work,
+            CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work,
                                     h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->zero_pending ? 1 : 0,
                                     h->num_sms, s));
         }
@@ -669,6 +672,14 @@ int muser_set_strategy(muser_imager* h, int strategy) {
     }
     h->strategy = strategy;
     return MUSER_OK;
+}
+
+int muser_set_tuning(muser_imager* h, int key, int value) {
+    if (!h) return MUSER_EINVAL;
+    if (key < 0 || key >= MUSER_TUNE_COUNT) return fail(h, MUSER_EINVAL, "unknown tuning key");
+    if (key == MUSER_TUNE_ITEM_SIZE && value != 0 && (value < 256 || value > (1 << 20))) return fail(h, MUSER_EINVAL, "item_size must be 0 (automatic) or in [256, 2^20]");
+    h->tune[key] = value;
+    return rebuild_geom(h);
 }
 
 int muser_set_grid_correction(muser_imager* h, int enabled) {

@@ -236,8 +236,8 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
 //   k_owner_scan_reduce   per-CTA totals of (samples, chunk items of heavy tiles, light non-empty tiles)
 //   k_owner_scan_tops     one CTA: exclusive scan of the per-CTA totals, grand totals, work counter reset
 //   k_owner_scan_write    per-CTA local scan + base: sample offsets, chunk items of the heavy tiles (more than
-//                         item_size samples), the work list of light non-empty tiles; re-zeroes the histogram
-//                         (k_owner_scatter reuses it as its cursor)
+//                         item_size samples), the work list of light non-empty tiles; re-zeroes the histogram (for
+//                         the next call's O1) and the scatter cursor (for this call's O3)
 struct OwScan3 { uint32_t c, m, l; };
 
 __device__ __forceinline__ OwScan3 ow_block_scan3(OwScan3 v, OwScan3& total, uint32_t (*s_w)[32]) {
@@ -314,6 +314,7 @@ __global__ void __launch_bounds__(1024) k_owner_scan_tops(const Geom g, const ui
 // SINGLE: the whole histogram fits one CTA (<= 4096 bins): no reduce / tops launches, this kernel also writes the totals.
 template <int SINGLE>
 __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_t* __restrict__ bin_count,
+                                                           uint32_t* __restrict__ cursor,
                                                            const uint32_t item_size, const uint32_t* __restrict__ tops,
                                                            uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
                                                            uint4* __restrict__ work, uint32_t* __restrict__ nitems,
@@ -322,7 +323,8 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
     const uint32_t b0 = blockIdx.x * 4096u + 4u * threadIdx.x;
     uint32_t c[4], m[4];
     const OwScan3 t = ow_load4(g, bin_count, b0, item_size, c, m);
-    if (t.c) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);
+    if (t.c) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);      // ready for the next call's O1
+    if (b0 < g.onbins) *reinterpret_cast<uint4*>(cursor + b0) = make_uint4(0, 0, 0, 0);   // ready for this call's O3
     OwScan3 total;
     const OwScan3 ex = ow_block_scan3(t, total, s_w);
     uint32_t off = ex.c, slot = ex.m, wpos = ex.l;
@@ -339,7 +341,7 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
             if (c[j] != 0u && m[j] == 0u) {                            // light non-empty tile: one work unit
                 const uint32_t gi = b / (uint32_t)g.ontiles, tile = b - gi * (uint32_t)g.ontiles;
                 const uint32_t ty = tile / (uint32_t)g.otx;
-                work[wpos++] = make_uint4(b, gi, (ty << 16) | (tile - ty * (uint32_t)g.otx), c[j]);
+                work[wpos++] = make_uint4(off, gi, (ty << 16) | (tile - ty * (uint32_t)g.otx), c[j]);
             }
             for (uint32_t q = 0; q < m[j]; ++q) {
                 OwItem it;
@@ -589,7 +591,7 @@ __device__ __forceinline__ void ow_fill_row(const Geom& g, const uint32_t* __res
 template <int STORE>
 __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
                                                           const uint32_t* __restrict__ bin_offset,
-                                                          uint32_t* __restrict__ cursor, const OwItem* __restrict__ items,
+                                                          const OwItem* __restrict__ items,
                                                           const uint32_t* __restrict__ nitems,
                                                           const uint4* __restrict__ work, uint32_t* __restrict__ ctl,
                                                           const float* __restrict__ tt2, GridPtrs grids,
@@ -630,7 +632,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     __syncthreads();
     const uint32_t wi = sWork;
     if (wi >= n_work) break;
-    uint32_t bin, gi, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
+    uint32_t gi, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
     int tx, ty;
     const bool heavy = wi < n_items;
     uint32_t li = wi - n_items;                                       // index into the light-tile list
@@ -645,16 +647,13 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     }
     if (heavy) {
         const OwItem it = items[wi];
-        bin = it.bin; start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
-        if (chunk == 0 && tid == 0) cursor[bin] = 0;
-        gi = bin / (uint32_t)g.ontiles;
-        const uint32_t tile = bin - gi * (uint32_t)g.ontiles;
+        start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
+        gi = it.bin / (uint32_t)g.ontiles;
+        const uint32_t tile = it.bin - gi * (uint32_t)g.ontiles;
         ty = (int)(tile / (uint32_t)g.otx); tx = (int)(tile - (uint32_t)ty * (uint32_t)g.otx);
     } else {
-        const uint4 wk = __ldg(work + li);                           // {bin, grid, ty << 16 | tx, count}
-        bin = wk.x; gi = wk.y; ty = (int)(wk.z >> 16); tx = (int)(wk.z & 0xFFFFu); cnt = wk.w;
-        start = bin_offset[bin];
-        if (tid == 0) cursor[bin] = 0;
+        const uint4 wk = __ldg(work + li);                           // {start, grid, ty << 16 | tx, count}
+        start = wk.x; gi = wk.y; ty = (int)(wk.z >> 16); tx = (int)(wk.z & 0xFFFFu); cnt = wk.w;
     }
     const int x0 = tx * kOwTW - kOwTW / 2, y0 = (g.ny >> 1) + ty * kTile;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
@@ -890,16 +889,17 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
     return cudaGetLastError();
 }
 
-cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, OwItem* items, uint32_t* nitems,
-                              uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops, cudaStream_t s) {
+cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* cursor, uint32_t* bin_offset, OwItem* items,
+                              uint32_t* nitems, uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops,
+                              cudaStream_t s) {
     const uint32_t nblocks = (g.onbins + 4095u) / 4096u;
     if (nblocks == 1) {
-        k_owner_scan_write<1><<<1, 1024, 0, s>>>(g, bin_count, item_size, tops, bin_offset, items, work, nitems, ctl);
+        k_owner_scan_write<1><<<1, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl);
         return cudaGetLastError();
     }
     k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
     k_owner_scan_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems, ctl);
-    k_owner_scan_write<0><<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops, bin_offset, items, work, nitems, ctl);
+    k_owner_scan_write<0><<<nblocks, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl);
     return cudaGetLastError();
 }
 
@@ -918,17 +918,17 @@ cudaError_t owner_kernel_setup(int max_smem_bytes) {
     return cudaSuccess;
 }
 
-cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset, uint32_t* cursor,
+cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
                               const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, int store_mode,
                               int num_sms, cudaStream_t s) {
     const size_t smem = owner_smem_bytes(g.Q);
     const unsigned blocks = (unsigned)num_sms * 4u;
     if (store_mode) {
-        k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, work, ctl, tt2, grids,
+        k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids,
                                                      scratch, tickets);
     } else {
-        k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, cursor, items, nitems, work, ctl, tt2, grids,
+        k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids,
                                                      scratch, tickets);
     }
     return cudaGetLastError();
