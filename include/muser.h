@@ -82,8 +82,9 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
 int muser_set_strategy(muser_imager* h, int strategy);
 /* Tuning knobs of the OWNER strategy (results do not depend on them beyond fp32 summation order).  ITEM_SIZE: records
  * per chunk of a heavy tile (a tile with more records is split into chunks gridded by different CTAs and summed);
- * 0 (default) = chosen from the size of the call. */
-enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_COUNT = 1 };
+ * 0 (default) = chosen from the size of the call.  BIN_VPT: visibilities per thread of the binning kernels (1, 2, 4;
+ * 0 = automatic). */
+enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_BIN_VPT = 1, MUSER_TUNE_COUNT = 2 };
 int muser_set_tuning(muser_imager* h, int key, int value);
 /* 1 (default): A6 divides by the kernel's transform; 0: A6 only shifts/takes the real part (parity gate R9(i)). */
 int muser_set_grid_correction(muser_imager* h, int enabled);

@@ -368,11 +368,12 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         h->fft_valid = false;
         {
             StageScope sc(h, MUSER_STAGE_BIN, s);
-            CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, h->ow_loc, s));
+            CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, h->ow_loc,
+                                     h->tune[MUSER_TUNE_BIN_VPT], s));
             CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size,
                                     h->ow_work, h->ow_ctl, h->ow_tops, s));
             CU(h, launch_owner_scatter(g, h->ow_loc, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_cursor,
-                                       h->ow_sorted, s));
+                                       h->ow_sorted, h->tune[MUSER_TUNE_BIN_VPT], s));
         }
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
@@ -678,6 +679,7 @@ int muser_set_tuning(muser_imager* h, int key, int value) {
     if (!h) return MUSER_EINVAL;
     if (key < 0 || key >= MUSER_TUNE_COUNT) return fail(h, MUSER_EINVAL, "unknown tuning key");
     if (key == MUSER_TUNE_ITEM_SIZE && value != 0 && (value < 256 || value > (1 << 20))) return fail(h, MUSER_EINVAL, "item_size must be 0 (automatic) or in [256, 2^20]");
+    if (key == MUSER_TUNE_BIN_VPT && value != 0 && value != 1 && value != 2 && value != 4) return fail(h, MUSER_EINVAL, "bin_vpt must be 0, 1, 2 or 4");
     h->tune[key] = value;
     return rebuild_geom(h);
 }

@@ -97,13 +97,13 @@ struct OwItem {                              // one chunk of a heavy tile (more 
 };
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                                const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, uint4* loc,
-                               cudaStream_t s);
+                               int vpt_forced, cudaStream_t s);
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* cursor, uint32_t* bin_offset, OwItem* items,
                               uint32_t* nitems, uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops,
                               cudaStream_t s);
 cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float2* vis, const float* wt, const int* grid_id,
                                  long long nvis, const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted,
-                                 cudaStream_t s);
+                                 int vpt_forced, cudaStream_t s);
 cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,

@@ -52,10 +52,12 @@ struct OwLoc {
     int gid;
 };
 
+// `f_cache`/`il_cache`: the division f/c is repeated only when the frequency differs from the thread's previous
+// visibility (a thread's visibilities are 256 apart: almost always the same channel).
 __device__ __forceinline__ void ow_locate(const Geom& g, const float* __restrict__ uvw, const double* __restrict__ freq,
                                           const float2* __restrict__ vis, const float* __restrict__ weight,
                                           const int* __restrict__ grid_id, long long k, long long nvis, OwLoc& L,
-                                          float2& Vraw) {
+                                          float2& Vraw, double& f_cache, double& il_cache) {
     L.state = 0;
     if (k >= nvis) return;
     const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
@@ -64,7 +66,8 @@ __device__ __forceinline__ void ow_locate(const Geom& g, const float* __restrict
     const float wt = weight[k];
     const int gid = grid_id ? grid_id[k] : 0;
     Vraw = V;
-    const double il = __ddiv_rn(f, kC);
+    if (f != f_cache) { il_cache = __ddiv_rn(f, kC); f_cache = f; }
+    const double il = il_cache;
     const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
     const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) && isfinite(V.y) &&
                     isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
@@ -116,18 +119,6 @@ __device__ __forceinline__ uint32_t ow_agg_inc(uint32_t* __restrict__ cnt, uint3
 constexpr int kBinThreads = 256;
 constexpr int kBinSmemTiles = 4096;      // two u32 arrays of this many tiles must fit the default 48 KB
 
-// One barrier: zero the CTA histogram(s), then agree (barrier-and) that every kept visibility of the CTA has the grid id
-// of the CTA's first visibility.  Returns that grid id, or -1 if the CTA must take the global-atomics path.
-__device__ __forceinline__ int ow_cta_uniform_grid(const Geom& g, const OwLoc& L, const int* __restrict__ grid_id,
-                                                   uint32_t* s_hist, int nhist) {
-    const bool fits = g.ontiles <= kBinSmemTiles;
-    if (fits)
-        for (int i = threadIdx.x; i < nhist * g.ontiles; i += blockDim.x) s_hist[i] = 0;
-    const int ref = grid_id ? grid_id[(long long)blockIdx.x * blockDim.x] : 0;
-    const int same = __syncthreads_and(L.state != 3 || L.gid == ref);
-    return (fits && same && ref >= 0 && ref < g.ngrids) ? ref : -1;
-}
-
 // The (at most 2 x 2) tiles a 7x7 footprint at nearest cell (cu, cv) touches: first tile (tx0, ty0) and whether the
 // footprint also reaches the next tile in x / in y.
 struct OwTiles { int tx0, ty0, t00; bool mx, my, up; };
@@ -144,67 +135,102 @@ __device__ __forceinline__ OwTiles ow_tiles(const Geom& g, int cu, int cv) {
 }
 
 // ------------------------------------------------------------------------------------------------- O1 count
+// packed tiles of one sample: first tile t00 | reaches the next tile in x << 29 | in y << 30 | touches the stored
+// half-plane << 31 (0 = the sample has no record)
+__device__ __forceinline__ uint32_t ow_tiles_packed(const Geom& g, int cu, int cv) {
+    const OwTiles t = ow_tiles(g, cu, cv);
+    return t.up ? ((uint32_t)t.t00 | (t.mx ? 1u << 29 : 0u) | (t.my ? 1u << 30 : 0u) | 1u << 31) : 0u;
+}
+
+// A CTA handles 256 * VPT consecutive visibilities (thread: k, k + 256, ...), so that the per-CTA work (histogram
+// zeroing and flush, statistics reduction) is shared by VPT visibilities per thread; VPT = 1 for small calls.
+template <int VPT>
 __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const float* __restrict__ uvw,
                                                              const double* __restrict__ freq, const float2* __restrict__ vis,
                                                              const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                              const long long nvis, uint32_t* __restrict__ bin_count,
                                                              Stats* __restrict__ stats, uint4* __restrict__ loc) {
     extern __shared__ uint32_t s_hist[];
-    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long base = (long long)blockIdx.x * (kBinThreads * VPT);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    OwLoc L;
-    float2 V;
-    ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V);
-    if (k < nvis) {                                                   // integer result of O1 for k_owner_scatter
-        uint4 o = make_uint4(0u, 0u, (uint32_t)L.state << 30, 0u);
-        if (L.state == 3) {
-            o.x = (uint32_t)L.cu[0] | ((uint32_t)L.cv[0] << 16);
-            o.y = (uint32_t)L.cu[1] | ((uint32_t)L.cv[1] << 16);
-            o.z |= (uint32_t)L.rx[0] | ((uint32_t)L.ry[0] << 9) | ((uint32_t)L.rx[1] << 18);
-            o.w = (uint32_t)L.ry[1];
+    const bool fits = g.ontiles <= kBinSmemTiles;
+    if (fits)
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
+    const int ref = grid_id ? grid_id[base] : 0;                      // base < nvis by the launch geometry
+    uint32_t tp[VPT][2];
+    int gidv[VPT];
+    int kept = 0, dropped = 0, flagged = 0, same = 1;
+    double wsum = 0.0, v2sum = 0.0, w2sum = 0.0, f_cache = 0.0, il_cache = 0.0;
+#pragma unroll
+    for (int j = 0; j < VPT; ++j) {
+        const long long k = base + j * kBinThreads + threadIdx.x;
+        OwLoc L;
+        float2 V;
+        ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V, f_cache, il_cache);
+        tp[j][0] = tp[j][1] = 0u;
+        gidv[j] = 0;
+        if (k < nvis) {                                               // integer result of O1 for k_owner_scatter
+            uint4 o = make_uint4(0u, 0u, (uint32_t)L.state << 30, 0u);
+            if (L.state == 3) {
+                o.x = (uint32_t)L.cu[0] | ((uint32_t)L.cv[0] << 16);
+                o.y = (uint32_t)L.cu[1] | ((uint32_t)L.cv[1] << 16);
+                o.z |= (uint32_t)L.rx[0] | ((uint32_t)L.ry[0] << 9) | ((uint32_t)L.rx[1] << 18);
+                o.w = (uint32_t)L.ry[1];
+                tp[j][0] = ow_tiles_packed(g, L.cu[0], L.cv[0]);
+                tp[j][1] = ow_tiles_packed(g, L.cu[1], L.cv[1]);
+                gidv[j] = L.gid;
+                same &= (L.gid == ref);
+                ++kept;
+                wsum += 2.0 * (double)L.wt;
+                const double w2 = (double)L.wt * (double)L.wt;
+                w2sum += w2;
+                v2sum += w2 * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
+            }
+            dropped += L.state == 2;
+            flagged += L.state == 1;
+            loc[k] = o;
         }
-        loc[k] = o;
     }
-    const int kept = L.state == 3, dropped = L.state == 2, flagged = L.state == 1;
-    double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
-    if (kept) {
-        wsum = 2.0 * (double)L.wt;
-        w2sum = (double)L.wt * (double)L.wt;
-        v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
-    }
-    const int ugrid = ow_cta_uniform_grid(g, L, grid_id, s_hist, 1);
+    // one barrier: the histogram is zeroed, and the CTA agrees whether all its kept visibilities share one grid
+    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
     if (ugrid >= 0) {
-        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
-        if (kept) {
+#pragma unroll
+        for (int j = 0; j < VPT; ++j)
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
-                const OwTiles t = ow_tiles(g, L.cu[s], L.cv[s]);
-                if (!t.up) continue;
-                atomicAdd(&s_hist[t.t00], 1u);
-                if (t.mx) atomicAdd(&s_hist[t.t00 + 1], 1u);
-                if (t.my) atomicAdd(&s_hist[t.t00 + g.otx], 1u);
-                if (t.mx && t.my) atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u);
+                const uint32_t t = tp[j][s];
+                if (!(t >> 31)) continue;
+                const uint32_t t00 = t & 0x1FFFFFFFu;
+                const bool mx = (t >> 29) & 1u, my = (t >> 30) & 1u;
+                atomicAdd(&s_hist[t00], 1u);
+                if (mx) atomicAdd(&s_hist[t00 + 1], 1u);
+                if (my) atomicAdd(&s_hist[t00 + g.otx], 1u);
+                if (mx && my) atomicAdd(&s_hist[t00 + g.otx + 1], 1u);
             }
-        }
         __syncthreads();
-        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) {
+        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
             const uint32_t n = s_hist[i];
             if (n) atomicAdd(&bin_count[gbase + i], n);
         }
-    } else if (__any_sync(kFull, kept)) {
+    } else {
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
+        for (int j = 0; j < VPT; ++j)
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                int tx, ty;
-                const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
-                if (__any_sync(kFull, bin != kNoBin)) ow_agg_inc(bin_count, bin, lane);
-            }
-        }
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t t = tp[j][s];
+                    const bool on = (t >> 31) && (!(q & 1) || ((t >> 29) & 1u)) && (!(q & 2) || ((t >> 30) & 1u));
+                    const uint32_t bin = on ? (uint32_t)gidv[j] * (uint32_t)g.ontiles + (t & 0x1FFFFFFFu) + (q & 1) +
+                                                  ((q & 2) ? (uint32_t)g.otx : 0u)
+                                            : kNoBin;
+                    if (__any_sync(kFull, on)) ow_agg_inc(bin_count, bin, lane);
+                }
     }
     // block reduction of the counters, one atomic set per block
-    __shared__ int s_cnt[3][32];
-    __shared__ double s_w[3][32];
+    __shared__ int s_cnt[3][8];
+    __shared__ double s_w[3][8];
     const int c0 = __reduce_add_sync(kFull, kept), c1 = __reduce_add_sync(kFull, dropped), c2 = __reduce_add_sync(kFull, flagged);
     for (int o = 16; o > 0; o >>= 1) {
         wsum += __shfl_xor_sync(kFull, wsum, o);
@@ -216,7 +242,7 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
     if (threadIdx.x == 0) {
         int t0 = 0, t1 = 0, t2 = 0;
         double tw = 0.0, tv2 = 0.0, tw2 = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
+        for (int w = 0; w < kBinThreads / 32; ++w) {
             t0 += s_cnt[0][w]; t1 += s_cnt[1][w]; t2 += s_cnt[2][w];
             tw += s_w[0][w]; tv2 += s_w[1][w]; tw2 += s_w[2][w];
         }
@@ -374,77 +400,98 @@ __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, i
     *dst = o;
 }
 
+template <int VPT>
 __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, const uint4* __restrict__ loc,
                                                                const float2* __restrict__ vis,
                                                                const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                                const long long nvis, const uint32_t* __restrict__ bin_offset,
                                                                uint32_t* __restrict__ cursor, uint4* __restrict__ sorted) {
     extern __shared__ uint32_t s_hist[];
-    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long base = (long long)blockIdx.x * (kBinThreads * VPT);
     const int lane = threadIdx.x & 31;
-    OwLoc L;
-    L.state = 0;
-    if (k < nvis) {                                                   // k_owner_count's integer decisions
-        const uint4 o = __ldg(loc + k);
-        L.state = (int)(o.z >> 30);
-        if (L.state == 3) {
-            L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
-            L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
-            L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
-            L.ry[1] = (int)(o.w & 511u);
-            const float2 V = vis[k];
-            const float wt = weight[k];
-            L.re = wt * V.x; L.im = wt * V.y; L.wt = wt; L.gid = grid_id ? grid_id[k] : 0;
+    const bool fits = g.ontiles <= kBinSmemTiles;
+    if (fits)
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
+    const int ref = grid_id ? grid_id[base] : 0;
+    OwLoc L[VPT];
+    int same = 1;
+#pragma unroll
+    for (int j = 0; j < VPT; ++j) {
+        const long long k = base + j * kBinThreads + threadIdx.x;
+        L[j].state = 0;
+        if (k < nvis) {                                               // k_owner_count's integer decisions
+            const uint4 o = __ldg(loc + k);
+            L[j].state = (int)(o.z >> 30);
+            if (L[j].state == 3) {
+                L[j].cu[0] = (int)(o.x & 0xFFFFu); L[j].cv[0] = (int)(o.x >> 16);
+                L[j].cu[1] = (int)(o.y & 0xFFFFu); L[j].cv[1] = (int)(o.y >> 16);
+                L[j].rx[0] = (int)(o.z & 511u); L[j].ry[0] = (int)((o.z >> 9) & 511u); L[j].rx[1] = (int)((o.z >> 18) & 511u);
+                L[j].ry[1] = (int)(o.w & 511u);
+                const float2 V = vis[k];
+                const float wt = weight[k];
+                L[j].re = wt * V.x; L[j].im = wt * V.y; L[j].wt = wt; L[j].gid = grid_id ? grid_id[k] : 0;
+                same &= (L[j].gid == ref);
+            }
         }
     }
-    const int kept = L.state == 3;
-    const int ugrid = ow_cta_uniform_grid(g, L, grid_id, s_hist, 1);
+    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
     if (ugrid >= 0) {
+        // phase A: count this CTA's records per tile; reserve a run in each touched tile; phase B: the same shared
+        // counters, zeroed again, hand out the positions inside the runs (no per-record rank is kept in registers)
         const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
         uint32_t* s_base = s_hist + g.ontiles;                         // global position of this CTA's run in each tile
-        OwTiles T[2];
-        uint32_t rk[2][4];
-        if (kept) {
+#pragma unroll
+        for (int j = 0; j < VPT; ++j) {
+            if (L[j].state != 3) continue;
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
-                T[s] = ow_tiles(g, L.cu[s], L.cv[s]);
-                if (!T[s].up) continue;
-                rk[s][0] = atomicAdd(&s_hist[T[s].t00], 1u);
-                if (T[s].mx) rk[s][1] = atomicAdd(&s_hist[T[s].t00 + 1], 1u);
-                if (T[s].my) rk[s][2] = atomicAdd(&s_hist[T[s].t00 + g.otx], 1u);
-                if (T[s].mx && T[s].my) rk[s][3] = atomicAdd(&s_hist[T[s].t00 + g.otx + 1], 1u);
+                const OwTiles t = ow_tiles(g, L[j].cu[s], L[j].cv[s]);
+                if (!t.up) continue;
+                atomicAdd(&s_hist[t.t00], 1u);
+                if (t.mx) atomicAdd(&s_hist[t.t00 + 1], 1u);
+                if (t.my) atomicAdd(&s_hist[t.t00 + g.otx], 1u);
+                if (t.mx && t.my) atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u);
             }
         }
         __syncthreads();
-        for (int i = threadIdx.x; i < g.ontiles; i += blockDim.x) {     // reserve this CTA's run in each touched tile
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
             const uint32_t n = s_hist[i];
-            if (n) s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n);
+            if (n) { s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n); s_hist[i] = 0; }
         }
         __syncthreads();
-        if (kept) {
+#pragma unroll
+        for (int j = 0; j < VPT; ++j) {
+            if (L[j].state != 3) continue;
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
-                const OwTiles t = T[s];
+                const OwTiles t = ow_tiles(g, L[j].cu[s], L[j].cv[s]);
                 if (!t.up) continue;
-                ow_write_record(g, L, s, t.tx0, t.ty0, sorted + s_base[t.t00] + rk[s][0]);
-                if (t.mx) ow_write_record(g, L, s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + rk[s][1]);
-                if (t.my) ow_write_record(g, L, s, t.tx0, t.ty0 + 1, sorted + s_base[t.t00 + g.otx] + rk[s][2]);
+                ow_write_record(g, L[j], s, t.tx0, t.ty0, sorted + s_base[t.t00] + atomicAdd(&s_hist[t.t00], 1u));
+                if (t.mx) ow_write_record(g, L[j], s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + atomicAdd(&s_hist[t.t00 + 1], 1u));
+                if (t.my)
+                    ow_write_record(g, L[j], s, t.tx0, t.ty0 + 1,
+                                    sorted + s_base[t.t00 + g.otx] + atomicAdd(&s_hist[t.t00 + g.otx], 1u));
                 if (t.mx && t.my)
-                    ow_write_record(g, L, s, t.tx0 + 1, t.ty0 + 1, sorted + s_base[t.t00 + g.otx + 1] + rk[s][3]);
+                    ow_write_record(g, L[j], s, t.tx0 + 1, t.ty0 + 1,
+                                    sorted + s_base[t.t00 + g.otx + 1] + atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u));
             }
         }
         return;
     }
-    if (!__any_sync(kFull, kept)) return;
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
+    for (int j = 0; j < VPT; ++j) {
+        const int kept = L[j].state == 3;
+        if (!__any_sync(kFull, kept)) continue;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            int tx = 0, ty = 0;
-            const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
-            if (!__any_sync(kFull, bin != kNoBin)) continue;
-            const uint32_t rank = ow_agg_inc(cursor, bin, lane);
-            if (bin != kNoBin) ow_write_record(g, L, s, tx, ty, sorted + bin_offset[bin] + rank);
+        for (int s = 0; s < 2; ++s) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                int tx = 0, ty = 0;
+                const uint32_t bin = kept ? ow_bin(g, L[j].gid, L[j].cu[s], L[j].cv[s], q, tx, ty) : kNoBin;
+                if (!__any_sync(kFull, bin != kNoBin)) continue;
+                const uint32_t rank = ow_agg_inc(cursor, bin, lane);
+                if (bin != kNoBin) ow_write_record(g, L[j], s, tx, ty, sorted + bin_offset[bin] + rank);
+            }
         }
     }
 }
@@ -881,11 +928,26 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
 // ------------------------------------------------------------------------------------------------- launchers
 static size_t bin_smem_bytes(const Geom& g) { return g.ontiles <= kBinSmemTiles ? (size_t)2 * g.ontiles * sizeof(uint32_t) : 0; }
 
+// visibilities per thread of the binning kernels (MUSER_TUNE_BIN_VPT)
+static int bin_vpt(long long nvis, int forced) {
+    (void)nvis;
+    // measured on B200 (cfg 3, 4.5 M visibilities per call): 1 -> 2.26, 2 -> 2.50, 4 -> 2.58 us per frame for the whole
+    // binning stage: the kernels are issue-bound and the extra registers of several visibilities per thread cost
+    // more occupancy than the shared per-CTA work saves
+    return (forced == 2 || forced == 4) ? forced : 1;
+}
+
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                                const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, uint4* loc,
-                               cudaStream_t s) {
-    k_owner_count<<<(unsigned)((nvis + kBinThreads - 1) / kBinThreads), kBinThreads, bin_smem_bytes(g), s>>>(
-        g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
+                               int vpt_forced, cudaStream_t s) {
+    const int vpt = bin_vpt(nvis, vpt_forced);
+    const unsigned blocks = (unsigned)((nvis + kBinThreads * vpt - 1) / (kBinThreads * vpt));
+    if (vpt == 4)
+        k_owner_count<4><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
+    else if (vpt == 2)
+        k_owner_count<2><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
+    else
+        k_owner_count<1><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
     return cudaGetLastError();
 }
 
@@ -905,9 +967,15 @@ cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* curs
 
 cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float2* vis, const float* wt, const int* grid_id,
                                  long long nvis, const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted,
-                                 cudaStream_t s) {
-    k_owner_scatter<<<(unsigned)((nvis + kBinThreads - 1) / kBinThreads), kBinThreads, bin_smem_bytes(g), s>>>(
-        g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
+                                 int vpt_forced, cudaStream_t s) {
+    const int vpt = bin_vpt(nvis, vpt_forced);
+    const unsigned blocks = (unsigned)((nvis + kBinThreads * vpt - 1) / (kBinThreads * vpt));
+    if (vpt == 4)
+        k_owner_scatter<4><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
+    else if (vpt == 2)
+        k_owner_scatter<2><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
+    else
+        k_owner_scatter<1><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
     return cudaGetLastError();
 }
 
