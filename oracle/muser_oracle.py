@@ -24,8 +24,10 @@ Two layers:
   (II) the algorithm step by step: O1 coordinates -> O2 table -> O3 gridding -> O4 transform -> O5 correction
        (+ O6 w-projection planes)                            -> `coordinates`, `table_*`, `grid`, `transform`,
                                                                 `corrector`, `dirty_image`
-Pins (tests/test_oracle_*.py, all `-m "not gpu"`): P1..P12 of DESIGN.md.  No function here is unpinned;
-what stays unpinned *by the paper* is the identity of its own GCF coefficients and w-kernels (R2, R15).
+Pins (tests/test_oracle_*.py, all `-m "not gpu"`): P1..P12 of DESIGN.md for the path, N1..N4 (tests/test_oracle_next.py)
+for the NEXT rows at the end of this file (channelised input, Hermitian half-plane, uniform weighting as the paper
+prints it, phase correction, peak / histogram).  No function here is unpinned; what stays unpinned *by the paper* is
+the identity of its own GCF coefficients and w-kernels (R2, R15).
 """
 from __future__ import annotations
 
@@ -257,6 +259,8 @@ class Imager:
         self.wc = None
         self.tables = None
         self.supports = None
+        self.weighting = 0                       # 0 natural, 1 uniform (wgt_grid)
+        self.offset = (0.0, 0.0)                 # phase-centre offset (dl, dm), NEXT-3
         self.reset()
 
     def set_wplanes(self, nplanes, w_max, tables=None, supports=None, wc=None):
@@ -274,10 +278,13 @@ class Imager:
         wmode = self.wc is not None
         self.G = np.zeros((self.ngrids, self.ny, self.nx), np.complex128)
         self.Gw = np.zeros((self.ngrids, self.ny, self.nx), np.complex128 if wmode else np.float64)
+        self.cnt = np.zeros((self.ngrids, self.ny, self.nx), np.int64)
         self.stats = dict(sum_weights=0.0, n_gridded=0, n_dropped=0, n_flagged=0)
 
     def grid(self, uvw_m, freq_hz, vis, weight, grid_id=None, gridder=None):
         wmode = self.wc is not None
+        if self.offset != (0.0, 0.0):
+            vis = phase_correct(uvw_m, freq_hz, vis, *self.offset)
         smp = coordinates(uvw_m, freq_hz, vis, weight, self.nx, self.ny, self.cell, self.Q,
                           self.supports if wmode else self.S, self.wc, grid_id)
         gfun = grid if gridder is None else gridder
@@ -285,6 +292,7 @@ class Imager:
                      self.nx, self.ny, self.ngrids, wmode)
         self.G += G
         self.Gw += Gw
+        self.cnt += hit_counts(smp, self.nx, self.ny, self.ngrids)
         for k, val in smp["stats"].items():
             self.stats[k] += val
         return smp
@@ -294,12 +302,137 @@ class Imager:
         S0 = int(self.supports[0]) if self.wc is not None else self.S
         return corrector(T0, S0, self.Q, self.nx), corrector(T0, S0, self.Q, self.ny)
 
+    def weighted(self):
+        """The grids after wgtGrid_kernel (identity in natural mode)."""
+        return wgt_grid(self.G, self.cnt, self.weighting), wgt_grid(self.Gw, self.cnt, self.weighting)
+
     def dirty(self):
         cx, cy = self.correctors()
-        out = [dirty_image(self.G[g], cx, cy) for g in range(self.ngrids)]
+        Gv, _ = self.weighted()
+        out = [dirty_image(Gv[g], cx, cy) for g in range(self.ngrids)]
         return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
 
     def psf(self):
         cx, cy = self.correctors()
-        out = [dirty_image(self.Gw[g].astype(np.complex128), cx, cy) for g in range(self.ngrids)]
+        _, Gwv = self.weighted()
+        out = [dirty_image(Gwv[g].astype(np.complex128), cx, cy) for g in range(self.ngrids)]
         return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
+
+
+# =========================================================================== NEXT rows of SURVEY.md 8(f)
+# --------------------------------------------------------------------------- NEXT-1: channelised input
+def grid_rows_inputs(uvw_m, freq_hz, vis, weight):
+    """NEXT-1 (a 3 ms frame is 16 channels x 2 polarisations of the SAME baselines).  Channelised layout:
+    uvw_m [ntime][nrow][3] f32, freq_hz [nchan] f64, vis / weight [ntime][npol][nchan][nrow].  The method is unchanged:
+    visibility (t, p, c, r) has coordinates uvw_m[t][r] * freq_hz[c] / c0, so this writes the loop out, in the order
+    t, p, c, r, as the flat per-visibility arrays of O1 -- the result is DEFINED as the flat path's on these arrays."""
+    uvw_m = np.asarray(uvw_m, np.float32)
+    vis = np.asarray(vis)
+    ntime, npol, nchan, nrow = vis.shape
+    assert uvw_m.shape == (ntime, nrow, 3) and np.asarray(freq_hz).shape == (nchan,)
+    uvw = np.empty((ntime, npol, nchan, nrow, 3), np.float32)
+    f = np.empty((ntime, npol, nchan, nrow), np.float64)
+    for t in range(ntime):
+        for p in range(npol):
+            for c in range(nchan):
+                uvw[t, p, c] = uvw_m[t]
+                f[t, p, c] = freq_hz[c]
+    return (uvw.reshape(-1, 3), f.reshape(-1), np.ascontiguousarray(vis).reshape(-1),
+            np.ascontiguousarray(np.asarray(weight, np.float32)).reshape(-1))
+
+
+def rows_grid_ids(grid_id, ntime, npol, nchan, nrow, pols_split):
+    """Per-visibility grid ids of the channelised call: grid_id is [ntime][nchan] (polarisations summed onto one grid)
+    or [ntime][npol][nchan] (one grid per polarisation); None = everything onto grid 0."""
+    if grid_id is None:
+        return None
+    g = np.asarray(grid_id, np.int64)
+    g = g.reshape(ntime, npol, nchan) if pols_split else np.broadcast_to(g.reshape(ntime, 1, nchan), (ntime, npol, nchan))
+    return np.ascontiguousarray(np.broadcast_to(g[..., None], (ntime, npol, nchan, nrow))).reshape(-1)
+
+
+# --------------------------------------------------------------------------- NEXT-1b: Hermitian half-plane
+def grid_halfplane(samples, tables, supports, Q, nx, ny, ngrids=1, wmode=False):
+    """"half the grid (as the data is Hermitian)": O3/O6 restricted to grid rows iv >= ny/2.  Every sample
+    (each visibility AND its conjugate, each with its own O1 coordinates) contributes the cells of its footprint that
+    lie in those rows; rows below ny/2 stay zero.  `full_from_halfplane` rebuilds the rest."""
+    G, Gw = grid(samples, tables, supports, Q, nx, ny, ngrids, wmode)
+    G[:, :ny // 2, :] = 0
+    Gw[:, :ny // 2, :] = 0
+    return G, Gw
+
+
+def full_from_halfplane(H):
+    """Hermitian completion about the centre cell [ny/2][nx/2]: H[ny-y][nx-x] = conj H[y][x] for y in (ny/2, ny-1],
+    x in [1, nx-1]; row 0 and column 0 have no mirror and are empty (drop rule R5)."""
+    H = np.array(H)
+    ny, nx = H.shape[-2:]
+    y = np.arange(1, ny // 2)
+    x = np.arange(1, nx)
+    H[..., y[:, None], x[None, :]] = np.conj(H[..., (ny - y)[:, None], (nx - x)[None, :]])
+    H[..., 0, :] = 0
+    H[..., :ny // 2, 0] = 0
+    return H
+
+
+def image_from_halfplane(H):
+    """Real image of a Hermitian grid given by its rows >= ny/2 only: O4 applied to the completed grid.  (A complex-
+    to-real transform; written through the completion so that it can be checked by eye.)"""
+    return transform(full_from_halfplane(H)).real
+
+
+# --------------------------------------------------------------------------- NEXT-2: uniform weighting as printed
+def hit_counts(samples, nx, ny, ngrids=1):
+    """Integer hit-count grid `cnt` of Alg. 1 l.1: cnt[g][iv0][iu0] += 1 for every gridded sample (each
+    visibility and its conjugate) at its NEAREST cell (reading R22: the paper does not print where cnt is filled)."""
+    cnt = np.zeros((ngrids, ny, nx), np.int64)
+    for s in range(samples["val"].shape[0]):
+        cnt[int(samples["grid"][s]), int(samples["iv0"][s]), int(samples["iu0"][s])] += 1
+    return cnt
+
+
+def wgt_grid(Grd, cnt, mode):
+    """wgtGrid_kernel of Alg. 1 l.1-16 over the whole grid: where cnt != 0 the cell is multiplied
+    by wgt = 1/cnt (mode 1, uniform) or 1 (natural); cells with cnt == 0 are left alone.  The paper runs it on half
+    the grid because the data are Hermitian; cnt is Hermitian too, so running it on every cell is the same thing.
+    Applied to the visibility grid and, for a consistent beam, to the weight grid (R22)."""
+    out = np.array(Grd)
+    if mode == 1:
+        nz = cnt != 0
+        out[nz] = out[nz] * (1.0 / cnt[nz])
+    return out
+
+
+# --------------------------------------------------------------------------- NEXT-3: phase correction of visibilities
+def phase_correct(uvw_m, freq_hz, vis, dl, dm):
+    """Phase correction by a (RA, DEC) offset (PAPER.md:174 step 3, :286 Alg. 1 IMPROVED_CLEAN): the visibility of
+    baseline (u, v) in wavelengths is multiplied by exp(+2 pi i (u dl + v dm)), which moves a source at direction
+    cosines (dl, dm) to the phase centre (sign convention R7: the image is sum V exp(+2 pi i (u l + v m)))."""
+    il = np.asarray(freq_hz, np.float64) / C_M_S
+    ul = np.asarray(uvw_m)[:, 0].astype(np.float64) * il
+    vl = np.asarray(uvw_m)[:, 1].astype(np.float64) * il
+    return np.asarray(vis).astype(np.complex128) * np.exp(2j * np.pi * (ul * dl + vl * dm))
+
+
+# --------------------------------------------------------------------------- NEXT-4: consumers of the dirty image
+def image_peak(img):
+    """Strength and position of the peak of the dirty map (Alg. 1 l.33/36): maximum value and its
+    (y, x); on equal values the lowest flat index.  Also the minimum (the histogram's lower edge)."""
+    img = np.asarray(img)
+    k = int(np.argmax(img))
+    return float(img.reshape(-1)[k]), k // img.shape[1], k % img.shape[1], float(img.min())
+
+
+def image_histogram(img, nbins, lo, hi):
+    """"the data from a dirty image is divided into 2000 ranges": nbins equal ranges of [lo, hi]
+    (reading R23: lo, hi = the image's minimum and maximum unless the caller fixes them), bin = floor((v - lo) * (nbins /
+    (hi - lo))), the value hi itself in the last bin, values outside [lo, hi] not counted.  The decision is taken in
+    fp32, the precision of the image (both sides take it in the same precision)."""
+    v = np.asarray(img, np.float32).reshape(-1)
+    lo32, hi32 = np.float32(lo), np.float32(hi)
+    scale = np.float32(nbins) / (hi32 - lo32)
+    t = (v - lo32) * scale
+    b = np.floor(t).astype(np.int64)
+    ok = (v >= lo32) & (v <= hi32)
+    b = np.minimum(b, nbins - 1)
+    return np.bincount(b[ok], minlength=nbins).astype(np.int64)

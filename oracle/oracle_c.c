@@ -29,11 +29,13 @@ static void cell_phase(double c_lambda, double scale, int n, int Q, double* i0, 
 /* tables[p]: S_p*Q+1 doubles (2-D mode, wmode=0) or S_p*Q+1 (re,im) pairs (wmode=1).
  * G: [ngrids][ny][nx] (re,im) doubles.  Gw: [ngrids][ny][nx] doubles (wmode=0) or (re,im) pairs (wmode=1).
  * stats[4]: sum_weights, n_gridded (kept visibilities), n_dropped (off grid), n_flagged (weight<=0 / non-finite).
- * Accumulates into G, Gw, stats (callers zero them). */
+ * cnt (may be NULL): [ngrids][ny][nx] hit counts, +1 per gridded sample at its nearest cell (Alg. 1 l.1 `cnt`).
+ * (dl, dm): phase-centre offset; V is multiplied by exp(+2 pi i (u dl + v dm)) first (PAPER.md:174 step 3; 0, 0 = none).
+ * Accumulates into G, Gw, cnt, stats (callers zero them). */
 int oracle_grid(const float* uvw_m, const double* freq_hz, const float* vis_ri, const float* weight,
                 const int* grid_id, long long nvis, int nx, int ny, double cell_arcsec, int Q,
                 int nplanes, const double* wc, const int* supports, const double* const* tables, int wmode,
-                double* G, double* Gw, double* stats) {
+                double dl, double dm, double* G, double* Gw, long long* cnt, double* stats) {
     const double cell = cell_arcsec * ARCSEC;
     const double su = (double)nx * cell, sv = (double)ny * cell;
     for (long long k = 0; k < nvis; ++k) {
@@ -42,11 +44,17 @@ int oracle_grid(const float* uvw_m, const double* freq_hz, const float* vis_ri, 
         const double vl = (double)uvw_m[3 * k + 1] * il;
         const double wl = (double)uvw_m[3 * k + 2] * il;
         const double wt = (double)weight[k];
-        const double vr = (double)vis_ri[2 * k], vi = (double)vis_ri[2 * k + 1];
+        double vr = (double)vis_ri[2 * k], vi = (double)vis_ri[2 * k + 1];
         if (!(isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(vr) && isfinite(vi) &&
               isfinite(freq_hz[k]) && wt > 0.0)) {
             stats[3] += 1.0;
             continue;
+        }
+        if (dl != 0.0 || dm != 0.0) {          /* NEXT-3: V * exp(+2 pi i (u dl + v dm)) */
+            const double ph = 2.0 * 3.14159265358979323846 * (ul * dl + vl * dm);
+            const double c = cos(ph), s = sin(ph), r0 = vr, i0 = vi;
+            vr = r0 * c - i0 * s;
+            vi = r0 * s + i0 * c;
         }
         int p = 0;
         if (wmode) {                          /* O6: nearest plane centre in |w|, tie -> lower p */
@@ -75,6 +83,7 @@ int oracle_grid(const float* uvw_m, const double* freq_hz, const float* vis_ri, 
             const double valr = wt * vr, vali = wt * (s ? -vi : vi);     /* conjugate sample carries conj V */
             const int kconj = wmode && (sgn * wl < 0.0);                 /* conjugate kernel iff sample's w < 0 */
             const int cu = (int)iu0[s], cv = (int)iv0[s], pu = (int)ru[s], pv = (int)rv[s];
+            if (cnt) cnt[(g * (size_t)ny + (size_t)cv) * (size_t)nx + (size_t)cu] += 1;
             for (int jy = -h; jy <= h; ++jy) {
                 const int ty = jy * Q - pv + S * Q / 2;
                 for (int jx = -h; jx <= h; ++jx) {

@@ -34,9 +34,11 @@ def _p(a):
     return a.ctypes.data_as(ctypes.c_void_p)
 
 
-def grid(uvw_m, freq_hz, vis, weight, nx, ny, cell_arcsec, Q, supports, tables, wc=None, grid_id=None, ngrids=1):
+def grid(uvw_m, freq_hz, vis, weight, nx, ny, cell_arcsec, Q, supports, tables, wc=None, grid_id=None, ngrids=1,
+         offset=(0.0, 0.0), counts=False):
     """O1+O3 (2-D: supports=int S, tables=real table) or O1+O6 (w-mode: wc, supports[p], complex tables[p]).
-    Returns G complex128 [ngrids,ny,nx], Gw (float64, or complex128 in w-mode), stats dict."""
+    offset = (dl, dm): phase correction of the visibilities first (NEXT-3); counts=True: also the hit-count grid (NEXT-2).
+    Returns G complex128 [ngrids,ny,nx], Gw (float64, or complex128 in w-mode), stats dict (with "cnt" if asked)."""
     lib = _load()
     wmode = wc is not None
     uvw = np.ascontiguousarray(uvw_m, np.float32)
@@ -58,14 +60,18 @@ def grid(uvw_m, freq_hz, vis, weight, nx, ny, cell_arcsec, Q, supports, tables, 
     G = np.zeros((ngrids, ny, nx), np.complex128)
     Gw = np.zeros((ngrids, ny, nx), np.complex128 if wmode else np.float64)
     stats = np.zeros(4, np.float64)
+    cnt = np.zeros((ngrids, ny, nx), np.int64) if counts else None
     gid = None if grid_id is None else np.ascontiguousarray(grid_id, np.int32)
     rc = lib.oracle_grid(_p(uvw), _p(f), _p(v), _p(w), None if gid is None else _p(gid),
                          ctypes.c_longlong(nvis), ctypes.c_int(nx), ctypes.c_int(ny),
                          ctypes.c_double(cell_arcsec), ctypes.c_int(Q), ctypes.c_int(len(tabs)),
-                         _p(wc_a), _p(sup), tptr, ctypes.c_int(1 if wmode else 0), _p(G), _p(Gw), _p(stats))
+                         _p(wc_a), _p(sup), tptr, ctypes.c_int(1 if wmode else 0), ctypes.c_double(offset[0]),
+                         ctypes.c_double(offset[1]), _p(G), _p(Gw), None if cnt is None else _p(cnt), _p(stats))
     assert rc == 0
-    return G, Gw, dict(sum_weights=float(stats[0]), n_gridded=int(stats[1]), n_dropped=int(stats[2]),
-                       n_flagged=int(stats[3]))
+    out = dict(sum_weights=float(stats[0]), n_gridded=int(stats[1]), n_dropped=int(stats[2]), n_flagged=int(stats[3]))
+    if counts:
+        out["cnt"] = cnt
+    return G, Gw, out
 
 
 def dft(u, v, w, val, l, m, use_w=False):
