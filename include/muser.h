@@ -88,6 +88,24 @@ enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_BIN_VPT = 1, MUSER_TUNE_COUNT = 2 };
 int muser_set_tuning(muser_imager* h, int key, int value);
 /* 1 (default): A6 divides by the kernel's transform; 0: A6 only shifts/takes the real part (parity gate R9(i)). */
 int muser_set_grid_correction(muser_imager* h, int enabled);
+/* Weighting mode of Alg. 1 ("weighting mode: weight_mode, natural or uniform").  NATURAL (default): the
+ * per-visibility weight only.  UNIFORM: the gridder also keeps the integer hit-count grid `cnt` (one hit per gridded
+ * sample -- visibility or conjugate -- at its nearest cell) and the paper's wgtGrid_kernel is applied where the grids
+ * enter the FFT: a cell of the visibility grid AND of the beam grid is multiplied by 1/cnt where cnt != 0, and left
+ * alone where cnt == 0 (reading R22).  The accumulated grids are not modified; muser_get_weighted_grid shows the
+ * weighted ones.  Changing the mode reallocates and zeroes the grids.  May synchronise. */
+enum { MUSER_WEIGHT_NATURAL = 0, MUSER_WEIGHT_UNIFORM = 1 };
+int muser_set_weighting(muser_imager* h, int mode);
+/* Phase correction of the visibilities (PAPER.md:174 step 3, :286 Alg. 1 IMPROVED_CLEAN; Table 3 row 4), fused into A1:
+ * from the next muser_grid on, every visibility is multiplied by exp(+2 pi i (u dl + v dm)) (u, v in wavelengths) before
+ * it is gridded, which moves the point at direction cosines (dl, dm) -- the measured offset of the solar disk -- to the
+ * phase centre (reading R24).  (0, 0) switches it off.  The beam does not depend on it. */
+int muser_set_phase_offset(muser_imager* h, double dl, double dm);
+/* NEXT-2b: CLEAN wants a beam twice the size of the image.  When enabled, every muser_grid /
+ * muser_grid_batched call also grids the weights onto a second set of grids of 2nx x 2ny cells (same cell size, same
+ * kernel), and muser_psf2x returns that beam: DEVICE float [ngrids][2ny][2nx].  2-D mode only.  May synchronise. */
+int muser_set_psf2x(muser_imager* h, int enabled);
+int muser_psf2x(muser_imager* h, float* beam2x_out, muser_stream s);
 
 /* ---- A1..A4 gridding --------------------------------------------------------------------------------------
  * Zero the grids, the sum of weights and the counters (asynchronous on s). */
@@ -114,6 +132,19 @@ int muser_dirty(muser_imager* h, float* image_out, muser_stream s);
 int muser_psf(muser_imager* h, float* beam_out, muser_stream s);
 int muser_dirty_psf(muser_imager* h, float* image_out, float* beam_out, muser_stream s);
 
+/* ---- consumers of the dirty image (NEXT-4) -----------------------------------------------------------------------
+ * "Find the strength and position of the peak in the dirty map" (Alg. 1 l.33/36): when enabled, every
+ * muser_dirty / muser_dirty_psf also keeps, per grid, the maximum of the dirty image with its position (lowest index
+ * among equal values) and the minimum, found in the epilogue that writes the image (no extra pass).  muser_get_peak
+ * synchronises the last stream; HOST outputs of ngrids entries, any may be NULL. */
+int muser_set_peak_search(muser_imager* h, int enabled);
+int muser_get_peak(muser_imager* h, float* peak_value, int* peak_x, int* peak_y, float* min_value);
+/* "the data from a dirty image is divided into 2000 ranges" (the input of the GMM): histogram of `image`
+ * (DEVICE float [ngrids][ny][nx]) into nbins equal ranges of [lo, hi]: bin = floor((v - lo) * (nbins / (hi - lo))) in
+ * fp32, hi itself in the last bin, values outside not counted.  lo >= hi: each grid's own minimum and maximum from the
+ * peak search of the last muser_dirty (reading R23).  hist_out: DEVICE unsigned [ngrids][nbins], overwritten. */
+int muser_histogram(muser_imager* h, const float* image, int nbins, float lo, float hi, unsigned int* hist_out, muser_stream s);
+
 /* ---- whole path with HOST buffers (end-to-end entry point) ------------------------------------------------
  * reset -> copy the inputs to the device -> grid -> dirty + psf -> copy the images back, all on s, then
  * synchronises s.  HOST pointers (pinned memory makes the copies asynchronous); grid_id may be NULL;
@@ -126,6 +157,10 @@ int muser_frame_host(muser_imager* h, const float* uvw_m, const double* freq_hz,
  * Copy the centred grids (DC at [ny/2][nx/2]) to DEVICE buffers: grid_c64_out float [ngrids][ny][nx][2];
  * wgrid_out float [ngrids][ny][nx] (2-D mode) or [ngrids][ny][nx][2] (w mode).  Either may be NULL. */
 int muser_get_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_stream s);
+/* Uniform mode only: the hit counts, DEVICE int [ngrids][ny][nx]; and the grids as wgtGrid_kernel leaves them (same
+ * layouts as muser_get_grid; in natural mode the same as muser_get_grid). */
+int muser_get_counts(muser_imager* h, int* counts_out, muser_stream s);
+int muser_get_weighted_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_stream s);
 /* Kernel table of `plane` as used on the device, in the oracle's order T[t], t = 0..S*Q (2-D mode: floats;
  * w mode: (re,im) pairs).  HOST output; *len in: capacity in floats, out: floats written. */
 int muser_get_table(muser_imager* h, int plane, float* table_out_host, int* len);

@@ -16,6 +16,7 @@ MUSER_OK, MUSER_EINVAL, MUSER_ECUDA, MUSER_ENOMEM, MUSER_ESTATE, MUSER_EUNSUPPOR
 MUSER_KERNEL_PSWF, MUSER_KERNEL_GAUSS = 0, 1
 MUSER_STRATEGY_AUTO, MUSER_STRATEGY_TILED, MUSER_STRATEGY_OWNER = 0, 2, 3
 MUSER_TUNE_ITEM_SIZE, MUSER_TUNE_BIN_VPT = 0, 1
+MUSER_WEIGHT_NATURAL, MUSER_WEIGHT_UNIFORM = 0, 1
 STAGES = ("bin", "grid", "pack", "fft", "correct")
 
 _c = ctypes
@@ -31,6 +32,15 @@ SIGNATURES = {
     "muser_set_strategy": (_i, [_vp, _i]),
     "muser_set_tuning": (_i, [_vp, _i, _i]),
     "muser_set_grid_correction": (_i, [_vp, _i]),
+    "muser_set_weighting": (_i, [_vp, _i]),
+    "muser_set_phase_offset": (_i, [_vp, _d, _d]),
+    "muser_set_psf2x": (_i, [_vp, _i]),
+    "muser_psf2x": (_i, [_vp, _vp, _vp]),
+    "muser_get_counts": (_i, [_vp, _vp, _vp]),
+    "muser_get_weighted_grid": (_i, [_vp, _vp, _vp, _vp]),
+    "muser_set_peak_search": (_i, [_vp, _i]),
+    "muser_get_peak": (_i, [_vp, _vp, _vp, _vp, _vp]),
+    "muser_histogram": (_i, [_vp, _vp, _i, _c.c_float, _c.c_float, _vp, _vp]),
     "muser_reset": (_i, [_vp, _vp]),
     "muser_grid": (_i, [_vp, _vp, _vp, _vp, _vp, _ll, _vp]),
     "muser_grid_batched": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _ll, _vp]),
@@ -153,6 +163,32 @@ class Imager:
     def set_grid_correction(self, enabled):
         self._ck(lib().muser_set_grid_correction(self._h, 1 if enabled else 0))
 
+    def set_weighting(self, mode):
+        self._ck(lib().muser_set_weighting(self._h, mode))
+
+    def set_phase_offset(self, dl, dm):
+        self._ck(lib().muser_set_phase_offset(self._h, float(dl), float(dm)))
+
+    def set_psf2x(self, enabled):
+        self._ck(lib().muser_set_psf2x(self._h, 1 if enabled else 0))
+
+    def psf2x(self, beam2x_out, stream=None):
+        self._ck(lib().muser_psf2x(self._h, _ptr(beam2x_out), _stream(stream)))
+
+    def set_peak_search(self, enabled):
+        self._ck(lib().muser_set_peak_search(self._h, 1 if enabled else 0))
+
+    def get_peak(self):
+        """Per grid: (peak value, x, y, minimum) of the last dirty image."""
+        n = self.ngrids
+        v, m = (ctypes.c_float * n)(), (ctypes.c_float * n)()
+        x, y = (ctypes.c_int * n)(), (ctypes.c_int * n)()
+        self._ck(lib().muser_get_peak(self._h, v, x, y, m))
+        return [(v[i], x[i], y[i], m[i]) for i in range(n)]
+
+    def histogram(self, image, nbins, lo, hi, hist_out, stream=None):
+        self._ck(lib().muser_histogram(self._h, _ptr(image), nbins, lo, hi, _ptr(hist_out), _stream(stream)))
+
     # ---- path
     def reset(self, stream=None):
         self._ck(lib().muser_reset(self._h, _stream(stream)))
@@ -182,6 +218,12 @@ class Imager:
     # ---- inspection
     def get_grid(self, grid_out, wgrid_out, stream=None):
         self._ck(lib().muser_get_grid(self._h, _ptr(grid_out), _ptr(wgrid_out), _stream(stream)))
+
+    def get_counts(self, counts_out, stream=None):
+        self._ck(lib().muser_get_counts(self._h, _ptr(counts_out), _stream(stream)))
+
+    def get_weighted_grid(self, grid_out, wgrid_out, stream=None):
+        self._ck(lib().muser_get_weighted_grid(self._h, _ptr(grid_out), _ptr(wgrid_out), _stream(stream)))
 
     def get_table(self, plane=0):
         import numpy as np

@@ -41,6 +41,12 @@ struct muser_imager {
     float2* G = nullptr;
     float* Gw = nullptr;
     float2* H = nullptr;
+    int* cnt = nullptr;                     // hit counts (uniform weighting only)
+    int weighting = MUSER_WEIGHT_NATURAL;
+    double off_l = 0.0, off_m = 0.0;        // phase-centre offset (NEXT-3)
+    bool peak_search = false;               // NEXT-4: peak / minimum of the dirty image kept per grid
+    PeakSlot* peaks_d = nullptr;
+    muser_imager* child2x = nullptr;        // NEXT-2b: imager of 2nx x 2ny pixels gridding the weights only
     Staged* staged = nullptr;
     Sample* sorted = nullptr;
     size_t sample_cap = 0;
@@ -57,6 +63,7 @@ struct muser_imager {
     uint4 *ow_sorted = nullptr, *ow_loc = nullptr;          // tile-sorted records; per-visibility integer result of O1
     uint32_t *ow_count = nullptr, *ow_cursor = nullptr, *ow_offset = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
     uint4* ow_work = nullptr;
+    bool weights_only = false;              // the 2x-beam child: muser_grid is called without visibilities
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     bool lower_valid = true;                // rows 0 .. ny/2-1 of G, Gw are up to date (the owner gridder stores rows >= ny/2 only)
     cufftHandle plan = 0, plan_rows = 0;
@@ -113,8 +120,9 @@ size_t grid_cells(const muser_imager* h) { return (size_t)h->ngrids * h->ny * h-
 bool wmode(const muser_imager* h) { return h->nplanes > 0; }
 
 void free_grids(muser_imager* h) {
-    cudaFree(h->G); cudaFree(h->Gw); cudaFree(h->H); cudaFree(h->out_dirty); cudaFree(h->out_psf);
-    h->G = nullptr; h->Gw = nullptr; h->H = nullptr; h->out_dirty = h->out_psf = nullptr;
+    cudaFree(h->G); cudaFree(h->Gw); cudaFree(h->H); cudaFree(h->out_dirty); cudaFree(h->out_psf); cudaFree(h->cnt);
+    cudaFree(h->peaks_d);
+    h->G = nullptr; h->Gw = nullptr; h->H = nullptr; h->out_dirty = h->out_psf = nullptr; h->cnt = nullptr; h->peaks_d = nullptr;
     if (h->plan_ok) { cufftDestroy(h->plan); h->plan_ok = false; }
     if (h->plan_rows_ok) { cufftDestroy(h->plan_rows); h->plan_rows_ok = false; }
 }
@@ -146,6 +154,9 @@ int rebuild_geom(muser_imager* h) {
     g.oty = (h->ny / 2 + kTile - 1) / kTile;
     g.ontiles = g.oty * g.otx;
     g.onbins = (uint32_t)h->ngrids * (uint32_t)g.ontiles;
+    g.phase_on = (h->off_l != 0.0 || h->off_m != 0.0) ? 1 : 0;
+    g.dl = h->off_l; g.dm = h->off_m;
+    g.uniform = h->weighting == MUSER_WEIGHT_UNIFORM ? 1 : 0;
     return MUSER_OK;
 }
 
@@ -162,6 +173,12 @@ int alloc_grids(muser_imager* h) {
     CU(h, cudaMemset(h->G, 0, nc * sizeof(float2)));
     CU(h, cudaMemset(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float))));
     CU(h, cudaMemset(h->stats_d, 0, sizeof(Stats)));
+    if (h->weighting == MUSER_WEIGHT_UNIFORM) {
+        CU(h, cudaMalloc(&h->cnt, nc * sizeof(int)));
+        CU(h, cudaMemset(h->cnt, 0, nc * sizeof(int)));
+    }
+    CU(h, cudaMalloc(&h->peaks_d, (size_t)h->ngrids * sizeof(PeakSlot)));
+    CU(h, cudaMemset(h->peaks_d, 0, (size_t)h->ngrids * sizeof(PeakSlot)));
     CU(h, cudaDeviceSynchronize());
     h->fft_valid = false;
     h->zero_pending = false;
@@ -180,10 +197,12 @@ int flush_zero(muser_imager* h, cudaStream_t s) {
     return MUSER_OK;
 }
 
+GridPtrs grid_ptrs(const muser_imager* h) { return GridPtrs{h->G, h->Gw, h->cnt}; }
+
 // rebuild rows 0 .. ny/2-1 of the grids from the stored half-plane (consumers of the full grids call this first)
 int ensure_lower(muser_imager* h, cudaStream_t s) {
     if (h->lower_valid) return MUSER_OK;
-    CU(h, launch_mirror_lower(h->geom, GridPtrs{h->G, h->Gw}, s));
+    CU(h, launch_mirror_lower(h->geom, grid_ptrs(h), s));
     h->n_launches += 1;
     h->lower_valid = true;
     return MUSER_OK;
@@ -353,10 +372,10 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
               const int* gid, long long nvis, cudaStream_t s) {
     if (nvis < 0 || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "nvis out of range [0, 2^30]");
     if (nvis == 0) return MUSER_OK;
-    if (!uvw || !freq || !vis || !wt) return fail(h, MUSER_EINVAL, "null input pointer");
+    if (!uvw || !freq || !wt || (!vis && !h->weights_only)) return fail(h, MUSER_EINVAL, "null input pointer");
     const int strat = pick_strategy(h);
     const Geom& g = h->geom;
-    GridPtrs gp{h->G, h->Gw};
+    GridPtrs gp = grid_ptrs(h);
     if (strat == MUSER_STRATEGY_OWNER) {
         if (!owner_capable(h)) return fail(h, MUSER_EUNSUPPORTED, "the owner-tile strategy needs 2-D mode and support 7");
         const uint32_t item_size = owner_item_size(nvis, h->num_sms, h->tune[MUSER_TUNE_ITEM_SIZE]);
@@ -372,8 +391,8 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
                                      h->tune[MUSER_TUNE_BIN_VPT], s));
             CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size,
                                     h->ow_work, h->ow_ctl, h->ow_tops, s));
-            CU(h, launch_owner_scatter(g, h->ow_loc, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_cursor,
-                                       h->ow_sorted, h->tune[MUSER_TUNE_BIN_VPT], s));
+            CU(h, launch_owner_scatter(g, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_cursor,
+                                       h->ow_sorted, h->cnt, h->tune[MUSER_TUNE_BIN_VPT], s));
         }
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
@@ -396,7 +415,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
         CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
-                            h->stats_d, s));
+                            h->stats_d, h->cnt, s));
         CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, s));
         CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
         h->n_launches += 3;
@@ -421,14 +440,16 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         // transform, so muser_dirty followed by muser_psf repeats only the column pass
         if (!h->fft_valid) {
             StageScope sc(h, MUSER_STAGE_FFT, s);
-            CU(h, launch_fft_rows_half(h->geom, h->G, h->Gw, h->tw_rows_d, h->stats_d, h->H, h->num_sms, s));
+            CU(h, launch_fft_rows_half(h->geom, h->G, h->Gw, h->cnt, h->tw_rows_d, h->stats_d, h->H, h->num_sms, s));
             h->n_launches += 1;
             h->fft_valid = true;
         }
         StageScope sc(h, MUSER_STAGE_CORRECT, s);
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, s));
+        PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
+        if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, s));
         h->n_launches += 1;
         return MUSER_OK;
     }
@@ -445,7 +466,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
                 int rc = ensure_lower(h, s);
                 if (rc) return rc;
                 StageScope sc(h, MUSER_STAGE_PACK, s);
-                CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, h->stats_d, s));
+                CU(h, launch_pack(h->geom, grid_ptrs(h), h->H, h->stats_d, s));
                 h->n_launches += 1;
             }
             StageScope sc(h, MUSER_STAGE_FFT, s);
@@ -457,7 +478,9 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         StageScope sc(h, MUSER_STAGE_CORRECT, s);
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, s));
+        PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
+        if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, s));
         h->n_launches += 1;
         return MUSER_OK;
     }
@@ -472,7 +495,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
             int rc = ensure_lower(h, s);
             if (rc) return rc;
             StageScope sc(h, MUSER_STAGE_PACK, s);
-            CU(h, launch_pack(h->geom, GridPtrs{h->G, h->Gw}, h->H, h->stats_d, s));
+            CU(h, launch_pack(h->geom, grid_ptrs(h), h->H, h->stats_d, s));
             h->n_launches += 1;
         }
         {
@@ -487,7 +510,9 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         StageScope sc(h, MUSER_STAGE_CORRECT, s);
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
-        CU(h, launch_correct(h->geom, h->H, cx, cy, h->stats_d, dirty, psf, s));
+        PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
+        if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
+        CU(h, launch_correct(h->geom, h->H, cx, cy, h->stats_d, dirty, psf, peaks, s));
         h->n_launches += 1;
     }
     return MUSER_OK;
@@ -504,6 +529,8 @@ int reset_impl(muser_imager* h, cudaStream_t s) {
         if (rc) return rc;
     }
     CU(h, cudaMemsetAsync(h->stats_d, 0, sizeof(Stats), s));
+    if (h->cnt) CU(h, cudaMemsetAsync(h->cnt, 0, grid_cells(h) * sizeof(int), s));
+    if (h->child2x) return reset_impl(h->child2x, s);
     return MUSER_OK;
 }
 
@@ -576,6 +603,7 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
 
 int muser_imager_destroy(muser_imager* h) {
     if (!h) return MUSER_OK;
+    if (h->child2x) { muser_imager_destroy(h->child2x); h->child2x = nullptr; }
     cudaDeviceSynchronize();
     free_grids(h);
     free_bins(h);
@@ -614,7 +642,9 @@ int muser_set_batch(muser_imager* h, int ngrids) {
     h->ngrids = ngrids;
     int rc = rebuild_geom(h);
     if (rc) { h->ngrids = old; rebuild_geom(h); return rc; }
-    return alloc_grids(h);
+    if ((rc = alloc_grids(h))) return rc;
+    if (h->child2x) return muser_set_batch(h->child2x, ngrids);
+    return MUSER_OK;
 }
 
 int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, const int* supports,
@@ -687,7 +717,129 @@ int muser_set_tuning(muser_imager* h, int key, int value) {
 int muser_set_grid_correction(muser_imager* h, int enabled) {
     if (!h) return MUSER_EINVAL;
     h->correction = enabled ? 1 : 0;
+    if (h->child2x) h->child2x->correction = h->correction;
     return MUSER_OK;
+}
+
+int muser_set_weighting(muser_imager* h, int mode) {
+    if (!h) return MUSER_EINVAL;
+    if (mode != MUSER_WEIGHT_NATURAL && mode != MUSER_WEIGHT_UNIFORM) return fail(h, MUSER_EINVAL, "unknown weighting mode");
+    cudaDeviceSynchronize();
+    const int old = h->weighting;
+    h->weighting = mode;
+    int rc = rebuild_geom(h);
+    if (rc == MUSER_OK) rc = alloc_grids(h);
+    if (rc) { h->weighting = old; rebuild_geom(h); return rc; }
+    if (h->child2x) return muser_set_weighting(h->child2x, mode);
+    return MUSER_OK;
+}
+
+int muser_set_phase_offset(muser_imager* h, double dl, double dm) {
+    if (!h) return MUSER_EINVAL;
+    if (!std::isfinite(dl) || !std::isfinite(dm) || std::fabs(dl) > 1.0 || std::fabs(dm) > 1.0)
+        return fail(h, MUSER_EINVAL, "phase offset must be finite direction cosines");
+    h->off_l = dl; h->off_m = dm;
+    return rebuild_geom(h);                                           // the beam does not depend on it: the 2x child is left alone
+}
+
+int muser_set_peak_search(muser_imager* h, int enabled) {
+    if (!h) return MUSER_EINVAL;
+    h->peak_search = enabled != 0;
+    return MUSER_OK;
+}
+
+int muser_get_peak(muser_imager* h, float* peak_value, int* peak_x, int* peak_y, float* min_value) {
+    if (!h) return MUSER_EINVAL;
+    if (!h->peak_search) return fail(h, MUSER_ESTATE, "peak search is off (muser_set_peak_search)");
+    CU(h, cudaStreamSynchronize(h->last_stream));
+    std::vector<PeakSlot> p((size_t)h->ngrids);
+    CU(h, cudaMemcpy(p.data(), h->peaks_d, p.size() * sizeof(PeakSlot), cudaMemcpyDeviceToHost));
+    for (int g = 0; g < h->ngrids; ++g) {
+        if (p[g].maxkey == 0ull) return fail(h, MUSER_ESTATE, "no dirty image has been made since the peak search was enabled");
+        const unsigned int ord = (unsigned int)(p[g].maxkey >> 32), idx = ~(unsigned int)(p[g].maxkey & 0xFFFFFFFFull);
+        const unsigned int lo = ~p[g].minkey;
+        float v, m;
+        const unsigned int vb = (ord & 0x80000000u) ? (ord & 0x7FFFFFFFu) : ~ord, mb = (lo & 0x80000000u) ? (lo & 0x7FFFFFFFu) : ~lo;
+        std::memcpy(&v, &vb, 4); std::memcpy(&m, &mb, 4);
+        if (peak_value) peak_value[g] = v;
+        if (peak_x) peak_x[g] = (int)(idx % (unsigned int)h->nx);
+        if (peak_y) peak_y[g] = (int)(idx / (unsigned int)h->nx);
+        if (min_value) min_value[g] = m;
+    }
+    return MUSER_OK;
+}
+
+int muser_histogram(muser_imager* h, const float* image, int nbins, float lo, float hi, unsigned int* hist_out, muser_stream sv) {
+    if (!h) return MUSER_EINVAL;
+    if (!image || !hist_out) return fail(h, MUSER_EINVAL, "null pointer");
+    if (nbins < 1 || nbins > 8192) return fail(h, MUSER_EINVAL, "nbins must be in [1, 8192]");
+    const bool own_range = !(lo < hi);
+    if (own_range && !h->peak_search) return fail(h, MUSER_ESTATE, "lo >= hi asks for the image's own range: enable the peak search first");
+    if (h->ngrids > 65535) return fail(h, MUSER_EUNSUPPORTED, "histogram of more than 65535 grids per call");
+    cudaStream_t s = (cudaStream_t)sv;
+    h->last_stream = s;
+    CU(h, cudaMemsetAsync(hist_out, 0, (size_t)h->ngrids * nbins * sizeof(unsigned int), s));
+    CU(h, launch_histogram(image, (size_t)h->ny * h->nx, h->ngrids, nbins, lo, hi, own_range ? h->peaks_d : nullptr, hist_out, s));
+    h->n_launches += 1;
+    return MUSER_OK;
+}
+
+int muser_get_counts(muser_imager* h, int* counts_out, muser_stream sv) {
+    if (!h) return MUSER_EINVAL;
+    if (!counts_out) return fail(h, MUSER_EINVAL, "counts_out is null");
+    if (!h->cnt) return fail(h, MUSER_ESTATE, "hit counts exist in uniform weighting mode only");
+    cudaStream_t s = (cudaStream_t)sv;
+    h->last_stream = s;
+    int rc = flush_zero(h, s);
+    if (rc == MUSER_OK) rc = ensure_lower(h, s);
+    if (rc) return rc;
+    CU(h, cudaMemcpyAsync(counts_out, h->cnt, grid_cells(h) * sizeof(int), cudaMemcpyDeviceToDevice, s));
+    return MUSER_OK;
+}
+
+int muser_get_weighted_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_stream sv) {
+    if (!h) return MUSER_EINVAL;
+    cudaStream_t s = (cudaStream_t)sv;
+    h->last_stream = s;
+    int rc = flush_zero(h, s);
+    if (rc == MUSER_OK) rc = ensure_lower(h, s);
+    if (rc) return rc;
+    CU(h, launch_weighted_copy(h->geom, grid_ptrs(h), (float2*)grid_c64_out, wgrid_out, s));
+    h->n_launches += 1;
+    return MUSER_OK;
+}
+
+int muser_set_psf2x(muser_imager* h, int enabled) {
+    if (!h) return MUSER_EINVAL;
+    cudaDeviceSynchronize();
+    if (!enabled) {
+        if (h->child2x) { muser_imager_destroy(h->child2x); h->child2x = nullptr; }
+        return MUSER_OK;
+    }
+    if (h->child2x) return MUSER_OK;
+    if (wmode(h)) return fail(h, MUSER_EUNSUPPORTED, "the 2x beam is built in 2-D mode only");
+    if (2 * h->nx > 32768 || 2 * h->ny > 32768) return fail(h, MUSER_EINVAL, "2x beam too large");
+    muser_imager* c = muser_imager_create(2 * h->nx, 2 * h->ny, h->cell_arcsec, h->S, h->Q);
+    if (!c) return fail(h, MUSER_ENOMEM, std::string("2x beam: ") + g_create_error);
+    c->weights_only = true;
+    int rc = MUSER_OK;
+    if (h->kind != MUSER_KERNEL_PSWF) rc = muser_set_kernel(c, h->kind, h->gauss_a);
+    if (rc == MUSER_OK && h->ngrids != 1) rc = muser_set_batch(c, h->ngrids);
+    if (rc == MUSER_OK && h->weighting != MUSER_WEIGHT_NATURAL) rc = muser_set_weighting(c, h->weighting);
+    if (rc == MUSER_OK) rc = muser_set_strategy(c, h->strategy);
+    if (rc) { h->err = "2x beam: " + c->err; muser_imager_destroy(c); return rc; }
+    c->correction = h->correction;
+    h->child2x = c;
+    return MUSER_OK;
+}
+
+int muser_psf2x(muser_imager* h, float* beam2x_out, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    if (!beam2x_out) return fail(h, MUSER_EINVAL, "beam2x_out is null");
+    if (!h->child2x) return fail(h, MUSER_ESTATE, "the 2x beam is off (muser_set_psf2x)");
+    int rc = image_impl(h->child2x, nullptr, beam2x_out, (cudaStream_t)s);
+    if (rc) h->err = "2x beam: " + h->child2x->err;
+    return rc;
 }
 
 int muser_reset(muser_imager* h, muser_stream s) {
@@ -698,14 +850,24 @@ int muser_reset(muser_imager* h, muser_stream s) {
 int muser_grid(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64, const float* weight,
                long long nvis, muser_stream s) {
     if (!h) return MUSER_EINVAL;
-    return grid_impl(h, uvw_m, freq_hz, vis_c64, weight, nullptr, nvis, (cudaStream_t)s);
+    int rc = grid_impl(h, uvw_m, freq_hz, vis_c64, weight, nullptr, nvis, (cudaStream_t)s);
+    if (rc == MUSER_OK && h->child2x) {
+        rc = grid_impl(h->child2x, uvw_m, freq_hz, nullptr, weight, nullptr, nvis, (cudaStream_t)s);
+        if (rc) h->err = "2x beam: " + h->child2x->err;
+    }
+    return rc;
 }
 
 int muser_grid_batched(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
                        const float* weight, const int* grid_id, long long nvis, muser_stream s) {
     if (!h) return MUSER_EINVAL;
     if (!grid_id && nvis > 0) return fail(h, MUSER_EINVAL, "grid_id is required");
-    return grid_impl(h, uvw_m, freq_hz, vis_c64, weight, grid_id, nvis, (cudaStream_t)s);
+    int rc = grid_impl(h, uvw_m, freq_hz, vis_c64, weight, grid_id, nvis, (cudaStream_t)s);
+    if (rc == MUSER_OK && h->child2x) {
+        rc = grid_impl(h->child2x, uvw_m, freq_hz, nullptr, weight, grid_id, nvis, (cudaStream_t)s);
+        if (rc) h->err = "2x beam: " + h->child2x->err;
+    }
+    return rc;
 }
 
 int muser_dirty(muser_imager* h, float* image_out, muser_stream s) {

@@ -11,6 +11,8 @@
 // bank-conflict free.
 #include "muser_internal.h"
 
+#include <algorithm>
+
 namespace muser {
 
 constexpr int kFftC = 8;                       // columns per CTA
@@ -32,14 +34,16 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
                                                                                const float* __restrict__ icx,
                                                                                const float* __restrict__ icy,
                                                                                const Stats* __restrict__ stats,
-                                                                               float* __restrict__ dirty, float* __restrict__ psf) {
+                                                                               float* __restrict__ dirty, float* __restrict__ psf,
+                                                                               PeakSlot* __restrict__ peaks, const int grid0) {
     constexpr int T = N / 4;                   // butterflies per column and stage
     constexpr int NT = N / 2;                  // threads: thread (j, half) owns butterfly j of columns 4 half .. 4 half + 3
     constexpr int PITCH = N + N / 16 + 2;      // float4 per column pair, = 2 (mod 8)
     extern __shared__ __align__(16) float4 sm[];
     const int tid = threadIdx.x;
     const int sx0 = blockIdx.x * kFftC;        // source columns sx0 .. sx0 + 7
-    const size_t gbase = (size_t)blockIdx.y * N * nx;
+    const int gi = grid0 + (int)blockIdx.y;
+    const size_t gbase = (size_t)gi * N * nx;
     auto pad = [](int i) { return i + (i >> 4); };
 
     constexpr int R1 = (N == 256 || N == 1024) ? 16 : 8;                                   // radix of the first stage
@@ -136,15 +140,39 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
     const int x0 = (sx0 + (nx >> 1)) % nx + 4 * half;                                      // output columns x0 .. x0 + 3
     const float4 cx = *reinterpret_cast<const float4*>(icx + x0);
     const float ia = stats->inv_alpha;
-    const size_t obase = (size_t)blockIdx.y * N * nx;
+    const size_t obase = (size_t)gi * N * nx;
+    unsigned long long best = 0ull;                                                        // NEXT-4 peak search (see PeakSlot)
+    unsigned int lowest = 0u;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int ky = j + i * T, y = (ky + N / 2) & (N - 1);
         const float cy = (y & 1) ? -icy[y] : icy[y];                                       // x0 is a multiple of 4: sign = (-1)^y * (+,-,+,-)
         const float m0 = cx.x * cy, m1 = -cx.y * cy, m2 = cx.z * cy, m3 = -cx.w * cy;
         const size_t o = obase + (size_t)y * nx + x0;
-        if (dirty) *reinterpret_cast<float4*>(dirty + o) = make_float4(v[0][i].x * m0, v[1][i].x * m1, v[2][i].x * m2, v[3][i].x * m3);
+        if (dirty) {
+            const float4 d = make_float4(v[0][i].x * m0, v[1][i].x * m1, v[2][i].x * m2, v[3][i].x * m3);
+            *reinterpret_cast<float4*>(dirty + o) = d;
+            if (peaks) {
+                const unsigned int base = (unsigned int)(y * nx + x0);
+                const float dv[4] = {d.x, d.y, d.z, d.w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const unsigned int ord = peak_ordered(dv[c]);
+                    const unsigned long long key = ((unsigned long long)ord << 32) | (unsigned long long)(~(base + c));
+                    best = key > best ? key : best;
+                    lowest = max(lowest, ~ord);
+                }
+            }
+        }
         if (psf) *reinterpret_cast<float4*>(psf + o) = make_float4(v[0][i].y * m0 * ia, v[1][i].y * m1 * ia, v[2][i].y * m2 * ia, v[3][i].y * m3 * ia);
+    }
+    if (dirty && peaks) {                                                                  // one atomic pair per warp
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long ob = __shfl_xor_sync(0xffffffffu, best, o);
+            best = ob > best ? ob : best;
+            lowest = max(lowest, __shfl_xor_sync(0xffffffffu, lowest, o));
+        }
+        if ((tid & 31) == 0) { atomicMax(&peaks[gi].maxkey, best); atomicMax(&peaks[gi].minkey, lowest); }
     }
 }
 
@@ -201,8 +229,9 @@ __device__ __forceinline__ void idft8_half(float2 (&v)[8]) {
 
 template <int N, int WMODE>
 __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int ngroups, const float2* __restrict__ G,
-                                                         const float* __restrict__ Gw, const float2* __restrict__ tw,
-                                                         Stats* __restrict__ stats, float2* __restrict__ Z) {
+                                                         const float* __restrict__ Gw, const int* __restrict__ cnt,
+                                                         const float2* __restrict__ tw, Stats* __restrict__ stats,
+                                                         float2* __restrict__ Z) {
     using C = RowCfg<N, WMODE>;
     constexpr int T = C::T, PITCH = C::PITCH, R1 = C::R1, ROWS = C::ROWS, NSEQ = C::NSEQ, NP = C::NP;
     extern __shared__ __align__(16) float4 sm[];
@@ -225,25 +254,46 @@ __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int
         for (int task = tid; task < NSEQ * (N / R1); task += T) {
             const int s = task / (N / R1), j = task - s * (N / R1);
             float2 v[R1];
+            // wgtGrid_kernel (Alg. 1 l.1-16) in uniform mode: a cell is multiplied by 1 / count where
+            // count != 0, here as the cell is loaded
+            auto wgt = [&](size_t cell) -> float {
+                if (!cnt) return 1.0f;
+                const int c = __ldg(cnt + cell);
+                return c ? 1.0f / (float)c : 1.0f;
+            };
             if (WMODE) {
                 const size_t row = gbase + (size_t)(iy0 + (s >> 1)) * N;
                 if (s & 1) {
                     const float2* src = reinterpret_cast<const float2*>(Gw) + row;
 #pragma unroll
-                    for (int i = 0; i < R1; ++i) { const float2 q = __ldg(src + j + i * (N / R1)); v[i] = make_float2(al * q.x, al * q.y); }
+                    for (int i = 0; i < R1; ++i) {
+                        const float2 q = __ldg(src + j + i * (N / R1));
+                        const float u = al * wgt(row + j + i * (N / R1));
+                        v[i] = make_float2(u * q.x, u * q.y);
+                    }
                 } else {
 #pragma unroll
-                    for (int i = 0; i < R1; ++i) v[i] = __ldg(G + row + j + i * (N / R1));
+                    for (int i = 0; i < R1; ++i) {
+                        const float2 q = __ldg(G + row + j + i * (N / R1));
+                        const float u = wgt(row + j + i * (N / R1));
+                        v[i] = make_float2(u * q.x, u * q.y);
+                    }
                 }
             } else if (s < ROWS) {
                 const size_t row = gbase + (size_t)(iy0 + s) * N;
 #pragma unroll
-                for (int i = 0; i < R1; ++i) v[i] = __ldg(G + row + j + i * (N / R1));
+                for (int i = 0; i < R1; ++i) {
+                    const float2 q = __ldg(G + row + j + i * (N / R1));
+                    const float u = wgt(row + j + i * (N / R1));
+                    v[i] = make_float2(u * q.x, u * q.y);
+                }
             } else {
                 const size_t row = gbase + (size_t)(iy0 + 2 * (s - ROWS)) * N;
 #pragma unroll
-                for (int i = 0; i < R1; ++i)
-                    v[i] = make_float2(al * __ldg(Gw + row + j + i * (N / R1)), al * __ldg(Gw + row + N + j + i * (N / R1)));
+                for (int i = 0; i < R1; ++i) {
+                    const size_t c0 = row + j + i * (N / R1);
+                    v[i] = make_float2(al * wgt(c0) * __ldg(Gw + c0), al * wgt(c0 + N) * __ldg(Gw + c0 + N));
+                }
             }
             float2* dst = reinterpret_cast<float2*>(sm + (s >> 1) * PITCH) + (s & 1);
             if constexpr (R1 == 16) {
@@ -349,14 +399,14 @@ cudaError_t fft_cols_setup() {
 }
 
 template <int N, int WMODE>
-static cudaError_t launch_rows_t(const Geom& g, const float2* G, const float* Gw, const float2* tw, Stats* stats, float2* Z,
-                                 int num_sms, cudaStream_t s) {
+static cudaError_t launch_rows_t(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw, Stats* stats,
+                                 float2* Z, int num_sms, cudaStream_t s) {
     using C = RowCfg<N, WMODE>;
     const int ngroups = g.ngrids * ((g.ny / 2) / C::ROWS);
     int per_sm = (int)(200 * 1024 / (C::SMEM + 1024));
     per_sm = per_sm < 1 ? 1 : (per_sm > 2048 / C::T ? 2048 / C::T : per_sm);
     const int blocks = ngroups < num_sms * per_sm ? ngroups : num_sms * per_sm;
-    k_fft_rows_half<N, WMODE><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, tw, stats, Z);
+    k_fft_rows_half<N, WMODE><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, g.uniform ? cnt : nullptr, tw, stats, Z);
     return cudaGetLastError();
 }
 
@@ -385,12 +435,12 @@ cudaError_t fft_rows_setup() {
     return rows_setup_t<4096>();
 }
 
-cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const float2* tw, Stats* stats, float2* Z,
-                                 int num_sms, cudaStream_t s) {
+cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
+                                 Stats* stats, float2* Z, int num_sms, cudaStream_t s) {
 #define MUSER_ROWS_CASE(NN)                                                                                     \
     case NN:                                                                                                    \
-        return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, tw, stats, Z, num_sms, s)                               \
-                       : launch_rows_t<NN, 0>(g, G, Gw, tw, stats, Z, num_sms, s);
+        return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, cnt, tw, stats, Z, num_sms, s)                          \
+                       : launch_rows_t<NN, 0>(g, G, Gw, cnt, tw, stats, Z, num_sms, s);
     switch (g.nx) {
         MUSER_ROWS_CASE(64) MUSER_ROWS_CASE(128) MUSER_ROWS_CASE(256) MUSER_ROWS_CASE(512) MUSER_ROWS_CASE(1024)
         MUSER_ROWS_CASE(2048) MUSER_ROWS_CASE(4096)
@@ -400,14 +450,16 @@ cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw
 }
 
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
-                                    const Stats* stats, float* dirty, float* psf, cudaStream_t s) {
-    const dim3 blocks((unsigned)(g.nx / kFftC), (unsigned)g.ngrids);
-    if (g.ny == 256)
-        k_fft_cols_correct<256><<<blocks, 128, fft_smem_bytes(256), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
-    else if (g.ny == 512)
-        k_fft_cols_correct<512><<<blocks, 256, fft_smem_bytes(512), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
-    else
-        k_fft_cols_correct<1024><<<blocks, 512, fft_smem_bytes(1024), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf);
+                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, cudaStream_t s) {
+    for (int grid0 = 0; grid0 < g.ngrids; grid0 += 65535) {              // gridDim.y holds at most 65535 grids
+        const dim3 blocks((unsigned)(g.nx / kFftC), (unsigned)std::min(65535, g.ngrids - grid0));
+        if (g.ny == 256)
+            k_fft_cols_correct<256><<<blocks, 128, fft_smem_bytes(256), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+        else if (g.ny == 512)
+            k_fft_cols_correct<512><<<blocks, 256, fft_smem_bytes(512), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+        else
+            k_fft_cols_correct<1024><<<blocks, 512, fft_smem_bytes(1024), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+    }
     return cudaGetLastError();
 }
 

@@ -23,6 +23,9 @@ struct Geom {
     int otx, oty, ontiles;         // owner-tile path: tiles per row (kOwTileW cells wide), tile rows of the stored
                                    // half-plane (rows ny/2 .. ny-1, 32 cells tall), tiles per grid = oty*otx
     uint32_t onbins;               // ngrids*ontiles
+    int phase_on;                  // NEXT-3: V *= exp(+2 pi i (u dl + v dm)) before gridding
+    double dl, dm;
+    int uniform;                   // NEXT-2: hit counts are accumulated and wgtGrid (cell / count) is applied at the FFT input
 };
 
 // Per-plane kernel metadata in constant-ish device memory.
@@ -64,12 +67,36 @@ struct Stats {
 struct GridPtrs {
     float2* G;                     // [ngrids][ny][nx] complex
     float* Gw;                     // [ngrids][ny][nx] real (2-D) or complex interleaved (w mode)
+    int* cnt;                      // [ngrids][ny][nx] hit counts (uniform weighting only, else null); rows >= ny/2 are
+                                   // accumulated, the rest is mirrored on demand like G
 };
+
+// NEXT-3 (PAPER.md:174 step 3, :286): V * exp(+2 pi i (u dl + v dm)), u, v in wavelengths; the phase is reduced in fp64,
+// the rotation is fp32
+__device__ __forceinline__ float2 phase_rotate(const Geom& g, float um, float vm, double f, float2 V) {
+    const double il = __ddiv_rn(f, 299792458.0);
+    double x = __dmul_rn((double)um, il) * g.dl + __dmul_rn((double)vm, il) * g.dm;
+    x -= rint(x);
+    float sn, cs;
+    sincospif(2.0f * (float)x, &sn, &cs);
+    return make_float2(V.x * cs - V.y * sn, V.x * sn + V.y * cs);
+}
+
+// NEXT-4: per-grid peak search of the dirty image.  key = ordered(value) << 32 | ~flat index: atomicMax keeps the largest
+// value and, among equal values, the lowest index; the minimum is kept as the maximum of the inverted ordered value.
+struct PeakSlot { unsigned long long maxkey; unsigned int minkey; unsigned int pad; };
+__device__ __forceinline__ unsigned int peak_ordered(float v) {
+    const unsigned int b = __float_as_uint(v);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float peak_unordered(unsigned int o) {
+    return __uint_as_float((o & 0x80000000u) ? (o & 0x7FFFFFFFu) : ~o);
+}
 
 // ---- launch wrappers (muser_kernels.cu); all asynchronous on `s` -------------------------------------------
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                           const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
-                          uint32_t* bin_count, Stats* stats, cudaStream_t s);
+                          uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s);
 cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,
                               uint32_t* nitems, cudaStream_t s);
 cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsamples, const uint32_t* bin_offset,
@@ -78,9 +105,12 @@ cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* i
                               const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
                               GridPtrs grids, int num_sms, cudaStream_t s);
 cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, Stats* stats, cudaStream_t s);
+cudaError_t launch_weighted_copy(const Geom& g, GridPtrs grids, float2* G_out, float* Gw_out, cudaStream_t s);
+cudaError_t launch_histogram(const float* image, size_t npix, int ngrids, int nbins, float lo, float hi, const PeakSlot* peaks,
+                             unsigned int* hist, cudaStream_t s);
 cudaError_t launch_mirror_lower(const Geom& g, GridPtrs grids, cudaStream_t s);
 cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, const Stats* stats,
-                           float* dirty, float* psf, cudaStream_t s);
+                           float* dirty, float* psf, PeakSlot* peaks, cudaStream_t s);
 cudaError_t tiled_kernel_setup(int max_smem_bytes);
 
 // ---- owner-tile path (muser_owner.cu): 2-D mode, support 7.  The grids are Hermitian (every visibility is gridded
@@ -101,9 +131,9 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* cursor, uint32_t* bin_offset, OwItem* items,
                               uint32_t* nitems, uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops,
                               cudaStream_t s);
-cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float2* vis, const float* wt, const int* grid_id,
-                                 long long nvis, const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted,
-                                 int vpt_forced, cudaStream_t s);
+cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* uvw, const double* freq, const float2* vis,
+                                 const float* wt, const int* grid_id, long long nvis, const uint32_t* bin_offset,
+                                 uint32_t* cursor, uint4* sorted, int* cnt, int vpt_forced, cudaStream_t s);
 cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
@@ -118,9 +148,9 @@ cudaError_t fft_cols_setup();
 bool fft_rows_supported(int nx, int ny, int wmode);
 int fft_rows_first_radix(int nx);
 cudaError_t fft_rows_setup();
-cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const float2* tw, Stats* stats, float2* Z,
-                                 int num_sms, cudaStream_t s);
+cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
+                                 Stats* stats, float2* Z, int num_sms, cudaStream_t s);
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
-                                    const Stats* stats, float* dirty, float* psf, cudaStream_t s);
+                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, cudaStream_t s);
 
 }  // namespace muser

@@ -13,6 +13,8 @@
 
 #include <math_constants.h>
 
+#include <algorithm>
+
 namespace muser {
 
 static constexpr double kC = 299792458.0;   // m/s
@@ -32,7 +34,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                                                 const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                 const long long nvis, const PlaneMeta* __restrict__ planes,
                                                 Staged* __restrict__ staged, uint32_t* __restrict__ bin_count,
-                                                Stats* __restrict__ stats) {
+                                                Stats* __restrict__ stats, int* __restrict__ cnt) {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int flagged = 0, dropped = 0, kept = 0;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
@@ -42,7 +44,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
     if (k < nvis) {
         const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
         const double f = freq[k];
-        const float2 V = vis[k];
+        float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
         const float wt = weight[k];
         const int gid = grid_id ? grid_id[k] : 0;
         const double il = __ddiv_rn(f, kC);
@@ -76,6 +78,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                 dropped = 1;
             } else {
                 kept = 1;
+                if (g.phase_on) V = phase_rotate(g, um, vm, f, V);
                 wsum = 2.0 * (double)wt;
                 w2sum = (double)wt * (double)wt;
                 v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
@@ -94,6 +97,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                     o.gp = (uint32_t)gid | ((uint32_t)p << 24);
                     const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
                     o.bin = (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
+                    if (cnt) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, 1);   // NEXT-2 (this strategy grids both half-planes)
                 }
             }
         }
@@ -449,7 +453,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
 // and are empty by the drop rule R5.
 template <int WMODE>
 __global__ void __launch_bounds__(256) k_mirror_lower(const int nx, const int ny, const size_t total, float2* __restrict__ G,
-                                                      float* __restrict__ Gw) {
+                                                      float* __restrict__ Gw, int* __restrict__ cnt) {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // over [ngrids][ny/2][nx]
     if (t >= total) return;
     const int x = (int)(t % nx);
@@ -458,13 +462,16 @@ __global__ void __launch_bounds__(256) k_mirror_lower(const int nx, const int ny
     const size_t gbase = (row / (ny >> 1)) * (size_t)ny * nx;
     const size_t dst = gbase + (size_t)y * nx + x;
     float2 v = make_float2(0.f, 0.f), w = make_float2(0.f, 0.f);
+    int c = 0;
     if (x > 0 && y > 0) {
         const size_t src = gbase + (size_t)(ny - y) * nx + (nx - x);
         v = G[src];
         v.y = -v.y;
         if (WMODE) { w = reinterpret_cast<const float2*>(Gw)[src]; w.y = -w.y; }
         else w.x = Gw[src];
+        if (cnt) c = cnt[src];
     }
+    if (cnt) cnt[dst] = c;
     G[dst] = v;
     if (WMODE) reinterpret_cast<float2*>(Gw)[dst] = w;
     else Gw[dst] = w.x;
@@ -477,8 +484,8 @@ __global__ void __launch_bounds__(256) k_mirror_lower(const int nx, const int ny
 // not leak into the dirty image; a power of two keeps the scaling exact.
 template <int WMODE>
 __global__ void __launch_bounds__(256) k_pack(const size_t ncell2, const float4* __restrict__ G,
-                                              const float* __restrict__ Gw, float4* __restrict__ H,
-                                              Stats* __restrict__ stats) {
+                                              const float* __restrict__ Gw, const int* __restrict__ cnt,
+                                              float4* __restrict__ H, Stats* __restrict__ stats) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // two cells per thread
     const double v2 = stats->sum_val2, w2 = stats->sum_wt2;
     float al = 1.0f;
@@ -486,14 +493,22 @@ __global__ void __launch_bounds__(256) k_pack(const size_t ncell2, const float4*
     al = fminf(fmaxf(al, 9.5367431640625e-07f), 1048576.0f);
     if (i == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
     if (i >= ncell2) return;
-    const float4 gv = G[i];
+    float4 gv = G[i];
+    // wgtGrid_kernel (Alg. 1 l.1-16): uniform mode multiplies a cell by 1 / count where count != 0
+    float u0 = 1.0f, u1 = 1.0f;
+    if (cnt) {
+        const int2 c = reinterpret_cast<const int2*>(cnt)[i];
+        if (c.x) u0 = 1.0f / (float)c.x;
+        if (c.y) u1 = 1.0f / (float)c.y;
+        gv.x *= u0; gv.y *= u0; gv.z *= u1; gv.w *= u1;
+    }
     float4 o;
     if (WMODE == 0) {
         const float2 w = reinterpret_cast<const float2*>(Gw)[i];
-        o = make_float4(gv.x, gv.y + al * w.x, gv.z, gv.w + al * w.y);
+        o = make_float4(gv.x, gv.y + al * (w.x * u0), gv.z, gv.w + al * (w.y * u1));
     } else {
         const float4 w = reinterpret_cast<const float4*>(Gw)[i];
-        o = make_float4(gv.x - al * w.y, gv.y + al * w.x, gv.z - al * w.w, gv.w + al * w.z);
+        o = make_float4(gv.x - al * (w.y * u0), gv.y + al * (w.x * u0), gv.z - al * (w.w * u1), gv.w + al * (w.z * u1));
     }
     H[i] = o;
 }
@@ -503,7 +518,8 @@ __global__ void __launch_bounds__(256) k_pack(const size_t ncell2, const float4*
 __global__ void __launch_bounds__(256) k_correct(const int nx, const int ny, const int ngrids,
                                                  const float2* __restrict__ F, const float* __restrict__ icx,
                                                  const float* __restrict__ icy, const Stats* __restrict__ stats,
-                                                 float* __restrict__ dirty, float* __restrict__ psf) {
+                                                 float* __restrict__ dirty, float* __restrict__ psf,
+                                                 PeakSlot* __restrict__ peaks) {
     const int nx4 = nx >> 2;
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t total = (size_t)ngrids * ny * nx4;
@@ -521,11 +537,73 @@ __global__ void __launch_bounds__(256) k_correct(const int nx, const int ny, con
     const float cy = (y & 1) ? -icy[y] : icy[y];                         // x is a multiple of 4: sign = (-1)^y * (+,-,+,-)
     const float m0 = cx.x * cy, m1 = -cx.y * cy, m2 = cx.z * cy, m3 = -cx.w * cy;
     const size_t o = (gi * ny + y) * (size_t)nx + x;
-    if (dirty) *reinterpret_cast<float4*>(dirty + o) = make_float4(f01.x * m0, f01.z * m1, f23.x * m2, f23.z * m3);
+    if (dirty) {
+        const float4 d = make_float4(f01.x * m0, f01.z * m1, f23.x * m2, f23.z * m3);
+        *reinterpret_cast<float4*>(dirty + o) = d;
+        if (peaks) {                                                     // NEXT-4: strength and position of the peak, minimum
+            const unsigned int base = (unsigned int)((size_t)y * nx + x);
+            const float v[4] = {d.x, d.y, d.z, d.w};
+            unsigned long long best = 0ull;
+            unsigned int lo = 0u;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const unsigned int ord = peak_ordered(v[i]);
+                const unsigned long long key = ((unsigned long long)ord << 32) | (unsigned long long)(~(base + i));
+                best = key > best ? key : best;
+                lo = max(lo, ~ord);
+            }
+            atomicMax(&peaks[gi].maxkey, best);
+            atomicMax(&peaks[gi].minkey, lo);
+        }
+    }
     if (psf) {
         const float ia = stats->inv_alpha;                               // exact power of two
         *reinterpret_cast<float4*>(psf + o) = make_float4(f01.y * m0 * ia, f01.w * m1 * ia, f23.y * m2 * ia, f23.w * m3 * ia);
     }
+}
+
+// The grids as wgtGrid_kernel leaves them (for inspection; the imaging path applies the same factor at the FFT input).
+template <int WMODE>
+__global__ void __launch_bounds__(256) k_weighted_copy(const size_t ncell, const float2* __restrict__ G,
+                                                       const float* __restrict__ Gw, const int* __restrict__ cnt,
+                                                       float2* __restrict__ G_out, float* __restrict__ Gw_out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ncell) return;
+    float u = 1.0f;
+    if (cnt) { const int c = cnt[i]; if (c) u = 1.0f / (float)c; }
+    if (G_out) { const float2 v = G[i]; G_out[i] = make_float2(v.x * u, v.y * u); }
+    if (Gw_out) {
+        if (WMODE) { const float2 w = reinterpret_cast<const float2*>(Gw)[i]; reinterpret_cast<float2*>(Gw_out)[i] = make_float2(w.x * u, w.y * u); }
+        else Gw_out[i] = Gw[i] * u;
+    }
+}
+
+// NEXT-4: "the data from a dirty image is divided into 2000 ranges".  bin = floor((v - lo) * (nbins /
+// (hi - lo))) in fp32 without contraction, hi itself in the last bin, values outside [lo, hi] not counted; lo >= hi: the
+// grid's own minimum and maximum from the peak search.  Shared-memory histogram per CTA, one global add per non-empty bin.
+__global__ void __launch_bounds__(256) k_histogram(const float* __restrict__ image, const size_t npix, const int nbins,
+                                                   float lo, float hi, const PeakSlot* __restrict__ peaks,
+                                                   unsigned int* __restrict__ hist) {
+    extern __shared__ unsigned int s_h[];
+    const int gi = blockIdx.y;
+    for (int i = threadIdx.x; i < nbins; i += 256) s_h[i] = 0u;
+    if (!(lo < hi) && peaks) {
+        hi = peak_unordered((unsigned int)(peaks[gi].maxkey >> 32));
+        lo = peak_unordered(~peaks[gi].minkey);
+    }
+    const float scale = __fdiv_rn((float)nbins, __fsub_rn(hi, lo));
+    __syncthreads();
+    const float* img = image + (size_t)gi * npix;
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < npix; i += (size_t)gridDim.x * 256) {
+        const float v = img[i];
+        if (v >= lo && v <= hi) {
+            const int b = min((int)floorf(__fmul_rn(__fsub_rn(v, lo), scale)), nbins - 1);
+            atomicAdd(&s_h[b], 1u);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < nbins; i += 256)
+        if (s_h[i]) atomicAdd(&hist[(size_t)gi * nbins + i], s_h[i]);
 }
 
 // ------------------------------------------------------------------------------------------------- launchers
@@ -533,9 +611,9 @@ static inline unsigned blocks_for(long long n, int per) { return (unsigned)((n +
 
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                           const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
-                          uint32_t* bin_count, Stats* stats, cudaStream_t s) {
+                          uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s) {
     k_coords<<<blocks_for(nvis, 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, planes, staged, bin_count,
-                                                   stats);
+                                                   stats, cnt);
     return cudaGetLastError();
 }
 
@@ -587,23 +665,41 @@ cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* i
 cudaError_t launch_pack(const Geom& g, GridPtrs grids, float2* H, Stats* stats, cudaStream_t s) {
     const size_t ncell2 = (size_t)g.ngrids * g.ny * g.nx / 2;
     const unsigned blocks = (unsigned)((ncell2 + 255) / 256);
-    if (g.wmode) k_pack<1><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H), stats);
-    else k_pack<0><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, reinterpret_cast<float4*>(H), stats);
+    const int* cnt = g.uniform ? grids.cnt : nullptr;
+    if (g.wmode) k_pack<1><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, cnt, reinterpret_cast<float4*>(H), stats);
+    else k_pack<0><<<blocks, 256, 0, s>>>(ncell2, reinterpret_cast<const float4*>(grids.G), grids.Gw, cnt, reinterpret_cast<float4*>(H), stats);
     return cudaGetLastError();
 }
 
 cudaError_t launch_mirror_lower(const Geom& g, GridPtrs grids, cudaStream_t s) {
     const size_t total = (size_t)g.ngrids * (g.ny / 2) * g.nx;
     const unsigned blocks = (unsigned)((total + 255) / 256);
-    if (g.wmode) k_mirror_lower<1><<<blocks, 256, 0, s>>>(g.nx, g.ny, total, grids.G, grids.Gw);
-    else k_mirror_lower<0><<<blocks, 256, 0, s>>>(g.nx, g.ny, total, grids.G, grids.Gw);
+    if (g.wmode) k_mirror_lower<1><<<blocks, 256, 0, s>>>(g.nx, g.ny, total, grids.G, grids.Gw, grids.cnt);
+    else k_mirror_lower<0><<<blocks, 256, 0, s>>>(g.nx, g.ny, total, grids.G, grids.Gw, grids.cnt);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_weighted_copy(const Geom& g, GridPtrs grids, float2* G_out, float* Gw_out, cudaStream_t s) {
+    const size_t ncell = (size_t)g.ngrids * g.ny * g.nx;
+    const unsigned blocks = (unsigned)((ncell + 255) / 256);
+    const int* cnt = g.uniform ? grids.cnt : nullptr;
+    if (g.wmode) k_weighted_copy<1><<<blocks, 256, 0, s>>>(ncell, grids.G, grids.Gw, cnt, G_out, Gw_out);
+    else k_weighted_copy<0><<<blocks, 256, 0, s>>>(ncell, grids.G, grids.Gw, cnt, G_out, Gw_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_histogram(const float* image, size_t npix, int ngrids, int nbins, float lo, float hi, const PeakSlot* peaks,
+                             unsigned int* hist, cudaStream_t s) {
+    const unsigned bx = (unsigned)std::min<size_t>((npix + 256 * 16 - 1) / (256 * 16), 592);
+    k_histogram<<<dim3(bx ? bx : 1, (unsigned)ngrids), 256, (size_t)nbins * sizeof(unsigned int), s>>>(image, npix, nbins, lo, hi,
+                                                                                                         peaks, hist);
     return cudaGetLastError();
 }
 
 cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, const Stats* stats,
-                           float* dirty, float* psf, cudaStream_t s) {
+                           float* dirty, float* psf, PeakSlot* peaks, cudaStream_t s) {
     const size_t total = (size_t)g.ngrids * g.ny * (g.nx / 4);
-    k_correct<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(g.nx, g.ny, g.ngrids, F, icx, icy, stats, dirty, psf);
+    k_correct<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(g.nx, g.ny, g.ngrids, F, icx, icy, stats, dirty, psf, peaks);
     return cudaGetLastError();
 }
 

@@ -402,10 +402,12 @@ __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, i
 
 template <int VPT>
 __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, const uint4* __restrict__ loc,
+                                                               const float* __restrict__ uvw, const double* __restrict__ freq,
                                                                const float2* __restrict__ vis,
                                                                const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                                const long long nvis, const uint32_t* __restrict__ bin_offset,
-                                                               uint32_t* __restrict__ cursor, uint4* __restrict__ sorted) {
+                                                               uint32_t* __restrict__ cursor, uint4* __restrict__ sorted,
+                                                               int* __restrict__ cnt) {
     extern __shared__ uint32_t s_hist[];
     const long long base = (long long)blockIdx.x * (kBinThreads * VPT);
     const int lane = threadIdx.x & 31;
@@ -427,10 +429,17 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
                 L[j].cu[1] = (int)(o.y & 0xFFFFu); L[j].cv[1] = (int)(o.y >> 16);
                 L[j].rx[0] = (int)(o.z & 511u); L[j].ry[0] = (int)((o.z >> 9) & 511u); L[j].rx[1] = (int)((o.z >> 18) & 511u);
                 L[j].ry[1] = (int)(o.w & 511u);
-                const float2 V = vis[k];
+                float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
+                if (g.phase_on) V = phase_rotate(g, uvw[3 * k], uvw[3 * k + 1], freq[k], V);
                 const float wt = weight[k];
                 L[j].re = wt * V.x; L[j].im = wt * V.y; L[j].wt = wt; L[j].gid = grid_id ? grid_id[k] : 0;
                 same &= (L[j].gid == ref);
+                if (cnt) {                                            // NEXT-2: one hit per sample at its nearest cell (stored half-plane)
+#pragma unroll
+                    for (int s = 0; s < 2; ++s)
+                        if (L[j].cv[s] >= (g.ny >> 1))
+                            atomicAdd(cnt + ((size_t)L[j].gid * g.ny + L[j].cv[s]) * g.nx + L[j].cu[s], 1);
+                }
             }
         }
     }
@@ -683,7 +692,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     int tx, ty;
     const bool heavy = wi < n_items;
     uint32_t li = wi - n_items;                                       // index into the light-tile list
-    if (STORE && !heavy) {
+    if constexpr (STORE != 0) if (!heavy) {
         const uint32_t j = li, f = j / kfill;
         if (f < n_fill && j == f * kfill) {                           // fill unit f: zero the empty tiles of one tile row
             ow_fill_row(g, bin_offset, grids, (int)(f / (uint32_t)g.oty), (int)(f % (uint32_t)g.oty),
@@ -965,17 +974,17 @@ cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* curs
     return cudaGetLastError();
 }
 
-cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float2* vis, const float* wt, const int* grid_id,
-                                 long long nvis, const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted,
-                                 int vpt_forced, cudaStream_t s) {
+cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* uvw, const double* freq, const float2* vis,
+                                 const float* wt, const int* grid_id, long long nvis, const uint32_t* bin_offset,
+                                 uint32_t* cursor, uint4* sorted, int* cnt, int vpt_forced, cudaStream_t s) {
     const int vpt = bin_vpt(nvis, vpt_forced);
     const unsigned blocks = (unsigned)((nvis + kBinThreads * vpt - 1) / (kBinThreads * vpt));
     if (vpt == 4)
-        k_owner_scatter<4><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
+        k_owner_scatter<4><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted, cnt);
     else if (vpt == 2)
-        k_owner_scatter<2><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
+        k_owner_scatter<2><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted, cnt);
     else
-        k_owner_scatter<1><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, vis, wt, grid_id, nvis, bin_offset, cursor, sorted);
+        k_owner_scatter<1><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted, cnt);
     return cudaGetLastError();
 }
 
