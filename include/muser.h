@@ -123,6 +123,26 @@ int muser_grid(muser_imager* h, const float* uvw_m, const double* freq_hz, const
 int muser_grid_batched(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
                        const float* weight, const int* grid_id, long long nvis, muser_stream s);
 
+/* NEXT-1, the channelised call (a 3 ms frame is 16 channels x 2 polarisations of the SAME baselines): the
+ * same gridding as muser_grid on the visibilities (t, p, c, r) with coordinates uvw_m[t][r] * freq_hz[c] / c, in the
+ * instrument's own layout, 12.4 instead of 32 bytes per visibility.  DEVICE pointers:
+ *   uvw_m   float  [ntime][nrow][3]           baseline coordinates in metres, one set per time step
+ *   freq_hz double [nchan]                    channel frequencies
+ *   vis_c64 float  [ntime][npol][nchan][nrow][2]
+ *   weight  float  [ntime][npol][nchan][nrow]
+ *   grid_id int    MUSER_POLS_SUM:   [ntime][nchan]        the polarisations of a (time, channel) go onto one grid; their
+ *                                                          weighted visibilities are added up before gridding (one
+ *                                                          kernel evaluation per baseline and channel instead of npol)
+ *                  MUSER_POLS_SPLIT: [ntime][npol][nchan]  one grid per polarisation (the paper's per-channel,
+ *                                                          per-polarisation images)
+ *                  NULL: everything onto grid 0
+ * The result is that of muser_grid(_batched) on the flattened arrays (the order of the fp32 sums differs); flags, drops
+ * and counters are per visibility as there.  nchan <= 512, npol <= 8.  Owner-tile strategy only (2-D mode, support 7),
+ * else MUSER_EUNSUPPORTED. */
+enum { MUSER_POLS_SUM = 0, MUSER_POLS_SPLIT = 1 };
+int muser_grid_rows(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64, const float* weight,
+                    const int* grid_id, long long nrow, int nchan, int npol, int ntime, int pol_mode, muser_stream s);
+
 /* ---- A5 + A6 imaging --------------------------------------------------------------------------------------
  * DEVICE outputs float [ngrids][ny][nx].  One complex inverse FFT of H = G + i*Gw yields both images (the
  * dirty image is its real part, the beam its imaginary part, because G and Gw are Hermitian); muser_dirty and

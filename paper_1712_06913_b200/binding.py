@@ -17,6 +17,7 @@ MUSER_KERNEL_PSWF, MUSER_KERNEL_GAUSS = 0, 1
 MUSER_STRATEGY_AUTO, MUSER_STRATEGY_TILED, MUSER_STRATEGY_OWNER = 0, 2, 3
 MUSER_TUNE_ITEM_SIZE, MUSER_TUNE_BIN_VPT = 0, 1
 MUSER_WEIGHT_NATURAL, MUSER_WEIGHT_UNIFORM = 0, 1
+MUSER_POLS_SUM, MUSER_POLS_SPLIT = 0, 1
 STAGES = ("bin", "grid", "pack", "fft", "correct")
 
 _c = ctypes
@@ -44,6 +45,7 @@ SIGNATURES = {
     "muser_reset": (_i, [_vp, _vp]),
     "muser_grid": (_i, [_vp, _vp, _vp, _vp, _vp, _ll, _vp]),
     "muser_grid_batched": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _ll, _vp]),
+    "muser_grid_rows": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _ll, _i, _i, _i, _i, _vp]),
     "muser_dirty": (_i, [_vp, _vp, _vp]),
     "muser_psf": (_i, [_vp, _vp, _vp]),
     "muser_dirty_psf": (_i, [_vp, _vp, _vp, _vp]),
@@ -200,6 +202,12 @@ class Imager:
     def grid_batched(self, uvw_m, freq_hz, vis, weight, grid_id, stream=None):
         self._ck(lib().muser_grid_batched(self._h, _ptr(uvw_m), _ptr(freq_hz), _ptr(vis), _ptr(weight),
                                           _ptr(grid_id), int(vis.shape[0]), _stream(stream)))
+
+    def grid_rows(self, uvw_m, freq_hz, vis, weight, grid_id=None, pol_mode=MUSER_POLS_SUM, stream=None):
+        """uvw_m [ntime][nrow][3], freq_hz [nchan], vis / weight [ntime][npol][nchan][nrow] (device tensors)."""
+        ntime, npol, nchan, nrow = (int(x) for x in vis.shape[:4])
+        self._ck(lib().muser_grid_rows(self._h, _ptr(uvw_m), _ptr(freq_hz), _ptr(vis), _ptr(weight), _ptr(grid_id),
+                                       nrow, nchan, npol, ntime, pol_mode, _stream(stream)))
 
     def dirty(self, image_out, stream=None):
         self._ck(lib().muser_dirty(self._h, _ptr(image_out), _stream(stream)))

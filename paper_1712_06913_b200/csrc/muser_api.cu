@@ -429,6 +429,48 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     return MUSER_OK;
 }
 
+// NEXT-1: the channelised call.  Owner-tile strategy only (2-D mode, support 7): its binning kernels have the rows variant.
+int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const void* vis, const float* wt, const int* gid,
+                   long long nrow, int nchan, int npol, int ntime, int pol_mode, cudaStream_t s) {
+    if (nrow < 0 || nchan < 1 || npol < 1 || ntime < 1 || nchan > rows_max_channels() || npol > 8)
+        return fail(h, MUSER_EINVAL, "rows call: need nrow >= 0, 1 <= nchan <= 512, 1 <= npol <= 8, ntime >= 1");
+    if (pol_mode != MUSER_POLS_SUM && pol_mode != MUSER_POLS_SPLIT) return fail(h, MUSER_EINVAL, "unknown pol_mode");
+    const long long nvis = nrow * nchan * npol * ntime;
+    if (nrow > (1LL << 30) || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "too many visibilities in one call (2^30)");
+    if (nvis == 0) return MUSER_OK;
+    if (!uvw || !freq || !wt || (!vis && !h->weights_only)) return fail(h, MUSER_EINVAL, "null input pointer");
+    if (pick_strategy(h) != MUSER_STRATEGY_OWNER || !owner_capable(h))
+        return fail(h, MUSER_EUNSUPPORTED, "muser_grid_rows needs the owner-tile strategy (2-D mode, support 7)");
+    const Geom& g = h->geom;
+    const int split = pol_mode == MUSER_POLS_SPLIT ? 1 : 0;
+    const long long nelem = split ? nvis : nvis / npol;
+    const uint32_t item_size = owner_item_size(nelem, h->num_sms, h->tune[MUSER_TUNE_ITEM_SIZE]);
+    uint32_t max_items = 0;
+    int rc = ensure_owner_scratch(h, nelem, item_size, &max_items, s);
+    if (rc) return rc;
+    if (g.oty > 65535 || g.otx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
+    h->last_stream = s;
+    h->fft_valid = false;
+    {
+        StageScope sc(h, MUSER_STAGE_BIN, s);
+        CU(h, launch_rows_count(g, ntime, npol, nchan, (int)nrow, split, uvw, freq, (const float2*)vis, wt, gid, h->ow_count,
+                                h->stats_d, h->ow_loc, s));
+        CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size, h->ow_work,
+                                h->ow_ctl, h->ow_tops, s));
+        CU(h, launch_rows_scatter(g, ntime, npol, nchan, (int)nrow, split, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid,
+                                  h->ow_offset, h->ow_cursor, h->ow_sorted, h->cnt, s));
+    }
+    {
+        StageScope sc(h, MUSER_STAGE_GRID, s);
+        CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work, h->ow_ctl, h->ttp_d,
+                                grid_ptrs(h), h->ow_scratch, h->ow_tickets, h->zero_pending ? 1 : 0, h->num_sms, s));
+    }
+    h->n_launches += g.onbins <= 4096u ? 4 : 6;
+    h->zero_pending = false;
+    h->lower_valid = false;
+    return MUSER_OK;
+}
+
 int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     if (!dirty && !psf) return MUSER_OK;
     h->last_stream = s;
@@ -865,6 +907,17 @@ int muser_grid_batched(muser_imager* h, const float* uvw_m, const double* freq_h
     int rc = grid_impl(h, uvw_m, freq_hz, vis_c64, weight, grid_id, nvis, (cudaStream_t)s);
     if (rc == MUSER_OK && h->child2x) {
         rc = grid_impl(h->child2x, uvw_m, freq_hz, nullptr, weight, grid_id, nvis, (cudaStream_t)s);
+        if (rc) h->err = "2x beam: " + h->child2x->err;
+    }
+    return rc;
+}
+
+int muser_grid_rows(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64, const float* weight,
+                    const int* grid_id, long long nrow, int nchan, int npol, int ntime, int pol_mode, muser_stream s) {
+    if (!h) return MUSER_EINVAL;
+    int rc = grid_rows_impl(h, uvw_m, freq_hz, vis_c64, weight, grid_id, nrow, nchan, npol, ntime, pol_mode, (cudaStream_t)s);
+    if (rc == MUSER_OK && h->child2x) {
+        rc = grid_rows_impl(h->child2x, uvw_m, freq_hz, nullptr, weight, grid_id, nrow, nchan, npol, ntime, pol_mode, (cudaStream_t)s);
         if (rc) h->err = "2x beam: " + h->child2x->err;
     }
     return rc;

@@ -505,6 +505,288 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, con
     }
 }
 
+// ------------------------------------------------------------------------------------------------- O1r / O3r rows
+// NEXT-1, the channelised entry point (a 3 ms frame is 16 channels x 2 polarisations of the SAME baselines):
+//   uvw_m [ntime][nrow][3], freq_hz [nchan], vis / weight [ntime][npol][nchan][nrow], 12.4 bytes per visibility.
+// An ELEMENT is (t, po, c, r): one baseline at one channel.  Its O1 coordinates are computed once -- f/c once per channel
+// and CTA -- and shared by the polarisations of the element: in SUM mode (npo = 1, npi = npol) they all go onto one
+// grid, so their weighted visibilities and weights are added up BEFORE gridding and the element becomes one record
+// per sample instead of npol (identical cells and kernel weights; only the order of the fp32 sums changes); in SPLIT mode
+// (npo = npol, npi = 1) every polarisation has its own grid.  From the records on, the path is the flat one.
+struct RowsShape { int ntime, npo, npi, nchan, nrow; };
+
+// the polarisations p = po + pi of one element: flag, drop or keep each; sums over the kept ones
+struct RowsSum { int kept, flagged; float re, im, wt; double wsum, v2sum, w2sum; };
+__device__ __forceinline__ RowsSum rows_sum_pols(const Geom& g, const RowsShape& sh, const float2* __restrict__ vis,
+                                                 const float* __restrict__ weight, const int t, const int po, const int c,
+                                                 const int r, const bool geom_ok, const bool inside, const float um,
+                                                 const float vm, const double f) {
+    RowsSum o = {0, 0, 0.f, 0.f, 0.f, 0.0, 0.0, 0.0};
+    const int npol = sh.npo * sh.npi;
+#pragma unroll 2
+    for (int pi = 0; pi < sh.npi; ++pi) {
+        const size_t k = (((size_t)t * npol + (po + pi)) * sh.nchan + c) * sh.nrow + r;
+        float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
+        const float wt = weight[k];
+        if (!(geom_ok && isfinite(wt) && isfinite(V.x) && isfinite(V.y) && wt > 0.0f)) { ++o.flagged; continue; }
+        if (!inside) continue;
+        ++o.kept;
+        o.wsum += 2.0 * (double)wt;
+        const double w2 = (double)wt * (double)wt;
+        o.w2sum += w2;
+        o.v2sum += w2 * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
+        if (g.phase_on) V = phase_rotate(g, um, vm, f, V);
+        o.re += wt * V.x; o.im += wt * V.y; o.wt += wt;
+    }
+    return o;
+}
+
+// element -> (t, po, c, r), coordinates and keep/drop of its two samples (same arithmetic as ow_locate)
+struct RowsElem { int t, po, c, r, gid; bool geom_ok, inside; float um, vm; double f; OwLoc L; };
+__device__ __forceinline__ void rows_locate(const Geom& g, const RowsShape& sh, const float* __restrict__ uvw,
+                                            const double* __restrict__ freq, const int* __restrict__ grid_id,
+                                            const double* s_il, const long long e, RowsElem& E) {
+    const long long per_c = sh.nrow, per_po = per_c * sh.nchan, per_t = per_po * sh.npo;
+    E.t = (int)(e / per_t);
+    long long rem = e - (long long)E.t * per_t;
+    E.po = (int)(rem / per_po); rem -= (long long)E.po * per_po;
+    E.c = (int)(rem / per_c);
+    E.r = (int)(rem - (long long)E.c * per_c);
+    const size_t ub = ((size_t)E.t * sh.nrow + E.r) * 3;
+    const float um = uvw[ub], vm = uvw[ub + 1], wm = uvw[ub + 2];
+    E.um = um; E.vm = vm; E.f = freq[E.c];
+    E.gid = grid_id ? grid_id[((size_t)E.t * sh.npo + E.po) * sh.nchan + E.c] : 0;
+    const double il = s_il[E.c];
+    const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
+    E.geom_ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(E.f) && E.gid >= 0 && E.gid < g.ngrids;
+    E.inside = false;
+    if (!E.geom_ok) return;
+    const int h = (g.S - 1) >> 1;
+    bool inside = true;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const double sgn = s ? -1.0 : 1.0;
+        double iu, iv, ru, rv;
+        ow_cell_phase(sgn * ul, g.su, g.nx, g.Q, iu, ru);
+        ow_cell_phase(sgn * vl, g.sv, g.ny, g.Q, iv, rv);
+        inside = inside && iu >= (double)(h + 1) && iu <= (double)(g.nx - 1 - h) && iv >= (double)(h + 1) &&
+                 iv <= (double)(g.ny - 1 - h);
+        E.L.cu[s] = (int)iu; E.L.cv[s] = (int)iv;
+        E.L.rx[s] = g.Q / 2 - (int)ru; E.L.ry[s] = g.Q / 2 - (int)rv;
+    }
+    E.inside = inside;
+}
+
+// f / c of every channel, once per CTA (the flat path divides once per visibility)
+__device__ __forceinline__ void rows_channel_scale(const RowsShape& sh, const double* __restrict__ freq, double* s_il) {
+    for (int c = threadIdx.x; c < sh.nchan; c += kBinThreads) s_il[c] = __ddiv_rn(freq[c], kC);
+}
+
+constexpr int kRowsMaxChan = 512;
+
+__global__ void __launch_bounds__(kBinThreads) k_rows_count(const Geom g, const RowsShape sh, const float* __restrict__ uvw,
+                                                            const double* __restrict__ freq, const float2* __restrict__ vis,
+                                                            const float* __restrict__ weight, const int* __restrict__ grid_id,
+                                                            const long long nelem, uint32_t* __restrict__ bin_count,
+                                                            Stats* __restrict__ stats, uint4* __restrict__ loc) {
+    extern __shared__ uint32_t s_hist[];
+    __shared__ double s_il[kRowsMaxChan];
+    const long long e = (long long)blockIdx.x * kBinThreads + threadIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool fits = g.ontiles <= kBinSmemTiles;
+    if (fits)
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
+    rows_channel_scale(sh, freq, s_il);
+    __syncthreads();
+    uint32_t tp[2] = {0u, 0u};
+    int kept = 0, dropped = 0, flagged = 0, same = 1, gid = 0, ref = 0;
+    double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
+    {   // the reference grid of the CTA: that of its first element
+        RowsElem E0;
+        rows_locate(g, sh, uvw, freq, grid_id, s_il, (long long)blockIdx.x * kBinThreads, E0);
+        ref = E0.gid;
+    }
+    if (e < nelem) {
+        RowsElem E;
+        rows_locate(g, sh, uvw, freq, grid_id, s_il, e, E);
+        const RowsSum S = rows_sum_pols(g, sh, vis, weight, E.t, E.po, E.c, E.r, E.geom_ok, E.inside, E.um, E.vm, E.f);
+        kept = S.kept; flagged = S.flagged; dropped = sh.npi - S.kept - S.flagged;
+        wsum = S.wsum; v2sum = S.v2sum; w2sum = S.w2sum;
+        uint4 o = make_uint4(0u, 0u, (S.kept ? 3u : 0u) << 30, 0u);
+        if (S.kept) {
+            o.x = (uint32_t)E.L.cu[0] | ((uint32_t)E.L.cv[0] << 16);
+            o.y = (uint32_t)E.L.cu[1] | ((uint32_t)E.L.cv[1] << 16);
+            o.z |= (uint32_t)E.L.rx[0] | ((uint32_t)E.L.ry[0] << 9) | ((uint32_t)E.L.rx[1] << 18);
+            o.w = (uint32_t)E.L.ry[1];
+            tp[0] = ow_tiles_packed(g, E.L.cu[0], E.L.cv[0]);
+            tp[1] = ow_tiles_packed(g, E.L.cu[1], E.L.cv[1]);
+            gid = E.gid;
+            same = gid == ref;
+        }
+        loc[e] = o;
+    }
+    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
+    if (ugrid >= 0) {
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const uint32_t t = tp[s];
+            if (!(t >> 31)) continue;
+            const uint32_t t00 = t & 0x1FFFFFFFu;
+            const bool mx = (t >> 29) & 1u, my = (t >> 30) & 1u;
+            atomicAdd(&s_hist[t00], 1u);
+            if (mx) atomicAdd(&s_hist[t00 + 1], 1u);
+            if (my) atomicAdd(&s_hist[t00 + g.otx], 1u);
+            if (mx && my) atomicAdd(&s_hist[t00 + g.otx + 1], 1u);
+        }
+        __syncthreads();
+        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
+            const uint32_t n = s_hist[i];
+            if (n) atomicAdd(&bin_count[gbase + i], n);
+        }
+    } else {
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const uint32_t t = tp[s];
+                const bool on = (t >> 31) && (!(q & 1) || ((t >> 29) & 1u)) && (!(q & 2) || ((t >> 30) & 1u));
+                const uint32_t bin = on ? (uint32_t)gid * (uint32_t)g.ontiles + (t & 0x1FFFFFFFu) + (q & 1) +
+                                              ((q & 2) ? (uint32_t)g.otx : 0u)
+                                        : kNoBin;
+                if (__any_sync(kFull, on)) ow_agg_inc(bin_count, bin, lane);
+            }
+    }
+    __shared__ int s_cnt[3][8];
+    __shared__ double s_w[3][8];
+    const int c0 = __reduce_add_sync(kFull, kept), c1 = __reduce_add_sync(kFull, dropped), c2 = __reduce_add_sync(kFull, flagged);
+    for (int o = 16; o > 0; o >>= 1) {
+        wsum += __shfl_xor_sync(kFull, wsum, o);
+        v2sum += __shfl_xor_sync(kFull, v2sum, o);
+        w2sum += __shfl_xor_sync(kFull, w2sum, o);
+    }
+    if (lane == 0) { s_cnt[0][warp] = c0; s_cnt[1][warp] = c1; s_cnt[2][warp] = c2; s_w[0][warp] = wsum; s_w[1][warp] = v2sum; s_w[2][warp] = w2sum; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t0 = 0, t1 = 0, t2 = 0;
+        double tw = 0.0, tv2 = 0.0, tw2 = 0.0;
+        for (int w = 0; w < kBinThreads / 32; ++w) {
+            t0 += s_cnt[0][w]; t1 += s_cnt[1][w]; t2 += s_cnt[2][w];
+            tw += s_w[0][w]; tv2 += s_w[1][w]; tw2 += s_w[2][w];
+        }
+        if (t0) {
+            atomicAdd(&stats->n_gridded, (unsigned long long)t0);
+            atomicAdd(&stats->sum_weights, tw);
+            atomicAdd(&stats->sum_val2, tv2);
+            atomicAdd(&stats->sum_wt2, tw2);
+        }
+        if (t1) atomicAdd(&stats->n_dropped, (unsigned long long)t1);
+        if (t2) atomicAdd(&stats->n_flagged, (unsigned long long)t2);
+    }
+}
+
+__global__ void __launch_bounds__(kBinThreads) k_rows_scatter(const Geom g, const RowsShape sh, const uint4* __restrict__ loc,
+                                                              const float* __restrict__ uvw, const double* __restrict__ freq,
+                                                              const float2* __restrict__ vis, const float* __restrict__ weight,
+                                                              const int* __restrict__ grid_id, const long long nelem,
+                                                              const uint32_t* __restrict__ bin_offset,
+                                                              uint32_t* __restrict__ cursor, uint4* __restrict__ sorted,
+                                                              int* __restrict__ cnt) {
+    extern __shared__ uint32_t s_hist[];
+    const long long e = (long long)blockIdx.x * kBinThreads + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool fits = g.ontiles <= kBinSmemTiles;
+    if (fits)
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
+    const long long per_c = sh.nrow, per_po = per_c * sh.nchan, per_t = per_po * sh.npo;
+    auto gid_of = [&](long long ee, int& t, int& po, int& c, int& r) -> int {
+        t = (int)(ee / per_t);
+        long long rem = ee - (long long)t * per_t;
+        po = (int)(rem / per_po); rem -= (long long)po * per_po;
+        c = (int)(rem / per_c);
+        r = (int)(rem - (long long)c * per_c);
+        return grid_id ? grid_id[((size_t)t * sh.npo + po) * sh.nchan + c] : 0;
+    };
+    int t0_, po0_, c0_, r0_;
+    const int ref = gid_of((long long)blockIdx.x * kBinThreads, t0_, po0_, c0_, r0_);
+    OwLoc L;
+    L.state = 0;
+    int same = 1;
+    if (e < nelem) {
+        const uint4 o = __ldg(loc + e);
+        L.state = (int)(o.z >> 30);
+        if (L.state == 3) {
+            L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
+            L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
+            L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
+            L.ry[1] = (int)(o.w & 511u);
+            int t, po, c, r;
+            L.gid = gid_of(e, t, po, c, r);
+            const size_t ub = ((size_t)t * sh.nrow + r) * 3;
+            const RowsSum S = rows_sum_pols(g, sh, vis, weight, t, po, c, r, true, true, uvw[ub], uvw[ub + 1], freq[c]);
+            L.re = S.re; L.im = S.im; L.wt = S.wt;
+            same = L.gid == ref;
+            if (cnt) {                                                // NEXT-2: one hit per visibility and sample
+#pragma unroll
+                for (int s = 0; s < 2; ++s)
+                    if (L.cv[s] >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)L.gid * g.ny + L.cv[s]) * g.nx + L.cu[s], S.kept);
+            }
+        }
+    }
+    const int kept = L.state == 3;
+    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
+    if (ugrid >= 0) {
+        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
+        uint32_t* s_base = s_hist + g.ontiles;
+        OwTiles T[2];
+        if (kept) {
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                T[s] = ow_tiles(g, L.cu[s], L.cv[s]);
+                if (!T[s].up) continue;
+                atomicAdd(&s_hist[T[s].t00], 1u);
+                if (T[s].mx) atomicAdd(&s_hist[T[s].t00 + 1], 1u);
+                if (T[s].my) atomicAdd(&s_hist[T[s].t00 + g.otx], 1u);
+                if (T[s].mx && T[s].my) atomicAdd(&s_hist[T[s].t00 + g.otx + 1], 1u);
+            }
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
+            const uint32_t n = s_hist[i];
+            if (n) { s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n); s_hist[i] = 0; }
+        }
+        __syncthreads();
+        if (kept) {
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const OwTiles t = T[s];
+                if (!t.up) continue;
+                ow_write_record(g, L, s, t.tx0, t.ty0, sorted + s_base[t.t00] + atomicAdd(&s_hist[t.t00], 1u));
+                if (t.mx) ow_write_record(g, L, s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + atomicAdd(&s_hist[t.t00 + 1], 1u));
+                if (t.my)
+                    ow_write_record(g, L, s, t.tx0, t.ty0 + 1,
+                                    sorted + s_base[t.t00 + g.otx] + atomicAdd(&s_hist[t.t00 + g.otx], 1u));
+                if (t.mx && t.my)
+                    ow_write_record(g, L, s, t.tx0 + 1, t.ty0 + 1,
+                                    sorted + s_base[t.t00 + g.otx + 1] + atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u));
+            }
+        }
+        return;
+    }
+    if (!__any_sync(kFull, kept)) return;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            int tx = 0, ty = 0;
+            const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
+            if (!__any_sync(kFull, bin != kNoBin)) continue;
+            const uint32_t rank = ow_agg_inc(cursor, bin, lane);
+            if (bin != kNoBin) ow_write_record(g, L, s, tx, ty, sorted + bin_offset[bin] + rank);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------- O4 gridding
 __device__ __forceinline__ unsigned long long ow_pack(float x, float y) {
     unsigned long long r;
@@ -959,6 +1241,29 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
         k_owner_count<1><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
     return cudaGetLastError();
 }
+
+cudaError_t launch_rows_count(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const float* uvw,
+                              const double* freq, const float2* vis, const float* wt, const int* grid_id, uint32_t* bin_count,
+                              Stats* stats, uint4* loc, cudaStream_t s) {
+    const RowsShape sh = {ntime, pols_split ? npol : 1, pols_split ? 1 : npol, nchan, nrow};
+    const long long nelem = (long long)ntime * sh.npo * nchan * nrow;
+    const unsigned blocks = (unsigned)((nelem + kBinThreads - 1) / kBinThreads);
+    k_rows_count<<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, sh, uvw, freq, vis, wt, grid_id, nelem, bin_count, stats, loc);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rows_scatter(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const uint4* loc,
+                                const float* uvw, const double* freq, const float2* vis, const float* wt, const int* grid_id,
+                                const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted, int* cnt, cudaStream_t s) {
+    const RowsShape sh = {ntime, pols_split ? npol : 1, pols_split ? 1 : npol, nchan, nrow};
+    const long long nelem = (long long)ntime * sh.npo * nchan * nrow;
+    const unsigned blocks = (unsigned)((nelem + kBinThreads - 1) / kBinThreads);
+    k_rows_scatter<<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, sh, loc, uvw, freq, vis, wt, grid_id, nelem, bin_offset, cursor,
+                                                                  sorted, cnt);
+    return cudaGetLastError();
+}
+
+int rows_max_channels() { return kRowsMaxChan; }
 
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* cursor, uint32_t* bin_offset, OwItem* items,
                               uint32_t* nitems, uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops,

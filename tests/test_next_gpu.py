@@ -224,3 +224,88 @@ def test_table2_non_power_of_two_image_size(n):
         gu.check_images(im, G_or, Gw_or, T, 7, Q)
     finally:
         im.destroy()
+
+
+def _rows_inputs(cfg, ntime, seed=0):
+    """Channelised inputs with the shape of a MUSER frame: baselines of synth's array at `ntime` hour angles."""
+    fr = synth.make_frame(cfg)
+    p = fr.params
+    nchan, npol = 16, 2
+    nrow = fr.nvis // (nchan * npol)
+    uvw1 = fr.uvw_m.reshape(npol, nchan, nrow, 3)[0, 0]
+    freq = fr.freq_hz.reshape(npol, nchan, nrow)[0, :, 0].copy()
+    rng = np.random.default_rng(100 + seed)
+    uvw = np.stack([uvw1 * (1.0 - 0.01 * t) for t in range(ntime)]).astype(np.float32)
+    vis = np.stack([fr.vis.reshape(npol, nchan, nrow)] * ntime).copy()
+    vis += (0.05 * (rng.standard_normal(vis.shape) + 1j * rng.standard_normal(vis.shape))).astype(np.complex64)
+    wt = rng.uniform(0.5, 1.5, vis.shape).astype(np.float32)
+    return p, uvw, freq, vis.astype(np.complex64), wt
+
+
+@pytest.mark.parametrize("mode", ["sum_one_grid", "sum_per_time_channel", "split"])
+def test_channelised_rows_call_equals_the_oracle_on_the_flattened_arrays(mode):
+    import torch
+    ntime = 2
+    p, uvw, freq, vis, wt = _rows_inputs(2, ntime)
+    _, npol, nchan, nrow = vis.shape
+    # flags in single polarisations and an off-grid baseline: per-visibility counters
+    wt[0, 1, 3, 5] = 0.0
+    wt[1, 0, 7, 11] = np.nan
+    vis[1, 1, 2, 9] = complex(np.inf, 0.0)
+    uvw[0, 17, 0] = 1.0e7
+    if mode == "sum_one_grid":
+        gid, split, ngrids = None, False, 1
+    elif mode == "sum_per_time_channel":
+        gid, split = (np.arange(ntime * nchan) % 5).reshape(ntime, nchan).astype(np.int32), False
+        ngrids = 5
+    else:
+        gid, split = (np.arange(ntime * npol * nchan) % 6).reshape(ntime, npol, nchan).astype(np.int32), True
+        ngrids = 6
+    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample, ngrids=ngrids)
+    try:
+        im.set_weighting(binding.MUSER_WEIGHT_UNIFORM)       # the hit counts check the per-visibility bookkeeping too
+        im.reset()
+        im.grid_rows(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), None if gid is None else gu.to_dev(gid),
+                     binding.MUSER_POLS_SPLIT if split else binding.MUSER_POLS_SUM)
+        fu, ff, fv, fw = mo.grid_rows_inputs(uvw, freq, vis, wt)
+        fg = mo.rows_grid_ids(gid, ntime, npol, nchan, nrow, split)
+        T = mo.table_pswf(p.support, p.oversample)
+        G_or, Gw_or, st = oc.grid(fu, ff, fv, fw, p.n, p.n, p.cell_arcsec, p.oversample, p.support, T, grid_id=fg, ngrids=ngrids,
+                                  counts=True)
+        got = im.get_stats()
+        assert (got["n_gridded"], got["n_dropped"], got["n_flagged"]) == (st["n_gridded"], st["n_dropped"], st["n_flagged"])
+        assert st["n_flagged"] == 3 and st["n_dropped"] >= npol * nchan
+        assert abs(got["sum_weights"] - st["sum_weights"]) <= 1e-9 * st["sum_weights"]
+        G, Gw = gu.gpu_grids(im)
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL and gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        cnt = torch.empty((ngrids, p.n, p.n), dtype=torch.int32, device="cuda")
+        im.get_counts(cnt)
+        torch.cuda.synchronize()
+        assert np.array_equal(cnt.cpu().numpy().astype(np.int64), st["cnt"])
+        im.set_weighting(binding.MUSER_WEIGHT_NATURAL)
+        im.reset()
+        im.grid_rows(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), None if gid is None else gu.to_dev(gid),
+                     binding.MUSER_POLS_SPLIT if split else binding.MUSER_POLS_SUM)
+        gu.check_images(im, G_or, Gw_or, T, p.support, p.oversample)
+    finally:
+        im.destroy()
+
+
+def test_channelised_rows_call_with_phase_offset_and_accumulation():
+    ntime = 3
+    p, uvw, freq, vis, wt = _rows_inputs(2, ntime, seed=1)
+    off = (1.3e-4, 0.9e-4)
+    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample)
+    try:
+        im.set_phase_offset(*off)
+        im.reset()
+        for t in range(ntime):                               # one call per time step, accumulating
+            im.grid_rows(gu.to_dev(uvw[t:t + 1]), gu.to_dev(freq), gu.to_dev(vis[t:t + 1]), gu.to_dev(wt[t:t + 1]))
+        fu, ff, fv, fw = mo.grid_rows_inputs(uvw, freq, vis, wt)
+        T = mo.table_pswf(p.support, p.oversample)
+        G_or, Gw_or, st = oc.grid(fu, ff, fv, fw, p.n, p.n, p.cell_arcsec, p.oversample, p.support, T, offset=off)
+        assert im.get_stats()["n_gridded"] == st["n_gridded"]
+        G, Gw = gu.gpu_grids(im)
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL and gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+    finally:
+        im.destroy()
