@@ -172,6 +172,12 @@ int muser_histogram(muser_imager* h, const float* image, int nbins, float lo, fl
 int muser_frame_host(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
                      const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
                      muser_stream s);
+/* The same without the final synchronisation (after the first call has sized the staging buffers it only enqueues):
+ * with pinned HOST buffers, two handles on two streams overlap one batch's copy back with the next batch's upload and
+ * imaging.  The caller synchronises the stream before reading the images or re-using the input buffers. */
+int muser_frame_host_async(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                           const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
+                           muser_stream s);
 
 /* ---- inspection ---------------------------------------------------------------------------------------------
  * Copy the centred grids (DC at [ny/2][nx/2]) to DEVICE buffers: grid_c64_out float [ngrids][ny][nx][2];

@@ -50,6 +50,7 @@ SIGNATURES = {
     "muser_psf": (_i, [_vp, _vp, _vp]),
     "muser_dirty_psf": (_i, [_vp, _vp, _vp, _vp]),
     "muser_frame_host": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _ll, _vp, _vp, _vp]),
+    "muser_frame_host_async": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _ll, _vp, _vp, _vp]),
     "muser_get_grid": (_i, [_vp, _vp, _vp, _vp]),
     "muser_get_table": (_i, [_vp, _i, _vp, _vp]),
     "muser_get_stats": (_i, [_vp, _vp, _vp, _vp, _vp]),
@@ -222,6 +223,11 @@ class Imager:
         """HOST buffers (numpy or pinned CPU tensors) in, HOST images out; synchronises the stream."""
         self._ck(lib().muser_frame_host(self._h, _ptr(uvw_m), _ptr(freq_hz), _ptr(vis), _ptr(weight), _ptr(grid_id),
                                         int(vis.shape[0]), _ptr(image_out), _ptr(beam_out), _stream(stream)))
+
+    def frame_host_async(self, uvw_m, freq_hz, vis, weight, grid_id, image_out, beam_out, stream=None):
+        """As frame_host without the final synchronisation (pinned buffers; synchronise the stream before reading)."""
+        self._ck(lib().muser_frame_host_async(self._h, _ptr(uvw_m), _ptr(freq_hz), _ptr(vis), _ptr(weight), _ptr(grid_id),
+                                              int(vis.shape[0]), _ptr(image_out), _ptr(beam_out), _stream(stream)))
 
     # ---- inspection
     def get_grid(self, grid_out, wgrid_out, stream=None):

@@ -940,9 +940,9 @@ int muser_dirty_psf(muser_imager* h, float* image_out, float* beam_out, muser_st
     return image_impl(h, image_out, beam_out, (cudaStream_t)s);
 }
 
-int muser_frame_host(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
-                     const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
-                     muser_stream sv) {
+static int frame_host_impl(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                           const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
+                           muser_stream sv, bool synchronise) {
     if (!h) return MUSER_EINVAL;
     if (nvis < 0 || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "nvis out of range");
     if (nvis > 0 && (!uvw_m || !freq_hz || !vis_c64 || !weight)) return fail(h, MUSER_EINVAL, "null input pointer");
@@ -976,8 +976,20 @@ int muser_frame_host(muser_imager* h, const float* uvw_m, const double* freq_hz,
     if (rc) return rc;
     if (image_out) CU(h, cudaMemcpyAsync(image_out, h->out_dirty, img_bytes, cudaMemcpyDeviceToHost, s));
     if (beam_out) CU(h, cudaMemcpyAsync(beam_out, h->out_psf, img_bytes, cudaMemcpyDeviceToHost, s));
-    CU(h, cudaStreamSynchronize(s));
+    if (synchronise) CU(h, cudaStreamSynchronize(s));
     return MUSER_OK;
+}
+
+int muser_frame_host(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                     const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
+                     muser_stream s) {
+    return frame_host_impl(h, uvw_m, freq_hz, vis_c64, weight, grid_id, nvis, image_out, beam_out, s, true);
+}
+
+int muser_frame_host_async(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64,
+                           const float* weight, const int* grid_id, long long nvis, float* image_out, float* beam_out,
+                           muser_stream s) {
+    return frame_host_impl(h, uvw_m, freq_hz, vis_c64, weight, grid_id, nvis, image_out, beam_out, s, false);
 }
 
 int muser_get_grid(muser_imager* h, void* grid_c64_out, float* wgrid_out, muser_stream sv) {

@@ -227,7 +227,7 @@ __device__ __forceinline__ void idft8_half(float2 (&v)[8]) {
     v[7] = cmul(v[7], make_float2(-h, h));
 }
 
-template <int N, int WMODE>
+template <int N, int WMODE, int UNIFORM>
 __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int ngroups, const float2* __restrict__ G,
                                                          const float* __restrict__ Gw, const int* __restrict__ cnt,
                                                          const float2* __restrict__ tw, Stats* __restrict__ stats,
@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int
             // wgtGrid_kernel (Alg. 1 l.1-16) in uniform mode: a cell is multiplied by 1 / count where
             // count != 0, here as the cell is loaded
             auto wgt = [&](size_t cell) -> float {
-                if (!cnt) return 1.0f;
+                if constexpr (UNIFORM == 0) return 1.0f;
                 const int c = __ldg(cnt + cell);
                 return c ? 1.0f / (float)c : 1.0f;
             };
@@ -406,15 +406,18 @@ static cudaError_t launch_rows_t(const Geom& g, const float2* G, const float* Gw
     int per_sm = (int)(200 * 1024 / (C::SMEM + 1024));
     per_sm = per_sm < 1 ? 1 : (per_sm > 2048 / C::T ? 2048 / C::T : per_sm);
     const int blocks = ngroups < num_sms * per_sm ? ngroups : num_sms * per_sm;
-    k_fft_rows_half<N, WMODE><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, g.uniform ? cnt : nullptr, tw, stats, Z);
+    if (g.uniform && cnt) k_fft_rows_half<N, WMODE, 1><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, cnt, tw, stats, Z);
+    else k_fft_rows_half<N, WMODE, 0><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, nullptr, tw, stats, Z);
     return cudaGetLastError();
 }
 
 template <int N>
 static cudaError_t rows_setup_t() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_fft_rows_half<N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 0>::SMEM))) return e;
-    return cudaFuncSetAttribute(k_fft_rows_half<N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 1>::SMEM);
+    if ((e = cudaFuncSetAttribute(k_fft_rows_half<N, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 0>::SMEM))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_rows_half<N, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 0>::SMEM))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_rows_half<N, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 1>::SMEM))) return e;
+    return cudaFuncSetAttribute(k_fft_rows_half<N, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<N, 1>::SMEM);
 }
 
 int fft_rows_first_radix(int nx) { return (nx == 64 || nx == 256 || nx == 1024 || nx == 4096) ? 16 : 8; }

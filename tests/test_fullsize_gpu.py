@@ -48,7 +48,7 @@ def _images_of(im, gi_list, G_or, Gw_or, T, S, Q):
 def test_cfg3_batch_of_80_frames_as_benched():
     import torch
     import bench
-    params, frames = bench.make_frames(bench.FRAMES_PER_STEP)
+    params, frames = bench.make_frames(bench.FRAMES_PER_STEP[3])
     B, n, nvis = len(frames), params.n, frames[0][2].shape[0]
     host = [np.ascontiguousarray(np.concatenate([fr[i] for fr in frames])) for i in range(4)]
     gid = np.repeat(np.arange(B, dtype=np.int32), nvis)
