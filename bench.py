@@ -69,7 +69,7 @@ def _committed_traffic(kernel):
 def make_frames(nframes, seed0=0, cfg=3):
     """nframes distinct frames of the config's shape: the array geometry and sky are those of synth.make_frame(cfg); every
     frame gets its own noise realisation (so buffers differ and nothing is cached between frames)."""
-    from paper_1712_06913_b200 import synth
+    from inputs import synth
     base = synth.make_frame(cfg)
     frames = []
     for k in range(nframes):
@@ -184,7 +184,7 @@ def cpu_direct_dft_cfg1():
     """the direct-DFT imager (definition (I)) on cfg 1, every pixel (1,560 samples x 65,536 pixels)."""
     from oracle import muser_oracle as mo
     from oracle import oracle_c as oc
-    from paper_1712_06913_b200 import synth
+    from inputs import synth
     fr = synth.make_frame(1)
     p = fr.params
     smp = mo.coordinates(fr.uvw_m, fr.freq_hz, fr.vis, fr.weight, p.n, p.n, p.cell_arcsec, p.oversample, p.support)
@@ -462,7 +462,7 @@ def bench_frames(args, cfg, torch, binding, shard, dist, rank, world, local):
 
 def bench_cfg4(args, torch, binding, shard, dist, rank, world, local):
     """cfg 4: a chunk of 64 frames = 2048 independent 512^2 grids of 1770 visibilities (the full config is 500 such chunks)."""
-    from paper_1712_06913_b200 import synth
+    from inputs import synth
     W = max(args.warmup, 3)
     fr = synth.make_frame(4, nframes=64)
     p = fr.params
@@ -529,7 +529,7 @@ def bench_cfg4(args, torch, binding, shard, dist, rank, world, local):
 
 def bench_cfg5(args, torch, binding, shard, dist, rank, world, local):
     """cfg 5: the whole configuration per step, 17 M visibilities onto one 4096^2 grid through 32 w-planes."""
-    from paper_1712_06913_b200 import synth
+    from inputs import synth
     W = max(args.warmup, 3)
     fr = synth.make_frame(5)
     p = fr.params

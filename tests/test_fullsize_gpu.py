@@ -13,7 +13,8 @@ import pytest
 
 from oracle import muser_oracle as mo
 from oracle import oracle_c as oc
-from paper_1712_06913_b200 import binding, synth
+from paper_1712_06913_b200 import binding
+from inputs import synth
 
 import gpu_util as gu
 

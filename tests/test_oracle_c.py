@@ -5,7 +5,7 @@ import pytest
 
 from oracle import muser_oracle as mo
 from oracle import oracle_c as oc
-from paper_1712_06913_b200 import synth
+from inputs import synth
 
 ARCSEC = np.pi / 648000.0
 
@@ -96,7 +96,7 @@ def test_cfg3_uv_coverage_is_centrally_condensed():
 def test_oracle_c_counts_and_phase_offset_equal_the_numpy_oracle():
     """NEXT-2 / NEXT-3 in the plain-C transcription: hit counts equal mo.hit_counts exactly; a phase offset equals
     mo.phase_correct applied first (fp64 on both sides)."""
-    from paper_1712_06913_b200 import synth
+    from inputs import synth
     fr = synth.make_frame(1)
     p = fr.params
     T = mo.table_gauss(p.support, p.oversample)

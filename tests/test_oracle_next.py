@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from oracle import muser_oracle as mo
-from paper_1712_06913_b200 import synth
+from inputs import synth
 
 
 def _small_rows(seed=3, ntime=2, npol=2, nchan=3, nrow=25, n=64, cell=60.0):

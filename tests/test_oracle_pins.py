@@ -7,7 +7,7 @@ from scipy import special as sp
 
 from oracle import muser_oracle as mo
 from oracle import oracle_c as oc
-from paper_1712_06913_b200 import synth
+from inputs import synth
 
 ARCSEC = np.pi / 648000.0
 C = 299792458.0

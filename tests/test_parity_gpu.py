@@ -6,7 +6,8 @@ import pytest
 
 from oracle import muser_oracle as mo
 from oracle import oracle_c as oc
-from paper_1712_06913_b200 import binding, synth
+from paper_1712_06913_b200 import binding
+from inputs import synth
 
 import gpu_util as gu
 
@@ -395,3 +396,43 @@ def test_images_on_fused_and_library_fft_paths(nx, ny):
         assert torch.equal(d, d2) and torch.equal(p, p2)
     finally:
         im.destroy()
+
+
+def test_owner_fixed_point_merge_bound_per_cell_with_a_1e6_outlier():
+    """The owner gridder merges register sums into a 32-bit fixed-point tile whose unit is 2^-31 / 0.98 of the work unit's
+    L1 bound B = max(sum |wt Re V|, sum |wt Im V|) (sum wt for the weight grid).  Guarantee: every merge rounds to the
+    nearest unit, so a cell that received m merges is off by at most m * 2^-32 * B / 0.98, plus the fp32 rounding of
+    the register sums (a few 1e-7 of the cell's own magnitude).  One visibility 1e6 times brighter than 300 unit ones
+    in the same tile: the global rel-L2 is trivially fine, the per-cell bound is what is checked -- and it shows the
+    dynamic-range limit: cells 1e6 times fainter than the tile's bound keep ~3 significant digits."""
+    n, cell, Q = 256, 20.0, 32
+    rng = np.random.default_rng(77)
+    nvis = 301
+    fov = n * cell * mo.ARCSEC
+    # all samples inside the tile x in [96, 160), y in [128, 160) (cells relative to the centre (128, 128): u in [-28, 28), v in [4, 28))
+    cu = rng.uniform(-26.0, 26.0, nvis); cv = rng.uniform(6.0, 26.0, nvis)
+    cu[0], cv[0] = 20.3, 20.4                                 # the outlier
+    far = np.hypot(cu - cu[0], cv - cv[0]) > 9.0              # unit samples whose footprint does not overlap the outlier's
+    far[0] = True
+    cu, cv = cu[far], cv[far]
+    nvis = cu.size
+    freq = np.full(nvis, 1.0e9)
+    uvw = np.zeros((nvis, 3), np.float32)
+    uvw[:, 0] = (cu / fov * mo.C_M_S / 1.0e9).astype(np.float32)
+    uvw[:, 1] = (cv / fov * mo.C_M_S / 1.0e9).astype(np.float32)
+    vis = (rng.standard_normal(nvis) + 1j * rng.standard_normal(nvis)).astype(np.complex64)
+    vis[0] = 1.0e6 * (0.6 + 0.8j)
+    wt = np.ones(nvis, np.float32)
+    res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, Q, strategy=OWNER, images=False)
+    G, G_or = res["G"][0], res["G_or"][0]
+    up = slice(n // 2, n)                                     # the tile sits in the stored half-plane; the rest is its mirror
+    B = max(np.abs(vis.real).sum(), np.abs(vis.imag).sum())
+    unit = B / (0.98 * 2.0 ** 31)
+    m_max = 2 * nvis                                          # at most one merge per record
+    err = np.abs(G[up] - G_or[up])
+    bound = m_max * 0.5 * unit * np.sqrt(2.0) + 2e-6 * np.abs(G_or[up])
+    assert (err <= bound).all(), f"worst excess {np.max(err - bound):.3e}"
+    # away from the outlier the cells are O(1): the absolute error there really is of the order of the unit, not of 1e-7
+    faint = (np.abs(G_or[up]) > 0.05) & (np.abs(G_or[up]) < 50.0)
+    assert faint.sum() > 500 and err[faint].max() <= m_max * 0.5 * unit * np.sqrt(2.0)
+    assert err[faint].max() < 20 * unit                       # in practice a handful of merges per cell
