@@ -82,9 +82,9 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
 int muser_set_strategy(muser_imager* h, int strategy);
 /* Tuning knobs of the OWNER strategy (results do not depend on them beyond fp32 summation order).  ITEM_SIZE: records
  * per chunk of a heavy tile (a tile with more records is split into chunks gridded by different CTAs and summed);
- * 0 (default) = chosen from the size of the call.  BIN_VPT: visibilities per thread of the binning kernels (1, 2, 4;
- * 0 = automatic). */
-enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_BIN_VPT = 1, MUSER_TUNE_COUNT = 2 };
+ * 0 (default) = chosen from the size of the call.  BIN_ITERS: blocks of 256 visibilities a binning CTA loops over
+ * (1..64; 0 = automatic). */
+enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_BIN_ITERS = 1, MUSER_TUNE_COUNT = 2 };
 int muser_set_tuning(muser_imager* h, int key, int value);
 /* 1 (default): A6 divides by the kernel's transform; 0: A6 only shifts/takes the real part (parity gate R9(i)). */
 int muser_set_grid_correction(muser_imager* h, int enabled);
@@ -137,7 +137,7 @@ int muser_grid_batched(muser_imager* h, const float* uvw_m, const double* freq_h
  *                                                          per-polarisation images)
  *                  NULL: everything onto grid 0
  * The result is that of muser_grid(_batched) on the flattened arrays (the order of the fp32 sums differs); flags, drops
- * and counters are per visibility as there.  nchan <= 512, npol <= 8.  Owner-tile strategy only (2-D mode, support 7),
+ * and counters are per visibility as there.  npol <= 8.  Owner-tile strategy only (2-D mode, support 7),
  * else MUSER_EUNSUPPORTED. */
 enum { MUSER_POLS_SUM = 0, MUSER_POLS_SPLIT = 1 };
 int muser_grid_rows(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64, const float* weight,

@@ -63,6 +63,8 @@ struct muser_imager {
     uint4 *ow_sorted = nullptr, *ow_loc = nullptr;          // tile-sorted records; per-visibility integer result of O1
     uint32_t *ow_count = nullptr, *ow_cursor = nullptr, *ow_offset = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
     uint4* ow_work = nullptr;
+    uint32_t* ow_cta_hist = nullptr;        // per binning CTA: its shared tile histogram (k_owner_count -> k_owner_scatter)
+    size_t ow_cta_hist_cap = 0;
     bool weights_only = false;              // the 2x-beam child: muser_grid is called without visibilities
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
     bool lower_valid = true;                // rows 0 .. ny/2-1 of G, Gw are up to date (the owner gridder stores rows >= ny/2 only)
@@ -131,7 +133,9 @@ void free_bins(muser_imager* h) {
     cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
     h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
     cudaFree(h->ow_count); cudaFree(h->ow_cursor); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
+    cudaFree(h->ow_cta_hist);
     h->ow_count = h->ow_cursor = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
+    h->ow_cta_hist = nullptr; h->ow_cta_hist_cap = 0;
 }
 
 int rebuild_geom(muser_imager* h) {
@@ -382,17 +386,26 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         uint32_t max_items = 0;
         int rc = ensure_owner_scratch(h, nvis, item_size, &max_items, s);
         if (rc) return rc;
+        const int iters = owner_bin_iters(nvis, h->tune[MUSER_TUNE_BIN_ITERS]);
+        {
+            const size_t need = owner_bin_ctas(nvis, iters) * (size_t)g.ontiles;
+            if (need > h->ow_cta_hist_cap) {
+                cudaFree(h->ow_cta_hist); h->ow_cta_hist = nullptr; h->ow_cta_hist_cap = 0;
+                CU(h, cudaMalloc(&h->ow_cta_hist, (need + need / 4) * sizeof(uint32_t)));
+                h->ow_cta_hist_cap = need + need / 4;
+            }
+        }
         if (g.oty > 65535 || g.otx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
         h->last_stream = s;
         h->fft_valid = false;
         {
             StageScope sc(h, MUSER_STAGE_BIN, s);
-            CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->stats_d, h->ow_loc,
-                                     h->tune[MUSER_TUNE_BIN_VPT], s));
+            CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->ow_cta_hist, h->stats_d,
+                                     h->ow_loc, iters, s));
             CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size,
                                     h->ow_work, h->ow_ctl, h->ow_tops, s));
-            CU(h, launch_owner_scatter(g, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_cursor,
-                                       h->ow_sorted, h->cnt, h->tune[MUSER_TUNE_BIN_VPT], s));
+            CU(h, launch_owner_scatter(g, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_cta_hist,
+                                       h->ow_cursor, h->ow_sorted, h->cnt, iters, s));
         }
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
@@ -433,7 +446,8 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
 int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const void* vis, const float* wt, const int* gid,
                    long long nrow, int nchan, int npol, int ntime, int pol_mode, cudaStream_t s) {
     if (nrow < 0 || nchan < 1 || npol < 1 || ntime < 1 || nchan > rows_max_channels() || npol > 8)
-        return fail(h, MUSER_EINVAL, "rows call: need nrow >= 0, 1 <= nchan <= 512, 1 <= npol <= 8, ntime >= 1");
+        return fail(h, MUSER_EINVAL, "rows call: need nrow >= 0, 1 <= nchan <= 65535, 1 <= npol <= 8, ntime >= 1");
+    if ((long long)ntime * npol * nchan > 32768LL * 65535LL) return fail(h, MUSER_EINVAL, "rows call: too many (time, pol, channel) blocks");
     if (pol_mode != MUSER_POLS_SUM && pol_mode != MUSER_POLS_SPLIT) return fail(h, MUSER_EINVAL, "unknown pol_mode");
     const long long nvis = nrow * nchan * npol * ntime;
     if (nrow > (1LL << 30) || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "too many visibilities in one call (2^30)");
@@ -751,7 +765,7 @@ int muser_set_tuning(muser_imager* h, int key, int value) {
     if (!h) return MUSER_EINVAL;
     if (key < 0 || key >= MUSER_TUNE_COUNT) return fail(h, MUSER_EINVAL, "unknown tuning key");
     if (key == MUSER_TUNE_ITEM_SIZE && value != 0 && (value < 256 || value > (1 << 20))) return fail(h, MUSER_EINVAL, "item_size must be 0 (automatic) or in [256, 2^20]");
-    if (key == MUSER_TUNE_BIN_VPT && value != 0 && value != 1 && value != 2 && value != 4) return fail(h, MUSER_EINVAL, "bin_vpt must be 0, 1, 2 or 4");
+    if (key == MUSER_TUNE_BIN_ITERS && (value < 0 || value > 64)) return fail(h, MUSER_EINVAL, "bin_iters must be in [0, 64]");
     h->tune[key] = value;
     return rebuild_geom(h);
 }

@@ -125,15 +125,18 @@ constexpr int kOwTileFloats = kOwTileW * 32 * 3;   // one partial tile in the sc
 struct OwItem {                              // one chunk of a heavy tile (more than item_size samples)
     uint32_t bin, start, count, first_slot, nchunks, chunk;
 };
+int owner_bin_iters(long long nvis, int forced);
+size_t owner_bin_ctas(long long nvis, int iters);
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
-                               const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, uint4* loc,
-                               int vpt_forced, cudaStream_t s);
+                               const int* grid_id, long long nvis, uint32_t* bin_count, uint32_t* cta_hist, Stats* stats,
+                               uint4* loc, int iters, cudaStream_t s);
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* cursor, uint32_t* bin_offset, OwItem* items,
                               uint32_t* nitems, uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops,
                               cudaStream_t s);
 cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* uvw, const double* freq, const float2* vis,
                                  const float* wt, const int* grid_id, long long nvis, const uint32_t* bin_offset,
-                                 uint32_t* cursor, uint4* sorted, int* cnt, int vpt_forced, cudaStream_t s);
+                                 const uint32_t* cta_hist, uint32_t* cursor, uint4* sorted, int* cnt, int iters,
+                                 cudaStream_t s);
 // channelised entry point (NEXT-1): elements (t, po, c, r); pols_split = 0: the polarisations of an element are summed
 cudaError_t launch_rows_count(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const float* uvw,
                               const double* freq, const float2* vis, const float* wt, const int* grid_id, uint32_t* bin_count,

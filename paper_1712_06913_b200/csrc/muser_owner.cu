@@ -142,33 +142,35 @@ __device__ __forceinline__ uint32_t ow_tiles_packed(const Geom& g, int cu, int c
     return t.up ? ((uint32_t)t.t00 | (t.mx ? 1u << 29 : 0u) | (t.my ? 1u << 30 : 0u) | 1u << 31) : 0u;
 }
 
-// A CTA handles 256 * VPT consecutive visibilities (thread: k, k + 256, ...), so that the per-CTA work (histogram
-// zeroing and flush, statistics reduction) is shared by VPT visibilities per thread; VPT = 1 for small calls.
-template <int VPT>
-__global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const float* __restrict__ uvw,
+// A CTA handles kBinThreads * iters consecutive visibilities in a loop (thread: k, k + 256, ...): the per-CTA work --
+// histogram zeroing and flush, statistics reduction -- is shared by `iters` visibilities per thread at no cost in
+// registers.  Records of the CTA's reference grid (that of its first visibility; every record when the call has one grid)
+// are counted in the shared histogram, ONE global atomic per touched tile per CTA (MUSER's central tile takes a third of
+// all samples: per-sample global atomics would serialise on it); records of other grids, and every record when the
+// grid's tiles do not fit the shared histogram, take warp-aggregated global atomics straight away.  The CTA's shared
+// histogram is also saved (cta_hist) so that k_owner_scatter does not have to count again.
+__global__ void __launch_bounds__(kBinThreads, 4) k_owner_count(const Geom g, const float* __restrict__ uvw,
                                                              const double* __restrict__ freq, const float2* __restrict__ vis,
                                                              const float* __restrict__ weight, const int* __restrict__ grid_id,
-                                                             const long long nvis, uint32_t* __restrict__ bin_count,
+                                                             const long long nvis, const int iters,
+                                                             uint32_t* __restrict__ bin_count, uint32_t* __restrict__ cta_hist,
                                                              Stats* __restrict__ stats, uint4* __restrict__ loc) {
     extern __shared__ uint32_t s_hist[];
-    const long long base = (long long)blockIdx.x * (kBinThreads * VPT);
+    const long long base = (long long)blockIdx.x * kBinThreads * iters;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool fits = g.ontiles <= kBinSmemTiles;
     if (fits)
         for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
     const int ref = grid_id ? grid_id[base] : 0;                      // base < nvis by the launch geometry
-    uint32_t tp[VPT][2];
-    int gidv[VPT];
-    int kept = 0, dropped = 0, flagged = 0, same = 1;
+    __syncthreads();
+    int kept = 0, dropped = 0, flagged = 0;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0, f_cache = 0.0, il_cache = 0.0;
-#pragma unroll
-    for (int j = 0; j < VPT; ++j) {
-        const long long k = base + j * kBinThreads + threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+        const long long k = base + (long long)it * kBinThreads + threadIdx.x;
         OwLoc L;
         float2 V;
         ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V, f_cache, il_cache);
-        tp[j][0] = tp[j][1] = 0u;
-        gidv[j] = 0;
+        uint32_t tp[2] = {0u, 0u};
         if (k < nvis) {                                               // integer result of O1 for k_owner_scatter
             uint4 o = make_uint4(0u, 0u, (uint32_t)L.state << 30, 0u);
             if (L.state == 3) {
@@ -176,10 +178,8 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
                 o.y = (uint32_t)L.cu[1] | ((uint32_t)L.cv[1] << 16);
                 o.z |= (uint32_t)L.rx[0] | ((uint32_t)L.ry[0] << 9) | ((uint32_t)L.rx[1] << 18);
                 o.w = (uint32_t)L.ry[1];
-                tp[j][0] = ow_tiles_packed(g, L.cu[0], L.cv[0]);
-                tp[j][1] = ow_tiles_packed(g, L.cu[1], L.cv[1]);
-                gidv[j] = L.gid;
-                same &= (L.gid == ref);
+                tp[0] = ow_tiles_packed(g, L.cu[0], L.cv[0]);
+                tp[1] = ow_tiles_packed(g, L.cu[1], L.cv[1]);
                 ++kept;
                 wsum += 2.0 * (double)L.wt;
                 const double w2 = (double)L.wt * (double)L.wt;
@@ -190,15 +190,11 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
             flagged += L.state == 1;
             loc[k] = o;
         }
-    }
-    // one barrier: the histogram is zeroed, and the CTA agrees whether all its kept visibilities share one grid
-    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
-    if (ugrid >= 0) {
-#pragma unroll
-        for (int j = 0; j < VPT; ++j)
+        const bool local = fits && L.state == 3 && L.gid == ref;
+        if (local) {
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
-                const uint32_t t = tp[j][s];
+                const uint32_t t = tp[s];
                 if (!(t >> 31)) continue;
                 const uint32_t t00 = t & 0x1FFFFFFFu;
                 const bool mx = (t >> 29) & 1u, my = (t >> 30) & 1u;
@@ -207,26 +203,32 @@ __global__ void __launch_bounds__(kBinThreads) k_owner_count(const Geom g, const
                 if (my) atomicAdd(&s_hist[t00 + g.otx], 1u);
                 if (mx && my) atomicAdd(&s_hist[t00 + g.otx + 1], 1u);
             }
-        __syncthreads();
-        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
-        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
-            const uint32_t n = s_hist[i];
-            if (n) atomicAdd(&bin_count[gbase + i], n);
         }
-    } else {
-#pragma unroll
-        for (int j = 0; j < VPT; ++j)
+        if (__any_sync(kFull, L.state == 3 && !local)) {              // other grids / huge grids: global atomics now
 #pragma unroll
             for (int s = 0; s < 2; ++s)
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const uint32_t t = tp[j][s];
-                    const bool on = (t >> 31) && (!(q & 1) || ((t >> 29) & 1u)) && (!(q & 2) || ((t >> 30) & 1u));
-                    const uint32_t bin = on ? (uint32_t)gidv[j] * (uint32_t)g.ontiles + (t & 0x1FFFFFFFu) + (q & 1) +
+                    const uint32_t t = tp[s];
+                    const bool on = L.state == 3 && !local && (t >> 31) && (!(q & 1) || ((t >> 29) & 1u)) &&
+                                    (!(q & 2) || ((t >> 30) & 1u));
+                    const uint32_t bin = on ? (uint32_t)L.gid * (uint32_t)g.ontiles + (t & 0x1FFFFFFFu) + (q & 1) +
                                                   ((q & 2) ? (uint32_t)g.otx : 0u)
                                             : kNoBin;
                     if (__any_sync(kFull, on)) ow_agg_inc(bin_count, bin, lane);
                 }
+        }
+    }
+    __syncthreads();
+    if (fits) {
+        const bool ok = ref >= 0 && ref < g.ngrids;
+        const uint32_t gbase = ok ? (uint32_t)ref * (uint32_t)g.ontiles : 0u;
+        uint32_t* mine = cta_hist + (size_t)blockIdx.x * g.ontiles;
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
+            const uint32_t n = s_hist[i];
+            mine[i] = n;
+            if (n && ok) atomicAdd(&bin_count[gbase + i], n);
+        }
     }
     // block reduction of the counters, one atomic set per block
     __shared__ int s_cnt[3][8];
@@ -400,106 +402,87 @@ __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, i
     *dst = o;
 }
 
-template <int VPT>
-__global__ void __launch_bounds__(kBinThreads) k_owner_scatter(const Geom g, const uint4* __restrict__ loc,
+// Same CTA -> visibility mapping as k_owner_count.  The CTA's per-tile counts of its reference grid come from cta_hist:
+// it reserves a run in each touched tile (one global atomic per tile), then hands out the positions inside the runs with
+// the shared counters; records of other grids take warp-aggregated global cursors.
+__global__ void __launch_bounds__(kBinThreads, 5) k_owner_scatter(const Geom g, const uint4* __restrict__ loc,
                                                                const float* __restrict__ uvw, const double* __restrict__ freq,
                                                                const float2* __restrict__ vis,
                                                                const float* __restrict__ weight, const int* __restrict__ grid_id,
-                                                               const long long nvis, const uint32_t* __restrict__ bin_offset,
+                                                               const long long nvis, const int iters,
+                                                               const uint32_t* __restrict__ bin_offset,
+                                                               const uint32_t* __restrict__ cta_hist,
                                                                uint32_t* __restrict__ cursor, uint4* __restrict__ sorted,
                                                                int* __restrict__ cnt) {
     extern __shared__ uint32_t s_hist[];
-    const long long base = (long long)blockIdx.x * (kBinThreads * VPT);
+    const long long base = (long long)blockIdx.x * kBinThreads * iters;
     const int lane = threadIdx.x & 31;
     const bool fits = g.ontiles <= kBinSmemTiles;
-    if (fits)
-        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
     const int ref = grid_id ? grid_id[base] : 0;
-    OwLoc L[VPT];
-    int same = 1;
-#pragma unroll
-    for (int j = 0; j < VPT; ++j) {
-        const long long k = base + j * kBinThreads + threadIdx.x;
-        L[j].state = 0;
+    uint32_t* s_base = s_hist + g.ontiles;                             // global position of this CTA's run in each tile
+    if (fits) {
+        const bool ok = ref >= 0 && ref < g.ngrids;
+        const uint32_t gbase = ok ? (uint32_t)ref * (uint32_t)g.ontiles : 0u;
+        const uint32_t* mine = cta_hist + (size_t)blockIdx.x * g.ontiles;
+        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
+            const uint32_t n = mine[i];
+            s_hist[i] = 0;
+            if (n && ok) s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n);
+        }
+    }
+    __syncthreads();
+    for (int it = 0; it < iters; ++it) {
+        const long long k = base + (long long)it * kBinThreads + threadIdx.x;
+        OwLoc L;
+        L.state = 0;
         if (k < nvis) {                                               // k_owner_count's integer decisions
             const uint4 o = __ldg(loc + k);
-            L[j].state = (int)(o.z >> 30);
-            if (L[j].state == 3) {
-                L[j].cu[0] = (int)(o.x & 0xFFFFu); L[j].cv[0] = (int)(o.x >> 16);
-                L[j].cu[1] = (int)(o.y & 0xFFFFu); L[j].cv[1] = (int)(o.y >> 16);
-                L[j].rx[0] = (int)(o.z & 511u); L[j].ry[0] = (int)((o.z >> 9) & 511u); L[j].rx[1] = (int)((o.z >> 18) & 511u);
-                L[j].ry[1] = (int)(o.w & 511u);
+            L.state = (int)(o.z >> 30);
+            if (L.state == 3) {
+                L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
+                L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
+                L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
+                L.ry[1] = (int)(o.w & 511u);
                 float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
                 if (g.phase_on) V = phase_rotate(g, uvw[3 * k], uvw[3 * k + 1], freq[k], V);
                 const float wt = weight[k];
-                L[j].re = wt * V.x; L[j].im = wt * V.y; L[j].wt = wt; L[j].gid = grid_id ? grid_id[k] : 0;
-                same &= (L[j].gid == ref);
+                L.re = wt * V.x; L.im = wt * V.y; L.wt = wt; L.gid = grid_id ? grid_id[k] : 0;
                 if (cnt) {                                            // NEXT-2: one hit per sample at its nearest cell (stored half-plane)
 #pragma unroll
                     for (int s = 0; s < 2; ++s)
-                        if (L[j].cv[s] >= (g.ny >> 1))
-                            atomicAdd(cnt + ((size_t)L[j].gid * g.ny + L[j].cv[s]) * g.nx + L[j].cu[s], 1);
+                        if (L.cv[s] >= (g.ny >> 1))
+                            atomicAdd(cnt + ((size_t)L.gid * g.ny + L.cv[s]) * g.nx + L.cu[s], 1);
                 }
             }
         }
-    }
-    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
-    if (ugrid >= 0) {
-        // phase A: count this CTA's records per tile; reserve a run in each touched tile; phase B: the same shared
-        // counters, zeroed again, hand out the positions inside the runs (no per-record rank is kept in registers)
-        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
-        uint32_t* s_base = s_hist + g.ontiles;                         // global position of this CTA's run in each tile
-#pragma unroll
-        for (int j = 0; j < VPT; ++j) {
-            if (L[j].state != 3) continue;
+        const bool kept = L.state == 3;
+        const bool local = fits && kept && L.gid == ref;
+        if (local) {
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
-                const OwTiles t = ow_tiles(g, L[j].cu[s], L[j].cv[s]);
+                const OwTiles t = ow_tiles(g, L.cu[s], L.cv[s]);
                 if (!t.up) continue;
-                atomicAdd(&s_hist[t.t00], 1u);
-                if (t.mx) atomicAdd(&s_hist[t.t00 + 1], 1u);
-                if (t.my) atomicAdd(&s_hist[t.t00 + g.otx], 1u);
-                if (t.mx && t.my) atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u);
-            }
-        }
-        __syncthreads();
-        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
-            const uint32_t n = s_hist[i];
-            if (n) { s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n); s_hist[i] = 0; }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int j = 0; j < VPT; ++j) {
-            if (L[j].state != 3) continue;
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                const OwTiles t = ow_tiles(g, L[j].cu[s], L[j].cv[s]);
-                if (!t.up) continue;
-                ow_write_record(g, L[j], s, t.tx0, t.ty0, sorted + s_base[t.t00] + atomicAdd(&s_hist[t.t00], 1u));
-                if (t.mx) ow_write_record(g, L[j], s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + atomicAdd(&s_hist[t.t00 + 1], 1u));
+                ow_write_record(g, L, s, t.tx0, t.ty0, sorted + s_base[t.t00] + atomicAdd(&s_hist[t.t00], 1u));
+                if (t.mx) ow_write_record(g, L, s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + atomicAdd(&s_hist[t.t00 + 1], 1u));
                 if (t.my)
-                    ow_write_record(g, L[j], s, t.tx0, t.ty0 + 1,
+                    ow_write_record(g, L, s, t.tx0, t.ty0 + 1,
                                     sorted + s_base[t.t00 + g.otx] + atomicAdd(&s_hist[t.t00 + g.otx], 1u));
                 if (t.mx && t.my)
-                    ow_write_record(g, L[j], s, t.tx0 + 1, t.ty0 + 1,
+                    ow_write_record(g, L, s, t.tx0 + 1, t.ty0 + 1,
                                     sorted + s_base[t.t00 + g.otx + 1] + atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u));
             }
         }
-        return;
-    }
+        if (__any_sync(kFull, kept && !local)) {
 #pragma unroll
-    for (int j = 0; j < VPT; ++j) {
-        const int kept = L[j].state == 3;
-        if (!__any_sync(kFull, kept)) continue;
+            for (int s = 0; s < 2; ++s) {
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                int tx = 0, ty = 0;
-                const uint32_t bin = kept ? ow_bin(g, L[j].gid, L[j].cu[s], L[j].cv[s], q, tx, ty) : kNoBin;
-                if (!__any_sync(kFull, bin != kNoBin)) continue;
-                const uint32_t rank = ow_agg_inc(cursor, bin, lane);
-                if (bin != kNoBin) ow_write_record(g, L[j], s, tx, ty, sorted + bin_offset[bin] + rank);
+                for (int q = 0; q < 4; ++q) {
+                    int tx = 0, ty = 0;
+                    const uint32_t bin = (kept && !local) ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
+                    if (!__any_sync(kFull, bin != kNoBin)) continue;
+                    const uint32_t rank = ow_agg_inc(cursor, bin, lane);
+                    if (bin != kNoBin) ow_write_record(g, L, s, tx, ty, sorted + bin_offset[bin] + rank);
+                }
             }
         }
     }
@@ -542,21 +525,24 @@ __device__ __forceinline__ RowsSum rows_sum_pols(const Geom& g, const RowsShape&
 }
 
 // element -> (t, po, c, r), coordinates and keep/drop of its two samples (same arithmetic as ow_locate)
+// A CTA handles 256 rows of ONE (t, po, c): blockIdx.y = (t * npo + po) * nchan + c (folded over gridDim.y, gridDim.z),
+// blockIdx.x = block of rows.  All its elements share the grid id and f/c.
 struct RowsElem { int t, po, c, r, gid; bool geom_ok, inside; float um, vm; double f; OwLoc L; };
+__device__ __forceinline__ void rows_block(const RowsShape& sh, int& t, int& po, int& c) {
+    const unsigned tpc = blockIdx.y + blockIdx.z * gridDim.y;
+    c = (int)(tpc % (unsigned)sh.nchan);
+    const unsigned tp = tpc / (unsigned)sh.nchan;
+    po = (int)(tp % (unsigned)sh.npo);
+    t = (int)(tp / (unsigned)sh.npo);
+}
 __device__ __forceinline__ void rows_locate(const Geom& g, const RowsShape& sh, const float* __restrict__ uvw,
-                                            const double* __restrict__ freq, const int* __restrict__ grid_id,
-                                            const double* s_il, const long long e, RowsElem& E) {
-    const long long per_c = sh.nrow, per_po = per_c * sh.nchan, per_t = per_po * sh.npo;
-    E.t = (int)(e / per_t);
-    long long rem = e - (long long)E.t * per_t;
-    E.po = (int)(rem / per_po); rem -= (long long)E.po * per_po;
-    E.c = (int)(rem / per_c);
-    E.r = (int)(rem - (long long)E.c * per_c);
+                                            const double f, const double il, const int gid, const int t, const int po,
+                                            const int c, const int r, RowsElem& E) {
+    E.t = t; E.po = po; E.c = c; E.r = r;
     const size_t ub = ((size_t)E.t * sh.nrow + E.r) * 3;
     const float um = uvw[ub], vm = uvw[ub + 1], wm = uvw[ub + 2];
-    E.um = um; E.vm = vm; E.f = freq[E.c];
-    E.gid = grid_id ? grid_id[((size_t)E.t * sh.npo + E.po) * sh.nchan + E.c] : 0;
-    const double il = s_il[E.c];
+    E.um = um; E.vm = vm; E.f = f;
+    E.gid = gid;
     const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
     E.geom_ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(E.f) && E.gid >= 0 && E.gid < g.ngrids;
     E.inside = false;
@@ -577,38 +563,34 @@ __device__ __forceinline__ void rows_locate(const Geom& g, const RowsShape& sh, 
     E.inside = inside;
 }
 
-// f / c of every channel, once per CTA (the flat path divides once per visibility)
-__device__ __forceinline__ void rows_channel_scale(const RowsShape& sh, const double* __restrict__ freq, double* s_il) {
-    for (int c = threadIdx.x; c < sh.nchan; c += kBinThreads) s_il[c] = __ddiv_rn(freq[c], kC);
-}
-
-constexpr int kRowsMaxChan = 512;
+constexpr int kRowsMaxChan = 65535;
 
 __global__ void __launch_bounds__(kBinThreads) k_rows_count(const Geom g, const RowsShape sh, const float* __restrict__ uvw,
                                                             const double* __restrict__ freq, const float2* __restrict__ vis,
                                                             const float* __restrict__ weight, const int* __restrict__ grid_id,
-                                                            const long long nelem, uint32_t* __restrict__ bin_count,
+                                                            uint32_t* __restrict__ bin_count,
                                                             Stats* __restrict__ stats, uint4* __restrict__ loc) {
     extern __shared__ uint32_t s_hist[];
-    __shared__ double s_il[kRowsMaxChan];
-    const long long e = (long long)blockIdx.x * kBinThreads + threadIdx.x;
+    __shared__ double s_il;
+    int t, po, c;
+    rows_block(sh, t, po, c);
+    if (t >= sh.ntime) return;                                        // padding of the folded launch grid (whole CTA)
+    const int r = blockIdx.x * kBinThreads + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool fits = g.ontiles <= kBinSmemTiles;
     if (fits)
         for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
-    rows_channel_scale(sh, freq, s_il);
+    const double f = freq[c];
+    if (threadIdx.x == 0) s_il = __ddiv_rn(f, kC);                    // f / c once per CTA (the flat path: per visibility)
+    const int ref = grid_id ? grid_id[((size_t)t * sh.npo + po) * sh.nchan + c] : 0;
     __syncthreads();
     uint32_t tp[2] = {0u, 0u};
-    int kept = 0, dropped = 0, flagged = 0, same = 1, gid = 0, ref = 0;
+    int kept = 0, dropped = 0, flagged = 0;
+    const int gid = ref;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
-    {   // the reference grid of the CTA: that of its first element
-        RowsElem E0;
-        rows_locate(g, sh, uvw, freq, grid_id, s_il, (long long)blockIdx.x * kBinThreads, E0);
-        ref = E0.gid;
-    }
-    if (e < nelem) {
+    if (r < sh.nrow) {
         RowsElem E;
-        rows_locate(g, sh, uvw, freq, grid_id, s_il, e, E);
+        rows_locate(g, sh, uvw, f, s_il, ref, t, po, c, r, E);
         const RowsSum S = rows_sum_pols(g, sh, vis, weight, E.t, E.po, E.c, E.r, E.geom_ok, E.inside, E.um, E.vm, E.f);
         kept = S.kept; flagged = S.flagged; dropped = sh.npi - S.kept - S.flagged;
         wsum = S.wsum; v2sum = S.v2sum; w2sum = S.w2sum;
@@ -620,12 +602,10 @@ __global__ void __launch_bounds__(kBinThreads) k_rows_count(const Geom g, const 
             o.w = (uint32_t)E.L.ry[1];
             tp[0] = ow_tiles_packed(g, E.L.cu[0], E.L.cv[0]);
             tp[1] = ow_tiles_packed(g, E.L.cu[1], E.L.cv[1]);
-            gid = E.gid;
-            same = gid == ref;
         }
-        loc[e] = o;
+        loc[(((size_t)t * sh.npo + po) * sh.nchan + c) * sh.nrow + r] = o;
     }
-    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
+    const int ugrid = (fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
     if (ugrid >= 0) {
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
@@ -688,44 +668,34 @@ __global__ void __launch_bounds__(kBinThreads) k_rows_count(const Geom g, const 
 __global__ void __launch_bounds__(kBinThreads) k_rows_scatter(const Geom g, const RowsShape sh, const uint4* __restrict__ loc,
                                                               const float* __restrict__ uvw, const double* __restrict__ freq,
                                                               const float2* __restrict__ vis, const float* __restrict__ weight,
-                                                              const int* __restrict__ grid_id, const long long nelem,
+                                                              const int* __restrict__ grid_id,
                                                               const uint32_t* __restrict__ bin_offset,
                                                               uint32_t* __restrict__ cursor, uint4* __restrict__ sorted,
                                                               int* __restrict__ cnt) {
     extern __shared__ uint32_t s_hist[];
-    const long long e = (long long)blockIdx.x * kBinThreads + threadIdx.x;
+    int t, po, c;
+    rows_block(sh, t, po, c);
+    if (t >= sh.ntime) return;
+    const int r = blockIdx.x * kBinThreads + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const bool fits = g.ontiles <= kBinSmemTiles;
     if (fits)
         for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
-    const long long per_c = sh.nrow, per_po = per_c * sh.nchan, per_t = per_po * sh.npo;
-    auto gid_of = [&](long long ee, int& t, int& po, int& c, int& r) -> int {
-        t = (int)(ee / per_t);
-        long long rem = ee - (long long)t * per_t;
-        po = (int)(rem / per_po); rem -= (long long)po * per_po;
-        c = (int)(rem / per_c);
-        r = (int)(rem - (long long)c * per_c);
-        return grid_id ? grid_id[((size_t)t * sh.npo + po) * sh.nchan + c] : 0;
-    };
-    int t0_, po0_, c0_, r0_;
-    const int ref = gid_of((long long)blockIdx.x * kBinThreads, t0_, po0_, c0_, r0_);
+    const int ref = grid_id ? grid_id[((size_t)t * sh.npo + po) * sh.nchan + c] : 0;
     OwLoc L;
     L.state = 0;
-    int same = 1;
-    if (e < nelem) {
-        const uint4 o = __ldg(loc + e);
+    if (r < sh.nrow) {
+        const uint4 o = __ldg(loc + (((size_t)t * sh.npo + po) * sh.nchan + c) * sh.nrow + r);
         L.state = (int)(o.z >> 30);
         if (L.state == 3) {
             L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
             L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
             L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
             L.ry[1] = (int)(o.w & 511u);
-            int t, po, c, r;
-            L.gid = gid_of(e, t, po, c, r);
+            L.gid = ref;
             const size_t ub = ((size_t)t * sh.nrow + r) * 3;
             const RowsSum S = rows_sum_pols(g, sh, vis, weight, t, po, c, r, true, true, uvw[ub], uvw[ub + 1], freq[c]);
             L.re = S.re; L.im = S.im; L.wt = S.wt;
-            same = L.gid == ref;
             if (cnt) {                                                // NEXT-2: one hit per visibility and sample
 #pragma unroll
                 for (int s = 0; s < 2; ++s)
@@ -733,8 +703,9 @@ __global__ void __launch_bounds__(kBinThreads) k_rows_scatter(const Geom g, cons
             }
         }
     }
+    __syncthreads();                                                  // the histogram is zeroed
     const int kept = L.state == 3;
-    const int ugrid = (__syncthreads_and(same) && fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
+    const int ugrid = (fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
     if (ugrid >= 0) {
         const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
         uint32_t* s_base = s_hist + g.ontiles;
@@ -1219,36 +1190,45 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
 // ------------------------------------------------------------------------------------------------- launchers
 static size_t bin_smem_bytes(const Geom& g) { return g.ontiles <= kBinSmemTiles ? (size_t)2 * g.ontiles * sizeof(uint32_t) : 0; }
 
-// visibilities per thread of the binning kernels (MUSER_TUNE_BIN_VPT)
-static int bin_vpt(long long nvis, int forced) {
-    (void)nvis;
-    // measured on B200 (cfg 3, 4.5 M visibilities per call): 1 -> 2.26, 2 -> 2.50, 4 -> 2.58 us per frame for the whole
-    // binning stage: the kernels are issue-bound and the extra registers of several visibilities per thread cost
-    // more occupancy than the shared per-CTA work saves
-    return (forced == 2 || forced == 4) ? forced : 1;
+// visibilities per thread of the binning kernels (MUSER_TUNE_BIN_ITERS): a CTA loops over `iters` blocks of 256
+int owner_bin_iters(long long nvis, int forced) {
+    if (forced >= 1 && forced <= 64) return forced;
+    // enough CTAs to fill the machine a few times over, else one block per CTA (a single small frame)
+    int it = 8;
+    while (it > 1 && nvis / (kBinThreads * it) < 148 * 8) it >>= 1;
+    return it;
 }
+size_t owner_bin_ctas(long long nvis, int iters) { return (size_t)((nvis + (long long)kBinThreads * iters - 1) / ((long long)kBinThreads * iters)); }
 
 cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
-                               const int* grid_id, long long nvis, uint32_t* bin_count, Stats* stats, uint4* loc,
-                               int vpt_forced, cudaStream_t s) {
-    const int vpt = bin_vpt(nvis, vpt_forced);
-    const unsigned blocks = (unsigned)((nvis + kBinThreads * vpt - 1) / (kBinThreads * vpt));
-    if (vpt == 4)
-        k_owner_count<4><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
-    else if (vpt == 2)
-        k_owner_count<2><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
-    else
-        k_owner_count<1><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, uvw, freq, vis, wt, grid_id, nvis, bin_count, stats, loc);
+                               const int* grid_id, long long nvis, uint32_t* bin_count, uint32_t* cta_hist, Stats* stats,
+                               uint4* loc, int iters, cudaStream_t s) {
+    k_owner_count<<<(unsigned)owner_bin_ctas(nvis, iters), kBinThreads, bin_smem_bytes(g), s>>>(
+        g, uvw, freq, vis, wt, grid_id, nvis, iters, bin_count, cta_hist, stats, loc);
     return cudaGetLastError();
+}
+
+cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* uvw, const double* freq, const float2* vis,
+                                 const float* wt, const int* grid_id, long long nvis, const uint32_t* bin_offset,
+                                 const uint32_t* cta_hist, uint32_t* cursor, uint4* sorted, int* cnt, int iters,
+                                 cudaStream_t s) {
+    k_owner_scatter<<<(unsigned)owner_bin_ctas(nvis, iters), kBinThreads, bin_smem_bytes(g), s>>>(
+        g, loc, uvw, freq, vis, wt, grid_id, nvis, iters, bin_offset, cta_hist, cursor, sorted, cnt);
+    return cudaGetLastError();
+}
+
+static dim3 rows_grid(const RowsShape& sh) {
+    // x: blocks of 256 rows; (t, po, c) folded over y (<= 32768) and z
+    const unsigned tpc = (unsigned)sh.ntime * (unsigned)sh.npo * (unsigned)sh.nchan;
+    const unsigned gy = tpc < 32768u ? tpc : 32768u;
+    return dim3((unsigned)((sh.nrow + kBinThreads - 1) / kBinThreads), gy, (tpc + gy - 1) / gy);
 }
 
 cudaError_t launch_rows_count(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const float* uvw,
                               const double* freq, const float2* vis, const float* wt, const int* grid_id, uint32_t* bin_count,
                               Stats* stats, uint4* loc, cudaStream_t s) {
     const RowsShape sh = {ntime, pols_split ? npol : 1, pols_split ? 1 : npol, nchan, nrow};
-    const long long nelem = (long long)ntime * sh.npo * nchan * nrow;
-    const unsigned blocks = (unsigned)((nelem + kBinThreads - 1) / kBinThreads);
-    k_rows_count<<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, sh, uvw, freq, vis, wt, grid_id, nelem, bin_count, stats, loc);
+    k_rows_count<<<rows_grid(sh), kBinThreads, bin_smem_bytes(g), s>>>(g, sh, uvw, freq, vis, wt, grid_id, bin_count, stats, loc);
     return cudaGetLastError();
 }
 
@@ -1256,10 +1236,8 @@ cudaError_t launch_rows_scatter(const Geom& g, int ntime, int npol, int nchan, i
                                 const float* uvw, const double* freq, const float2* vis, const float* wt, const int* grid_id,
                                 const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted, int* cnt, cudaStream_t s) {
     const RowsShape sh = {ntime, pols_split ? npol : 1, pols_split ? 1 : npol, nchan, nrow};
-    const long long nelem = (long long)ntime * sh.npo * nchan * nrow;
-    const unsigned blocks = (unsigned)((nelem + kBinThreads - 1) / kBinThreads);
-    k_rows_scatter<<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, sh, loc, uvw, freq, vis, wt, grid_id, nelem, bin_offset, cursor,
-                                                                  sorted, cnt);
+    k_rows_scatter<<<rows_grid(sh), kBinThreads, bin_smem_bytes(g), s>>>(g, sh, loc, uvw, freq, vis, wt, grid_id, bin_offset, cursor,
+                                                                        sorted, cnt);
     return cudaGetLastError();
 }
 
@@ -1276,20 +1254,6 @@ cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* curs
     k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
     k_owner_scan_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems, ctl);
     k_owner_scan_write<0><<<nblocks, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* uvw, const double* freq, const float2* vis,
-                                 const float* wt, const int* grid_id, long long nvis, const uint32_t* bin_offset,
-                                 uint32_t* cursor, uint4* sorted, int* cnt, int vpt_forced, cudaStream_t s) {
-    const int vpt = bin_vpt(nvis, vpt_forced);
-    const unsigned blocks = (unsigned)((nvis + kBinThreads * vpt - 1) / (kBinThreads * vpt));
-    if (vpt == 4)
-        k_owner_scatter<4><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted, cnt);
-    else if (vpt == 2)
-        k_owner_scatter<2><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted, cnt);
-    else
-        k_owner_scatter<1><<<blocks, kBinThreads, bin_smem_bytes(g), s>>>(g, loc, uvw, freq, vis, wt, grid_id, nvis, bin_offset, cursor, sorted, cnt);
     return cudaGetLastError();
 }
 
