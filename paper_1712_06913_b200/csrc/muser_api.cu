@@ -463,16 +463,25 @@ int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const 
     int rc = ensure_owner_scratch(h, nelem, item_size, &max_items, s);
     if (rc) return rc;
     if (g.oty > 65535 || g.otx > 1024 + 8) return fail(h, MUSER_EUNSUPPORTED, "too many tiles per axis");
+    const int cpc = rows_cpc(ntime, split ? npol : 1, nchan, (int)nrow);
+    {
+        const size_t need = rows_ctas(ntime, npol, nchan, (int)nrow, split, cpc) * (size_t)g.ontiles;
+        if (need > h->ow_cta_hist_cap) {
+            cudaFree(h->ow_cta_hist); h->ow_cta_hist = nullptr; h->ow_cta_hist_cap = 0;
+            CU(h, cudaMalloc(&h->ow_cta_hist, (need + need / 4) * sizeof(uint32_t)));
+            h->ow_cta_hist_cap = need + need / 4;
+        }
+    }
     h->last_stream = s;
     h->fft_valid = false;
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
-        CU(h, launch_rows_count(g, ntime, npol, nchan, (int)nrow, split, uvw, freq, (const float2*)vis, wt, gid, h->ow_count,
-                                h->stats_d, h->ow_loc, s));
+        CU(h, launch_rows_count(g, ntime, npol, nchan, (int)nrow, split, cpc, uvw, freq, (const float2*)vis, wt, gid, h->ow_count,
+                                h->ow_cta_hist, h->stats_d, h->ow_loc, s));
         CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size, h->ow_work,
                                 h->ow_ctl, h->ow_tops, s));
-        CU(h, launch_rows_scatter(g, ntime, npol, nchan, (int)nrow, split, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid,
-                                  h->ow_offset, h->ow_cursor, h->ow_sorted, h->cnt, s));
+        CU(h, launch_rows_scatter(g, ntime, npol, nchan, (int)nrow, split, cpc, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid,
+                                  h->ow_offset, h->ow_cta_hist, h->ow_cursor, h->ow_sorted, h->cnt, s));
     }
     {
         StageScope sc(h, MUSER_STAGE_GRID, s);

@@ -138,12 +138,15 @@ cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* u
                                  const uint32_t* cta_hist, uint32_t* cursor, uint4* sorted, int* cnt, int iters,
                                  cudaStream_t s);
 // channelised entry point (NEXT-1): elements (t, po, c, r); pols_split = 0: the polarisations of an element are summed
-cudaError_t launch_rows_count(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const float* uvw,
+int rows_cpc(int ntime, int npo, int nchan, int nrow);
+size_t rows_ctas(int ntime, int npol, int nchan, int nrow, int pols_split, int cpc);
+cudaError_t launch_rows_count(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, int cpc, const float* uvw,
                               const double* freq, const float2* vis, const float* wt, const int* grid_id, uint32_t* bin_count,
-                              Stats* stats, uint4* loc, cudaStream_t s);
-cudaError_t launch_rows_scatter(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const uint4* loc,
-                                const float* uvw, const double* freq, const float2* vis, const float* wt, const int* grid_id,
-                                const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted, int* cnt, cudaStream_t s);
+                              uint32_t* cta_hist, Stats* stats, uint4* loc, cudaStream_t s);
+cudaError_t launch_rows_scatter(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, int cpc,
+                                const uint4* loc, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                                const int* grid_id, const uint32_t* bin_offset, const uint32_t* cta_hist, uint32_t* cursor,
+                                uint4* sorted, int* cnt, cudaStream_t s);
 int rows_max_channels();
 cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,

@@ -525,16 +525,19 @@ __device__ __forceinline__ RowsSum rows_sum_pols(const Geom& g, const RowsShape&
 }
 
 // element -> (t, po, c, r), coordinates and keep/drop of its two samples (same arithmetic as ow_locate)
-// A CTA handles 256 rows of ONE (t, po, c): blockIdx.y = (t * npo + po) * nchan + c (folded over gridDim.y, gridDim.z),
-// blockIdx.x = block of rows.  All its elements share the grid id and f/c.
+// A CTA handles 256 rows of ONE (t, po) and a GROUP of `cpc` consecutive channels, looping over them: blockIdx.y =
+// (t * npo + po) * ncg + channel group (folded over gridDim.y, gridDim.z), blockIdx.x = block of rows.  The per-CTA work
+// (histogram zeroing and flush, statistics reduction) is shared by the channels of the group.
 struct RowsElem { int t, po, c, r, gid; bool geom_ok, inside; float um, vm; double f; OwLoc L; };
-__device__ __forceinline__ void rows_block(const RowsShape& sh, int& t, int& po, int& c) {
+__device__ __forceinline__ void rows_block(const RowsShape& sh, const int cpc, int& t, int& po, int& c0) {
+    const unsigned ncg = (unsigned)((sh.nchan + cpc - 1) / cpc);
     const unsigned tpc = blockIdx.y + blockIdx.z * gridDim.y;
-    c = (int)(tpc % (unsigned)sh.nchan);
-    const unsigned tp = tpc / (unsigned)sh.nchan;
+    c0 = (int)(tpc % ncg) * cpc;
+    const unsigned tp = tpc / ncg;
     po = (int)(tp % (unsigned)sh.npo);
     t = (int)(tp / (unsigned)sh.npo);
 }
+__device__ __forceinline__ size_t rows_cta(void) { return blockIdx.x + (size_t)gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z); }
 __device__ __forceinline__ void rows_locate(const Geom& g, const RowsShape& sh, const float* __restrict__ uvw,
                                             const double f, const double il, const int gid, const int t, const int po,
                                             const int c, const int r, RowsElem& E) {
@@ -565,87 +568,99 @@ __device__ __forceinline__ void rows_locate(const Geom& g, const RowsShape& sh, 
 
 constexpr int kRowsMaxChan = 65535;
 
-__global__ void __launch_bounds__(kBinThreads) k_rows_count(const Geom g, const RowsShape sh, const float* __restrict__ uvw,
-                                                            const double* __restrict__ freq, const float2* __restrict__ vis,
-                                                            const float* __restrict__ weight, const int* __restrict__ grid_id,
-                                                            uint32_t* __restrict__ bin_count,
-                                                            Stats* __restrict__ stats, uint4* __restrict__ loc) {
+constexpr int kRowsMaxCpc = 32;                                       // channels a CTA loops over
+
+__global__ void __launch_bounds__(kBinThreads, 4) k_rows_count(const Geom g, const RowsShape sh, const int cpc,
+                                                               const float* __restrict__ uvw, const double* __restrict__ freq,
+                                                               const float2* __restrict__ vis, const float* __restrict__ weight,
+                                                               const int* __restrict__ grid_id, uint32_t* __restrict__ bin_count,
+                                                               uint32_t* __restrict__ cta_hist, Stats* __restrict__ stats,
+                                                               uint4* __restrict__ loc) {
     extern __shared__ uint32_t s_hist[];
-    __shared__ double s_il;
-    int t, po, c;
-    rows_block(sh, t, po, c);
+    __shared__ double s_il[kRowsMaxCpc];
+    int t, po, c0;
+    rows_block(sh, cpc, t, po, c0);
     if (t >= sh.ntime) return;                                        // padding of the folded launch grid (whole CTA)
     const int r = blockIdx.x * kBinThreads + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool fits = g.ontiles <= kBinSmemTiles;
     if (fits)
         for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
-    const double f = freq[c];
-    if (threadIdx.x == 0) s_il = __ddiv_rn(f, kC);                    // f / c once per CTA (the flat path: per visibility)
-    const int ref = grid_id ? grid_id[((size_t)t * sh.npo + po) * sh.nchan + c] : 0;
+    const int nc = min(cpc, sh.nchan - c0);
+    if (threadIdx.x < nc) s_il[threadIdx.x] = __ddiv_rn(freq[c0 + threadIdx.x], kC);   // f / c once per channel and CTA
+    const int* gids = grid_id ? grid_id + ((size_t)t * sh.npo + po) * sh.nchan : nullptr;
+    const int ref = gids ? gids[c0] : 0;
     __syncthreads();
-    uint32_t tp[2] = {0u, 0u};
     int kept = 0, dropped = 0, flagged = 0;
-    const int gid = ref;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
-    if (r < sh.nrow) {
-        RowsElem E;
-        rows_locate(g, sh, uvw, f, s_il, ref, t, po, c, r, E);
-        const RowsSum S = rows_sum_pols(g, sh, vis, weight, E.t, E.po, E.c, E.r, E.geom_ok, E.inside, E.um, E.vm, E.f);
-        kept = S.kept; flagged = S.flagged; dropped = sh.npi - S.kept - S.flagged;
-        wsum = S.wsum; v2sum = S.v2sum; w2sum = S.w2sum;
-        uint4 o = make_uint4(0u, 0u, (S.kept ? 3u : 0u) << 30, 0u);
-        if (S.kept) {
-            o.x = (uint32_t)E.L.cu[0] | ((uint32_t)E.L.cv[0] << 16);
-            o.y = (uint32_t)E.L.cu[1] | ((uint32_t)E.L.cv[1] << 16);
-            o.z |= (uint32_t)E.L.rx[0] | ((uint32_t)E.L.ry[0] << 9) | ((uint32_t)E.L.rx[1] << 18);
-            o.w = (uint32_t)E.L.ry[1];
-            tp[0] = ow_tiles_packed(g, E.L.cu[0], E.L.cv[0]);
-            tp[1] = ow_tiles_packed(g, E.L.cu[1], E.L.cv[1]);
+    for (int ci = 0; ci < nc; ++ci) {
+        const int c = c0 + ci;
+        const int gid = gids ? gids[c] : 0;
+        uint32_t tp[2] = {0u, 0u};
+        if (r < sh.nrow) {
+            RowsElem E;
+            rows_locate(g, sh, uvw, freq[c], s_il[ci], gid, t, po, c, r, E);
+            const RowsSum S = rows_sum_pols(g, sh, vis, weight, E.t, E.po, E.c, E.r, E.geom_ok, E.inside, E.um, E.vm, E.f);
+            kept += S.kept; flagged += S.flagged; dropped += sh.npi - S.kept - S.flagged;
+            wsum += S.wsum; v2sum += S.v2sum; w2sum += S.w2sum;
+            uint4 o = make_uint4(0u, 0u, (S.kept ? 3u : 0u) << 30, 0u);
+            if (S.kept) {
+                o.x = (uint32_t)E.L.cu[0] | ((uint32_t)E.L.cv[0] << 16);
+                o.y = (uint32_t)E.L.cu[1] | ((uint32_t)E.L.cv[1] << 16);
+                o.z |= (uint32_t)E.L.rx[0] | ((uint32_t)E.L.ry[0] << 9) | ((uint32_t)E.L.rx[1] << 18);
+                o.w = (uint32_t)E.L.ry[1];
+                tp[0] = ow_tiles_packed(g, E.L.cu[0], E.L.cv[0]);
+                tp[1] = ow_tiles_packed(g, E.L.cu[1], E.L.cv[1]);
+            }
+            loc[(((size_t)t * sh.npo + po) * sh.nchan + c) * sh.nrow + r] = o;
         }
-        loc[(((size_t)t * sh.npo + po) * sh.nchan + c) * sh.nrow + r] = o;
-    }
-    const int ugrid = (fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
-    if (ugrid >= 0) {
+        const bool local = fits && gid == ref;                        // uniform over the CTA
+        if (local) {
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            const uint32_t t = tp[s];
-            if (!(t >> 31)) continue;
-            const uint32_t t00 = t & 0x1FFFFFFFu;
-            const bool mx = (t >> 29) & 1u, my = (t >> 30) & 1u;
-            atomicAdd(&s_hist[t00], 1u);
-            if (mx) atomicAdd(&s_hist[t00 + 1], 1u);
-            if (my) atomicAdd(&s_hist[t00 + g.otx], 1u);
-            if (mx && my) atomicAdd(&s_hist[t00 + g.otx + 1], 1u);
+            for (int s = 0; s < 2; ++s) {
+                const uint32_t tt = tp[s];
+                if (!(tt >> 31)) continue;
+                const uint32_t t00 = tt & 0x1FFFFFFFu;
+                const bool mx = (tt >> 29) & 1u, my = (tt >> 30) & 1u;
+                atomicAdd(&s_hist[t00], 1u);
+                if (mx) atomicAdd(&s_hist[t00 + 1], 1u);
+                if (my) atomicAdd(&s_hist[t00 + g.otx], 1u);
+                if (mx && my) atomicAdd(&s_hist[t00 + g.otx + 1], 1u);
+            }
+        } else {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t tt = tp[s];
+                    const bool on = (tt >> 31) && (!(q & 1) || ((tt >> 29) & 1u)) && (!(q & 2) || ((tt >> 30) & 1u));
+                    const uint32_t bin = on ? (uint32_t)gid * (uint32_t)g.ontiles + (tt & 0x1FFFFFFFu) + (q & 1) +
+                                                  ((q & 2) ? (uint32_t)g.otx : 0u)
+                                            : kNoBin;
+                    if (__any_sync(kFull, on)) ow_agg_inc(bin_count, bin, lane);
+                }
         }
-        __syncthreads();
-        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
+    }
+    __syncthreads();
+    if (fits) {
+        const bool ok = ref >= 0 && ref < g.ngrids;
+        const uint32_t gbase = ok ? (uint32_t)ref * (uint32_t)g.ontiles : 0u;
+        uint32_t* mine = cta_hist + rows_cta() * g.ontiles;
         for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
             const uint32_t n = s_hist[i];
-            if (n) atomicAdd(&bin_count[gbase + i], n);
+            mine[i] = n;
+            if (n && ok) atomicAdd(&bin_count[gbase + i], n);
         }
-    } else {
-#pragma unroll
-        for (int s = 0; s < 2; ++s)
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const uint32_t t = tp[s];
-                const bool on = (t >> 31) && (!(q & 1) || ((t >> 29) & 1u)) && (!(q & 2) || ((t >> 30) & 1u));
-                const uint32_t bin = on ? (uint32_t)gid * (uint32_t)g.ontiles + (t & 0x1FFFFFFFu) + (q & 1) +
-                                              ((q & 2) ? (uint32_t)g.otx : 0u)
-                                        : kNoBin;
-                if (__any_sync(kFull, on)) ow_agg_inc(bin_count, bin, lane);
-            }
     }
     __shared__ int s_cnt[3][8];
     __shared__ double s_w[3][8];
-    const int c0 = __reduce_add_sync(kFull, kept), c1 = __reduce_add_sync(kFull, dropped), c2 = __reduce_add_sync(kFull, flagged);
+    const int q0 = __reduce_add_sync(kFull, kept), q1 = __reduce_add_sync(kFull, dropped), q2 = __reduce_add_sync(kFull, flagged);
     for (int o = 16; o > 0; o >>= 1) {
         wsum += __shfl_xor_sync(kFull, wsum, o);
         v2sum += __shfl_xor_sync(kFull, v2sum, o);
         w2sum += __shfl_xor_sync(kFull, w2sum, o);
     }
-    if (lane == 0) { s_cnt[0][warp] = c0; s_cnt[1][warp] = c1; s_cnt[2][warp] = c2; s_w[0][warp] = wsum; s_w[1][warp] = v2sum; s_w[2][warp] = w2sum; }
+    if (lane == 0) { s_cnt[0][warp] = q0; s_cnt[1][warp] = q1; s_cnt[2][warp] = q2; s_w[0][warp] = wsum; s_w[1][warp] = v2sum; s_w[2][warp] = w2sum; }
     __syncthreads();
     if (threadIdx.x == 0) {
         int t0 = 0, t1 = 0, t2 = 0;
@@ -665,95 +680,89 @@ __global__ void __launch_bounds__(kBinThreads) k_rows_count(const Geom g, const 
     }
 }
 
-__global__ void __launch_bounds__(kBinThreads) k_rows_scatter(const Geom g, const RowsShape sh, const uint4* __restrict__ loc,
-                                                              const float* __restrict__ uvw, const double* __restrict__ freq,
-                                                              const float2* __restrict__ vis, const float* __restrict__ weight,
-                                                              const int* __restrict__ grid_id,
-                                                              const uint32_t* __restrict__ bin_offset,
-                                                              uint32_t* __restrict__ cursor, uint4* __restrict__ sorted,
-                                                              int* __restrict__ cnt) {
+__global__ void __launch_bounds__(kBinThreads, 5) k_rows_scatter(const Geom g, const RowsShape sh, const int cpc,
+                                                                 const uint4* __restrict__ loc, const float* __restrict__ uvw,
+                                                                 const double* __restrict__ freq, const float2* __restrict__ vis,
+                                                                 const float* __restrict__ weight, const int* __restrict__ grid_id,
+                                                                 const uint32_t* __restrict__ bin_offset,
+                                                                 const uint32_t* __restrict__ cta_hist,
+                                                                 uint32_t* __restrict__ cursor, uint4* __restrict__ sorted,
+                                                                 int* __restrict__ cnt) {
     extern __shared__ uint32_t s_hist[];
-    int t, po, c;
-    rows_block(sh, t, po, c);
+    int t, po, c0;
+    rows_block(sh, cpc, t, po, c0);
     if (t >= sh.ntime) return;
     const int r = blockIdx.x * kBinThreads + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const bool fits = g.ontiles <= kBinSmemTiles;
-    if (fits)
-        for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) s_hist[i] = 0;
-    const int ref = grid_id ? grid_id[((size_t)t * sh.npo + po) * sh.nchan + c] : 0;
-    OwLoc L;
-    L.state = 0;
-    if (r < sh.nrow) {
-        const uint4 o = __ldg(loc + (((size_t)t * sh.npo + po) * sh.nchan + c) * sh.nrow + r);
-        L.state = (int)(o.z >> 30);
-        if (L.state == 3) {
-            L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
-            L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
-            L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
-            L.ry[1] = (int)(o.w & 511u);
-            L.gid = ref;
-            const size_t ub = ((size_t)t * sh.nrow + r) * 3;
-            const RowsSum S = rows_sum_pols(g, sh, vis, weight, t, po, c, r, true, true, uvw[ub], uvw[ub + 1], freq[c]);
-            L.re = S.re; L.im = S.im; L.wt = S.wt;
-            if (cnt) {                                                // NEXT-2: one hit per visibility and sample
-#pragma unroll
-                for (int s = 0; s < 2; ++s)
-                    if (L.cv[s] >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)L.gid * g.ny + L.cv[s]) * g.nx + L.cu[s], S.kept);
-            }
-        }
-    }
-    __syncthreads();                                                  // the histogram is zeroed
-    const int kept = L.state == 3;
-    const int ugrid = (fits && ref >= 0 && ref < g.ngrids) ? ref : -1;
-    if (ugrid >= 0) {
-        const uint32_t gbase = (uint32_t)ugrid * (uint32_t)g.ontiles;
-        uint32_t* s_base = s_hist + g.ontiles;
-        OwTiles T[2];
-        if (kept) {
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                T[s] = ow_tiles(g, L.cu[s], L.cv[s]);
-                if (!T[s].up) continue;
-                atomicAdd(&s_hist[T[s].t00], 1u);
-                if (T[s].mx) atomicAdd(&s_hist[T[s].t00 + 1], 1u);
-                if (T[s].my) atomicAdd(&s_hist[T[s].t00 + g.otx], 1u);
-                if (T[s].mx && T[s].my) atomicAdd(&s_hist[T[s].t00 + g.otx + 1], 1u);
-            }
-        }
-        __syncthreads();
+    const int nc = min(cpc, sh.nchan - c0);
+    const int* gids = grid_id ? grid_id + ((size_t)t * sh.npo + po) * sh.nchan : nullptr;
+    const int ref = gids ? gids[c0] : 0;
+    uint32_t* s_base = s_hist + g.ontiles;
+    if (fits) {
+        const bool ok = ref >= 0 && ref < g.ngrids;
+        const uint32_t gbase = ok ? (uint32_t)ref * (uint32_t)g.ontiles : 0u;
+        const uint32_t* mine = cta_hist + rows_cta() * g.ontiles;
         for (int i = threadIdx.x; i < g.ontiles; i += kBinThreads) {
-            const uint32_t n = s_hist[i];
-            if (n) { s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n); s_hist[i] = 0; }
+            const uint32_t n = mine[i];
+            s_hist[i] = 0;
+            if (n && ok) s_base[i] = bin_offset[gbase + i] + atomicAdd(&cursor[gbase + i], n);
         }
-        __syncthreads();
-        if (kept) {
+    }
+    __syncthreads();
+    for (int ci = 0; ci < nc; ++ci) {
+        const int c = c0 + ci;
+        const int gid = gids ? gids[c] : 0;
+        OwLoc L;
+        L.state = 0;
+        if (r < sh.nrow) {
+            const uint4 o = __ldg(loc + (((size_t)t * sh.npo + po) * sh.nchan + c) * sh.nrow + r);
+            L.state = (int)(o.z >> 30);
+            if (L.state == 3) {
+                L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
+                L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
+                L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
+                L.ry[1] = (int)(o.w & 511u);
+                L.gid = gid;
+                const size_t ub = ((size_t)t * sh.nrow + r) * 3;
+                const RowsSum S = rows_sum_pols(g, sh, vis, weight, t, po, c, r, true, true, uvw[ub], uvw[ub + 1], freq[c]);
+                L.re = S.re; L.im = S.im; L.wt = S.wt;
+                if (cnt) {                                            // NEXT-2: one hit per visibility and sample
 #pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                const OwTiles t = T[s];
-                if (!t.up) continue;
-                ow_write_record(g, L, s, t.tx0, t.ty0, sorted + s_base[t.t00] + atomicAdd(&s_hist[t.t00], 1u));
-                if (t.mx) ow_write_record(g, L, s, t.tx0 + 1, t.ty0, sorted + s_base[t.t00 + 1] + atomicAdd(&s_hist[t.t00 + 1], 1u));
-                if (t.my)
-                    ow_write_record(g, L, s, t.tx0, t.ty0 + 1,
-                                    sorted + s_base[t.t00 + g.otx] + atomicAdd(&s_hist[t.t00 + g.otx], 1u));
-                if (t.mx && t.my)
-                    ow_write_record(g, L, s, t.tx0 + 1, t.ty0 + 1,
-                                    sorted + s_base[t.t00 + g.otx + 1] + atomicAdd(&s_hist[t.t00 + g.otx + 1], 1u));
+                    for (int s = 0; s < 2; ++s)
+                        if (L.cv[s] >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)L.gid * g.ny + L.cv[s]) * g.nx + L.cu[s], S.kept);
+                }
             }
         }
-        return;
-    }
-    if (!__any_sync(kFull, kept)) return;
+        const bool kept = L.state == 3;
+        if (fits && gid == ref) {                                     // uniform over the CTA
+            if (kept) {
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
+                for (int s = 0; s < 2; ++s) {
+                    const OwTiles tt = ow_tiles(g, L.cu[s], L.cv[s]);
+                    if (!tt.up) continue;
+                    ow_write_record(g, L, s, tt.tx0, tt.ty0, sorted + s_base[tt.t00] + atomicAdd(&s_hist[tt.t00], 1u));
+                    if (tt.mx) ow_write_record(g, L, s, tt.tx0 + 1, tt.ty0, sorted + s_base[tt.t00 + 1] + atomicAdd(&s_hist[tt.t00 + 1], 1u));
+                    if (tt.my)
+                        ow_write_record(g, L, s, tt.tx0, tt.ty0 + 1,
+                                        sorted + s_base[tt.t00 + g.otx] + atomicAdd(&s_hist[tt.t00 + g.otx], 1u));
+                    if (tt.mx && tt.my)
+                        ow_write_record(g, L, s, tt.tx0 + 1, tt.ty0 + 1,
+                                        sorted + s_base[tt.t00 + g.otx + 1] + atomicAdd(&s_hist[tt.t00 + g.otx + 1], 1u));
+                }
+            }
+        } else if (__any_sync(kFull, kept)) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            int tx = 0, ty = 0;
-            const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
-            if (!__any_sync(kFull, bin != kNoBin)) continue;
-            const uint32_t rank = ow_agg_inc(cursor, bin, lane);
-            if (bin != kNoBin) ow_write_record(g, L, s, tx, ty, sorted + bin_offset[bin] + rank);
+            for (int s = 0; s < 2; ++s) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    int tx = 0, ty = 0;
+                    const uint32_t bin = kept ? ow_bin(g, L.gid, L.cu[s], L.cv[s], q, tx, ty) : kNoBin;
+                    if (!__any_sync(kFull, bin != kNoBin)) continue;
+                    const uint32_t rank = ow_agg_inc(cursor, bin, lane);
+                    if (bin != kNoBin) ow_write_record(g, L, s, tx, ty, sorted + bin_offset[bin] + rank);
+                }
+            }
         }
     }
 }
@@ -1217,27 +1226,41 @@ cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* u
     return cudaGetLastError();
 }
 
-static dim3 rows_grid(const RowsShape& sh) {
-    // x: blocks of 256 rows; (t, po, c) folded over y (<= 32768) and z
-    const unsigned tpc = (unsigned)sh.ntime * (unsigned)sh.npo * (unsigned)sh.nchan;
+// channels per CTA of the rows kernels: enough CTAs to fill the machine a few times over
+int rows_cpc(int ntime, int npo, int nchan, int nrow) {
+    int cpc = nchan < kRowsMaxCpc ? nchan : kRowsMaxCpc;
+    const long long rb = (nrow + kBinThreads - 1) / kBinThreads;
+    while (cpc > 1 && rb * ntime * npo * ((nchan + cpc - 1) / cpc) < 148LL * 8) cpc = (cpc + 1) / 2;
+    return cpc;
+}
+static dim3 rows_grid(const RowsShape& sh, int cpc) {
+    // x: blocks of 256 rows; (t, po, channel group) folded over y (<= 32768) and z
+    const unsigned tpc = (unsigned)sh.ntime * (unsigned)sh.npo * (unsigned)((sh.nchan + cpc - 1) / cpc);
     const unsigned gy = tpc < 32768u ? tpc : 32768u;
     return dim3((unsigned)((sh.nrow + kBinThreads - 1) / kBinThreads), gy, (tpc + gy - 1) / gy);
 }
-
-cudaError_t launch_rows_count(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const float* uvw,
-                              const double* freq, const float2* vis, const float* wt, const int* grid_id, uint32_t* bin_count,
-                              Stats* stats, uint4* loc, cudaStream_t s) {
+size_t rows_ctas(int ntime, int npol, int nchan, int nrow, int pols_split, int cpc) {
     const RowsShape sh = {ntime, pols_split ? npol : 1, pols_split ? 1 : npol, nchan, nrow};
-    k_rows_count<<<rows_grid(sh), kBinThreads, bin_smem_bytes(g), s>>>(g, sh, uvw, freq, vis, wt, grid_id, bin_count, stats, loc);
+    const dim3 d = rows_grid(sh, cpc);
+    return (size_t)d.x * d.y * d.z;
+}
+
+cudaError_t launch_rows_count(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, int cpc, const float* uvw,
+                              const double* freq, const float2* vis, const float* wt, const int* grid_id, uint32_t* bin_count,
+                              uint32_t* cta_hist, Stats* stats, uint4* loc, cudaStream_t s) {
+    const RowsShape sh = {ntime, pols_split ? npol : 1, pols_split ? 1 : npol, nchan, nrow};
+    k_rows_count<<<rows_grid(sh, cpc), kBinThreads, bin_smem_bytes(g), s>>>(g, sh, cpc, uvw, freq, vis, wt, grid_id, bin_count,
+                                                                           cta_hist, stats, loc);
     return cudaGetLastError();
 }
 
-cudaError_t launch_rows_scatter(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, const uint4* loc,
-                                const float* uvw, const double* freq, const float2* vis, const float* wt, const int* grid_id,
-                                const uint32_t* bin_offset, uint32_t* cursor, uint4* sorted, int* cnt, cudaStream_t s) {
+cudaError_t launch_rows_scatter(const Geom& g, int ntime, int npol, int nchan, int nrow, int pols_split, int cpc,
+                                const uint4* loc, const float* uvw, const double* freq, const float2* vis, const float* wt,
+                                const int* grid_id, const uint32_t* bin_offset, const uint32_t* cta_hist, uint32_t* cursor,
+                                uint4* sorted, int* cnt, cudaStream_t s) {
     const RowsShape sh = {ntime, pols_split ? npol : 1, pols_split ? 1 : npol, nchan, nrow};
-    k_rows_scatter<<<rows_grid(sh), kBinThreads, bin_smem_bytes(g), s>>>(g, sh, loc, uvw, freq, vis, wt, grid_id, bin_offset, cursor,
-                                                                        sorted, cnt);
+    k_rows_scatter<<<rows_grid(sh, cpc), kBinThreads, bin_smem_bytes(g), s>>>(g, sh, cpc, loc, uvw, freq, vis, wt, grid_id, bin_offset,
+                                                                             cta_hist, cursor, sorted, cnt);
     return cudaGetLastError();
 }
 
