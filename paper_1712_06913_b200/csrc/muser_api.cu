@@ -422,9 +422,9 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     int rc = ensure_scratch(h, nvis, s);
     if (rc) return rc;
     if ((rc = flush_zero(h, s))) return rc;
-    if ((rc = ensure_lower(h, s))) return rc;                         // the generic gridder adds to both half-planes
     h->last_stream = s;
     h->fft_valid = false;
+    h->lower_valid = false;                                           // like the owner path, it grids rows >= ny/2 only
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
         CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,

@@ -95,9 +95,13 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                     o.cell = (uint32_t)cu | ((uint32_t)cv << 16);
                     o.phase = (uint32_t)rx | ((uint32_t)ry << 9) | ((uint32_t)kconj << 18);
                     o.gp = (uint32_t)gid | ((uint32_t)p << 24);
-                    const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
-                    o.bin = (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
-                    if (cnt) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, 1);   // NEXT-2 (this strategy grids both half-planes)
+                    // the grids are Hermitian: only rows >= ny/2 are computed and stored ("half the grid"); a
+                    // sample whose footprint stays below them is not gridded (its partner covers the mirror cells)
+                    if (cv + h >= (g.ny >> 1)) {
+                        const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
+                        o.bin = (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
+                    }
+                    if (cnt && cv >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, 1);   // NEXT-2
                 }
             }
         }
@@ -235,18 +239,24 @@ __device__ __forceinline__ void decode_bin(const Geom& g, uint32_t bin, int& gi,
 }
 
 // Generic tiled gridder (any support, 2-D or w mode): one work item = <= chunk samples of one (grid, plane,
-// tile).  The CTA accumulates the tile plus its halo ((32+2h)^2 cells) in shared memory with one warp per
-// sample, then adds the touched cells to the grids with vector reductions.
+// tile).  The CTA accumulates the tile plus its halo ((32+2h)^2 cells) in shared memory, then adds the touched cells
+// to the grids with vector reductions.
+//   - the plane's kernel table is staged in shared memory per item (<= 16.6 KB at S = 31, Q = 64);
+//   - a sample is handled by S lanes, lane = footprint COLUMN jx, looping over the S rows: the row's ky * (wt V) and
+//     ky * wt are formed once per row (separable kernel), each lane then needs one complex multiply per grid;
+//     floor(32 / S) samples share a warp (4 at S = 7, 2 at S = 11..15, 1 above);
+//   - the region is accumulated in 32-bit FIXED POINT: integer shared-memory adds are native single instructions,
+//     fp32 adds are compare-and-swap loops.  Per item the scales map the largest possible cell sum (sum of
+//     |wt Re V| + |wt Im V| resp. wt over the item's samples, times the plane's bound on |kx ky|) to 0.98 * 2^31.
 template <int WMODE>
 __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const Sample* __restrict__ sorted,
                                                             const Item* __restrict__ items,
                                                             const uint32_t* __restrict__ nitems,
                                                             const PlaneMeta* __restrict__ planes,
-                                                            const float* __restrict__ tables, GridPtrs grids) {
-    // The region is accumulated in 32-bit FIXED POINT: integer shared-memory adds are native single instructions,
-    // fp32 adds are compare-and-swap loops.  Per item the scales map the largest possible cell sum (sum of
-    // |wt Re V| + |wt Im V| resp. wt over the item's samples, times the plane's bound on |kx ky|) to 0.98 * 2^31.
+                                                            const float* __restrict__ tables, GridPtrs grids,
+                                                            const int region_ints) {
     extern __shared__ __align__(16) int smem_i[];
+    float* s_tab = reinterpret_cast<float*>(smem_i + region_ints);  // TT[r][j] of the item's plane (floats, or float2 in w mode)
     __shared__ float s_sum[8][2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t n_items = *nitems;
@@ -256,10 +266,13 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
         decode_bin(g, item.bin, gi, p, ty, tx);
         const PlaneMeta pm = planes[p];
         const int S = pm.support, h = (S - 1) >> 1, R = kTile + 2 * h, RR = R * R;
-        const int q32 = 32 / S, r32 = 32 - q32 * S;                 // 32 = q32 * S + r32: how (jy, jx) advance per pass
-        const int jy0 = lane / S, jx0 = lane - jy0 * S;             // footprint cell of this lane in the first pass
         constexpr int NPL = WMODE ? 4 : 3;                          // planes: G.re G.im W(.re) [W.im]
         for (int i = threadIdx.x; i < NPL * RR; i += blockDim.x) smem_i[i] = 0;
+        {   // stage the plane's table
+            const int nfl = (g.Q + 1) * pm.pitch * (WMODE ? 2 : 1);
+            const float* src = tables + (size_t)pm.offset * (WMODE ? 2 : 1);
+            for (int i = threadIdx.x; i < nfl; i += blockDim.x) s_tab[i] = __ldg(src + i);
+        }
         float mv = 0.f, mw = 0.f;
         for (uint32_t i = threadIdx.x; i < item.count; i += blockDim.x) {
             const uint4 a = __ldg(reinterpret_cast<const uint4*>(sorted + item.start + i));
@@ -273,29 +286,44 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
         for (int w = 0; w < 8; ++w) { mv += s_sum[w][0]; mw += s_sum[w][1]; }
         const float kb = __int_as_float(pm.pad);                    // bound on |kx ky| of this plane (>= 1)
         const float sv = 2104533975.0f / fmaxf(mv * kb, 1e-30f), sw = 2104533975.0f / fmaxf(mw * kb, 1e-30f);
-        for (uint32_t i = warp; i < item.count; i += 8) {
+        const int per = 32 / S > 0 ? 32 / S : 1;                    // samples per warp pass (S <= 63: S > 32 takes two column passes)
+        const int sub = lane / S, j0 = lane - sub * S;
+        const bool on = sub < per;
+        for (uint32_t i0 = (uint32_t)(warp * per); i0 < item.count; i0 += 8u * per) {
+            const uint32_t i = i0 + (uint32_t)sub;
+            if (!on || i >= item.count) continue;
             const uint4 a = __ldg(reinterpret_cast<const uint4*>(sorted + item.start + i));
             const float re = __uint_as_float(a.x) * sv, im = __uint_as_float(a.y) * sv, wt = __uint_as_float(a.z) * sw;
             const int lx = (int)(a.w & 31u), ly = (int)((a.w >> 5) & 31u);
             const int rx = (int)((a.w >> 10) & 511u), ry = (int)((a.w >> 19) & 511u), kc = (int)((a.w >> 28) & 1u);
-            int jy = jy0, jx = jx0;                                 // advanced by 32 cells per pass
-            for (int c = lane; c < S * S; c += 32, jx += r32, jy += q32) {
-                if (jx >= S) { jx -= S; ++jy; }
-                const int si = (ly + jy) * R + lx + jx;              // region origin is (tile origin - h)
+            for (int jx = j0; jx < S; jx += 32) {                   // one pass unless S > 32
+                int* cell = smem_i + ly * R + lx + jx;               // region origin is (tile origin - h)
                 if (WMODE == 0) {
-                    const float kk = __ldg(tables + pm.offset + rx * pm.pitch + jx) * __ldg(tables + pm.offset + ry * pm.pitch + jy);
-                    atomicAdd(&smem_i[si], __float2int_rn(kk * re));
-                    atomicAdd(&smem_i[RR + si], __float2int_rn(kk * im));
-                    atomicAdd(&smem_i[2 * RR + si], __float2int_rn(kk * wt));
+                    const float kx = s_tab[rx * pm.pitch + jx];
+                    const float* kyp = s_tab + ry * pm.pitch;
+                    for (int jy = 0; jy < S; ++jy, cell += R) {
+                        const float kk = kx * kyp[jy];
+                        atomicAdd(cell, __float2int_rn(kk * re));
+                        atomicAdd(cell + RR, __float2int_rn(kk * im));
+                        atomicAdd(cell + 2 * RR, __float2int_rn(kk * wt));
+                    }
                 } else {
-                    const float2* tc = reinterpret_cast<const float2*>(tables);
-                    float2 kx = __ldg(tc + pm.offset + rx * pm.pitch + jx), ky = __ldg(tc + pm.offset + ry * pm.pitch + jy);
-                    if (kc) { kx.y = -kx.y; ky.y = -ky.y; }
-                    const float kr = kx.x * ky.x - kx.y * ky.y, ki = kx.x * ky.y + kx.y * ky.x;
-                    atomicAdd(&smem_i[si], __float2int_rn(kr * re - ki * im));
-                    atomicAdd(&smem_i[RR + si], __float2int_rn(kr * im + ki * re));
-                    atomicAdd(&smem_i[2 * RR + si], __float2int_rn(kr * wt));
-                    atomicAdd(&smem_i[3 * RR + si], __float2int_rn(ki * wt));
+                    const float2* tc = reinterpret_cast<const float2*>(s_tab);
+                    float2 kx = tc[rx * pm.pitch + jx];
+                    const float cs = kc ? -1.0f : 1.0f;               // conjugate kernel for w < 0
+                    kx.y *= cs;
+                    const float2* kyp = tc + ry * pm.pitch;
+                    for (int jy = 0; jy < S; ++jy, cell += R) {
+                        float2 ky = kyp[jy];
+                        ky.y *= cs;
+                        // row factors (same for every lane of the sample), then one complex multiply per grid
+                        const float tr = ky.x * re - ky.y * im, ti = ky.x * im + ky.y * re;
+                        const float ur = ky.x * wt, ui = ky.y * wt;
+                        atomicAdd(cell, __float2int_rn(kx.x * tr - kx.y * ti));
+                        atomicAdd(cell + RR, __float2int_rn(kx.x * ti + kx.y * tr));
+                        atomicAdd(cell + 2 * RR, __float2int_rn(kx.x * ur - kx.y * ui));
+                        atomicAdd(cell + 3 * RR, __float2int_rn(kx.x * ui + kx.y * ur));
+                    }
                 }
             }
         }
@@ -307,7 +335,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_generic(const Geom g, const 
           for (int x = lane; x < R; x += 32) {
             const int i = y * R + x;
             const int gx = x0 + x, gy = y0 + y;
-            if (gx < 0 || gx >= g.nx || gy < 0 || gy >= g.ny) continue;
+            if (gx < 0 || gx >= g.nx || gy < (g.ny >> 1) || gy >= g.ny) continue;   // the stored half-plane only
             const size_t idx = gbase + (size_t)gy * g.nx + gx;
             const int vr = smem_i[i], vi = smem_i[RR + i], wr = smem_i[2 * RR + i];
             if (vr | vi) atomicAdd(&grids.G[idx], make_float2((float)vr * iv, (float)vi * iv));
@@ -436,7 +464,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
         for (int i = threadIdx.x; i < PL; i += blockDim.x) {
             const int y = i / kFastPitch, x = i - y * kFastPitch;
             const int gx = x0 + x, gy = y0 + y;
-            if (x >= kFastR || gx < 0 || gx >= g.nx || gy < 0 || gy >= g.ny) continue;
+            if (x >= kFastR || gx < 0 || gx >= g.nx || gy < (g.ny >> 1) || gy >= g.ny) continue;   // the stored half-plane only
             const size_t idx = gbase + (size_t)gy * g.nx + gx;
             const float vr = s_re[i], vi = s_im[i], vw = s_w[i];
             if (vr != 0.f || vi != 0.f) atomicAdd(&grids.G[idx], make_float2(vr, vi));
@@ -629,9 +657,12 @@ cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsampl
     return cudaGetLastError();
 }
 
-static size_t generic_smem_bytes(int wmode, int smax) {
+static int generic_region_ints(int wmode, int smax) {
     const int R = kTile + (smax - 1);
-    return (size_t)(wmode ? 4 : 3) * R * R * sizeof(float);
+    return ((wmode ? 4 : 3) * R * R + 3) & ~3;
+}
+static size_t generic_smem_bytes(int wmode, int smax, int Q, int pitch_max) {
+    return (size_t)generic_region_ints(wmode, smax) * sizeof(int) + (size_t)(Q + 1) * pitch_max * (wmode ? 2 : 1) * sizeof(float);
 }
 static size_t fast_smem_bytes(int Q) {
     return (size_t)(3 * kFastR * kFastPitch + 1024 + 4 * kFastChunk + (Q + 1) * 8) * sizeof(float);
@@ -654,10 +685,14 @@ cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* i
     if (!g.wmode && smax == 7 && g.chunk == kFastChunk) {
         k_grid_tiled_s7<<<num_sms * 4, 256, fast_smem_bytes(g.Q), s>>>(g, sorted, items, nitems, planes, tables, grids);
     } else {
-        const size_t smem = generic_smem_bytes(g.wmode, smax);
-        const int per_sm = smem > 110 * 1024 ? 1 : (smem > 70 * 1024 ? 2 : 4);
-        if (g.wmode) k_grid_tiled_generic<1><<<num_sms * per_sm, 256, smem, s>>>(g, sorted, items, nitems, planes, tables, grids);
-        else k_grid_tiled_generic<0><<<num_sms * per_sm, 256, smem, s>>>(g, sorted, items, nitems, planes, tables, grids);
+        int pitch_max = 4;
+        for (int p = 0; p < P; ++p) pitch_max = planes_host[p].pitch > pitch_max ? planes_host[p].pitch : pitch_max;
+        const size_t smem = generic_smem_bytes(g.wmode, smax, g.Q, pitch_max);
+        const int region = generic_region_ints(g.wmode, smax);
+        int per_sm = (int)(220 * 1024 / (smem + 1024));
+        per_sm = per_sm < 1 ? 1 : (per_sm > 4 ? 4 : per_sm);
+        if (g.wmode) k_grid_tiled_generic<1><<<num_sms * per_sm, 256, smem, s>>>(g, sorted, items, nitems, planes, tables, grids, region);
+        else k_grid_tiled_generic<0><<<num_sms * per_sm, 256, smem, s>>>(g, sorted, items, nitems, planes, tables, grids, region);
     }
     return cudaGetLastError();
 }
