@@ -50,7 +50,7 @@ struct muser_imager {
     Staged* staged = nullptr;
     Sample* sorted = nullptr;
     size_t sample_cap = 0;
-    uint32_t *bin_count = nullptr, *bin_offset = nullptr, *nitems_d = nullptr;
+    uint32_t *bin_count = nullptr, *bin_offset = nullptr, *nitems_d = nullptr, *bin_tops = nullptr;
     Item* items = nullptr;
     size_t bins_cap = 0, items_cap = 0;
     Stats* stats_d = nullptr;
@@ -130,8 +130,8 @@ void free_grids(muser_imager* h) {
 }
 
 void free_bins(muser_imager* h) {
-    cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items);
-    h->bin_count = h->bin_offset = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
+    cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->items); cudaFree(h->bin_tops);
+    h->bin_count = h->bin_offset = h->bin_tops = nullptr; h->items = nullptr; h->bins_cap = h->items_cap = 0;
     cudaFree(h->ow_count); cudaFree(h->ow_cursor); cudaFree(h->ow_offset); cudaFree(h->ow_work); cudaFree(h->ow_tops);
     cudaFree(h->ow_cta_hist);
     h->ow_count = h->ow_cursor = h->ow_offset = h->ow_tops = nullptr; h->ow_work = nullptr; h->ow_bins_cap = 0;
@@ -300,8 +300,9 @@ int ensure_scratch(muser_imager* h, long long nvis, cudaStream_t s) {
     }
     const size_t nb = h->geom.nbins;
     if (nb + 1 > h->bins_cap) {
-        cudaFree(h->bin_count); cudaFree(h->bin_offset);
-        h->bin_count = h->bin_offset = nullptr; h->bins_cap = 0;
+        cudaFree(h->bin_count); cudaFree(h->bin_offset); cudaFree(h->bin_tops);
+        h->bin_count = h->bin_offset = h->bin_tops = nullptr; h->bins_cap = 0;
+        CU(h, cudaMalloc(&h->bin_tops, (nb / 4096 + 2) * 2 * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->bin_count, (nb + 1) * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->bin_offset, (nb + 1) * sizeof(uint32_t)));
         // K2 re-zeroes the histogram after every use; this first zeroing is ordered on the caller's stream
@@ -429,9 +430,9 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         StageScope sc(h, MUSER_STAGE_BIN, s);
         CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
                             h->stats_d, h->cnt, s));
-        CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, s));
+        CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, h->bin_tops, s));
         CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
-        h->n_launches += 3;
+        h->n_launches += g.nbins <= 4096u ? 3 : 5;
     }
     {
         StageScope sc(h, MUSER_STAGE_GRID, s);

@@ -98,7 +98,7 @@ cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, c
                           const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
                           uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s);
 cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,
-                              uint32_t* nitems, cudaStream_t s);
+                              uint32_t* nitems, uint32_t* tops, cudaStream_t s);
 cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsamples, const uint32_t* bin_offset,
                            Sample* sorted, cudaStream_t s);
 cudaError_t launch_grid_tiled(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* nitems,

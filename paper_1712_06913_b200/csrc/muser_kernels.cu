@@ -161,53 +161,104 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
 }
 
 // ------------------------------------------------------------------------------------------------- K2
-// One CTA walks the histogram 1024 bins at a time: exclusive offsets, work items, and re-zeroes the histogram
-// for the next call.
-__global__ void __launch_bounds__(1024) k_scan_items(const Geom g, uint32_t* __restrict__ bin_count,
-                                                     uint32_t* __restrict__ bin_offset, Item* __restrict__ items,
-                                                     uint32_t* __restrict__ nitems) {
-    __shared__ uint32_t s_wsum[2][32];
-    __shared__ uint32_t s_carry[2];
+// Exclusive scan of the tile histogram -> sample offsets and work items of <= chunk samples; re-zeroes the histogram
+// for the next call.  Multi-CTA: per-block totals (4096 bins per CTA), one CTA scans the totals, every CTA writes its
+// block (one launch when the histogram fits one block).
+struct Scan2 { uint32_t c, n; };
+__device__ __forceinline__ Scan2 block_scan2(Scan2 v, Scan2& total, uint32_t (*s_w)[32]) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) { s_carry[0] = 0; s_carry[1] = 0; }
+    Scan2 inc = v;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t xc = __shfl_up_sync(0xffffffffu, inc.c, o), xn = __shfl_up_sync(0xffffffffu, inc.n, o);
+        if (lane >= o) { inc.c += xc; inc.n += xn; }
+    }
+    if (lane == 31) { s_w[0][warp] = inc.c; s_w[1][warp] = inc.n; }
     __syncthreads();
-    const uint32_t CH = (uint32_t)g.chunk;
-    for (uint32_t base = 0; base < g.nbins; base += 1024) {
-        const uint32_t b = base + threadIdx.x;
-        uint32_t c = 0;
-        if (b < g.nbins) { c = bin_count[b]; if (c) bin_count[b] = 0; }
-        const uint32_t n = (c + CH - 1) / CH;
-        uint32_t ic = c, in = n;                                      // inclusive warp scans
+    if (warp == 0) {
+        uint32_t wc = s_w[0][lane], wn = s_w[1][lane];
         for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t tc = __shfl_up_sync(0xffffffffu, ic, o), tn = __shfl_up_sync(0xffffffffu, in, o);
-            if (lane >= o) { ic += tc; in += tn; }
+            const uint32_t xc = __shfl_up_sync(0xffffffffu, wc, o), xn = __shfl_up_sync(0xffffffffu, wn, o);
+            if (lane >= o) { wc += xc; wn += xn; }
         }
-        if (lane == 31) { s_wsum[0][warp] = ic; s_wsum[1][warp] = in; }
-        __syncthreads();
-        if (warp == 0) {
-            uint32_t wc = s_wsum[0][lane], wn = s_wsum[1][lane];
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t tc = __shfl_up_sync(0xffffffffu, wc, o), tn = __shfl_up_sync(0xffffffffu, wn, o);
-                if (lane >= o) { wc += tc; wn += tn; }
-            }
-            s_wsum[0][lane] = wc; s_wsum[1][lane] = wn;               // inclusive over warps
-        }
-        __syncthreads();
-        const uint32_t off = s_carry[0] + (warp ? s_wsum[0][warp - 1] : 0) + ic - c;
-        const uint32_t ioff = s_carry[1] + (warp ? s_wsum[1][warp - 1] : 0) + in - n;
+        s_w[0][lane] = wc; s_w[1][lane] = wn;
+    }
+    __syncthreads();
+    Scan2 ex;
+    ex.c = (warp ? s_w[0][warp - 1] : 0u) + inc.c - v.c;
+    ex.n = (warp ? s_w[1][warp - 1] : 0u) + inc.n - v.n;
+    total.c = s_w[0][31]; total.n = s_w[1][31];
+    __syncthreads();
+    return ex;
+}
+__device__ __forceinline__ Scan2 scan_load4(const Geom& g, const uint32_t* __restrict__ bin_count, uint32_t b0, uint32_t c[4]) {
+    Scan2 t = {0u, 0u};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        c[j] = (b0 + j < g.nbins) ? bin_count[b0 + j] : 0u;
+        t.c += c[j];
+        t.n += (c[j] + (uint32_t)g.chunk - 1u) / (uint32_t)g.chunk;
+    }
+    return t;
+}
+
+__global__ void __launch_bounds__(1024) k_scan_items_reduce(const Geom g, const uint32_t* __restrict__ bin_count,
+                                                            uint32_t* __restrict__ tops) {
+    __shared__ uint32_t s_w[2][32];
+    uint32_t c[4];
+    const Scan2 t = scan_load4(g, bin_count, blockIdx.x * 4096u + 4u * threadIdx.x, c);
+    Scan2 total;
+    block_scan2(t, total, s_w);
+    if (threadIdx.x == 0) { tops[2 * blockIdx.x] = total.c; tops[2 * blockIdx.x + 1] = total.n; }
+}
+
+__global__ void __launch_bounds__(1024) k_scan_items_tops(const Geom g, const uint32_t nblocks, uint32_t* __restrict__ tops,
+                                                          uint32_t* __restrict__ bin_offset, uint32_t* __restrict__ nitems) {
+    __shared__ uint32_t s_w[2][32];
+    Scan2 carry = {0u, 0u};
+    for (uint32_t base = 0; base < nblocks; base += 1024) {
+        const uint32_t b = base + threadIdx.x;
+        Scan2 v = {0u, 0u};
+        if (b < nblocks) { v.c = tops[2 * b]; v.n = tops[2 * b + 1]; }
+        Scan2 total;
+        const Scan2 ex = block_scan2(v, total, s_w);
+        if (b < nblocks) { tops[2 * b] = carry.c + ex.c; tops[2 * b + 1] = carry.n + ex.n; }
+        carry.c += total.c; carry.n += total.n;
+    }
+    if (threadIdx.x == 0) { bin_offset[g.nbins] = carry.c; *nitems = carry.n; }
+}
+
+template <int SINGLE>
+__global__ void __launch_bounds__(1024) k_scan_items_write(const Geom g, uint32_t* __restrict__ bin_count,
+                                                           const uint32_t* __restrict__ tops, uint32_t* __restrict__ bin_offset,
+                                                           Item* __restrict__ items, uint32_t* __restrict__ nitems) {
+    __shared__ uint32_t s_w[2][32];
+    const uint32_t b0 = blockIdx.x * 4096u + 4u * threadIdx.x;
+    uint32_t c[4];
+    const Scan2 t = scan_load4(g, bin_count, b0, c);
+    Scan2 total;
+    const Scan2 ex = block_scan2(t, total, s_w);
+    uint32_t off = ex.c, ioff = ex.n;
+    if (SINGLE) {
+        if (threadIdx.x == 0) { bin_offset[g.nbins] = total.c; *nitems = total.n; }
+    } else {
+        off += tops[2 * blockIdx.x]; ioff += tops[2 * blockIdx.x + 1];
+    }
+    const uint32_t CH = (uint32_t)g.chunk;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t b = b0 + j;
         if (b < g.nbins) {
             bin_offset[b] = off;
-            for (uint32_t j = 0; j < n; ++j) {
+            if (c[j]) bin_count[b] = 0;
+            const uint32_t n = (c[j] + CH - 1u) / CH;
+            for (uint32_t q = 0; q < n; ++q) {
                 Item it;
-                it.bin = b; it.start = off + j * CH; it.count = min(CH, c - j * CH);
-                items[ioff + j] = it;
+                it.bin = b; it.start = off + q * CH; it.count = min(CH, c[j] - q * CH);
+                items[ioff + q] = it;
             }
+            off += c[j]; ioff += n;
         }
-        __syncthreads();
-        if (threadIdx.x == 1023) { s_carry[0] = off + c; s_carry[1] = ioff + n; }
-        __syncthreads();
     }
-    if (threadIdx.x == 0) { bin_offset[g.nbins] = s_carry[0]; *nitems = s_carry[1]; }
 }
 
 // ------------------------------------------------------------------------------------------------- K3
@@ -646,8 +697,15 @@ cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, c
 }
 
 cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,
-                              uint32_t* nitems, cudaStream_t s) {
-    k_scan_items<<<1, 1024, 0, s>>>(g, bin_count, bin_offset, items, nitems);
+                              uint32_t* nitems, uint32_t* tops, cudaStream_t s) {
+    const uint32_t nblocks = (g.nbins + 4095u) / 4096u;
+    if (nblocks == 1) {
+        k_scan_items_write<1><<<1, 1024, 0, s>>>(g, bin_count, tops, bin_offset, items, nitems);
+        return cudaGetLastError();
+    }
+    k_scan_items_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, tops);
+    k_scan_items_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems);
+    k_scan_items_write<0><<<nblocks, 1024, 0, s>>>(g, bin_count, tops, bin_offset, items, nitems);
     return cudaGetLastError();
 }
 
