@@ -37,13 +37,29 @@ constexpr int kOwKXB = kOwTWS;                   // bits of the window column in
 constexpr uint32_t kOwKeyMask = (1u << (5 + kOwKXB)) - 1u;
 
 // ------------------------------------------------------------------------------------------------- coordinates
-// O1 for one axis (same operation order as the oracle; _rn intrinsics forbid FMA contraction).
-__device__ __forceinline__ void ow_cell_phase(double c_lambda, double scale, int n, int Q, double& i0, double& r) {
-    const double p = __dadd_rn(__dmul_rn(c_lambda, scale), (double)(n / 2));
-    i0 = floor(__dadd_rn(p, 0.5));
-    const double fr = __dsub_rn(p, i0);
-    r = floor(__dadd_rn(__dmul_rn(fr, (double)Q), 0.5));
+// O1 for one axis (same operation order and the same fp64 roundings as the oracle; _rn intrinsics forbid FMA
+// contraction).  xs = c_lambda * scale already rounded (the conjugate sample negates it: exact).  The two floors and the
+// conversions to int are done in the FP64 add pipe with the 1.5 * 2^52 constant (x + M rounds x to the nearest integer,
+// whose two's complement sits in the low word; one compare turns nearest into floor) instead of FRND.F64 / F2I.F64,
+// which are conversion-unit instructions at a fraction of the FP64 rate.  Exact for |x| < 2^31 (callers test |xs| < 1e9).
+struct OwAxes { double hx, hy, Qd; };
+__device__ __forceinline__ OwAxes ow_axes(const Geom& g) { return {(double)(g.nx / 2), (double)(g.ny / 2), (double)g.Q}; }
+__device__ __forceinline__ void ow_cell_phase(const double xs, const double half, const double Qd, int& i0, int& r) {
+    constexpr double M = 6755399441055744.0;
+    const double p = __dadd_rn(xs, half);
+    const double t = __dadd_rn(p, 0.5);
+    const double tm = __dadd_rn(t, M);
+    double fl = __dadd_rn(tm, -M);
+    int i = __double2loint(tm);
+    if (fl > t) { fl = __dadd_rn(fl, -1.0); --i; }                    // i0 = floor(p + 0.5)
+    const double fr = __dsub_rn(p, fl);
+    const double u = __dadd_rn(__dmul_rn(fr, Qd), 0.5);
+    const double um = __dadd_rn(u, M);
+    int q = __double2loint(um);
+    if (__dadd_rn(um, -M) > u) --q;                                   // r = floor(fr * Q + 0.5)
+    i0 = i; r = q;
 }
+__device__ __noinline__ double ow_freq_over_c(const double f) { return __ddiv_rn(f, kC); }
 
 struct OwLoc {
     int state;                 // 0 none (k >= nvis), 1 flagged, 2 dropped, 3 kept
@@ -54,36 +70,47 @@ struct OwLoc {
 
 // `f_cache`/`il_cache`: the division f/c is repeated only when the frequency differs from the thread's previous
 // visibility (a thread's visibilities are 256 apart: almost always the same channel).
-__device__ __forceinline__ void ow_locate(const Geom& g, const float* __restrict__ uvw, const double* __restrict__ freq,
-                                          const float2* __restrict__ vis, const float* __restrict__ weight,
-                                          const int* __restrict__ grid_id, long long k, long long nvis, OwLoc& L,
-                                          float2& Vraw, double& f_cache, double& il_cache) {
+struct OwIn { float um, vm, wm, wt; double f; float2 V; int gid; };   // one visibility's inputs
+__device__ __forceinline__ OwIn ow_load(const float* __restrict__ uvw, const double* __restrict__ freq,
+                                        const float2* __restrict__ vis, const float* __restrict__ weight,
+                                        const int* __restrict__ grid_id, const long long k, const long long nvis) {
+    OwIn in = {0.f, 0.f, 0.f, 0.f, 0.0, make_float2(0.f, 0.f), 0};
+    if (k < nvis) {
+        in.um = __ldg(uvw + 3 * k); in.vm = __ldg(uvw + 3 * k + 1); in.wm = __ldg(uvw + 3 * k + 2);
+        in.f = __ldg(freq + k);
+        if (vis) in.V = __ldg(vis + k);
+        in.wt = __ldg(weight + k);
+        if (grid_id) in.gid = __ldg(grid_id + k);
+    }
+    return in;
+}
+__device__ __forceinline__ void ow_locate(const Geom& g, const OwIn& in, long long k, long long nvis, OwLoc& L,
+                                          float2& Vraw, double& f_cache, double& il_cache, const OwAxes& ax) {
     L.state = 0;
     if (k >= nvis) return;
-    const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
-    const double f = freq[k];
-    const float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
-    const float wt = weight[k];
-    const int gid = grid_id ? grid_id[k] : 0;
+    const float um = in.um, vm = in.vm, wm = in.wm;
+    const double f = in.f;
+    const float2 V = in.V;
+    const float wt = in.wt;
+    const int gid = in.gid;
     Vraw = V;
-    if (f != f_cache) { il_cache = __ddiv_rn(f, kC); f_cache = f; }
+    if (f != f_cache) { il_cache = ow_freq_over_c(f); f_cache = f; }   // a call: taken once per channel and thread
     const double il = il_cache;
     const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
     const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) && isfinite(V.y) &&
                     isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
     if (!ok) { L.state = 1; return; }
     const int h = (g.S - 1) >> 1;
-    bool inside = true;
+    const double xu = __dmul_rn(ul, g.su), xv = __dmul_rn(vl, g.sv);
+    bool inside = fabs(xu) < 1.0e9 && fabs(xv) < 1.0e9;               // beyond: off any grid, and outside the int range
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
-        const double sgn = s ? -1.0 : 1.0;
-        double iu, iv, ru, rv;
-        ow_cell_phase(sgn * ul, g.su, g.nx, g.Q, iu, ru);
-        ow_cell_phase(sgn * vl, g.sv, g.ny, g.Q, iv, rv);
-        inside = inside && iu >= (double)(h + 1) && iu <= (double)(g.nx - 1 - h) && iv >= (double)(h + 1) &&
-                 iv <= (double)(g.ny - 1 - h);
-        L.cu[s] = (int)iu; L.cv[s] = (int)iv;
-        L.rx[s] = g.Q / 2 - (int)ru; L.ry[s] = g.Q / 2 - (int)rv;
+        int iu, iv, ru, rv;
+        ow_cell_phase(s ? -xu : xu, ax.hx, ax.Qd, iu, ru);
+        ow_cell_phase(s ? -xv : xv, ax.hy, ax.Qd, iv, rv);
+        inside = inside && iu >= h + 1 && iu <= g.nx - 1 - h && iv >= h + 1 && iv <= g.ny - 1 - h;
+        L.cu[s] = iu; L.cv[s] = iv;
+        L.rx[s] = g.Q / 2 - ru; L.ry[s] = g.Q / 2 - rv;
     }
     if (!inside) { L.state = 2; return; }
     L.state = 3;
@@ -165,11 +192,14 @@ __global__ void __launch_bounds__(kBinThreads, 4) k_owner_count(const Geom g, co
     __syncthreads();
     int kept = 0, dropped = 0, flagged = 0;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0, f_cache = 0.0, il_cache = 0.0;
+    const OwAxes ax = ow_axes(g);
+    float w2f = 0.f, v2f = 0.f;
     for (int it = 0; it < iters; ++it) {
         const long long k = base + (long long)it * kBinThreads + threadIdx.x;
+        const OwIn cur = ow_load(uvw, freq, vis, weight, grid_id, k, nvis);
         OwLoc L;
         float2 V;
-        ow_locate(g, uvw, freq, vis, weight, grid_id, k, nvis, L, V, f_cache, il_cache);
+        ow_locate(g, cur, k, nvis, L, V, f_cache, il_cache, ax);
         uint32_t tp[2] = {0u, 0u};
         if (k < nvis) {                                               // integer result of O1 for k_owner_scatter
             uint4 o = make_uint4(0u, 0u, (uint32_t)L.state << 30, 0u);
@@ -182,9 +212,9 @@ __global__ void __launch_bounds__(kBinThreads, 4) k_owner_count(const Geom g, co
                 tp[1] = ow_tiles_packed(g, L.cu[1], L.cv[1]);
                 ++kept;
                 wsum += 2.0 * (double)L.wt;
-                const double w2 = (double)L.wt * (double)L.wt;
-                w2sum += w2;
-                v2sum += w2 * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
+                const float w2 = L.wt * L.wt;                          // feed alpha only (a power of two): fp32 per thread
+                w2f += w2;
+                v2f += w2 * (V.x * V.x + V.y * V.y);
             }
             dropped += L.state == 2;
             flagged += L.state == 1;
@@ -219,6 +249,7 @@ __global__ void __launch_bounds__(kBinThreads, 4) k_owner_count(const Geom g, co
                 }
         }
     }
+    v2sum = (double)v2f; w2sum = (double)w2f;
     __syncthreads();
     if (fits) {
         const bool ok = ref >= 0 && ref < g.ngrids;
@@ -405,7 +436,7 @@ __device__ __forceinline__ void ow_write_record(const Geom& g, const OwLoc& L, i
 // Same CTA -> visibility mapping as k_owner_count.  The CTA's per-tile counts of its reference grid come from cta_hist:
 // it reserves a run in each touched tile (one global atomic per tile), then hands out the positions inside the runs with
 // the shared counters; records of other grids take warp-aggregated global cursors.
-__global__ void __launch_bounds__(kBinThreads, 5) k_owner_scatter(const Geom g, const uint4* __restrict__ loc,
+__global__ void __launch_bounds__(kBinThreads, 4) k_owner_scatter(const Geom g, const uint4* __restrict__ loc,
                                                                const float* __restrict__ uvw, const double* __restrict__ freq,
                                                                const float2* __restrict__ vis,
                                                                const float* __restrict__ weight, const int* __restrict__ grid_id,
@@ -431,22 +462,39 @@ __global__ void __launch_bounds__(kBinThreads, 5) k_owner_scatter(const Geom g, 
         }
     }
     __syncthreads();
+    // the loads of a visibility do not depend on one another (flagged visibilities are rare: vis / weight are read
+    // unconditionally) and are issued one iteration ahead
+    struct ScIn { uint4 o; float2 V; float wt; int gid; };
+    auto load = [&](const long long k) {
+        ScIn r;
+        r.o = make_uint4(0u, 0u, 0u, 0u); r.V = make_float2(0.f, 0.f); r.wt = 0.f; r.gid = 0;
+        if (k < nvis) {
+            r.o = __ldg(loc + k);
+            if (vis) r.V = __ldg(vis + k);
+            r.wt = __ldg(weight + k);
+            if (grid_id) r.gid = __ldg(grid_id + k);
+        }
+        return r;
+    };
+    ScIn nxt = load(base + threadIdx.x);
     for (int it = 0; it < iters; ++it) {
         const long long k = base + (long long)it * kBinThreads + threadIdx.x;
+        const ScIn cur = nxt;
+        if (it + 1 < iters) nxt = load(k + kBinThreads);
         OwLoc L;
         L.state = 0;
         if (k < nvis) {                                               // k_owner_count's integer decisions
-            const uint4 o = __ldg(loc + k);
+            const uint4 o = cur.o;
             L.state = (int)(o.z >> 30);
             if (L.state == 3) {
                 L.cu[0] = (int)(o.x & 0xFFFFu); L.cv[0] = (int)(o.x >> 16);
                 L.cu[1] = (int)(o.y & 0xFFFFu); L.cv[1] = (int)(o.y >> 16);
                 L.rx[0] = (int)(o.z & 511u); L.ry[0] = (int)((o.z >> 9) & 511u); L.rx[1] = (int)((o.z >> 18) & 511u);
                 L.ry[1] = (int)(o.w & 511u);
-                float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
+                float2 V = cur.V;
                 if (g.phase_on) V = phase_rotate(g, uvw[3 * k], uvw[3 * k + 1], freq[k], V);
-                const float wt = weight[k];
-                L.re = wt * V.x; L.im = wt * V.y; L.wt = wt; L.gid = grid_id ? grid_id[k] : 0;
+                const float wt = cur.wt;
+                L.re = wt * V.x; L.im = wt * V.y; L.wt = wt; L.gid = cur.gid;
                 if (cnt) {                                            // NEXT-2: one hit per sample at its nearest cell (stored half-plane)
 #pragma unroll
                     for (int s = 0; s < 2; ++s)
@@ -540,7 +588,7 @@ __device__ __forceinline__ void rows_block(const RowsShape& sh, const int cpc, i
 __device__ __forceinline__ size_t rows_cta(void) { return blockIdx.x + (size_t)gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z); }
 __device__ __forceinline__ void rows_locate(const Geom& g, const RowsShape& sh, const float* __restrict__ uvw,
                                             const double f, const double il, const int gid, const int t, const int po,
-                                            const int c, const int r, RowsElem& E) {
+                                            const int c, const int r, const OwAxes& ax, RowsElem& E) {
     E.t = t; E.po = po; E.c = c; E.r = r;
     const size_t ub = ((size_t)E.t * sh.nrow + E.r) * 3;
     const float um = uvw[ub], vm = uvw[ub + 1], wm = uvw[ub + 2];
@@ -551,17 +599,16 @@ __device__ __forceinline__ void rows_locate(const Geom& g, const RowsShape& sh, 
     E.inside = false;
     if (!E.geom_ok) return;
     const int h = (g.S - 1) >> 1;
-    bool inside = true;
+    const double xu = __dmul_rn(ul, g.su), xv = __dmul_rn(vl, g.sv);
+    bool inside = fabs(xu) < 1.0e9 && fabs(xv) < 1.0e9;
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
-        const double sgn = s ? -1.0 : 1.0;
-        double iu, iv, ru, rv;
-        ow_cell_phase(sgn * ul, g.su, g.nx, g.Q, iu, ru);
-        ow_cell_phase(sgn * vl, g.sv, g.ny, g.Q, iv, rv);
-        inside = inside && iu >= (double)(h + 1) && iu <= (double)(g.nx - 1 - h) && iv >= (double)(h + 1) &&
-                 iv <= (double)(g.ny - 1 - h);
-        E.L.cu[s] = (int)iu; E.L.cv[s] = (int)iv;
-        E.L.rx[s] = g.Q / 2 - (int)ru; E.L.ry[s] = g.Q / 2 - (int)rv;
+        int iu, iv, ru, rv;
+        ow_cell_phase(s ? -xu : xu, ax.hx, ax.Qd, iu, ru);
+        ow_cell_phase(s ? -xv : xv, ax.hy, ax.Qd, iv, rv);
+        inside = inside && iu >= h + 1 && iu <= g.nx - 1 - h && iv >= h + 1 && iv <= g.ny - 1 - h;
+        E.L.cu[s] = iu; E.L.cv[s] = iv;
+        E.L.rx[s] = g.Q / 2 - ru; E.L.ry[s] = g.Q / 2 - rv;
     }
     E.inside = inside;
 }
@@ -593,13 +640,14 @@ __global__ void __launch_bounds__(kBinThreads, 4) k_rows_count(const Geom g, con
     __syncthreads();
     int kept = 0, dropped = 0, flagged = 0;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
+    const OwAxes ax = ow_axes(g);
     for (int ci = 0; ci < nc; ++ci) {
         const int c = c0 + ci;
         const int gid = gids ? gids[c] : 0;
         uint32_t tp[2] = {0u, 0u};
         if (r < sh.nrow) {
             RowsElem E;
-            rows_locate(g, sh, uvw, freq[c], s_il[ci], gid, t, po, c, r, E);
+            rows_locate(g, sh, uvw, freq[c], s_il[ci], gid, t, po, c, r, ax, E);
             const RowsSum S = rows_sum_pols(g, sh, vis, weight, E.t, E.po, E.c, E.r, E.geom_ok, E.inside, E.um, E.vm, E.f);
             kept += S.kept; flagged += S.flagged; dropped += sh.npi - S.kept - S.flagged;
             wsum += S.wsum; v2sum += S.v2sum; w2sum += S.w2sum;
