@@ -47,9 +47,12 @@ enum { MUSER_KERNEL_PSWF = 0, MUSER_KERNEL_GAUSS = 1 };
  * shared memory and stores it once (no memset, no global atomics; 2-D mode with support 7 only, else
  * MUSER_EUNSUPPORTED at muser_grid); the other half-plane is rebuilt on demand (muser_get_grid).  TILED: work items of
  * <= 512 samples per 32x32 tile, shared memory accumulation, global reductions at the flush (any support, w planes).
- * AUTO picks OWNER where it applies, else TILED.  (Value 1 was a per-sample global-reduction strategy; it missed the
- * image tolerance on dense grids and was removed.) */
-enum { MUSER_STRATEGY_AUTO = 0, MUSER_STRATEGY_TILED = 2, MUSER_STRATEGY_OWNER = 3 };
+ * WPLANE (w mode, every plane support <= 31): work items of <= 4096 records of one 32x32 tile, sorted by
+ * plane; a run of records whose footprints share a 2x2-aligned (S+1) x (S+1) window is accumulated in registers and
+ * merged into a fixed-point shared-memory region, which is added to the grids once per item.
+ * AUTO picks OWNER where it applies, else WPLANE where it applies, else TILED.  (Value 1 was a per-sample
+ * global-reduction strategy; it missed the image tolerance on dense grids and was removed.) */
+enum { MUSER_STRATEGY_AUTO = 0, MUSER_STRATEGY_TILED = 2, MUSER_STRATEGY_OWNER = 3, MUSER_STRATEGY_WPLANE = 4 };
 /* stage ids of muser_get_profile.  On the fused imaging path (ny = 256, 512, 1024 and nx a multiple of 16) FFT is
  * cuFFT's row pass and CORRECT the library's own column transform with the shift/correction epilogue; otherwise FFT
  * is cuFFT's 2-D transform and CORRECT the stand-alone correction kernel.  PACK only runs when the gridder has not

@@ -63,6 +63,9 @@ struct muser_imager {
     uint4 *ow_sorted = nullptr, *ow_loc = nullptr;          // tile-sorted records; per-visibility integer result of O1
     uint32_t *ow_count = nullptr, *ow_cursor = nullptr, *ow_offset = nullptr, *ow_ctl = nullptr, *ow_tops = nullptr;
     uint4* ow_work = nullptr;
+    uint32_t* wg_ctl = nullptr;             // work counters and list lengths of the w-plane window gridder (per window shape)
+    uint32_t* wg_lists = nullptr;           // per shape: the items that hold records of it
+    size_t wg_list_cap = 0;
     uint32_t* ow_cta_hist = nullptr;        // per binning CTA: its shared tile histogram (k_owner_count -> k_owner_scatter)
     size_t ow_cta_hist_cap = 0;
     bool weights_only = false;              // the 2x-beam child: muser_grid is called without visibilities
@@ -161,6 +164,7 @@ int rebuild_geom(muser_imager* h) {
     g.phase_on = (h->off_l != 0.0 || h->off_m != 0.0) ? 1 : 0;
     g.dl = h->off_l; g.dm = h->off_m;
     g.uniform = h->weighting == MUSER_WEIGHT_UNIFORM ? 1 : 0;
+    g.wtile = 0;
     return MUSER_OK;
 }
 
@@ -318,9 +322,14 @@ int ensure_scratch(muser_imager* h, long long nvis, cudaStream_t s) {
     return MUSER_OK;
 }
 
+bool wplane_capable(const muser_imager* h) {
+    return wmode(h) && wgrid_supported(h->planes_h.data(), (int)h->planes_h.size(), h->Q, h->max_smem);
+}
+
 int pick_strategy(const muser_imager* h) {
     if (h->strategy != MUSER_STRATEGY_AUTO) return h->strategy;
-    return owner_capable(h) ? MUSER_STRATEGY_OWNER : MUSER_STRATEGY_TILED;
+    if (owner_capable(h)) return MUSER_STRATEGY_OWNER;
+    return wplane_capable(h) ? MUSER_STRATEGY_WPLANE : MUSER_STRATEGY_TILED;
 }
 
 uint32_t owner_item_size(long long nvis, int num_sms, int item_override) {
@@ -378,9 +387,14 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     if (nvis < 0 || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "nvis out of range [0, 2^30]");
     if (nvis == 0) return MUSER_OK;
     if (!uvw || !freq || !wt || (!vis && !h->weights_only)) return fail(h, MUSER_EINVAL, "null input pointer");
-    const int strat = pick_strategy(h);
+    int strat = pick_strategy(h);
     const Geom& g = h->geom;
     GridPtrs gp = grid_ptrs(h);
+    if (strat == MUSER_STRATEGY_WPLANE && (unsigned long long)h->ngrids * g.ntiles + (unsigned long long)nvis / 2048 + 2 >= (1ull << 24)) {
+        // its work lists hold 24-bit item indices
+        if (h->strategy != MUSER_STRATEGY_AUTO) return fail(h, MUSER_EUNSUPPORTED, "too many tiles for the w-plane window strategy");
+        strat = MUSER_STRATEGY_TILED;
+    }
     if (strat == MUSER_STRATEGY_OWNER) {
         if (!owner_capable(h)) return fail(h, MUSER_EUNSUPPORTED, "the owner-tile strategy needs 2-D mode and support 7");
         const uint32_t item_size = owner_item_size(nvis, h->num_sms, h->tune[MUSER_TUNE_ITEM_SIZE]);
@@ -419,13 +433,42 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         h->lower_valid = false;                                       // rows < ny/2 are rebuilt on demand (ensure_lower)
         return MUSER_OK;
     }
-    if (strat != MUSER_STRATEGY_TILED) return fail(h, MUSER_EUNSUPPORTED, "unknown gridding strategy");
+    if (strat != MUSER_STRATEGY_TILED && strat != MUSER_STRATEGY_WPLANE) return fail(h, MUSER_EUNSUPPORTED, "unknown gridding strategy");
+    if (strat == MUSER_STRATEGY_WPLANE && !wplane_capable(h))
+        return fail(h, MUSER_EUNSUPPORTED, "the w-plane window strategy needs w mode with every plane support <= 31");
     int rc = ensure_scratch(h, nvis, s);
     if (rc) return rc;
     if ((rc = flush_zero(h, s))) return rc;
     h->last_stream = s;
     h->fft_valid = false;
     h->lower_valid = false;                                           // like the owner path, it grids rows >= ny/2 only
+    if (strat == MUSER_STRATEGY_WPLANE) {
+        // bins ordered (grid, tile, plane); work items = <= 4096 consecutive records of one tile
+        Geom gw = g;
+        gw.wtile = 1;
+        if (!h->wg_ctl) CU(h, cudaMalloc(&h->wg_ctl, 16 * sizeof(uint32_t)));
+        const size_t list_cap = wgrid_list_cap(gw, h->sample_cap);
+        if (list_cap > h->wg_list_cap) {
+            cudaFree(h->wg_lists); h->wg_lists = nullptr; h->wg_list_cap = 0;
+            CU(h, cudaMalloc(&h->wg_lists, 8 * list_cap * sizeof(uint32_t)));
+            h->wg_list_cap = list_cap;
+        }
+        {
+            StageScope sc(h, MUSER_STAGE_BIN, s);
+            CU(h, launch_coords(gw, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
+                                h->stats_d, h->cnt, s));
+            CU(h, launch_scan_items(gw, h->bin_count, h->bin_offset, nullptr, nullptr, h->bin_tops, s));
+            CU(h, launch_wtile_items(gw, h->bin_offset, h->planes_d, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->nitems_d, h->wg_ctl, s));
+            CU(h, launch_scatter(gw, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
+            h->n_launches += g.nbins <= 4096u ? 4 : 6;
+        }
+        StageScope sc(h, MUSER_STAGE_GRID, s);
+        cudaError_t ce = cudaSuccess;
+        h->n_launches += launch_wgrid(gw, h->sorted, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->wg_ctl, h->bin_offset, h->planes_d,
+                                      h->planes_h.data(), h->tables_d, gp, h->num_sms, s, &ce);
+        CU(h, ce);
+        return MUSER_OK;
+    }
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
         CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
@@ -635,7 +678,8 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
         return nullptr;
     };
     if (rc) return bail("geometry");
-    if (tiled_kernel_setup(h->max_smem) != cudaSuccess || owner_kernel_setup(h->max_smem) != cudaSuccess) { h->err = cudaGetErrorString(cudaGetLastError()); return bail("kernel setup"); }
+    if (tiled_kernel_setup(h->max_smem) != cudaSuccess || owner_kernel_setup(h->max_smem) != cudaSuccess ||
+        wgrid_kernel_setup(h->max_smem) != cudaSuccess) { h->err = cudaGetErrorString(cudaGetLastError()); return bail("kernel setup"); }
     if (cudaMalloc(&h->stats_d, sizeof(Stats)) != cudaSuccess || cudaMalloc(&h->nitems_d, sizeof(uint32_t)) != cudaSuccess) {
         h->err = "cudaMalloc failed"; return bail("alloc");
     }
@@ -677,7 +721,7 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
     cudaFree(h->ttp_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
-    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->tw_d); cudaFree(h->tw_rows_d);
+    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->wg_ctl); cudaFree(h->wg_lists); cudaFree(h->tw_d); cudaFree(h->tw_rows_d);
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete h;
@@ -761,7 +805,8 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
 
 int muser_set_strategy(muser_imager* h, int strategy) {
     if (!h) return MUSER_EINVAL;
-    if (strategy != MUSER_STRATEGY_AUTO && strategy != MUSER_STRATEGY_TILED && strategy != MUSER_STRATEGY_OWNER)
+    if (strategy != MUSER_STRATEGY_AUTO && strategy != MUSER_STRATEGY_TILED && strategy != MUSER_STRATEGY_OWNER &&
+        strategy != MUSER_STRATEGY_WPLANE)
         return fail(h, MUSER_EINVAL, "unknown strategy");
     if (h->zero_pending) {                                            // do not carry a deferred reset across strategies
         int rc = flush_zero(h, h->last_stream);

@@ -26,6 +26,8 @@ struct Geom {
     int phase_on;                  // NEXT-3: V *= exp(+2 pi i (u dl + v dm)) before gridding
     double dl, dm;
     int uniform;                   // NEXT-2: hit counts are accumulated and wgtGrid (cell / count) is applied at the FFT input
+    int wtile;                     // generic binning: bins ordered (grid, tile, plane) instead of (grid, plane, tile) -- the
+                                   // w-projection window gridder (muser_wgrid.cu) works through a tile's planes in one item
 };
 
 // Per-plane kernel metadata in constant-ish device memory.
@@ -97,6 +99,7 @@ __device__ __forceinline__ float peak_unordered(unsigned int o) {
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
                           const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
                           uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s);
+// items == nullptr: offsets only (the caller builds its own work items from them)
 cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,
                               uint32_t* nitems, uint32_t* tops, cudaStream_t s);
 cudaError_t launch_scatter(const Geom& g, const Staged* staged, long long nsamples, const uint32_t* bin_offset,
@@ -112,6 +115,16 @@ cudaError_t launch_mirror_lower(const Geom& g, GridPtrs grids, cudaStream_t s);
 cudaError_t launch_correct(const Geom& g, const float2* F, const float* icx, const float* icy, const Stats* stats,
                            float* dirty, float* psf, PeakSlot* peaks, cudaStream_t s);
 cudaError_t tiled_kernel_setup(int max_smem_bytes);
+
+// ---- w-projection window gridder (muser_wgrid.cu): w mode, every plane support <= 31
+bool wgrid_supported(const PlaneMeta* planes_host, int P, int Q, int max_smem_bytes);
+cudaError_t wgrid_kernel_setup(int max_smem_bytes);
+size_t wgrid_list_cap(const Geom& g, size_t nsamples);
+cudaError_t launch_wtile_items(const Geom& g, const uint32_t* bin_offset, const PlaneMeta* planes, Item* items, uint32_t* lists,
+                               uint32_t list_cap, uint32_t* nitems, uint32_t* ctl, cudaStream_t s);
+int launch_wgrid(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* lists, uint32_t list_cap, uint32_t* ctl,
+                 const uint32_t* bin_offset, const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
+                 GridPtrs grids, int num_sms, cudaStream_t s, cudaError_t* err);
 
 // ---- owner-tile path (muser_owner.cu): 2-D mode, support 7.  The grids are Hermitian (every visibility is gridded
 // with its conjugate), so only the half-plane of rows ny/2 .. ny-1 is computed and stored; k_mirror_lower rebuilds

@@ -99,7 +99,8 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                     // sample whose footprint stays below them is not gridded (its partner covers the mirror cells)
                     if (cv + h >= (g.ny >> 1)) {
                         const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
-                        o.bin = (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
+                        o.bin = g.wtile ? (uint32_t)((((long long)gid * g.nty + ty) * g.ntx + tx) * P + p)
+                                        : (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
                     }
                     if (cnt && cv >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, 1);   // NEXT-2
                 }
@@ -224,7 +225,7 @@ __global__ void __launch_bounds__(1024) k_scan_items_tops(const Geom g, const ui
         if (b < nblocks) { tops[2 * b] = carry.c + ex.c; tops[2 * b + 1] = carry.n + ex.n; }
         carry.c += total.c; carry.n += total.n;
     }
-    if (threadIdx.x == 0) { bin_offset[g.nbins] = carry.c; *nitems = carry.n; }
+    if (threadIdx.x == 0) { bin_offset[g.nbins] = carry.c; if (nitems) *nitems = carry.n; }
 }
 
 template <int SINGLE>
@@ -239,7 +240,7 @@ __global__ void __launch_bounds__(1024) k_scan_items_write(const Geom g, uint32_
     const Scan2 ex = block_scan2(t, total, s_w);
     uint32_t off = ex.c, ioff = ex.n;
     if (SINGLE) {
-        if (threadIdx.x == 0) { bin_offset[g.nbins] = total.c; *nitems = total.n; }
+        if (threadIdx.x == 0) { bin_offset[g.nbins] = total.c; if (nitems) *nitems = total.n; }
     } else {
         off += tops[2 * blockIdx.x]; ioff += tops[2 * blockIdx.x + 1];
     }
@@ -251,7 +252,7 @@ __global__ void __launch_bounds__(1024) k_scan_items_write(const Geom g, uint32_
             bin_offset[b] = off;
             if (c[j]) bin_count[b] = 0;
             const uint32_t n = (c[j] + CH - 1u) / CH;
-            for (uint32_t q = 0; q < n; ++q) {
+            for (uint32_t q = 0; items && q < n; ++q) {
                 Item it;
                 it.bin = b; it.start = off + q * CH; it.count = min(CH, c[j] - q * CH);
                 items[ioff + q] = it;
@@ -270,7 +271,8 @@ __global__ void __launch_bounds__(256) k_scatter(const Geom g, const Staged* __r
     const uint4* src = reinterpret_cast<const uint4*>(staged + i);
     const uint4 a = src[0], b = src[1];                                // a: re im wt cell ; b: phase bin rank gp
     if (b.y == kNoBin) return;
-    const uint32_t tx = b.y % (uint32_t)g.ntx, ty = (b.y / (uint32_t)g.ntx) % (uint32_t)g.nty;
+    const uint32_t tb = g.wtile ? b.y / (uint32_t)g.nplanes : b.y;          // tile-major order: plane is the minor index
+    const uint32_t tx = tb % (uint32_t)g.ntx, ty = (tb / (uint32_t)g.ntx) % (uint32_t)g.nty;
     const int cu = (int)(a.w & 0xFFFFu), cv = (int)(a.w >> 16);
     const int lx = cu - ((int)tx * kTile - kTile / 2), ly = cv - ((int)ty * kTile - kTile / 2);
     const uint32_t rx = b.x & 511u, ry = (b.x >> 9) & 511u, kc = (b.x >> 18) & 1u;

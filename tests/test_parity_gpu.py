@@ -13,7 +13,7 @@ import gpu_util as gu
 
 pytestmark = pytest.mark.gpu
 
-TILED, OWNER = binding.MUSER_STRATEGY_TILED, binding.MUSER_STRATEGY_OWNER
+TILED, OWNER, WPLANE = binding.MUSER_STRATEGY_TILED, binding.MUSER_STRATEGY_OWNER, binding.MUSER_STRATEGY_WPLANE
 
 
 @pytest.mark.parametrize("strategy", [OWNER, TILED])
@@ -253,7 +253,7 @@ def _wplane_case(n, cell, P, Q, nvis, w_max, seed, library_tables):
     return wc, sup, tabs, (uvw, freq, vis, wt)
 
 
-@pytest.mark.parametrize("strategy", [TILED])
+@pytest.mark.parametrize("strategy", [TILED, WPLANE])
 @pytest.mark.parametrize("library_tables", [False, True])
 def test_wprojection_planes_match_oracle(strategy, library_tables):
     n, cell, P, Q, w_max = 256, 60.0, 6, 16, 4000.0          # fov 4.3 deg: supports 7..17
@@ -272,6 +272,38 @@ def test_wprojection_planes_match_oracle(strategy, library_tables):
         gu.check_images(im, G_or, Gw_or, tabs[0].real, int(sup[0]), Q)
         for p_ in range(P):
             assert np.abs(im.get_table(p_).view(np.complex64) - tabs[p_]).max() <= 2e-7
+    finally:
+        im.destroy()
+
+
+@pytest.mark.parametrize("strategy", [TILED, WPLANE])
+@pytest.mark.parametrize("ngrids", [1, 3])
+def test_wprojection_every_support_class_dense_runs_and_batches(strategy, ngrids):
+    """Supports 7..31 (all three classes of the window gridder), dense uv coverage near the origin (long runs of records
+    per window, items of 4096 records split across CTAs), positive and negative w, several grids."""
+    n, cell, P, Q, w_max = 256, 60.0, 14, 8, 9000.0
+    wc, sup, tabs, (uvw, freq, vis, wt) = _wplane_case(n, cell, P, Q, 40000, w_max, 23, False)
+    assert sup.min() == 7 and sup.max() == 31 and len(set(sup.tolist())) >= 10
+    uvw = uvw.copy()
+    uvw[::2, :2] *= 0.12                                      # half of the visibilities crowd a few tiles around the origin
+    vis = (1.0 + 0.2 * vis).astype(np.complex64)              # a source at the phase centre (no w phase there) + noise: the
+                                                              # image has a real peak for the 1e-4-of-peak gate to refer to
+    gid = (np.arange(uvw.shape[0]) % ngrids).astype(np.int32) if ngrids > 1 else None
+    im = gu.make_imager(n, cell, 7, Q, strategy=strategy, ngrids=ngrids)
+    try:
+        im.set_wplanes(wc, sup, [t.astype(np.complex64) for t in tabs])
+        if gid is None:
+            im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        else:
+            im.grid_batched(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), gu.to_dev(gid))
+        G, Gw = gu.gpu_grids(im)
+        G_or, Gw_or, st_or = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, sup, tabs, wc=wc, grid_id=gid, ngrids=ngrids)
+        st = im.get_stats()
+        assert (st["n_gridded"], st["n_dropped"], st["n_flagged"]) == (st_or["n_gridded"], st_or["n_dropped"], st_or["n_flagged"])
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL
+        assert gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        if ngrids == 1:
+            gu.check_images(im, G_or, Gw_or, tabs[0].real, int(sup[0]), Q)
     finally:
         im.destroy()
 
