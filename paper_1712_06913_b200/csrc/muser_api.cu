@@ -66,6 +66,9 @@ struct muser_imager {
     uint32_t* wg_ctl = nullptr;             // work counters and list lengths of the w-plane window gridder (per window shape)
     uint32_t* wg_lists = nullptr;           // per shape: the items that hold records of it
     size_t wg_list_cap = 0;
+    cudaStream_t wg_side[7] = {};           // side streams / fork-join events of its per-shape kernels
+    cudaEvent_t wg_ev[8] = {};
+    bool wg_streams_ok = false;
     uint32_t* ow_cta_hist = nullptr;        // per binning CTA: its shared tile histogram (k_owner_count -> k_owner_scatter)
     size_t ow_cta_hist_cap = 0;
     bool weights_only = false;              // the 2x-beam child: muser_grid is called without visibilities
@@ -464,8 +467,13 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         }
         StageScope sc(h, MUSER_STAGE_GRID, s);
         cudaError_t ce = cudaSuccess;
+        if (!h->wg_streams_ok) {
+            for (int i = 0; i < 7; ++i) CU(h, cudaStreamCreateWithFlags(&h->wg_side[i], cudaStreamNonBlocking));
+            for (int i = 0; i < 8; ++i) CU(h, cudaEventCreateWithFlags(&h->wg_ev[i], cudaEventDisableTiming));
+            h->wg_streams_ok = true;
+        }
         h->n_launches += launch_wgrid(gw, h->sorted, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->wg_ctl, h->bin_offset, h->planes_d,
-                                      h->planes_h.data(), h->tables_d, gp, h->num_sms, s, &ce);
+                                      h->planes_h.data(), h->tables_d, gp, h->num_sms, s, h->wg_side, h->wg_ev, &ce);
         CU(h, ce);
         return MUSER_OK;
     }
@@ -722,6 +730,10 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
     cudaFree(h->ttp_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
     cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->wg_ctl); cudaFree(h->wg_lists); cudaFree(h->tw_d); cudaFree(h->tw_rows_d);
+    if (h->wg_streams_ok) {
+        for (int i = 0; i < 7; ++i) cudaStreamDestroy(h->wg_side[i]);
+        for (int i = 0; i < 8; ++i) cudaEventDestroy(h->wg_ev[i]);
+    }
     for (auto& ev : h->ev_used) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto& ev : h->ev_free) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete h;

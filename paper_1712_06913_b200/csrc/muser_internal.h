@@ -124,7 +124,7 @@ cudaError_t launch_wtile_items(const Geom& g, const uint32_t* bin_offset, const 
                                uint32_t list_cap, uint32_t* nitems, uint32_t* ctl, cudaStream_t s);
 int launch_wgrid(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* lists, uint32_t list_cap, uint32_t* ctl,
                  const uint32_t* bin_offset, const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
-                 GridPtrs grids, int num_sms, cudaStream_t s, cudaError_t* err);
+                 GridPtrs grids, int num_sms, cudaStream_t s, const cudaStream_t* side, const cudaEvent_t* ev, cudaError_t* err);
 
 // ---- owner-tile path (muser_owner.cu): 2-D mode, support 7.  The grids are Hermitian (every visibility is gridded
 // with its conjugate), so only the half-plane of rows ny/2 .. ny-1 is computed and stored; k_mirror_lower rebuilds

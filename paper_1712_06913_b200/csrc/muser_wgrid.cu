@@ -518,9 +518,12 @@ cudaError_t launch_wtile_items(const Geom& g, const uint32_t* bin_offset, const 
 // entries per shape list: an item is listed at most 16 times (items < 2^24 by the 2^30 bound on visibilities per call)
 size_t wgrid_list_cap(const Geom& g, size_t nsamples) { return 16 * ((size_t)g.ngrids * g.ntiles + nsamples / kWgChunk + 2); }
 
+// One launch per window shape that occurs.  side != nullptr: 7 side streams and 8 events (ev[0] forks, ev[1..7] join): the
+// kernels are persistent and of very different length, so they are enqueued on separate streams (longest first) and
+// the CTAs of the next one start as those of the previous one run out of work; all of them add into the grids atomically.
 int launch_wgrid(const Geom& g, const Sample* sorted, const Item* items, const uint32_t* lists, uint32_t list_cap, uint32_t* ctl,
                  const uint32_t* bin_offset, const PlaneMeta* planes, const PlaneMeta* planes_host, const float* tables,
-                 GridPtrs grids, int num_sms, cudaStream_t s, cudaError_t* err) {
+                 GridPtrs grids, int num_sms, cudaStream_t s, const cudaStream_t* side, const cudaEvent_t* ev, cudaError_t* err) {
     bool present[kWgShapes] = {false};
     present[7] = true;                                                // small segments of any support
     float kbmax = 1.0f;
@@ -531,14 +534,31 @@ int launch_wgrid(const Geom& g, const Sample* sorted, const Item* items, const u
         kbmax = kb > kbmax ? kb : kbmax;
     }
     int launches = 0;
+    *err = cudaSuccess;
+    if (side && (*err = cudaEventRecord(ev[0], s)) != cudaSuccess) return 0;
+    int nside = 0;
+    auto stream_for = [&](void) -> cudaStream_t {
+        if (!side || launches == 0) return s;                         // the first (longest) kernel stays on the caller's stream
+        cudaStream_t t = side[nside];
+        if (*err == cudaSuccess) *err = cudaStreamWaitEvent(t, ev[0], 0);
+        return t;
+    };
+    auto joined = [&](cudaStream_t t) {
+        if (t == s) return;
+        if (*err == cudaSuccess) *err = cudaEventRecord(ev[1 + nside], t);
+        if (*err == cudaSuccess) *err = cudaStreamWaitEvent(s, ev[1 + nside], 0);
+        ++nside;
+    };
 #define WG_LAUNCH(SHP)                                                                                                  \
     if (present[SHP]) {                                                                                                 \
-        wg_launch<SHP>(g, sorted, items, lists, list_cap, ctl, bin_offset, planes, tables, grids, kbmax, num_sms, s);  \
+        cudaStream_t t = stream_for();                                                                                  \
+        wg_launch<SHP>(g, sorted, items, lists, list_cap, ctl, bin_offset, planes, tables, grids, kbmax, num_sms, t);  \
         ++launches;                                                                                                     \
+        joined(t);                                                                                                      \
     }
-    WG_LAUNCH(0) WG_LAUNCH(1) WG_LAUNCH(2) WG_LAUNCH(3) WG_LAUNCH(4) WG_LAUNCH(5) WG_LAUNCH(6) WG_LAUNCH(7)
+    WG_LAUNCH(0) WG_LAUNCH(3) WG_LAUNCH(1) WG_LAUNCH(2) WG_LAUNCH(7) WG_LAUNCH(4) WG_LAUNCH(6) WG_LAUNCH(5)
 #undef WG_LAUNCH
-    *err = cudaGetLastError();
+    if (*err == cudaSuccess) *err = cudaGetLastError();
     return launches;
 }
 
