@@ -569,12 +569,12 @@ def bench_cfg5(args, torch, binding, shard, dist, rank, world, local):
     line = {"metric": METRIC, "value": args.steps * nvis / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": W,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": {"workload": WORKLOADS[5], "entry": "muser_grid (w-planes: generic tiled strategy)", "nvis_per_step": nvis,
+            "config": {"workload": WORKLOADS[5], "entry": "muser_grid (w-planes: MUSER_STRATEGY_WPLANE, window gridder k_wgrid<shape>)", "nvis_per_step": nvis,
                        "l2_policy": "544 MB of inputs per step stream through a 126 MB L2", "launch": "stream",
                        "plane_histogram_visibilities": hist.tolist(), "plane_supports": sup.tolist(),
                        "gridding_flop_8_sum_Np_Sp2": flop},
             "images_per_s": args.steps / (ms * 1e-3), "gpu_launches": int(launches), "clocks": sampler.result(),
-            "roofline": {"bound": "alu", "kernel": "k_grid_tiled_generic<1> (A3)", "achieved": flop / (su["grid"] * 1e-6) / 1e12,
+            "roofline": {"bound": "alu", "kernel": "k_wgrid<0..7> (A3: one kernel per window shape, overlapped on side streams; flop = 8 S_p^2 per sample of the full plane, the stored half-plane needs half of them)", "achieved": flop / (su["grid"] * 1e-6) / 1e12,
                          "peak": fpeak / 1e12, "unit": "TFLOP/s", "frac": flop / (su["grid"] * 1e-6) / fpeak, "traffic": None,
                          "peak_source": "measured in this run (muser_microbench fp32_fma_flops)", "stage_us_per_launch": su},
             "e2e": None, "cpu_baseline": None, "device_limits": limits}

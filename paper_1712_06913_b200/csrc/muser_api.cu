@@ -69,6 +69,7 @@ struct muser_imager {
     cudaStream_t wg_side[7] = {};           // side streams / fork-join events of its per-shape kernels
     cudaEvent_t wg_ev[8] = {};
     bool wg_streams_ok = false;
+    double wstep = 0.0;                     // > 0: the plane centres are the ladder p * wstep (O(1) plane search in K1)
     uint32_t* ow_cta_hist = nullptr;        // per binning CTA: its shared tile histogram (k_owner_count -> k_owner_scatter)
     size_t ow_cta_hist_cap = 0;
     bool weights_only = false;              // the 2x-beam child: muser_grid is called without visibilities
@@ -251,6 +252,14 @@ int upload_tables(muser_imager* h, const std::vector<std::vector<double>>& t64, 
             for (int j = 0; j < S; ++j)
                 for (int c = 0; c < comp; ++c)
                     dev[base + ((size_t)r * pitch + j) * comp + c] = h->tables_f32[p][((size_t)j * Q + r) * comp + c];
+    }
+    // a ladder of centres wc[p] = p * wc[1] (to rounding), strictly increasing: K1 searches three planes instead of all
+    h->wstep = 0.0;
+    if (wm && P >= 2 && wc[0] == 0.0 && wc[1] > 0.0) {
+        bool ladder = true;
+        for (int p = 1; p < P; ++p)
+            ladder = ladder && wc[p] > wc[p - 1] && std::fabs(wc[p] - (double)p * wc[1]) <= 1e-9 * wc[1];
+        if (ladder) h->wstep = wc[1];
     }
     cudaFree(h->tables_d); cudaFree(h->planes_d);
     h->tables_d = nullptr; h->planes_d = nullptr;
@@ -458,7 +467,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         }
         {
             StageScope sc(h, MUSER_STAGE_BIN, s);
-            CU(h, launch_coords(gw, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
+            CU(h, launch_coords(gw, uvw, freq, (const float2*)vis, wt, gid, nvis, h->wstep, h->planes_d, h->staged, h->bin_count,
                                 h->stats_d, h->cnt, s));
             CU(h, launch_scan_items(gw, h->bin_count, h->bin_offset, nullptr, nullptr, h->bin_tops, s));
             CU(h, launch_wtile_items(gw, h->bin_offset, h->planes_d, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->nitems_d, h->wg_ctl, s));
@@ -479,7 +488,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     }
     {
         StageScope sc(h, MUSER_STAGE_BIN, s);
-        CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->planes_d, h->staged, h->bin_count,
+        CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->wstep, h->planes_d, h->staged, h->bin_count,
                             h->stats_d, h->cnt, s));
         CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, h->bin_tops, s));
         CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));

@@ -20,115 +20,189 @@ namespace muser {
 static constexpr double kC = 299792458.0;   // m/s
 
 // ------------------------------------------------------------------------------------------------- K1
-// O1 for one axis: p = c*scale + n/2; i0 = floor(p + 0.5); r = floor((p - i0)*Q + 0.5).  Explicit _rn
-// intrinsics keep nvcc from contracting mul+add into an FMA (the oracle has none).
-__device__ __forceinline__ void cell_phase(double c_lambda, double scale, int n, int Q, double& i0, double& r) {
-    const double p = __dadd_rn(__dmul_rn(c_lambda, scale), (double)(n / 2));
-    i0 = floor(__dadd_rn(p, 0.5));
-    const double fr = __dsub_rn(p, i0);
-    r = floor(__dadd_rn(__dmul_rn(fr, (double)Q), 0.5));
+// O1 for one axis: p = xs + n/2 (xs = c_lambda * scale, already rounded); i0 = floor(p + 0.5); r = floor((p - i0)*Q + 0.5).
+// Explicit _rn intrinsics keep nvcc from contracting mul+add into an FMA (the oracle has none).  The two floors and the
+// conversions to int run in the FP64 add pipe with the 1.5 * 2^52 constant (x + M rounds x to the nearest integer, whose
+// two's complement sits in the low word; one compare turns nearest into floor): exact for |xs| < 2^31 (callers test 1e9).
+__device__ __forceinline__ void cell_phase(const double xs, const double half, const double Qd, int& i0, int& r) {
+    constexpr double M = 6755399441055744.0;
+    const double p = __dadd_rn(xs, half);
+    const double t = __dadd_rn(p, 0.5);
+    const double tm = __dadd_rn(t, M);
+    double fl = __dadd_rn(tm, -M);
+    int i = __double2loint(tm);
+    if (fl > t) { fl = __dadd_rn(fl, -1.0); --i; }
+    const double fr = __dsub_rn(p, fl);
+    const double u = __dadd_rn(__dmul_rn(fr, Qd), 0.5);
+    const double um = __dadd_rn(u, M);
+    int q = __double2loint(um);
+    if (__dadd_rn(um, -M) > u) --q;
+    i0 = i; r = q;
 }
 
+// A CTA loops over `iters` blocks of 256 visibilities (statistics reduced once per CTA).  wstep > 0: the plane centres
+// are the ladder wc[p] = p * wstep (checked on the host), so the nearest centre is looked for among the three around
+// floor(|w| / wstep + 1/2) with the same fp64 comparisons as the full scan (identical result); else all planes are scanned.
+// A sample that is not gridded (flagged, dropped, footprint below the stored half-plane) only writes its bin word.
+// Histogram: a third of a MUSER frame lands in the few bins around the uv origin, and atomics on one address serialise
+// in L2, so the CTA first counts in a shared-memory hash table (1024 slots keyed by bin, two probes; a sample that finds
+// both taken falls back to a warp-aggregated global atomic at once) and hands out CTA-local ranks; after the loop every
+// occupied slot reserves its run with ONE global atomic and the threads add the slot's base to the ranks they hold.
+constexpr int kHashSlots = 1024;
 __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __restrict__ uvw,
                                                 const double* __restrict__ freq, const float2* __restrict__ vis,
                                                 const float* __restrict__ weight, const int* __restrict__ grid_id,
-                                                const long long nvis, const PlaneMeta* __restrict__ planes,
+                                                const long long nvis, const int iters, const double wstep,
+                                                const PlaneMeta* __restrict__ planes,
                                                 Staged* __restrict__ staged, uint32_t* __restrict__ bin_count,
                                                 Stats* __restrict__ stats, int* __restrict__ cnt) {
-    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ double s_wc[kMaxPlanes];
+    __shared__ int s_sup[kMaxPlanes];
+    __shared__ uint32_t s_tag[kHashSlots], s_num[kHashSlots];
+    const int P = g.wmode ? g.nplanes : 1;
+    for (int p = threadIdx.x; p < P; p += 256) { s_wc[p] = planes[p].wc; s_sup[p] = planes[p].support; }
+    for (int i = threadIdx.x; i < kHashSlots; i += 256) { s_tag[i] = kNoBin; s_num[i] = 0u; }
+    uint32_t held[8];                                              // per sample of this thread: slot << 16 | local rank, or ~0
+    __syncthreads();
+    const long long base = (long long)blockIdx.x * 256 * iters;
+    const double hx = (double)(g.nx / 2), hy = (double)(g.ny / 2), Qd = (double)g.Q;
+    const double inv_wstep = wstep > 0.0 ? 1.0 / wstep : 0.0;
     int flagged = 0, dropped = 0, kept = 0;
     double wsum = 0.0, v2sum = 0.0, w2sum = 0.0;
-    Staged s0, s1;
-    s0.bin = s1.bin = kNoBin;
-    s0.rank = s1.rank = 0u;
-    if (k < nvis) {
-        const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
-        const double f = freq[k];
-        float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
-        const float wt = weight[k];
-        const int gid = grid_id ? grid_id[k] : 0;
-        const double il = __ddiv_rn(f, kC);
-        const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
-        const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) &&
-                        isfinite(V.y) && isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
-        if (!ok) {
-            flagged = 1;
-        } else {
-            int p = 0;
-            if (g.wmode) {                                   // O6: nearest plane centre in |w|, tie -> lower p
-                const double aw = fabs(wl);
-                double best = fabs(__dsub_rn(aw, planes[0].wc));
-                for (int q = 1; q < g.nplanes; ++q) {
-                    const double d = fabs(__dsub_rn(aw, planes[q].wc));
-                    if (d < best) { best = d; p = q; }
-                }
-            }
-            const int S = planes[p].support, h = (S - 1) >> 1;
-            double iu[2], iv[2], ru[2], rv[2];
-            bool inside = true;
-#pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                const double sgn = s ? -1.0 : 1.0;
-                cell_phase(sgn * ul, g.su, g.nx, g.Q, iu[s], ru[s]);
-                cell_phase(sgn * vl, g.sv, g.ny, g.Q, iv[s], rv[s]);
-                inside = inside && iu[s] >= (double)(h + 1) && iu[s] <= (double)(g.nx - 1 - h) &&
-                         iv[s] >= (double)(h + 1) && iv[s] <= (double)(g.ny - 1 - h);
-            }
-            if (!inside) {
-                dropped = 1;
+    for (int it = 0; it < iters; ++it) {
+        const long long k = base + (long long)it * 256 + threadIdx.x;
+        Staged s0, s1;
+        s0.bin = s1.bin = kNoBin;
+        s0.rank = s1.rank = 0u;
+        if (k < nvis) {
+            const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
+            const double f = freq[k];
+            float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
+            const float wt = weight[k];
+            const int gid = grid_id ? grid_id[k] : 0;
+            const double il = __ddiv_rn(f, kC);
+            const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
+            const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) &&
+                            isfinite(V.y) && isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
+            if (!ok) {
+                ++flagged;
             } else {
-                kept = 1;
-                if (g.phase_on) V = phase_rotate(g, um, vm, f, V);
-                wsum = 2.0 * (double)wt;
-                w2sum = (double)wt * (double)wt;
-                v2sum = w2sum * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
-                const int P = g.wmode ? g.nplanes : 1;
+                int p = 0;
+                if (g.wmode) {                                   // O6: nearest plane centre in |w|, tie -> lower p
+                    const double aw = fabs(wl);
+                    int lo = 0, hi = g.nplanes - 1;
+                    if (wstep > 0.0) {
+                        const int q0 = __double2int_rz(fmin(__dadd_rn(__dmul_rn(aw, inv_wstep), 0.5), (double)(g.nplanes - 1)));
+                        lo = max(q0 - 1, 0); hi = min(q0 + 1, g.nplanes - 1);
+                    }
+                    p = lo;
+                    double best = fabs(__dsub_rn(aw, s_wc[lo]));
+                    for (int q = lo + 1; q <= hi; ++q) {
+                        const double d = fabs(__dsub_rn(aw, s_wc[q]));
+                        if (d < best) { best = d; p = q; }
+                    }
+                }
+                const int S = s_sup[p], h = (S - 1) >> 1;
+                const double xu = __dmul_rn(ul, g.su), xv = __dmul_rn(vl, g.sv);
+                int iu[2], iv[2], ru[2], rv[2];
+                bool inside = fabs(xu) < 1.0e9 && fabs(xv) < 1.0e9;   // beyond: off any grid, and outside the int range
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
-                    Staged& o = s ? s1 : s0;
-                    const int cu = (int)iu[s], cv = (int)iv[s];
-                    const int rx = g.Q / 2 - (int)ru[s], ry = g.Q / 2 - (int)rv[s];
-                    const int kconj = g.wmode && ((s ? -wl : wl) < 0.0);
-                    o.re = wt * V.x;
-                    o.im = s ? -(wt * V.y) : wt * V.y;
-                    o.wt = wt;
-                    o.cell = (uint32_t)cu | ((uint32_t)cv << 16);
-                    o.phase = (uint32_t)rx | ((uint32_t)ry << 9) | ((uint32_t)kconj << 18);
-                    o.gp = (uint32_t)gid | ((uint32_t)p << 24);
-                    // the grids are Hermitian: only rows >= ny/2 are computed and stored ("half the grid"); a
-                    // sample whose footprint stays below them is not gridded (its partner covers the mirror cells)
-                    if (cv + h >= (g.ny >> 1)) {
-                        const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
-                        o.bin = g.wtile ? (uint32_t)((((long long)gid * g.nty + ty) * g.ntx + tx) * P + p)
-                                        : (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
+                    cell_phase(s ? -xu : xu, hx, Qd, iu[s], ru[s]);
+                    cell_phase(s ? -xv : xv, hy, Qd, iv[s], rv[s]);
+                    inside = inside && iu[s] >= h + 1 && iu[s] <= g.nx - 1 - h && iv[s] >= h + 1 && iv[s] <= g.ny - 1 - h;
+                }
+                if (!inside) {
+                    ++dropped;
+                } else {
+                    ++kept;
+                    if (g.phase_on) V = phase_rotate(g, um, vm, f, V);
+                    wsum += 2.0 * (double)wt;
+                    const double w2 = (double)wt * (double)wt;
+                    w2sum += w2;
+                    v2sum += w2 * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
+#pragma unroll
+                    for (int s = 0; s < 2; ++s) {
+                        Staged& o = s ? s1 : s0;
+                        const int cu = iu[s], cv = iv[s];
+                        const int rx = g.Q / 2 - ru[s], ry = g.Q / 2 - rv[s];
+                        const int kconj = g.wmode && ((s ? -wl : wl) < 0.0);
+                        o.re = wt * V.x;
+                        o.im = s ? -(wt * V.y) : wt * V.y;
+                        o.wt = wt;
+                        o.cell = (uint32_t)cu | ((uint32_t)cv << 16);
+                        o.phase = (uint32_t)rx | ((uint32_t)ry << 9) | ((uint32_t)kconj << 18);
+                        o.gp = (uint32_t)gid | ((uint32_t)p << 24);
+                        // the grids are Hermitian: only rows >= ny/2 are computed and stored ("half the grid"); a
+                        // sample whose footprint stays below them is not gridded (its partner covers the mirror cells)
+                        if (cv + h >= (g.ny >> 1)) {
+                            const int tx = (cu + kTile / 2) >> kTileShift, ty = (cv + kTile / 2) >> kTileShift;
+                            o.bin = g.wtile ? (uint32_t)((((long long)gid * g.nty + ty) * g.ntx + tx) * P + p)
+                                            : (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
+                        }
+                        if (cnt && cv >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, 1);   // NEXT-2
                     }
-                    if (cnt && cv >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, 1);   // NEXT-2
                 }
             }
         }
-    }
-    {
-        // warp-aggregated histogram: lanes with the same bin issue one atomic (the tile at the uv origin receives a
-        // third of a MUSER frame; per-sample atomics serialise on it)
-        const unsigned full_ = 0xffffffffu;
-        const int lane_ = threadIdx.x & 31;
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
             Staged& o = s ? s1 : s0;
-            if (!__any_sync(full_, o.bin != kNoBin)) continue;
-            const unsigned m = __match_any_sync(full_, o.bin);
-            const int leader = __ffs(m) - 1;
-            uint32_t base = 0;
-            if (o.bin != kNoBin && lane_ == leader) base = atomicAdd(&bin_count[o.bin], (uint32_t)__popc(m));
-            base = __shfl_sync(full_, base, leader);
-            o.rank = base + (uint32_t)__popc(m & ((1u << lane_) - 1u));
+            uint32_t hold = 0xFFFFFFFFu;
+            bool global_now = false;
+            if (o.bin != kNoBin) {
+                uint32_t slot = (o.bin * 2654435761u) >> 22;
+                global_now = true;
+#pragma unroll
+                for (int probe = 0; probe < 2; ++probe) {
+                    const uint32_t old = atomicCAS(&s_tag[slot], kNoBin, o.bin);
+                    if (old == kNoBin || old == o.bin) {
+                        hold = slot << 16 | atomicAdd(&s_num[slot], 1u);
+                        global_now = false;
+                        break;
+                    }
+                    slot = (slot + 1u) & (kHashSlots - 1);
+                }
+            }
+            if (it < 4) held[2 * it + s] = hold;
+            if (__any_sync(0xffffffffu, global_now)) {                // both probes taken: warp-aggregated global atomic
+                const unsigned full_ = 0xffffffffu;
+                const int lane_ = threadIdx.x & 31;
+                const uint32_t key = global_now ? o.bin : kNoBin;
+                const unsigned m = __match_any_sync(full_, key);
+                const int leader = __ffs(m) - 1;
+                uint32_t b0 = 0;
+                if (global_now && lane_ == leader) b0 = atomicAdd(&bin_count[o.bin], (uint32_t)__popc(m));
+                b0 = __shfl_sync(full_, b0, leader);
+                if (global_now) o.rank = b0 + (uint32_t)__popc(m & ((1u << lane_) - 1u));
+            }
+        }
+        if (k < nvis) {
+            uint4* dst = reinterpret_cast<uint4*>(staged + 2 * k);
+            const uint4* a = reinterpret_cast<const uint4*>(&s0);
+            const uint4* b = reinterpret_cast<const uint4*>(&s1);
+            if (s0.bin != kNoBin) dst[0] = a[0];
+            dst[1] = a[1];
+            if (s1.bin != kNoBin) dst[2] = b[0];
+            dst[3] = b[1];
         }
     }
-    if (k < nvis) {
-        uint4* dst = reinterpret_cast<uint4*>(staged + 2 * k);
-        const uint4* a = reinterpret_cast<const uint4*>(&s0);
-        const uint4* b = reinterpret_cast<const uint4*>(&s1);
-        dst[0] = a[0]; dst[1] = a[1]; dst[2] = b[0]; dst[3] = b[1];
+    // every occupied slot reserves its run in its bin; the ranks held by the threads become global
+    __syncthreads();
+    for (int i = threadIdx.x; i < kHashSlots; i += 256) {
+        const uint32_t tag = s_tag[i];
+        if (tag != kNoBin) s_num[i] = atomicAdd(&bin_count[tag], s_num[i]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+        const long long k = base + (long long)it * 256 + threadIdx.x;
+        if (it >= iters || k >= nvis) continue;
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const uint32_t hold = held[2 * it + s];
+            if (hold != 0xFFFFFFFFu) staged[2 * k + s].rank = s_num[hold >> 16] + (hold & 0xFFFFu);
+        }
     }
     // block reduction of the counters, one atomic set per block
     __shared__ int s_cnt[3][8];
@@ -269,8 +343,9 @@ __global__ void __launch_bounds__(256) k_scatter(const Geom g, const Staged* __r
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= nsamples) return;
     const uint4* src = reinterpret_cast<const uint4*>(staged + i);
-    const uint4 a = src[0], b = src[1];                                // a: re im wt cell ; b: phase bin rank gp
-    if (b.y == kNoBin) return;
+    const uint4 b = src[1];                                            // b: phase bin rank gp
+    if (b.y == kNoBin) return;                                         // (a was not written)
+    const uint4 a = src[0];                                            // a: re im wt cell
     const uint32_t tb = g.wtile ? b.y / (uint32_t)g.nplanes : b.y;          // tile-major order: plane is the minor index
     const uint32_t tx = tb % (uint32_t)g.ntx, ty = (tb / (uint32_t)g.ntx) % (uint32_t)g.nty;
     const int cu = (int)(a.w & 0xFFFFu), cv = (int)(a.w >> 16);
@@ -691,10 +766,12 @@ __global__ void __launch_bounds__(256) k_histogram(const float* __restrict__ ima
 static inline unsigned blocks_for(long long n, int per) { return (unsigned)((n + per - 1) / per); }
 
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
-                          const int* grid_id, long long nvis, const PlaneMeta* planes, Staged* staged,
+                          const int* grid_id, long long nvis, double wstep, const PlaneMeta* planes, Staged* staged,
                           uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s) {
-    k_coords<<<blocks_for(nvis, 256), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, planes, staged, bin_count,
-                                                   stats, cnt);
+    int iters = 4;                                                     // (the kernel holds the ranks of at most 4 blocks) enough CTAs to fill the machine a few times over
+    while (iters > 1 && nvis / (256 * iters) < 148 * 8) iters >>= 1;
+    k_coords<<<blocks_for(nvis, 256 * iters), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, iters, wstep, planes, staged,
+                                                           bin_count, stats, cnt);
     return cudaGetLastError();
 }
 

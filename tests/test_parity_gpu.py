@@ -276,6 +276,29 @@ def test_wprojection_planes_match_oracle(strategy, library_tables):
         im.destroy()
 
 
+def test_wprojection_unevenly_spaced_planes_take_the_full_plane_scan():
+    """Plane centres that are not a ladder p * step: K1 scans all planes (the O(1) search only applies to ladders)."""
+    n, cell, P, Q, w_max = 256, 60.0, 6, 16, 4000.0
+    wc, sup = mo.wplane_layout(n, cell, P, w_max)
+    wc = wc * (1.0 + 0.35 * np.arange(P) / P)                 # stretched: uneven spacing, still increasing
+    fov = n * cell * mo.ARCSEC
+    sup = (7 + 2 * np.floor(wc * fov * fov / 4.0 + 0.5)).astype(np.int64)
+    tabs = [mo.table_wkernel(int(S), Q, float(w), fov) for S, w in zip(sup, wc)]
+    uvw, freq, vis, wt = synth.random_visibilities(29, 3000, n, cell, margin_cells=sup.max() / 2 + 2, w_max_lambda=w_max)
+    im = gu.make_imager(n, cell, 7, Q)
+    try:
+        im.set_wplanes(wc, sup, [t.astype(np.complex64) for t in tabs])
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        G, Gw = gu.gpu_grids(im)
+        G_or, Gw_or, st_or = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, sup, tabs, wc=wc)
+        st = im.get_stats()
+        assert (st["n_gridded"], st["n_dropped"], st["n_flagged"]) == (st_or["n_gridded"], st_or["n_dropped"], st_or["n_flagged"])
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL
+        assert gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+    finally:
+        im.destroy()
+
+
 @pytest.mark.parametrize("strategy", [TILED, WPLANE])
 @pytest.mark.parametrize("ngrids", [1, 3])
 def test_wprojection_every_support_class_dense_runs_and_batches(strategy, ngrids):
