@@ -18,6 +18,7 @@ using namespace muser;
 
 static thread_local std::string g_create_error;
 static const double kArcsec = 3.14159265358979323846 / 648000.0;
+static const bool kColsTmaDefault = true;      // column pass staged by TMA unless MUSER_TUNE_COLS_TMA says otherwise (measured: DESIGN.md 5)
 
 struct StageEvent {
     cudaEvent_t a, b;
@@ -69,6 +70,8 @@ struct muser_imager {
     cudaStream_t wg_side[7] = {};           // side streams / fork-join events of its per-shape kernels
     cudaEvent_t wg_ev[8] = {};
     bool wg_streams_ok = false;
+    alignas(64) unsigned char tmap[128] = {};   // CUtensorMap of H (column pass staged by TMA)
+    bool tmap_tried = false, tmap_ok = false;
     double wstep = 0.0;                     // > 0: the plane centres are the ladder p * wstep (O(1) plane search in K1)
     uint32_t* ow_cta_hist = nullptr;        // per binning CTA: its shared tile histogram (k_owner_count -> k_owner_scatter)
     size_t ow_cta_hist_cap = 0;
@@ -131,6 +134,7 @@ bool wmode(const muser_imager* h) { return h->nplanes > 0; }
 void free_grids(muser_imager* h) {
     cudaFree(h->G); cudaFree(h->Gw); cudaFree(h->H); cudaFree(h->out_dirty); cudaFree(h->out_psf); cudaFree(h->cnt);
     cudaFree(h->peaks_d);
+    h->tmap_tried = h->tmap_ok = false;
     h->G = nullptr; h->Gw = nullptr; h->H = nullptr; h->out_dirty = h->out_psf = nullptr; h->cnt = nullptr; h->peaks_d = nullptr;
     if (h->plan_ok) { cufftDestroy(h->plan); h->plan_ok = false; }
     if (h->plan_rows_ok) { cufftDestroy(h->plan_rows); h->plan_rows_ok = false; }
@@ -555,6 +559,17 @@ int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const 
     return MUSER_OK;
 }
 
+// tensor map of H for the TMA-staged column pass (MUSER_TUNE_COLS_TMA: 0 = default, 1 = per-lane loads, 2 = TMA)
+const void* cols_tmap(muser_imager* h) {
+    const int mode = h->tune[MUSER_TUNE_COLS_TMA];
+    if (mode == 1 || (mode == 0 && !kColsTmaDefault)) return nullptr;
+    if (!h->tmap_tried) {
+        h->tmap_tried = true;
+        h->tmap_ok = fft_cols_make_tmap(h->tmap, h->H, h->nx, h->ny, h->ngrids);
+    }
+    return h->tmap_ok ? h->tmap : nullptr;
+}
+
 int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     if (!dirty && !psf) return MUSER_OK;
     h->last_stream = s;
@@ -575,7 +590,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
         if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, s));
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
         h->n_launches += 1;
         return MUSER_OK;
     }
@@ -606,7 +621,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
         if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, s));
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
         h->n_launches += 1;
         return MUSER_OK;
     }
@@ -842,6 +857,7 @@ int muser_set_tuning(muser_imager* h, int key, int value) {
     if (key < 0 || key >= MUSER_TUNE_COUNT) return fail(h, MUSER_EINVAL, "unknown tuning key");
     if (key == MUSER_TUNE_ITEM_SIZE && value != 0 && (value < 256 || value > (1 << 20))) return fail(h, MUSER_EINVAL, "item_size must be 0 (automatic) or in [256, 2^20]");
     if (key == MUSER_TUNE_BIN_ITERS && (value < 0 || value > 64)) return fail(h, MUSER_EINVAL, "bin_iters must be in [0, 64]");
+    if (key == MUSER_TUNE_COLS_TMA && (value < 0 || value > 2)) return fail(h, MUSER_EINVAL, "cols_tma must be 0, 1 or 2");
     h->tune[key] = value;
     return rebuild_geom(h);
 }

@@ -11,7 +11,10 @@
 // bank-conflict free.
 #include "muser_internal.h"
 
+#include <cuda.h>
+
 #include <algorithm>
+#include <cstring>
 
 namespace muser {
 
@@ -28,8 +31,65 @@ __device__ __forceinline__ void idft4(float2& a, float2& b, float2& c, float2& d
     d = make_float2(s1.x + s3.y, s1.y - s3.x);
 }
 
-template <int N>
-__global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_fft_cols_correct(const int nx, const float2* __restrict__ F1,
+// 16-point inverse DFT in registers: in v[i] = x[i], out v[4 b + c] = X[b + 4 c]
+__device__ __forceinline__ void idft16(float2 (&v)[16]) {
+#pragma unroll
+    for (int a = 0; a < 4; ++a) idft4(v[a], v[a + 4], v[a + 8], v[a + 12]);              // -> u[a][b] at v[a + 4 b]
+    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
+    v[1 + 4 * 1] = cmul(v[1 + 4 * 1], make_float2(c1, s1));
+    v[2 + 4 * 1] = cmul(v[2 + 4 * 1], make_float2(h, h));
+    v[3 + 4 * 1] = cmul(v[3 + 4 * 1], make_float2(s1, c1));
+    v[1 + 4 * 2] = cmul(v[1 + 4 * 2], make_float2(h, h));
+    v[2 + 4 * 2] = make_float2(-v[2 + 4 * 2].y, v[2 + 4 * 2].x);
+    v[3 + 4 * 2] = cmul(v[3 + 4 * 2], make_float2(-h, h));
+    v[1 + 4 * 3] = cmul(v[1 + 4 * 3], make_float2(s1, c1));
+    v[2 + 4 * 3] = cmul(v[2 + 4 * 3], make_float2(-h, h));
+    v[3 + 4 * 3] = cmul(v[3 + 4 * 3], make_float2(-c1, -s1));
+#pragma unroll
+    for (int b = 0; b < 4; ++b) idft4(v[4 * b], v[4 * b + 1], v[4 * b + 2], v[4 * b + 3]);
+}
+// 8-point inverse DFT in registers: in v[i] = x[i], out X[b] = v[2 b] + v[2 b + 1], X[b + 4] = v[2 b] - v[2 b + 1]
+__device__ __forceinline__ void idft8_half(float2 (&v)[8]) {
+    idft4(v[0], v[2], v[4], v[6]);
+    idft4(v[1], v[3], v[5], v[7]);
+    const float h = 0.70710678118654752f;
+    v[3] = cmul(v[3], make_float2(h, h));
+    v[5] = make_float2(-v[5].y, v[5].x);
+    v[7] = cmul(v[7], make_float2(-h, h));
+}
+
+// ---- TMA staging of the column strip (TMA = 1): the strip of 8 columns x N rows (64 bytes per row) is fetched by N / 256
+// cp.async.bulk.tensor.2d copies (box 8 columns x 256 rows) into a dense [N][8] float2 tile that ALIASES the stage
+// buffers: every thread takes its first-stage inputs from it into registers, a barrier, then the stage-1 outputs
+// overwrite it.  The load side then issues no per-lane global requests at all (the 64-byte row segments cost one L1
+// request per 4 rows otherwise).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(phase) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int N, int TMA>
+__global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_fft_cols_correct(const __grid_constant__ CUtensorMap tmap,
+                                                                               const int nx, const float2* __restrict__ F1,
                                                                                const float2* __restrict__ tw,
                                                                                const float* __restrict__ icx,
                                                                                const float* __restrict__ icy,
@@ -39,7 +99,7 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
     constexpr int T = N / 4;                   // butterflies per column and stage
     constexpr int NT = N / 2;                  // threads: thread (j, half) owns butterfly j of columns 4 half .. 4 half + 3
     constexpr int PITCH = N + N / 16 + 2;      // float4 per column pair, = 2 (mod 8)
-    extern __shared__ __align__(16) float4 sm[];
+    extern __shared__ __align__(128) float4 sm[];
     const int tid = threadIdx.x;
     const int sx0 = blockIdx.x * kFftC;        // source columns sx0 .. sx0 + 7
     const int gi = grid0 + (int)blockIdx.y;
@@ -47,7 +107,48 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
     auto pad = [](int i) { return i + (i >> 4); };
 
     constexpr int R1 = (N == 256 || N == 1024) ? 16 : 8;                                   // radix of the first stage
-    if (R1 == 8) {
+    if constexpr (TMA != 0) {
+        __shared__ __align__(8) uint64_t bar;
+        constexpr int TPT = (N / R1) * kFftC / NT;                                         // first-stage tasks per thread (1 or 2)
+        if (tid == 0) {
+            mbar_init(&bar, 1);
+            mbar_expect_tx(&bar, (uint32_t)(N * kFftC * sizeof(float2)));
+#pragma unroll
+            for (int b = 0; b < N / 256; ++b)
+                tma_load_2d(reinterpret_cast<float2*>(sm) + b * 256 * kFftC, &tmap, 2 * sx0, gi * N + b * 256, &bar);
+        }
+        __syncthreads();                                                                   // the barrier is initialised
+        mbar_wait(&bar, 0);
+        const float2* raw = reinterpret_cast<const float2*>(sm);                           // [N][8]
+        float2 v[TPT][R1];
+#pragma unroll
+        for (int t = 0; t < TPT; ++t) {
+            const int task = tid + t * NT, c = task & (kFftC - 1), j = task >> 3;
+#pragma unroll
+            for (int i = 0; i < R1; ++i) v[t][i] = raw[(j + i * (N / R1)) * kFftC + c];
+        }
+        __syncthreads();                                                                   // everyone holds its inputs: the tile may be overwritten
+#pragma unroll
+        for (int t = 0; t < TPT; ++t) {
+            const int task = tid + t * NT, c = task & (kFftC - 1), j = task >> 3;
+            float2* dst = reinterpret_cast<float2*>(sm + (c >> 1) * PITCH) + (c & 1);
+            if constexpr (R1 == 16) {
+                idft16(v[t]);
+#pragma unroll
+                for (int b = 0; b < 4; ++b)
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc) dst[2 * pad(16 * j + b + 4 * cc)] = v[t][4 * b + cc];
+            } else {
+                idft8_half(v[t]);
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const float2 p0 = v[t][2 * b], p1 = v[t][2 * b + 1];
+                    dst[2 * pad(8 * j + b)] = make_float2(p0.x + p1.x, p0.y + p1.y);
+                    dst[2 * pad(8 * j + b + 4)] = make_float2(p0.x - p1.x, p0.y - p1.y);
+                }
+            }
+        }
+    } else if (R1 == 8) {
         // ---- stage 1: radix 8, Ns = 1, straight from global memory; outputs y[8 j + i]
         for (int task = tid; task < (N / 8) * kFftC; task += NT) {
             const int c = task & (kFftC - 1), j = task >> 3;
@@ -199,33 +300,6 @@ struct RowCfg {
     static constexpr int R1 = (N == 64 || N == 256 || N == 1024 || N == 4096) ? 16 : 8;
     static constexpr size_t SMEM = (size_t)NP * PITCH * sizeof(float4);
 };
-
-// 16-point inverse DFT in registers: in v[i] = x[i], out v[4 b + c] = X[b + 4 c]
-__device__ __forceinline__ void idft16(float2 (&v)[16]) {
-#pragma unroll
-    for (int a = 0; a < 4; ++a) idft4(v[a], v[a + 4], v[a + 8], v[a + 12]);              // -> u[a][b] at v[a + 4 b]
-    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
-    v[1 + 4 * 1] = cmul(v[1 + 4 * 1], make_float2(c1, s1));
-    v[2 + 4 * 1] = cmul(v[2 + 4 * 1], make_float2(h, h));
-    v[3 + 4 * 1] = cmul(v[3 + 4 * 1], make_float2(s1, c1));
-    v[1 + 4 * 2] = cmul(v[1 + 4 * 2], make_float2(h, h));
-    v[2 + 4 * 2] = make_float2(-v[2 + 4 * 2].y, v[2 + 4 * 2].x);
-    v[3 + 4 * 2] = cmul(v[3 + 4 * 2], make_float2(-h, h));
-    v[1 + 4 * 3] = cmul(v[1 + 4 * 3], make_float2(s1, c1));
-    v[2 + 4 * 3] = cmul(v[2 + 4 * 3], make_float2(-h, h));
-    v[3 + 4 * 3] = cmul(v[3 + 4 * 3], make_float2(-c1, -s1));
-#pragma unroll
-    for (int b = 0; b < 4; ++b) idft4(v[4 * b], v[4 * b + 1], v[4 * b + 2], v[4 * b + 3]);
-}
-// 8-point inverse DFT in registers: in v[i] = x[i], out X[b] = v[2 b] + v[2 b + 1], X[b + 4] = v[2 b] - v[2 b + 1]
-__device__ __forceinline__ void idft8_half(float2 (&v)[8]) {
-    idft4(v[0], v[2], v[4], v[6]);
-    idft4(v[1], v[3], v[5], v[7]);
-    const float h = 0.70710678118654752f;
-    v[3] = cmul(v[3], make_float2(h, h));
-    v[5] = make_float2(-v[5].y, v[5].x);
-    v[7] = cmul(v[7], make_float2(-h, h));
-}
 
 template <int N, int WMODE, int UNIFORM>
 __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int ngroups, const float2* __restrict__ G,
@@ -392,10 +466,42 @@ int fft_cols_first_radix(int ny) { return (ny == 256 || ny == 1024) ? 16 : 8; }
 
 cudaError_t fft_cols_setup() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
     return cudaSuccess;
+}
+
+// Tensor map of the column pass's input F1 [ngrids * ny][nx] float2 seen as fp32 [rows][2 nx], box = 16 floats (8 columns)
+// x 256 rows, no swizzle.  `map128` = 128 bytes, 64-byte aligned.  The driver entry point is looked up at run time (the
+// library does not link libcuda).  Returns false when the map cannot be made (the per-lane load path is used then).
+bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngrids) {
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+            qres != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            return false;
+        }
+        encode = reinterpret_cast<EncodeFn>(fn);
+    }
+    const unsigned long long rows = (unsigned long long)ngrids * ny;
+    if (ny % 256 != 0 || rows >= (1ull << 32)) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)2 * nx, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)nx * sizeof(float2)};
+    const cuuint32_t box[2] = {2 * kFftC, 256};
+    const cuuint32_t estr[2] = {1, 1};
+    return encode(reinterpret_cast<CUtensorMap*>(map128), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float2*>(F1), dims, strides,
+                  box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <int N, int WMODE>
@@ -453,15 +559,20 @@ cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw
 }
 
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
-                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, cudaStream_t s) {
+                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, const void* tmap128,
+                                    cudaStream_t s) {
+    CUtensorMap map;
+    memset(&map, 0, sizeof(map));
+    if (tmap128) memcpy(&map, tmap128, sizeof(map));
     for (int grid0 = 0; grid0 < g.ngrids; grid0 += 65535) {              // gridDim.y holds at most 65535 grids
         const dim3 blocks((unsigned)(g.nx / kFftC), (unsigned)std::min(65535, g.ngrids - grid0));
-        if (g.ny == 256)
-            k_fft_cols_correct<256><<<blocks, 128, fft_smem_bytes(256), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
-        else if (g.ny == 512)
-            k_fft_cols_correct<512><<<blocks, 256, fft_smem_bytes(512), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
-        else
-            k_fft_cols_correct<1024><<<blocks, 512, fft_smem_bytes(1024), s>>>(g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+#define MUSER_COLS_CASE(NN)                                                                                                   \
+        if (tmap128) k_fft_cols_correct<NN, 1><<<blocks, NN / 2, fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0); \
+        else k_fft_cols_correct<NN, 0><<<blocks, NN / 2, fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+        if (g.ny == 256) { MUSER_COLS_CASE(256) }
+        else if (g.ny == 512) { MUSER_COLS_CASE(512) }
+        else { MUSER_COLS_CASE(1024) }
+#undef MUSER_COLS_CASE
     }
     return cudaGetLastError();
 }

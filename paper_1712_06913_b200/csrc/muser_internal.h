@@ -178,7 +178,10 @@ int fft_rows_first_radix(int nx);
 cudaError_t fft_rows_setup();
 cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
                                  Stats* stats, float2* Z, int num_sms, cudaStream_t s);
+// tmap128 != nullptr: the strip is staged by TMA (tensor map from fft_cols_make_tmap), else by per-lane loads
+bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngrids);
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
-                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, cudaStream_t s);
+                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, const void* tmap128,
+                                    cudaStream_t s);
 
 }  // namespace muser

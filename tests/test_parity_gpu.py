@@ -378,6 +378,30 @@ def test_cfg5_reduced_wprojection_4096():
         im.destroy()
 
 
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_column_pass_staged_by_tma_equals_per_lane_loads_bit_for_bit(cfg):
+    """MUSER_TUNE_COLS_TMA: the strip of the fused column transform fetched by cp.async.bulk.tensor or by per-lane loads --
+    the arithmetic after the staging is the same, so the images must be identical (ny = 256, 512, 1024; two grids)."""
+    import torch
+    fr = synth.make_frame(cfg)
+    p = fr.params
+    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample, kernel=p.kernel, ngrids=2)
+    try:
+        gid = (np.arange(fr.nvis) % 2).astype(np.int32)
+        im.grid_batched(gu.to_dev(fr.uvw_m), gu.to_dev(fr.freq_hz), gu.to_dev(fr.vis), gu.to_dev(fr.weight), gu.to_dev(gid))
+        out = {}
+        for mode in (1, 2):
+            im.set_tuning(binding.MUSER_TUNE_COLS_TMA, mode)
+            d = torch.zeros((2, p.n, p.n), device="cuda"); b = torch.zeros_like(d)
+            im.dirty_psf(d, b)
+            torch.cuda.synchronize()
+            out[mode] = (d.cpu().numpy(), b.cpu().numpy())
+        assert np.abs(out[1][0]).max() > 0
+        assert np.array_equal(out[1][0], out[2][0]) and np.array_equal(out[1][1], out[2][1])
+    finally:
+        im.destroy()
+
+
 def test_frame_host_end_to_end_equals_device_path():
     import torch
     fr = synth.make_frame(2)
