@@ -18,7 +18,8 @@
 
 namespace muser {
 
-constexpr int kFftC = 8;                       // columns per CTA
+// columns per CTA: 8 (ny <= 1024: 64-byte row segments) or 4 (ny = 2048, 4096: the strip has to fit shared memory)
+__host__ __device__ constexpr int fft_cols_per_cta(int N) { return N <= 1024 ? 8 : 4; }
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 // 4-point inverse DFT (kernel exp(+2 pi i nk/4)): in place on (a, b, c, d) -> (X0, X1, X2, X3)
@@ -88,7 +89,7 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
 }
 
 template <int N, int TMA>
-__global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_fft_cols_correct(const __grid_constant__ CUtensorMap tmap,
+__global__ void __launch_bounds__((N / 4) * (fft_cols_per_cta(N) / 4), N >= 4096 ? 1 : (N >= 1024 ? 2 : (N == 512 ? 4 : 8))) k_fft_cols_correct(const __grid_constant__ CUtensorMap tmap,
                                                                                const int nx, const float2* __restrict__ F1,
                                                                                const float2* __restrict__ tw,
                                                                                const float* __restrict__ icx,
@@ -97,7 +98,8 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
                                                                                float* __restrict__ dirty, float* __restrict__ psf,
                                                                                PeakSlot* __restrict__ peaks, const int grid0) {
     constexpr int T = N / 4;                   // butterflies per column and stage
-    constexpr int NT = N / 2;                  // threads: thread (j, half) owns butterfly j of columns 4 half .. 4 half + 3
+    constexpr int kFftC = fft_cols_per_cta(N), NH = kFftC / 4, CS = kFftC == 8 ? 3 : 2;
+    constexpr int NT = T * NH;                 // threads: thread (j, half) owns butterfly j of columns 4 half .. 4 half + 3
     constexpr int PITCH = N + N / 16 + 2;      // float4 per column pair, = 2 (mod 8)
     extern __shared__ __align__(128) float4 sm[];
     const int tid = threadIdx.x;
@@ -106,7 +108,7 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
     const size_t gbase = (size_t)gi * N * nx;
     auto pad = [](int i) { return i + (i >> 4); };
 
-    constexpr int R1 = (N == 256 || N == 1024) ? 16 : 8;                                   // radix of the first stage
+    constexpr int R1 = (N == 256 || N == 1024 || N == 4096) ? 16 : 8;                      // radix of the first stage
     if constexpr (TMA != 0) {
         __shared__ __align__(8) uint64_t bar;
         constexpr int TPT = (N / R1) * kFftC / NT;                                         // first-stage tasks per thread (1 or 2)
@@ -123,14 +125,14 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
         float2 v[TPT][R1];
 #pragma unroll
         for (int t = 0; t < TPT; ++t) {
-            const int task = tid + t * NT, c = task & (kFftC - 1), j = task >> 3;
+            const int task = tid + t * NT, c = task & (kFftC - 1), j = task >> CS;
 #pragma unroll
             for (int i = 0; i < R1; ++i) v[t][i] = raw[(j + i * (N / R1)) * kFftC + c];
         }
         __syncthreads();                                                                   // everyone holds its inputs: the tile may be overwritten
 #pragma unroll
         for (int t = 0; t < TPT; ++t) {
-            const int task = tid + t * NT, c = task & (kFftC - 1), j = task >> 3;
+            const int task = tid + t * NT, c = task & (kFftC - 1), j = task >> CS;
             float2* dst = reinterpret_cast<float2*>(sm + (c >> 1) * PITCH) + (c & 1);
             if constexpr (R1 == 16) {
                 idft16(v[t]);
@@ -151,7 +153,7 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
     } else if (R1 == 8) {
         // ---- stage 1: radix 8, Ns = 1, straight from global memory; outputs y[8 j + i]
         for (int task = tid; task < (N / 8) * kFftC; task += NT) {
-            const int c = task & (kFftC - 1), j = task >> 3;
+            const int c = task & (kFftC - 1), j = task >> CS;
             float2 v[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] = __ldg(F1 + gbase + (size_t)(j + i * (N / 8)) * nx + sx0 + c);
@@ -173,7 +175,7 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
     } else
     // ---- stage 1: radix 16, Ns = 1, straight from global memory; outputs y[16 j + i]
     for (int task = tid; task < (N / 16) * kFftC; task += NT) {
-        const int c = task & (kFftC - 1), j = task >> 3;
+        const int c = task & (kFftC - 1), j = task >> CS;
         float2 v[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) v[i] = __ldg(F1 + gbase + (size_t)(j + i * (N / 16)) * nx + sx0 + c);
@@ -204,7 +206,7 @@ __global__ void __launch_bounds__(N / 2, N == 1024 ? 2 : (N == 512 ? 4 : 8)) k_f
 
     // ---- radix-4 stages in shared memory: Ns = 16, 64, ... ; the last one (Ns = N/4) ends in registers.
     // tw[(3 stage + i - 1) T + j] = exp(+2 pi i * i * (j mod Ns) / (4 Ns)): per-stage tables in butterfly order.
-    const int j = tid >> 1, half = tid & 1;
+    const int j = tid / NH, half = tid - j * NH;
     float2 v[4][4];
     const float2* twp = tw + j;
     float4* colp = sm + 2 * half * PITCH;      // this thread's two column pairs
@@ -459,10 +461,10 @@ __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int
     }
 }
 
-static size_t fft_smem_bytes(int N) { return (size_t)(kFftC / 2) * (N + N / 16 + 2) * sizeof(float4); }
+static size_t fft_smem_bytes(int N) { return (size_t)(fft_cols_per_cta(N) / 2) * (N + N / 16 + 2) * sizeof(float4); }
 
-bool fft_cols_supported(int nx, int ny) { return (ny == 256 || ny == 512 || ny == 1024) && (nx % 16) == 0; }
-int fft_cols_first_radix(int ny) { return (ny == 256 || ny == 1024) ? 16 : 8; }
+bool fft_cols_supported(int nx, int ny) { return (ny == 256 || ny == 512 || ny == 1024 || ny == 2048 || ny == 4096) && (nx % 16) == 0; }
+int fft_cols_first_radix(int ny) { return (ny == 256 || ny == 1024 || ny == 4096) ? 16 : 8; }
 
 cudaError_t fft_cols_setup() {
     cudaError_t e;
@@ -472,6 +474,10 @@ cudaError_t fft_cols_setup() {
     if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
     if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
     if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<2048, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(2048)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<2048, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(2048)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<4096, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(4096)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<4096, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(4096)))) return e;
     return cudaSuccess;
 }
 
@@ -497,7 +503,7 @@ bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngri
     if (ny % 256 != 0 || rows >= (1ull << 32)) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)2 * nx, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {(cuuint64_t)nx * sizeof(float2)};
-    const cuuint32_t box[2] = {2 * kFftC, 256};
+    const cuuint32_t box[2] = {(cuuint32_t)(2 * fft_cols_per_cta(ny)), 256};
     const cuuint32_t estr[2] = {1, 1};
     return encode(reinterpret_cast<CUtensorMap*>(map128), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float2*>(F1), dims, strides,
                   box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -565,13 +571,15 @@ cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float
     memset(&map, 0, sizeof(map));
     if (tmap128) memcpy(&map, tmap128, sizeof(map));
     for (int grid0 = 0; grid0 < g.ngrids; grid0 += 65535) {              // gridDim.y holds at most 65535 grids
-        const dim3 blocks((unsigned)(g.nx / kFftC), (unsigned)std::min(65535, g.ngrids - grid0));
+        const dim3 blocks((unsigned)(g.nx / fft_cols_per_cta(g.ny)), (unsigned)std::min(65535, g.ngrids - grid0));
 #define MUSER_COLS_CASE(NN)                                                                                                   \
-        if (tmap128) k_fft_cols_correct<NN, 1><<<blocks, NN / 2, fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0); \
-        else k_fft_cols_correct<NN, 0><<<blocks, NN / 2, fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+        if (tmap128) k_fft_cols_correct<NN, 1><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0); \
+        else k_fft_cols_correct<NN, 0><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
         if (g.ny == 256) { MUSER_COLS_CASE(256) }
         else if (g.ny == 512) { MUSER_COLS_CASE(512) }
-        else { MUSER_COLS_CASE(1024) }
+        else if (g.ny == 1024) { MUSER_COLS_CASE(1024) }
+        else if (g.ny == 2048) { MUSER_COLS_CASE(2048) }
+        else { MUSER_COLS_CASE(4096) }
 #undef MUSER_COLS_CASE
     }
     return cudaGetLastError();

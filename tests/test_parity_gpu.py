@@ -450,10 +450,11 @@ def test_microbenchmarks_report_plausible_device_limits():
     assert mb["global_f32_red_adds"] > 1e11
 
 
-@pytest.mark.parametrize("nx,ny", [(512, 256), (256, 512), (1024, 1024), (272, 1024)])
+@pytest.mark.parametrize("nx,ny", [(512, 256), (256, 512), (1024, 1024), (272, 1024), (512, 2048), (2048, 512), (256, 4096)])
 def test_images_on_fused_and_library_fft_paths(nx, ny):
-    """ny = 256 / 1024 with nx a multiple of 16 takes the fused path (cuFFT rows + k_fft_cols_correct), everything else
-    cuFFT 2-D + k_correct; non-square grids; dirty image and beam against the oracle's O4 + O5."""
+    """ny = 256 ... 4096 (a power of two) with nx a multiple of 16 takes the fused column pass (8 columns per CTA up to 1024,
+    4 above), with the own row pass when nx is a power of two too, else cuFFT rows; non-square grids; dirty image and beam
+    against the oracle's O4 + O5."""
     import torch
     cell, Q = 30.0, 32
     n = min(nx, ny)
