@@ -141,8 +141,8 @@ int muser_grid_batched(muser_imager* h, const float* uvw_m, const double* freq_h
  *                                                          per-polarisation images)
  *                  NULL: everything onto grid 0
  * The result is that of muser_grid(_batched) on the flattened arrays (the order of the fp32 sums differs); flags, drops
- * and counters are per visibility as there.  npol <= 8.  Owner-tile strategy only (2-D mode, support 7),
- * else MUSER_EUNSUPPORTED. */
+ * and counters are per visibility as there.  npol <= 8.  Every strategy has the channelised binning kernels (owner tiles:
+ * k_rows_count / k_rows_scatter; w planes and other supports: k_coords<ROWS>). */
 enum { MUSER_POLS_SUM = 0, MUSER_POLS_SPLIT = 1 };
 int muser_grid_rows(muser_imager* h, const float* uvw_m, const double* freq_hz, const void* vis_c64, const float* weight,
                     const int* grid_id, long long nrow, int nchan, int npol, int ntime, int pol_mode, muser_stream s);

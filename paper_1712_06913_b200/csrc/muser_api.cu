@@ -398,6 +398,70 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
     return MUSER_OK;
 }
 
+// TILED and WPLANE strategies: generic binning (K1-K3) + their gridders.  n = visibilities (flat call) or elements
+// (channelised call, rows != nullptr: the polarisations of an element are summed by K1).
+int grid_generic(muser_imager* h, int strat, const float* uvw, const double* freq, const void* vis, const float* wt,
+                 const int* gid, long long nvis, const RowsShapeG* rows, cudaStream_t s) {
+    const Geom& g = h->geom;
+    GridPtrs gp = grid_ptrs(h);
+    if (strat != MUSER_STRATEGY_TILED && strat != MUSER_STRATEGY_WPLANE) return fail(h, MUSER_EUNSUPPORTED, "unknown gridding strategy");
+    if (strat == MUSER_STRATEGY_WPLANE && !wplane_capable(h))
+        return fail(h, MUSER_EUNSUPPORTED, "the w-plane window strategy needs w mode with every plane support <= 31");
+    int rc = ensure_scratch(h, nvis, s);
+    if (rc) return rc;
+    if ((rc = flush_zero(h, s))) return rc;
+    h->last_stream = s;
+    h->fft_valid = false;
+    h->lower_valid = false;                                           // like the owner path, it grids rows >= ny/2 only
+    if (strat == MUSER_STRATEGY_WPLANE) {
+        // bins ordered (grid, tile, plane); work items = <= 4096 consecutive records of one tile
+        Geom gw = g;
+        gw.wtile = 1;
+        if (!h->wg_ctl) CU(h, cudaMalloc(&h->wg_ctl, 16 * sizeof(uint32_t)));
+        const size_t list_cap = wgrid_list_cap(gw, h->sample_cap);
+        if (list_cap > h->wg_list_cap) {
+            cudaFree(h->wg_lists); h->wg_lists = nullptr; h->wg_list_cap = 0;
+            CU(h, cudaMalloc(&h->wg_lists, 8 * list_cap * sizeof(uint32_t)));
+            h->wg_list_cap = list_cap;
+        }
+        {
+            StageScope sc(h, MUSER_STAGE_BIN, s);
+            CU(h, launch_coords(gw, uvw, freq, (const float2*)vis, wt, gid, nvis, rows, h->wstep, h->planes_d, h->staged, h->bin_count,
+                                h->stats_d, h->cnt, s));
+            CU(h, launch_scan_items(gw, h->bin_count, h->bin_offset, nullptr, nullptr, h->bin_tops, s));
+            CU(h, launch_wtile_items(gw, h->bin_offset, h->planes_d, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->nitems_d, h->wg_ctl, s));
+            CU(h, launch_scatter(gw, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
+            h->n_launches += g.nbins <= 4096u ? 4 : 6;
+        }
+        StageScope sc(h, MUSER_STAGE_GRID, s);
+        cudaError_t ce = cudaSuccess;
+        if (!h->wg_streams_ok) {
+            for (int i = 0; i < 7; ++i) CU(h, cudaStreamCreateWithFlags(&h->wg_side[i], cudaStreamNonBlocking));
+            for (int i = 0; i < 8; ++i) CU(h, cudaEventCreateWithFlags(&h->wg_ev[i], cudaEventDisableTiming));
+            h->wg_streams_ok = true;
+        }
+        h->n_launches += launch_wgrid(gw, h->sorted, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->wg_ctl, h->bin_offset, h->planes_d,
+                                      h->planes_h.data(), h->tables_d, gp, h->num_sms, s, h->wg_side, h->wg_ev, &ce);
+        CU(h, ce);
+        return MUSER_OK;
+    }
+    {
+        StageScope sc(h, MUSER_STAGE_BIN, s);
+        CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, rows, h->wstep, h->planes_d, h->staged, h->bin_count,
+                            h->stats_d, h->cnt, s));
+        CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, h->bin_tops, s));
+        CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
+        h->n_launches += g.nbins <= 4096u ? 3 : 5;
+    }
+    {
+        StageScope sc(h, MUSER_STAGE_GRID, s);
+        CU(h, launch_grid_tiled(g, h->sorted, h->items, h->nitems_d, h->planes_d, h->planes_h.data(), h->tables_d,
+                                gp, h->num_sms, s));
+        h->n_launches += 1;
+    }
+    return MUSER_OK;
+}
+
 int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void* vis, const float* wt,
               const int* gid, long long nvis, cudaStream_t s) {
     if (nvis < 0 || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "nvis out of range [0, 2^30]");
@@ -449,62 +513,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         h->lower_valid = false;                                       // rows < ny/2 are rebuilt on demand (ensure_lower)
         return MUSER_OK;
     }
-    if (strat != MUSER_STRATEGY_TILED && strat != MUSER_STRATEGY_WPLANE) return fail(h, MUSER_EUNSUPPORTED, "unknown gridding strategy");
-    if (strat == MUSER_STRATEGY_WPLANE && !wplane_capable(h))
-        return fail(h, MUSER_EUNSUPPORTED, "the w-plane window strategy needs w mode with every plane support <= 31");
-    int rc = ensure_scratch(h, nvis, s);
-    if (rc) return rc;
-    if ((rc = flush_zero(h, s))) return rc;
-    h->last_stream = s;
-    h->fft_valid = false;
-    h->lower_valid = false;                                           // like the owner path, it grids rows >= ny/2 only
-    if (strat == MUSER_STRATEGY_WPLANE) {
-        // bins ordered (grid, tile, plane); work items = <= 4096 consecutive records of one tile
-        Geom gw = g;
-        gw.wtile = 1;
-        if (!h->wg_ctl) CU(h, cudaMalloc(&h->wg_ctl, 16 * sizeof(uint32_t)));
-        const size_t list_cap = wgrid_list_cap(gw, h->sample_cap);
-        if (list_cap > h->wg_list_cap) {
-            cudaFree(h->wg_lists); h->wg_lists = nullptr; h->wg_list_cap = 0;
-            CU(h, cudaMalloc(&h->wg_lists, 8 * list_cap * sizeof(uint32_t)));
-            h->wg_list_cap = list_cap;
-        }
-        {
-            StageScope sc(h, MUSER_STAGE_BIN, s);
-            CU(h, launch_coords(gw, uvw, freq, (const float2*)vis, wt, gid, nvis, h->wstep, h->planes_d, h->staged, h->bin_count,
-                                h->stats_d, h->cnt, s));
-            CU(h, launch_scan_items(gw, h->bin_count, h->bin_offset, nullptr, nullptr, h->bin_tops, s));
-            CU(h, launch_wtile_items(gw, h->bin_offset, h->planes_d, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->nitems_d, h->wg_ctl, s));
-            CU(h, launch_scatter(gw, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
-            h->n_launches += g.nbins <= 4096u ? 4 : 6;
-        }
-        StageScope sc(h, MUSER_STAGE_GRID, s);
-        cudaError_t ce = cudaSuccess;
-        if (!h->wg_streams_ok) {
-            for (int i = 0; i < 7; ++i) CU(h, cudaStreamCreateWithFlags(&h->wg_side[i], cudaStreamNonBlocking));
-            for (int i = 0; i < 8; ++i) CU(h, cudaEventCreateWithFlags(&h->wg_ev[i], cudaEventDisableTiming));
-            h->wg_streams_ok = true;
-        }
-        h->n_launches += launch_wgrid(gw, h->sorted, h->items, h->wg_lists, (uint32_t)h->wg_list_cap, h->wg_ctl, h->bin_offset, h->planes_d,
-                                      h->planes_h.data(), h->tables_d, gp, h->num_sms, s, h->wg_side, h->wg_ev, &ce);
-        CU(h, ce);
-        return MUSER_OK;
-    }
-    {
-        StageScope sc(h, MUSER_STAGE_BIN, s);
-        CU(h, launch_coords(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->wstep, h->planes_d, h->staged, h->bin_count,
-                            h->stats_d, h->cnt, s));
-        CU(h, launch_scan_items(g, h->bin_count, h->bin_offset, h->items, h->nitems_d, h->bin_tops, s));
-        CU(h, launch_scatter(g, h->staged, 2 * nvis, h->bin_offset, h->sorted, s));
-        h->n_launches += g.nbins <= 4096u ? 3 : 5;
-    }
-    {
-        StageScope sc(h, MUSER_STAGE_GRID, s);
-        CU(h, launch_grid_tiled(g, h->sorted, h->items, h->nitems_d, h->planes_d, h->planes_h.data(), h->tables_d,
-                                gp, h->num_sms, s));
-        h->n_launches += 1;
-    }
-    return MUSER_OK;
+    return grid_generic(h, strat, uvw, freq, vis, wt, gid, nvis, nullptr, s);
 }
 
 // NEXT-1: the channelised call.  Owner-tile strategy only (2-D mode, support 7): its binning kernels have the rows variant.
@@ -518,11 +527,21 @@ int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const 
     if (nrow > (1LL << 30) || nvis > (1LL << 30)) return fail(h, MUSER_EINVAL, "too many visibilities in one call (2^30)");
     if (nvis == 0) return MUSER_OK;
     if (!uvw || !freq || !wt || (!vis && !h->weights_only)) return fail(h, MUSER_EINVAL, "null input pointer");
-    if (pick_strategy(h) != MUSER_STRATEGY_OWNER || !owner_capable(h))
-        return fail(h, MUSER_EUNSUPPORTED, "muser_grid_rows needs the owner-tile strategy (2-D mode, support 7)");
     const Geom& g = h->geom;
     const int split = pol_mode == MUSER_POLS_SPLIT ? 1 : 0;
     const long long nelem = split ? nvis : nvis / npol;
+    int strat = pick_strategy(h);
+    if (strat == MUSER_STRATEGY_OWNER && !owner_capable(h))
+        return fail(h, MUSER_EUNSUPPORTED, "the owner-tile strategy needs 2-D mode and support 7");
+    if (strat != MUSER_STRATEGY_OWNER) {
+        // w planes / other supports: the generic binning kernel has the channelised variant, the rest of the path is the flat one
+        if (strat == MUSER_STRATEGY_WPLANE && (unsigned long long)h->ngrids * g.ntiles + (unsigned long long)nelem / 2048 + 2 >= (1ull << 24)) {
+            if (h->strategy != MUSER_STRATEGY_AUTO) return fail(h, MUSER_EUNSUPPORTED, "too many tiles for the w-plane window strategy");
+            strat = MUSER_STRATEGY_TILED;
+        }
+        const RowsShapeG sh = {ntime, split ? npol : 1, split ? 1 : npol, nchan, (int)nrow};
+        return grid_generic(h, strat, uvw, freq, vis, wt, gid, nelem, &sh, s);
+    }
     const uint32_t item_size = owner_item_size(nelem, h->num_sms, h->tune[MUSER_TUNE_ITEM_SIZE]);
     uint32_t max_items = 0;
     int rc = ensure_owner_scratch(h, nelem, item_size, &max_items, s);

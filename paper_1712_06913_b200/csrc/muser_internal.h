@@ -96,9 +96,12 @@ __device__ __forceinline__ float peak_unordered(unsigned int o) {
 }
 
 // ---- launch wrappers (muser_kernels.cu); all asynchronous on `s` -------------------------------------------
-// wstep > 0: the plane centres are exactly the ladder p * wstep (the nearest plane is then found in O(1))
+// channelised input of the generic binning kernel: elements (t, po, c, r), npi polarisations summed per element
+struct RowsShapeG { int ntime, npo, npi, nchan, nrow; };
+// nvis: visibilities (flat call, rows == nullptr) or elements (rows call).  wstep > 0: the plane centres are exactly the
+// ladder p * wstep (the nearest plane is then found in O(1))
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
-                          const int* grid_id, long long nvis, double wstep, const PlaneMeta* planes, Staged* staged,
+                          const int* grid_id, long long nvis, const RowsShapeG* rows, double wstep, const PlaneMeta* planes, Staged* staged,
                           uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s);
 // items == nullptr: offsets only (the caller builds its own work items from them)
 cudaError_t launch_scan_items(const Geom& g, uint32_t* bin_count, uint32_t* bin_offset, Item* items,

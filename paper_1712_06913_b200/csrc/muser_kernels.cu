@@ -48,8 +48,14 @@ __device__ __forceinline__ void cell_phase(const double xs, const double half, c
 // in L2, so the CTA first counts in a shared-memory hash table (1024 slots keyed by bin, two probes; a sample that finds
 // both taken falls back to a warp-aggregated global atomic at once) and hands out CTA-local ranks; after the loop every
 // occupied slot reserves its run with ONE global atomic and the threads add the slot's base to the ranks they hold.
+// ROWS (NEXT-1, the channelised call): the unit of work is an ELEMENT (t, po, c, r) -- one baseline at one
+// channel -- in the order of the flat layout; uvw_m [ntime][nrow][3], freq_hz [nchan], vis / weight [ntime][npol][nchan][nrow],
+// grid_id [ntime][npo][nchan].  Its npi polarisations po + pi share the coordinates; they are flagged / dropped / kept one
+// by one (counters per visibility, as in the flat call) and the kept ones are added up BEFORE gridding (npo = 1: all the
+// polarisations of a channel go onto one grid) -- same cells and kernel values, only the order of the fp32 sums differs.
 constexpr int kHashSlots = 1024;
-__global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __restrict__ uvw,
+template <int ROWS>
+__global__ void __launch_bounds__(256) k_coords(const Geom g, const RowsShapeG sh, const float* __restrict__ uvw,
                                                 const double* __restrict__ freq, const float2* __restrict__ vis,
                                                 const float* __restrict__ weight, const int* __restrict__ grid_id,
                                                 const long long nvis, const int iters, const double wstep,
@@ -75,18 +81,51 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
         s0.bin = s1.bin = kNoBin;
         s0.rank = s1.rank = 0u;
         if (k < nvis) {
-            const float um = uvw[3 * k + 0], vm = uvw[3 * k + 1], wm = uvw[3 * k + 2];
-            const double f = freq[k];
-            float2 V = vis ? vis[k] : make_float2(0.f, 0.f);
-            const float wt = weight[k];
-            const int gid = grid_id ? grid_id[k] : 0;
+            float um, vm, wm;
+            double f;
+            int gid, npi = 1;
+            size_t k0 = (size_t)k, kstep = 0;                         // index of the first polarisation's value, stride to the next
+            if (ROWS) {
+                const int r = (int)(k % sh.nrow);
+                const long long q = k / sh.nrow;
+                const int c = (int)(q % sh.nchan);
+                const long long tp = q / sh.nchan;
+                const int po = (int)(tp % sh.npo), t = (int)(tp / sh.npo);
+                const size_t ub = ((size_t)t * sh.nrow + r) * 3;
+                um = uvw[ub]; vm = uvw[ub + 1]; wm = uvw[ub + 2];
+                f = freq[c];
+                gid = grid_id ? grid_id[((size_t)t * sh.npo + po) * sh.nchan + c] : 0;
+                npi = sh.npi;
+                kstep = (size_t)sh.nchan * sh.nrow;
+                k0 = (((size_t)t * sh.npo * sh.npi + po) * sh.nchan + c) * sh.nrow + r;
+            } else {
+                um = uvw[3 * k + 0]; vm = uvw[3 * k + 1]; wm = uvw[3 * k + 2];
+                f = freq[k];
+                gid = grid_id ? grid_id[k] : 0;
+            }
             const double il = __ddiv_rn(f, kC);
             const double ul = __dmul_rn((double)um, il), vl = __dmul_rn((double)vm, il), wl = __dmul_rn((double)wm, il);
-            const bool ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(wt) && isfinite(V.x) &&
-                            isfinite(V.y) && isfinite(f) && wt > 0.0f && gid >= 0 && gid < g.ngrids;
-            if (!ok) {
-                ++flagged;
-            } else {
+            const bool geom_ok = isfinite(ul) && isfinite(vl) && isfinite(wl) && isfinite(f) && gid >= 0 && gid < g.ngrids;
+            // the polarisations of the element (one in the flat call): flag each, add the others up
+            float2 V = make_float2(0.f, 0.f);                        // sum of wt * V (phase-rotated) over the unflagged ones
+            float wt = 0.f;                                           // sum of their weights
+            int nok = 0;
+            double e_wsum = 0.0, e_w2 = 0.0, e_v2 = 0.0;
+            for (int pi = 0; pi < npi; ++pi) {
+                const size_t kk = k0 + pi * kstep;
+                float2 Vp = vis ? vis[kk] : make_float2(0.f, 0.f);
+                const float wp = weight[kk];
+                if (!(geom_ok && isfinite(wp) && isfinite(Vp.x) && isfinite(Vp.y) && wp > 0.0f)) { ++flagged; continue; }
+                ++nok;
+                e_wsum += 2.0 * (double)wp;
+                const double w2 = (double)wp * (double)wp;
+                e_w2 += w2;
+                e_v2 += w2 * ((double)Vp.x * (double)Vp.x + (double)Vp.y * (double)Vp.y);
+                if (g.phase_on) Vp = phase_rotate(g, um, vm, f, Vp);
+                if (ROWS) { V.x += wp * Vp.x; V.y += wp * Vp.y; wt += wp; }
+                else { V = make_float2(wp * Vp.x, wp * Vp.y); wt = wp; }
+            }
+            if (nok) {
                 int p = 0;
                 if (g.wmode) {                                   // O6: nearest plane centre in |w|, tie -> lower p
                     const double aw = fabs(wl);
@@ -113,22 +152,18 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                     inside = inside && iu[s] >= h + 1 && iu[s] <= g.nx - 1 - h && iv[s] >= h + 1 && iv[s] <= g.ny - 1 - h;
                 }
                 if (!inside) {
-                    ++dropped;
+                    dropped += nok;
                 } else {
-                    ++kept;
-                    if (g.phase_on) V = phase_rotate(g, um, vm, f, V);
-                    wsum += 2.0 * (double)wt;
-                    const double w2 = (double)wt * (double)wt;
-                    w2sum += w2;
-                    v2sum += w2 * ((double)V.x * (double)V.x + (double)V.y * (double)V.y);
+                    kept += nok;
+                    wsum += e_wsum; w2sum += e_w2; v2sum += e_v2;
 #pragma unroll
                     for (int s = 0; s < 2; ++s) {
                         Staged& o = s ? s1 : s0;
                         const int cu = iu[s], cv = iv[s];
                         const int rx = g.Q / 2 - ru[s], ry = g.Q / 2 - rv[s];
                         const int kconj = g.wmode && ((s ? -wl : wl) < 0.0);
-                        o.re = wt * V.x;
-                        o.im = s ? -(wt * V.y) : wt * V.y;
+                        o.re = V.x;
+                        o.im = s ? -V.y : V.y;
                         o.wt = wt;
                         o.cell = (uint32_t)cu | ((uint32_t)cv << 16);
                         o.phase = (uint32_t)rx | ((uint32_t)ry << 9) | ((uint32_t)kconj << 18);
@@ -140,7 +175,7 @@ __global__ void __launch_bounds__(256) k_coords(const Geom g, const float* __res
                             o.bin = g.wtile ? (uint32_t)((((long long)gid * g.nty + ty) * g.ntx + tx) * P + p)
                                             : (uint32_t)((((long long)gid * P + p) * g.nty + ty) * g.ntx + tx);
                         }
-                        if (cnt && cv >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, 1);   // NEXT-2
+                        if (cnt && cv >= (g.ny >> 1)) atomicAdd(cnt + ((size_t)gid * g.ny + cv) * g.nx + cu, nok);   // NEXT-2: one hit per visibility
                     }
                 }
             }
@@ -766,12 +801,14 @@ __global__ void __launch_bounds__(256) k_histogram(const float* __restrict__ ima
 static inline unsigned blocks_for(long long n, int per) { return (unsigned)((n + per - 1) / per); }
 
 cudaError_t launch_coords(const Geom& g, const float* uvw, const double* freq, const float2* vis, const float* wt,
-                          const int* grid_id, long long nvis, double wstep, const PlaneMeta* planes, Staged* staged,
-                          uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s) {
+                          const int* grid_id, long long nvis, const RowsShapeG* rows, double wstep, const PlaneMeta* planes,
+                          Staged* staged, uint32_t* bin_count, Stats* stats, int* cnt, cudaStream_t s) {
     int iters = 4;                                                     // (the kernel holds the ranks of at most 4 blocks) enough CTAs to fill the machine a few times over
     while (iters > 1 && nvis / (256 * iters) < 148 * 8) iters >>= 1;
-    k_coords<<<blocks_for(nvis, 256 * iters), 256, 0, s>>>(g, uvw, freq, vis, wt, grid_id, nvis, iters, wstep, planes, staged,
-                                                           bin_count, stats, cnt);
+    if (rows) k_coords<1><<<blocks_for(nvis, 256 * iters), 256, 0, s>>>(g, *rows, uvw, freq, vis, wt, grid_id, nvis, iters, wstep, planes, staged,
+                                                                       bin_count, stats, cnt);
+    else k_coords<0><<<blocks_for(nvis, 256 * iters), 256, 0, s>>>(g, RowsShapeG{}, uvw, freq, vis, wt, grid_id, nvis, iters, wstep, planes, staged,
+                                                                   bin_count, stats, cnt);
     return cudaGetLastError();
 }
 

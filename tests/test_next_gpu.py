@@ -243,8 +243,9 @@ def _rows_inputs(cfg, ntime, seed=0):
     return p, uvw, freq, vis.astype(np.complex64), wt
 
 
+@pytest.mark.parametrize("strategy", [binding.MUSER_STRATEGY_AUTO, TILED])
 @pytest.mark.parametrize("mode", ["sum_one_grid", "sum_per_time_channel", "split"])
-def test_channelised_rows_call_equals_the_oracle_on_the_flattened_arrays(mode):
+def test_channelised_rows_call_equals_the_oracle_on_the_flattened_arrays(mode, strategy):
     import torch
     ntime = 2
     p, uvw, freq, vis, wt = _rows_inputs(2, ntime)
@@ -262,7 +263,7 @@ def test_channelised_rows_call_equals_the_oracle_on_the_flattened_arrays(mode):
     else:
         gid, split = (np.arange(ntime * npol * nchan) % 6).reshape(ntime, npol, nchan).astype(np.int32), True
         ngrids = 6
-    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample, ngrids=ngrids)
+    im = gu.make_imager(p.n, p.cell_arcsec, p.support, p.oversample, ngrids=ngrids, strategy=strategy)
     try:
         im.set_weighting(binding.MUSER_WEIGHT_UNIFORM)       # the hit counts check the per-visibility bookkeeping too
         im.reset()
@@ -288,6 +289,47 @@ def test_channelised_rows_call_equals_the_oracle_on_the_flattened_arrays(mode):
         im.grid_rows(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), None if gid is None else gu.to_dev(gid),
                      binding.MUSER_POLS_SPLIT if split else binding.MUSER_POLS_SUM)
         gu.check_images(im, G_or, Gw_or, T, p.support, p.oversample)
+    finally:
+        im.destroy()
+
+
+@pytest.mark.parametrize("split", [False, True])
+def test_channelised_rows_call_with_w_planes(split):
+    """muser_grid_rows in w mode (generic binning kernel k_coords<ROWS> + the w-plane window gridder): polarisations summed
+    before gridding or split over grids, flags in single polarisations, against the oracle on the flattened arrays."""
+    n, cell, P, Q, w_max = 256, 60.0, 6, 16, 4000.0
+    wc, sup = mo.wplane_layout(n, cell, P, w_max)
+    fov = n * cell * mo.ARCSEC
+    tabs = [mo.table_wkernel(int(S), Q, float(w), fov) for S, w in zip(sup, wc)]
+    ntime, npol, nchan, nrow = 2, 2, 4, 700
+    rng = np.random.default_rng(77)
+    uvw = np.stack([synth.random_visibilities(40 + t, nrow, n, cell, margin_cells=sup.max() / 2 + 2, w_max_lambda=w_max)[0]
+                    for t in range(ntime)]).astype(np.float32)
+    freq = 1.0e9 * (1.0 + 0.01 * np.arange(nchan))
+    vis = (1.0 + 0.2 * (rng.standard_normal((ntime, npol, nchan, nrow)) + 1j * rng.standard_normal((ntime, npol, nchan, nrow)))).astype(np.complex64)
+    wt = rng.uniform(0.5, 1.5, vis.shape).astype(np.float32)
+    wt[0, 1, 2, 5] = 0.0
+    vis[1, 0, 3, 9] = complex(np.nan, 0.0)
+    if split:
+        gid, ngrids = (np.arange(ntime * npol * nchan) % 3).reshape(ntime, npol, nchan).astype(np.int32), 3
+    else:
+        gid, ngrids = None, 1
+    im = gu.make_imager(n, cell, 7, Q, ngrids=ngrids)
+    try:
+        im.set_wplanes(wc, sup, [t.astype(np.complex64) for t in tabs])
+        im.grid_rows(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), None if gid is None else gu.to_dev(gid),
+                     binding.MUSER_POLS_SPLIT if split else binding.MUSER_POLS_SUM)
+        fu, ff, fv, fw = mo.grid_rows_inputs(uvw, freq, vis, wt)
+        fg = mo.rows_grid_ids(gid, ntime, npol, nchan, nrow, split)
+        G_or, Gw_or, st = oc.grid(fu, ff, fv, fw, n, n, cell, Q, sup, tabs, wc=wc, grid_id=fg, ngrids=ngrids)
+        got = im.get_stats()
+        assert (got["n_gridded"], got["n_dropped"], got["n_flagged"]) == (st["n_gridded"], st["n_dropped"], st["n_flagged"])
+        assert st["n_flagged"] == 2
+        assert abs(got["sum_weights"] - st["sum_weights"]) <= 1e-9 * st["sum_weights"]
+        G, Gw = gu.gpu_grids(im)
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL and gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        if not split:
+            gu.check_images(im, G_or, Gw_or, tabs[0].real, int(sup[0]), Q)
     finally:
         im.destroy()
 
