@@ -53,10 +53,10 @@ enum { MUSER_KERNEL_PSWF = 0, MUSER_KERNEL_GAUSS = 1 };
  * AUTO picks OWNER where it applies, else WPLANE where it applies, else TILED.  (Value 1 was a per-sample
  * global-reduction strategy; it missed the image tolerance on dense grids and was removed.) */
 enum { MUSER_STRATEGY_AUTO = 0, MUSER_STRATEGY_TILED = 2, MUSER_STRATEGY_OWNER = 3, MUSER_STRATEGY_WPLANE = 4 };
-/* stage ids of muser_get_profile.  On the fused imaging path (ny = 256, 512, 1024 and nx a multiple of 16) FFT is
- * cuFFT's row pass and CORRECT the library's own column transform with the shift/correction epilogue; otherwise FFT
- * is cuFFT's 2-D transform and CORRECT the stand-alone correction kernel.  PACK only runs when the gridder has not
- * already written the FFT input (accumulating calls, generic strategies). */
+/* stage ids of muser_get_profile.  On the fused imaging path (ny = 256 ... 4096 a power of two, nx a multiple of 16) FFT is
+ * the row pass (the library's own on the stored half-plane when nx is a power of two in [64, 4096], else cuFFT's on the
+ * packed grid) and CORRECT the library's own column transform with the shift/correction epilogue; otherwise FFT is
+ * cuFFT's 2-D transform and CORRECT the stand-alone correction kernel.  PACK only runs on the cuFFT paths. */
 enum { MUSER_STAGE_BIN = 0, MUSER_STAGE_GRID = 1, MUSER_STAGE_PACK = 2, MUSER_STAGE_FFT = 3, MUSER_STAGE_CORRECT = 4,
        MUSER_STAGE_COUNT = 5 };
 
