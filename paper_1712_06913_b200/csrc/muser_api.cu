@@ -853,9 +853,16 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
     }
     h->nplanes = nplanes;
     int rc = rebuild_geom(h);
-    if (rc) return rc;
-    if ((rc = upload_tables(h, t64, sup, wc))) return rc;
-    return alloc_grids(h);
+    if (!rc) rc = upload_tables(h, t64, sup, wc);
+    if (!rc) rc = alloc_grids(h);
+    if (rc) {
+        // do not leave the handle half-way (w mode with the 2-D beam grid or the old tables): fall back to 2-D mode
+        const std::string why = h->err;
+        h->nplanes = 0;
+        if (rebuild_geom(h) == MUSER_OK && build_2d_tables(h) == MUSER_OK) alloc_grids(h);
+        h->err = why + " (the handle is back in 2-D mode)";
+    }
+    return rc;
 }
 
 int muser_set_strategy(muser_imager* h, int strategy) {

@@ -1127,15 +1127,20 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                     if (p + 32 + lane < e) { nidx = sI[p + 32 + lane]; nxt = __ldg(src + (nidx & 0xFFFu)); }
                     const uint4* __restrict__ q = wb + buf * 32;
                     int j = 0;
+                    uint4 st = q[0];
                     while (j < m) {
                         const bool closes = ends != 0u;
                         const int len = closes ? __ffs(ends) : m - j;  // records j .. j + len - 1 share one window
                         if (!open) ow_window(A, __shfl_sync(kFull, mykey, j), r, c);
+                        j += len;
 #pragma unroll 2
-                        for (int t = 0; t < len; ++t) ow_add(A, q[j + t], tbx, tby);
+                        for (int t = len; t > 0; --t) {                // the next record is fetched before this one's FMAs
+                            const uint4 cur = st;
+                            st = q[min(j - t + 1, 31)];
+                            ow_add(A, cur, tbx, tby);
+                        }
                         if (closes) ow_flush(A, sA, sB);
                         open = !closes;
-                        j += len;
                         ends = len < 32 ? ends >> len : 0u;
                     }
                     buf ^= 1;
