@@ -77,6 +77,8 @@ struct muser_imager {
     size_t ow_cta_hist_cap = 0;
     bool weights_only = false;              // the 2x-beam child: muser_grid is called without visibilities
     bool zero_pending = false;              // muser_reset was called and the grids have not been zeroed yet
+    uint32_t* ow_valid = nullptr;           // owner path: per (grid, tile) flag, 0 = not written since the last reset (stands for zeros)
+    bool sparse = false;                    // some flags may be 0: G, Gw are not dense (flush_zero makes them so)
     bool lower_valid = true;                // rows 0 .. ny/2-1 of G, Gw are up to date (the owner gridder stores rows >= ny/2 only)
     cufftHandle plan = 0, plan_rows = 0;
     bool plan_ok = false, plan_rows_ok = false, fft_valid = false;
@@ -133,7 +135,7 @@ bool wmode(const muser_imager* h) { return h->nplanes > 0; }
 
 void free_grids(muser_imager* h) {
     cudaFree(h->G); cudaFree(h->Gw); cudaFree(h->H); cudaFree(h->out_dirty); cudaFree(h->out_psf); cudaFree(h->cnt);
-    cudaFree(h->peaks_d);
+    cudaFree(h->peaks_d); cudaFree(h->ow_valid); h->ow_valid = nullptr;
     h->tmap_tried = h->tmap_ok = false;
     h->G = nullptr; h->Gw = nullptr; h->H = nullptr; h->out_dirty = h->out_psf = nullptr; h->cnt = nullptr; h->peaks_d = nullptr;
     if (h->plan_ok) { cufftDestroy(h->plan); h->plan_ok = false; }
@@ -193,6 +195,12 @@ int alloc_grids(muser_imager* h) {
         CU(h, cudaMalloc(&h->cnt, nc * sizeof(int)));
         CU(h, cudaMemset(h->cnt, 0, nc * sizeof(int)));
     }
+    {
+        const size_t nb = ((size_t)h->geom.onbins + 8) & ~(size_t)3;
+        CU(h, cudaMalloc(&h->ow_valid, nb * sizeof(uint32_t)));
+        CU(h, cudaMemset(h->ow_valid, 0xFF, nb * sizeof(uint32_t)));  // the grids are zeroed and dense
+    }
+    h->sparse = false;
     CU(h, cudaMalloc(&h->peaks_d, (size_t)h->ngrids * sizeof(PeakSlot)));
     CU(h, cudaMemset(h->peaks_d, 0, (size_t)h->ngrids * sizeof(PeakSlot)));
     CU(h, cudaDeviceSynchronize());
@@ -202,18 +210,29 @@ int alloc_grids(muser_imager* h) {
     return MUSER_OK;
 }
 
+GridPtrs grid_ptrs(const muser_imager* h) { return GridPtrs{h->G, h->Gw, h->cnt}; }
+
 // the lazily deferred part of muser_reset: zero the grids now (every consumer but the owner-tile gridder needs it)
 int flush_zero(muser_imager* h, cudaStream_t s) {
-    if (!h->zero_pending) return MUSER_OK;
-    const size_t nc = grid_cells(h);
-    CU(h, cudaMemsetAsync(h->G, 0, nc * sizeof(float2), s));
-    CU(h, cudaMemsetAsync(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), s));
-    h->zero_pending = false;
-    h->lower_valid = true;
+    if (h->zero_pending) {
+        const size_t nc = grid_cells(h);
+        CU(h, cudaMemsetAsync(h->G, 0, nc * sizeof(float2), s));
+        CU(h, cudaMemsetAsync(h->Gw, 0, nc * (wmode(h) ? sizeof(float2) : sizeof(float)), s));
+        CU(h, cudaMemsetAsync(h->ow_valid, 0xFF, (((size_t)h->geom.onbins + 8) & ~(size_t)3) * sizeof(uint32_t), s));
+        h->zero_pending = false;
+        h->sparse = false;
+        h->lower_valid = true;
+        return MUSER_OK;
+    }
+    if (h->sparse) {
+        // the owner gridder left the tiles it did not write untouched (flag 0 = zeros): make the stored half-plane dense
+        CU(h, launch_owner_fill_invalid(h->geom, grid_ptrs(h), h->ow_valid, s));
+        h->n_launches += 1;
+        h->sparse = false;
+    }
     return MUSER_OK;
 }
 
-GridPtrs grid_ptrs(const muser_imager* h) { return GridPtrs{h->G, h->Gw, h->cnt}; }
 
 // rebuild rows 0 .. ny/2-1 of the grids from the stored half-plane (consumers of the full grids call this first)
 int ensure_lower(muser_imager* h, cudaStream_t s) {
@@ -498,18 +517,18 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
             CU(h, launch_owner_count(g, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_count, h->ow_cta_hist, h->stats_d,
                                      h->ow_loc, iters, s));
             CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size,
-                                    h->ow_work, h->ow_ctl, h->ow_tops, s));
+                                    h->ow_work, h->ow_ctl, h->ow_tops, h->zero_pending ? h->ow_valid : nullptr, s));
             CU(h, launch_owner_scatter(g, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid, nvis, h->ow_offset, h->ow_cta_hist,
                                        h->ow_cursor, h->ow_sorted, h->cnt, iters, s));
         }
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
             CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work,
-                                    h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->zero_pending ? 1 : 0,
-                                    h->num_sms, s));
+                                    h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->ow_valid, h->num_sms, s));
         }
         h->n_launches += g.onbins <= 4096u ? 4 : 6;                   // count, scan (1 or 3 launches), scatter, grid
-        h->zero_pending = false;                                      // store mode wrote every tile of the stored half-plane
+        if (h->zero_pending) h->sparse = true;                        // first call after a reset: the tiles it did not write keep flag 0
+        h->zero_pending = false;
         h->lower_valid = false;                                       // rows < ny/2 are rebuilt on demand (ensure_lower)
         return MUSER_OK;
     }
@@ -563,16 +582,17 @@ int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const 
         CU(h, launch_rows_count(g, ntime, npol, nchan, (int)nrow, split, cpc, uvw, freq, (const float2*)vis, wt, gid, h->ow_count,
                                 h->ow_cta_hist, h->stats_d, h->ow_loc, s));
         CU(h, launch_owner_scan(g, h->ow_count, h->ow_cursor, h->ow_offset, h->ow_items, h->nitems_d, item_size, h->ow_work,
-                                h->ow_ctl, h->ow_tops, s));
+                                h->ow_ctl, h->ow_tops, h->zero_pending ? h->ow_valid : nullptr, s));
         CU(h, launch_rows_scatter(g, ntime, npol, nchan, (int)nrow, split, cpc, h->ow_loc, uvw, freq, (const float2*)vis, wt, gid,
                                   h->ow_offset, h->ow_cta_hist, h->ow_cursor, h->ow_sorted, h->cnt, s));
     }
     {
         StageScope sc(h, MUSER_STAGE_GRID, s);
         CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work, h->ow_ctl, h->ttp_d,
-                                grid_ptrs(h), h->ow_scratch, h->ow_tickets, h->zero_pending ? 1 : 0, h->num_sms, s));
+                                grid_ptrs(h), h->ow_scratch, h->ow_tickets, h->ow_valid, h->num_sms, s));
     }
     h->n_launches += g.onbins <= 4096u ? 4 : 6;
+    if (h->zero_pending) h->sparse = true;
     h->zero_pending = false;
     h->lower_valid = false;
     return MUSER_OK;
@@ -592,15 +612,21 @@ const void* cols_tmap(muser_imager* h) {
 int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     if (!dirty && !psf) return MUSER_OK;
     h->last_stream = s;
-    int rcz = flush_zero(h, s);
-    if (rcz) return rcz;
+    // the half-plane row pass takes the owner gridder's tile flags (unwritten tiles are not loaded); every other path wants
+    // dense grids
+    const bool rows_take_flags = h->fused_fft && h->fused_rows && !h->zero_pending && h->geom.otx <= 96;
+    if (!rows_take_flags) {
+        int rcz = flush_zero(h, s);
+        if (rcz) return rcz;
+    }
     if (h->fused_fft && h->fused_rows) {
         // A5 rows by k_fft_rows_half straight from the stored half-planes of G and Gw (H = G + i alpha Gw is never
         // materialised and rows < ny/2 are never read), A5 columns + A6 by the fused column kernel; H keeps the row
         // transform, so muser_dirty followed by muser_psf repeats only the column pass
         if (!h->fft_valid) {
             StageScope sc(h, MUSER_STAGE_FFT, s);
-            CU(h, launch_fft_rows_half(h->geom, h->G, h->Gw, h->cnt, h->tw_rows_d, h->stats_d, h->H, h->num_sms, s));
+            CU(h, launch_fft_rows_half(h->geom, h->G, h->Gw, h->cnt, h->tw_rows_d, h->stats_d, h->H, h->sparse ? h->ow_valid : nullptr,
+                                       h->num_sms, s));
             h->n_launches += 1;
             h->fft_valid = true;
         }
@@ -681,8 +707,9 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
 int reset_impl(muser_imager* h, cudaStream_t s) {
     h->last_stream = s;
     h->fft_valid = false;
-    // The grids are zeroed lazily: the owner-tile gridder writes every tile of every grid with plain stores, so a
-    // reset followed by muser_grid needs no memset at all; any other consumer calls flush_zero first.
+    // The grids are zeroed lazily: the next owner-tile muser_grid clears the tile flags, stores the tiles it grids and leaves
+    // the others alone (flag 0 = zeros; the row transform skips them), so a reset followed by muser_grid needs no memset and
+    // no zero fill at all; any consumer of the dense grids calls flush_zero first.
     h->zero_pending = true;
     if (!(owner_capable(h) && pick_strategy(h) == MUSER_STRATEGY_OWNER)) {
         int rc = flush_zero(h, s);
@@ -870,7 +897,7 @@ int muser_set_strategy(muser_imager* h, int strategy) {
     if (strategy != MUSER_STRATEGY_AUTO && strategy != MUSER_STRATEGY_TILED && strategy != MUSER_STRATEGY_OWNER &&
         strategy != MUSER_STRATEGY_WPLANE)
         return fail(h, MUSER_EINVAL, "unknown strategy");
-    if (h->zero_pending) {                                            // do not carry a deferred reset across strategies
+    if (h->zero_pending || h->sparse) {                               // do not carry a deferred reset / unwritten tiles across strategies
         int rc = flush_zero(h, h->last_stream);
         if (rc) return rc;
     }

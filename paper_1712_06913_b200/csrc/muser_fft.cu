@@ -303,11 +303,25 @@ struct RowCfg {
     static constexpr size_t SMEM = (size_t)NP * PITCH * sizeof(float4);
 };
 
+// predicated read-only loads (no branch: the 8 or 16 loads of a first-stage butterfly stay in flight together)
+__device__ __forceinline__ float2 ldg_f2_if(const float2* p, const bool ok) {
+    float2 v;
+    asm("{\n.reg .pred q;\nsetp.ne.s32 q, %3, 0;\nmov.f32 %0, 0f00000000;\nmov.f32 %1, 0f00000000;\n@q ld.global.nc.v2.f32 {%0, %1}, [%2];\n}"
+        : "=f"(v.x), "=f"(v.y) : "l"(p), "r"((int)ok));
+    return v;
+}
+__device__ __forceinline__ float ldg_f_if(const float* p, const bool ok) {
+    float v;
+    asm("{\n.reg .pred q;\nsetp.ne.s32 q, %2, 0;\nmov.f32 %0, 0f00000000;\n@q ld.global.nc.f32 %0, [%1];\n}" : "=f"(v) : "l"(p), "r"((int)ok));
+    return v;
+}
+
 template <int N, int WMODE, int UNIFORM>
-__global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int ngroups, const float2* __restrict__ G,
+__global__ void __launch_bounds__(N / 4, N == 1024 ? 3 : (N == 512 ? 6 : 1)) k_fft_rows_half(const int ny, const int ngroups, const float2* __restrict__ G,
                                                          const float* __restrict__ Gw, const int* __restrict__ cnt,
                                                          const float2* __restrict__ tw, Stats* __restrict__ stats,
-                                                         float2* __restrict__ Z) {
+                                                         float2* __restrict__ Z, const uint32_t* __restrict__ valid,
+                                                         const int otx) {
     using C = RowCfg<N, WMODE>;
     constexpr int T = C::T, PITCH = C::PITCH, R1 = C::R1, ROWS = C::ROWS, NSEQ = C::NSEQ, NP = C::NP;
     extern __shared__ __align__(16) float4 sm[];
@@ -322,9 +336,34 @@ __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int
         if (blockIdx.x == 0 && tid == 0) { stats->alpha = al; stats->inv_alpha = 1.0f / al; }
     }
     const int hy = ny >> 1, gpg = hy / ROWS;                       // row groups per grid
+    // tile flags of a group's row of tiles, one per lane and word of 32 tiles (fetched one group ahead)
+    uint32_t nflag[3] = {0u, 0u, 0u};
+    auto load_flags = [&](const int grp) {
+        if (grp >= ngroups) return;
+        const int gi = grp / gpg, ty = ((grp - gi * gpg) * ROWS) / kTile;
+        const uint32_t* vrow = valid + ((size_t)gi * (size_t)((hy + kTile - 1) / kTile) + ty) * otx;
+#pragma unroll
+        for (int w = 0; w < 3; ++w) {
+            const int t = 32 * w + (tid & 31);
+            nflag[w] = t < otx ? __ldg(vrow + t) : 0u;
+        }
+    };
+    if (valid) load_flags(blockIdx.x);
     for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
         const int gi = grp / gpg, iy0 = hy + (grp - gi * gpg) * ROWS;
         const size_t gbase = (size_t)gi * ny * N;
+        // tile flags of this row of 64 x 32 tiles (the rows of a group lie in one tile row): a tile that has not been written
+        // since the last reset stands for zeros and is not loaded (`valid` == nullptr: the grids are dense)
+        uint32_t vm[3] = {0xffffffffu, 0xffffffffu, 0xffffffffu};
+        if (valid) {
+#pragma unroll
+            for (int w = 0; w < 3; ++w) vm[w] = __ballot_sync(__activemask(), nflag[w] != 0u);   // (N = 64: a CTA of 16 threads)
+            load_flags(grp + (int)gridDim.x);                      // the next group's flags: in flight during this group
+        }
+        auto live = [&](int x) -> bool {                           // column x lies in a written tile
+            const int t = (x + kOwTileW / 2) / kOwTileW;
+            return ((t < 32 ? vm[0] : (t < 64 ? vm[1] : vm[2])) >> (t & 31)) & 1u;
+        };
         __syncthreads();                                           // the previous group is done with the shared buffers
         // ---- stage 1: radix R1 straight from global memory; sequence s, butterfly j -> y_s[R1 j + i]
         for (int task = tid; task < NSEQ * (N / R1); task += T) {
@@ -343,14 +382,14 @@ __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int
                     const float2* src = reinterpret_cast<const float2*>(Gw) + row;
 #pragma unroll
                     for (int i = 0; i < R1; ++i) {
-                        const float2 q = __ldg(src + j + i * (N / R1));
+                        const float2 q = ldg_f2_if(src + j + i * (N / R1), live(j + i * (N / R1)));
                         const float u = al * wgt(row + j + i * (N / R1));
                         v[i] = make_float2(u * q.x, u * q.y);
                     }
                 } else {
 #pragma unroll
                     for (int i = 0; i < R1; ++i) {
-                        const float2 q = __ldg(G + row + j + i * (N / R1));
+                        const float2 q = ldg_f2_if(G + row + j + i * (N / R1), live(j + i * (N / R1)));
                         const float u = wgt(row + j + i * (N / R1));
                         v[i] = make_float2(u * q.x, u * q.y);
                     }
@@ -359,7 +398,7 @@ __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int
                 const size_t row = gbase + (size_t)(iy0 + s) * N;
 #pragma unroll
                 for (int i = 0; i < R1; ++i) {
-                    const float2 q = __ldg(G + row + j + i * (N / R1));
+                    const float2 q = ldg_f2_if(G + row + j + i * (N / R1), live(j + i * (N / R1)));
                     const float u = wgt(row + j + i * (N / R1));
                     v[i] = make_float2(u * q.x, u * q.y);
                 }
@@ -368,7 +407,8 @@ __global__ void __launch_bounds__(N / 4) k_fft_rows_half(const int ny, const int
 #pragma unroll
                 for (int i = 0; i < R1; ++i) {
                     const size_t c0 = row + j + i * (N / R1);
-                    v[i] = make_float2(al * wgt(c0) * __ldg(Gw + c0), al * wgt(c0 + N) * __ldg(Gw + c0 + N));
+                    const bool ok = live(j + i * (N / R1));
+                    v[i] = make_float2(al * wgt(c0) * ldg_f_if(Gw + c0, ok), al * wgt(c0 + N) * ldg_f_if(Gw + c0 + N, ok));
                 }
             }
             float2* dst = reinterpret_cast<float2*>(sm + (s >> 1) * PITCH) + (s & 1);
@@ -512,14 +552,14 @@ bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngri
 
 template <int N, int WMODE>
 static cudaError_t launch_rows_t(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw, Stats* stats,
-                                 float2* Z, int num_sms, cudaStream_t s) {
+                                 float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s) {
     using C = RowCfg<N, WMODE>;
     const int ngroups = g.ngrids * ((g.ny / 2) / C::ROWS);
     int per_sm = (int)(200 * 1024 / (C::SMEM + 1024));
     per_sm = per_sm < 1 ? 1 : (per_sm > 2048 / C::T ? 2048 / C::T : per_sm);
     const int blocks = ngroups < num_sms * per_sm ? ngroups : num_sms * per_sm;
-    if (g.uniform && cnt) k_fft_rows_half<N, WMODE, 1><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, cnt, tw, stats, Z);
-    else k_fft_rows_half<N, WMODE, 0><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, nullptr, tw, stats, Z);
+    if (g.uniform && cnt) k_fft_rows_half<N, WMODE, 1><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, cnt, tw, stats, Z, valid, g.otx);
+    else k_fft_rows_half<N, WMODE, 0><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, nullptr, tw, stats, Z, valid, g.otx);
     return cudaGetLastError();
 }
 
@@ -551,11 +591,12 @@ cudaError_t fft_rows_setup() {
 }
 
 cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
-                                 Stats* stats, float2* Z, int num_sms, cudaStream_t s) {
+                                 Stats* stats, float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s) {
+    if (g.otx > 96) valid = nullptr;                                     // (the caller made the grids dense: see fft_rows_valid_ok)
 #define MUSER_ROWS_CASE(NN)                                                                                     \
     case NN:                                                                                                    \
-        return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, cnt, tw, stats, Z, num_sms, s)                          \
-                       : launch_rows_t<NN, 0>(g, G, Gw, cnt, tw, stats, Z, num_sms, s);
+        return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, cnt, tw, stats, Z, valid, num_sms, s)                   \
+                       : launch_rows_t<NN, 0>(g, G, Gw, cnt, tw, stats, Z, valid, num_sms, s);
     switch (g.nx) {
         MUSER_ROWS_CASE(64) MUSER_ROWS_CASE(128) MUSER_ROWS_CASE(256) MUSER_ROWS_CASE(512) MUSER_ROWS_CASE(1024)
         MUSER_ROWS_CASE(2048) MUSER_ROWS_CASE(4096)

@@ -149,7 +149,7 @@ cudaError_t launch_owner_count(const Geom& g, const float* uvw, const double* fr
                                uint4* loc, int iters, cudaStream_t s);
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* cursor, uint32_t* bin_offset, OwItem* items,
                               uint32_t* nitems, uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops,
-                              cudaStream_t s);
+                              uint32_t* valid_reset, cudaStream_t s);   // valid_reset != nullptr: clear the tile flags (first call after a reset)
 cudaError_t launch_owner_scatter(const Geom& g, const uint4* loc, const float* uvw, const double* freq, const float2* vis,
                                  const float* wt, const int* grid_id, long long nvis, const uint32_t* bin_offset,
                                  const uint32_t* cta_hist, uint32_t* cursor, uint4* sorted, int* cnt, int iters,
@@ -168,8 +168,11 @@ int rows_max_channels();
 cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
-                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, int store_mode,
+                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, uint32_t* valid,
                               int num_sms, cudaStream_t s);
+// valid [ngrids * ontiles (+ pad to a multiple of 4)]: 0 = the tile has not been written since the last reset (its cells
+// stand for zeros whatever they hold).  Zero those tiles and flag them:
+cudaError_t launch_owner_fill_invalid(const Geom& g, GridPtrs grids, uint32_t* valid, cudaStream_t s);
 
 // ---- fused column transform + correction (muser_fft.cu): ny = 256, 512 or 1024, nx a multiple of 16
 bool fft_cols_supported(int nx, int ny);
@@ -179,8 +182,9 @@ cudaError_t fft_cols_setup();
 bool fft_rows_supported(int nx, int ny, int wmode);
 int fft_rows_first_radix(int nx);
 cudaError_t fft_rows_setup();
+// valid != nullptr: tile flags of the owner gridder (tiles at 0 stand for zeros and are not loaded); at most 96 tiles per row
 cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
-                                 Stats* stats, float2* Z, int num_sms, cudaStream_t s);
+                                 Stats* stats, float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s);
 // tmap128 != nullptr: the strip is staged by TMA (tensor map from fft_cols_make_tmap), else by per-lane loads
 bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngrids);
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,

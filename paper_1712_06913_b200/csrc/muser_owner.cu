@@ -7,8 +7,9 @@
 //   O2  k_owner_scan_*     A1: multi-CTA exclusive scan of the histogram (3 small launches): sample offsets, chunk
 //                              items of heavy tiles (> item_size samples), work list of light non-empty tiles
 //   O3  k_owner_scatter    A1: reads O1's integer result and writes one 16-byte record per (sample, touched tile)
-//   O4a ow_fill_row        A2: store mode only: zero-fill units (one per grid and row of tiles) in the gridder's work
-//                              queue zero the EMPTY tiles of G, Gw and H in long contiguous runs
+//   O4a (tile flags)       A2: a tile that has not been written since the last reset has its flag in `valid` at 0: it is
+//                              never zero-filled -- the gridder stores instead of adding, the row transform skips its
+//                              loads, and k_owner_fill_invalid zeroes such tiles for the consumers of the dense grids
 //   O4  k_grid_owner_s7    A2/A4: persistent kernel, 4 CTAs per SM pulling work units (chunks of heavy tiles first,
 //                              then light 64x32 tiles interleaved with the fill units) from a device counter.  Per unit: counting sort of <= 4096 records by
 //                              8x8 window (shared histogram, 2-byte positions); every warp then streams an equal share
@@ -377,13 +378,14 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
                                                            const uint32_t item_size, const uint32_t* __restrict__ tops,
                                                            uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
                                                            uint4* __restrict__ work, uint32_t* __restrict__ nitems,
-                                                           uint32_t* __restrict__ ctl) {
+                                                           uint32_t* __restrict__ ctl, uint32_t* __restrict__ valid_reset) {
     __shared__ uint32_t s_w[3][32];
     const uint32_t b0 = blockIdx.x * 4096u + 4u * threadIdx.x;
     uint32_t c[4], m[4];
     const OwScan3 t = ow_load4(g, bin_count, b0, item_size, c, m);
     if (t.c) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);      // ready for the next call's O1
     if (b0 < g.onbins) *reinterpret_cast<uint4*>(cursor + b0) = make_uint4(0, 0, 0, 0);   // ready for this call's O3
+    if (valid_reset && b0 < g.onbins) *reinterpret_cast<uint4*>(valid_reset + b0) = make_uint4(0, 0, 0, 0);   // first call after a reset
     OwScan3 total;
     const OwScan3 ex = ow_block_scan3(t, total, s_w);
     uint32_t off = ex.c, slot = ex.m, wpos = ex.l;
@@ -924,44 +926,17 @@ __device__ __forceinline__ OwScale ow_scale_from(float3 s) {
     return sc;
 }
 
-// ------------------------------------------------------------------------------------------------- O4a fill
-// STORE mode: zero the EMPTY tiles of one row of tiles of one grid in G and Gw, as long contiguous runs of each
-// cell row (16-byte stores, consecutive threads -> consecutive addresses).  A thread owns column chunks: the emptiness
-// test is done once per chunk, the loop over the rows only stores.  Called by all 256 threads of a CTA.
-__device__ __forceinline__ void ow_fill_row(const Geom& g, const uint32_t* __restrict__ bin_offset, GridPtrs grids,
-                                            const int gi, const int ty, unsigned char* s_empty) {
-    const uint32_t bin0 = (uint32_t)gi * (uint32_t)g.ontiles + (uint32_t)ty * (uint32_t)g.otx;
-    for (int t = threadIdx.x; t < g.otx; t += blockDim.x) s_empty[t] = bin_offset[bin0 + t + 1] == bin_offset[bin0 + t];
-    __syncthreads();
-    const int y0 = (g.ny >> 1) + ty * kTile, y1 = min(y0 + kTile, g.ny);
-    const int nx2 = g.nx >> 1, nx4 = g.nx >> 2;
-    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-    const size_t row0 = ((size_t)gi * g.ny + y0) * (size_t)g.nx;
-    for (int i = threadIdx.x; i < nx2; i += blockDim.x) {              // 2 cells of G per store
-        if (!s_empty[(2 * i + kOwTW / 2) >> kOwTWS]) continue;
-        float4* __restrict__ gr = reinterpret_cast<float4*>(grids.G + row0) + i;
-#pragma unroll 4
-        for (int y = y0; y < y1; ++y, gr += nx2) *gr = z;
-    }
-    for (int i = threadIdx.x; i < nx4; i += blockDim.x) {              // 4 cells of Gw per store
-        if (!s_empty[(4 * i + kOwTW / 2) >> kOwTWS]) continue;
-        float4* __restrict__ wr = reinterpret_cast<float4*>(grids.Gw + row0) + i;
-#pragma unroll 4
-        for (int y = y0; y < y1; ++y, wr += nx4) *wr = z;
-    }
-}
-
 // Persistent kernel: 4 CTAs per SM pull work units from a device-side counter.  Units [0, nitems) are the chunk items
 // of heavy tiles (started first), units [nitems, nitems + nlight) the light non-empty tiles listed by k_owner_scan.
-// In STORE mode the zero-fill units of the empty tiles are part of the same queue.
-template <int STORE>
+// Empty tiles are not touched: their flag in `valid` stays 0 and every consumer takes them as zeros.
 __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
                                                           const uint32_t* __restrict__ bin_offset,
                                                           const OwItem* __restrict__ items,
                                                           const uint32_t* __restrict__ nitems,
                                                           const uint4* __restrict__ work, uint32_t* __restrict__ ctl,
                                                           const float* __restrict__ tt2, GridPtrs grids,
-                                                          float* __restrict__ scratch, uint32_t* __restrict__ tickets) {
+                                                          float* __restrict__ scratch, uint32_t* __restrict__ tickets,
+                                                          uint32_t* __restrict__ valid) {
     extern __shared__ __align__(16) unsigned char smem[];
     int* sA = reinterpret_cast<int*>(smem + kOwOffA);
     int* sB = reinterpret_cast<int*>(smem + kOwOffB);
@@ -984,13 +959,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     const int r = lane >> 2, c = lane & 3;
     const char* tbx = reinterpret_cast<const char*>(sT + 2 * c);
     const char* tby = reinterpret_cast<const char*>(sT + r);
-    // Work units: [0, n_items) chunks of heavy tiles; then n_light light tiles with, in STORE mode, the n_fill
-    // zero-fill units (one per grid and row of tiles) spread evenly between them (every k-th position), so that the
-    // store-bound fills and the issue-bound gridding units are resident on an SM at the same time.
+    // Work units: [0, n_items) chunks of heavy tiles, then the n_light light non-empty tiles.
     const uint32_t n_items = *nitems, n_light = ctl[0];
-    const uint32_t n_fill = STORE ? (uint32_t)g.ngrids * (uint32_t)g.oty : 0u;
-    const uint32_t n_rest = n_light + n_fill, n_work = n_items + n_rest;
-    const uint32_t kfill = n_fill ? max(n_rest / n_fill, 1u) : 1u;
+    const uint32_t n_work = n_items + n_light;
 
   for (;;) {
     __syncthreads();                                                  // the previous unit is done with the shared tile
@@ -1001,16 +972,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     uint32_t gi, start, cnt, first_slot = 0, nchunks = 0, chunk = 0;
     int tx, ty;
     const bool heavy = wi < n_items;
-    uint32_t li = wi - n_items;                                       // index into the light-tile list
-    if constexpr (STORE != 0) if (!heavy) {
-        const uint32_t j = li, f = j / kfill;
-        if (f < n_fill && j == f * kfill) {                           // fill unit f: zero the empty tiles of one tile row
-            ow_fill_row(g, bin_offset, grids, (int)(f / (uint32_t)g.oty), (int)(f % (uint32_t)g.oty),
-                        reinterpret_cast<unsigned char*>(sH));
-            continue;
-        }
-        li = j - min(n_fill, f + 1u);
-    }
+    const uint32_t li = wi - n_items;                                 // index into the light-tile list
     if (heavy) {
         const OwItem it = items[wi];
         start = it.start; cnt = it.count; first_slot = it.first_slot; nchunks = it.nchunks; chunk = it.chunk;
@@ -1021,6 +983,11 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         const uint4 wk = __ldg(work + li);                           // {start, grid, ty << 16 | tx, count}
         start = wk.x; gi = wk.y; ty = (int)(wk.z >> 16); tx = (int)(wk.z & 0xFFFFu); cnt = wk.w;
     }
+    // `valid` = 0: the tile has not been written since the last reset -- its cells in G, Gw hold garbage that stands for
+    // zeros (nobody zero-fills empty tiles; the row transform skips them): the tile is stored, else added to.  One writer
+    // per tile and launch (for a heavy tile: the last chunk to arrive), which also sets the flag.
+    uint32_t* vflag = valid + (size_t)gi * g.ontiles + (size_t)ty * g.otx + tx;
+    const bool STORE = *vflag == 0u;
     const int x0 = tx * kOwTW - kOwTW / 2, y0 = (g.ny >> 1) + ty * kTile;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
     float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
@@ -1195,6 +1162,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
                 }
             }
         }
+        if (tid == 0) *vflag = 1u;
         continue;
     }
     for (int i = tid; i < 32 * kG4; i += 256) {                       // heavy chunk: publish the partial tile
@@ -1245,7 +1213,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             *dst = v;
         }
     }
-    if (tid == 0) tickets[first_slot] = 0;
+    if (tid == 0) { tickets[first_slot] = 0; *vflag = 1u; }
   }
 }
 
@@ -1321,38 +1289,55 @@ int rows_max_channels() { return kRowsMaxChan; }
 
 cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* cursor, uint32_t* bin_offset, OwItem* items,
                               uint32_t* nitems, uint32_t item_size, uint4* work, uint32_t* ctl, uint32_t* tops,
-                              cudaStream_t s) {
+                              uint32_t* valid_reset, cudaStream_t s) {
     const uint32_t nblocks = (g.onbins + 4095u) / 4096u;
     if (nblocks == 1) {
-        k_owner_scan_write<1><<<1, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl);
+        k_owner_scan_write<1><<<1, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl, valid_reset);
         return cudaGetLastError();
     }
     k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
     k_owner_scan_tops<<<1, 1024, 0, s>>>(g, nblocks, tops, bin_offset, nitems, ctl);
-    k_owner_scan_write<0><<<nblocks, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl);
+    k_owner_scan_write<0><<<nblocks, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl, valid_reset);
     return cudaGetLastError();
 }
 
 cudaError_t owner_kernel_setup(int max_smem_bytes) {
-    cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_grid_owner_s7<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
-    if ((e = cudaFuncSetAttribute(k_grid_owner_s7<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024))) return e;
-    return cudaSuccess;
+    return cudaFuncSetAttribute(k_grid_owner_s7, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024);
 }
 
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
-                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, int store_mode,
+                              const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, uint32_t* valid,
                               int num_sms, cudaStream_t s) {
     const size_t smem = owner_smem_bytes(g.Q);
     const unsigned blocks = (unsigned)num_sms * 4u;
-    if (store_mode) {
-        k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids,
-                                                     scratch, tickets);
-    } else {
-        k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids,
-                                                     scratch, tickets);
+    k_grid_owner_s7<<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids, scratch, tickets, valid);
+    return cudaGetLastError();
+}
+
+// zero the tiles of the stored half-plane that have not been written since the last reset and flag them (consumers of the
+// dense grids call this first): one CTA per (grid, tile)
+__global__ void __launch_bounds__(256) k_owner_fill_invalid(const Geom g, GridPtrs grids, uint32_t* __restrict__ valid) {
+    const uint32_t b = blockIdx.x;
+    if (valid[b] != 0u) return;
+    const uint32_t gi = b / (uint32_t)g.ontiles, tile = b - gi * (uint32_t)g.ontiles;
+    const int ty = (int)(tile / (uint32_t)g.otx), tx = (int)(tile - (uint32_t)ty * (uint32_t)g.otx);
+    const int x0 = tx * kOwTW - kOwTW / 2, y0 = (g.ny >> 1) + ty * kTile;
+    float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
+    float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
+    for (int i = threadIdx.x; i < kTile * kOwTW; i += 256) {
+        const int x = x0 + (i & (kOwTW - 1)), y = y0 + (i >> kOwTWS);
+        if ((unsigned)x < (unsigned)g.nx && y < g.ny) {
+            Gt[(size_t)y * g.nx + x] = make_float2(0.f, 0.f);
+            Wt[(size_t)y * g.nx + x] = 0.f;
+        }
     }
+    __syncthreads();
+    if (threadIdx.x == 0) valid[b] = 1u;
+}
+
+cudaError_t launch_owner_fill_invalid(const Geom& g, GridPtrs grids, uint32_t* valid, cudaStream_t s) {
+    k_owner_fill_invalid<<<g.onbins, 256, 0, s>>>(g, grids, valid);
     return cudaGetLastError();
 }
 

@@ -43,6 +43,40 @@ def test_accumulation_over_calls_equals_one_call(strategy):
                 strategy=strategy, splits=5, images=False)
 
 
+def test_owner_tiles_never_written_stand_for_zeros_until_a_later_call_or_a_dense_consumer():
+    """The owner gridder does not zero-fill empty tiles: a tile keeps flag 0 ("zeros", whatever its memory holds) until a
+    later accumulating call stores into it or a consumer of the dense grids fills it.  The grids are pre-filled with
+    rubbish (a first dense cycle), reset, then gridded in two calls that touch different tiles; images straight from
+    the flagged half-plane after each call, then the dense grids."""
+    import torch
+    n, cell, S, Q = 512, 20.0, 7, 32
+    uvw, freq, vis, wt = synth.random_visibilities(61, 6000, n, cell, margin_cells=6.0)
+    vis = (1.0 + 0.1 * vis).astype(np.complex64)
+    r = np.hypot(uvw[:, 0], uvw[:, 1])
+    inner, outer = r < np.median(r) * 0.5, r >= np.median(r) * 0.5
+    im = gu.make_imager(n, cell, S, Q, strategy=OWNER)
+    T = gu.oracle_table("pswf", S, Q)
+    try:
+        big = [gu.to_dev(a) for a in (uvw, freq, (vis * 1e3).astype(np.complex64), wt)]
+        im.grid(*big)                                        # every tile that will matter now holds large stale values
+        gu.gpu_grids(im)                                     # (dense consumer: fills the rest)
+        im.reset()
+        sel = [gu.to_dev(np.ascontiguousarray(a[inner])) for a in (uvw, freq, vis, wt)]
+        im.grid(*sel)
+        G1, W1, _ = oc.grid(uvw[inner], freq[inner], vis[inner], wt[inner], n, n, cell, Q, S, T)
+        gu.check_images(im, G1, W1, T, S, Q)                 # row transform on the flagged half-plane
+        sel = [gu.to_dev(np.ascontiguousarray(a[outer])) for a in (uvw, freq, vis, wt)]
+        im.grid(*sel)                                        # accumulating call: stores into tiles still at flag 0
+        G2, W2, st = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, S, T)
+        gu.check_images(im, G2, W2, T, S, Q)
+        G, Gw = gu.gpu_grids(im)                             # dense grids: unwritten tiles read back as exact zeros
+        assert gu.rel_l2(G, G2) <= gu.GRID_TOL and gu.rel_l2(Gw, W2) <= gu.GRID_TOL
+        assert np.all(G[0][np.abs(G2[0]) == 0] == 0)
+        assert im.get_stats()["n_gridded"] == st["n_gridded"]
+    finally:
+        im.destroy()
+
+
 @pytest.mark.parametrize("strategy", [OWNER, TILED])
 def test_flagged_and_off_grid_visibilities_are_skipped_and_counted(strategy):
     n, cell = 256, 20.0
