@@ -308,8 +308,8 @@ def bench_frames(args, cfg, torch, binding, shard, dist, rank, world, local):
     traffic, traffic_src = _committed_traffic("k_grid_owner_s7")
     frac_a1a2 = (in_bytes + grid_bytes) / ((bin_us + grid_us) * 1e-6) / 1e9 / peak
     roofline = {
-        "bound": "hbm", "kernel": "A1 + A2: k_owner_count, k_owner_scan_*, k_owner_scatter (binning) + k_grid_owner_s7 (gridding, "
-                                  "zero-fill units of empty tiles included)",
+        "bound": "hbm", "kernel": "A1 + A2: k_owner_count, k_owner_scan_*, k_owner_scatter (binning) + k_grid_owner_s7 (gridding; "
+                                  "tiles without samples are flagged, not zero-filled)",
         "achieved": (in_bytes + grid_bytes) / ((bin_us + grid_us) * 1e-6) / 1e9, "peak": peak, "unit": "GB/s", "frac": frac_a1a2,
         "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
         "algorithmic_bytes_per_launch": in_bytes + grid_bytes,
@@ -320,7 +320,8 @@ def bench_frames(args, cfg, torch, binding, shard, dist, rank, world, local):
             "k4_half_plane_bytes_written_over_grid_time": 0.5 * grid_bytes / (grid_us * 1e-6) / 1e9 / peak,
         },
         "note": "frac = A1+A2 algorithmic bytes (32 B/vis + 12 B/cell) over binning + gridding time; the gridder stores the "
-                "Hermitian half-plane only (6 B/cell actually written, last fraction)",
+                "non-empty tiles of the Hermitian half-plane only (at most 6 B/cell actually written: last fraction; `traffic` is "
+                "what ncu measured)",
         "kernel_us": bin_us + grid_us, "stage_us_per_launch": stage_us,
         "stage_us_per_frame": {k: (v / B if v else None) for k, v in stage_us.items()}}
 

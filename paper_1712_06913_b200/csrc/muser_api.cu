@@ -524,7 +524,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
         {
             StageScope sc(h, MUSER_STAGE_GRID, s);
             CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work,
-                                    h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->ow_valid, h->num_sms, s));
+                                    h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->ow_valid, h->zero_pending ? 1 : 0, h->num_sms, s));
         }
         h->n_launches += g.onbins <= 4096u ? 4 : 6;                   // count, scan (1 or 3 launches), scatter, grid
         if (h->zero_pending) h->sparse = true;                        // first call after a reset: the tiles it did not write keep flag 0
@@ -589,7 +589,7 @@ int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const 
     {
         StageScope sc(h, MUSER_STAGE_GRID, s);
         CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work, h->ow_ctl, h->ttp_d,
-                                grid_ptrs(h), h->ow_scratch, h->ow_tickets, h->ow_valid, h->num_sms, s));
+                                grid_ptrs(h), h->ow_scratch, h->ow_tickets, h->ow_valid, h->zero_pending ? 1 : 0, h->num_sms, s));
     }
     h->n_launches += g.onbins <= 4096u ? 4 : 6;
     if (h->zero_pending) h->sparse = true;

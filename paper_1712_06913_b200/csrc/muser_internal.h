@@ -169,7 +169,7 @@ cudaError_t owner_kernel_setup(int max_smem_bytes);
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
                               const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, uint32_t* valid,
-                              int num_sms, cudaStream_t s);
+                              int first, int num_sms, cudaStream_t s);   // first: first call after a reset (every tile is stored)
 // valid [ngrids * ontiles (+ pad to a multiple of 4)]: 0 = the tile has not been written since the last reset (its cells
 // stand for zeros whatever they hold).  Zero those tiles and flag them:
 cudaError_t launch_owner_fill_invalid(const Geom& g, GridPtrs grids, uint32_t* valid, cudaStream_t s);

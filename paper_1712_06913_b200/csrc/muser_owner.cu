@@ -929,6 +929,8 @@ __device__ __forceinline__ OwScale ow_scale_from(float3 s) {
 // Persistent kernel: 4 CTAs per SM pull work units from a device-side counter.  Units [0, nitems) are the chunk items
 // of heavy tiles (started first), units [nitems, nitems + nlight) the light non-empty tiles listed by k_owner_scan.
 // Empty tiles are not touched: their flag in `valid` stays 0 and every consumer takes them as zeros.
+// FIRST: the first call after a reset (the scan has just cleared every flag): every tile is stored
+template <int FIRST>
 __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const uint4* __restrict__ sorted,
                                                           const uint32_t* __restrict__ bin_offset,
                                                           const OwItem* __restrict__ items,
@@ -987,7 +989,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
     // zeros (nobody zero-fills empty tiles; the row transform skips them): the tile is stored, else added to.  One writer
     // per tile and launch (for a heavy tile: the last chunk to arrive), which also sets the flag.
     uint32_t* vflag = valid + (size_t)gi * g.ontiles + (size_t)ty * g.otx + tx;
-    const bool STORE = *vflag == 0u;
+    const bool STORE = FIRST ? true : (*vflag == 0u);
     const int x0 = tx * kOwTW - kOwTW / 2, y0 = (g.ny >> 1) + ty * kTile;
     float2* __restrict__ Gt = grids.G + (size_t)gi * g.ny * g.nx;
     float* __restrict__ Wt = grids.Gw + (size_t)gi * g.ny * g.nx;
@@ -1302,16 +1304,19 @@ cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* curs
 }
 
 cudaError_t owner_kernel_setup(int max_smem_bytes) {
-    return cudaFuncSetAttribute(k_grid_owner_s7, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024);
+    cudaError_t e = cudaFuncSetAttribute(k_grid_owner_s7<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024);
+    if (e) return e;
+    return cudaFuncSetAttribute(k_grid_owner_s7<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 1024);
 }
 
 cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t* bin_offset,
                               const OwItem* items, const uint32_t* nitems, const uint4* work, uint32_t* ctl,
                               const float* tt2, GridPtrs grids, float* scratch, uint32_t* tickets, uint32_t* valid,
-                              int num_sms, cudaStream_t s) {
+                              int first, int num_sms, cudaStream_t s) {
     const size_t smem = owner_smem_bytes(g.Q);
     const unsigned blocks = (unsigned)num_sms * 4u;
-    k_grid_owner_s7<<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids, scratch, tickets, valid);
+    if (first) k_grid_owner_s7<1><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids, scratch, tickets, valid);
+    else k_grid_owner_s7<0><<<blocks, 256, smem, s>>>(g, sorted, bin_offset, items, nitems, work, ctl, tt2, grids, scratch, tickets, valid);
     return cudaGetLastError();
 }
 
