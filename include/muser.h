@@ -112,7 +112,9 @@ int muser_set_psf2x(muser_imager* h, int enabled);
 int muser_psf2x(muser_imager* h, float* beam2x_out, muser_stream s);
 
 /* ---- A1..A4 gridding --------------------------------------------------------------------------------------
- * Zero the grids, the sum of weights and the counters (asynchronous on s). */
+ * Zero the grids, the sum of weights and the counters (asynchronous on s).  On the OWNER strategy the zeroing is lazy: the
+ * tiles of the stored half-plane that the following muser_grid calls do not touch are flagged as zeros and never written
+ * (the row transform skips them); muser_get_grid and every other consumer of the dense grids see exact zeros there. */
 int muser_reset(muser_imager* h, muser_stream s);
 /* Grid nvis visibilities AND their Hermitian conjugates (-u,-v,-w, conj V) (R6), accumulating
  * onto what is already there (time integration; R16).  DEVICE pointers:
