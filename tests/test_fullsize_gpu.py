@@ -1,7 +1,7 @@
 """-m gpu parity at BASELINE.json's FULL sizes, in the launch configurations that are actually used:
 
   * cfg 3 as bench.py times it: 80 distinct MUSER-II frames, one muser_grid_batched + muser_dirty_psf call (owner-tile
-    gridder, store mode writes G, Gw and the FFT input H); three of the 80 grids are compared cell by cell and pixel by
+    gridder: the first call after a reset stores the non-empty tiles of the half-plane and flags them); three of the 80 grids are compared cell by cell and pixel by
     pixel with the oracle, the counters over all of them.
   * cfg 4: a 64-frame chunk = 2048 independent 512x512 grids of 1770 visibilities (the full config is 500 such chunks;
     one chunk is what fits comfortably beside its images); sampled grids against the oracle, counters over all.
