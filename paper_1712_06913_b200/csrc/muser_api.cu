@@ -85,6 +85,7 @@ struct muser_imager {
     bool fused_fft = false;                 // row pass by cuFFT, column pass + correction by k_fft_cols_correct
     bool fused_rows = false;                // row pass by k_fft_rows_half on the stored half-plane (nx a power of two)
     float2* tw_d = nullptr;                 // per-stage twiddles of the fused column transform
+    float2* tw8_d = nullptr;                // ... of its radix-8 variant (ny = 512, 1024)
     float2* tw_rows_d = nullptr;            // ... and of the row transform
     cudaStream_t last_stream = nullptr;
     // host-frame staging (muser_frame_host)
@@ -635,7 +636,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
         if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
         h->n_launches += 1;
         return MUSER_OK;
     }
@@ -666,7 +667,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
         if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
         h->n_launches += 1;
         return MUSER_OK;
     }
@@ -778,8 +779,22 @@ muser_imager* muser_imager_create(int nx, int ny, double cell_arcsec, int suppor
         return cudaMalloc(out, tw.size() * sizeof(float2)) == cudaSuccess &&
                cudaMemcpy(*out, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess;
     };
+    // radix-8 stages: tw8[(7 stage + i - 1) (n/8) + j] = exp(+2 pi i * i * (j mod Ns) / (8 Ns)), Ns = R1 * 8^stage
+    auto twiddles8 = [&](int n, int r1, float2** out) -> bool {
+        const int T8 = n / 8;
+        std::vector<float2> tw;
+        for (int Ns = r1; Ns < n; Ns *= 8)
+            for (int i = 1; i <= 7; ++i)
+                for (int j = 0; j < T8; ++j) {
+                    const double a = 2.0 * 3.14159265358979323846 * (double)i * (double)(j % Ns) / (8.0 * (double)Ns);
+                    tw.push_back(make_float2((float)std::cos(a), (float)std::sin(a)));
+                }
+        return cudaMalloc(out, tw.size() * sizeof(float2)) == cudaSuccess &&
+               cudaMemcpy(*out, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess;
+    };
     if (fft_cols_supported(nx, ny) && fft_cols_setup() == cudaSuccess) {
         if (!twiddles(ny, fft_cols_first_radix(ny), &h->tw_d)) { h->err = "twiddle table"; return bail("fft"); }
+        if (fft_cols_radix8(ny) && !twiddles8(ny, fft_cols_first_radix(ny), &h->tw8_d)) { h->err = "twiddle table"; return bail("fft"); }
         h->fused_fft = true;
         if (fft_rows_supported(nx, ny, 0) && fft_rows_supported(nx, ny, 1) && fft_rows_setup() == cudaSuccess) {
             if (!twiddles(nx, fft_rows_first_radix(nx), &h->tw_rows_d)) { h->err = "twiddle table"; return bail("fft"); }
@@ -799,7 +814,7 @@ int muser_imager_destroy(muser_imager* h) {
     cudaFree(h->tables_d); cudaFree(h->planes_d); cudaFree(h->icx_d); cudaFree(h->icy_d); cudaFree(h->ones_d);
     cudaFree(h->in_uvw); cudaFree(h->in_freq); cudaFree(h->in_vis); cudaFree(h->in_wt); cudaFree(h->in_gid);
     cudaFree(h->ttp_d); cudaFree(h->ow_items); cudaFree(h->ow_tickets); cudaFree(h->ow_scratch);
-    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->wg_ctl); cudaFree(h->wg_lists); cudaFree(h->tw_d); cudaFree(h->tw_rows_d);
+    cudaFree(h->ow_sorted); cudaFree(h->ow_loc); cudaFree(h->ow_ctl); cudaFree(h->wg_ctl); cudaFree(h->wg_lists); cudaFree(h->tw_d); cudaFree(h->tw8_d); cudaFree(h->tw_rows_d);
     if (h->wg_streams_ok) {
         for (int i = 0; i < 7; ++i) cudaStreamDestroy(h->wg_side[i]);
         for (int i = 0; i < 8; ++i) cudaEventDestroy(h->wg_ev[i]);

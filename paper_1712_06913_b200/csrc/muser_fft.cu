@@ -88,7 +88,10 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
                  ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
 }
 
-template <int N, int TMA>
+// R8 (ny = 512, 1024): after the first stage the remaining factor 64 is done as TWO radix-8 stages instead of three radix-4
+// ones -- one shared-memory round trip less (the kernel is bound by its shared-memory traffic); a thread then owns one radix-8
+// butterfly of one column pair; tw8[(7 stage + i - 1) (N/8) + j] = exp(+2 pi i * i * (j mod Ns) / (8 Ns)).
+template <int N, int TMA, int R8>
 __global__ void __launch_bounds__((N / 4) * (fft_cols_per_cta(N) / 4), N >= 4096 ? 1 : (N >= 1024 ? 2 : (N == 512 ? 4 : 8))) k_fft_cols_correct(const __grid_constant__ CUtensorMap tmap,
                                                                                const int nx, const float2* __restrict__ F1,
                                                                                const float2* __restrict__ tw,
@@ -203,6 +206,84 @@ __global__ void __launch_bounds__((N / 4) * (fft_cols_per_cta(N) / 4), N >= 4096
             for (int cc = 0; cc < 4; ++cc) dst[2 * pad(16 * j + b + 4 * cc)] = v[4 * b + cc];
     }
     __syncthreads();
+
+    if constexpr (R8 != 0) {
+        constexpr int T8 = N / 8;
+        const int j = tid >> 2, cp = tid & 3;                                              // butterfly j of column pair cp
+        float4* col = sm + cp * PITCH;
+        const float2* twp = tw + j;
+        float2 a[8], b[8];                                                                 // the two columns of the pair
+#pragma unroll 1
+        for (int Ns = R1; Ns < N; Ns *= 8, twp += 7 * T8) {
+            const int k = j & (Ns - 1);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float4 q = col[pad(j + i * T8)];
+                a[i] = make_float2(q.x, q.y); b[i] = make_float2(q.z, q.w);
+            }
+#pragma unroll
+            for (int i = 1; i < 8; ++i) {
+                const float2 w = __ldg(twp + (i - 1) * T8);
+                a[i] = cmul(a[i], w); b[i] = cmul(b[i], w);
+            }
+            idft8_half(a); idft8_half(b);                                                  // X[m] = v[2m] + v[2m+1], X[m+4] = v[2m] - v[2m+1]
+            if (Ns * 8 == N) break;                                                        // results stay in registers
+            __syncthreads();
+            const int o = (j - k) * 8 + k;
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                col[pad(o + m * Ns)] = make_float4(a[2 * m].x + a[2 * m + 1].x, a[2 * m].y + a[2 * m + 1].y,
+                                                   b[2 * m].x + b[2 * m + 1].x, b[2 * m].y + b[2 * m + 1].y);
+                col[pad(o + (m + 4) * Ns)] = make_float4(a[2 * m].x - a[2 * m + 1].x, a[2 * m].y - a[2 * m + 1].y,
+                                                         b[2 * m].x - b[2 * m + 1].x, b[2 * m].y - b[2 * m + 1].y);
+            }
+            __syncthreads();
+        }
+        // epilogue: F[ky = j + m T8][sx0 + 2 cp + {0, 1}]; the four lanes of a butterfly write one 32-byte sector per row
+        const int x0 = (sx0 + (nx >> 1)) % nx + 2 * cp;
+        const float2 cx = *reinterpret_cast<const float2*>(icx + x0);
+        const float ia = stats->inv_alpha;
+        const size_t obase = (size_t)gi * N * nx;
+        unsigned long long best = 0ull;
+        unsigned int lowest = 0u;
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            const int h2 = m & 3;
+            const float2 fa = m < 4 ? make_float2(a[2 * h2].x + a[2 * h2 + 1].x, a[2 * h2].y + a[2 * h2 + 1].y)
+                                    : make_float2(a[2 * h2].x - a[2 * h2 + 1].x, a[2 * h2].y - a[2 * h2 + 1].y);
+            const float2 fb = m < 4 ? make_float2(b[2 * h2].x + b[2 * h2 + 1].x, b[2 * h2].y + b[2 * h2 + 1].y)
+                                    : make_float2(b[2 * h2].x - b[2 * h2 + 1].x, b[2 * h2].y - b[2 * h2 + 1].y);
+            const int ky = j + m * T8, y = (ky + N / 2) & (N - 1);
+            const float cy = (y & 1) ? -icy[y] : icy[y];                                   // x0 is even: sign = (-1)^y * (+, -)
+            const float m0 = cx.x * cy, m1 = -cx.y * cy;
+            const size_t o = obase + (size_t)y * nx + x0;
+            if (dirty) {
+                const float2 d = make_float2(fa.x * m0, fb.x * m1);
+                *reinterpret_cast<float2*>(dirty + o) = d;
+                if (peaks) {
+                    const unsigned int base = (unsigned int)(y * nx + x0);
+                    const float dv[2] = {d.x, d.y};
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        const unsigned int ord = peak_ordered(dv[c]);
+                        const unsigned long long key = ((unsigned long long)ord << 32) | (unsigned long long)(~(base + c));
+                        best = key > best ? key : best;
+                        lowest = max(lowest, ~ord);
+                    }
+                }
+            }
+            if (psf) *reinterpret_cast<float2*>(psf + o) = make_float2(fa.y * m0 * ia, fb.y * m1 * ia);
+        }
+        if (dirty && peaks) {
+            for (int o = 16; o > 0; o >>= 1) {
+                const unsigned long long ob = __shfl_xor_sync(0xffffffffu, best, o);
+                best = ob > best ? ob : best;
+                lowest = max(lowest, __shfl_xor_sync(0xffffffffu, lowest, o));
+            }
+            if ((tid & 31) == 0) { atomicMax(&peaks[gi].maxkey, best); atomicMax(&peaks[gi].minkey, lowest); }
+        }
+        return;
+    }
 
     // ---- radix-4 stages in shared memory: Ns = 16, 64, ... ; the last one (Ns = N/4) ends in registers.
     // tw[(3 stage + i - 1) T + j] = exp(+2 pi i * i * (j mod Ns) / (4 Ns)): per-stage tables in butterfly order.
@@ -508,16 +589,18 @@ int fft_cols_first_radix(int ny) { return (ny == 256 || ny == 1024 || ny == 4096
 
 cudaError_t fft_cols_setup() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<2048, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(2048)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<2048, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(2048)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<4096, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(4096)))) return e;
-    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<4096, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(4096)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<256, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(256)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<2048, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(2048)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<2048, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(2048)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<4096, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(4096)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<4096, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(4096)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<512, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(512)))) return e;
+    if ((e = cudaFuncSetAttribute(k_fft_cols_correct<1024, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes(1024)))) return e;
     return cudaSuccess;
 }
 
@@ -605,17 +688,27 @@ cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw
 #undef MUSER_ROWS_CASE
 }
 
-cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
-                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, const void* tmap128,
-                                    cudaStream_t s) {
+bool fft_cols_radix8(int ny) { return ny == 512 || ny == 1024; }
+
+cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float2* tw8, const float* icx,
+                                    const float* icy, const Stats* stats, float* dirty, float* psf, PeakSlot* peaks,
+                                    const void* tmap128, cudaStream_t s) {
     CUtensorMap map;
     memset(&map, 0, sizeof(map));
     if (tmap128) memcpy(&map, tmap128, sizeof(map));
     for (int grid0 = 0; grid0 < g.ngrids; grid0 += 65535) {              // gridDim.y holds at most 65535 grids
         const dim3 blocks((unsigned)(g.nx / fft_cols_per_cta(g.ny)), (unsigned)std::min(65535, g.ngrids - grid0));
 #define MUSER_COLS_CASE(NN)                                                                                                   \
-        if (tmap128) k_fft_cols_correct<NN, 1><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0); \
-        else k_fft_cols_correct<NN, 0><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+        if (tmap128) k_fft_cols_correct<NN, 1, 0><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0); \
+        else k_fft_cols_correct<NN, 0, 0><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);
+        if (tmap128 && tw8 && g.ny == 512) {
+            k_fft_cols_correct<512, 1, 1><<<blocks, 256, fft_smem_bytes(512), s>>>(map, g.nx, F1, tw8, icx, icy, stats, dirty, psf, peaks, grid0);
+            continue;
+        }
+        if (tmap128 && tw8 && g.ny == 1024) {
+            k_fft_cols_correct<1024, 1, 1><<<blocks, 512, fft_smem_bytes(1024), s>>>(map, g.nx, F1, tw8, icx, icy, stats, dirty, psf, peaks, grid0);
+            continue;
+        }
         if (g.ny == 256) { MUSER_COLS_CASE(256) }
         else if (g.ny == 512) { MUSER_COLS_CASE(512) }
         else if (g.ny == 1024) { MUSER_COLS_CASE(1024) }

@@ -187,8 +187,10 @@ cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw
                                  Stats* stats, float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s);
 // tmap128 != nullptr: the strip is staged by TMA (tensor map from fft_cols_make_tmap), else by per-lane loads
 bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngrids);
-cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float* icx, const float* icy,
-                                    const Stats* stats, float* dirty, float* psf, PeakSlot* peaks, const void* tmap128,
-                                    cudaStream_t s);
+// tw8 != nullptr (ny = 512, 1024, with the TMA staging): two radix-8 stages after the first one instead of three radix-4 ones
+bool fft_cols_radix8(int ny);
+cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float2* tw8, const float* icx,
+                                    const float* icy, const Stats* stats, float* dirty, float* psf, PeakSlot* peaks,
+                                    const void* tmap128, cudaStream_t s);
 
 }  // namespace muser
