@@ -441,6 +441,16 @@ __global__ void __launch_bounds__(N / 4, N == 1024 ? 3 : (N == 512 ? 6 : 1)) k_f
             for (int w = 0; w < 3; ++w) vm[w] = __ballot_sync(__activemask(), nflag[w] != 0u);   // (N = 64: a CTA of 16 threads)
             load_flags(grp + (int)gridDim.x);                      // the next group's flags: in flight during this group
         }
+        if (valid && (vm[0] | vm[1] | vm[2]) == 0u) {              // no tile of this row of tiles has been written: zeros
+            for (int r = 0; r < ROWS; ++r) {
+                const int iy = iy0 + r;
+                for (int kx = tid; kx < N; kx += T) {
+                    Z[gbase + (size_t)iy * N + kx] = make_float2(0.f, 0.f);
+                    Z[gbase + (size_t)(iy == hy ? 0 : ny - iy) * N + kx] = make_float2(0.f, 0.f);
+                }
+            }
+            continue;
+        }
         auto live = [&](int x) -> bool {                           // column x lies in a written tile
             const int t = (x + kOwTileW / 2) / kOwTileW;
             return ((t < 32 ? vm[0] : (t < 64 ? vm[1] : vm[2])) >> (t & 31)) & 1u;
