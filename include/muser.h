@@ -78,7 +78,9 @@ int muser_set_batch(muser_imager* h, int ngrids);
 /* A3: w-projection with nplanes planes (R15).  HOST arrays, copied: w_centres[p] >= 0 (plane
  * centres in wavelengths of |w|), supports[p] odd in [1,63]; tables_c64[p] = supports[p]*oversample+1
  * interleaved (re,im) FLOAT pairs of the per-axis kernel, or tables_c64 == NULL: the library generates the
- * Fresnel-separable kernels of R15.  Plane 0's (real part) table defines the grid correction.
+ * Fresnel-separable kernels of R15.  Caller tables must be EVEN, T[t] = T[S*Q - t] to 1e-5 of their maximum (else MUSER_EINVAL):
+ * the gridders compute the Hermitian half-plane only, which equals the full gridding for even kernels (every gridding
+ * kernel is).  Plane 0's (real part) table defines the grid correction.
  * nplanes == 0 returns to 2-D mode.  Zeroes the grids (the beam grid becomes complex). */
 int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, const int* supports,
                       const float* const* tables_c64);

@@ -883,6 +883,15 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
             const size_t L = ((size_t)sup[p] * h->Q + 1) * 2;
             t64[p].resize(L);
             for (size_t i = 0; i < L; ++i) t64[p][i] = (double)tables_c64[p][i];
+            // the gridders compute the Hermitian half-plane only and take the other half as its conjugate mirror: that holds
+            // for EVEN kernels, k(-x) = k(x) (every gridding kernel is: PSWF, Gaussian, the Fresnel w-kernels)
+            double tmax = 0.0, asym = 0.0;
+            const size_t n1 = (size_t)sup[p] * h->Q;
+            for (size_t t = 0; t <= n1; ++t) {
+                tmax = std::max(tmax, std::hypot(t64[p][2 * t], t64[p][2 * t + 1]));
+                asym = std::max(asym, std::hypot(t64[p][2 * t] - t64[p][2 * (n1 - t)], t64[p][2 * t + 1] - t64[p][2 * (n1 - t) + 1]));
+            }
+            if (!(asym <= 1e-5 * tmax)) return fail(h, MUSER_EINVAL, "plane tables must be even: T[t] = T[S*Q - t]");
         }
     } else {
         const muser_host::WKernelGen gen(4096);

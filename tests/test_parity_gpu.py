@@ -334,6 +334,44 @@ def test_wprojection_unevenly_spaced_planes_take_the_full_plane_scan():
 
 
 @pytest.mark.parametrize("strategy", [TILED, WPLANE])
+def test_wprojection_small_supports_and_arbitrary_caller_tables(strategy):
+    """Supports 1, 3, 5 (windows smaller than their register layout), 7 and 9 with arbitrary complex tables supplied by the
+    caller (parity does not depend on what the tables mean), uniform weighting on (hit counts through the generic binning)."""
+    import torch
+    n, cell, Q = 128, 60.0, 4
+    sup = np.array([1, 3, 5, 7, 9], np.int64)
+    wc = np.array([0.0, 300.0, 700.0, 1200.0, 2000.0])
+    rng = np.random.default_rng(314)
+    tabs = [(rng.uniform(0.2, 1.0, S * Q + 1) + 1j * rng.uniform(-0.5, 0.5, S * Q + 1)) for S in sup]
+    tabs = [0.5 * (t + t[::-1]) for t in tabs]                # even, as every gridding kernel is (the half-plane design needs it)
+    tabs[0] = tabs[0].real.astype(np.complex128)              # plane 0's real part defines the grid correction
+    uvw, freq, vis, wt = synth.random_visibilities(19, 20000, n, cell, margin_cells=7.0, w_max_lambda=2200.0)
+    uvw = uvw.copy(); uvw[::3, :2] *= 0.1                     # a dense patch: runs of several records per window
+    im = gu.make_imager(n, cell, 7, Q, strategy=strategy)
+    try:
+        im.set_weighting(binding.MUSER_WEIGHT_UNIFORM)
+        bad = [t.astype(np.complex64) for t in tabs]
+        bad[2] = bad[2].copy(); bad[2][1] += 0.3              # an odd component: refused
+        with pytest.raises(binding.MuserError):
+            im.set_wplanes(wc, sup, bad)
+        im.set_wplanes(wc, sup, [t.astype(np.complex64) for t in tabs])
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        G, Gw = gu.gpu_grids(im)
+        tabs32 = [t.astype(np.complex64).astype(np.complex128) for t in tabs]
+        G_or, Gw_or, st_or = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, sup, tabs32, wc=wc, counts=True)
+        st = im.get_stats()
+        assert (st["n_gridded"], st["n_dropped"], st["n_flagged"]) == (st_or["n_gridded"], st_or["n_dropped"], st_or["n_flagged"])
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL
+        assert gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        cnt = torch.empty((1, n, n), dtype=torch.int32, device="cuda")
+        im.get_counts(cnt)
+        torch.cuda.synchronize()
+        assert np.array_equal(cnt.cpu().numpy().astype(np.int64), st_or["cnt"])
+    finally:
+        im.destroy()
+
+
+@pytest.mark.parametrize("strategy", [TILED, WPLANE])
 @pytest.mark.parametrize("ngrids", [1, 3])
 def test_wprojection_every_support_class_dense_runs_and_batches(strategy, ngrids):
     """Supports 7..31 (all three classes of the window gridder), dense uv coverage near the origin (long runs of records
