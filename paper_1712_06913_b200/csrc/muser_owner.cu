@@ -1177,24 +1177,46 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         const int4 a = *reinterpret_cast<const int4*>(sB + row * kOwPitch + 4 * c4);
         __stcg(part + 32 * kG4 + i, make_float4((float)a.x * iw, (float)a.y * iw, (float)a.z * iw, (float)a.w * iw));
     }
-    // heavy tile: the last chunk to arrive adds the published partial tiles up in chunk order
+    // heavy tile: the partial tiles are added up in two levels, always in chunk order.  The chunks form groups of G
+    // (G^2 >= nchunks); the last chunk of a GROUP to arrive sums its group into the group's first slot, the last group to
+    // finish sums the group sums and writes the tile.  One CTA reading all nchunks x 24 KB (37 chunks for the central tile
+    // of a single MUSER-II frame) was the critical path of a single frame; no CTA ever waits for another.
+    uint32_t G = 2;
+    while (G * G < nchunks) ++G;
+    const uint32_t ngroups = (nchunks + G - 1u) / G, g0 = (chunk / G) * G, gn = min(G, nchunks - g0);
     __threadfence();
     __syncthreads();
     if (tid == 0) {
-        const uint32_t t = atomicAdd(&tickets[first_slot], 1u);
-        sLast = (t == nchunks - 1u);
+        const uint32_t t = atomicAdd(&tickets[first_slot + g0], 1u);   // group counters sit at the groups' first slots
+        sLast = (t == gn - 1u);
     }
     __syncthreads();
     if (!sLast) continue;
     __threadfence();
-    const float4* parts = reinterpret_cast<const float4*>(scratch + (size_t)first_slot * kOwTileFloats);
-    for (int j = tid; j < 32 * kW4; j += 256) {                       // weights first
-        const int i = 32 * kG4 + j;
+    float4* parts = reinterpret_cast<float4*>(scratch + (size_t)first_slot * kOwTileFloats);
+    auto sum_slots = [&](const int i, const uint32_t first, const uint32_t count, const uint32_t stride) -> float4 {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (uint32_t q = 0; q < nchunks; ++q) {
-            const float4 p = __ldcg(parts + (size_t)q * (kOwTileFloats / 4) + i);
+        for (uint32_t q = 0; q < count; ++q) {
+            const float4 p = __ldcg(parts + (size_t)(first + q * stride) * (kOwTileFloats / 4) + i);
             v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
         }
+        return v;
+    };
+    if (ngroups > 1u) {
+        for (int i = tid; i < kOwTileFloats / 4; i += 256) __stcg(parts + (size_t)g0 * (kOwTileFloats / 4) + i, sum_slots(i, g0, gn, 1u));
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            const uint32_t t = atomicAdd(&tickets[first_slot + 1u], 1u);   // tile counter (slot 1 is never a group's first: G >= 2)
+            sLast = (t == ngroups - 1u);
+        }
+        __syncthreads();
+        if (!sLast) continue;
+        __threadfence();
+    }
+    const uint32_t nsl = ngroups > 1u ? ngroups : nchunks, stride = ngroups > 1u ? G : 1u;
+    for (int j = tid; j < 32 * kW4; j += 256) {                       // weights first
+        float4 v = sum_slots(32 * kG4 + j, 0u, nsl, stride);
         const int gx = x0 + 4 * (j % kW4), gy = y0 + (j / kW4);
         if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
             float4* dst = reinterpret_cast<float4*>(Wt + (size_t)gy * g.nx + gx);
@@ -1203,11 +1225,7 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
         }
     }
     for (int i = tid; i < 32 * kG4; i += 256) {
-        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (uint32_t q = 0; q < nchunks; ++q) {
-            const float4 p = __ldcg(parts + (size_t)q * (kOwTileFloats / 4) + i);
-            v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
-        }
+        float4 v = sum_slots(i, 0u, nsl, stride);
         const int gx = x0 + 2 * (i % kG4), gy = y0 + (i / kG4);
         if ((unsigned)gx < (unsigned)g.nx && (unsigned)gy < (unsigned)g.ny) {
             float4* dst = reinterpret_cast<float4*>(Gt + (size_t)gy * g.nx + gx);
@@ -1215,7 +1233,9 @@ __global__ void __launch_bounds__(256, 4) k_grid_owner_s7(const Geom g, const ui
             *dst = v;
         }
     }
-    if (tid == 0) { tickets[first_slot] = 0; *vflag = 1u; }
+    for (uint32_t q = tid; q < ngroups; q += 256) tickets[first_slot + q * G] = 0;
+    if (tid == 0) tickets[first_slot + 1u] = 0;
+    if (tid == 0) *vflag = 1u;
   }
 }
 
