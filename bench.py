@@ -305,7 +305,8 @@ def bench_frames(args, cfg, torch, binding, shard, dist, rank, world, local):
     # algorithmic bytes: 32 B per input visibility (read by the BINNING kernels) + every cell of G (8 B)
     # and Gw (4 B) written once (by the GRIDDING kernel); one launch handles B frames
     in_bytes, grid_bytes = B * 32.0 * nvis, B * 12.0 * n * n
-    traffic, traffic_src = _committed_traffic("k_grid_owner_s7")
+    # the committed ncu capture is of cfg 3 with 80 frames per launch: it says nothing about any other workload
+    traffic, traffic_src = _committed_traffic("k_grid_owner_s7") if (cfg == 3 and B == 80) else (None, None)
     frac_a1a2 = (in_bytes + grid_bytes) / ((bin_us + grid_us) * 1e-6) / 1e9 / peak
     roofline = {
         "bound": "hbm", "kernel": "A1 + A2: k_owner_count, k_owner_scan_*, k_owner_scatter (binning) + k_grid_owner_s7 (gridding; "
