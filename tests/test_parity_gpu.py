@@ -77,6 +77,66 @@ def test_owner_tiles_never_written_stand_for_zeros_until_a_later_call_or_a_dense
         im.destroy()
 
 
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4])
+def test_random_call_sequences_keep_the_lazy_state_consistent(seed):
+    """reset / grid (pieces of the data, by the owner or the generic gridder) / images / dense read-backs in random order: after
+    every step that produces something, it equals the oracle on the pieces gridded since the last reset.  Exercises the
+    deferred reset, the tile flags, the lower half-plane mirror and the cached row transform together."""
+    import torch
+    rng = np.random.default_rng(1000 + seed)
+    n, cell, S, Q = 256, 20.0, 7, 16
+    uvw, freq, vis, wt = synth.random_visibilities(70 + seed, 4000, n, cell, margin_cells=6.0)
+    vis = (1.0 + 0.2 * vis).astype(np.complex64)
+    r = np.hypot(uvw[:, 0], uvw[:, 1])
+    order = np.argsort(r)                                    # pieces are rings in uv: different calls touch different tiles
+    pieces = np.array_split(order, 8)
+    T = gu.oracle_table("pswf", S, Q)
+    im = gu.make_imager(n, cell, S, Q)
+    since = []                                               # pieces gridded since the last reset
+    def expected():
+        if not since:
+            return np.zeros((1, n, n), np.complex128), np.zeros((1, n, n)), 0
+        idx = np.concatenate(since)
+        G, W, st = oc.grid(uvw[idx], freq[idx], vis[idx], wt[idx], n, n, cell, Q, S, T)
+        return G, W, st["n_gridded"]
+    try:
+        for step in range(24):
+            op = rng.choice(["reset", "grid", "grid", "grid_tiled", "images", "dense", "dirty_only"])
+            if op == "reset":
+                im.reset(); since = []
+            elif op in ("grid", "grid_tiled"):
+                im.set_strategy(TILED if op == "grid_tiled" else binding.MUSER_STRATEGY_AUTO)
+                idx = pieces[rng.integers(len(pieces))]
+                im.grid(*[gu.to_dev(np.ascontiguousarray(a[idx])) for a in (uvw, freq, vis, wt)])
+                since.append(idx)
+            elif op == "dense":
+                G, Gw = gu.gpu_grids(im)
+                G_or, W_or, ng = expected()
+                assert im.get_stats()["n_gridded"] == ng
+                if ng:
+                    assert gu.rel_l2(G, G_or) <= gu.GRID_TOL and gu.rel_l2(Gw, W_or) <= gu.GRID_TOL, (step, op)
+                else:
+                    assert not G.any() and not Gw.any(), (step, op)
+            else:
+                d = torch.full((1, n, n), 7.0, device="cuda"); b = torch.full((1, n, n), 7.0, device="cuda")
+                if op == "images":
+                    im.dirty_psf(d, b)
+                else:
+                    im.dirty(d); im.psf(b)
+                torch.cuda.synchronize()
+                G_or, W_or, ng = expected()
+                if ng:
+                    _, cor_d, _, cor_p, _ = gu.oracle_images(G_or, W_or, T, S, Q)
+                    q = n // 8
+                    for got, ref in ((d.cpu().numpy(), cor_d), (b.cpu().numpy(), cor_p)):
+                        err = np.abs(got - ref)[:, q:-q, q:-q].max() / np.abs(ref[:, q:-q, q:-q]).max()
+                        assert err <= gu.IMG_TOL, (step, op, err)
+                else:
+                    assert not d.cpu().numpy().any() and not b.cpu().numpy().any(), (step, op)
+    finally:
+        im.destroy()
+
+
 @pytest.mark.parametrize("strategy", [OWNER, TILED])
 def test_flagged_and_off_grid_visibilities_are_skipped_and_counted(strategy):
     n, cell = 256, 20.0
