@@ -399,7 +399,8 @@ int ensure_owner_scratch(muser_imager* h, long long nvis, uint32_t item_size, ui
         CU(h, cudaMalloc(&h->ow_cursor, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_offset, nb * sizeof(uint32_t)));
         CU(h, cudaMalloc(&h->ow_work, nb * sizeof(uint4)));
-        CU(h, cudaMalloc(&h->ow_tops, (nb / 4096 + 2) * 3 * sizeof(uint32_t)));
+        CU(h, cudaMalloc(&h->ow_tops, (nb / 4096 + 3) * 4 * sizeof(uint32_t)));
+        CU(h, cudaMemsetAsync(h->ow_tops, 0, (nb / 4096 + 3) * 4 * sizeof(uint32_t), s));   // flags of the chained scan: zero when idle
         if (!h->ow_ctl) CU(h, cudaMalloc(&h->ow_ctl, 4 * sizeof(uint32_t)));
         CU(h, cudaMemsetAsync(h->ow_count, 0, nb * sizeof(uint32_t), s));   // ordered on the caller's stream; every later use leaves it zeroed
         h->ow_bins_cap = nb;
@@ -528,7 +529,7 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
             CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work,
                                     h->ow_ctl, h->ttp_d, gp, h->ow_scratch, h->ow_tickets, h->ow_valid, h->zero_pending ? 1 : 0, h->num_sms, s));
         }
-        h->n_launches += g.onbins <= 4096u ? 4 : 6;                   // count, scan (1 or 3 launches), scatter, grid
+        h->n_launches += g.onbins <= 4096u * 1024u ? 4 : 6;           // count, scan (1 launch up to 4 M bins, else 3), scatter, grid
         if (h->zero_pending) h->sparse = true;                        // first call after a reset: the tiles it did not write keep flag 0
         h->zero_pending = false;
         h->lower_valid = false;                                       // rows < ny/2 are rebuilt on demand (ensure_lower)
@@ -593,7 +594,7 @@ int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const 
         CU(h, launch_owner_grid(g, h->ow_sorted, h->ow_offset, h->ow_items, h->nitems_d, h->ow_work, h->ow_ctl, h->ttp_d,
                                 grid_ptrs(h), h->ow_scratch, h->ow_tickets, h->ow_valid, h->zero_pending ? 1 : 0, h->num_sms, s));
     }
-    h->n_launches += g.onbins <= 4096u ? 4 : 6;
+    h->n_launches += g.onbins <= 4096u * 1024u ? 4 : 6;
     if (h->zero_pending) h->sparse = true;
     h->zero_pending = false;
     h->lower_valid = false;

@@ -371,16 +371,27 @@ __global__ void __launch_bounds__(1024) k_owner_scan_tops(const Geom g, const ui
     if (threadIdx.x == 0) { bin_offset[g.onbins] = carry.c; *nitems = carry.m; ctl[0] = carry.l; ctl[1] = 0; }
 }
 
-// SINGLE: the whole histogram fits one CTA (<= 4096 bins): no reduce / tops launches, this kernel also writes the totals.
+// SINGLE = 1: the whole histogram fits one CTA (<= 4096 bins): no reduce / tops launches, this kernel also writes the totals.
+// SINGLE = 2: chained scan in ONE launch for up to 1024 CTAs: a CTA publishes its totals (tops[4 b + 0..2], then the flag
+// tops[4 b + 3]), waits for the flags of the CTAs before it and adds their totals up.  b is the CTA's arrival ticket
+// (tops[4 nblocks + 1]), so a CTA only ever waits for CTAs that are already running; the last CTA to have read
+// its predecessors clears the flags for the next launch (tops[4 nblocks] counts them), so there is no state to reset.
 template <int SINGLE>
 __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_t* __restrict__ bin_count,
                                                            uint32_t* __restrict__ cursor,
-                                                           const uint32_t item_size, const uint32_t* __restrict__ tops,
+                                                           const uint32_t item_size, uint32_t* tops,
                                                            uint32_t* __restrict__ bin_offset, OwItem* __restrict__ items,
                                                            uint4* __restrict__ work, uint32_t* __restrict__ nitems,
                                                            uint32_t* __restrict__ ctl, uint32_t* __restrict__ valid_reset) {
     __shared__ uint32_t s_w[3][32];
-    const uint32_t b0 = blockIdx.x * 4096u + 4u * threadIdx.x;
+    __shared__ uint32_t s_me;
+    uint32_t blk = blockIdx.x;
+    if (SINGLE == 2) {                                                // block index = arrival ticket: a CTA only waits for CTAs that run
+        if (threadIdx.x == 0) s_me = atomicAdd(&tops[4 * gridDim.x + 1], 1u);
+        __syncthreads();
+        blk = s_me;
+    }
+    const uint32_t b0 = blk * 4096u + 4u * threadIdx.x;
     uint32_t c[4], m[4];
     const OwScan3 t = ow_load4(g, bin_count, b0, item_size, c, m);
     if (t.c) *reinterpret_cast<uint4*>(bin_count + b0) = make_uint4(0, 0, 0, 0);      // ready for the next call's O1
@@ -389,8 +400,35 @@ __global__ void __launch_bounds__(1024) k_owner_scan_write(const Geom g, uint32_
     OwScan3 total;
     const OwScan3 ex = ow_block_scan3(t, total, s_w);
     uint32_t off = ex.c, slot = ex.m, wpos = ex.l;
-    if (SINGLE) {
+    if (SINGLE == 1) {
         if (threadIdx.x == 0) { bin_offset[g.onbins] = total.c; *nitems = total.m; ctl[0] = total.l; ctl[1] = 0; }
+    } else if (SINGLE == 2) {
+        __shared__ uint32_t s_base[3];
+        volatile uint32_t* vt = tops;
+        const uint32_t me = blk, nb = gridDim.x;
+        if (threadIdx.x == 0) {
+            vt[4 * me] = total.c; vt[4 * me + 1] = total.m; vt[4 * me + 2] = total.l;
+            __threadfence();
+            vt[4 * me + 3] = 1u;
+        }
+        OwScan3 pre = {0u, 0u, 0u};
+        if (threadIdx.x < me) {                                       // predecessor threadIdx.x (me < 1024)
+            while (vt[4 * threadIdx.x + 3] == 0u) {}
+            __threadfence();
+            pre.c = vt[4 * threadIdx.x]; pre.m = vt[4 * threadIdx.x + 1]; pre.l = vt[4 * threadIdx.x + 2];
+        }
+        OwScan3 sum;
+        ow_block_scan3(pre, sum, s_w);                                // (only the block sum is used)
+        if (threadIdx.x == 0) {
+            s_base[0] = sum.c; s_base[1] = sum.m; s_base[2] = sum.l;
+            if (me == nb - 1u) { bin_offset[g.onbins] = sum.c + total.c; *nitems = sum.m + total.m; ctl[0] = sum.l + total.l; ctl[1] = 0; }
+            if (atomicAdd(&tops[4 * nb], 1u) == nb - 1u) {            // everybody has read its predecessors: re-arm
+                for (uint32_t i = 0; i < nb; ++i) vt[4 * i + 3] = 0u;
+                vt[4 * nb] = 0u; vt[4 * nb + 1] = 0u;
+            }
+        }
+        __syncthreads();
+        off += s_base[0]; slot += s_base[1]; wpos += s_base[2];
     } else {
         off += tops[3 * blockIdx.x]; slot += tops[3 * blockIdx.x + 1]; wpos += tops[3 * blockIdx.x + 2];
     }
@@ -1315,6 +1353,10 @@ cudaError_t launch_owner_scan(const Geom& g, uint32_t* bin_count, uint32_t* curs
     const uint32_t nblocks = (g.onbins + 4095u) / 4096u;
     if (nblocks == 1) {
         k_owner_scan_write<1><<<1, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl, valid_reset);
+        return cudaGetLastError();
+    }
+    if (nblocks <= 1024u) {                                           // (tops: 4 (nblocks + 1) words, zero when idle)
+        k_owner_scan_write<2><<<nblocks, 1024, 0, s>>>(g, bin_count, cursor, item_size, tops, bin_offset, items, work, nitems, ctl, valid_reset);
         return cudaGetLastError();
     }
     k_owner_scan_reduce<<<nblocks, 1024, 0, s>>>(g, bin_count, item_size, tops);
