@@ -528,13 +528,14 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
                                                        const float* __restrict__ tables, GridPtrs grids) {
     extern __shared__ __align__(16) float smem[];
     constexpr int PL = kFastR * kFastPitch;                 // floats per accumulator plane
-    float* s_re = smem;
-    float* s_im = smem + PL;
-    float* s_w = smem + 2 * PL;
+    int* s_re = reinterpret_cast<int*>(smem);               // 32-bit fixed point (native shared adds; an fp32 add is a CAS loop)
+    int* s_im = s_re + PL;
+    int* s_w = s_re + 2 * PL;
     uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + 3 * PL);           // 1024 cells of the tile
     float4* s_rec = reinterpret_cast<float4*>(smem + 3 * PL + 1024);         // kFastChunk samples, cell-sorted
     float* s_tt = smem + 3 * PL + 1024 + 4 * kFastChunk;                    // (Q+1) x 8 transposed table
     __shared__ uint32_t s_wsum[8];
+    __shared__ float s_bound[8][2];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int jx = lane & 7, jy = lane >> 3;
@@ -552,6 +553,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
         __syncthreads();
         // (1) local counting sort by cell
         float4 rec[kFastChunk / 256];
+        float bv = 0.f, bw = 0.f;
         uint32_t rnk[kFastChunk / 256];
 #pragma unroll
         for (int j = 0; j < kFastChunk / 256; ++j) {
@@ -559,9 +561,17 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
             if (i < item.count) {
                 rec[j] = __ldg(reinterpret_cast<const float4*>(sorted + item.start + i));
                 rnk[j] = atomicAdd(&s_hist[__float_as_uint(rec[j].w) & 1023u], 1u);
+                bv += fabsf(rec[j].x) + fabsf(rec[j].y);
+                bw += rec[j].z;
             }
         }
+        for (int o = 16; o > 0; o >>= 1) { bv += __shfl_xor_sync(0xffffffffu, bv, o); bw += __shfl_xor_sync(0xffffffffu, bw, o); }
+        if (lane == 0) { s_bound[warp][0] = bv; s_bound[warp][1] = bw; }
         __syncthreads();
+        bv = 0.f; bw = 0.f;
+        for (int w = 0; w < 8; ++w) { bv += s_bound[w][0]; bw += s_bound[w][1]; }
+        // the item's largest possible cell sum (the kernel never exceeds 1) maps to 0.98 * 2^31
+        const float sv = 2104533975.0f / fmaxf(bv, 1e-30f), sw = 2104533975.0f / fmaxf(bw, 1e-30f);
         {
             uint4 hv = reinterpret_cast<uint4*>(s_hist)[threadIdx.x];
             const uint32_t tot = hv.x + hv.y + hv.z + hv.w;
@@ -595,10 +605,10 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
                 if (cur >= 0 && jx < 7) {
                     const int lx = cur & 31, ly = cur >> 5;
                     const int s0 = (ly + jy) * kFastPitch + lx + jx;
-                    atomicAdd(&s_re[s0], a0r); atomicAdd(&s_im[s0], a0i); atomicAdd(&s_w[s0], a0w);
+                    atomicAdd(&s_re[s0], __float2int_rn(a0r * sv)); atomicAdd(&s_im[s0], __float2int_rn(a0i * sv)); atomicAdd(&s_w[s0], __float2int_rn(a0w * sw));
                     if (jy < 3) {
                         const int s1 = s0 + 4 * kFastPitch;
-                        atomicAdd(&s_re[s1], a1r); atomicAdd(&s_im[s1], a1i); atomicAdd(&s_w[s1], a1w);
+                        atomicAdd(&s_re[s1], __float2int_rn(a1r * sv)); atomicAdd(&s_im[s1], __float2int_rn(a1i * sv)); atomicAdd(&s_w[s1], __float2int_rn(a1w * sw));
                     }
                 }
             };
@@ -622,6 +632,7 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
         }
         __syncthreads();
         // (3) add the touched cells of the region to the grids
+        const float isv = 1.0f / sv, isw = 1.0f / sw;
         const int x0 = tx * kTile - kTile / 2 - 3, y0 = ty * kTile - kTile / 2 - 3;
         const size_t gbase = (size_t)gi * g.ny * g.nx;
         for (int i = threadIdx.x; i < PL; i += blockDim.x) {
@@ -629,9 +640,9 @@ __global__ void __launch_bounds__(256) k_grid_tiled_s7(const Geom g, const Sampl
             const int gx = x0 + x, gy = y0 + y;
             if (x >= kFastR || gx < 0 || gx >= g.nx || gy < (g.ny >> 1) || gy >= g.ny) continue;   // the stored half-plane only
             const size_t idx = gbase + (size_t)gy * g.nx + gx;
-            const float vr = s_re[i], vi = s_im[i], vw = s_w[i];
-            if (vr != 0.f || vi != 0.f) atomicAdd(&grids.G[idx], make_float2(vr, vi));
-            if (vw != 0.f) atomicAdd(&grids.Gw[idx], vw);
+            const int vr = s_re[i], vi = s_im[i], vw = s_w[i];
+            if (vr | vi) atomicAdd(&grids.G[idx], make_float2((float)vr * isv, (float)vi * isv));
+            if (vw) atomicAdd(&grids.Gw[idx], (float)vw * isw);
         }
         __syncthreads();
     }
