@@ -47,7 +47,7 @@ enum { MUSER_KERNEL_PSWF = 0, MUSER_KERNEL_GAUSS = 1 };
  * shared memory and stores it once (no memset, no global atomics; 2-D mode with support 7 only, else
  * MUSER_EUNSUPPORTED at muser_grid); the other half-plane is rebuilt on demand (muser_get_grid).  TILED: work items of
  * <= 512 samples per 32x32 tile, shared memory accumulation, global reductions at the flush (any support, w planes).
- * WPLANE (w mode, every plane support <= 31): work items of <= 4096 records of one 32x32 tile, sorted by
+ * WPLANE (w mode, PAPER.md:126, and 2-D mode with a support other than 7; every support <= 31): work items of <= 4096 records of one 32x32 tile, sorted by
  * plane; a run of records whose footprints share a 2x2-aligned (S+1) x (S+1) window is accumulated in registers and
  * merged into a fixed-point shared-memory region, which is added to the grids once per item.
  * AUTO picks OWNER where it applies, else WPLANE where it applies, else TILED.  (Value 1 was a per-sample

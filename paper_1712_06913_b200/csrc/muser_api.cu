@@ -358,8 +358,8 @@ int ensure_scratch(muser_imager* h, long long nvis, cudaStream_t s) {
     return MUSER_OK;
 }
 
-bool wplane_capable(const muser_imager* h) {
-    return wmode(h) && wgrid_supported(h->planes_h.data(), (int)h->planes_h.size(), h->Q, h->max_smem);
+bool wplane_capable(const muser_imager* h) {     // w mode, or 2-D mode (one plane, real table); every support <= 31
+    return !h->planes_h.empty() && wgrid_supported(h->planes_h.data(), (int)h->planes_h.size(), h->Q, h->max_smem);
 }
 
 int pick_strategy(const muser_imager* h) {
@@ -428,7 +428,7 @@ int grid_generic(muser_imager* h, int strat, const float* uvw, const double* fre
     GridPtrs gp = grid_ptrs(h);
     if (strat != MUSER_STRATEGY_TILED && strat != MUSER_STRATEGY_WPLANE) return fail(h, MUSER_EUNSUPPORTED, "unknown gridding strategy");
     if (strat == MUSER_STRATEGY_WPLANE && !wplane_capable(h))
-        return fail(h, MUSER_EUNSUPPORTED, "the w-plane window strategy needs w mode with every plane support <= 31");
+        return fail(h, MUSER_EUNSUPPORTED, "the window strategy needs every support <= 31 (and a table that fits shared memory)");
     int rc = ensure_scratch(h, nvis, s);
     if (rc) return rc;
     if ((rc = flush_zero(h, s))) return rc;

@@ -1,4 +1,5 @@
-// W-projection gridder (A3: per-plane complex separable kernels, supports 1..31), sm_100a.
+// W-projection gridder (A3: per-plane complex separable kernels, supports 1..31), sm_100a; also the 2-D gridder for supports
+// other than 7 (one plane with a real table: the imaginary halves of the packed FMAs then carry zeros).
 //
 //   Kw1 k_wtile_items   work items: <= 4096 consecutive records of one 32x32 tile (bins are ordered tile-major,
 //                       plane-minor, so an item is a sequence of plane segments)
@@ -227,9 +228,13 @@ __device__ __forceinline__ void wg_stream(const uint4* __restrict__ src, const i
 // shape 7 (direct): S lanes per record, lane = footprint column, floor(32 / S) records per warp pass; loop over the rows;
 // the row factors ky * (wt V), ky * wt are formed once per row; table TT[r][j] (pitch tp) read through L1
 template <int PR, int PL>
-__device__ __forceinline__ void wg_direct(const uint4* __restrict__ src, const int n, const float2* __restrict__ tab, const int tp,
-                                          const int S, const int dh, int* __restrict__ sReg, const float sv, const float sw,
-                                          const int lane, const int warp) {
+__device__ __forceinline__ void wg_direct(const uint4* __restrict__ src, const int n, const float* __restrict__ tabf, const bool cplx,
+                                          const int tp, const int S, const int dh, int* __restrict__ sReg, const float sv,
+                                          const float sw, const int lane, const int warp) {
+    // entry i of the plane's table: complex (w mode) or real (2-D mode, any support)
+    auto entry = [&](const int i) -> float2 {
+        return cplx ? __ldg(reinterpret_cast<const float2*>(tabf) + i) : make_float2(__ldg(tabf + i), 0.f);
+    };
     const int per = 32 / S, sub = lane / S, jx = lane - sub * S;
     if (sub >= per) return;
     for (int i = warp * per + sub; i < n; i += 8 * per) {
@@ -239,12 +244,12 @@ __device__ __forceinline__ void wg_direct(const uint4* __restrict__ src, const i
         const float re = __uint_as_float(a.x) * sv, im = __uint_as_float(a.y) * sv, wt = __uint_as_float(a.z) * sw;
         const int lx = (int)(w & 31u), ly = (int)((w >> 5) & 31u);
         const int rx = (int)((w >> 10) & 511u), ry = (int)((w >> 19) & 511u);
-        const float2 kx2 = __ldg(tab + rx * tp + jx);
+        const float2 kx2 = entry(rx * tp + jx);
         const float kxr = kx2.x, kxi = kx2.y * cs;
-        const float2* __restrict__ kyp = tab + ry * tp;
+        const int kyb = ry * tp;
         int* cell = sReg + (ly + dh) * PR + lx + dh + jx;
         for (int jy = 0; jy < S; ++jy, cell += PR) {
-            const float2 ky2 = __ldg(kyp + jy);
+            const float2 ky2 = entry(kyb + jy);
             const float kyr = ky2.x, kyi = ky2.y * cs;
             const float tr = kyr * re - kyi * im, ti = kyr * im + kyi * re;
             const float ur = kyr * wt, ui = kyi * wt;
@@ -353,17 +358,18 @@ __global__ void __launch_bounds__(256, WgShape<SHP>::MINB) k_wgrid(const Geom g,
             const uint4* __restrict__ src = reinterpret_cast<const uint4*>(sorted + a);
             if constexpr (C::LR == 0) {                               // direct: no per-segment state in shared memory
                 const PlaneMeta pm = planes[p];
-                wg_direct<PR, PL>(src, n, reinterpret_cast<const float2*>(tables) + pm.offset, pm.pitch, S, dh, sReg, sv, sw, lane, warp);
+                wg_direct<PR, PL>(src, n, tables + (size_t)pm.offset * (g.wmode ? 2 : 1), g.wmode != 0, pm.pitch, S, dh, sReg, sv, sw, lane, warp);
                 continue;
             }
             __syncthreads();                                          // the previous segment is done with sH / sP / the table
             if (cached != p) {                                        // stage the plane's table: entry e = footprint index + 1
                 const PlaneMeta pm = planes[p];
-                const float2* tc = reinterpret_cast<const float2*>(tables) + pm.offset;
+                const float2* tc = reinterpret_cast<const float2*>(tables) + pm.offset;   // w mode: complex entries
+                const float* tr = tables + pm.offset;                                       // 2-D mode: real entries
                 for (int i = tid; i < (g.Q + 1) * PT; i += 256) {
                     const int r = i / PT, e = i - r * PT, j = e - 1;
                     float2 v = make_float2(0.f, 0.f);
-                    if (j >= 0 && j < S) v = __ldg(tc + r * pm.pitch + j);
+                    if (j >= 0 && j < S) v = g.wmode ? __ldg(tc + r * pm.pitch + j) : make_float2(__ldg(tr + r * pm.pitch + j), 0.f);
                     sTab[i] = v;
                 }
                 cached = p;
@@ -410,7 +416,8 @@ __global__ void __launch_bounds__(256, WgShape<SHP>::MINB) k_wgrid(const Geom g,
             const int vr = sReg[i], vi = sReg[PL + i], wr = sReg[2 * PL + i], wim = sReg[3 * PL + i];
             const size_t idx = gbase + (size_t)gy * g.nx + gx;
             if (vr | vi) atomicAdd(&grids.G[idx], make_float2((float)vr * iv, (float)vi * iv));
-            if (wr | wim) atomicAdd(&Gw2[idx], make_float2((float)wr * iw, (float)wim * iw));
+            if (g.wmode) { if (wr | wim) atomicAdd(&Gw2[idx], make_float2((float)wr * iw, (float)wim * iw)); }
+            else if (wr) atomicAdd(&grids.Gw[idx], (float)wr * iw);                         // 2-D mode: the weight grid is real
         }
     }
 }

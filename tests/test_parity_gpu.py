@@ -26,9 +26,9 @@ def test_single_grid_configs_match_oracle(cfg, strategy):
     assert res["stats"]["n_gridded"] > 0.9 * fr.nvis
 
 
-@pytest.mark.parametrize("strategy", [TILED])
+@pytest.mark.parametrize("strategy", [TILED, WPLANE])
 @pytest.mark.parametrize("S,Q,nvis", [(7, 128, 1), (7, 16, 31), (7, 128, 5000), (3, 8, 777), (5, 32, 1000), (9, 64, 1500),
-                                      (1, 2, 100), (15, 16, 300)])
+                                      (1, 2, 100), (15, 16, 300), (9, 16, 30000), (21, 8, 4000), (31, 4, 2000)])
 def test_random_visibilities_any_support(S, Q, nvis, strategy):
     n, cell = 128, 40.0
     uvw, freq, vis, wt = synth.random_visibilities(7 + S, nvis, n, cell, margin_cells=S / 2 + 2)
