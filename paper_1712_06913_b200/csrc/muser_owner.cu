@@ -4,22 +4,22 @@
 //                              result per visibility (16 B) and histograms the tiles each sample's 7x7 footprint
 //                              touches (1, 2 or 4) in a CTA-private shared histogram (one global atomic per touched
 //                              tile per CTA)
-//   O2  k_owner_scan_*     A1: multi-CTA exclusive scan of the histogram (3 small launches): sample offsets, chunk
+//   O2  k_owner_scan_*     A1: multi-CTA exclusive scan of the histogram (one chained launch): sample offsets, chunk
 //                              items of heavy tiles (> item_size samples), work list of light non-empty tiles
 //   O3  k_owner_scatter    A1: reads O1's integer result and writes one 16-byte record per (sample, touched tile)
 //   O4a (tile flags)       A2: a tile that has not been written since the last reset has its flag in `valid` at 0: it is
 //                              never zero-filled -- the gridder stores instead of adding, the row transform skips its
 //                              loads, and k_owner_fill_invalid zeroes such tiles for the consumers of the dense grids
 //   O4  k_grid_owner_s7    A2/A4: persistent kernel, 4 CTAs per SM pulling work units (chunks of heavy tiles first,
-//                              then light 64x32 tiles interleaved with the fill units) from a device counter.  Per unit: counting sort of <= 4096 records by
-//                              8x8 window (shared histogram, 2-byte positions); every warp then streams an equal share
+//                              then the light non-empty 64x32 tiles) from a device counter.  Per unit: counting sort of
+//                              <= 4096 records by 8x8 window (shared histogram, 2-byte positions); every warp then streams an equal share
 //                              of the sorted order through a private 2 x 32-record buffer (gather loads one batch
 //                              ahead, records staged in fixed-point units with table row offsets); a run of equal
 //                              window is accumulated in registers (lane = row r, column pair c; three packed FFMA2 per
 //                              sample; kernel table in shared memory) and merged into the 32-bit fixed-point shared
-//                              tile with native integer adds.  The tile is written to G, Gw and (store mode) the FFT
-//                              input H with plain coalesced stores: no memset, no global atomics.  Chunks of a heavy
-//                              tile publish partial tiles; the last chunk to arrive adds them up in chunk order.
+//                              tile with native integer adds.  The tile is written to G and Gw with plain coalesced
+//                              stores: no memset, no global atomics.  Chunks of a heavy tile publish partial tiles,
+//                              which are added up in two levels, always in chunk order (no CTA waits for another).
 // Passages: PAPER.md:78 (gridding = convolution onto a regular grid), :136-138 (spheroidal GCF), :216-228 (float2
 // grid, row-major, Hermitian), :249-256 (DIRTY_IMAGE).  The binning and tiling are this build's design.
 #include "muser_internal.h"
