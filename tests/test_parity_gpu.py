@@ -393,6 +393,44 @@ def test_wprojection_unevenly_spaced_planes_take_the_full_plane_scan():
         im.destroy()
 
 
+def test_wprojection_calls_capture_into_a_cuda_graph():
+    """reset -> grid -> dirty_psf in w mode only enqueue work (the per-shape kernels fork onto side streams and join the
+    caller's stream with events), so the sequence captures into a CUDA graph; the replay equals the plain calls."""
+    import torch
+    n, cell, P, Q, w_max = 256, 60.0, 6, 16, 4000.0
+    wc, sup = mo.wplane_layout(n, cell, P, w_max)
+    uvw, freq, vis, wt = synth.random_visibilities(11, 20000, n, cell, margin_cells=sup.max() / 2 + 2, w_max_lambda=w_max)
+    vis = (1.0 + 0.2 * vis).astype(np.complex64)
+    im = gu.make_imager(n, cell, 7, Q)
+    try:
+        im.set_wplanes(wc, sup, None)
+        dev = [gu.to_dev(a) for a in (uvw, freq, vis, wt)]
+        d = torch.empty((1, n, n), device="cuda"); b = torch.empty_like(d)
+
+        def step(s=None):
+            im.reset(s); im.grid(*dev, stream=s); im.dirty_psf(d, b, s)
+
+        step()
+        torch.cuda.synchronize()
+        ref_d, ref_b = d.clone(), b.clone()
+        side = torch.cuda.Stream()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            step(side.cuda_stream)                           # allocations happen outside the capture
+            torch.cuda.synchronize()
+            with torch.cuda.graph(graph, stream=side):
+                step(side.cuda_stream)
+        d.zero_(); b.zero_()
+        for _ in range(3):
+            graph.replay()
+        torch.cuda.synchronize()
+        q = n // 4                                           # (the corrected corners amplify fp32 reordering noise)
+        for got, ref in ((d, ref_d), (b, ref_b)):
+            assert float((got - ref)[:, q:-q, q:-q].abs().max()) <= 1e-5 * float(ref[:, q:-q, q:-q].abs().max())
+    finally:
+        im.destroy()
+
+
 @pytest.mark.parametrize("strategy", [TILED, WPLANE])
 def test_wprojection_small_supports_and_arbitrary_caller_tables(strategy):
     """Supports 1, 3, 5 (windows smaller than their register layout), 7 and 9 with arbitrary complex tables supplied by the
