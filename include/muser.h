@@ -173,6 +173,26 @@ int muser_get_peak(muser_imager* h, float* peak_value, int* peak_x, int* peak_y,
  * peak search of the last muser_dirty (reading R23).  hist_out: DEVICE unsigned [ngrids][nbins], overwritten. */
 int muser_histogram(muser_imager* h, const float* image, int nbins, float lo, float hi, unsigned int* hist_out, muser_stream s);
 
+/* The same own-range histogram for callers that cannot allocate device memory: no handle, no cudaMalloc / cudaFree and no
+ * allocating library call, on any call.  Meant for a steady-state monitoring loop, where cudaMalloc would
+ * synchronise the device and stall the imaging streams, and for processes in which another allocator (a framework's caching
+ * pool) already holds the HBM so that cudaMalloc fails.  The only scratch the histogram needs -- one minimum / maximum slot per
+ * image -- is a fixed __device__ array inside the library (16 KB, held by every GPU that loads libmuser.so until exit).
+ *   image    DEVICE float [ngrids][npix]      any images (non-finite pixels are ignored), on the CURRENT device
+ *   hist_out DEVICE unsigned [ngrids][nbins]  overwritten; image g is binned over its own [min, max] exactly as
+ *                                             muser_histogram(lo >= hi) bins the dirty image (reading R23); an image without a
+ *                                             finite pixel gives zeros, a constant image puts everything into bin 0
+ *   err_out  HOST char [err_cap] or NULL      text of the error when the return code is not MUSER_OK
+ * Limits and sharing: 1 <= ngrids <= MUSER_STATIC_MAX_GRIDS, else MUSER_EINVAL and nothing is enqueued; 1 <= nbins <= 8192;
+ * npix >= 1.  All calls on a device share the one array.  Each call first clears the slots it uses (they still hold the
+ * previous call's values), so calls queued on ONE stream are independent of each other; calls that may overlap on the GPU
+ * (different streams without an event between them) race on the slots.  The first call on each device also looks up the
+ * array's device address (cudaGetSymbolAddress; the runtime loads the module then): make it at start-up, before any stream
+ * capture.  Only enqueues on s (two memsets, two kernels); the caller synchronises s before reading hist_out. */
+#define MUSER_STATIC_MAX_GRIDS 1024
+int muser_histogram_static(const float* image, long long npix, int ngrids, int nbins, unsigned int* hist_out, muser_stream s,
+                           char* err_out, int err_cap);
+
 /* ---- whole path with HOST buffers (end-to-end entry point) ------------------------------------------------
  * reset -> copy the inputs to the device -> grid -> dirty + psf -> copy the images back, all on s, then
  * synchronises s.  HOST pointers (pinned memory makes the copies asynchronous); grid_id may be NULL;

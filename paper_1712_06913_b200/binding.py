@@ -42,6 +42,7 @@ SIGNATURES = {
     "muser_set_peak_search": (_i, [_vp, _i]),
     "muser_get_peak": (_i, [_vp, _vp, _vp, _vp, _vp]),
     "muser_histogram": (_i, [_vp, _vp, _i, _c.c_float, _c.c_float, _vp, _vp]),
+    "muser_histogram_static": (_i, [_vp, _ll, _i, _i, _vp, _vp, _vp, _i]),
     "muser_reset": (_i, [_vp, _vp]),
     "muser_grid": (_i, [_vp, _vp, _vp, _vp, _vp, _ll, _vp]),
     "muser_grid_batched": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _ll, _vp]),
@@ -293,6 +294,22 @@ def host_corrector(table, support, oversample, n):
     if rc:
         raise MuserError(rc, "muser_host_corrector")
     return out
+
+
+MUSER_STATIC_MAX_GRIDS = 1024
+
+
+def histogram_static(image, nbins, hist_out, stream=None):
+    """muser_histogram_static: own-range histograms of `image` (device float [ngrids][...]) into `hist_out` (device
+    uint32/int32 [ngrids][nbins]) without a handle and without any device allocation inside the library: for callers that
+    cannot cudaMalloc (a steady-state monitoring loop, a process whose HBM belongs to another allocator).  At most
+    MUSER_STATIC_MAX_GRIDS images per call; calls share one scratch array per device, so keep them on one stream."""
+    ngrids = int(image.shape[0])
+    npix = int(image.numel() // max(ngrids, 1))
+    err = ctypes.create_string_buffer(256)
+    rc = lib().muser_histogram_static(_ptr(image), npix, ngrids, int(nbins), _ptr(hist_out), _stream(stream), err, len(err))
+    if rc:
+        raise MuserError(rc, err.value.decode())
 
 
 MICROBENCH = ("fp32_fma_flops", "fp32_ffma2_flops", "shared_int_adds", "shared_f32_cas_adds", "global_f32_red_adds")

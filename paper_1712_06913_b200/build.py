@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmuser.so")
-SOURCES = ["muser_api.cu", "muser_kernels.cu", "muser_owner.cu", "muser_wgrid.cu", "muser_fft.cu", "muser_microbench.cu", "tables.cpp"]
+SOURCES = ["muser_api.cu", "muser_kernels.cu", "muser_owner.cu", "muser_wgrid.cu", "muser_fft.cu", "muser_microbench.cu", "muser_static.cu", "tables.cpp"]
 HEADERS = ["muser_internal.h", "tables.h", os.path.join("..", "..", "include", "muser.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
