@@ -2,7 +2,8 @@
  *
  * The path: calibrated visibilities -> [A1] coordinates + binning (counting sort by uv tile)
  *        -> [A2/A3/A4] convolutional gridding (2-D, w-projection planes, batched grids)
- *        -> [A5] 2-D inverse FFT (cuFFT) -> [A6] fused grid correction + fftshift + real part
+ *        -> [A5] 2-D inverse FFT (the library's own half-plane row pass + column pass for power-of-two sizes, cuFFT otherwise)
+ *        -> [A6] grid correction + fftshift + real part (the column pass's epilogue)
  *        -> dirty image and dirty beam (PSF).
  * Paper passages (PAPER.md = the paper's text; DESIGN.md restates every reading R1..R21):
  *   "Gridding is the convolution of the visibilities with a particular function, which resamples the
@@ -109,7 +110,9 @@ int muser_set_weighting(muser_imager* h, int mode);
 int muser_set_phase_offset(muser_imager* h, double dl, double dm);
 /* NEXT-2b: CLEAN wants a beam twice the size of the image.  When enabled, every muser_grid /
  * muser_grid_batched call also grids the weights onto a second set of grids of 2nx x 2ny cells (same cell size, same
- * kernel), and muser_psf2x returns that beam: DEVICE float [ngrids][2ny][2nx].  2-D mode only.  May synchronise. */
+ * kernel), and muser_psf2x returns that beam: DEVICE float [ngrids][2ny][2nx].  muser_frame_host(_async) grids it too.  Later
+ * muser_set_kernel / muser_set_strategy / muser_set_batch / muser_set_weighting calls apply to it as well.  2-D mode only:
+ * while it is enabled muser_set_wplanes(n > 0) returns MUSER_EUNSUPPORTED.  May synchronise. */
 int muser_set_psf2x(muser_imager* h, int enabled);
 int muser_psf2x(muser_imager* h, float* beam2x_out, muser_stream s);
 
@@ -170,7 +173,8 @@ int muser_get_peak(muser_imager* h, float* peak_value, int* peak_x, int* peak_y,
 /* "the data from a dirty image is divided into 2000 ranges" (the input of the GMM): histogram of `image`
  * (DEVICE float [ngrids][ny][nx]) into nbins equal ranges of [lo, hi]: bin = floor((v - lo) * (nbins / (hi - lo))) in
  * fp32, hi itself in the last bin, values outside not counted.  lo >= hi: each grid's own minimum and maximum from the
- * peak search of the last muser_dirty (reading R23).  hist_out: DEVICE unsigned [ngrids][nbins], overwritten. */
+ * peak search of the last muser_dirty (reading R23); MUSER_ESTATE if the peak search is off or no dirty image has been made
+ * since it was switched on; a constant image (minimum == maximum) goes to bin 0.  hist_out: DEVICE unsigned [ngrids][nbins], overwritten. */
 int muser_histogram(muser_imager* h, const float* image, int nbins, float lo, float hi, unsigned int* hist_out, muser_stream s);
 
 /* The same own-range histogram for callers that cannot allocate device memory: no handle, no cudaMalloc / cudaFree and no

@@ -47,6 +47,7 @@ struct muser_imager {
     double off_l = 0.0, off_m = 0.0;        // phase-centre offset (NEXT-3)
     bool peak_search = false;               // NEXT-4: peak / minimum of the dirty image kept per grid
     PeakSlot* peaks_d = nullptr;
+    bool peaks_valid = false;               // a dirty image has filled peaks_d since the search was enabled / the grids were (re)allocated
     muser_imager* child2x = nullptr;        // NEXT-2b: imager of 2nx x 2ny pixels gridding the weights only
     Staged* staged = nullptr;
     Sample* sorted = nullptr;
@@ -204,6 +205,7 @@ int alloc_grids(muser_imager* h) {
     h->sparse = false;
     CU(h, cudaMalloc(&h->peaks_d, (size_t)h->ngrids * sizeof(PeakSlot)));
     CU(h, cudaMemset(h->peaks_d, 0, (size_t)h->ngrids * sizeof(PeakSlot)));
+    h->peaks_valid = false;
     CU(h, cudaDeviceSynchronize());
     h->fft_valid = false;
     h->zero_pending = false;
@@ -369,7 +371,8 @@ int pick_strategy(const muser_imager* h) {
 }
 
 uint32_t owner_item_size(long long nvis, int num_sms, int item_override) {
-    // Heavy tiles are split into chunks of item_size samples.  4096 (the gridder's sort capacity) when the call has
+    // Heavy tiles are split into chunks of item_size samples.  4096 (the gridder sorts a chunk in units of kOwUnit = 4096
+    // records; a larger chunk -- MUSER_TUNE_ITEM_SIZE up to 2^20, or the growth rule below -- is several units) when the call has
     // enough work to fill the machine; down to 256 for a single small frame, whose latency is the critical path of
     // one chunk (a third of a MUSER frame sits in the tile around the uv origin; the partial tiles are summed in two
     // levels, so 147 chunks cost less than 37 did: measured 76 us per frame at 256 against 88 at 1024).  For huge inputs
@@ -538,7 +541,8 @@ int grid_impl(muser_imager* h, const float* uvw, const double* freq, const void*
     return grid_generic(h, strat, uvw, freq, vis, wt, gid, nvis, nullptr, s);
 }
 
-// NEXT-1: the channelised call.  Owner-tile strategy only (2-D mode, support 7): its binning kernels have the rows variant.
+// NEXT-1: the channelised call.  Every strategy: the owner-tile path has its own rows binning kernels (k_rows_count /
+// k_rows_scatter); TILED and WPLANE go through grid_generic with k_coords<ROWS>.
 int grid_rows_impl(muser_imager* h, const float* uvw, const double* freq, const void* vis, const float* wt, const int* gid,
                    long long nrow, int nchan, int npol, int ntime, int pol_mode, cudaStream_t s) {
     if (nrow < 0 || nchan < 1 || npol < 1 || ntime < 1 || nchan > rows_max_channels() || npol > 8)
@@ -637,7 +641,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
-        if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
+        if (peaks) { CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s)); h->peaks_valid = true; }
         CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
         h->n_launches += 1;
         return MUSER_OK;
@@ -668,7 +672,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
-        if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
+        if (peaks) { CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s)); h->peaks_valid = true; }
         CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
         h->n_launches += 1;
         return MUSER_OK;
@@ -700,7 +704,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
-        if (peaks) CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s));
+        if (peaks) { CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s)); h->peaks_valid = true; }
         CU(h, launch_correct(h->geom, h->H, cx, cy, h->stats_d, dirty, psf, peaks, s));
         h->n_launches += 1;
     }
@@ -721,6 +725,15 @@ int reset_impl(muser_imager* h, cudaStream_t s) {
     CU(h, cudaMemsetAsync(h->stats_d, 0, sizeof(Stats), s));
     if (h->cnt) CU(h, cudaMemsetAsync(h->cnt, 0, grid_cells(h) * sizeof(int), s));
     if (h->child2x) return reset_impl(h->child2x, s);
+    return MUSER_OK;
+}
+
+// The set_* calls reset on the legacy stream; a caller's cudaStreamNonBlocking stream is not ordered after that stream, so
+// they wait for the memsets here (they are set-up calls: every one of them synchronises the device at entry already).
+int reset_sync(muser_imager* h) {
+    int rc = reset_impl(h, nullptr);
+    if (rc) return rc;
+    CU(h, cudaDeviceSynchronize());
     return MUSER_OK;
 }
 
@@ -839,8 +852,12 @@ int muser_set_kernel(muser_imager* h, int kind, double param) {
     int rc = rebuild_geom(h);
     if (rc) return rc;
     if ((rc = build_2d_tables(h))) return rc;
-    if (was_w) return alloc_grids(h);
-    return reset_impl(h, nullptr);
+    rc = was_w ? alloc_grids(h) : reset_sync(h);
+    if (rc == MUSER_OK && h->child2x) {                               // the 2x beam is gridded with the same kernel
+        rc = muser_set_kernel(h->child2x, kind, param);
+        if (rc) h->err = "2x beam: " + h->child2x->err;
+    }
+    return rc;
 }
 
 int muser_set_batch(muser_imager* h, int ngrids) {
@@ -867,8 +884,9 @@ int muser_set_wplanes(muser_imager* h, int nplanes, const double* w_centres, con
         int rc = rebuild_geom(h);
         if (rc) return rc;
         if ((rc = build_2d_tables(h))) return rc;
-        return was_w ? alloc_grids(h) : reset_impl(h, nullptr);
+        return was_w ? alloc_grids(h) : reset_sync(h);
     }
+    if (h->child2x) return fail(h, MUSER_EUNSUPPORTED, "the 2x beam is built in 2-D mode only: switch it off (muser_set_psf2x(h, 0)) before entering w mode");
     if (!w_centres || !supports) return fail(h, MUSER_EINVAL, "w_centres and supports are required");
     std::vector<int> sup(nplanes);
     std::vector<double> wc(nplanes);
@@ -928,6 +946,10 @@ int muser_set_strategy(muser_imager* h, int strategy) {
         if (rc) return rc;
     }
     h->strategy = strategy;
+    if (h->child2x) {
+        int rc = muser_set_strategy(h->child2x, strategy);
+        if (rc) { h->err = "2x beam: " + h->child2x->err; return rc; }
+    }
     return MUSER_OK;
 }
 
@@ -971,6 +993,7 @@ int muser_set_phase_offset(muser_imager* h, double dl, double dm) {
 
 int muser_set_peak_search(muser_imager* h, int enabled) {
     if (!h) return MUSER_EINVAL;
+    if ((enabled != 0) != h->peak_search) h->peaks_valid = false;
     h->peak_search = enabled != 0;
     return MUSER_OK;
 }
@@ -1002,6 +1025,7 @@ int muser_histogram(muser_imager* h, const float* image, int nbins, float lo, fl
     if (nbins < 1 || nbins > 8192) return fail(h, MUSER_EINVAL, "nbins must be in [1, 8192]");
     const bool own_range = !(lo < hi);
     if (own_range && !h->peak_search) return fail(h, MUSER_ESTATE, "lo >= hi asks for the image's own range: enable the peak search first");
+    if (own_range && !h->peaks_valid) return fail(h, MUSER_ESTATE, "lo >= hi asks for the image's own range: no dirty image has been made since the peak search was enabled");
     if (h->ngrids > 65535) return fail(h, MUSER_EUNSUPPORTED, "histogram of more than 65535 grids per call");
     cudaStream_t s = (cudaStream_t)sv;
     h->last_stream = s;
@@ -1156,6 +1180,10 @@ static int frame_host_impl(muser_imager* h, const float* uvw_m, const double* fr
         if (grid_id) CU(h, cudaMemcpyAsync(h->in_gid, grid_id, (size_t)nvis * sizeof(int), cudaMemcpyHostToDevice, s));
         rc = grid_impl(h, h->in_uvw, h->in_freq, h->in_vis, h->in_wt, grid_id ? h->in_gid : nullptr, nvis, s);
         if (rc) return rc;
+        if (h->child2x) {                                             // reset_impl above has reset the child as well
+            rc = grid_impl(h->child2x, h->in_uvw, h->in_freq, nullptr, h->in_wt, grid_id ? h->in_gid : nullptr, nvis, s);
+            if (rc) { h->err = "2x beam: " + h->child2x->err; return rc; }
+        }
     }
     rc = image_impl(h, image_out ? h->out_dirty : nullptr, beam_out ? h->out_psf : nullptr, s);
     if (rc) return rc;

@@ -685,7 +685,7 @@ cudaError_t fft_rows_setup() {
 
 cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
                                  Stats* stats, float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s) {
-    if (g.otx > 96) valid = nullptr;                                     // (the caller made the grids dense: see fft_rows_valid_ok)
+    if (g.otx > 96) valid = nullptr;                                     // (image_impl made the grids dense: its rows_take_flags needs otx <= 96)
 #define MUSER_ROWS_CASE(NN)                                                                                     \
     case NN:                                                                                                    \
         return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, cnt, tw, stats, Z, valid, num_sms, s)                   \

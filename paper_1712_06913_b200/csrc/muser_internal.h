@@ -174,7 +174,7 @@ cudaError_t launch_owner_grid(const Geom& g, const uint4* sorted, const uint32_t
 // stand for zeros whatever they hold).  Zero those tiles and flag them:
 cudaError_t launch_owner_fill_invalid(const Geom& g, GridPtrs grids, uint32_t* valid, cudaStream_t s);
 
-// ---- fused column transform + correction (muser_fft.cu): ny = 256, 512 or 1024, nx a multiple of 16
+// ---- fused column transform + correction (muser_fft.cu): ny = 256, 512, 1024, 2048 or 4096, nx a multiple of 16
 bool fft_cols_supported(int nx, int ny);
 int fft_cols_first_radix(int ny);
 cudaError_t fft_cols_setup();

@@ -793,7 +793,7 @@ __global__ void __launch_bounds__(256) k_histogram(const float* __restrict__ ima
         hi = peak_unordered((unsigned int)(peaks[gi].maxkey >> 32));
         lo = peak_unordered(~peaks[gi].minkey);
     }
-    const float scale = __fdiv_rn((float)nbins, __fsub_rn(hi, lo));
+    const float scale = (lo < hi) ? __fdiv_rn((float)nbins, __fsub_rn(hi, lo)) : 0.0f;     // constant image (own range, hi == lo): everything in bin 0
     __syncthreads();
     const float* img = image + (size_t)gi * npix;
     for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < npix; i += (size_t)gridDim.x * 256) {

@@ -108,10 +108,12 @@ def check_images(im, G_or, Gw_or, T, S, Q, tol=IMG_TOL):
 
 
 def run_case(uvw, freq, vis, wt, n, cell, S, Q, kernel="pswf", gauss_a=0.0, strategy=binding.MUSER_STRATEGY_AUTO,
-             grid_id=None, ngrids=1, splits=1, images=True):
+             grid_id=None, ngrids=1, splits=1, images=True, item_size=0):
     """Grid on the GPU (optionally in `splits` accumulating calls) and in the oracle; assert parity; return both."""
     im = make_imager(n, cell, S, Q, kernel, gauss_a, ngrids, strategy)
     try:
+        if item_size:
+            im.set_tuning(binding.MUSER_TUNE_ITEM_SIZE, item_size)
         d = [to_dev(uvw), to_dev(freq), to_dev(vis), to_dev(wt)]
         dg = to_dev(np.asarray(grid_id, np.int32)) if grid_id is not None else None
         nvis = vis.shape[0]

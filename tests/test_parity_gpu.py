@@ -180,9 +180,12 @@ def test_owner_strategy_random_visibilities(Q, nvis, n, ny):
             im.destroy()
 
 
-def test_owner_heavy_tile_is_split_into_chunks_and_summed():
+@pytest.mark.parametrize("item_size", [0, 10000, 1 << 20])
+def test_owner_heavy_tile_is_split_into_chunks_and_summed(item_size):
     """40,000 visibilities inside +-6 cells of the uv origin: the centre tile holds ~80,000 samples = 20 chunk items
-    whose partial tiles the last chunk adds up; the second call exercises accumulate mode on a heavy tile."""
+    whose partial tiles the last chunk adds up; the second call exercises accumulate mode on a heavy tile.
+    item_size 10000: chunks of several sort units (kOwUnit = 4096) with a ragged last unit; 2^20: the whole tile is one
+    item of ~10 units (the multi-unit path of k_grid_owner_s7, no partial-tile sum)."""
     n, cell, Q = 256, 20.0, 64
     rng = np.random.default_rng(99)
     nvis = 40000
@@ -195,7 +198,7 @@ def test_owner_heavy_tile_is_split_into_chunks_and_summed():
     wt = rng.uniform(0.5, 1.5, nvis).astype(np.float32)
     # images=False: with all the power inside +-6 cells of the origin the image is smooth and small against the fp32
     # FFT noise that 1/(cx*cy) amplifies towards the edge of the 75% box; the grid gates are what this case is about
-    res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, Q, strategy=OWNER, splits=2, images=False)
+    res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, Q, strategy=OWNER, splits=2, images=False, item_size=item_size)
     assert res["stats"]["n_gridded"] == nvis
 
 
