@@ -24,7 +24,8 @@ Two layers:
   (II) the algorithm step by step: O1 coordinates -> O2 table -> O3 gridding -> O4 transform -> O5 correction
        (+ O6 w-projection planes)                            -> `coordinates`, `table_*`, `grid`, `transform`,
                                                                 `corrector`, `dirty_image`
-Pins (tests/test_oracle_*.py, all `-m "not gpu"`): P1..P12 of DESIGN.md for the path, N1..N4 (tests/test_oracle_next.py)
+Pins (tests/test_oracle_*.py, all `-m "not gpu"`): P1..P16 of DESIGN.md for the path (P13..P16, tests/test_oracle_pins2.py:
+keep / drop boundary, plane selection, flag rule and the fp32 bin decision, each by hand), N1..N4 (tests/test_oracle_next.py)
 for the NEXT rows at the end of this file (channelised input, Hermitian half-plane, uniform weighting as the paper
 prints it, phase correction, peak / histogram).  No function here is unpinned; what stays unpinned *by the paper* is
 the identity of its own GCF coefficients and w-kernels (R2, R15).

@@ -694,3 +694,83 @@ def test_owner_fixed_point_merge_bound_per_cell_with_a_1e6_outlier():
     faint = (np.abs(G_or[up]) > 0.05) & (np.abs(G_or[up]) < 50.0)
     assert faint.sum() > 500 and err[faint].max() <= m_max * 0.5 * unit * np.sqrt(2.0)
     assert err[faint].max() < 20 * unit                       # in practice a handful of merges per cell
+
+
+def _edge_visibilities(n, cell, h, seed, w_max=0.0):
+    """Visibilities whose nearest cell is h, h + 1, n - 1 - h or n - h on one axis or on both (the keep / drop boundary of R5,
+    oracle pin P13), at random sub-cell offsets, plus exact half-cell ties at the boundary (frequency scanned ulp by ulp so
+    that O1's own operation order lands on the tie exactly)."""
+    rng = np.random.default_rng([7, seed])
+    su = n * cell * mo.ARCSEC
+    edge = np.array([h, h + 1, n - 1 - h, n - h], np.float64)
+    m = 600
+    pu = rng.choice(edge, m) + rng.uniform(-0.49, 0.49, m)
+    pv = rng.uniform(h + 2, n - h - 2, m)
+    pu[m // 3:2 * m // 3], pv[m // 3:2 * m // 3] = pv[m // 3:2 * m // 3].copy(), (rng.choice(edge, m) + rng.uniform(-0.49, 0.49, m))[m // 3:2 * m // 3]
+    pv[2 * m // 3:] = rng.choice(edge, m - 2 * m // 3) + rng.uniform(-0.49, 0.49, m - 2 * m // 3)      # corners: both axes at the edge
+    freq = np.full(m, 1.0e9)
+    lam = mo.C_M_S / 1.0e9
+    uvw = np.zeros((m, 3), np.float32)
+    uvw[:, 0] = ((pu - n / 2) / su * lam).astype(np.float32)
+    uvw[:, 1] = ((pv - n / 2) / su * lam).astype(np.float32)
+    ties = []
+    for off in (n / 2 - h - 0.5, -(n / 2 - h - 0.5), n / 2 - h - 1.5, -(n / 2 - h - 1.5)):
+        um = np.float32(off / su * lam)
+        f = off / (float(um) * su) * mo.C_M_S
+        for _ in range(4000):
+            f = np.nextafter(f, -np.inf)
+        for _ in range(8000):
+            if float(um) * (f / mo.C_M_S) * su == off:
+                ties.append((um, float(f)))
+                break
+            f = np.nextafter(f, np.inf)
+    assert len(ties) >= 2
+    tu = np.zeros((2 * len(ties), 3), np.float32)
+    tf = np.empty(2 * len(ties))
+    for i, (um, f) in enumerate(ties):
+        tu[2 * i, 0] = um; tu[2 * i + 1, 1] = um                      # the tie on the u axis, then on the v axis
+        tf[2 * i] = tf[2 * i + 1] = f
+    uvw = np.concatenate([uvw, tu]); freq = np.concatenate([freq, tf])
+    nv = uvw.shape[0]
+    if w_max > 0:
+        uvw[:, 2] = (rng.uniform(-w_max, w_max, nv) * lam).astype(np.float32)
+    vis = (rng.standard_normal(nv) + 1j * rng.standard_normal(nv)).astype(np.complex64)
+    wt = rng.uniform(0.5, 1.5, nv).astype(np.float32)
+    return uvw, freq, vis, wt
+
+
+@pytest.mark.parametrize("strategy", [OWNER, TILED])
+def test_keep_drop_boundary_cells_2d(strategy):
+    """Samples on cells h, h+1, n-1-h, n-h (and exact ties there): kept / dropped counts and grids equal the oracle's (P13 pins
+    the oracle's rule by hand); nothing is written to row / column 0."""
+    n, cell, Q = 256, 20.0, 16
+    uvw, freq, vis, wt = _edge_visibilities(n, cell, 3, 1)
+    res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, Q, strategy=strategy, images=False)
+    assert res["stats"]["n_dropped"] > 100 and res["stats"]["n_gridded"] > 100
+    assert not res["G"][0][0, :].any() and not res["G"][0][:, 0].any()
+    assert res["G"][0][:, 1].any() and res["G"][0][:, n - 1].any()
+
+
+@pytest.mark.parametrize("strategy", [TILED, WPLANE])
+def test_keep_drop_boundary_cells_wplanes(strategy):
+    """The same with two w planes of supports 7 and 9: the boundary depends on the plane a visibility falls into."""
+    n, cell, Q = 256, 20.0, 16
+    wc, sup = np.array([0.0, 400.0]), np.array([7, 9])
+    fov = n * cell * mo.ARCSEC
+    tabs = [mo.table_wkernel(int(s_), Q, float(w_), fov) for s_, w_ in zip(sup, wc)]
+    uvw3, freq3, vis3, wt3 = _edge_visibilities(n, cell, 3, 2, w_max=400.0)
+    uvw4, freq4, vis4, wt4 = _edge_visibilities(n, cell, 4, 3, w_max=400.0)
+    uvw, freq, vis, wt = (np.concatenate(a) for a in ((uvw3, uvw4), (freq3, freq4), (vis3, vis4), (wt3, wt4)))
+    im = gu.make_imager(n, cell, 7, Q, strategy=strategy)
+    try:
+        im.set_wplanes(wc, sup, [t.astype(np.complex64) for t in tabs])
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        G, Gw = gu.gpu_grids(im)
+        G_or, Gw_or, st_or = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, sup, tabs, wc=wc)
+        st = im.get_stats()
+        assert (st["n_gridded"], st["n_dropped"], st["n_flagged"]) == (st_or["n_gridded"], st_or["n_dropped"], st_or["n_flagged"])
+        assert st["n_dropped"] > 200 and st["n_gridded"] > 200
+        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL and gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        assert not G[0][0, :].any() and not G[0][:, 0].any()
+    finally:
+        im.destroy()
