@@ -237,7 +237,8 @@ def _stage_us(im, step, reps):
         step()
     prof = im.get_profile()
     im.set_profiling(False)
-    return {k: (1e3 * v[0] / v[1] if v[1] else None) for k, v in prof.items()}
+    # per STEP (a stage may be several launches per step: the transform runs rows -> columns over sub-batches of grids)
+    return {k: (1e3 * v[0] / reps if v[1] else None) for k, v in prof.items()}
 
 
 def _timed(torch, stream, fn, steps, barrier):

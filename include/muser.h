@@ -90,8 +90,10 @@ int muser_set_strategy(muser_imager* h, int strategy);
  * per chunk of a heavy tile (a tile with more records is split into chunks gridded by different CTAs and summed);
  * 0 (default) = chosen from the size of the call.  BIN_ITERS: blocks of 256 visibilities a binning CTA loops over
  * (1..64; 0 = automatic).  COLS_TMA: how the fused column transform fetches its strip of 8 columns: 1 = per-lane loads,
- * 2 = cp.async.bulk.tensor (TMA) into shared memory, 0 = the library's default. */
-enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_BIN_ITERS = 1, MUSER_TUNE_COLS_TMA = 2, MUSER_TUNE_COUNT = 3 };
+ * 2 = cp.async.bulk.tensor (TMA) into shared memory, 0 = the library's default.  FFT_SUBBATCH: grids per rows -> columns
+ * sub-batch of the fused transform (the row transform of a sub-batch stays in L2 until its column pass has read it);
+ * 0 (default) or >= ngrids = all rows, then all columns, which measured fastest. */
+enum { MUSER_TUNE_ITEM_SIZE = 0, MUSER_TUNE_BIN_ITERS = 1, MUSER_TUNE_COLS_TMA = 2, MUSER_TUNE_FFT_SUBBATCH = 3, MUSER_TUNE_COUNT = 4 };
 int muser_set_tuning(muser_imager* h, int key, int value);
 /* 1 (default): A6 divides by the kernel's transform; 0: A6 only shifts/takes the real part (parity gate R9(i)). */
 int muser_set_grid_correction(muser_imager* h, int enabled);

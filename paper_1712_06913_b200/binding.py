@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libmuser.so")
 MUSER_OK, MUSER_EINVAL, MUSER_ECUDA, MUSER_ENOMEM, MUSER_ESTATE, MUSER_EUNSUPPORTED = range(6)
 MUSER_KERNEL_PSWF, MUSER_KERNEL_GAUSS = 0, 1
 MUSER_STRATEGY_AUTO, MUSER_STRATEGY_TILED, MUSER_STRATEGY_OWNER, MUSER_STRATEGY_WPLANE = 0, 2, 3, 4
-MUSER_TUNE_ITEM_SIZE, MUSER_TUNE_BIN_ITERS, MUSER_TUNE_COLS_TMA = 0, 1, 2
+MUSER_TUNE_ITEM_SIZE, MUSER_TUNE_BIN_ITERS, MUSER_TUNE_COLS_TMA, MUSER_TUNE_FFT_SUBBATCH = 0, 1, 2, 3
 MUSER_WEIGHT_NATURAL, MUSER_WEIGHT_UNIFORM = 0, 1
 MUSER_POLS_SUM, MUSER_POLS_SPLIT = 0, 1
 STAGES = ("bin", "grid", "pack", "fft", "correct")

@@ -616,6 +616,14 @@ const void* cols_tmap(muser_imager* h) {
     return h->tmap_ok ? h->tmap : nullptr;
 }
 
+// Grids per rows -> columns sub-batch of the fused transform: MUSER_TUNE_FFT_SUBBATCH, or (0, the default) every grid in
+// one batch.  Measured on cfg 3 (80 x 1024^2) and on 1024 x 512^2 (round 3): the partial waves of the smaller
+// launches cost more than the L2 hits of the column pass save at every sub-batch size, so the knob stays off.
+int fft_subbatch(const muser_imager* h) {
+    const int t = h->tune[MUSER_TUNE_FFT_SUBBATCH];
+    return t > 0 ? std::min(t, h->ngrids) : h->ngrids;
+}
+
 int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
     if (!dirty && !psf) return MUSER_OK;
     h->last_stream = s;
@@ -630,20 +638,29 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         // A5 rows by k_fft_rows_half straight from the stored half-planes of G and Gw (H = G + i alpha Gw is never
         // materialised and rows < ny/2 are never read), A5 columns + A6 by the fused column kernel; H keeps the row
         // transform, so muser_dirty followed by muser_psf repeats only the column pass
-        if (!h->fft_valid) {
-            StageScope sc(h, MUSER_STAGE_FFT, s);
-            CU(h, launch_fft_rows_half(h->geom, h->G, h->Gw, h->cnt, h->tw_rows_d, h->stats_d, h->H, h->sparse ? h->ow_valid : nullptr,
-                                       h->num_sms, s));
-            h->n_launches += 1;
-            h->fft_valid = true;
-        }
-        StageScope sc(h, MUSER_STAGE_CORRECT, s);
         const float* cx = h->correction ? h->icx_d : h->ones_d;
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
         if (peaks) { CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s)); h->peaks_valid = true; }
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
-        h->n_launches += 1;
+        // The row transform H of one grid (8 B per cell) is written by the row pass and read once by the column pass.  Running
+        // rows -> columns over sub-batches of a few grids would keep that round trip inside the 126 MB L2 instead of DRAM
+        // (MUSER_TUNE_FFT_SUBBATCH); measured slower than one batch at every size, so the default is one batch.
+        const int sub = fft_subbatch(h);
+        const void* tmap = cols_tmap(h);
+        const bool need_rows = !h->fft_valid;
+        for (int g0 = 0; g0 < h->ngrids; g0 += sub) {
+            const int gc = std::min(sub, h->ngrids - g0);
+            if (need_rows) {
+                StageScope sc(h, MUSER_STAGE_FFT, s);
+                CU(h, launch_fft_rows_half(h->geom, h->G, h->Gw, h->cnt, h->tw_rows_d, h->stats_d, h->H, h->sparse ? h->ow_valid : nullptr,
+                                           g0, gc, h->num_sms, s));
+                h->n_launches += 1;
+            }
+            StageScope sc(h, MUSER_STAGE_CORRECT, s);
+            CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, tmap, g0, gc, s));
+            h->n_launches += 1;
+        }
+        h->fft_valid = true;
         return MUSER_OK;
     }
     if (h->fused_fft) {
@@ -673,7 +690,7 @@ int image_impl(muser_imager* h, float* dirty, float* psf, cudaStream_t s) {
         const float* cy = h->correction ? h->icy_d : h->ones_d;
         PeakSlot* peaks = (h->peak_search && dirty) ? h->peaks_d : nullptr;
         if (peaks) { CU(h, cudaMemsetAsync(peaks, 0, (size_t)h->ngrids * sizeof(PeakSlot), s)); h->peaks_valid = true; }
-        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), s));
+        CU(h, launch_fft_cols_correct(h->geom, h->H, h->tw_d, h->tw8_d, cx, cy, h->stats_d, dirty, psf, peaks, cols_tmap(h), 0, h->ngrids, s));
         h->n_launches += 1;
         return MUSER_OK;
     }
@@ -959,6 +976,7 @@ int muser_set_tuning(muser_imager* h, int key, int value) {
     if (key == MUSER_TUNE_ITEM_SIZE && value != 0 && (value < 64 || value > (1 << 20))) return fail(h, MUSER_EINVAL, "item_size must be 0 (automatic) or in [64, 2^20]");
     if (key == MUSER_TUNE_BIN_ITERS && (value < 0 || value > 64)) return fail(h, MUSER_EINVAL, "bin_iters must be in [0, 64]");
     if (key == MUSER_TUNE_COLS_TMA && (value < 0 || value > 2)) return fail(h, MUSER_EINVAL, "cols_tma must be 0, 1 or 2");
+    if (key == MUSER_TUNE_FFT_SUBBATCH && value < 0) return fail(h, MUSER_EINVAL, "fft_subbatch must be 0 (automatic) or a number of grids >= 1");
     h->tune[key] = value;
     return rebuild_geom(h);
 }

@@ -398,7 +398,7 @@ __device__ __forceinline__ float ldg_f_if(const float* p, const bool ok) {
 }
 
 template <int N, int WMODE, int UNIFORM>
-__global__ void __launch_bounds__(N / 4, N == 1024 ? 3 : (N == 512 ? 6 : 1)) k_fft_rows_half(const int ny, const int ngroups, const float2* __restrict__ G,
+__global__ void __launch_bounds__(N / 4, N == 1024 ? 3 : (N == 512 ? 6 : 1)) k_fft_rows_half(const int ny, const int grp0, const int ngroups, const float2* __restrict__ G,
                                                          const float* __restrict__ Gw, const int* __restrict__ cnt,
                                                          const float2* __restrict__ tw, Stats* __restrict__ stats,
                                                          float2* __restrict__ Z, const uint32_t* __restrict__ valid,
@@ -429,8 +429,8 @@ __global__ void __launch_bounds__(N / 4, N == 1024 ? 3 : (N == 512 ? 6 : 1)) k_f
             nflag[w] = t < otx ? __ldg(vrow + t) : 0u;
         }
     };
-    if (valid) load_flags(blockIdx.x);
-    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    if (valid) load_flags(grp0 + (int)blockIdx.x);
+    for (int grp = grp0 + (int)blockIdx.x; grp < ngroups; grp += gridDim.x) {       // groups [grp0, ngroups): the grids of this sub-batch
         const int gi = grp / gpg, iy0 = hy + (grp - gi * gpg) * ROWS;
         const size_t gbase = (size_t)gi * ny * N;
         // tile flags of this row of 64 x 32 tiles (the rows of a group lie in one tile row): a tile that has not been written
@@ -645,14 +645,15 @@ bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngri
 
 template <int N, int WMODE>
 static cudaError_t launch_rows_t(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw, Stats* stats,
-                                 float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s) {
+                                 float2* Z, const uint32_t* valid, int grid_begin, int grid_count, int num_sms, cudaStream_t s) {
     using C = RowCfg<N, WMODE>;
-    const int ngroups = g.ngrids * ((g.ny / 2) / C::ROWS);
+    const int gpg = (g.ny / 2) / C::ROWS;
+    const int grp0 = grid_begin * gpg, ngroups = (grid_begin + grid_count) * gpg, mine = grid_count * gpg;
     int per_sm = (int)(200 * 1024 / (C::SMEM + 1024));
     per_sm = per_sm < 1 ? 1 : (per_sm > 2048 / C::T ? 2048 / C::T : per_sm);
-    const int blocks = ngroups < num_sms * per_sm ? ngroups : num_sms * per_sm;
-    if (g.uniform && cnt) k_fft_rows_half<N, WMODE, 1><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, cnt, tw, stats, Z, valid, g.otx);
-    else k_fft_rows_half<N, WMODE, 0><<<blocks, C::T, C::SMEM, s>>>(g.ny, ngroups, G, Gw, nullptr, tw, stats, Z, valid, g.otx);
+    const int blocks = mine < num_sms * per_sm ? mine : num_sms * per_sm;
+    if (g.uniform && cnt) k_fft_rows_half<N, WMODE, 1><<<blocks, C::T, C::SMEM, s>>>(g.ny, grp0, ngroups, G, Gw, cnt, tw, stats, Z, valid, g.otx);
+    else k_fft_rows_half<N, WMODE, 0><<<blocks, C::T, C::SMEM, s>>>(g.ny, grp0, ngroups, G, Gw, nullptr, tw, stats, Z, valid, g.otx);
     return cudaGetLastError();
 }
 
@@ -684,12 +685,13 @@ cudaError_t fft_rows_setup() {
 }
 
 cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
-                                 Stats* stats, float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s) {
+                                 Stats* stats, float2* Z, const uint32_t* valid, int grid_begin, int grid_count, int num_sms,
+                                 cudaStream_t s) {
     if (g.otx > 96) valid = nullptr;                                     // (image_impl made the grids dense: its rows_take_flags needs otx <= 96)
 #define MUSER_ROWS_CASE(NN)                                                                                     \
     case NN:                                                                                                    \
-        return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, cnt, tw, stats, Z, valid, num_sms, s)                   \
-                       : launch_rows_t<NN, 0>(g, G, Gw, cnt, tw, stats, Z, valid, num_sms, s);
+        return g.wmode ? launch_rows_t<NN, 1>(g, G, Gw, cnt, tw, stats, Z, valid, grid_begin, grid_count, num_sms, s) \
+                       : launch_rows_t<NN, 0>(g, G, Gw, cnt, tw, stats, Z, valid, grid_begin, grid_count, num_sms, s);
     switch (g.nx) {
         MUSER_ROWS_CASE(64) MUSER_ROWS_CASE(128) MUSER_ROWS_CASE(256) MUSER_ROWS_CASE(512) MUSER_ROWS_CASE(1024)
         MUSER_ROWS_CASE(2048) MUSER_ROWS_CASE(4096)
@@ -702,12 +704,13 @@ bool fft_cols_radix8(int ny) { return ny == 512 || ny == 1024; }
 
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float2* tw8, const float* icx,
                                     const float* icy, const Stats* stats, float* dirty, float* psf, PeakSlot* peaks,
-                                    const void* tmap128, cudaStream_t s) {
+                                    const void* tmap128, int grid_begin, int grid_count, cudaStream_t s) {
     CUtensorMap map;
     memset(&map, 0, sizeof(map));
     if (tmap128) memcpy(&map, tmap128, sizeof(map));
-    for (int grid0 = 0; grid0 < g.ngrids; grid0 += 65535) {              // gridDim.y holds at most 65535 grids
-        const dim3 blocks((unsigned)(g.nx / fft_cols_per_cta(g.ny)), (unsigned)std::min(65535, g.ngrids - grid0));
+    const int grid_end = grid_begin + grid_count;                        // the grids of this sub-batch
+    for (int grid0 = grid_begin; grid0 < grid_end; grid0 += 65535) {     // gridDim.y holds at most 65535 grids
+        const dim3 blocks((unsigned)(g.nx / fft_cols_per_cta(g.ny)), (unsigned)std::min(65535, grid_end - grid0));
 #define MUSER_COLS_CASE(NN)                                                                                                   \
         if (tmap128) k_fft_cols_correct<NN, 1, 0><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0); \
         else k_fft_cols_correct<NN, 0, 0><<<blocks, (NN / 4) * (fft_cols_per_cta(NN) / 4), fft_smem_bytes(NN), s>>>(map, g.nx, F1, tw, icx, icy, stats, dirty, psf, peaks, grid0);

@@ -184,13 +184,14 @@ int fft_rows_first_radix(int nx);
 cudaError_t fft_rows_setup();
 // valid != nullptr: tile flags of the owner gridder (tiles at 0 stand for zeros and are not loaded); at most 96 tiles per row
 cudaError_t launch_fft_rows_half(const Geom& g, const float2* G, const float* Gw, const int* cnt, const float2* tw,
-                                 Stats* stats, float2* Z, const uint32_t* valid, int num_sms, cudaStream_t s);
+                                 Stats* stats, float2* Z, const uint32_t* valid, int grid_begin, int grid_count, int num_sms,
+                                 cudaStream_t s);                       // grids [grid_begin, grid_begin + grid_count)
 // tmap128 != nullptr: the strip is staged by TMA (tensor map from fft_cols_make_tmap), else by per-lane loads
 bool fft_cols_make_tmap(void* map128, const float2* F1, int nx, int ny, int ngrids);
 // tw8 != nullptr (ny = 512, 1024, with the TMA staging): two radix-8 stages after the first one instead of three radix-4 ones
 bool fft_cols_radix8(int ny);
 cudaError_t launch_fft_cols_correct(const Geom& g, const float2* F1, const float2* tw, const float2* tw8, const float* icx,
                                     const float* icy, const Stats* stats, float* dirty, float* psf, PeakSlot* peaks,
-                                    const void* tmap128, cudaStream_t s);
+                                    const void* tmap128, int grid_begin, int grid_count, cudaStream_t s);
 
 }  // namespace muser

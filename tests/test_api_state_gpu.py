@@ -91,3 +91,44 @@ def test_own_range_histogram_needs_a_dirty_image_first():
             im.histogram(torch.zeros((2, n, n), device="cuda"), 100, 0.0, 0.0, torch.empty((2, 100), dtype=torch.int32, device="cuda"))
     finally:
         im.destroy()
+
+
+@pytest.mark.parametrize("sub", [1, 3, 100])
+def test_fft_subbatches_give_the_same_images(sub):
+    """MUSER_TUNE_FFT_SUBBATCH runs rows -> columns over sub-batches of grids: the same kernels on the same grids.  The grids
+    are re-gridded between the two runs (the only way to invalidate the cached row transform), and the order of the fp32 sums
+    inside the gridder differs from run to run, so the images are compared un-corrected to 1e-5 of the peak (a wrong grid offset
+    in a sub-batch would be an O(1) error); 7 grids, so 3 leaves a ragged tail.  The beam taken again from the cached row
+    transform (column passes only, still per sub-batch) must be bit-identical."""
+    import torch
+    ngrids, n = 7, 256
+    uvw, freq, vis, wt = synth.random_visibilities(31, 4000, n, 30.0, margin_cells=6.0)
+    gid = (np.arange(4000) % ngrids).astype(np.int32)
+    im = gu.make_imager(n, 30.0, 7, 16, ngrids=ngrids)
+    try:
+        im.set_peak_search(True)
+        im.set_grid_correction(False)
+        im.reset()
+        im.grid_batched(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), gu.to_dev(gid))
+        d0, p0 = (torch.empty((ngrids, n, n), device="cuda") for _ in range(2))
+        im.dirty_psf(d0, p0)
+        torch.cuda.synchronize()
+        peaks0 = im.get_peak()
+        im.set_tuning(binding.MUSER_TUNE_FFT_SUBBATCH, sub)
+        im.reset()
+        im.grid_batched(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt), gu.to_dev(gid))
+        d1, p1 = (torch.zeros((ngrids, n, n), device="cuda") for _ in range(2))
+        im.dirty_psf(d1, p1)
+        torch.cuda.synchronize()
+        for g in range(ngrids):
+            assert float((d0[g] - d1[g]).abs().max()) <= 1e-5 * float(d0[g].abs().max())
+            assert float((p0[g] - p1[g]).abs().max()) <= 1e-5 * float(p0[g].abs().max())
+        peaks1 = im.get_peak()
+        for a, b in zip(peaks0, peaks1):
+            assert a[1:3] == b[1:3] and abs(a[0] - b[0]) <= 1e-5 * abs(a[0])
+        p2 = torch.zeros_like(p1)
+        im.psf(p2)
+        torch.cuda.synchronize()
+        assert torch.equal(p2, p1)
+    finally:
+        im.destroy()

@@ -96,6 +96,33 @@ def test_P13_keep_drop_boundary_is_footprint_inside_cells_1_to_n_minus_1(axis, o
         assert not G[:, 0].any() and not G[0, :].any()           # the Nyquist row / column is never written
 
 
+def test_P13b_exact_tie_footprints_are_not_mirror_images_by_one_edge_cell():
+    """The degenerate case of R4 + R6: on an exact half-cell tie BOTH samples of a visibility round up.  By hand (n = 64, Q = 8):
+    u = 5.5 cells -> primary p = 37.5 -> i0 = 38, cells 35..41; conjugate p' = 26.5 -> i0 = 27, cells 24..30.  The mirror
+    (x -> 64 - x) of 35..41 is 23..29: the two footprints agree on 24..29 (same kernel values: the kernel is even) and differ
+    in one edge cell each (41 <-> 23 missing, 30 <-> 34 missing), where the kernel is T[0] = T[S*Q] (distance 3.5 cells).
+    So the full-grid oracle is Hermitian except for those cells; a gridder that computes one half-plane and mirrors it (the CUDA
+    path) differs from it there, in the half it does not compute (tests/test_parity_gpu.py::test_keep_drop_boundary_cells_*)."""
+    um = _metres(5.5)
+    f = 5.5 / (float(um) * SU) * C
+    for _ in range(4000):
+        f = np.nextafter(f, -np.inf)
+    for _ in range(8000):
+        if float(um) * (f / C) * SU == 5.5:
+            break
+        f = np.nextafter(f, np.inf)
+    assert float(um) * (f / C) * SU == 5.5
+    uvw = np.array([[um, 0.0, 0.0]], np.float32)
+    T = mo.table_gauss(S, Q)
+    for G, Gw, st in _both_oracles(uvw, np.array([float(f)]), np.array([2 + 1j], np.complex64), np.array([1.5], np.float32), T):
+        row = G[32]
+        assert np.flatnonzero(row).tolist() == list(range(24, 31)) + list(range(35, 42))
+        for x in range(24, 30):
+            assert row[x] == np.conj(row[64 - x])                # the overlap is Hermitian, exactly
+        assert row[41] == T[0] * T[S * Q // 2] * 1.5 * (2 + 1j) and row[23] == 0       # edge cell of the primary, no mirror
+        assert row[30] == T[S * Q] * T[S * Q // 2] * 1.5 * (2 - 1j) and row[34] == 0   # edge cell of the conjugate, no mirror
+
+
 # ------------------------------------------------------------------ P14: plane selection (R15) and the conjugate-kernel flag
 def test_P14_nearest_plane_centre_ties_go_down_and_negative_w_takes_the_conjugate_kernel():
     """Plane of a visibility = the centre nearest to |w| (tie -> lower plane); a SAMPLE whose own w is negative takes the

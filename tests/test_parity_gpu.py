@@ -696,7 +696,7 @@ def test_owner_fixed_point_merge_bound_per_cell_with_a_1e6_outlier():
     assert err[faint].max() < 20 * unit                       # in practice a handful of merges per cell
 
 
-def _edge_visibilities(n, cell, h, seed, w_max=0.0):
+def _edge_visibilities(n, cell, h, seed, w_max=0.0, with_ties=True):
     """Visibilities whose nearest cell is h, h + 1, n - 1 - h or n - h on one axis or on both (the keep / drop boundary of R5,
     oracle pin P13), at random sub-cell offsets, plus exact half-cell ties at the boundary (frequency scanned ulp by ulp so
     that O1's own operation order lands on the tie exactly)."""
@@ -724,7 +724,9 @@ def _edge_visibilities(n, cell, h, seed, w_max=0.0):
                 ties.append((um, float(f)))
                 break
             f = np.nextafter(f, np.inf)
-    assert len(ties) >= 2
+    assert len(ties) == 4
+    if not with_ties:
+        ties = []
     tu = np.zeros((2 * len(ties), 3), np.float32)
     tf = np.empty(2 * len(ties))
     for i, (um, f) in enumerate(ties):
@@ -739,16 +741,43 @@ def _edge_visibilities(n, cell, h, seed, w_max=0.0):
     return uvw, freq, vis, wt
 
 
+def _check_stored_halfplane_and_mirror(G, G_or):
+    """Exact half-cell ties (R4): both samples of a visibility round UP, so the full-grid oracle's two footprints are
+    not mirror images of each other (one edge cell each) and its grid is Hermitian only up to that.  The CUDA path computes
+    the rows >= ny/2 with the oracle's rule and completes the rest as the Hermitian mirror.  What is unique: the stored
+    half-plane equals the oracle's; what must be valid: the other half is the conjugate mirror of it."""
+    ny, nx = G.shape[-2:]
+    up = slice(ny // 2, ny)
+    assert gu.rel_l2(G[..., up, :], G_or[..., up, :]) <= gu.GRID_TOL
+    low, mir = G[..., 1:ny // 2, 1:], np.conj(G[..., ny - 1:ny // 2:-1, :0:-1])
+    assert gu.rel_l2(low, mir) <= 1e-6
+
+
 @pytest.mark.parametrize("strategy", [OWNER, TILED])
 def test_keep_drop_boundary_cells_2d(strategy):
-    """Samples on cells h, h+1, n-1-h, n-h (and exact ties there): kept / dropped counts and grids equal the oracle's (P13 pins
-    the oracle's rule by hand); nothing is written to row / column 0."""
+    """Samples on cells h, h+1, n-1-h, n-h: kept / dropped counts and grids equal the oracle's (P13 pins the oracle's rule by
+    hand); nothing is written to row / column 0.  Then the same with exact half-cell ties at the boundary added."""
     n, cell, Q = 256, 20.0, 16
-    uvw, freq, vis, wt = _edge_visibilities(n, cell, 3, 1)
+    uvw, freq, vis, wt = _edge_visibilities(n, cell, 3, 1, with_ties=False)
     res = gu.run_case(uvw, freq, vis, wt, n, cell, 7, Q, strategy=strategy, images=False)
     assert res["stats"]["n_dropped"] > 100 and res["stats"]["n_gridded"] > 100
     assert not res["G"][0][0, :].any() and not res["G"][0][:, 0].any()
     assert res["G"][0][:, 1].any() and res["G"][0][:, n - 1].any()
+    uvw, freq, vis, wt = _edge_visibilities(n, cell, 3, 1)
+    im = gu.make_imager(n, cell, 7, Q, strategy=strategy)
+    try:
+        im.reset()
+        im.grid(gu.to_dev(uvw), gu.to_dev(freq), gu.to_dev(vis), gu.to_dev(wt))
+        G, Gw = gu.gpu_grids(im)
+        G_or, Gw_or, st_or = oc.grid(uvw, freq, vis, wt, n, n, cell, Q, 7, gu.oracle_table("pswf", 7, Q, 0.0))
+        st = im.get_stats()
+        assert (st["n_gridded"], st["n_dropped"], st["n_flagged"]) == (st_or["n_gridded"], st_or["n_dropped"], st_or["n_flagged"])
+        assert st["n_gridded"] == res["stats"]["n_gridded"] + 4 and st["n_dropped"] == res["stats"]["n_dropped"] + 4   # by hand: P13
+        _check_stored_halfplane_and_mirror(G, G_or)
+        _check_stored_halfplane_and_mirror(Gw, Gw_or)
+        assert not G[0][0, :].any() and not G[0][:, 0].any()
+    finally:
+        im.destroy()
 
 
 @pytest.mark.parametrize("strategy", [TILED, WPLANE])
@@ -770,7 +799,8 @@ def test_keep_drop_boundary_cells_wplanes(strategy):
         st = im.get_stats()
         assert (st["n_gridded"], st["n_dropped"], st["n_flagged"]) == (st_or["n_gridded"], st_or["n_dropped"], st_or["n_flagged"])
         assert st["n_dropped"] > 200 and st["n_gridded"] > 200
-        assert gu.rel_l2(G, G_or) <= gu.GRID_TOL and gu.rel_l2(Gw, Gw_or) <= gu.GRID_TOL
+        _check_stored_halfplane_and_mirror(G, G_or)              # the input holds exact ties
+        _check_stored_halfplane_and_mirror(Gw, Gw_or)
         assert not G[0][0, :].any() and not G[0][:, 0].any()
     finally:
         im.destroy()
