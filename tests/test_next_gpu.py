@@ -207,7 +207,7 @@ def test_peak_search_and_histogram_equal_the_oracle_on_the_same_image(nx, ny, ng
         im.destroy()
 
 
-@pytest.mark.parametrize("n", [1280])
+@pytest.mark.parametrize("n", [1280, 2560])
 def test_table2_non_power_of_two_image_size(n):
     """PAPER.md:114-116 (Table 2): 1280^2 (2560^2 and 5120^2 take the same code path: cuFFT 2-D + k_correct)."""
     cell, Q = 8.0, 32
